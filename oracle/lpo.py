@@ -1,0 +1,178 @@
+"""ctypes binding of the CPU oracle (oracle/lpo_oracle.c).
+
+TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke() and
+bench.py's cpu_baseline / ``--impl reference`` legs may import this module.  It
+imports nothing from paper_1611_04255_b200 and the CUDA path imports nothing
+from here.
+
+All functions take a list of P contiguous float32 numpy arrays of equal length
+(the P virtual ranks' vectors) and work in place, like the C functions they
+call.  Citations live in lpo_oracle.c next to each function.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "lpo_oracle.c")
+_SO = os.path.join(_HERE, "liblpo.so")
+
+GCC_FLAGS = ["-O2", "-std=c11", "-ffp-contract=off", "-fno-fast-math", "-fopenmp",
+             "-fPIC", "-shared"]
+
+OP_BROADCAST, OP_REDUCE, OP_ALLREDUCE = 0, 1, 2
+ALGO_LP, ALGO_MST, ALGO_BE = 0, 1, 2
+READING_A_REVERSE, READING_B_RING = 0, 1
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (no CUDA involved). Returns the .so path."""
+    if (not force and os.path.exists(_SO)
+            and os.path.getmtime(_SO) >= os.path.getmtime(_SRC)):
+        return _SO
+    cmd = ["gcc", *GCC_FLAGS, _SRC, "-o", _SO, "-lm"]
+    subprocess.run(cmd, check=True)
+    return _SO
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    global _lib
+    if _lib is None:
+        build()
+        L = ctypes.CDLL(_SO)
+        pp = ctypes.POINTER(ctypes.c_void_p)
+        sz, i32, u64, f32 = ctypes.c_size_t, ctypes.c_int, ctypes.c_uint64, ctypes.c_float
+        pu64 = ctypes.POINTER(u64)
+        L.lpo_chain_sum.argtypes = [pp, i32, sz, ctypes.c_void_p]
+        L.lpo_chain_sum.restype = None
+        for name in ("lpo_broadcast", "lpo_reduce", "lpo_mst_broadcast", "lpo_mst_reduce",
+                     "lpo_be_broadcast", "lpo_be_reduce"):
+            getattr(L, name).argtypes = [pp, i32, sz, i32]
+        for name in ("lpo_allreduce", "lpo_allreduce_omp", "lpo_mst_allreduce",
+                     "lpo_be_allreduce"):
+            getattr(L, name).argtypes = [pp, i32, sz]
+        for name in ("lpo_bsp_sgd_step", "lpo_bsp_sgd_step_omp"):
+            getattr(L, name).argtypes = [pp, pp, i32, sz, i32, f32]
+        L.lpo_lp_blocked.argtypes = [pp, i32, sz, sz, i32, i32, pu64]
+        L.lpo_num_blocks.argtypes = [sz, sz]
+        L.lpo_num_blocks.restype = u64
+        L.lpo_stage_block.argtypes = [i32, u64, u64, i32]
+        L.lpo_stage_block.restype = ctypes.c_int64
+        L.lpo_stage_ticks.argtypes = [i32, u64]
+        L.lpo_stage_ticks.restype = u64
+        L.lpo_link_sim.argtypes = [i32, u64, i32, i32, pu64, pu64]
+        L.lpo_link_sim_reduce_ready.argtypes = [i32, u64, pu64]
+        L.lpo_mst_levels.argtypes = [i32]
+        L.lpo_cost.argtypes = [i32, i32] + [ctypes.c_double] * 6
+        L.lpo_cost.restype = ctypes.c_double
+        L.lpo_num_threads.restype = i32
+        _lib = L
+    return _lib
+
+
+def _ptrs(bufs):
+    for b in bufs:
+        if not (isinstance(b, np.ndarray) and b.dtype == np.float32 and b.flags.c_contiguous
+                and b.flags.writeable):
+            raise TypeError("oracle buffers must be writable C-contiguous float32 numpy arrays")
+    n = bufs[0].size if bufs else 0
+    if any(b.size != n for b in bufs):
+        raise ValueError("all ranks must hold vectors of the same length")
+    arr = (ctypes.c_void_p * len(bufs))(*[b.ctypes.data for b in bufs])
+    return arr, n
+
+
+def _check(rc, what):
+    if rc != 0:
+        raise RuntimeError(f"oracle {what} failed with status {rc}")
+
+
+def chain_sum(bufs) -> np.ndarray:
+    arr, n = _ptrs(bufs)
+    out = np.empty(n, dtype=np.float32)
+    lib().lpo_chain_sum(arr, len(bufs), n, out.ctypes.data)
+    return out
+
+
+def broadcast(bufs, root=0, algo=ALGO_LP):
+    arr, n = _ptrs(bufs)
+    f = {ALGO_LP: "lpo_broadcast", ALGO_MST: "lpo_mst_broadcast", ALGO_BE: "lpo_be_broadcast"}[algo]
+    _check(getattr(lib(), f)(arr, len(bufs), n, root), f)
+
+
+def reduce(bufs, root=0, algo=ALGO_LP):
+    arr, n = _ptrs(bufs)
+    f = {ALGO_LP: "lpo_reduce", ALGO_MST: "lpo_mst_reduce", ALGO_BE: "lpo_be_reduce"}[algo]
+    _check(getattr(lib(), f)(arr, len(bufs), n, root), f)
+
+
+def allreduce(bufs, algo=ALGO_LP, omp=False):
+    arr, n = _ptrs(bufs)
+    f = {ALGO_LP: "lpo_allreduce_omp" if omp else "lpo_allreduce",
+         ALGO_MST: "lpo_mst_allreduce", ALGO_BE: "lpo_be_allreduce"}[algo]
+    _check(getattr(lib(), f)(arr, len(bufs), n), f)
+
+
+def bsp_sgd_step(grads, weights, root=0, lr=0.01, omp=False):
+    ga, n = _ptrs(grads)
+    wa, nw = _ptrs(weights)
+    if n != nw or len(grads) != len(weights):
+        raise ValueError("grads and weights must match in P and n")
+    f = "lpo_bsp_sgd_step_omp" if omp else "lpo_bsp_sgd_step"
+    _check(getattr(lib(), f)(ga, wa, len(grads), n, root, ctypes.c_float(lr)), f)
+
+
+def lp_blocked(bufs, block, op, root=0) -> int:
+    """Tick-by-tick LP pipeline (stage model). Returns the tick count."""
+    arr, n = _ptrs(bufs)
+    ticks = ctypes.c_uint64(0)
+    _check(lib().lpo_lp_blocked(arr, len(bufs), n, block, root, op, ctypes.byref(ticks)),
+           "lpo_lp_blocked")
+    return ticks.value
+
+
+def num_blocks(n, block) -> int:
+    return lib().lpo_num_blocks(n, block)
+
+
+def stage_block(P, nb, t, r) -> int:
+    return lib().lpo_stage_block(P, nb, t, r)
+
+
+def stage_ticks(P, nb) -> int:
+    return lib().lpo_stage_ticks(P, nb)
+
+
+def link_sim(P, nb, op, reading=READING_A_REVERSE, per_block=False):
+    steps = ctypes.c_uint64(0)
+    done = (ctypes.c_uint64 * max(nb, 1))()
+    _check(lib().lpo_link_sim(P, nb, op, reading, ctypes.byref(steps), done), "lpo_link_sim")
+    if per_block:
+        return steps.value, [done[k] for k in range(nb)]
+    return steps.value
+
+
+def link_sim_reduce_ready(P, nb):
+    done = (ctypes.c_uint64 * max(nb, 1))()
+    _check(lib().lpo_link_sim_reduce_ready(P, nb, done), "lpo_link_sim_reduce_ready")
+    return [done[k] for k in range(nb)]
+
+
+def mst_levels(P) -> int:
+    return lib().lpo_mst_levels(P)
+
+
+def cost(algo, op, p, n, b, alpha, beta, gamma) -> float:
+    return lib().lpo_cost(algo, op, float(p), float(n), float(b), float(alpha), float(beta),
+                          float(gamma))
+
+
+def num_threads() -> int:
+    return lib().lpo_num_threads()
