@@ -1,0 +1,405 @@
+#!/usr/bin/env python
+"""bench.py -- LP allreduce algorithm GB/s and fraction of the HBM roofline on one B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 1] [--block B]
+
+A step is one LP allreduce (a1 partition, a2 schedule, a4 reduce stage, a3 broadcast stage = a5) of the
+workload -- by default BASELINE.json configs[1]: P=6 virtual ranks, n=61,000,000 fp32 per rank, N(0,1e-3),
+seed 1 -- through the C ABI (lp_allreduce) with the inputs already resident in HBM.  `value` = algbw =
+n*4 bytes / t (nccl-tests convention) summed over the N replicas; `roofline.achieved` = minimum HBM bytes
+2*P*n*4 / t against the measured copy peak of MEASURED_PEAKS.json.  `e2e` = the same metric through
+lp_allreduce_host with pinned HOST buffers (H2D + kernel + D2H inside the timed region).  `cpu_baseline` /
+`--impl reference` time the CPU oracle as it stands on the box's host cores.  Prints ONE JSON line (rank 0).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+from paper_1611_04255_b200 import inputs  # noqa: E402
+
+METRIC = "lp_allreduce_algbw"
+UNIT = "GB/s (algbw = n*4 bytes per rank / time; roofline on min bytes 2*P*n*4)"
+FALLBACK_HBM_GBS = 6650.0  # B200_PROFILING.md fallback, used only if MEASURED_PEAKS.json is absent
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json configs (1 or 4 for allreduce)")
+    ap.add_argument("--block", type=int, default=0, help="LP block in elements (0 = the config's)")
+    ap.add_argument("--variant", default="pipeline", choices=["pipeline", "direct", "cluster", "copy_engine"])
+    ap.add_argument("--no-detail", action="store_true", help="skip the secondary measurements")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    return ap.parse_args()
+
+
+def workload(cfg_idx):
+    c = inputs.CONFIGS[cfg_idx]
+    if "allreduce" not in c["ops"] or not isinstance(c["P"], int):
+        raise SystemExit(f"config {cfg_idx} is not a single allreduce workload")
+    return c
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, torch copy)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+# ---- clocks ------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f,
+                                      stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        if self.p is None:
+            return out
+        time.sleep(0.15)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        rows = [r.split(",") for r in open(self.f.name).read().strip().splitlines() if r.count(",") >= 5]
+        os.unlink(self.f.name)
+        sm, names = [], ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = set()
+        for r in rows:
+            try:
+                sm.append(float(r[0]))
+                out["sm_max_mhz"] = float(r[1])
+            except ValueError:
+                continue
+            for name, v in zip(names, r[2:6]):
+                if v.strip().lower().startswith("active"):
+                    reasons.add(name)
+        if sm:
+            out["sm_mhz"] = float(np.median(sm))
+        out["reasons"] = sorted(reasons)
+        out["samples"] = len(sm)
+        return out
+
+
+# ---- distributed plumbing (replicas only: no data-path collective) ------------------------------------
+def dist_setup(n_gpus):
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        import torch
+        backend = "nccl" if torch.cuda.is_available() else "gloo"
+        dist.init_process_group(backend=backend, rank=rank, world_size=world)
+    return rank, world, local
+
+
+def barrier(world):
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+
+
+def max_over_ranks(value, world, device=None):
+    """Max of a python float over all ranks (timing rule: the slowest rank counts)."""
+    if world == 1:
+        return value
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def sum_over_ranks(value, world, device=None):
+    if world == 1:
+        return value
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([value], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return float(t.item())
+
+
+# ---- the oracle on the host cores (cpu_baseline leg and --impl reference) ------------------------------
+def time_oracle(P, n_sample, dist_kind, sigma, seed, passes):
+    """Times oracle.lpo.allreduce(omp=True) as it stands on a bounded sample: the first n_sample elements of every
+    rank's vector.  Returns (seconds per pass list, cores)."""
+    from oracle import lpo
+    src = inputs.rank_vectors(seed, P, n_sample, dist_kind, sigma)
+    work = [s.copy() for s in src]
+    lpo.allreduce(work, omp=True)  # warm-up (page faults, thread pool)
+    times = []
+    for _ in range(passes):
+        for w, s in zip(work, src):
+            np.copyto(w, s)
+        t0 = time.perf_counter()
+        lpo.allreduce(work, omp=True)
+        times.append(time.perf_counter() - t0)
+    return times, lpo.num_threads()
+
+
+def run_reference(args, c, rank, world):
+    """--impl reference: the CPU oracle, unmodified, on the host cores.  Rank 0 only."""
+    if rank != 0:
+        return
+    P, n = c["P"], c["n"]
+    n_sample = min(n, 16_000_000)
+    times, cores = time_oracle(P, n_sample, c["dist"], c.get("sigma", 1.0), args.config, args.warmup + args.steps)
+    timed = times[args.warmup:]
+    t = sum(timed) / len(timed)
+    value = n_sample * 4 / t / 1e9
+    sample = f"first {n_sample} of {n} elements per rank, P={P}, oracle lpo_allreduce_omp, {len(timed)} passes"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": t * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"BASELINE.json configs[{args.config}]: {c['name']}", "P": P, "n": n,
+                   "sample_n": n_sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ---- our arm ------------------------------------------------------------------------------------------------
+def timed_steps(torch, step_fn, restore_fn, n_steps, safe_run):
+    """Runs n_steps back to back between CUDA events on the current stream; every `safe_run` steps the inputs are
+    restored OUTSIDE the event pair (an in-place allreduce multiplies magnitudes by ~P per call).  Returns ms."""
+    total_ms, done = 0.0, 0
+    while done < n_steps:
+        seg = min(safe_run, n_steps - done)
+        restore_fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for i in range(seg):
+            step_fn(done + i)
+        e1.record()
+        torch.cuda.synchronize()
+        total_ms += e0.elapsed_time(e1)
+        done += seg
+    return total_ms
+
+
+def run_ours(args, c, rank, world, local):
+    import torch
+
+    from paper_1611_04255_b200 import binding as lp
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the CUDA library is the product, there is no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    lp.lib()
+    variant = {"pipeline": 0, "direct": 1, "cluster": 2, "copy_engine": 3}[args.variant]
+    lp.lp_set_variant(variant)
+    P, n = c["P"], c["n"]
+    block = args.block or c["block"]
+    sigma = c.get("sigma", 1.0)
+    min_bytes = lp.lp_min_bytes(lp.OP_ALLREDUCE, P, n)
+
+    # synthetic inputs, generated on the host, uploaded once
+    host = inputs.rank_vectors(args.config, P, n, c["dist"], sigma)
+    pristine = [torch.from_numpy(h).to(dev) for h in host]
+    n_sets = 3  # rotating buffer sets; one set (P*n*4 bytes) is already >> the 126 MB L2
+    free_b, _ = torch.cuda.mem_get_info()
+    while n_sets > 1 and n_sets * P * n * 4 > 0.6 * free_b:
+        n_sets -= 1
+    sets = [[torch.empty_like(p) for p in pristine] for _ in range(n_sets)]
+
+    def restore():
+        for s in sets:
+            for d, p in zip(s, pristine):
+                d.copy_(p)
+
+    def step(i):
+        lp.lp_allreduce(sets[i % n_sets], block)
+
+    # growth per call ~P: keep |x| * P^k far below fp32 max
+    vmax = max(float(np.abs(h).max()) for h in host)
+    safe_uses = max(1, int(np.floor(np.log(1e30 / max(vmax, 1e-30)) / np.log(max(P, 2)))))
+    safe_run = safe_uses * n_sets
+
+    barrier(world)
+    timed_steps(torch, step, restore, max(args.warmup, 3), safe_run)  # warm-up (>= 3)
+    barrier(world)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local) if rank == 0 else None
+    launches0 = lp.lp_launch_count()
+    total_ms = timed_steps(torch, step, restore, args.steps, safe_run)
+    launches = lp.lp_launch_count() - launches0
+    barrier(world)
+    torch.cuda.synchronize()
+    clocks = sampler.stop() if sampler else None
+    total_ms = max_over_ranks(total_ms, world, dev)
+    ms_per_step = total_ms / args.steps
+    algbw = world * n * 4 / (ms_per_step * 1e-3) / 1e9
+    hbm = min_bytes / (ms_per_step * 1e-3) / 1e9  # per GPU
+    peak, peak_src = measured_peak()
+    plan = lp.lp_plan_query(lp.OP_ALLREDUCE, P, n, block)
+
+    # e2e: host buffers through lp_allreduce_host, copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        pinned = [torch.from_numpy(h.copy()).pin_memory() for h in host]
+        k_e2e = max(1, min(args.steps, 5))
+        lp.lp_allreduce_host(pinned, block)  # warm-up (allocates the staging chunks)
+        for p_, h in zip(pinned, host):
+            p_.copy_(torch.from_numpy(h))
+        barrier(world)
+        t0 = time.perf_counter()
+        for _ in range(k_e2e):
+            lp.lp_allreduce_host(pinned, block)  # synchronous
+        t_e2e = (time.perf_counter() - t0) / k_e2e
+        t_e2e = max_over_ranks(t_e2e, world, dev)
+        e2e = {"value": world * n * 4 / t_e2e / 1e9, "unit": UNIT, "h2d_bytes_per_step": P * n * 4,
+               "d2h_bytes_per_step": P * n * 4, "ms_per_step": t_e2e * 1e3, "steps": k_e2e,
+               "api": "lp_allreduce_host (pinned host buffers, chunked H2D/kernel/D2H pipeline)"}
+        del pinned
+
+    detail = None
+    if rank == 0 and not args.no_detail:
+        detail = secondary(torch, lp, dev, pristine, sets[0], P, n, block, peak)
+
+    cpu = None
+    if rank == 0 and not args.no_cpu:
+        n_sample = min(n, 16_000_000)
+        times, cores = time_oracle(P, n_sample, c["dist"], sigma, args.config, 5)
+        t = sum(times) / len(times)
+        cpu = {"value": n_sample * 4 / t / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": f"first {n_sample} of {n} elements per rank, P={P}, lpo_allreduce_omp, 5 passes, "
+                         f"{t * 1e3:.1f} ms per pass"}
+
+    if rank != 0:
+        return
+    line = {
+        "metric": METRIC, "value": algbw, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"BASELINE.json configs[{args.config}]: {c['name']}", "P": P, "n": n, "block": block,
+                   "variant": args.variant, "plan": plan, "parallelism": f"replicas x{world} (no collective)",
+                   "l2": f"inputs {P * n * 4 / 1e6:.0f} MB per set >> 126 MB L2, {n_sets} rotating sets"},
+        "roofline": {"bound": "hbm", "achieved": hbm, "peak": peak, "unit": "GB/s", "frac": hbm / peak,
+                     "traffic": None, "peak_source": peak_src, "frac_of_nominal_8TBs": hbm / 8000.0,
+                     "kernel": "lp_pipeline_kernel" if variant == 0 else args.variant,
+                     "algorithmic_bytes_per_launch": min_bytes},
+        "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "detail": detail,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def secondary(torch, lp, dev, pristine, work, P, n, block, peak):
+    """Secondary measurements reported under "detail" (same inputs, same timing method, 5 timed calls each):
+    the other LP ops, the other variants, the MST baseline, the block sweep of configs[1], and the fused
+    BSP-SGD step + BE baseline on configs[2] (P=8, n=7,000,000)."""
+    def restore():
+        for d, p in zip(work, pristine):
+            d.copy_(p)
+
+    def measure(fn, min_bytes, iters=5, restore_fn=restore):
+        ms = []
+        for it in range(iters + 2):
+            restore_fn()
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            fn()
+            e1.record()
+            torch.cuda.synchronize()
+            if it >= 2:
+                ms.append(e0.elapsed_time(e1))
+        t = float(np.median(ms))
+        gbs = min_bytes / (t * 1e-3) / 1e9
+        return {"ms": round(t, 4), "hbm_GBps_min_bytes": round(gbs, 1), "frac_of_measured_peak": round(gbs / peak, 4)}
+
+    out = {"note": "median of 5 single calls, inputs restored before each; min bytes per SURVEY 8(d)"}
+    mb = lambda op, p=P, m=n: lp.lp_min_bytes(op, p, m)  # noqa: E731
+    out["lp_reduce_root0"] = measure(lambda: lp.lp_reduce(work, block, root=0), mb(lp.OP_REDUCE))
+    out["lp_broadcast_root0"] = measure(lambda: lp.lp_broadcast(work, block, root=0), mb(lp.OP_BROADCAST))
+    cur = lp.lp_get_variant()
+    for name, v in (("pipeline", lp.VARIANT_PIPELINE), ("direct", lp.VARIANT_DIRECT)):
+        lp.lp_set_variant(v)
+        out[f"lp_allreduce_{name}"] = measure(lambda: lp.lp_allreduce(work, block), mb(lp.OP_ALLREDUCE))
+    lp.lp_set_variant(cur)
+    sweep = {}
+    for b in (16_384, 65_536, 131_072, 262_144, 524_288, 1_048_576):
+        sweep[str(b)] = measure(lambda b=b: lp.lp_allreduce(work, b), mb(lp.OP_ALLREDUCE))
+    out["lp_allreduce_block_sweep"] = sweep
+    # MST moves 5(P-1)n*4 bytes; its GB/s is still quoted on the ALGORITHM's minimum bytes so rows compare
+    out["mst_allreduce"] = measure(lambda: lp.lp_mst_allreduce(work), mb(lp.OP_ALLREDUCE))
+    out["mst_reduce_root0"] = measure(lambda: lp.lp_mst_reduce(work, root=0), mb(lp.OP_REDUCE))
+    out["mst_broadcast_root0"] = measure(lambda: lp.lp_mst_broadcast(work, root=0), mb(lp.OP_BROADCAST))
+    # configs[2]: fused BSP-SGD step, P=8, n=7,000,000; BE baseline on the same 8 vectors
+    c2 = inputs.CONFIGS[2]
+    P2, n2 = c2["P"], c2["n"]
+    g_h, w_h = inputs.sgd_inputs(2, P2, n2, c2["sigma"], c2["w_sigma"])
+    g = [torch.from_numpy(x).to(dev) for x in g_h]
+    w = [torch.from_numpy(x).to(dev) for x in w_h]
+    g0 = [x.clone() for x in g]
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)  # 256 MB > L2: written between calls
+
+    def restore2():
+        for d, p in zip(g, g0):
+            d.copy_(p)
+        flush.fill_(1)
+
+    out["lp_bsp_sgd_step_cfg2"] = measure(lambda: lp.lp_bsp_sgd_step(g, w, c2["block"], root=0, lr=c2["lr"]),
+                                          mb(lp.OP_BSP_SGD, P2, n2), restore_fn=restore2)
+    out["lp_allreduce_cfg2_P8"] = measure(lambda: lp.lp_allreduce(g, c2["block"]), mb(lp.OP_ALLREDUCE, P2, n2),
+                                          restore_fn=restore2)
+    out["be_allreduce_cfg2_P8"] = measure(lambda: lp.lp_be_allreduce(g), mb(lp.OP_ALLREDUCE, P2, n2),
+                                          restore_fn=restore2)
+    out["mst_allreduce_cfg2_P8"] = measure(lambda: lp.lp_mst_allreduce(g), mb(lp.OP_ALLREDUCE, P2, n2),
+                                           restore_fn=restore2)
+    return out
+
+
+def main():
+    args = parse_args()
+    c = workload(args.config)
+    rank, world, local = dist_setup(args.gpus)
+    try:
+        if args.impl == "reference":
+            run_reference(args, c, rank, world)
+        else:
+            run_ours(args, c, rank, world, local)
+    finally:
+        if world > 1:
+            import torch.distributed as dist
+            if dist.is_initialized():
+                dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,183 @@
+/*
+ * lp_collectives.h -- C ABI of liblp_b200.so: Linear Pipeline (LP) collectives of
+ * arXiv 1611.04255 over P *virtual* ranks (P disjoint device buffers in one
+ * B200's HBM), a fused BSP-SGD step, and same-GPU MST / BE baselines.
+ *
+ * Citations are PAPER.md:<line> + section; "U<k>" are
+ * the readings of the paper listed in DESIGN.md.
+ *
+ * Conventions for every entry point
+ *   - `bufs` (`grads`, `weights`) is a HOST array of P DEVICE pointers (entry
+ *     points ending in `_host` take a HOST array of P HOST pointers).  The array
+ *     is read during the call and not retained.  The caller owns every buffer.
+ *   - `n` and `block` are counted in fp32 ELEMENTS (U1; the paper counts bytes,
+ *     PAPER.md:85).  Every buffer holds n contiguous floats, is 16-byte aligned
+ *     and does not overlap another buffer of the same call.
+ *   - `block` is the LP block size b ("we dissect a long message into
+ *     fine-grained blocks"): nb = ceil(n / block), last block short (U6).
+ *     Results never depend on `block`; speed does.
+ *   - `cuda_stream` is a cudaStream_t (NULL = legacy default stream).  Work is
+ *     enqueued on it and the call returns without a host sync; results are valid
+ *     once the stream reaches that point.  `_host` entry points are synchronous.
+ *   - Arithmetic is fp32 IEEE-754 round-to-nearest-even, no FMA contraction, no
+ *     flush-to-zero.  LP sums are the left fold in rank order 0 -> P-1 whatever
+ *     the root (Fig. 2b; U4), so results are bit-exact to that fold.
+ *   - Return value: LP_OK or an LP_ERR_* code.  Arguments are validated before
+ *     anything is enqueued: on LP_ERR_INVALID_ARG / LP_ERR_UNSUPPORTED nothing
+ *     ran.  n == 0 and P == 1 are valid (no-ops, except that P == 1 reduce /
+ *     allreduce / broadcast leave the single buffer unchanged).  No exceptions,
+ *     no abort, nothing printed.
+ *   - The library owns only internal scratch (receive buffers of the
+ *     copy-engine variant, MST/BE working copies, host-staging chunks),
+ *     allocated lazily and freed by lp_shutdown().
+ *   - There is no CPU fallback: without a CUDA device the compute entry points
+ *     return LP_ERR_CUDA.
+ */
+#ifndef LP_COLLECTIVES_H
+#define LP_COLLECTIVES_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+/* every entry point below has default ELF visibility; the rest of the library is hidden */
+#if defined(__GNUC__)
+#define LP_API __attribute__((visibility("default")))
+#else
+#define LP_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* ---- status codes ------------------------------------------------------- */
+#define LP_OK 0
+#define LP_ERR_INVALID_ARG 1 /* P<1, P>LP_MAX_P, NULL pointer, block==0, root out of range,
+                                misaligned or overlapping buffers, unknown enum value */
+#define LP_ERR_UNSUPPORTED 2 /* BE with non-power-of-two P (U14); cluster variant with P it cannot hold */
+#define LP_ERR_CUDA 3        /* launch / allocation / copy failure, or no device */
+
+#define LP_MAX_P 32
+
+/* ---- enums ---------------------------------------------------------------- */
+/* collective, PAPER.md:57 (broadcast), :59 (reduce), :61,71 (allreduce), :144-180 (BSP-SGD Alg. 3) */
+#define LP_OP_BROADCAST 0
+#define LP_OP_REDUCE 1
+#define LP_OP_ALLREDUCE 2
+#define LP_OP_BSP_SGD 3
+
+/* realisation of the LP pipeline used by lp_broadcast/lp_reduce/lp_allreduce/lp_bsp_sgd_step */
+#define LP_VARIANT_PIPELINE 0    /* default: one persistent kernel; per CTA a TMA-bulk shared-memory ring
+                                    with mbarrier full/empty flags handed producer warp -> add warps -> store warp */
+#define LP_VARIANT_DIRECT 1      /* one persistent kernel, 128-bit register loads/stores, chain fold in registers */
+#define LP_VARIANT_CLUSTER 2     /* stage-per-rank: a thread-block cluster of P CTAs, CTA r owns rank r and hands
+                                    the running partial to CTA r+1 through distributed shared memory (P <= 16) */
+#define LP_VARIANT_COPY_ENGINE 3 /* the paper's own design: one cudaMemcpyAsync + one add kernel per (hop, block)
+                                    on two streams */
+
+/* schedule models of lp_schedule_steps (U2, U3) */
+#define LP_MODEL_STAGE 0        /* stages = the P ranks; pipeline length P - 1 + nb */
+#define LP_MODEL_LINK 1         /* stages = the P-1 links, Fig. 2; allreduce redistributes by reverse flow (U3-A) */
+#define LP_MODEL_LINK_RING 2    /* as LINK, allreduce redistributes by ring closure P-1 -> 0 -> ... (U3-B) */
+
+/* tuning keys of lp_set_tuning (0 = library default) */
+#define LP_TUNE_TILE_ELEMS 0    /* tile (sub-block) size in elements: 1024, 2048, 4096 or 8192 */
+#define LP_TUNE_STAGES 1        /* depth of the load ring (2..32) */
+#define LP_TUNE_OUT_STAGES 2    /* depth of the store ring (1..8) */
+#define LP_TUNE_CTAS_PER_SM 3   /* persistent CTAs per SM (1..8) */
+#define LP_TUNE_CE_STREAMS 4    /* copy-engine variant: number of streams / receive slots (paper: 2) */
+#define LP_TUNE_L2_HINT 5       /* 0 none, 1 evict_first on loads, 2 evict_first on loads and stores */
+#define LP_TUNE_COUNT 6
+
+/* ---- LP collectives (the hot path) ----------------------------------------- */
+
+/* Broadcast, PAPER.md:57 (Sec. 3, Fig. 2a): "copies the source vector to every GPUs".
+ * bufs[r][i] <- bufs[root][i] for every r != root, i in [0, n).  bufs[root] is only read. */
+LP_API int lp_broadcast(float *const *bufs, int P, size_t n, size_t block, int root, void *cuda_stream);
+
+/* Reduce, PAPER.md:59 (Sec. 3, Fig. 2b): "combines the elements provided in the vector of each GPU, and
+ * returns the combined value ... to a specific GPU".  bufs[root][i] <- S[i] with
+ * S[i] = ((bufs[0][i] + bufs[1][i]) + ...) + bufs[P-1][i]; buffers of the other ranks are unchanged (U5). */
+LP_API int lp_reduce(float *const *bufs, int P, size_t n, size_t block, int root, void *cuda_stream);
+
+/* Allreduce, PAPER.md:61,71 (Fig. 2c): "equivalent to a reduce followed by a broadcast", pipeline filled
+ * once.  bufs[r][i] <- S[i] for every r; the same bits on every rank. */
+LP_API int lp_allreduce(float *const *bufs, int P, size_t n, size_t block, void *cuda_stream);
+
+/* Fused BSP-SGD step = Alg. 3's communication + update (Eq. 5, 174, 180):
+ *   S = chain sum of grads;  g = S * invP, invP = fl(1.0f / P) (U7);  t = lr * g;  w' = weights[root][i] - t;
+ *   weights[r][i] <- w' for every r (U8).  Three separately rounded fp32 ops, no FMA.  grads are only read.
+ * grads[] and weights[] are 2P distinct buffers. */
+LP_API int lp_bsp_sgd_step(float *const *grads, float *const *weights, int P, size_t n, size_t block, int root,
+                    float lr, void *cuda_stream);
+
+/* ---- MST (binomial tree) and BE (recursive halving / doubling) baselines ------ */
+/* PAPER.md:93 (MST: "balanced tree of height ceil(log p)", whole-message steps) and
+ * PAPER.md:95 (BE: broadcast = MST scatter + BE allgather, reduce = reduce-scatter + gather, allreduce =
+ * reduce-scatter + allgather).  Same in-place semantics as the LP calls; the summation TREE differs
+ * (MST on virtual ranks v = (r - root) mod P; BE butterfly), so results agree with LP to
+ * |diff| <= 1e-6 * sum_r |x_r[i]| (U15), not bit for bit.  BE needs P a power of two (U14). */
+LP_API int lp_mst_broadcast(float *const *bufs, int P, size_t n, int root, void *cuda_stream);
+LP_API int lp_mst_reduce(float *const *bufs, int P, size_t n, int root, void *cuda_stream);
+LP_API int lp_mst_allreduce(float *const *bufs, int P, size_t n, void *cuda_stream);
+LP_API int lp_be_broadcast(float *const *bufs, int P, size_t n, int root, void *cuda_stream);
+LP_API int lp_be_reduce(float *const *bufs, int P, size_t n, int root, void *cuda_stream);
+LP_API int lp_be_allreduce(float *const *bufs, int P, size_t n, void *cuda_stream);
+
+/* ---- host-buffer entry points (end-to-end path) ------------------------------- */
+/* Same results as lp_allreduce / lp_bsp_sgd_step, but the P (2P) buffers live in HOST memory (pinned for
+ * full speed; pageable works).  The message is cut into chunks that flow host -> device -> kernel -> host
+ * on three streams, so the upload of chunk c+1, the LP kernel on chunk c and the download of chunk c-1
+ * overlap.  Synchronous: returns when every host buffer holds its result. */
+LP_API int lp_allreduce_host(float *const *host_bufs, int P, size_t n, size_t block);
+LP_API int lp_bsp_sgd_step_host(float *const *host_grads, float *const *host_weights, int P, size_t n, size_t block,
+                         int root, float lr);
+
+/* ---- schedule engine (host only; no device needed) ---------------------------- */
+/* a1: nb = ceil(n / block) (U6); 0 when block == 0. */
+LP_API uint64_t lp_num_blocks(size_t n, size_t block);
+/* a2: block handled by rank r at tick t in the stage model, k = t - r if 0 <= k < nb, else -1. */
+LP_API int64_t lp_stage_block(int P, uint64_t nb, uint64_t t, int r);
+/* Number of steps of `op` (LP_OP_BROADCAST / REDUCE / ALLREDUCE) over P ranks and nb = ceil(n/block) blocks
+ * under `model`: STAGE -> P - 1 + nb; LINK / LINK_RING -> the Fig. 2 schedule with one inbound
+ * and one outbound transfer per rank per step.  0 steps when n == 0 (or P == 1 in the
+ * link models). */
+LP_API int lp_schedule_steps(int P, size_t n, size_t block, int op, int model, uint64_t *steps_out);
+/* Number of whole-message levels of the MST baseline, ceil(log2 P). */
+LP_API int lp_mst_levels(int P);
+
+/* How the persistent kernel will cut and spread the work for (op, P, n, block) under the current variant
+ * and tuning: tile size, tile count, grid, threads, dynamic shared memory, ring depths. */
+typedef struct lp_plan_info {
+    uint64_t nb;              /* a1: number of LP blocks */
+    uint64_t n_tiles;         /* tiles (sub-blocks); a tile never straddles a block boundary */
+    uint32_t tile_elems;      /* elements per full tile */
+    uint32_t grid;            /* persistent CTAs (clusters * P for the cluster variant) */
+    uint32_t threads;         /* threads per CTA */
+    uint32_t smem_bytes;      /* dynamic shared memory per CTA */
+    uint32_t stages;          /* load-ring depth */
+    uint32_t out_stages;      /* store-ring depth */
+    uint32_t variant;         /* variant that will actually run (PIPELINE falls back to DIRECT when
+                                 block % 4 != 0 and nb > 1) */
+    uint32_t sm_count;        /* SMs assumed (device query, 148 when no device) */
+} lp_plan_info;
+LP_API int lp_plan_query(int op, int P, size_t n, size_t block, lp_plan_info *out);
+
+/* Minimum HBM bytes of one call (each input read once, each output written once):
+ * broadcast P*n*4, reduce (P+1)*n*4, allreduce 2*P*n*4, bsp_sgd (2P+1)*n*4. */
+LP_API uint64_t lp_min_bytes(int op, int P, size_t n);
+
+/* ---- control ------------------------------------------------------------------ */
+LP_API int lp_set_variant(int variant);             /* LP_VARIANT_*; affects the four LP calls */
+LP_API int lp_get_variant(void);
+LP_API int lp_set_tuning(int key, int value);       /* LP_TUNE_*; value 0 restores the default */
+LP_API int lp_get_tuning(int key);
+LP_API uint64_t lp_launch_count(void);              /* kernels + async copies enqueued by this library so far */
+LP_API int lp_shutdown(void);                       /* frees library scratch; safe to call twice */
+LP_API const char *lp_status_string(int status);    /* static string; appends the last CUDA error for LP_ERR_CUDA */
+LP_API int lp_version(void);                        /* 10000*major + 100*minor + patch */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LP_COLLECTIVES_H */

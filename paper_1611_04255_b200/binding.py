@@ -1,0 +1,262 @@
+"""Thin ctypes binding of ``liblp_b200.so`` (include/lp_collectives.h): same names, argument marshalling only.
+
+Device buffers are ``torch`` CUDA tensors (float32, contiguous); ``stream`` is a ``torch.cuda.Stream`` (default:
+the current stream).  PyTorch only owns memory and streams -- every step of the path runs in the library's
+kernels.  There is NO fallback: a missing library or a non-zero status raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+from . import build as _build
+
+# enums of include/lp_collectives.h
+LP_OK, LP_ERR_INVALID_ARG, LP_ERR_UNSUPPORTED, LP_ERR_CUDA = 0, 1, 2, 3
+LP_MAX_P = 32
+OP_BROADCAST, OP_REDUCE, OP_ALLREDUCE, OP_BSP_SGD = 0, 1, 2, 3
+VARIANT_PIPELINE, VARIANT_DIRECT, VARIANT_CLUSTER, VARIANT_COPY_ENGINE = 0, 1, 2, 3
+MODEL_STAGE, MODEL_LINK, MODEL_LINK_RING = 0, 1, 2
+TUNE_TILE_ELEMS, TUNE_STAGES, TUNE_OUT_STAGES, TUNE_CTAS_PER_SM, TUNE_CE_STREAMS, TUNE_L2_HINT = range(6)
+VARIANT_NAMES = {0: "pipeline", 1: "direct", 2: "cluster", 3: "copy_engine"}
+
+
+class LpError(RuntimeError):
+    def __init__(self, status, what):
+        self.status = status
+        super().__init__(f"{what}: status {status} ({status_string(status)})")
+
+
+class PlanInfo(ctypes.Structure):
+    _fields_ = [("nb", ctypes.c_uint64), ("n_tiles", ctypes.c_uint64), ("tile_elems", ctypes.c_uint32),
+                ("grid", ctypes.c_uint32), ("threads", ctypes.c_uint32), ("smem_bytes", ctypes.c_uint32),
+                ("stages", ctypes.c_uint32), ("out_stages", ctypes.c_uint32), ("variant", ctypes.c_uint32),
+                ("sm_count", ctypes.c_uint32)]
+
+    def as_dict(self):
+        return {k: int(getattr(self, k)) for k, _ in self._fields_}
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """Load liblp_b200.so (building it in-tree with nvcc if sources are newer). Raises if it cannot be had."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    so = _build.SO
+    if _build.needs_build():
+        if os.path.exists(_build.NVCC):
+            so = _build.build()
+        elif not os.path.exists(so):
+            raise RuntimeError("liblp_b200.so is missing and nvcc is not available: the CUDA library is the "
+                               "product, there is no fallback")
+    L = ctypes.CDLL(so)
+    pp = ctypes.POINTER(ctypes.c_void_p)
+    sz, i32, u64, f32, vp = ctypes.c_size_t, ctypes.c_int, ctypes.c_uint64, ctypes.c_float, ctypes.c_void_p
+    L.lp_broadcast.argtypes = [pp, i32, sz, sz, i32, vp]
+    L.lp_reduce.argtypes = [pp, i32, sz, sz, i32, vp]
+    L.lp_allreduce.argtypes = [pp, i32, sz, sz, vp]
+    L.lp_bsp_sgd_step.argtypes = [pp, pp, i32, sz, sz, i32, f32, vp]
+    for name in ("lp_mst_broadcast", "lp_mst_reduce", "lp_be_broadcast", "lp_be_reduce"):
+        getattr(L, name).argtypes = [pp, i32, sz, i32, vp]
+    for name in ("lp_mst_allreduce", "lp_be_allreduce"):
+        getattr(L, name).argtypes = [pp, i32, sz, vp]
+    L.lp_allreduce_host.argtypes = [pp, i32, sz, sz]
+    L.lp_bsp_sgd_step_host.argtypes = [pp, pp, i32, sz, sz, i32, f32]
+    L.lp_num_blocks.argtypes = [sz, sz]
+    L.lp_num_blocks.restype = u64
+    L.lp_stage_block.argtypes = [i32, u64, u64, i32]
+    L.lp_stage_block.restype = ctypes.c_int64
+    L.lp_schedule_steps.argtypes = [i32, sz, sz, i32, i32, ctypes.POINTER(u64)]
+    L.lp_mst_levels.argtypes = [i32]
+    L.lp_plan_query.argtypes = [i32, i32, sz, sz, ctypes.POINTER(PlanInfo)]
+    L.lp_min_bytes.argtypes = [i32, i32, sz]
+    L.lp_min_bytes.restype = u64
+    L.lp_set_variant.argtypes = [i32]
+    L.lp_set_tuning.argtypes = [i32, i32]
+    L.lp_get_tuning.argtypes = [i32]
+    L.lp_launch_count.restype = u64
+    L.lp_status_string.argtypes = [i32]
+    L.lp_status_string.restype = ctypes.c_char_p
+    _lib = L
+    return L
+
+
+def status_string(status: int) -> str:
+    return lib().lp_status_string(status).decode()
+
+
+def _check(rc, what):
+    if rc != LP_OK:
+        raise LpError(rc, what)
+
+
+def _dev_ptrs(bufs):
+    """Host array of device pointers from a list of CUDA float32 tensors (checks dtype / contiguity / length)."""
+    import torch
+    n = bufs[0].numel() if len(bufs) else 0
+    for b in bufs:
+        if not (isinstance(b, torch.Tensor) and b.is_cuda and b.dtype == torch.float32 and b.is_contiguous()):
+            raise TypeError("buffers must be contiguous float32 CUDA tensors")
+        if b.numel() != n:
+            raise ValueError("all ranks must hold vectors of the same length")
+    return (ctypes.c_void_p * len(bufs))(*[b.data_ptr() for b in bufs]), n
+
+
+def _host_ptrs(arrs):
+    """Host array of host pointers from numpy float32 arrays or CPU torch tensors (pinned for full speed)."""
+    ptrs, n = [], None
+    for a in arrs:
+        if hasattr(a, "data_ptr"):
+            if a.is_cuda or str(a.dtype) != "torch.float32" or not a.is_contiguous():
+                raise TypeError("host buffers must be contiguous float32 CPU tensors / numpy arrays")
+            p, m = a.data_ptr(), a.numel()
+        else:
+            if str(a.dtype) != "float32" or not a.flags.c_contiguous:
+                raise TypeError("host buffers must be contiguous float32 CPU tensors / numpy arrays")
+            p, m = a.ctypes.data, a.size
+        if n is not None and m != n:
+            raise ValueError("all ranks must hold vectors of the same length")
+        n = m
+        ptrs.append(p)
+    return (ctypes.c_void_p * len(ptrs))(*ptrs), (n or 0)
+
+
+def _stream_ptr(stream):
+    import torch
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return ctypes.c_void_p(s.cuda_stream)
+
+
+# ---- LP collectives ------------------------------------------------------------------------------------
+def lp_broadcast(bufs, block, root=0, stream=None):
+    arr, n = _dev_ptrs(bufs)
+    _check(lib().lp_broadcast(arr, len(bufs), n, block, root, _stream_ptr(stream)), "lp_broadcast")
+
+
+def lp_reduce(bufs, block, root=0, stream=None):
+    arr, n = _dev_ptrs(bufs)
+    _check(lib().lp_reduce(arr, len(bufs), n, block, root, _stream_ptr(stream)), "lp_reduce")
+
+
+def lp_allreduce(bufs, block, stream=None):
+    arr, n = _dev_ptrs(bufs)
+    _check(lib().lp_allreduce(arr, len(bufs), n, block, _stream_ptr(stream)), "lp_allreduce")
+
+
+def lp_bsp_sgd_step(grads, weights, block, root=0, lr=0.01, stream=None):
+    ga, n = _dev_ptrs(grads)
+    wa, nw = _dev_ptrs(weights)
+    if n != nw or len(grads) != len(weights):
+        raise ValueError("grads and weights must match in P and n")
+    _check(lib().lp_bsp_sgd_step(ga, wa, len(grads), n, block, root, ctypes.c_float(lr), _stream_ptr(stream)),
+           "lp_bsp_sgd_step")
+
+
+# ---- MST / BE baselines --------------------------------------------------------------------------------
+def _baseline(name, bufs, root, stream):
+    arr, n = _dev_ptrs(bufs)
+    f = getattr(lib(), name)
+    if root is None:
+        _check(f(arr, len(bufs), n, _stream_ptr(stream)), name)
+    else:
+        _check(f(arr, len(bufs), n, root, _stream_ptr(stream)), name)
+
+
+def lp_mst_broadcast(bufs, root=0, stream=None):
+    _baseline("lp_mst_broadcast", bufs, root, stream)
+
+
+def lp_mst_reduce(bufs, root=0, stream=None):
+    _baseline("lp_mst_reduce", bufs, root, stream)
+
+
+def lp_mst_allreduce(bufs, stream=None):
+    _baseline("lp_mst_allreduce", bufs, None, stream)
+
+
+def lp_be_broadcast(bufs, root=0, stream=None):
+    _baseline("lp_be_broadcast", bufs, root, stream)
+
+
+def lp_be_reduce(bufs, root=0, stream=None):
+    _baseline("lp_be_reduce", bufs, root, stream)
+
+
+def lp_be_allreduce(bufs, stream=None):
+    _baseline("lp_be_allreduce", bufs, None, stream)
+
+
+# ---- host-buffer entry points ----------------------------------------------------------------------------
+def lp_allreduce_host(host_bufs, block):
+    arr, n = _host_ptrs(host_bufs)
+    _check(lib().lp_allreduce_host(arr, len(host_bufs), n, block), "lp_allreduce_host")
+
+
+def lp_bsp_sgd_step_host(host_grads, host_weights, block, root=0, lr=0.01):
+    ga, n = _host_ptrs(host_grads)
+    wa, nw = _host_ptrs(host_weights)
+    if n != nw or len(host_grads) != len(host_weights):
+        raise ValueError("grads and weights must match in P and n")
+    _check(lib().lp_bsp_sgd_step_host(ga, wa, len(host_grads), n, block, root, ctypes.c_float(lr)),
+           "lp_bsp_sgd_step_host")
+
+
+# ---- schedule engine (host only) ---------------------------------------------------------------------------
+def lp_num_blocks(n, block) -> int:
+    return lib().lp_num_blocks(n, block)
+
+
+def lp_stage_block(P, nb, t, r) -> int:
+    return lib().lp_stage_block(P, nb, t, r)
+
+
+def lp_schedule_steps(P, n, block, op, model=MODEL_STAGE) -> int:
+    out = ctypes.c_uint64(0)
+    _check(lib().lp_schedule_steps(P, n, block, op, model, ctypes.byref(out)), "lp_schedule_steps")
+    return out.value
+
+
+def lp_mst_levels(P) -> int:
+    return lib().lp_mst_levels(P)
+
+
+def lp_plan_query(op, P, n, block) -> dict:
+    info = PlanInfo()
+    _check(lib().lp_plan_query(op, P, n, block, ctypes.byref(info)), "lp_plan_query")
+    return info.as_dict()
+
+
+def lp_min_bytes(op, P, n) -> int:
+    return lib().lp_min_bytes(op, P, n)
+
+
+# ---- control ---------------------------------------------------------------------------------------------
+def lp_set_variant(variant):
+    _check(lib().lp_set_variant(variant), "lp_set_variant")
+
+
+def lp_get_variant() -> int:
+    return lib().lp_get_variant()
+
+
+def lp_set_tuning(key, value):
+    _check(lib().lp_set_tuning(key, value), "lp_set_tuning")
+
+
+def lp_get_tuning(key) -> int:
+    return lib().lp_get_tuning(key)
+
+
+def lp_launch_count() -> int:
+    return lib().lp_launch_count()
+
+
+def lp_shutdown():
+    _check(lib().lp_shutdown(), "lp_shutdown")
+
+
+def lp_version() -> int:
+    return lib().lp_version()

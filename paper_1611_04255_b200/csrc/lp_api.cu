@@ -1,0 +1,465 @@
+// lp_api.cu -- the C ABI of include/lp_collectives.h: argument validation, the planner that turns
+// (op, P, n, block) into a kernel argument block + launch shape, variant dispatch, library scratch and the
+// host-buffer (end-to-end) entry points.  Every step of the path runs in the kernels of this library.
+#include <stdio.h>
+#include <string.h>
+
+#include <atomic>
+#include <mutex>
+
+#include "lp_common.cuh"
+
+cudaError_t lp_mst_run(int op, float *const *bufs, int P, size_t n, int root, int sm_count, cudaStream_t stream);
+cudaError_t lp_be_run(int op, float *const *bufs, int P, size_t n, int root, int sm_count, cudaStream_t stream);
+cudaError_t lp_copy_engine_run(int op, float *const *bufs, float *const *weights, int P, size_t n, size_t block,
+                               int root, float lr, const LpTuning &t, int sm_count, cudaStream_t stream);
+void lp_copy_engine_shutdown();
+
+namespace {
+
+std::mutex g_mu;
+int g_variant = LP_VARIANT_PIPELINE;
+LpTuning g_tuning = {{0, 0, 0, 0, 0, 0}};
+std::atomic<uint64_t> g_launches{0};
+char g_err[256] = "";
+int g_sm_count = 0;  // 0 = not queried yet
+
+constexpr int kScratchSlots = 2 * LP_MAX_P + 8;
+float *g_scratch[kScratchSlots];
+size_t g_scratch_bytes[kScratchSlots];
+
+int cuda_fail(cudaError_t e, const char *where) {
+    snprintf(g_err, sizeof(g_err), "CUDA error in %s: %s", where, cudaGetErrorString(e));
+    cudaGetLastError();  // clear the sticky-less error state
+    return LP_ERR_CUDA;
+}
+
+// SM count of the current device; <= 0 when there is no usable device.
+int sm_count_or_fail() {
+    if (g_sm_count > 0) return g_sm_count;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) {
+        cudaGetLastError();
+        return 0;
+    }
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+        cudaGetLastError();
+        return 0;
+    }
+    g_sm_count = sms;
+    return sms;
+}
+
+bool aligned16(const void *p) { return ((uintptr_t)p & 15u) == 0; }
+
+// NULL, alignment and pairwise-overlap checks over `count` buffers of n floats.
+int check_buffers(const float *const *ptrs, int count, size_t n) {
+    for (int i = 0; i < count; ++i)
+        if (ptrs[i] == nullptr || !aligned16(ptrs[i])) return LP_ERR_INVALID_ARG;
+    const size_t bytes = n * sizeof(float);
+    if (bytes == 0) return LP_OK;
+    for (int i = 0; i < count; ++i)
+        for (int j = i + 1; j < count; ++j) {
+            const uintptr_t a = (uintptr_t)ptrs[i], b = (uintptr_t)ptrs[j];
+            if (a < b + bytes && b < a + bytes) return LP_ERR_INVALID_ARG;
+        }
+    return LP_OK;
+}
+
+int validate(int op, float *const *bufs, float *const *weights, int P, size_t n, size_t block, int root) {
+    if (P < 1 || P > LP_MAX_P || bufs == nullptr || block == 0) return LP_ERR_INVALID_ARG;
+    if (root < 0 || root >= P) return LP_ERR_INVALID_ARG;
+    if (op == LP_OP_BSP_SGD && weights == nullptr) return LP_ERR_INVALID_ARG;
+    const float *all[2 * LP_MAX_P];
+    int m = 0;
+    for (int r = 0; r < P; ++r) all[m++] = bufs[r];
+    if (op == LP_OP_BSP_SGD)
+        for (int r = 0; r < P; ++r) all[m++] = weights[r];
+    return check_buffers(all, m, n);
+}
+
+// The kernel argument block of one collective (which vectors are folded, in which order; where the finished
+// tile goes).  The fold order is ALWAYS rank 0 -> P-1 (U4); `root` only selects sources / destinations.
+void fill_args(LpArgs &a, int op, float *const *bufs, float *const *weights, int P, int root, float lr) {
+    memset(&a, 0, sizeof(a));
+    a.lr = lr;
+    a.invP = 1.0f / (float)P;  // one RN division on the host (U7)
+    a.l2_hint = g_tuning.v[LP_TUNE_L2_HINT];
+    switch (op) {
+        case LP_OP_BROADCAST:
+            a.epilogue = LP_EPI_COPY;
+            a.n_sum = a.n_in = 1;
+            a.in[0] = bufs[root];
+            for (int r = 0; r < P; ++r)
+                if (r != root) a.out[a.n_out++] = bufs[r];
+            break;
+        case LP_OP_REDUCE:
+        case LP_OP_ALLREDUCE:
+            a.epilogue = LP_EPI_SUM;
+            a.n_sum = a.n_in = P;
+            for (int r = 0; r < P; ++r) a.in[r] = bufs[r];
+            if (op == LP_OP_REDUCE) {
+                a.out[a.n_out++] = bufs[root];
+            } else {
+                for (int r = 0; r < P; ++r) a.out[a.n_out++] = bufs[r];
+            }
+            break;
+        default:  // LP_OP_BSP_SGD
+            a.epilogue = LP_EPI_SGD;
+            a.n_sum = P;
+            a.n_in = P + 1;
+            for (int r = 0; r < P; ++r) a.in[r] = bufs[r];
+            a.in[P] = weights[root];
+            for (int r = 0; r < P; ++r) a.out[a.n_out++] = weights[r];
+            break;
+    }
+}
+
+// Variant that will really run: the TMA pipeline needs every tile to start on a 16-byte boundary.
+int effective_variant(int variant, size_t n, size_t block) {
+    if (variant == LP_VARIANT_PIPELINE || variant == LP_VARIANT_CLUSTER) {
+        const uint64_t nb = lp_num_blocks(n, block);
+        if (nb > 1 && (block % 4) != 0) return LP_VARIANT_DIRECT;
+    }
+    return variant;
+}
+
+// Plans (and unless dry_run, enqueues) one LP collective on device buffers.
+int plan_and_run(int op, float *const *bufs, float *const *weights, int P, size_t n, size_t block, int root, float lr,
+                 int sm_count, lp_plan_info *info, bool dry_run, cudaStream_t stream) {
+    const int variant = effective_variant(g_variant, n, block);
+    LpArgs a;
+    LpLaunch cfg = {0, 0, 0, 0, 0};
+    if (!dry_run)
+        fill_args(a, op, bufs, weights, P, root, lr);
+    else {
+        memset(&a, 0, sizeof(a));
+        a.epilogue = op == LP_OP_BROADCAST ? LP_EPI_COPY : (op == LP_OP_BSP_SGD ? LP_EPI_SGD : LP_EPI_SUM);
+        a.n_sum = op == LP_OP_BROADCAST ? 1 : P;
+        a.n_in = a.n_sum + (op == LP_OP_BSP_SGD ? 1 : 0);
+        a.n_out = op == LP_OP_BROADCAST ? P - 1 : (op == LP_OP_REDUCE ? 1 : P);
+    }
+    uint32_t tile;
+    switch (variant) {
+        case LP_VARIANT_DIRECT: tile = lp_direct_tile(g_tuning, a.n_in); break;
+        case LP_VARIANT_CLUSTER: tile = lp_cluster_tile(g_tuning); break;
+        default: tile = lp_pipeline_tile(g_tuning, n, block); break;
+    }
+    a.part = lp_make_partition(n, block, tile);
+    // identity collectives: nothing to move (P == 1 broadcast/reduce/allreduce; n == 0)
+    const bool noop = (n == 0) || (P == 1 && op != LP_OP_BSP_SGD);
+    cudaError_t e = cudaSuccess;
+    if (variant == LP_VARIANT_COPY_ENGINE) {
+        cfg.grid = cfg.threads = 0;
+        if (!dry_run && !noop) e = lp_copy_engine_run(op, bufs, weights, P, n, block, root, lr, g_tuning, sm_count, stream);
+    } else if (variant == LP_VARIANT_DIRECT) {
+        e = lp_direct_launch(a, g_tuning, sm_count, &cfg, dry_run || noop, stream);
+    } else if (variant == LP_VARIANT_CLUSTER) {
+        e = lp_cluster_launch(a, g_tuning, sm_count, &cfg, dry_run || noop, stream);
+        if (e == cudaErrorNotSupported) return LP_ERR_UNSUPPORTED;
+    } else {
+        e = lp_pipeline_launch(a, g_tuning, sm_count, &cfg, dry_run || noop, stream);
+    }
+    if (info) {
+        info->nb = a.part.nb;
+        info->n_tiles = a.part.n_tiles;
+        info->tile_elems = tile;
+        info->grid = cfg.grid;
+        info->threads = cfg.threads;
+        info->smem_bytes = cfg.smem_bytes;
+        info->stages = cfg.stages;
+        info->out_stages = cfg.out_stages;
+        info->variant = (uint32_t)variant;
+        info->sm_count = (uint32_t)sm_count;
+    }
+    if (e != cudaSuccess) return cuda_fail(e, "LP launch");
+    return LP_OK;
+}
+
+int run_device(int op, float *const *bufs, float *const *weights, int P, size_t n, size_t block, int root, float lr,
+               void *cuda_stream) {
+    int rc = validate(op, bufs, weights, P, n, block, root);
+    if (rc != LP_OK) return rc;
+    std::lock_guard<std::mutex> lock(g_mu);
+    if (g_variant == LP_VARIANT_CLUSTER && P > 16) return LP_ERR_UNSUPPORTED;
+    const int sms = sm_count_or_fail();
+    if (sms <= 0) {
+        snprintf(g_err, sizeof(g_err), "no CUDA device: liblp_b200 has no CPU fallback");
+        return LP_ERR_CUDA;
+    }
+    return plan_and_run(op, bufs, weights, P, n, block, root, lr, sms, nullptr, false, (cudaStream_t)cuda_stream);
+}
+
+int run_baseline(bool be, int op, float *const *bufs, int P, size_t n, int root, void *cuda_stream) {
+    int rc = validate(op, bufs, nullptr, P, n, 1, root);
+    if (rc != LP_OK) return rc;
+    if (be && (P & (P - 1)) != 0) return LP_ERR_UNSUPPORTED;  // U14
+    std::lock_guard<std::mutex> lock(g_mu);
+    const int sms = sm_count_or_fail();
+    if (sms <= 0) {
+        snprintf(g_err, sizeof(g_err), "no CUDA device: liblp_b200 has no CPU fallback");
+        return LP_ERR_CUDA;
+    }
+    cudaError_t e = be ? lp_be_run(op, bufs, P, n, root, sms, (cudaStream_t)cuda_stream)
+                       : lp_mst_run(op, bufs, P, n, root, sms, (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return cuda_fail(e, be ? "BE baseline" : "MST baseline");
+    return LP_OK;
+}
+
+}  // namespace
+
+void lp_count_launch(uint64_t k) { g_launches.fetch_add(k, std::memory_order_relaxed); }
+
+// Library scratch: grows on demand (cudaFree synchronises the device, so growing is safe against work in flight).
+cudaError_t lp_scratch_get(int slot, size_t bytes, float **ptr) {
+    if (slot < 0 || slot >= kScratchSlots) return cudaErrorInvalidValue;
+    if (g_scratch_bytes[slot] < bytes) {
+        if (g_scratch[slot]) cudaFree(g_scratch[slot]);
+        g_scratch[slot] = nullptr;
+        g_scratch_bytes[slot] = 0;
+        cudaError_t e = cudaMalloc((void **)&g_scratch[slot], bytes);
+        if (e != cudaSuccess) return e;
+        g_scratch_bytes[slot] = bytes;
+    }
+    *ptr = g_scratch[slot];
+    return cudaSuccess;
+}
+
+// ---- host-buffer (end-to-end) path ---------------------------------------------------------------------
+// The LP idea applied to the host link as well: the message is cut into chunks that flow
+// host -> device (stream up) -> LP kernel (stream mid) -> host (stream down); three chunk sets rotate, so
+// the upload of chunk c+1, the kernel on chunk c and the download of chunk c-1 overlap (PCI-E is full duplex).
+namespace {
+
+constexpr size_t kChunkElems = 4u << 20;  // 16 MB per rank per chunk
+constexpr int kSets = 3;
+cudaStream_t g_up, g_mid, g_down;
+cudaEvent_t g_ev_up[kSets], g_ev_done[kSets], g_ev_down[kSets];
+bool g_host_ready = false;
+
+#define LP_TRYC(x, where)                                  \
+    do {                                                   \
+        cudaError_t e__ = (x);                             \
+        if (e__ != cudaSuccess) return cuda_fail(e__, where); \
+    } while (0)
+
+int host_init() {
+    if (g_host_ready) return LP_OK;
+    LP_TRYC(cudaStreamCreateWithFlags(&g_up, cudaStreamNonBlocking), "host path init");
+    LP_TRYC(cudaStreamCreateWithFlags(&g_mid, cudaStreamNonBlocking), "host path init");
+    LP_TRYC(cudaStreamCreateWithFlags(&g_down, cudaStreamNonBlocking), "host path init");
+    for (int s = 0; s < kSets; ++s) {
+        LP_TRYC(cudaEventCreateWithFlags(&g_ev_up[s], cudaEventDisableTiming), "host path init");
+        LP_TRYC(cudaEventCreateWithFlags(&g_ev_done[s], cudaEventDisableTiming), "host path init");
+        LP_TRYC(cudaEventCreateWithFlags(&g_ev_down[s], cudaEventDisableTiming), "host path init");
+    }
+    g_host_ready = true;
+    return LP_OK;
+}
+
+int run_host(int op, float *const *hbufs, float *const *hweights, int P, size_t n, size_t block, int root, float lr) {
+    // host pointers: same structural checks, but only 4-byte alignment is needed
+    if (P < 1 || P > LP_MAX_P || hbufs == nullptr || block == 0 || root < 0 || root >= P) return LP_ERR_INVALID_ARG;
+    if (op == LP_OP_BSP_SGD && hweights == nullptr) return LP_ERR_INVALID_ARG;
+    for (int r = 0; r < P; ++r) {
+        if (hbufs[r] == nullptr || ((uintptr_t)hbufs[r] & 3u)) return LP_ERR_INVALID_ARG;
+        if (op == LP_OP_BSP_SGD && (hweights[r] == nullptr || ((uintptr_t)hweights[r] & 3u))) return LP_ERR_INVALID_ARG;
+    }
+    std::lock_guard<std::mutex> lock(g_mu);
+    const int sms = sm_count_or_fail();
+    if (sms <= 0) {
+        snprintf(g_err, sizeof(g_err), "no CUDA device: liblp_b200 has no CPU fallback");
+        return LP_ERR_CUDA;
+    }
+    if (n == 0) return LP_OK;
+    int rc = host_init();
+    if (rc != LP_OK) return rc;
+    const bool sgd = (op == LP_OP_BSP_SGD);
+    // chunk: a multiple of the LP block (so block boundaries fall where they would in the whole message)
+    size_t chunk = kChunkElems;
+    if (block < chunk) chunk = (chunk / block) * block;
+    else chunk = block;
+    if (chunk > n) chunk = n;
+    const size_t stride = (chunk + 63) & ~(size_t)63;  // keeps every device vector 16-byte (256-byte) aligned
+    const int per_set = sgd ? 2 * P : P;
+    float *set_base[kSets];
+    for (int s = 0; s < kSets; ++s)
+        LP_TRYC(lp_scratch_get(2 * LP_MAX_P + s, (size_t)per_set * stride * sizeof(float), &set_base[s]), "host path scratch");
+
+    const size_t n_chunks = (n + chunk - 1) / chunk;
+    for (size_t c = 0; c < n_chunks; ++c) {
+        const int s = (int)(c % kSets);
+        const size_t off = c * chunk;
+        const size_t len = off + chunk <= n ? chunk : n - off;
+        float *dg[LP_MAX_P], *dw[LP_MAX_P];
+        for (int r = 0; r < P; ++r) {
+            dg[r] = set_base[s] + (size_t)r * stride;
+            dw[r] = set_base[s] + (size_t)(P + r) * stride;
+        }
+        // upload (after the previous user of this set has been downloaded)
+        if (c >= (size_t)kSets) LP_TRYC(cudaStreamWaitEvent(g_up, g_ev_down[s], 0), "host path");
+        for (int r = 0; r < P; ++r)
+            LP_TRYC(cudaMemcpyAsync(dg[r], hbufs[r] + off, len * sizeof(float), cudaMemcpyHostToDevice, g_up), "H2D");
+        if (sgd)  // only the root's replica is read (U8)
+            LP_TRYC(cudaMemcpyAsync(dw[root], hweights[root] + off, len * sizeof(float), cudaMemcpyHostToDevice, g_up), "H2D");
+        lp_count_launch((uint64_t)P + (sgd ? 1 : 0));
+        LP_TRYC(cudaEventRecord(g_ev_up[s], g_up), "host path");
+        // LP kernel
+        LP_TRYC(cudaStreamWaitEvent(g_mid, g_ev_up[s], 0), "host path");
+        rc = plan_and_run(op, dg, sgd ? dw : nullptr, P, len, block, root, lr, sms, nullptr, false, g_mid);
+        if (rc != LP_OK) return rc;
+        LP_TRYC(cudaEventRecord(g_ev_done[s], g_mid), "host path");
+        // download
+        LP_TRYC(cudaStreamWaitEvent(g_down, g_ev_done[s], 0), "host path");
+        for (int r = 0; r < P; ++r) {
+            float *src = sgd ? dw[r] : dg[r];
+            float *dst = sgd ? hweights[r] : hbufs[r];
+            LP_TRYC(cudaMemcpyAsync(dst + off, src, len * sizeof(float), cudaMemcpyDeviceToHost, g_down), "D2H");
+        }
+        lp_count_launch((uint64_t)P);
+        LP_TRYC(cudaEventRecord(g_ev_down[s], g_down), "host path");
+    }
+    LP_TRYC(cudaStreamSynchronize(g_down), "host path sync");
+    return LP_OK;
+}
+
+}  // namespace
+
+// ---- C ABI -----------------------------------------------------------------------------------------------
+extern "C" {
+
+int lp_broadcast(float *const *bufs, int P, size_t n, size_t block, int root, void *cuda_stream) {
+    return run_device(LP_OP_BROADCAST, bufs, nullptr, P, n, block, root, 0.f, cuda_stream);
+}
+int lp_reduce(float *const *bufs, int P, size_t n, size_t block, int root, void *cuda_stream) {
+    return run_device(LP_OP_REDUCE, bufs, nullptr, P, n, block, root, 0.f, cuda_stream);
+}
+int lp_allreduce(float *const *bufs, int P, size_t n, size_t block, void *cuda_stream) {
+    return run_device(LP_OP_ALLREDUCE, bufs, nullptr, P, n, block, 0, 0.f, cuda_stream);
+}
+int lp_bsp_sgd_step(float *const *grads, float *const *weights, int P, size_t n, size_t block, int root, float lr,
+                    void *cuda_stream) {
+    return run_device(LP_OP_BSP_SGD, grads, weights, P, n, block, root, lr, cuda_stream);
+}
+
+int lp_mst_broadcast(float *const *bufs, int P, size_t n, int root, void *s) {
+    return run_baseline(false, LP_OP_BROADCAST, bufs, P, n, root, s);
+}
+int lp_mst_reduce(float *const *bufs, int P, size_t n, int root, void *s) {
+    return run_baseline(false, LP_OP_REDUCE, bufs, P, n, root, s);
+}
+int lp_mst_allreduce(float *const *bufs, int P, size_t n, void *s) {
+    return run_baseline(false, LP_OP_ALLREDUCE, bufs, P, n, 0, s);
+}
+int lp_be_broadcast(float *const *bufs, int P, size_t n, int root, void *s) {
+    return run_baseline(true, LP_OP_BROADCAST, bufs, P, n, root, s);
+}
+int lp_be_reduce(float *const *bufs, int P, size_t n, int root, void *s) {
+    return run_baseline(true, LP_OP_REDUCE, bufs, P, n, root, s);
+}
+int lp_be_allreduce(float *const *bufs, int P, size_t n, void *s) {
+    return run_baseline(true, LP_OP_ALLREDUCE, bufs, P, n, 0, s);
+}
+
+int lp_allreduce_host(float *const *host_bufs, int P, size_t n, size_t block) {
+    return run_host(LP_OP_ALLREDUCE, host_bufs, nullptr, P, n, block, 0, 0.f);
+}
+int lp_bsp_sgd_step_host(float *const *host_grads, float *const *host_weights, int P, size_t n, size_t block, int root,
+                         float lr) {
+    return run_host(LP_OP_BSP_SGD, host_grads, host_weights, P, n, block, root, lr);
+}
+
+int lp_plan_query(int op, int P, size_t n, size_t block, lp_plan_info *out) {
+    if (out == nullptr || P < 1 || P > LP_MAX_P || block == 0) return LP_ERR_INVALID_ARG;
+    if (op < LP_OP_BROADCAST || op > LP_OP_BSP_SGD) return LP_ERR_INVALID_ARG;
+    std::lock_guard<std::mutex> lock(g_mu);
+    int sms = sm_count_or_fail();
+    if (sms <= 0) sms = 148;  // planning works without a device: a B200 has 148 SMs
+    memset(out, 0, sizeof(*out));
+    return plan_and_run(op, nullptr, nullptr, P, n, block, 0, 0.f, sms, out, true, nullptr);
+}
+
+uint64_t lp_min_bytes(int op, int P, size_t n) {
+    const uint64_t v = (uint64_t)n * 4u;
+    switch (op) {
+        case LP_OP_BROADCAST: return (uint64_t)P * v;
+        case LP_OP_REDUCE: return (uint64_t)(P + 1) * v;
+        case LP_OP_ALLREDUCE: return 2u * (uint64_t)P * v;
+        case LP_OP_BSP_SGD: return (2u * (uint64_t)P + 1u) * v;
+        default: return 0;
+    }
+}
+
+int lp_set_variant(int variant) {
+    if (variant < LP_VARIANT_PIPELINE || variant > LP_VARIANT_COPY_ENGINE) return LP_ERR_INVALID_ARG;
+    std::lock_guard<std::mutex> lock(g_mu);
+    g_variant = variant;
+    return LP_OK;
+}
+int lp_get_variant(void) { return g_variant; }
+
+int lp_set_tuning(int key, int value) {
+    if (key < 0 || key >= LP_TUNE_COUNT || value < 0) return LP_ERR_INVALID_ARG;
+    switch (key) {
+        case LP_TUNE_TILE_ELEMS:
+            if (value != 0 && value != 1024 && value != 2048 && value != 4096 && value != 8192) return LP_ERR_INVALID_ARG;
+            break;
+        case LP_TUNE_STAGES:
+            if (value != 0 && (value < 2 || value > 32)) return LP_ERR_INVALID_ARG;
+            break;
+        case LP_TUNE_OUT_STAGES:
+        case LP_TUNE_CTAS_PER_SM:
+        case LP_TUNE_CE_STREAMS:
+            if (value > 8) return LP_ERR_INVALID_ARG;
+            break;
+        case LP_TUNE_L2_HINT:
+            if (value > 2) return LP_ERR_INVALID_ARG;
+            break;
+    }
+    std::lock_guard<std::mutex> lock(g_mu);
+    g_tuning.v[key] = value;
+    return LP_OK;
+}
+int lp_get_tuning(int key) { return (key < 0 || key >= LP_TUNE_COUNT) ? -1 : g_tuning.v[key]; }
+
+uint64_t lp_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+int lp_shutdown(void) {
+    std::lock_guard<std::mutex> lock(g_mu);
+    bool any = g_host_ready;
+    for (int s = 0; s < kScratchSlots; ++s) any = any || g_scratch[s] != nullptr;
+    if (any) cudaDeviceSynchronize();
+    for (int s = 0; s < kScratchSlots; ++s) {
+        if (g_scratch[s]) cudaFree(g_scratch[s]);
+        g_scratch[s] = nullptr;
+        g_scratch_bytes[s] = 0;
+    }
+    lp_copy_engine_shutdown();
+    if (g_host_ready) {
+        cudaStreamDestroy(g_up);
+        cudaStreamDestroy(g_mid);
+        cudaStreamDestroy(g_down);
+        for (int s = 0; s < kSets; ++s) {
+            cudaEventDestroy(g_ev_up[s]);
+            cudaEventDestroy(g_ev_done[s]);
+            cudaEventDestroy(g_ev_down[s]);
+        }
+        g_host_ready = false;
+    }
+    cudaGetLastError();
+    return LP_OK;
+}
+
+const char *lp_status_string(int status) {
+    switch (status) {
+        case LP_OK: return "LP_OK";
+        case LP_ERR_INVALID_ARG: return "LP_ERR_INVALID_ARG: bad P / pointer / block / root / alignment / overlap";
+        case LP_ERR_UNSUPPORTED: return "LP_ERR_UNSUPPORTED: BE needs a power-of-two P; cluster variant needs P <= 16";
+        case LP_ERR_CUDA: return g_err[0] ? g_err : "LP_ERR_CUDA";
+        default: return "unknown status";
+    }
+}
+
+int lp_version(void) { return 100; }  // 0.1.0
+
+}  // extern "C"

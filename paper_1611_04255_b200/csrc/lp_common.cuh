@@ -1,0 +1,176 @@
+// lp_common.cuh -- kernel argument block, PTX wrappers (mbarrier, TMA bulk copies) and the
+// internal launcher interface between lp_api.cu and the kernel translation units.  sm_100a only.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/lp_collectives.h"
+#include "lp_schedule.h"
+
+#define LP_MAX_IN (LP_MAX_P + 1)  // P gradient vectors + the root's weight vector
+
+// Epilogues of the chain fold.
+#define LP_EPI_SUM 0   // out = ((in0 + in1) + ...) + in[n_sum-1]
+#define LP_EPI_SGD 1   // out = in[n_sum] - lr * (S * invP), three RN ops      PAPER.md:172,174 (U7)
+#define LP_EPI_COPY 2  // out = in0 (broadcast)
+
+// One launch = one collective.  in[0..n_sum) are folded in that order (rank 0 -> P-1); for LP_EPI_SGD
+// in[n_sum] is weights[root]; out[0..n_out) all receive the finished tile.
+struct LpArgs {
+    const float *in[LP_MAX_IN];
+    float *out[LP_MAX_P];
+    int n_sum;     // number of folded inputs (1 for broadcast)
+    int n_in;      // n_sum (+1 for SGD)
+    int n_out;
+    int epilogue;
+    float lr, invP;
+    int l2_hint;
+    lp_partition part;
+};
+
+struct LpLaunch {
+    uint32_t grid, threads, smem_bytes, stages, out_stages;
+};
+
+// Tuning state resolved by the API layer (0 = default).
+struct LpTuning {
+    int v[LP_TUNE_COUNT];
+};
+
+// ---- launchers implemented in the kernel translation units ----------------------------------------
+// Each fills `cfg` (always) and, unless dry_run, enqueues the kernel(s) on `stream`.  Return cudaError_t.
+cudaError_t lp_pipeline_launch(const LpArgs &a, const LpTuning &t, int sm_count, LpLaunch *cfg, bool dry_run,
+                               cudaStream_t stream);
+cudaError_t lp_direct_launch(const LpArgs &a, const LpTuning &t, int sm_count, LpLaunch *cfg, bool dry_run,
+                             cudaStream_t stream);
+cudaError_t lp_cluster_launch(const LpArgs &a, const LpTuning &t, int sm_count, LpLaunch *cfg, bool dry_run,
+                              cudaStream_t stream);
+uint32_t lp_pipeline_tile(const LpTuning &t, uint64_t n, uint64_t block);
+uint32_t lp_direct_tile(const LpTuning &t, int n_in);
+uint32_t lp_cluster_tile(const LpTuning &t);
+
+// Segment jobs of the MST / BE baselines: dst[i] = a[i] + b[i] (b != NULL) or dst[i] = a[i], i in [0, len).
+struct LpSegJob {
+    float *dst;
+    const float *a;
+    const float *b;
+    uint64_t len;
+};
+#define LP_MAX_JOBS 32
+cudaError_t lp_seg_launch(const LpSegJob *jobs, int n_jobs, int sm_count, cudaStream_t stream);
+
+// Launch counter (kernels + async copies enqueued by the library).
+void lp_count_launch(uint64_t k);
+
+#if defined(__CUDACC__)
+// ---- PTX wrappers ------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t lp_smem_u32(const void *p) {
+    return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void lp_mbar_init(uint64_t *bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(lp_smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void lp_fence_mbar_init() {
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void lp_mbar_arrive(uint64_t *bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(lp_smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void lp_mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(lp_smem_u32(bar)), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void lp_mbar_wait(uint64_t *bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "LP_WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra LP_DONE_%=;\n"
+        "bra LP_WAIT_%=;\n"
+        "LP_DONE_%=:\n"
+        "}\n" ::"r"(lp_smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+// generic-proxy writes to shared memory -> visible to the async proxy (TMA store)
+__device__ __forceinline__ void lp_fence_proxy_async() {
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+__device__ __forceinline__ uint64_t lp_policy_evict_first() {
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+// TMA bulk copy global -> shared, completion counted in bytes on an mbarrier (SASS: UBLKCP)
+__device__ __forceinline__ void lp_bulk_g2s(void *smem_dst, const void *gsrc, uint32_t bytes, uint64_t *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     lp_smem_u32(smem_dst)),
+                 "l"(gsrc), "r"(bytes), "r"(lp_smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void lp_bulk_g2s_hint(void *smem_dst, const void *gsrc, uint32_t bytes, uint64_t *bar,
+                                                 uint64_t pol) {
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::
+            "r"(lp_smem_u32(smem_dst)),
+        "l"(gsrc), "r"(bytes), "r"(lp_smem_u32(bar)), "l"(pol)
+        : "memory");
+}
+// TMA bulk copy shared -> global, tracked by bulk async-groups
+__device__ __forceinline__ void lp_bulk_s2g(void *gdst, const void *smem_src, uint32_t bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst),
+                 "r"(lp_smem_u32(smem_src)), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void lp_bulk_s2g_hint(void *gdst, const void *smem_src, uint32_t bytes, uint64_t pol) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;" ::"l"(gdst),
+                 "r"(lp_smem_u32(smem_src)), "r"(bytes), "l"(pol)
+                 : "memory");
+}
+__device__ __forceinline__ void lp_bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void lp_bulk_wait_read() {
+    asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory");
+}
+template <int N>
+__device__ __forceinline__ void lp_bulk_wait() {
+    asm volatile("cp.async.bulk.wait_group %0;" ::"n"(N) : "memory");
+}
+
+// 128-bit streaming global accesses (no L1 allocation; every byte is touched once)
+__device__ __forceinline__ float4 lp_ldg_stream(const float *p) {
+    float4 v;
+    asm volatile("ld.global.L1::no_allocate.v4.f32 {%0, %1, %2, %3}, [%4];"
+                 : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
+                 : "l"(p));
+    return v;
+}
+__device__ __forceinline__ void lp_stg_stream(float *p, const float4 &v) {
+    asm volatile("st.global.L1::no_allocate.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(v.x), "f"(v.y),
+                 "f"(v.z), "f"(v.w)
+                 : "memory");
+}
+
+// fp32 RN arithmetic that ptxas may not contract into FMA
+__device__ __forceinline__ float4 lp_add4(const float4 &a, const float4 &b) {
+    return make_float4(__fadd_rn(a.x, b.x), __fadd_rn(a.y, b.y), __fadd_rn(a.z, b.z), __fadd_rn(a.w, b.w));
+}
+// w' = w - lr * (s * invP): three separately rounded operations (U7)
+__device__ __forceinline__ float lp_sgd1(float s, float w, float lr, float invP) {
+    return __fsub_rn(w, __fmul_rn(lr, __fmul_rn(s, invP)));
+}
+__device__ __forceinline__ float4 lp_sgd4(const float4 &s, const float4 &w, float lr, float invP) {
+    return make_float4(lp_sgd1(s.x, w.x, lr, invP), lp_sgd1(s.y, w.y, lr, invP), lp_sgd1(s.z, w.z, lr, invP),
+                       lp_sgd1(s.w, w.w, lr, invP));
+}
+
+// Scalar path for the (at most a few) elements of a tile outside its 16-byte aligned body: the chain fold,
+// epilogue and fan-out for element i, straight from and to global memory.
+__device__ __forceinline__ void lp_scalar_element(const LpArgs &a, uint64_t i) {
+    float s = a.in[0][i];
+    for (int r = 1; r < a.n_sum; ++r) s = __fadd_rn(s, a.in[r][i]);
+    if (a.epilogue == LP_EPI_SGD) s = lp_sgd1(s, a.in[a.n_sum][i], a.lr, a.invP);
+    for (int q = 0; q < a.n_out; ++q) a.out[q][i] = s;
+}
+#endif  // __CUDACC__

@@ -1,0 +1,123 @@
+// lp_direct.cu -- LP_VARIANT_DIRECT: the LP collective as one persistent kernel that keeps the running
+// partial of the chain (a0 -> a' = a0 + a1 -> a'' = a' + a2) in registers.  Each thread owns V
+// 16-byte vectors of a tile, issues the 128-bit streaming loads of up to 8 ranks at once (memory-level
+// parallelism replaces the paper's two DMA engines), folds them in rank order 0 -> P-1 with RN adds and
+// writes the finished vector to every destination rank.  It is also the path that takes any alignment:
+// a tile whose start is not a multiple of 4 elements (block % 4 != 0) gets a scalar head and tail.
+#include "lp_common.cuh"
+
+namespace {
+
+constexpr int kThreads = 256;
+constexpr int kRankChunk = 8;  // ranks whose loads are in flight together
+
+// NS > 0: number of folded inputs known at compile time (loops fully unrolled); NS == 0: runtime a.n_sum.
+template <int NS, int V>
+__global__ void __launch_bounds__(kThreads) lp_direct_kernel(const __grid_constant__ LpArgs a) {
+    const lp_partition &part = a.part;
+    const int n_sum = NS > 0 ? NS : a.n_sum;
+    const int tid = threadIdx.x;
+    for (uint64_t t = blockIdx.x; t < part.n_tiles; t += gridDim.x) {
+        uint64_t off;
+        uint32_t len;
+        lp_tile_range(part, t, off, len);
+        const uint64_t end = off + len;
+        uint64_t a0 = (off + 3) & ~(uint64_t)3;  // first 16-byte aligned element (all buffers are 16-byte aligned)
+        if (a0 > end) a0 = end;
+        uint64_t a1 = end & ~(uint64_t)3;
+        if (a1 < a0) a1 = a0;
+        const uint32_t nvec = (uint32_t)((a1 - a0) >> 2);
+        if ((uint64_t)tid < a0 - off) lp_scalar_element(a, off + tid);
+        if ((uint64_t)tid < end - a1) lp_scalar_element(a, a1 + tid);
+
+        float4 acc[V];
+        float4 w[V];
+        bool live[V];
+#pragma unroll
+        for (int v = 0; v < V; ++v) live[v] = (uint32_t)(tid + v * kThreads) < nvec;
+        if (a.epilogue == LP_EPI_SGD) {
+#pragma unroll
+            for (int v = 0; v < V; ++v)
+                if (live[v]) w[v] = lp_ldg_stream(a.in[n_sum] + a0 + 4 * (uint64_t)(tid + v * kThreads));
+        }
+        for (int r0 = 0; r0 < n_sum; r0 += kRankChunk) {
+            float4 x[V][kRankChunk];
+#pragma unroll
+            for (int j = 0; j < kRankChunk; ++j) {
+                if (NS > 0 ? (r0 + j < NS) : (r0 + j < n_sum)) {
+#pragma unroll
+                    for (int v = 0; v < V; ++v)
+                        if (live[v]) x[v][j] = lp_ldg_stream(a.in[r0 + j] + a0 + 4 * (uint64_t)(tid + v * kThreads));
+                }
+            }
+#pragma unroll
+            for (int j = 0; j < kRankChunk; ++j) {
+                if (NS > 0 ? (r0 + j < NS) : (r0 + j < n_sum)) {
+#pragma unroll
+                    for (int v = 0; v < V; ++v) acc[v] = (r0 + j == 0) ? x[v][j] : lp_add4(acc[v], x[v][j]);
+                }
+            }
+        }
+        if (a.epilogue == LP_EPI_SGD) {
+#pragma unroll
+            for (int v = 0; v < V; ++v) acc[v] = lp_sgd4(acc[v], w[v], a.lr, a.invP);
+        }
+        for (int q = 0; q < a.n_out; ++q) {
+#pragma unroll
+            for (int v = 0; v < V; ++v)
+                if (live[v]) lp_stg_stream(a.out[q] + a0 + 4 * (uint64_t)(tid + v * kThreads), acc[v]);
+        }
+    }
+}
+
+template <int V>
+cudaError_t launch_v(const LpArgs &a, const LpLaunch &cfg, cudaStream_t stream) {
+#define LP_DIRECT_CASE(NS)                                                         \
+    case NS:                                                                       \
+        lp_direct_kernel<NS, V><<<cfg.grid, cfg.threads, 0, stream>>>(a);         \
+        break;
+    switch (a.n_sum) {
+        LP_DIRECT_CASE(1)
+        LP_DIRECT_CASE(2)
+        LP_DIRECT_CASE(3)
+        LP_DIRECT_CASE(4)
+        LP_DIRECT_CASE(5)
+        LP_DIRECT_CASE(6)
+        LP_DIRECT_CASE(7)
+        LP_DIRECT_CASE(8)
+        LP_DIRECT_CASE(16)
+        default:
+            lp_direct_kernel<0, V><<<cfg.grid, cfg.threads, 0, stream>>>(a);
+            break;
+    }
+#undef LP_DIRECT_CASE
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+uint32_t lp_direct_tile(const LpTuning &t, int /*n_in*/) {
+    uint32_t tile = t.v[LP_TUNE_TILE_ELEMS] ? (uint32_t)t.v[LP_TUNE_TILE_ELEMS] : 2048u;
+    if (tile != 1024u && tile != 2048u && tile != 4096u) tile = 2048u;
+    return tile;
+}
+
+cudaError_t lp_direct_launch(const LpArgs &a, const LpTuning &t, int sm_count, LpLaunch *cfg, bool dry_run,
+                             cudaStream_t stream) {
+    const uint32_t ctas = t.v[LP_TUNE_CTAS_PER_SM] ? (uint32_t)t.v[LP_TUNE_CTAS_PER_SM] : 4u;
+    uint64_t grid = (uint64_t)sm_count * ctas;
+    if (grid > a.part.n_tiles) grid = a.part.n_tiles;
+    cfg->grid = (uint32_t)grid;
+    cfg->threads = kThreads;
+    cfg->smem_bytes = 0;
+    cfg->stages = 0;
+    cfg->out_stages = 0;
+    if (dry_run || grid == 0) return cudaSuccess;
+    lp_count_launch(1);
+    switch (a.part.tile) {
+        case 1024: return launch_v<1>(a, *cfg, stream);
+        case 2048: return launch_v<2>(a, *cfg, stream);
+        case 4096: return launch_v<4>(a, *cfg, stream);
+        default: return cudaErrorInvalidValue;
+    }
+}

@@ -1,0 +1,376 @@
+// lp_pipeline.cu -- LP_VARIANT_PIPELINE: the whole LP collective as ONE persistent sm_100a kernel.
+//
+// What survives of the paper's design on one B200: the message is cut into
+// blocks and each block flows down the chain rank 0 -> 1 -> ... -> P-1, every rank adding its
+// local block to the partial it received -- but the partial never goes back to HBM between
+// hops.  Per CTA:
+//
+//   producer warp   one thread issues TMA bulk loads (cp.async.bulk global -> shared) of (tile, rank r),
+//                   r = 0..P-1 in chain order, into a ring of `stages` slots; a slot's "full" mbarrier
+//                   completes when its bytes have landed (the paper's DMA1, inbound engine)
+//   add warps       wait "full", fold the slot into the running partial held in registers with fp32 RN
+//                   adds in rank order (the paper's per-hop reduce kernel), hand the slot back through its
+//                   "empty" mbarrier; after rank P-1 the finished tile goes to a slot of the store ring
+//   store warp      one thread waits "out full" and issues one TMA bulk store (shared -> global) per
+//                   destination rank (root only for reduce, all P for allreduce / SGD: the broadcast half
+//                   of PAPER.md:71), then returns the slot ("out empty") once the copies have read it
+//                   (the paper's DMA2, outbound engine)
+//
+// so loads of later tiles/ranks, adds and stores of earlier tiles overlap (reduction math overlaps
+// transfer), and the grid of 148 x k persistent CTAs walks the tile list round-robin (lp_schedule.h).
+// Broadcast has no math: its kernel is the producer and the store thread alone.
+#include "lp_common.cuh"
+
+namespace {
+
+__device__ __forceinline__ void wait_read_lag(int lag) {
+    switch (lag) {
+        case 0: lp_bulk_wait_read<0>(); break;
+        case 1: lp_bulk_wait_read<1>(); break;
+        case 2: lp_bulk_wait_read<2>(); break;
+        default: lp_bulk_wait_read<3>(); break;
+    }
+}
+
+struct Ring {
+    int slot;
+    uint32_t phase;
+    int depth;
+    __device__ __forceinline__ Ring(int d) : slot(0), phase(0), depth(d) {}
+    __device__ __forceinline__ void advance() {
+        if (++slot == depth) {
+            slot = 0;
+            phase ^= 1u;
+        }
+    }
+};
+
+// V float4 per add thread per tile, CW add warps: TILE = V * 4 * CW * 32 elements.
+template <int V, int CW>
+__global__ void __launch_bounds__((CW + 2) * 32) lp_pipeline_kernel(const __grid_constant__ LpArgs a, int stages,
+                                                                     int out_stages) {
+    constexpr int CT = CW * 32;
+    constexpr int TILE = V * 4 * CT;
+    extern __shared__ __align__(128) unsigned char lp_smem[];
+    float *in_ring = reinterpret_cast<float *>(lp_smem);
+    float *out_ring = in_ring + (size_t)stages * TILE;
+    uint64_t *full = reinterpret_cast<uint64_t *>(out_ring + (size_t)out_stages * TILE);
+    uint64_t *empty = full + stages;
+    uint64_t *ofull = empty + stages;
+    uint64_t *oempty = ofull + out_stages;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < stages; ++s) {
+            lp_mbar_init(&full[s], 1);    // the producer's arrive.expect_tx (+ the bytes)
+            lp_mbar_init(&empty[s], CW);  // lane 0 of every add warp
+        }
+        for (int s = 0; s < out_stages; ++s) {
+            lp_mbar_init(&ofull[s], CW);
+            lp_mbar_init(&oempty[s], 1);  // the store thread
+        }
+        lp_fence_mbar_init();
+    }
+    __syncthreads();
+
+    const int warp = threadIdx.x >> 5;
+    const int lane = threadIdx.x & 31;
+    const lp_partition &part = a.part;
+
+    if (warp == 0) {
+        // ---------------- producer: TMA bulk loads in chain order --------------------------------------
+        if (lane == 0) {
+            const uint64_t pol = lp_policy_evict_first();
+            const bool hint = a.l2_hint >= 1;
+            Ring ring(stages);
+            for (uint64_t t = blockIdx.x; t < part.n_tiles; t += gridDim.x) {
+                uint64_t off;
+                uint32_t len;
+                lp_tile_range(part, t, off, len);
+                const uint32_t bytes = (len & ~3u) * 4u;
+                for (int r = 0; r < a.n_in; ++r) {
+                    lp_mbar_wait(&empty[ring.slot], ring.phase ^ 1u);
+                    if (bytes) {
+                        lp_mbar_expect_tx(&full[ring.slot], bytes);
+                        float *dst = in_ring + (size_t)ring.slot * TILE;
+                        if (hint)
+                            lp_bulk_g2s_hint(dst, a.in[r] + off, bytes, &full[ring.slot], pol);
+                        else
+                            lp_bulk_g2s(dst, a.in[r] + off, bytes, &full[ring.slot]);
+                    } else {
+                        lp_mbar_arrive(&full[ring.slot]);
+                    }
+                    ring.advance();
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ---------------- store thread: TMA bulk stores to every destination rank -----------------------
+        if (lane == 0) {
+            const uint64_t pol = lp_policy_evict_first();
+            const bool hint = a.l2_hint >= 2;
+            const int lag = out_stages >= 3 ? 2 : (out_stages == 2 ? 1 : 0);
+            Ring ring(out_stages);
+            uint64_t issued = 0;
+            int free_slot = 0;  // oldest slot not yet handed back
+            for (uint64_t t = blockIdx.x; t < part.n_tiles; t += gridDim.x) {
+                uint64_t off;
+                uint32_t len;
+                lp_tile_range(part, t, off, len);
+                const uint32_t bytes = (len & ~3u) * 4u;
+                lp_mbar_wait(&ofull[ring.slot], ring.phase);
+                if (bytes) {
+                    const float *src = out_ring + (size_t)ring.slot * TILE;
+                    for (int q = 0; q < a.n_out; ++q) {
+                        if (hint)
+                            lp_bulk_s2g_hint(a.out[q] + off, src, bytes, pol);
+                        else
+                            lp_bulk_s2g(a.out[q] + off, src, bytes);
+                    }
+                }
+                lp_bulk_commit();
+                ++issued;
+                wait_read_lag(lag);  // all but the newest `lag` groups have finished reading shared memory
+                if (issued > (uint64_t)lag) {
+                    lp_mbar_arrive(&oempty[free_slot]);
+                    if (++free_slot == out_stages) free_slot = 0;
+                }
+                ring.advance();
+            }
+            lp_bulk_wait<0>();  // every store has completed before the CTA exits
+        }
+    } else {
+        // ---------------- add warps: chain fold in registers ----------------------------------------------
+        const int ctid = threadIdx.x - 64;
+        Ring ring(stages);
+        Ring oring(out_stages);
+        for (uint64_t t = blockIdx.x; t < part.n_tiles; t += gridDim.x) {
+            uint64_t off;
+            uint32_t len;
+            lp_tile_range(part, t, off, len);
+            float4 acc[V];
+            {  // rank 0: the partial starts as its block ("writing block a0 to a buffer on GPU1")
+                lp_mbar_wait(&full[ring.slot], ring.phase);
+                const float4 *s = reinterpret_cast<const float4 *>(in_ring + (size_t)ring.slot * TILE);
+#pragma unroll
+                for (int v = 0; v < V; ++v) acc[v] = s[ctid + v * CT];
+                __syncwarp();
+                if (lane == 0) lp_mbar_arrive(&empty[ring.slot]);
+                ring.advance();
+            }
+            for (int r = 1; r < a.n_sum; ++r) {  // rank r: partial <- partial + local block
+                lp_mbar_wait(&full[ring.slot], ring.phase);
+                const float4 *s = reinterpret_cast<const float4 *>(in_ring + (size_t)ring.slot * TILE);
+                float4 x[V];
+#pragma unroll
+                for (int v = 0; v < V; ++v) x[v] = s[ctid + v * CT];
+#pragma unroll
+                for (int v = 0; v < V; ++v) acc[v] = lp_add4(acc[v], x[v]);
+                __syncwarp();
+                if (lane == 0) lp_mbar_arrive(&empty[ring.slot]);
+                ring.advance();
+            }
+            if (a.epilogue == LP_EPI_SGD) {  // g = S/P, w' = w_root - lr g
+                lp_mbar_wait(&full[ring.slot], ring.phase);
+                const float4 *s = reinterpret_cast<const float4 *>(in_ring + (size_t)ring.slot * TILE);
+#pragma unroll
+                for (int v = 0; v < V; ++v) acc[v] = lp_sgd4(acc[v], s[ctid + v * CT], a.lr, a.invP);
+                __syncwarp();
+                if (lane == 0) lp_mbar_arrive(&empty[ring.slot]);
+                ring.advance();
+            }
+            // finished tile -> store ring
+            lp_mbar_wait(&oempty[oring.slot], oring.phase ^ 1u);
+            float4 *o = reinterpret_cast<float4 *>(out_ring + (size_t)oring.slot * TILE);
+#pragma unroll
+            for (int v = 0; v < V; ++v) o[ctid + v * CT] = acc[v];
+            lp_fence_proxy_async();
+            __syncwarp();
+            if (lane == 0) lp_mbar_arrive(&ofull[oring.slot]);
+            oring.advance();
+            // elements past the 16-byte body of the message's last tile
+            const uint32_t rem = len & 3u;
+            if ((uint32_t)ctid < rem) lp_scalar_element(a, off + (len & ~3u) + ctid);
+        }
+    }
+}
+
+// Broadcast: the root's tile is loaded once into the ring and stored to the P-1 other ranks
+// straight from the same slot.  Warp 0 lane 0 loads, warp 1 lane 0 stores, warp 2 copies the <= 3 tail elements.
+__global__ void __launch_bounds__(96) lp_bcast_kernel(const __grid_constant__ LpArgs a, int stages, int tile) {
+    extern __shared__ __align__(128) unsigned char lp_smem[];
+    float *ring_buf = reinterpret_cast<float *>(lp_smem);
+    uint64_t *full = reinterpret_cast<uint64_t *>(ring_buf + (size_t)stages * tile);
+    uint64_t *empty = full + stages;
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < stages; ++s) {
+            lp_mbar_init(&full[s], 1);
+            lp_mbar_init(&empty[s], 1);
+        }
+        lp_fence_mbar_init();
+    }
+    __syncthreads();
+    const int warp = threadIdx.x >> 5;
+    const int lane = threadIdx.x & 31;
+    const lp_partition &part = a.part;
+    if (warp == 0 && lane == 0) {
+        const uint64_t pol = lp_policy_evict_first();
+        const bool hint = a.l2_hint >= 1;
+        Ring ring(stages);
+        for (uint64_t t = blockIdx.x; t < part.n_tiles; t += gridDim.x) {
+            uint64_t off;
+            uint32_t len;
+            lp_tile_range(part, t, off, len);
+            const uint32_t bytes = (len & ~3u) * 4u;
+            lp_mbar_wait(&empty[ring.slot], ring.phase ^ 1u);
+            if (bytes) {
+                lp_mbar_expect_tx(&full[ring.slot], bytes);
+                float *dst = ring_buf + (size_t)ring.slot * tile;
+                if (hint)
+                    lp_bulk_g2s_hint(dst, a.in[0] + off, bytes, &full[ring.slot], pol);
+                else
+                    lp_bulk_g2s(dst, a.in[0] + off, bytes, &full[ring.slot]);
+            } else {
+                lp_mbar_arrive(&full[ring.slot]);
+            }
+            ring.advance();
+        }
+    } else if (warp == 1 && lane == 0) {
+        const uint64_t pol = lp_policy_evict_first();
+        const bool hint = a.l2_hint >= 2;
+        const int lag = stages >= 4 ? 2 : 1;
+        Ring ring(stages);
+        uint64_t issued = 0;
+        int free_slot = 0;
+        for (uint64_t t = blockIdx.x; t < part.n_tiles; t += gridDim.x) {
+            uint64_t off;
+            uint32_t len;
+            lp_tile_range(part, t, off, len);
+            const uint32_t bytes = (len & ~3u) * 4u;
+            lp_mbar_wait(&full[ring.slot], ring.phase);
+            if (bytes) {
+                const float *src = ring_buf + (size_t)ring.slot * tile;
+                for (int q = 0; q < a.n_out; ++q) {
+                    if (hint)
+                        lp_bulk_s2g_hint(a.out[q] + off, src, bytes, pol);
+                    else
+                        lp_bulk_s2g(a.out[q] + off, src, bytes);
+                }
+            }
+            lp_bulk_commit();
+            ++issued;
+            wait_read_lag(lag);
+            if (issued > (uint64_t)lag) {
+                lp_mbar_arrive(&empty[free_slot]);
+                if (++free_slot == stages) free_slot = 0;
+            }
+            ring.advance();
+        }
+        lp_bulk_wait<0>();
+    } else if (warp == 2) {
+        for (uint64_t t = blockIdx.x; t < part.n_tiles; t += gridDim.x) {
+            uint64_t off;
+            uint32_t len;
+            lp_tile_range(part, t, off, len);
+            const uint32_t rem = len & 3u;
+            if ((uint32_t)lane < rem) lp_scalar_element(a, off + (len & ~3u) + lane);
+        }
+    }
+}
+
+template <int V, int CW>
+cudaError_t launch_fold(const LpArgs &a, const LpLaunch &cfg, cudaStream_t stream) {
+    static bool attr_set = false;  // per instantiation
+    static int attr_bytes = 0;
+    if (!attr_set || (int)cfg.smem_bytes > attr_bytes) {
+        cudaError_t e = cudaFuncSetAttribute(lp_pipeline_kernel<V, CW>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             (int)cfg.smem_bytes);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+        attr_bytes = (int)cfg.smem_bytes;
+    }
+    lp_pipeline_kernel<V, CW><<<cfg.grid, cfg.threads, cfg.smem_bytes, stream>>>(a, (int)cfg.stages,
+                                                                                  (int)cfg.out_stages);
+    return cudaGetLastError();
+}
+
+constexpr uint32_t kSmemPerSm = 228u * 1024u;   // sm_100: 228 KB per SM, 227 KB max per CTA, 1 KB reserved per CTA
+constexpr uint32_t kSmemPerCtaMax = 227u * 1024u;
+
+}  // namespace
+
+// Tile size: the tuned or default 4096 elements (16 KB), halved while a whole block still fits in the
+// half (a block is never split finer than it has to be), floor 1024.
+uint32_t lp_pipeline_tile(const LpTuning &t, uint64_t n, uint64_t block) {
+    uint32_t tile = t.v[LP_TUNE_TILE_ELEMS] ? (uint32_t)t.v[LP_TUNE_TILE_ELEMS] : 4096u;
+    uint64_t blk = block < n ? block : n;
+    while (tile > 1024u && (uint64_t)(tile / 2) >= blk) tile /= 2;
+    return tile;
+}
+
+cudaError_t lp_pipeline_launch(const LpArgs &a, const LpTuning &t, int sm_count, LpLaunch *cfg, bool dry_run,
+                               cudaStream_t stream) {
+    const uint32_t tile = a.part.tile;
+    const bool bcast = a.epilogue == LP_EPI_COPY;
+    uint32_t ctas = t.v[LP_TUNE_CTAS_PER_SM] ? (uint32_t)t.v[LP_TUNE_CTAS_PER_SM] : 2u;
+    uint32_t stages = t.v[LP_TUNE_STAGES] ? (uint32_t)t.v[LP_TUNE_STAGES] : (bcast ? 6u : 4u);
+    uint32_t out_stages = bcast ? 0u : (t.v[LP_TUNE_OUT_STAGES] ? (uint32_t)t.v[LP_TUNE_OUT_STAGES] : 2u);
+    if (bcast && stages < 3) stages = 3;
+    auto smem_of = [&](uint32_t st, uint32_t ost) {
+        return (st + ost) * tile * 4u + (2u * st + 2u * ost) * 8u;
+    };
+    // shrink the rings until `ctas` CTAs fit one SM; if even the shallowest rings do not, take fewer CTAs
+    const uint32_t want_stages = stages, want_out = out_stages;
+    for (;;) {
+        const uint32_t share = kSmemPerSm / ctas - 1024u;
+        const uint32_t budget = share < kSmemPerCtaMax ? share : kSmemPerCtaMax;
+        stages = want_stages;
+        out_stages = want_out;
+        while (smem_of(stages, out_stages) > budget && stages > (bcast ? 3u : 2u)) --stages;
+        while (smem_of(stages, out_stages) > budget && out_stages > 1u) --out_stages;
+        if (smem_of(stages, out_stages) <= budget) break;
+        if (ctas == 1) return cudaErrorInvalidConfiguration;
+        --ctas;
+    }
+
+    uint32_t threads;
+    int V = 0, CW = 0;
+    if (bcast) {
+        threads = 96;
+    } else {
+        switch (tile) {
+            case 1024: V = 2, CW = 4; break;
+            case 2048: V = 4, CW = 4; break;
+            case 4096: V = 4, CW = 8; break;
+            case 8192: V = 8, CW = 8; break;
+            default: return cudaErrorInvalidValue;
+        }
+        threads = (uint32_t)(CW + 2) * 32u;
+    }
+    uint64_t grid = (uint64_t)sm_count * ctas;
+    if (grid > a.part.n_tiles) grid = a.part.n_tiles;
+    cfg->grid = (uint32_t)grid;
+    cfg->threads = threads;
+    cfg->smem_bytes = smem_of(stages, out_stages);
+    cfg->stages = stages;
+    cfg->out_stages = out_stages;
+    if (dry_run || grid == 0) return cudaSuccess;
+
+    lp_count_launch(1);
+    if (bcast) {
+        static int attr_bytes = 0;
+        if ((int)cfg->smem_bytes > attr_bytes) {
+            cudaError_t e = cudaFuncSetAttribute(lp_bcast_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                 (int)cfg->smem_bytes);
+            if (e != cudaSuccess) return e;
+            attr_bytes = (int)cfg->smem_bytes;
+        }
+        lp_bcast_kernel<<<cfg->grid, cfg->threads, cfg->smem_bytes, stream>>>(a, (int)stages, (int)tile);
+        return cudaGetLastError();
+    }
+    switch (tile) {
+        case 1024: return launch_fold<2, 4>(a, *cfg, stream);
+        case 2048: return launch_fold<4, 4>(a, *cfg, stream);
+        case 4096: return launch_fold<4, 8>(a, *cfg, stream);
+        default: return launch_fold<8, 8>(a, *cfg, stream);
+    }
+}

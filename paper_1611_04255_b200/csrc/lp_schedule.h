@@ -1,0 +1,58 @@
+// lp_schedule.h -- the LP schedule engine's index math, shared by the host planner and the kernels.
+//
+// a1: the message [0, n) is cut into nb = ceil(n / block) blocks of `block` elements,
+// the last one short (U6).  On one GPU a block is further cut into TILES of `tile` elements (the unit
+// one CTA keeps on chip while it walks the chain rank 0 -> P-1); a tile never straddles a block
+// boundary, so `block` stays the unit the pipeline is built from and small blocks really cost more
+// (the alpha term of PAPER.md:89).  Tiles are numbered block by block, and tile idx is handled by
+// persistent CTA (idx mod grid): at any moment the whole grid works on neighbouring tiles of the same
+// few blocks, the analogue of "the entire network is fully utilized once the pipeline is filled".
+#pragma once
+#include <stdint.h>
+
+#if defined(__CUDACC__)
+#define LP_HD __host__ __device__ __forceinline__
+#else
+#define LP_HD inline
+#endif
+
+struct lp_partition {
+    uint64_t n;                // elements per rank
+    uint64_t block;            // LP block b in elements (clamped to n, >= 1)
+    uint64_t nb;               // number of blocks
+    uint64_t tiles_per_block;  // ceil(block / tile)
+    uint64_t n_tiles;          // total tiles
+    uint32_t tile;             // elements per full tile
+};
+
+LP_HD lp_partition lp_make_partition(uint64_t n, uint64_t block, uint32_t tile) {
+    lp_partition p;
+    p.n = n;
+    p.tile = tile;
+    if (n == 0) {
+        p.block = block ? block : 1;
+        p.nb = 0;
+        p.tiles_per_block = 0;
+        p.n_tiles = 0;
+        return p;
+    }
+    if (block > n) block = n;  // "block > n => one block" (U6)
+    p.block = block;
+    p.nb = (n + block - 1) / block;
+    p.tiles_per_block = (block + tile - 1) / tile;
+    uint64_t last = n - (p.nb - 1) * block;  // length of the last block, 1..block
+    p.n_tiles = (p.nb - 1) * p.tiles_per_block + (last + tile - 1) / tile;
+    return p;
+}
+
+// Tile idx -> element range [off, off + len).
+LP_HD void lp_tile_range(const lp_partition &p, uint64_t idx, uint64_t &off, uint32_t &len) {
+    uint64_t k = idx / p.tiles_per_block;       // block index
+    uint64_t j = idx - k * p.tiles_per_block;   // tile within the block
+    uint64_t bstart = k * p.block;
+    uint64_t bend = bstart + p.block;
+    if (bend > p.n) bend = p.n;
+    off = bstart + j * (uint64_t)p.tile;
+    uint64_t rem = bend - off;
+    len = rem < p.tile ? (uint32_t)rem : p.tile;
+}

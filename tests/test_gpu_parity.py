@@ -1,0 +1,284 @@
+"""GPU parity: the CUDA library (through its C ABI / thin binding) against the CPU oracle, element by element on
+the same seeded inputs.  Bit-exact in chain order (north_star); MST / BE bit-exact against the same-tree oracle
+and within 1e-6 * sum|x| of the chain order (U15).  Needs a B200: every test is marked gpu.
+"""
+import numpy as np
+import pytest
+
+from paper_1611_04255_b200 import inputs
+from paper_1611_04255_b200 import binding as lp
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+LP, MST, BE = 0, 1, 2
+VARIANTS = [lp.VARIANT_PIPELINE, lp.VARIANT_DIRECT, lp.VARIANT_COPY_ENGINE]
+
+
+@pytest.fixture(autouse=True)
+def _device_and_defaults():
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    lp.lib()
+    lp.lp_set_variant(lp.VARIANT_PIPELINE)
+    for k in range(6):
+        lp.lp_set_tuning(k, 0)
+    yield
+    torch.cuda.synchronize()
+    lp.lp_set_variant(lp.VARIANT_PIPELINE)
+
+
+def up(arrs):
+    return [torch.from_numpy(a).cuda() for a in arrs]
+
+
+def down(tensors):
+    torch.cuda.synchronize()
+    return [t.cpu().numpy() for t in tensors]
+
+
+def same(a, b):
+    return a.shape == b.shape and a.tobytes() == b.tobytes()
+
+
+def copies(arrs):
+    return [a.copy() for a in arrs]
+
+
+def run_lp(op, dev, block, root=0, stream=None):
+    if op == "allreduce":
+        lp.lp_allreduce(dev, block, stream=stream)
+    elif op == "reduce":
+        lp.lp_reduce(dev, block, root=root, stream=stream)
+    else:
+        lp.lp_broadcast(dev, block, root=root, stream=stream)
+
+
+def run_oracle(oracle, op, host, root=0, algo=LP):
+    if op == "allreduce":
+        oracle.allreduce(host, algo=algo)
+    elif op == "reduce":
+        oracle.reduce(host, root=root, algo=algo)
+    else:
+        oracle.broadcast(host, root=root, algo=algo)
+
+
+# ---------------------------------------------------------------------------------------------------
+# BASELINE.json configs[0]: P=4, n=1Mi, b=65536, U[-1,1] seed 0; allreduce, reduce(0), broadcast(0)
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("op", ["allreduce", "reduce", "broadcast"])
+def test_config0_bit_exact(oracle, variant, op):
+    c = inputs.CONFIGS[0]
+    src = inputs.rank_vectors(0, c["P"], c["n"], "uniform")
+    want = copies(src)
+    run_oracle(oracle, op, want, root=0)
+    lp.lp_set_variant(variant)
+    dev = up(src)
+    run_lp(op, dev, c["block"], root=0)
+    got = down(dev)
+    for r in range(c["P"]):
+        assert same(got[r], want[r]), (op, variant, r)
+    # the stage-model tick count of this shape: P + nb - 1 = 19
+    assert lp.lp_schedule_steps(c["P"], c["n"], c["block"], 2) == 19
+
+
+# ---------------------------------------------------------------------------------------------------
+# ragged shapes: several tiles + tails, unaligned blocks, every root, all variants
+# ---------------------------------------------------------------------------------------------------
+SHAPES = [
+    # P, n, block
+    (1, 1000, 64), (2, 1, 1), (2, 3, 64), (2, 5, 4), (3, 1001, 100), (3, 4097, 1000), (4, 70_001, 4096),
+    (5, 300_003, 65_536), (6, 70_001, 1001), (7, 12_345, 333), (8, 262_147, 16_384), (16, 100_003, 8192),
+    (32, 20_001, 5000), (4, 8192 * 3 + 5, 8192), (6, 1 << 20, 1 << 22),
+]
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("P,n,block", SHAPES)
+def test_ragged_shapes_bit_exact(oracle, variant, P, n, block):
+    if variant == lp.VARIANT_COPY_ENGINE and n // block > 400:
+        pytest.skip("copy-engine variant: thousands of tiny copies, covered by smaller shapes")
+    lp.lp_set_variant(variant)
+    src = inputs.rank_vectors([7, n], P, n, "uniform")
+    for op in ("allreduce", "reduce", "broadcast"):
+        for root in sorted({0, P - 1, P // 2}):
+            if op == "allreduce" and root != 0:
+                continue
+            want = copies(src)
+            run_oracle(oracle, op, want, root=root)
+            dev = up(src)
+            run_lp(op, dev, block, root=root)
+            got = down(dev)
+            for r in range(P):
+                assert same(got[r], want[r]), (op, root, r)
+
+
+def test_tuning_space_bit_exact(oracle):
+    # every tile size / ring depth / CTA count / cache hint gives the same bits
+    P, n, block = 5, 400_003, 32_768
+    src = inputs.rank_vectors(8, P, n, "normal", 1e-3)
+    want = copies(src)
+    oracle.allreduce(want)
+    for tile in (1024, 2048, 4096, 8192):
+        for stages, out_stages, ctas, hint in ((2, 1, 1, 0), (3, 2, 2, 1), (8, 3, 1, 2), (4, 4, 3, 0)):
+            lp.lp_set_tuning(lp.TUNE_TILE_ELEMS, tile)
+            lp.lp_set_tuning(lp.TUNE_STAGES, stages)
+            lp.lp_set_tuning(lp.TUNE_OUT_STAGES, out_stages)
+            lp.lp_set_tuning(lp.TUNE_CTAS_PER_SM, ctas)
+            lp.lp_set_tuning(lp.TUNE_L2_HINT, hint)
+            dev = up(src)
+            lp.lp_allreduce(dev, block)
+            got = down(dev)
+            assert all(same(g, w) for g, w in zip(got, want)), (tile, stages, out_stages, ctas, hint)
+            dev = up(src)
+            lp.lp_broadcast(dev, block, root=3)
+            got = down(dev)
+            assert all(same(g, src[3]) for g in got), ("bcast", tile, stages)
+    for tile in (1024, 2048, 4096):
+        lp.lp_set_variant(lp.VARIANT_DIRECT)
+        lp.lp_set_tuning(lp.TUNE_TILE_ELEMS, tile)
+        dev = up(src)
+        lp.lp_allreduce(dev, block)
+        assert all(same(g, w) for g, w in zip(down(dev), want)), ("direct", tile)
+
+
+def test_chain_order_and_invariances(oracle):
+    # the non-associative triple of the oracle pin: a wrong fold order shows up in one element
+    vals = [1e8, -1e8, 1.0]
+    for variant in VARIANTS:
+        lp.lp_set_variant(variant)
+        for perm, want in (((0, 1, 2), 1.0), ((2, 0, 1), 0.0), ((1, 2, 0), 0.0), ((1, 0, 2), 1.0)):
+            dev = up([np.full(4100, vals[p], np.float32) for p in perm])
+            lp.lp_allreduce(dev, 1024)
+            got = down(dev)
+            assert all((g == np.float32(want)).all() for g in got), (variant, perm)
+    # result independent of block, root, stream; allreduce == broadcast(reduce)
+    lp.lp_set_variant(lp.VARIANT_PIPELINE)
+    P, n = 6, 123_457
+    src = inputs.rank_vectors(9, P, n, "uniform")
+    want = oracle.chain_sum(src)
+    side = torch.cuda.Stream()
+    for block in (4, 256, 4096, 40_000, n, 10 * n):
+        dev = up(src)
+        torch.cuda.synchronize()
+        lp.lp_allreduce(dev, block, stream=side)
+        side.synchronize()
+        assert all(same(g, want) for g in down(dev)), block
+    for root in range(P):
+        dev = up(src)
+        lp.lp_reduce(dev, 4096, root=root)
+        got = down(dev)
+        assert same(got[root], want)
+        assert all(same(got[r], src[r]) for r in range(P) if r != root)  # U5
+        lp.lp_broadcast(dev, 4096, root=root)
+        assert all(same(g, want) for g in down(dev))
+
+
+def test_noops_and_device_side_validation():
+    dev = up([np.arange(10, dtype=np.float32)])
+    lp.lp_allreduce(dev, 4)          # P == 1: identity
+    lp.lp_reduce(dev, 4, root=0)
+    lp.lp_broadcast(dev, 4, root=0)
+    assert same(down(dev)[0], np.arange(10, dtype=np.float32))
+    empty = [torch.empty(0, dtype=torch.float32, device="cuda") for _ in range(3)]
+    big = torch.zeros(64, dtype=torch.float32, device="cuda")
+    with pytest.raises(lp.LpError) as e:   # overlapping device buffers
+        lp.lp_allreduce([big[:32], big[16:48]], 8)
+    assert e.value.status == lp.LP_ERR_INVALID_ARG
+    with pytest.raises(lp.LpError) as e:   # misaligned device buffer
+        lp.lp_allreduce([big[1:17], big[32:48]], 8)
+    assert e.value.status == lp.LP_ERR_INVALID_ARG
+    with pytest.raises(lp.LpError) as e:
+        lp.lp_be_allreduce([big[0:16], big[16:32], big[32:48]])
+    assert e.value.status == lp.LP_ERR_UNSUPPORTED
+    assert not big.any().item()
+    before = lp.lp_launch_count()
+    dev = up([np.ones(5000, np.float32) for _ in range(3)])
+    lp.lp_allreduce(dev, 1024)
+    assert lp.lp_launch_count() == before + 1   # the whole pipeline is ONE launch
+    assert (down(dev)[2] == 3).all()
+    del empty
+
+
+# ---------------------------------------------------------------------------------------------------
+# fused BSP-SGD step (a6)
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("P,n,block,root", [(1, 1000, 256, 0), (2, 4099, 1024, 1), (6, 70_001, 1001, 2),
+                                            (8, 150_003, 16_384, 0), (16, 33_333, 4096, 15)])
+def test_sgd_step_bit_exact(oracle, variant, P, n, block, root):
+    lp.lp_set_variant(variant)
+    grads, weights = inputs.sgd_inputs([5, n], P, n)
+    weights[root] += np.float32(0.125)  # replicas differ: only weights[root] may be read (U8)
+    hg, hw = copies(grads), copies(weights)
+    dg, dw = up(grads), up(weights)
+    for it in range(3):
+        oracle.bsp_sgd_step(hg, hw, root=root, lr=0.01)
+        lp.lp_bsp_sgd_step(dg, dw, block, root=root, lr=0.01)
+        gw = down(dw)
+        for r in range(P):
+            assert same(gw[r], hw[r]), (it, r)
+    assert all(same(g, s) for g, s in zip(down(dg), grads))  # grads only read
+
+
+def test_config2_sgd_100_iterations(oracle):
+    # BASELINE.json configs[2]: P=8, n=7,000,000, grads N(0,1e-2), w N(0,0.05), lr=0.01, 100 iterations
+    c = inputs.CONFIGS[2]
+    P, n = c["P"], c["n"]
+    grads, weights = inputs.sgd_inputs(2, P, n, c["sigma"], c["w_sigma"])
+    hw = copies(weights)
+    dg, dw = up(grads), up(weights)
+    for it in range(1, c["iters"] + 1):
+        oracle.bsp_sgd_step(grads, hw, root=0, lr=c["lr"], omp=True)
+        lp.lp_bsp_sgd_step(dg, dw, c["block"], root=0, lr=c["lr"])
+        if it in (1, 5, 100):
+            gw = down(dw)
+            assert all(same(gw[r], hw[r]) for r in range(P)), it
+
+
+# ---------------------------------------------------------------------------------------------------
+# MST / BE baselines (a7, a8)
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("P,n", [(2, 1001), (3, 70_001), (4, 65_536), (5, 4099), (6, 300_003), (8, 100_001),
+                                 (16, 50_005), (7, 3)])
+def test_mst_be_against_same_tree_oracle(oracle, P, n):
+    src = inputs.rank_vectors([3, n], P, n, "uniform")
+    chain = oracle.chain_sum(src).astype(np.float64)
+    sabs = np.abs(np.stack(src).astype(np.float64)).sum(axis=0)
+    algos = [(MST, "mst")] + ([(BE, "be")] if P & (P - 1) == 0 else [])
+    for algo, name in algos:
+        for op in ("allreduce", "reduce", "broadcast"):
+            for root in sorted({0, P - 1}):
+                if op == "allreduce" and root != 0:
+                    continue
+                want = copies(src)
+                run_oracle(oracle, op, want, root=root, algo=algo)
+                dev = up(src)
+                f = getattr(lp, f"lp_{name}_{op}")
+                f(dev) if op == "allreduce" else f(dev, root=root)
+                got = down(dev)
+                for r in range(P):
+                    assert same(got[r], want[r]), (name, op, root, r)
+                if op != "broadcast":   # reordered sum vs chain order: north_star 1e-6, relative to sum|x| (U15)
+                    assert np.all(np.abs(got[root].astype(np.float64) - chain) <= 1e-6 * sabs)
+
+
+# ---------------------------------------------------------------------------------------------------
+# host-buffer entry points (the e2e path bench.py times)
+# ---------------------------------------------------------------------------------------------------
+def test_host_entry_points(oracle):
+    P, n, block = 3, 9_000_001, 65_536   # three 16 MB chunks per rank
+    src = inputs.rank_vectors(10, P, n, "normal", 1e-3)
+    want = copies(src)
+    oracle.allreduce(want, omp=True)
+    pinned = [torch.from_numpy(s.copy()).pin_memory() for s in src]
+    lp.lp_allreduce_host(pinned, block)
+    assert all(same(p.numpy(), w) for p, w in zip(pinned, want))
+    pageable = copies(src)
+    lp.lp_allreduce_host(pageable, block)
+    assert all(same(p, w) for p, w in zip(pageable, want))
+    grads, weights = inputs.sgd_inputs(11, 4, 5_000_003)
+    hw = copies(weights)
+    oracle.bsp_sgd_step(grads, hw, root=1, lr=0.05, omp=True)
+    lp.lp_bsp_sgd_step_host(grads, weights, 65_536, root=1, lr=0.05)
+    assert all(same(a, b) for a, b in zip(weights, hw))

@@ -1,0 +1,166 @@
+"""CPU-side checks of the CUDA library: it loads, exports every symbol include/lp_collectives.h declares, and
+its host-only schedule engine / planner / argument validation behave (no compute call needs a GPU here).
+
+The product's schedule engine (csrc/lp_host_schedule.cpp, csrc/lp_schedule.h) and the oracle's
+(oracle/lpo_oracle.c) are separate implementations; here they are compared with each other AND with the
+paper's printed values / closed forms.
+"""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_1611_04255_b200 import binding as lp
+from tests.conftest import ROOT, read_golden
+
+BCAST, REDUCE, ALLREDUCE, SGD = 0, 1, 2, 3
+
+
+def test_library_exports_every_declared_symbol():
+    header = open(os.path.join(ROOT, "include", "lp_collectives.h")).read()
+    names = re.findall(r"^LP_API [^;(]*?\b(lp_[a-z_0-9]+)\(", header, flags=re.M)
+    assert len(names) >= 25 and len(set(names)) == len(names)
+    L = lp.lib()
+    for name in names:
+        assert hasattr(L, name), name
+    assert lp.lp_version() >= 100
+    assert "LP_OK" in lp.status_string(0)
+
+
+def test_num_blocks_and_stage_block_closed_forms():
+    # a1 (U6) and a2
+    assert lp.lp_num_blocks(61_000_000, 65_536) == 931
+    assert lp.lp_num_blocks(138_000_000, 262_144) == 527
+    assert lp.lp_num_blocks(10, 0) == 0 and lp.lp_num_blocks(0, 7) == 0 and lp.lp_num_blocks(7, 100) == 1
+    P, nb = 5, 7
+    seen = set()
+    for t in range(P + nb - 1):
+        busy = 0
+        for r in range(P):
+            k = lp.lp_stage_block(P, nb, t, r)
+            if k >= 0:
+                assert k == t - r and (r, k) not in seen
+                seen.add((r, k))
+                busy += 1
+        if P - 1 <= t < nb:
+            assert busy == P  # "the entire network is fully utilized once the pipeline is filled"
+    assert len(seen) == P * nb
+    assert lp.lp_stage_block(P, nb, P + nb - 1, 0) == -1
+
+
+def test_stage_model_steps_closed_form():
+    # pipeline length p - 1 + n/b
+    for P in (1, 2, 3, 6, 16):
+        for n, b in ((1 << 20, 65_536), (61_000_000, 65_536), (5, 2), (0, 3)):
+            nb = -(-n // b)
+            for op in (BCAST, REDUCE, ALLREDUCE):
+                want = 0 if nb == 0 else P - 1 + nb
+                assert lp.lp_schedule_steps(P, n, b, op, lp.MODEL_STAGE) == want
+
+
+def test_link_model_matches_paper_worked_example():
+    # tests/golden/paper_fig2_link_steps.txt: PAPER.md:59,71 (3 GPUs, 4 blocks)
+    rows = {(int(P), int(nb), q): int(v) for P, nb, q, v in read_golden("paper_fig2_link_steps.txt")}
+    for model in (lp.MODEL_LINK, lp.MODEL_LINK_RING):
+        assert lp.lp_schedule_steps(3, 4, 1, REDUCE, model) == rows[(3, 4, "reduce_steps")]
+        assert lp.lp_schedule_steps(3, 4, 1, BCAST, model) == rows[(3, 4, "broadcast_steps")]
+        assert lp.lp_schedule_steps(3, 4, 1, ALLREDUCE, model) == rows[(3, 4, "allreduce_steps")]
+
+
+def test_link_model_matches_oracle_simulation(oracle):
+    # two independent implementations of the same greedy Fig. 2 schedule
+    for P in (2, 3, 4, 6, 8):
+        for nb in (1, 2, 4, 8, 16, 33):
+            for op in (BCAST, REDUCE, ALLREDUCE):
+                assert lp.lp_schedule_steps(P, nb, 1, op, lp.MODEL_LINK) == oracle.link_sim(P, nb, op, 0), (P, nb, op)
+                assert lp.lp_schedule_steps(P, nb, 1, op, lp.MODEL_LINK_RING) == oracle.link_sim(P, nb, op, 1), (P, nb, op)
+            assert lp.lp_schedule_steps(P, nb, 1, REDUCE, lp.MODEL_LINK) == P + nb - 2  # U2
+    assert lp.lp_schedule_steps(1, 100, 1, REDUCE, lp.MODEL_LINK) == 0
+
+
+def test_mst_levels_match_paper():
+    for P, steps in read_golden("paper_mst_steps.txt"):
+        assert lp.lp_mst_levels(int(P)) == int(steps)
+
+
+def test_min_bytes():
+    n = 1000
+    assert lp.lp_min_bytes(BCAST, 4, n) == 4 * n * 4
+    assert lp.lp_min_bytes(REDUCE, 4, n) == 5 * n * 4
+    assert lp.lp_min_bytes(ALLREDUCE, 6, n) == 2 * 6 * n * 4
+    assert lp.lp_min_bytes(SGD, 8, n) == 17 * n * 4
+
+
+@pytest.mark.parametrize("variant", [lp.VARIANT_PIPELINE, lp.VARIANT_DIRECT])
+@pytest.mark.parametrize("P,n,block", [(4, 1 << 20, 65_536), (6, 61_000_000, 65_536), (6, 61_000_000, 1 << 20),
+                                        (16, 138_000_000, 262_144), (3, 1001, 100), (2, 5, 64), (8, 7_000_000, 3000)])
+def test_plan_partition_covers_message_exactly(variant, P, n, block):
+    # the tile list of the persistent kernel: tiles never straddle a block, cover [0, n) once
+    lp.lp_set_variant(variant)
+    try:
+        info = lp.lp_plan_query(ALLREDUCE, P, n, block)
+    finally:
+        lp.lp_set_variant(lp.VARIANT_PIPELINE)
+    nb = -(-n // block)
+    assert info["nb"] == nb
+    tile = info["tile_elems"]
+    blk = min(block, n)
+    tpb = -(-blk // tile)
+    last = n - (nb - 1) * blk
+    assert info["n_tiles"] == (nb - 1) * tpb + -(-last // tile)
+    assert 1 <= info["grid"] <= info["n_tiles"]
+    assert info["grid"] <= info["sm_count"] * 8
+    if variant == lp.VARIANT_PIPELINE:
+        if block % 4 == 0 or nb == 1:
+            assert info["variant"] == lp.VARIANT_PIPELINE
+            assert info["smem_bytes"] <= 227 * 1024 and info["stages"] >= 2 and info["out_stages"] >= 1
+        else:
+            assert info["variant"] == lp.VARIANT_DIRECT  # unaligned tiles -> register path
+
+
+def test_argument_validation_needs_no_device():
+    L = lp.lib()
+    n = 64
+    raw = [np.zeros(n + 8, np.float32) for _ in range(4)]
+
+    def aligned(a, phase=0):
+        off = ((-a.ctypes.data) % 16) // 4
+        return a.ctypes.data + 4 * off + phase
+
+    ptrs = (ctypes.c_void_p * 4)(*[aligned(a) for a in raw])
+    null_stream = ctypes.c_void_p(0)
+    assert L.lp_allreduce(ptrs, 0, n, 16, null_stream) == lp.LP_ERR_INVALID_ARG          # P < 1
+    assert L.lp_allreduce(ptrs, 33, n, 16, null_stream) == lp.LP_ERR_INVALID_ARG         # P > LP_MAX_P
+    assert L.lp_allreduce(ptrs, 4, n, 0, null_stream) == lp.LP_ERR_INVALID_ARG           # block == 0
+    assert L.lp_reduce(ptrs, 4, n, 16, 4, null_stream) == lp.LP_ERR_INVALID_ARG          # root out of range
+    assert L.lp_broadcast(ptrs, 4, n, 16, -1, null_stream) == lp.LP_ERR_INVALID_ARG
+    assert L.lp_allreduce(None, 4, n, 16, null_stream) == lp.LP_ERR_INVALID_ARG          # NULL array
+    bad = (ctypes.c_void_p * 4)(ptrs[0], None, ptrs[2], ptrs[3])
+    assert L.lp_allreduce(bad, 4, n, 16, null_stream) == lp.LP_ERR_INVALID_ARG           # NULL buffer
+    mis = (ctypes.c_void_p * 4)(ptrs[0], aligned(raw[1], 4), ptrs[2], ptrs[3])
+    assert L.lp_allreduce(mis, 4, n, 16, null_stream) == lp.LP_ERR_INVALID_ARG           # not 16-byte aligned
+    ovl = (ctypes.c_void_p * 4)(ptrs[0], ptrs[0] + 16, ptrs[2], ptrs[3])
+    assert L.lp_allreduce(ovl, 4, n, 16, null_stream) == lp.LP_ERR_INVALID_ARG           # overlapping
+    assert L.lp_be_allreduce(ptrs, 3, n, null_stream) == lp.LP_ERR_UNSUPPORTED           # U14
+    assert L.lp_bsp_sgd_step(ptrs, None, 4, n, 16, 0, ctypes.c_float(0.1), null_stream) == lp.LP_ERR_INVALID_ARG
+    assert L.lp_set_variant(9) == lp.LP_ERR_INVALID_ARG
+    assert L.lp_set_tuning(lp.TUNE_TILE_ELEMS, 1000) == lp.LP_ERR_INVALID_ARG
+    out = ctypes.c_uint64(0)
+    assert L.lp_schedule_steps(4, n, 0, 0, 0, ctypes.byref(out)) == lp.LP_ERR_INVALID_ARG
+    assert L.lp_schedule_steps(4, n, 16, 7, 0, ctypes.byref(out)) == lp.LP_ERR_INVALID_ARG
+    for code in (0, 1, 2, 3):
+        assert lp.status_string(code)
+
+
+def test_compute_entry_fails_loudly_without_device():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a device is present")
+    L = lp.lib()
+    raw = [np.zeros(80, np.float32) for _ in range(2)]
+    ptrs = (ctypes.c_void_p * 2)(*[a.ctypes.data + ((-a.ctypes.data) % 16) for a in raw])
+    # valid arguments, no GPU: the library must refuse (LP_ERR_CUDA), never compute on the CPU
+    assert L.lp_allreduce(ptrs, 2, 64, 16, ctypes.c_void_p(0)) == lp.LP_ERR_CUDA
+    assert not raw[0].any() and not raw[1].any()
