@@ -143,7 +143,7 @@ int plan_and_run(int op, float *const *bufs, float *const *weights, int P, size_
     switch (variant) {
         case LP_VARIANT_DIRECT: tile = lp_direct_tile(g_tuning, a.n_in); break;
         case LP_VARIANT_CLUSTER: tile = lp_cluster_tile(g_tuning); break;
-        default: tile = lp_pipeline_tile(g_tuning, n, block); break;
+        default: tile = lp_pipeline_tile(g_tuning, a, n, block); break;
     }
     a.part = lp_make_partition(n, block, tile);
     // identity collectives: nothing to move (P == 1 broadcast/reduce/allreduce; n == 0)

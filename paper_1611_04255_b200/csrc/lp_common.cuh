@@ -45,7 +45,7 @@ cudaError_t lp_direct_launch(const LpArgs &a, const LpTuning &t, int sm_count, L
                              cudaStream_t stream);
 cudaError_t lp_cluster_launch(const LpArgs &a, const LpTuning &t, int sm_count, LpLaunch *cfg, bool dry_run,
                               cudaStream_t stream);
-uint32_t lp_pipeline_tile(const LpTuning &t, uint64_t n, uint64_t block);
+uint32_t lp_pipeline_tile(const LpTuning &t, const LpArgs &a, uint64_t n, uint64_t block);
 uint32_t lp_direct_tile(const LpTuning &t, int n_in);
 uint32_t lp_cluster_tile(const LpTuning &t);
 

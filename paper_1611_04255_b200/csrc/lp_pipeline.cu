@@ -298,10 +298,17 @@ constexpr uint32_t kSmemPerCtaMax = 227u * 1024u;
 
 }  // namespace
 
-// Tile size: the tuned or default 4096 elements (16 KB), halved while a whole block still fits in the
-// half (a block is never split finer than it has to be), floor 1024.
-uint32_t lp_pipeline_tile(const LpTuning &t, uint64_t n, uint64_t block) {
-    uint32_t tile = t.v[LP_TUNE_TILE_ELEMS] ? (uint32_t)t.v[LP_TUNE_TILE_ELEMS] : 4096u;
+// Defaults measured on B200 (profiles/r1_tuning.md): what matters is the number of load bytes in flight per SM.
+// A read-dominated fold (reduce: P reads, 1 write) wants ~96 KB (16 KB tiles, 3 slots, 2 CTAs/SM); once every
+// rank is written back too (allreduce, SGD) ~48 KB is best (8 KB tiles) -- deeper rings only lengthen the DRAM
+// queues the stores have to wait in.
+static bool read_dominated(const LpArgs &a) { return a.epilogue != LP_EPI_COPY && a.n_out == 1 && a.n_sum > 1; }
+
+// Tile size: the tuned or default size, halved while a whole block still fits in the half (a block is never
+// split finer than it has to be), floor 1024.
+uint32_t lp_pipeline_tile(const LpTuning &t, const LpArgs &a, uint64_t n, uint64_t block) {
+    uint32_t tile = t.v[LP_TUNE_TILE_ELEMS] ? (uint32_t)t.v[LP_TUNE_TILE_ELEMS]
+                    : (a.epilogue == LP_EPI_COPY ? 1024u : (read_dominated(a) ? 4096u : 2048u));
     uint64_t blk = block < n ? block : n;
     while (tile > 1024u && (uint64_t)(tile / 2) >= blk) tile /= 2;
     return tile;
@@ -312,7 +319,10 @@ cudaError_t lp_pipeline_launch(const LpArgs &a, const LpTuning &t, int sm_count,
     const uint32_t tile = a.part.tile;
     const bool bcast = a.epilogue == LP_EPI_COPY;
     uint32_t ctas = t.v[LP_TUNE_CTAS_PER_SM] ? (uint32_t)t.v[LP_TUNE_CTAS_PER_SM] : 2u;
-    uint32_t stages = t.v[LP_TUNE_STAGES] ? (uint32_t)t.v[LP_TUNE_STAGES] : (bcast ? 6u : 4u);
+    // broadcast is all stores: the fewer destinations a tile fans out to, the more CTAs it takes to keep HBM busy,
+    // and too many stores in flight cost ~10 % (profiles/r1_tuning.md): about 12 stores per SM in flight
+    if (bcast && !t.v[LP_TUNE_CTAS_PER_SM]) ctas = a.n_out >= 8 ? 1u : (a.n_out >= 3 ? 2u : 4u);
+    uint32_t stages = t.v[LP_TUNE_STAGES] ? (uint32_t)t.v[LP_TUNE_STAGES] : (bcast ? 4u : 3u);
     uint32_t out_stages = bcast ? 0u : (t.v[LP_TUNE_OUT_STAGES] ? (uint32_t)t.v[LP_TUNE_OUT_STAGES] : 2u);
     if (bcast && stages < 3) stages = 3;
     auto smem_of = [&](uint32_t st, uint32_t ost) {
