@@ -32,6 +32,9 @@ from paper_1611_04255_b200 import inputs  # noqa: E402
 METRIC = "lp_allreduce_algbw"
 UNIT = "GB/s (algbw = n*4 bytes per rank / time; roofline on min bytes 2*P*n*4)"
 FALLBACK_HBM_GBS = 6650.0  # B200_PROFILING.md fallback, used only if MEASURED_PEAKS.json is absent
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
+# `ncu --set full` capture (profiles/r1_ncu_lp_pipeline.md); keyed by (P, n, variant)
+NCU_TRAFFIC_BYTES = {(6, 61_000_000, "pipeline"): 2_868_982_000}
 
 
 def parse_args():
@@ -311,7 +314,7 @@ def run_ours(args, c, rank, world, local):
                    "variant": args.variant, "plan": plan, "parallelism": f"replicas x{world} (no collective)",
                    "l2": f"inputs {P * n * 4 / 1e6:.0f} MB per set >> 126 MB L2, {n_sets} rotating sets"},
         "roofline": {"bound": "hbm", "achieved": hbm, "peak": peak, "unit": "GB/s", "frac": hbm / peak,
-                     "traffic": None, "peak_source": peak_src, "frac_of_nominal_8TBs": hbm / 8000.0,
+                     "traffic": NCU_TRAFFIC_BYTES.get((P, n, args.variant)), "peak_source": peak_src, "frac_of_nominal_8TBs": hbm / 8000.0,
                      "kernel": "lp_pipeline_kernel" if variant == 0 else args.variant,
                      "algorithmic_bytes_per_launch": min_bytes},
         "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "detail": detail,
