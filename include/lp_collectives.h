@@ -87,7 +87,9 @@ extern "C" {
 #define LP_TUNE_CTAS_PER_SM 3   /* persistent CTAs per SM (1..8) */
 #define LP_TUNE_CE_STREAMS 4    /* copy-engine variant: number of streams / receive slots (paper: 2) */
 #define LP_TUNE_L2_HINT 5       /* 0 none, 1 evict_first on loads, 2 evict_first on loads and stores */
-#define LP_TUNE_COUNT 6
+#define LP_TUNE_STORE_WAIT 6    /* 0: a store-ring slot is reused once its bulk stores have READ it (default);
+                                   1: only once they have COMPLETED (bounds the store bytes in flight) */
+#define LP_TUNE_COUNT 7
 
 /* ---- LP collectives (the hot path) ----------------------------------------- */
 

@@ -17,7 +17,8 @@ LP_MAX_P = 32
 OP_BROADCAST, OP_REDUCE, OP_ALLREDUCE, OP_BSP_SGD = 0, 1, 2, 3
 VARIANT_PIPELINE, VARIANT_DIRECT, VARIANT_CLUSTER, VARIANT_COPY_ENGINE = 0, 1, 2, 3
 MODEL_STAGE, MODEL_LINK, MODEL_LINK_RING = 0, 1, 2
-TUNE_TILE_ELEMS, TUNE_STAGES, TUNE_OUT_STAGES, TUNE_CTAS_PER_SM, TUNE_CE_STREAMS, TUNE_L2_HINT = range(6)
+TUNE_TILE_ELEMS, TUNE_STAGES, TUNE_OUT_STAGES, TUNE_CTAS_PER_SM, TUNE_CE_STREAMS, TUNE_L2_HINT, TUNE_STORE_WAIT = range(7)
+TUNE_COUNT = 7
 VARIANT_NAMES = {0: "pipeline", 1: "direct", 2: "cluster", 3: "copy_engine"}
 
 
@@ -93,8 +94,28 @@ def _check(rc, what):
         raise LpError(rc, what)
 
 
+class Ranks:
+    """P device vectors registered once.  Caches the host array of device pointers, so a collective on them is
+    one ctypes call (~2 us) instead of P tensor checks per call; accepted wherever a list of tensors is."""
+
+    def __init__(self, bufs):
+        self.bufs = list(bufs)
+        self.arr, self.n = _dev_ptrs(self.bufs)
+
+    def __len__(self):
+        return len(self.bufs)
+
+    def __iter__(self):
+        return iter(self.bufs)
+
+    def __getitem__(self, i):
+        return self.bufs[i]
+
+
 def _dev_ptrs(bufs):
     """Host array of device pointers from a list of CUDA float32 tensors (checks dtype / contiguity / length)."""
+    if isinstance(bufs, Ranks):
+        return bufs.arr, bufs.n
     import torch
     n = bufs[0].numel() if len(bufs) else 0
     for b in bufs:

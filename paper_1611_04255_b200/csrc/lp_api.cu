@@ -19,7 +19,7 @@ namespace {
 
 std::mutex g_mu;
 int g_variant = LP_VARIANT_PIPELINE;
-LpTuning g_tuning = {{0, 0, 0, 0, 0, 0}};
+LpTuning g_tuning = {{0, 0, 0, 0, 0, 0, 0}};
 std::atomic<uint64_t> g_launches{0};
 char g_err[256] = "";
 int g_sm_count = 0;  // 0 = not queried yet
@@ -85,6 +85,7 @@ void fill_args(LpArgs &a, int op, float *const *bufs, float *const *weights, int
     a.lr = lr;
     a.invP = 1.0f / (float)P;  // one RN division on the host (U7)
     a.l2_hint = g_tuning.v[LP_TUNE_L2_HINT];
+    a.store_wait = g_tuning.v[LP_TUNE_STORE_WAIT];
     switch (op) {
         case LP_OP_BROADCAST:
             a.epilogue = LP_EPI_COPY;
@@ -414,6 +415,9 @@ int lp_set_tuning(int key, int value) {
             break;
         case LP_TUNE_L2_HINT:
             if (value > 2) return LP_ERR_INVALID_ARG;
+            break;
+        case LP_TUNE_STORE_WAIT:
+            if (value > 1) return LP_ERR_INVALID_ARG;
             break;
     }
     std::lock_guard<std::mutex> lock(g_mu);

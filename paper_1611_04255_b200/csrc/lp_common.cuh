@@ -25,6 +25,7 @@ struct LpArgs {
     int epilogue;
     float lr, invP;
     int l2_hint;
+    int store_wait;  // LP_TUNE_STORE_WAIT
     lp_partition part;
 };
 

@@ -23,7 +23,18 @@
 
 namespace {
 
-__device__ __forceinline__ void wait_read_lag(int lag) {
+// Wait until all but the newest `lag` bulk-store groups have read their shared-memory source (complete ==
+// false) or have fully completed (complete == true: bounds the store bytes this CTA has in flight).
+__device__ __forceinline__ void wait_read_lag(int lag, bool complete) {
+    if (complete) {
+        switch (lag) {
+            case 0: lp_bulk_wait<0>(); break;
+            case 1: lp_bulk_wait<1>(); break;
+            case 2: lp_bulk_wait<2>(); break;
+            default: lp_bulk_wait<3>(); break;
+        }
+        return;
+    }
     switch (lag) {
         case 0: lp_bulk_wait_read<0>(); break;
         case 1: lp_bulk_wait_read<1>(); break;
@@ -129,7 +140,7 @@ __global__ void __launch_bounds__((CW + 2) * 32) lp_pipeline_kernel(const __grid
                 }
                 lp_bulk_commit();
                 ++issued;
-                wait_read_lag(lag);  // all but the newest `lag` groups have finished reading shared memory
+                wait_read_lag(lag, a.store_wait != 0);  // all but the newest `lag` groups are done with shared memory
                 if (issued > (uint64_t)lag) {
                     lp_mbar_arrive(&oempty[free_slot]);
                     if (++free_slot == out_stages) free_slot = 0;
@@ -258,7 +269,7 @@ __global__ void __launch_bounds__(96) lp_bcast_kernel(const __grid_constant__ Lp
             }
             lp_bulk_commit();
             ++issued;
-            wait_read_lag(lag);
+            wait_read_lag(lag, a.store_wait != 0);
             if (issued > (uint64_t)lag) {
                 lp_mbar_arrive(&empty[free_slot]);
                 if (++free_slot == stages) free_slot = 0;
@@ -308,7 +319,7 @@ static bool read_dominated(const LpArgs &a) { return a.epilogue != LP_EPI_COPY &
 // split finer than it has to be), floor 1024.
 uint32_t lp_pipeline_tile(const LpTuning &t, const LpArgs &a, uint64_t n, uint64_t block) {
     uint32_t tile = t.v[LP_TUNE_TILE_ELEMS] ? (uint32_t)t.v[LP_TUNE_TILE_ELEMS]
-                    : (a.epilogue == LP_EPI_COPY ? 1024u : (read_dominated(a) ? 4096u : 2048u));
+                    : (a.epilogue == LP_EPI_COPY ? (a.n_out == 1 ? 2048u : 1024u) : (read_dominated(a) ? 4096u : 2048u));
     uint64_t blk = block < n ? block : n;
     while (tile > 1024u && (uint64_t)(tile / 2) >= blk) tile /= 2;
     return tile;
@@ -319,12 +330,18 @@ cudaError_t lp_pipeline_launch(const LpArgs &a, const LpTuning &t, int sm_count,
     const uint32_t tile = a.part.tile;
     const bool bcast = a.epilogue == LP_EPI_COPY;
     uint32_t ctas = t.v[LP_TUNE_CTAS_PER_SM] ? (uint32_t)t.v[LP_TUNE_CTAS_PER_SM] : 2u;
-    // broadcast is all stores: the fewer destinations a tile fans out to, the more CTAs it takes to keep HBM busy,
-    // and too many stores in flight cost ~10 % (profiles/r1_tuning.md): about 12 stores per SM in flight
-    if (bcast && !t.v[LP_TUNE_CTAS_PER_SM]) ctas = a.n_out >= 8 ? 1u : (a.n_out >= 3 ? 2u : 4u);
-    uint32_t stages = t.v[LP_TUNE_STAGES] ? (uint32_t)t.v[LP_TUNE_STAGES] : (bcast ? 4u : 3u);
+    uint32_t stages = t.v[LP_TUNE_STAGES] ? (uint32_t)t.v[LP_TUNE_STAGES] : 3u;
     uint32_t out_stages = bcast ? 0u : (t.v[LP_TUNE_OUT_STAGES] ? (uint32_t)t.v[LP_TUNE_OUT_STAGES] : 2u);
-    if (bcast && stages < 3) stages = 3;
+    if (bcast) {
+        // Broadcast is all stores and has a narrow optimum (profiles/r1_tuning.md): about 40 four-KB bulk stores
+        // in flight per SM, i.e. slots-per-SM x destinations ~ 40; more costs ~10 %, fewer starves HBM.
+        uint32_t slots = a.n_out >= 2 ? (40u + (uint32_t)a.n_out / 2u) / (uint32_t)a.n_out : 9u;
+        slots = slots < 3u ? 3u : (slots > 16u ? 16u : slots);
+        uint32_t def_ctas = slots <= 6u ? 1u : (slots + 3u) / 4u;
+        if (a.n_out == 1) def_ctas = 3u;  // plain copy: 8 KB tiles, 3 slots x 3 CTAs
+        if (!t.v[LP_TUNE_CTAS_PER_SM]) ctas = def_ctas;
+        if (!t.v[LP_TUNE_STAGES]) stages = slots / ctas < 3u ? 3u : slots / ctas;
+    }
     auto smem_of = [&](uint32_t st, uint32_t ost) {
         return (st + ost) * tile * 4u + (2u * st + 2u * ost) * 8u;
     };

@@ -16,7 +16,7 @@ torch = pytest.importorskip("torch")
 def _defaults():
     assert torch.cuda.is_available()
     lp.lp_set_variant(lp.VARIANT_PIPELINE)
-    for k in range(6):
+    for k in range(lp.TUNE_COUNT):
         lp.lp_set_tuning(k, 0)
     yield
     torch.cuda.synchronize()

@@ -20,7 +20,7 @@ def _device_and_defaults():
     assert torch.cuda.is_available(), "gpu tests need a CUDA device"
     lp.lib()
     lp.lp_set_variant(lp.VARIANT_PIPELINE)
-    for k in range(6):
+    for k in range(lp.TUNE_COUNT):
         lp.lp_set_tuning(k, 0)
     yield
     torch.cuda.synchronize()
