@@ -334,11 +334,15 @@ cudaError_t lp_pipeline_launch(const LpArgs &a, const LpTuning &t, int sm_count,
     uint32_t out_stages = bcast ? 0u : (t.v[LP_TUNE_OUT_STAGES] ? (uint32_t)t.v[LP_TUNE_OUT_STAGES] : 2u);
     if (bcast) {
         // Broadcast is all stores and has a narrow optimum (profiles/r1_tuning.md): about 40 four-KB bulk stores
-        // in flight per SM, i.e. slots-per-SM x destinations ~ 40; more costs ~10 %, fewer starves HBM.
-        uint32_t slots = a.n_out >= 2 ? (40u + (uint32_t)a.n_out / 2u) / (uint32_t)a.n_out : 9u;
-        slots = slots < 3u ? 3u : (slots > 16u ? 16u : slots);
-        uint32_t def_ctas = slots <= 6u ? 1u : (slots + 3u) / 4u;
-        if (a.n_out == 1) def_ctas = 3u;  // plain copy: 8 KB tiles, 3 slots x 3 CTAs
+        // in flight per SM (slots-per-SM x destinations); more costs ~10 %, fewer starves HBM.  Measured best
+        // (slots per CTA, CTAs per SM) by destination count:
+        uint32_t slots, def_ctas;
+        if (a.n_out <= 1) slots = 9u, def_ctas = 3u;        // plain copy, 8 KB tiles: 3 slots x 3 CTAs
+        else if (a.n_out == 2) slots = 16u, def_ctas = 4u;  // 4 x 4
+        else if (a.n_out == 3) slots = 12u, def_ctas = 3u;  // 4 x 3
+        else if (a.n_out <= 5) slots = 8u, def_ctas = 2u;   // 4 x 2
+        else if (a.n_out <= 7) slots = 6u, def_ctas = 1u;   // 6 x 1
+        else slots = a.n_out <= 10 ? 4u : 3u, def_ctas = 1u;
         if (!t.v[LP_TUNE_CTAS_PER_SM]) ctas = def_ctas;
         if (!t.v[LP_TUNE_STAGES]) stages = slots / ctas < 3u ? 3u : slots / ctas;
     }
