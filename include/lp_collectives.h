@@ -89,7 +89,10 @@ extern "C" {
 #define LP_TUNE_L2_HINT 5       /* 0 none, 1 evict_first on loads, 2 evict_first on loads and stores */
 #define LP_TUNE_STORE_WAIT 6    /* 0: a store-ring slot is reused once its bulk stores have READ it (default);
                                    1: only once they have COMPLETED (bounds the store bytes in flight) */
-#define LP_TUNE_COUNT 7
+#define LP_TUNE_SCHED 7         /* how persistent CTAs pick tiles: 0 (default) dynamic -- each CTA claims its next tile
+                                   from a device-side counter, so SMs that get more HBM bandwidth take more tiles
+                                   and all finish together; 1 static round robin (tile t -> CTA t mod grid) */
+#define LP_TUNE_COUNT 8
 
 /* ---- LP collectives (the hot path) ----------------------------------------- */
 

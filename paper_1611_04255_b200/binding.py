@@ -17,8 +17,9 @@ LP_MAX_P = 32
 OP_BROADCAST, OP_REDUCE, OP_ALLREDUCE, OP_BSP_SGD = 0, 1, 2, 3
 VARIANT_PIPELINE, VARIANT_DIRECT, VARIANT_CLUSTER, VARIANT_COPY_ENGINE = 0, 1, 2, 3
 MODEL_STAGE, MODEL_LINK, MODEL_LINK_RING = 0, 1, 2
-TUNE_TILE_ELEMS, TUNE_STAGES, TUNE_OUT_STAGES, TUNE_CTAS_PER_SM, TUNE_CE_STREAMS, TUNE_L2_HINT, TUNE_STORE_WAIT = range(7)
-TUNE_COUNT = 7
+TUNE_TILE_ELEMS, TUNE_STAGES, TUNE_OUT_STAGES, TUNE_CTAS_PER_SM, TUNE_CE_STREAMS, TUNE_L2_HINT, TUNE_STORE_WAIT, \
+    TUNE_SCHED = range(8)
+TUNE_COUNT = 8
 VARIANT_NAMES = {0: "pipeline", 1: "direct", 2: "cluster", 3: "copy_engine"}
 
 

@@ -19,10 +19,17 @@ namespace {
 
 std::mutex g_mu;
 int g_variant = LP_VARIANT_PIPELINE;
-LpTuning g_tuning = {{0, 0, 0, 0, 0, 0, 0}};
+LpTuning g_tuning = {{0, 0, 0, 0, 0, 0, 0, 0}};
 std::atomic<uint64_t> g_launches{0};
 char g_err[256] = "";
 int g_sm_count = 0;  // 0 = not queried yet
+
+// Tile-claim counters (LpArgs::sched): a ring of self-resetting pairs, one per launch, so launches that overlap
+// on different streams do not share a pair unless kSchedPairs of them are in flight at once.
+constexpr int kSchedPairs = 1024;
+constexpr int kSchedStride = 4;  // unsigned long longs per pair (32 bytes: one L2 sector each)
+unsigned long long *g_sched = nullptr;
+uint32_t g_sched_next = 0;
 
 constexpr int kScratchSlots = 2 * LP_MAX_P + 8;
 float *g_scratch[kScratchSlots];
@@ -86,6 +93,7 @@ void fill_args(LpArgs &a, int op, float *const *bufs, float *const *weights, int
     a.invP = 1.0f / (float)P;  // one RN division on the host (U7)
     a.l2_hint = g_tuning.v[LP_TUNE_L2_HINT];
     a.store_wait = g_tuning.v[LP_TUNE_STORE_WAIT];
+    a.sched = nullptr;  // set by plan_and_run for a real launch
     switch (op) {
         case LP_OP_BROADCAST:
             a.epilogue = LP_EPI_COPY;
@@ -147,6 +155,10 @@ int plan_and_run(int op, float *const *bufs, float *const *weights, int P, size_
         default: tile = lp_pipeline_tile(g_tuning, a, n, block); break;
     }
     a.part = lp_make_partition(n, block, tile);
+    if (!dry_run && g_tuning.v[LP_TUNE_SCHED] == 0 && variant != LP_VARIANT_COPY_ENGINE && a.part.n_tiles > 0) {
+        cudaError_t es = lp_sched_acquire(&a.sched);
+        if (es != cudaSuccess) return cuda_fail(es, "tile-claim counters");
+    }
     // identity collectives: nothing to move (P == 1 broadcast/reduce/allreduce; n == 0)
     const bool noop = (n == 0) || (P == 1 && op != LP_OP_BSP_SGD);
     cudaError_t e = cudaSuccess;
@@ -210,6 +222,24 @@ int run_baseline(bool be, int op, float *const *bufs, int P, size_t n, int root,
 }  // namespace
 
 void lp_count_launch(uint64_t k) { g_launches.fetch_add(k, std::memory_order_relaxed); }
+
+// Called with g_mu held.  The ring is allocated and zeroed once (synchronously: before any launch that uses it).
+cudaError_t lp_sched_acquire(unsigned long long **pair) {
+    if (g_sched == nullptr) {
+        const size_t bytes = (size_t)kSchedPairs * kSchedStride * sizeof(unsigned long long);
+        cudaError_t e = cudaMalloc((void **)&g_sched, bytes);
+        if (e != cudaSuccess) return e;
+        e = cudaMemset(g_sched, 0, bytes);
+        if (e == cudaSuccess) e = cudaDeviceSynchronize();
+        if (e != cudaSuccess) {
+            cudaFree(g_sched);
+            g_sched = nullptr;
+            return e;
+        }
+    }
+    *pair = g_sched + (size_t)(g_sched_next++ % kSchedPairs) * kSchedStride;
+    return cudaSuccess;
+}
 
 // Library scratch: grows on demand (cudaFree synchronises the device, so growing is safe against work in flight).
 cudaError_t lp_scratch_get(int slot, size_t bytes, float **ptr) {
@@ -417,6 +447,7 @@ int lp_set_tuning(int key, int value) {
             if (value > 2) return LP_ERR_INVALID_ARG;
             break;
         case LP_TUNE_STORE_WAIT:
+        case LP_TUNE_SCHED:
             if (value > 1) return LP_ERR_INVALID_ARG;
             break;
     }
@@ -430,9 +461,12 @@ uint64_t lp_launch_count(void) { return g_launches.load(std::memory_order_relaxe
 
 int lp_shutdown(void) {
     std::lock_guard<std::mutex> lock(g_mu);
-    bool any = g_host_ready;
+    bool any = g_host_ready || g_sched != nullptr;
     for (int s = 0; s < kScratchSlots; ++s) any = any || g_scratch[s] != nullptr;
     if (any) cudaDeviceSynchronize();
+    if (g_sched) cudaFree(g_sched);
+    g_sched = nullptr;
+    g_sched_next = 0;
     for (int s = 0; s < kScratchSlots; ++s) {
         if (g_scratch[s]) cudaFree(g_scratch[s]);
         g_scratch[s] = nullptr;

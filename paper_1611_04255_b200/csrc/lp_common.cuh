@@ -26,6 +26,9 @@ struct LpArgs {
     float lr, invP;
     int l2_hint;
     int store_wait;  // LP_TUNE_STORE_WAIT
+    // Dynamic tile claims (LP_TUNE_SCHED 0): sched[0] = tiles claimed beyond the first grid-full, sched[1] = CTAs
+    // that have finished claiming; the last CTA to finish zeroes both for the next launch.  NULL = static round robin.
+    unsigned long long *sched;
     lp_partition part;
 };
 
@@ -62,6 +65,8 @@ cudaError_t lp_seg_launch(const LpSegJob *jobs, int n_jobs, int sm_count, cudaSt
 
 // Launch counter (kernels + async copies enqueued by the library).
 void lp_count_launch(uint64_t k);
+// A zeroed, self-resetting {claimed, finished} counter pair for one launch (see LpArgs::sched).
+cudaError_t lp_sched_acquire(unsigned long long **pair);
 
 #if defined(__CUDACC__)
 // ---- PTX wrappers ------------------------------------------------------------------------------------
@@ -165,6 +170,33 @@ __device__ __forceinline__ float4 lp_sgd4(const float4 &s, const float4 &w, floa
     return make_float4(lp_sgd1(s.x, w.x, lr, invP), lp_sgd1(s.y, w.y, lr, invP), lp_sgd1(s.z, w.z, lr, invP),
                        lp_sgd1(s.w, w.w, lr, invP));
 }
+
+// The a2 schedule of one persistent CTA (lp_schedule.h): which tile it works on next.  Its first tile is
+// blockIdx.x; after that either the next unclaimed tile of the launch (dynamic: one atomicAdd per tile, issued
+// one tile ahead so its latency hides behind the current tile's loads) or blockIdx.x + k * gridDim.x (static).
+// SMs do not get equal shares of HBM bandwidth when the memory system is saturated; with static shares the
+// slow SMs finish last and alone, with claims every SM is busy until the tile list is empty.
+struct LpTileClaimer {
+    unsigned long long *ctr;
+    uint64_t next, n_tiles;
+    __device__ __forceinline__ LpTileClaimer(unsigned long long *c, uint64_t nt) : ctr(c), next(blockIdx.x), n_tiles(nt) {}
+    // tile to work on now (>= n_tiles: none left)
+    __device__ __forceinline__ uint64_t claim() {
+        const uint64_t t = next;
+        if (t < n_tiles) next = ctr ? (uint64_t)gridDim.x + atomicAdd(ctr, 1ull) : t + gridDim.x;
+        return t;
+    }
+    // after the last claim: count this CTA out; the last one re-arms the pair for the next launch
+    __device__ __forceinline__ void finish() {
+        if (!ctr) return;
+        __threadfence();
+        if (atomicAdd(ctr + 1, 1ull) == (unsigned long long)gridDim.x - 1ull) {
+            ctr[0] = 0ull;
+            ctr[1] = 0ull;
+            __threadfence();
+        }
+    }
+};
 
 // Scalar path for the (at most a few) elements of a tile outside its 16-byte aligned body: the chain fold,
 // epilogue and fan-out for element i, straight from and to global memory.

@@ -17,7 +17,13 @@ __global__ void __launch_bounds__(kThreads) lp_direct_kernel(const __grid_consta
     const lp_partition &part = a.part;
     const int n_sum = NS > 0 ? NS : a.n_sum;
     const int tid = threadIdx.x;
-    for (uint64_t t = blockIdx.x; t < part.n_tiles; t += gridDim.x) {
+    // a2: thread 0 claims the CTA's next tile one tile ahead (LpTileClaimer) and hands it over through shared memory
+    __shared__ unsigned long long s_tile[2];
+    LpTileClaimer claimer(a.sched, part.n_tiles);
+    uint64_t t = blockIdx.x;
+    if (tid == 0) claimer.claim();  // consumes blockIdx.x, prefetches the following tile
+    for (int it = 0; t < part.n_tiles; ++it) {
+        if (tid == 0) s_tile[it & 1] = claimer.claim();
         uint64_t off;
         uint32_t len;
         lp_tile_range(part, t, off, len);
@@ -67,7 +73,10 @@ __global__ void __launch_bounds__(kThreads) lp_direct_kernel(const __grid_consta
             for (int v = 0; v < V; ++v)
                 if (live[v]) lp_stg_stream(a.out[q] + a0 + 4 * (uint64_t)(tid + v * kThreads), acc[v]);
         }
+        __syncthreads();
+        t = s_tile[it & 1];
     }
+    if (tid == 0) claimer.finish();
 }
 
 template <int V>

@@ -57,6 +57,9 @@ struct Ring {
 };
 
 // V float4 per add thread per tile, CW add warps: TILE = V * 4 * CW * 32 elements.
+// Every ring slot carries the index of the tile it belongs to (tile_of / otile_of): the producer claims tiles
+// (LpTileClaimer) and the other two roles learn the tile from the slot; an index >= n_tiles is the end marker
+// that travels producer -> add warps -> store thread.
 template <int V, int CW>
 __global__ void __launch_bounds__((CW + 2) * 32) lp_pipeline_kernel(const __grid_constant__ LpArgs a, int stages,
                                                                      int out_stages) {
@@ -69,6 +72,8 @@ __global__ void __launch_bounds__((CW + 2) * 32) lp_pipeline_kernel(const __grid
     uint64_t *empty = full + stages;
     uint64_t *ofull = empty + stages;
     uint64_t *oempty = ofull + out_stages;
+    uint64_t *tile_of = oempty + out_stages;  // [stages]
+    uint64_t *otile_of = tile_of + stages;    // [out_stages]
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < stages; ++s) {
@@ -88,18 +93,27 @@ __global__ void __launch_bounds__((CW + 2) * 32) lp_pipeline_kernel(const __grid
     const lp_partition &part = a.part;
 
     if (warp == 0) {
-        // ---------------- producer: TMA bulk loads in chain order --------------------------------------
+        // ---------------- producer: claims tiles, TMA bulk loads in chain order ---------------------------
         if (lane == 0) {
             const uint64_t pol = lp_policy_evict_first();
             const bool hint = a.l2_hint >= 1;
             Ring ring(stages);
-            for (uint64_t t = blockIdx.x; t < part.n_tiles; t += gridDim.x) {
+            LpTileClaimer claimer(a.sched, part.n_tiles);
+            for (;;) {
+                const uint64_t t = claimer.claim();
+                if (t >= part.n_tiles) {  // end marker
+                    lp_mbar_wait(&empty[ring.slot], ring.phase ^ 1u);
+                    tile_of[ring.slot] = t;
+                    lp_mbar_arrive(&full[ring.slot]);
+                    break;
+                }
                 uint64_t off;
                 uint32_t len;
                 lp_tile_range(part, t, off, len);
                 const uint32_t bytes = (len & ~3u) * 4u;
                 for (int r = 0; r < a.n_in; ++r) {
                     lp_mbar_wait(&empty[ring.slot], ring.phase ^ 1u);
+                    tile_of[ring.slot] = t;
                     if (bytes) {
                         lp_mbar_expect_tx(&full[ring.slot], bytes);
                         float *dst = in_ring + (size_t)ring.slot * TILE;
@@ -113,22 +127,25 @@ __global__ void __launch_bounds__((CW + 2) * 32) lp_pipeline_kernel(const __grid
                     ring.advance();
                 }
             }
+            claimer.finish();
         }
     } else if (warp == 1) {
         // ---------------- store thread: TMA bulk stores to every destination rank -----------------------
         if (lane == 0) {
             const uint64_t pol = lp_policy_evict_first();
             const bool hint = a.l2_hint >= 2;
-            const int lag = out_stages >= 3 ? 2 : (out_stages == 2 ? 1 : 0);
+            const int lag = out_stages >= 3 ? 2 : (out_stages == 2 ? 1 : 0);  // < out_stages: the end marker finds a slot
             Ring ring(out_stages);
             uint64_t issued = 0;
             int free_slot = 0;  // oldest slot not yet handed back
-            for (uint64_t t = blockIdx.x; t < part.n_tiles; t += gridDim.x) {
+            for (;;) {
+                lp_mbar_wait(&ofull[ring.slot], ring.phase);
+                const uint64_t t = otile_of[ring.slot];
+                if (t >= part.n_tiles) break;
                 uint64_t off;
                 uint32_t len;
                 lp_tile_range(part, t, off, len);
                 const uint32_t bytes = (len & ~3u) * 4u;
-                lp_mbar_wait(&ofull[ring.slot], ring.phase);
                 if (bytes) {
                     const float *src = out_ring + (size_t)ring.slot * TILE;
                     for (int q = 0; q < a.n_out; ++q) {
@@ -154,13 +171,21 @@ __global__ void __launch_bounds__((CW + 2) * 32) lp_pipeline_kernel(const __grid
         const int ctid = threadIdx.x - 64;
         Ring ring(stages);
         Ring oring(out_stages);
-        for (uint64_t t = blockIdx.x; t < part.n_tiles; t += gridDim.x) {
+        for (;;) {
+            lp_mbar_wait(&full[ring.slot], ring.phase);
+            const uint64_t t = tile_of[ring.slot];
+            if (t >= part.n_tiles) {  // end marker: pass it on to the store thread
+                lp_mbar_wait(&oempty[oring.slot], oring.phase ^ 1u);
+                if (ctid == 0) otile_of[oring.slot] = t;
+                __syncwarp();
+                if (lane == 0) lp_mbar_arrive(&ofull[oring.slot]);
+                break;
+            }
             uint64_t off;
             uint32_t len;
             lp_tile_range(part, t, off, len);
             float4 acc[V];
             {  // rank 0: the partial starts as its block ("writing block a0 to a buffer on GPU1")
-                lp_mbar_wait(&full[ring.slot], ring.phase);
                 const float4 *s = reinterpret_cast<const float4 *>(in_ring + (size_t)ring.slot * TILE);
 #pragma unroll
                 for (int v = 0; v < V; ++v) acc[v] = s[ctid + v * CT];
@@ -194,6 +219,7 @@ __global__ void __launch_bounds__((CW + 2) * 32) lp_pipeline_kernel(const __grid
             float4 *o = reinterpret_cast<float4 *>(out_ring + (size_t)oring.slot * TILE);
 #pragma unroll
             for (int v = 0; v < V; ++v) o[ctid + v * CT] = acc[v];
+            if (ctid == 0) otile_of[oring.slot] = t;
             lp_fence_proxy_async();
             __syncwarp();
             if (lane == 0) lp_mbar_arrive(&ofull[oring.slot]);
@@ -206,12 +232,14 @@ __global__ void __launch_bounds__((CW + 2) * 32) lp_pipeline_kernel(const __grid
 }
 
 // Broadcast: the root's tile is loaded once into the ring and stored to the P-1 other ranks
-// straight from the same slot.  Warp 0 lane 0 loads, warp 1 lane 0 stores, warp 2 copies the <= 3 tail elements.
-__global__ void __launch_bounds__(96) lp_bcast_kernel(const __grid_constant__ LpArgs a, int stages, int tile) {
+// straight from the same slot.  Warp 0 lane 0 claims tiles and loads, warp 1 lane 0 stores (and copies the
+// <= 3 elements past the 16-byte body of the message's last tile).
+__global__ void __launch_bounds__(64) lp_bcast_kernel(const __grid_constant__ LpArgs a, int stages, int tile) {
     extern __shared__ __align__(128) unsigned char lp_smem[];
     float *ring_buf = reinterpret_cast<float *>(lp_smem);
     uint64_t *full = reinterpret_cast<uint64_t *>(ring_buf + (size_t)stages * tile);
     uint64_t *empty = full + stages;
+    uint64_t *tile_of = empty + stages;
     if (threadIdx.x == 0) {
         for (int s = 0; s < stages; ++s) {
             lp_mbar_init(&full[s], 1);
@@ -227,12 +255,19 @@ __global__ void __launch_bounds__(96) lp_bcast_kernel(const __grid_constant__ Lp
         const uint64_t pol = lp_policy_evict_first();
         const bool hint = a.l2_hint >= 1;
         Ring ring(stages);
-        for (uint64_t t = blockIdx.x; t < part.n_tiles; t += gridDim.x) {
+        LpTileClaimer claimer(a.sched, part.n_tiles);
+        for (;;) {
+            const uint64_t t = claimer.claim();
+            lp_mbar_wait(&empty[ring.slot], ring.phase ^ 1u);
+            tile_of[ring.slot] = t;
+            if (t >= part.n_tiles) {  // end marker
+                lp_mbar_arrive(&full[ring.slot]);
+                break;
+            }
             uint64_t off;
             uint32_t len;
             lp_tile_range(part, t, off, len);
             const uint32_t bytes = (len & ~3u) * 4u;
-            lp_mbar_wait(&empty[ring.slot], ring.phase ^ 1u);
             if (bytes) {
                 lp_mbar_expect_tx(&full[ring.slot], bytes);
                 float *dst = ring_buf + (size_t)ring.slot * tile;
@@ -245,19 +280,22 @@ __global__ void __launch_bounds__(96) lp_bcast_kernel(const __grid_constant__ Lp
             }
             ring.advance();
         }
+        claimer.finish();
     } else if (warp == 1 && lane == 0) {
         const uint64_t pol = lp_policy_evict_first();
         const bool hint = a.l2_hint >= 2;
-        const int lag = stages >= 4 ? 2 : 1;
+        const int lag = stages >= 4 ? 2 : 1;  // < stages - 1: loads keep a slot, and the end marker finds one
         Ring ring(stages);
         uint64_t issued = 0;
         int free_slot = 0;
-        for (uint64_t t = blockIdx.x; t < part.n_tiles; t += gridDim.x) {
+        for (;;) {
+            lp_mbar_wait(&full[ring.slot], ring.phase);
+            const uint64_t t = tile_of[ring.slot];
+            if (t >= part.n_tiles) break;
             uint64_t off;
             uint32_t len;
             lp_tile_range(part, t, off, len);
             const uint32_t bytes = (len & ~3u) * 4u;
-            lp_mbar_wait(&full[ring.slot], ring.phase);
             if (bytes) {
                 const float *src = ring_buf + (size_t)ring.slot * tile;
                 for (int q = 0; q < a.n_out; ++q) {
@@ -267,6 +305,7 @@ __global__ void __launch_bounds__(96) lp_bcast_kernel(const __grid_constant__ Lp
                         lp_bulk_s2g(a.out[q] + off, src, bytes);
                 }
             }
+            for (uint32_t e = len & ~3u; e < len; ++e) lp_scalar_element(a, off + e);
             lp_bulk_commit();
             ++issued;
             wait_read_lag(lag, a.store_wait != 0);
@@ -277,14 +316,6 @@ __global__ void __launch_bounds__(96) lp_bcast_kernel(const __grid_constant__ Lp
             ring.advance();
         }
         lp_bulk_wait<0>();
-    } else if (warp == 2) {
-        for (uint64_t t = blockIdx.x; t < part.n_tiles; t += gridDim.x) {
-            uint64_t off;
-            uint32_t len;
-            lp_tile_range(part, t, off, len);
-            const uint32_t rem = len & 3u;
-            if ((uint32_t)lane < rem) lp_scalar_element(a, off + (len & ~3u) + lane);
-        }
     }
 }
 
@@ -347,7 +378,7 @@ cudaError_t lp_pipeline_launch(const LpArgs &a, const LpTuning &t, int sm_count,
         if (!t.v[LP_TUNE_STAGES]) stages = slots / ctas < 3u ? 3u : slots / ctas;
     }
     auto smem_of = [&](uint32_t st, uint32_t ost) {
-        return (st + ost) * tile * 4u + (2u * st + 2u * ost) * 8u;
+        return (st + ost) * tile * 4u + (3u * st + 3u * ost) * 8u;  // rings + full/empty barriers + tile indices
     };
     // shrink the rings until `ctas` CTAs fit one SM; if even the shallowest rings do not, take fewer CTAs
     const uint32_t want_stages = stages, want_out = out_stages;
@@ -366,7 +397,7 @@ cudaError_t lp_pipeline_launch(const LpArgs &a, const LpTuning &t, int sm_count,
     uint32_t threads;
     int V = 0, CW = 0;
     if (bcast) {
-        threads = 96;
+        threads = 64;
     } else {
         switch (tile) {
             case 1024: V = 2, CW = 4; break;

@@ -120,7 +120,8 @@ def test_tuning_space_bit_exact(oracle):
     want = copies(src)
     oracle.allreduce(want)
     for tile in (1024, 2048, 4096, 8192):
-        for stages, out_stages, ctas, hint in ((2, 1, 1, 0), (3, 2, 2, 1), (8, 3, 1, 2), (4, 4, 3, 0)):
+        for stages, out_stages, ctas, hint, sched in ((2, 1, 1, 0, 0), (3, 2, 2, 1, 1), (8, 3, 1, 2, 0), (4, 4, 3, 0, 1)):
+            lp.lp_set_tuning(lp.TUNE_SCHED, sched)
             lp.lp_set_tuning(lp.TUNE_TILE_ELEMS, tile)
             lp.lp_set_tuning(lp.TUNE_STAGES, stages)
             lp.lp_set_tuning(lp.TUNE_OUT_STAGES, out_stages)
@@ -135,11 +136,48 @@ def test_tuning_space_bit_exact(oracle):
             got = down(dev)
             assert all(same(g, src[3]) for g in got), ("bcast", tile, stages)
     for tile in (1024, 2048, 4096):
-        lp.lp_set_variant(lp.VARIANT_DIRECT)
-        lp.lp_set_tuning(lp.TUNE_TILE_ELEMS, tile)
-        dev = up(src)
-        lp.lp_allreduce(dev, block)
-        assert all(same(g, w) for g, w in zip(down(dev), want)), ("direct", tile)
+        for sched in (0, 1):
+            lp.lp_set_variant(lp.VARIANT_DIRECT)
+            lp.lp_set_tuning(lp.TUNE_TILE_ELEMS, tile)
+            lp.lp_set_tuning(lp.TUNE_SCHED, sched)
+            dev = up(src)
+            lp.lp_allreduce(dev, block)
+            assert all(same(g, w) for g, w in zip(down(dev), want)), ("direct", tile, sched)
+
+
+def test_tile_claim_counters_rearm_and_streams(oracle):
+    # a2 with dynamic tile claims: every launch takes a self-resetting counter pair from a ring of 1024.  More
+    # launches than pairs (each pair reused), back to back on one stream and interleaved on two streams, must
+    # all give the oracle's bits: a pair that was not re-armed would skip or repeat tiles.
+    P, n, block = 3, 150_001, 8_192
+    src = inputs.rank_vectors(21, P, n, "uniform")
+    want = oracle.chain_sum(src)
+    for variant in (lp.VARIANT_PIPELINE, lp.VARIANT_DIRECT):
+        lp.lp_set_variant(variant)
+        pristine = up(src)
+        work = [torch.empty_like(t) for t in pristine]
+        streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+        sets = []
+        for s in streams:
+            with torch.cuda.stream(s):
+                sets.append(([torch.empty_like(t) for t in pristine], s))
+        torch.cuda.synchronize()
+        for it in range(1300):
+            for w, p in zip(work, pristine):
+                w.copy_(p)
+            lp.lp_reduce(work, block, root=it % P)
+            if it % 97 == 0 or it == 1299:
+                torch.cuda.synchronize()
+                assert same(work[it % P].cpu().numpy(), want), (variant, it)
+        for it in range(40):
+            for bufs, s in sets:
+                with torch.cuda.stream(s):
+                    for w, p in zip(bufs, pristine):
+                        w.copy_(p)
+                    lp.lp_allreduce(bufs, block, stream=s)
+            torch.cuda.synchronize()
+            for bufs, _ in sets:
+                assert all(same(b.cpu().numpy(), want) for b in bufs), (variant, "streams", it)
 
 
 def test_chain_order_and_invariances(oracle):
