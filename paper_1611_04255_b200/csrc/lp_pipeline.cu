@@ -340,19 +340,21 @@ constexpr uint32_t kSmemPerCtaMax = 227u * 1024u;
 
 }  // namespace
 
-// Defaults measured on B200 (profiles/r1_tuning.md): what matters is the number of load bytes in flight per SM.
-// A read-dominated fold (reduce: P reads, 1 write) wants ~96 KB (16 KB tiles, 3 slots, 2 CTAs/SM); once every
-// rank is written back too (allreduce, SGD) ~48 KB is best (8 KB tiles) -- deeper rings only lengthen the DRAM
-// queues the stores have to wait in.
+// Defaults measured on B200 with dynamic tile claims (profiles/r1_tuning.md).  With every SM busy until the tile
+// list is empty the optimum is broad; what matters is enough load bytes in flight per SM: 64 KB for a fold that
+// writes every rank back (allreduce, SGD: 8 KB tiles x 4 slots x 2 CTAs), 96 KB for the read-dominated reduce
+// (6 slots), and for broadcast a ring that covers the time its slots are pinned by n_out stores each.
 static bool read_dominated(const LpArgs &a) { return a.epilogue != LP_EPI_COPY && a.n_out == 1 && a.n_sum > 1; }
 
 // Tile size: the tuned or default size, halved while a whole block still fits in the half (a block is never
 // split finer than it has to be), floor 1024.
 uint32_t lp_pipeline_tile(const LpTuning &t, const LpArgs &a, uint64_t n, uint64_t block) {
     uint32_t tile = t.v[LP_TUNE_TILE_ELEMS] ? (uint32_t)t.v[LP_TUNE_TILE_ELEMS]
-                    : (a.epilogue == LP_EPI_COPY ? (a.n_out == 1 ? 2048u : 1024u) : (read_dominated(a) ? 4096u : 2048u));
+                    : (a.epilogue == LP_EPI_COPY && a.n_out >= 9 ? 1024u : 2048u);
     uint64_t blk = block < n ? block : n;
     while (tile > 1024u && (uint64_t)(tile / 2) >= blk) tile /= 2;
+    // latency regime: fewer tiles than SMs -> halve the tile so that twice as many SMs share the message
+    if (!t.v[LP_TUNE_TILE_ELEMS] && tile > 1024u && (n + tile - 1) / tile < 148u) tile = 1024u;
     return tile;
 }
 
@@ -360,22 +362,15 @@ cudaError_t lp_pipeline_launch(const LpArgs &a, const LpTuning &t, int sm_count,
                                cudaStream_t stream) {
     const uint32_t tile = a.part.tile;
     const bool bcast = a.epilogue == LP_EPI_COPY;
-    uint32_t ctas = t.v[LP_TUNE_CTAS_PER_SM] ? (uint32_t)t.v[LP_TUNE_CTAS_PER_SM] : 2u;
-    uint32_t stages = t.v[LP_TUNE_STAGES] ? (uint32_t)t.v[LP_TUNE_STAGES] : 3u;
+    uint32_t ctas = t.v[LP_TUNE_CTAS_PER_SM] ? (uint32_t)t.v[LP_TUNE_CTAS_PER_SM] : (bcast && a.n_out <= 2 ? 3u : 2u);
+    uint32_t stages = t.v[LP_TUNE_STAGES] ? (uint32_t)t.v[LP_TUNE_STAGES]
+                      : (bcast ? (a.n_out <= 2 ? 6u : 4u) : (read_dominated(a) ? 6u : 4u));
     uint32_t out_stages = bcast ? 0u : (t.v[LP_TUNE_OUT_STAGES] ? (uint32_t)t.v[LP_TUNE_OUT_STAGES] : 2u);
-    if (bcast) {
-        // Broadcast is all stores and has a narrow optimum (profiles/r1_tuning.md): about 40 four-KB bulk stores
-        // in flight per SM (slots-per-SM x destinations); more costs ~10 %, fewer starves HBM.  Measured best
-        // (slots per CTA, CTAs per SM) by destination count:
-        uint32_t slots, def_ctas;
-        if (a.n_out <= 1) slots = 9u, def_ctas = 3u;        // plain copy, 8 KB tiles: 3 slots x 3 CTAs
-        else if (a.n_out == 2) slots = 16u, def_ctas = 4u;  // 4 x 4
-        else if (a.n_out == 3) slots = 12u, def_ctas = 3u;  // 4 x 3
-        else if (a.n_out <= 5) slots = 8u, def_ctas = 2u;   // 4 x 2
-        else if (a.n_out <= 7) slots = 6u, def_ctas = 1u;   // 6 x 1
-        else slots = a.n_out <= 10 ? 4u : 3u, def_ctas = 1u;
-        if (!t.v[LP_TUNE_CTAS_PER_SM]) ctas = def_ctas;
-        if (!t.v[LP_TUNE_STAGES]) stages = slots / ctas < 3u ? 3u : slots / ctas;
+    // latency regime (at most one tile per SM): one CTA per SM and a ring deep enough to have the tile of every
+    // rank in flight at once -- the chain's P loads cost one HBM latency instead of P / stages of them
+    if (a.part.n_tiles <= (uint64_t)sm_count) {
+        if (!t.v[LP_TUNE_CTAS_PER_SM]) ctas = 1u;
+        if (!t.v[LP_TUNE_STAGES] && !bcast && stages < (uint32_t)a.n_in) stages = a.n_in < 24 ? (uint32_t)a.n_in : 24u;
     }
     auto smem_of = [&](uint32_t st, uint32_t ost) {
         return (st + ost) * tile * 4u + (3u * st + 3u * ost) * 8u;  // rings + full/empty barriers + tile indices
@@ -418,6 +413,13 @@ cudaError_t lp_pipeline_launch(const LpArgs &a, const LpTuning &t, int sm_count,
     if (dry_run || grid == 0) return cudaSuccess;
 
     lp_count_launch(1);
+    LpArgs a_static;
+    const LpArgs *ap = &a;
+    if (a.sched && a.part.n_tiles <= 2 * grid) {  // at most two tiles per CTA: nothing to balance, skip the claims
+        a_static = a;
+        a_static.sched = nullptr;
+        ap = &a_static;
+    }
     if (bcast) {
         static int attr_bytes = 0;
         if ((int)cfg->smem_bytes > attr_bytes) {
@@ -426,13 +428,13 @@ cudaError_t lp_pipeline_launch(const LpArgs &a, const LpTuning &t, int sm_count,
             if (e != cudaSuccess) return e;
             attr_bytes = (int)cfg->smem_bytes;
         }
-        lp_bcast_kernel<<<cfg->grid, cfg->threads, cfg->smem_bytes, stream>>>(a, (int)stages, (int)tile);
+        lp_bcast_kernel<<<cfg->grid, cfg->threads, cfg->smem_bytes, stream>>>(*ap, (int)stages, (int)tile);
         return cudaGetLastError();
     }
     switch (tile) {
-        case 1024: return launch_fold<2, 4>(a, *cfg, stream);
-        case 2048: return launch_fold<4, 4>(a, *cfg, stream);
-        case 4096: return launch_fold<4, 8>(a, *cfg, stream);
-        default: return launch_fold<8, 8>(a, *cfg, stream);
+        case 1024: return launch_fold<2, 4>(*ap, *cfg, stream);
+        case 2048: return launch_fold<4, 4>(*ap, *cfg, stream);
+        case 4096: return launch_fold<4, 8>(*ap, *cfg, stream);
+        default: return launch_fold<8, 8>(*ap, *cfg, stream);
     }
 }

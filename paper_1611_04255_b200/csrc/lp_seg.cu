@@ -20,38 +20,43 @@ __global__ void __launch_bounds__(kSegThreads) lp_seg_kernel(const __grid_consta
     const float *a = job.a;
     const float *b = job.b;
     const uint64_t len = job.len;
-    const uint64_t gtid = (uint64_t)blockIdx.x * kSegThreads + threadIdx.x;
-    const uint64_t gsize = (uint64_t)gridDim.x * kSegThreads;
+    // One CTA per chunk of kSegThreads * kSegUnroll 16-byte vectors: the hardware block scheduler hands chunks to
+    // SMs as they free up, so (as with the LP kernels' tile claims) no SM is left with a fixed share to finish alone.
     const uint32_t mis = (uint32_t)((uintptr_t)dst & 15u);
     const bool same = ((uintptr_t)a & 15u) == mis && (b == nullptr || ((uintptr_t)b & 15u) == mis);
     if (!same) {  // operands disagree on alignment: element-wise (never the case for the MST / BE segments)
-        for (uint64_t i = gtid; i < len; i += gsize) dst[i] = b ? __fadd_rn(a[i], b[i]) : a[i];
+        const uint64_t per = (uint64_t)kSegThreads * kSegUnroll * 4;
+        const uint64_t lo = (uint64_t)blockIdx.x * per;
+        const uint64_t hi = lo + per < len ? lo + per : len;
+        for (uint64_t i = lo + threadIdx.x; i < hi; i += kSegThreads) dst[i] = b ? __fadd_rn(a[i], b[i]) : a[i];
         return;
     }
     uint64_t head = ((16u - mis) & 15u) >> 2;
     if (head > len) head = len;
     const uint64_t nvec = (len - head) >> 2;
     const uint64_t tail0 = head + (nvec << 2);
-    if (gtid < head) dst[gtid] = b ? __fadd_rn(a[gtid], b[gtid]) : a[gtid];
-    if (gtid < len - tail0) dst[tail0 + gtid] = b ? __fadd_rn(a[tail0 + gtid], b[tail0 + gtid]) : a[tail0 + gtid];
+    if (blockIdx.x == 0) {
+        const uint64_t i = threadIdx.x;
+        if (i < head) dst[i] = b ? __fadd_rn(a[i], b[i]) : a[i];
+        if (i < len - tail0) dst[tail0 + i] = b ? __fadd_rn(a[tail0 + i], b[tail0 + i]) : a[tail0 + i];
+    }
     float *d4 = dst + head;
     const float *a4 = a + head;
     const float *b4 = b ? b + head : nullptr;
-    for (uint64_t v0 = gtid; v0 < nvec; v0 += gsize * kSegUnroll) {
-        float4 x[kSegUnroll], y[kSegUnroll];
+    const uint64_t v0 = (uint64_t)blockIdx.x * (kSegThreads * kSegUnroll) + threadIdx.x;
+    float4 x[kSegUnroll], y[kSegUnroll];
 #pragma unroll
-        for (int u = 0; u < kSegUnroll; ++u) {
-            const uint64_t v = v0 + (uint64_t)u * gsize;
-            if (v < nvec) {
-                x[u] = lp_ldg_stream(a4 + 4 * v);
-                if (b4) y[u] = lp_ldg_stream(b4 + 4 * v);
-            }
+    for (int u = 0; u < kSegUnroll; ++u) {
+        const uint64_t v = v0 + (uint64_t)u * kSegThreads;
+        if (v < nvec) {
+            x[u] = lp_ldg_stream(a4 + 4 * v);
+            if (b4) y[u] = lp_ldg_stream(b4 + 4 * v);
         }
+    }
 #pragma unroll
-        for (int u = 0; u < kSegUnroll; ++u) {
-            const uint64_t v = v0 + (uint64_t)u * gsize;
-            if (v < nvec) lp_stg_stream(d4 + 4 * v, b4 ? lp_add4(x[u], y[u]) : x[u]);
-        }
+    for (int u = 0; u < kSegUnroll; ++u) {
+        const uint64_t v = v0 + (uint64_t)u * kSegThreads;
+        if (v < nvec) lp_stg_stream(d4 + 4 * v, b4 ? lp_add4(x[u], y[u]) : x[u]);
     }
 }
 
@@ -68,11 +73,11 @@ cudaError_t lp_seg_launch(const LpSegJob *jobs, int n_jobs, int sm_count, cudaSt
     }
     if (m == 0) return cudaSuccess;
     for (int i = m; i < LP_MAX_JOBS; ++i) s.j[i] = LpSegJob{nullptr, nullptr, nullptr, 0};
-    // enough CTAs over all jobs to fill the chip 8 deep, no more than the longest job needs
-    uint64_t per_job = ((uint64_t)sm_count * 8 + m - 1) / m;
-    uint64_t need = (longest / 4 + (uint64_t)kSegThreads * kSegUnroll - 1) / ((uint64_t)kSegThreads * kSegUnroll);
-    if (need == 0) need = 1;
-    if (per_job > need) per_job = need;
+    // one CTA per chunk of the longest job (shorter jobs' surplus CTAs return at once)
+    (void)sm_count;
+    const uint64_t chunk = (uint64_t)kSegThreads * kSegUnroll * 4;  // elements
+    uint64_t per_job = (longest + chunk - 1) / chunk + 1;           // + 1: a misaligned head shifts the body
+    if (per_job > 0x7fffffffull) return cudaErrorInvalidValue;
     dim3 grid((unsigned)per_job, (unsigned)m, 1);
     lp_count_launch(1);
     lp_seg_kernel<<<grid, kSegThreads, 0, stream>>>(s);

@@ -9,7 +9,7 @@ bytes of the op (broadcast P*n*4, reduce (P+1)*n*4, allreduce 2*P*n*4) so LP, MS
 algbw = n*4 / t.  Timing: CUDA events around one replay of a CUDA graph holding K back-to-back calls (device-side
 time per call: the Python / ctypes call overhead of ~10 us is not billed), K chosen for ~2 ms per measurement,
 median of 3; working sets rotate through
->= 256 MB (2 x L2) where the message allows it, and are restored from pristine copies between measurements.
+>= 1 GB (8 x the 126 MB L2) where the arena allows it, and are restored from pristine copies between measurements.
 """
 from __future__ import annotations
 
@@ -51,10 +51,15 @@ def main(argv=None):
     ap.add_argument("--max-exp", type=int, default=27)
     ap.add_argument("--P", default="2,4,8,16")
     ap.add_argument("--block", type=int, default=65_536)
+    ap.add_argument("--variant", default="pipeline", choices=["pipeline", "direct"],
+                    help="LP realisation timed in the LP column (default: the library default)")
+    ap.add_argument("--algos", default="lp,mst,be")
     args = ap.parse_args(argv)
     assert torch.cuda.is_available(), "the sweep needs a CUDA device"
     dev = torch.device("cuda", 0)
     lp.lib()
+    lp.lp_set_variant({"pipeline": lp.VARIANT_PIPELINE, "direct": lp.VARIANT_DIRECT}[args.variant])
+    algos = tuple(a for a in ALGOS if a in args.algos.split(","))
     peak = 6553.3
     try:
         peak = float(json.load(open(os.path.join(os.path.dirname(__file__), "..", "MEASURED_PEAKS.json")))["hbm_gbs"])
@@ -69,13 +74,13 @@ def main(argv=None):
         work = [torch.empty_like(p) for p in pristine]
         for e in range(args.min_exp, args.max_exp + 1):
             n = 1 << e
-            n_sets = int(max(1, min(n_max // n, 64, -(-2 * L2_BYTES // (P * n * 4)))))
+            n_sets = int(max(1, min(n_max // n, 64, -(-8 * L2_BYTES // (P * n * 4)))))
             sets = [[w[s * n:(s + 1) * n] for w in work] for s in range(n_sets)]
             for op in OPS:
                 mb = lp.lp_min_bytes(OP_ID[op], P, n)
                 est = max(mb / 3e12, 4e-6)  # seconds per call, rough
                 K = int(min(max(2e-3 / est, 3), 20 * n_sets, 400))
-                for algo in ALGOS:
+                for algo in algos:
                     if algo == "be" and P & (P - 1):
                         continue
                     # K calls captured in one CUDA graph: device-side time per call, no host call overhead
@@ -124,7 +129,7 @@ def write_markdown(rows, path, peak, Ps, args):
     with open(path, "w") as f:
         f.write("# Message-size sweep (BASELINE.json configs[3]) — LP vs MST vs BE on one B200\n\n")
         f.write(f"Command: `python -m paper_1611_04255_b200.sweep --out {args.out} --min-exp {args.min_exp} "
-                f"--max-exp {args.max_exp} --P {args.P} --block {args.block}`\n\n")
+                f"--max-exp {args.max_exp} --P {args.P} --block {args.block} --variant {args.variant} --algos {args.algos}`\n\n")
         f.write(f"Cells: GB/s on the op's minimum HBM bytes (fraction of the measured copy peak {peak} GB/s); "
                 "LP block 65,536 elements; uniform[-1,1], seed [3, r]. North-star bar: LP >= 80 % of 8 TB/s = 6400 GB/s "
                 "for messages >= 64 MB, and LP faster than MST and BE.\n")
@@ -137,9 +142,10 @@ def write_markdown(rows, path, peak, Ps, args):
                     if not a:
                         continue
                     m, b = idx.get((op, "mst", P, n)), idx.get((op, "be", P, n))
+                    nan = float("nan")
                     f.write(f"| {size(n * 4)} | {a['us']:.1f} | {a['hbm_GBps']:.0f} ({a['frac_measured']:.2f}) | "
-                            f"{a['frac_8TBs']:.2f} | {m['hbm_GBps']:.0f} | {(b['hbm_GBps'] if b else float('nan')):.0f} | "
-                            f"{m['us'] / a['us']:.2f}x | {(b['us'] / a['us'] if b else float('nan')):.2f}x |\n")
+                            f"{a['frac_8TBs']:.2f} | {(m['hbm_GBps'] if m else nan):.0f} | {(b['hbm_GBps'] if b else nan):.0f} | "
+                            f"{(m['us'] / a['us'] if m else nan):.2f}x | {(b['us'] / a['us'] if b else nan):.2f}x |\n")
 
 
 if __name__ == "__main__":
