@@ -60,6 +60,8 @@ def lib() -> ctypes.CDLL:
             getattr(L, name).argtypes = [pp, i32, sz]
         for name in ("lpo_bsp_sgd_step", "lpo_bsp_sgd_step_omp"):
             getattr(L, name).argtypes = [pp, pp, i32, sz, i32, f32]
+        for name in ("lpo_bsp_sgd_momentum_step", "lpo_bsp_sgd_alg2_step"):
+            getattr(L, name).argtypes = [pp, pp, ctypes.c_void_p, i32, sz, i32, f32, f32]
         L.lpo_lp_blocked.argtypes = [pp, i32, sz, sz, i32, i32, pu64]
         L.lpo_num_blocks.argtypes = [sz, sz]
         L.lpo_num_blocks.restype = u64
@@ -127,6 +129,35 @@ def bsp_sgd_step(grads, weights, root=0, lr=0.01, omp=False):
         raise ValueError("grads and weights must match in P and n")
     f = "lpo_bsp_sgd_step_omp" if omp else "lpo_bsp_sgd_step"
     _check(getattr(lib(), f)(ga, wa, len(grads), n, root, ctypes.c_float(lr)), f)
+
+
+def _velocity_ptr(velocity, n):
+    if velocity is None:
+        return None
+    if not (isinstance(velocity, np.ndarray) and velocity.dtype == np.float32 and velocity.flags.c_contiguous
+            and velocity.flags.writeable and velocity.size == n):
+        raise TypeError("velocity must be a writable C-contiguous float32 numpy array of n elements")
+    return ctypes.c_void_p(velocity.ctypes.data)
+
+
+def bsp_sgd_momentum_step(grads, weights, velocity, root=0, lr=0.01, mu=0.9):
+    """Alg. 3 step with Caffe-style momentum (reading U18); velocity is one vector of n floats."""
+    ga, n = _ptrs(grads)
+    wa, nw = _ptrs(weights)
+    if n != nw or len(grads) != len(weights):
+        raise ValueError("grads and weights must match in P and n")
+    _check(lib().lpo_bsp_sgd_momentum_step(ga, wa, _velocity_ptr(velocity, n), len(grads), n, root,
+                                           ctypes.c_float(lr), ctypes.c_float(mu)), "lpo_bsp_sgd_momentum_step")
+
+
+def bsp_sgd_alg2_step(grads, weights, velocity=None, root=0, lr=0.01, mu=0.0):
+    """Alg. 2 step: reduce to root (grads[root] <- S), root update, broadcast; velocity None = plain SGD."""
+    ga, n = _ptrs(grads)
+    wa, nw = _ptrs(weights)
+    if n != nw or len(grads) != len(weights):
+        raise ValueError("grads and weights must match in P and n")
+    _check(lib().lpo_bsp_sgd_alg2_step(ga, wa, _velocity_ptr(velocity, n), len(grads), n, root,
+                                       ctypes.c_float(lr), ctypes.c_float(mu)), "lpo_bsp_sgd_alg2_step")
 
 
 def lp_blocked(bufs, block, op, root=0) -> int:

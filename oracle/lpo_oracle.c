@@ -142,6 +142,78 @@ int lpo_bsp_sgd_step(float *const *grads, float *const *weights, int P,
     return LPO_OK;
 }
 
+/* BSP-SGD step with momentum.  PAPER.md:216: "The solver is
+ * SGD + momentum"; the paper prints no formula.  Reading U18: the solver of
+ * the system the paper modifies (Caffe's SGD solver):
+ *   v' = mu * v + eta * grad ;  w' = w - v'
+ * with grad = S * (1/P) as in lpo_bsp_sgd_step.  Five separately
+ * rounded fp32 ops per element, in this order, no FMA:
+ *   g = S * invP ; t = lr * g ; m = mu * v ; v' = m + t ; w' = w_root - v'.
+ * The velocity is ONE vector of n floats: it lives where the update is
+ * computed (in Alg. 3 every replica of it would hold the same bits).  The new
+ * w' goes to every weight replica (U8); grads are unchanged.  mu = 0 with
+ * v = 0 is lpo_bsp_sgd_step. */
+int lpo_bsp_sgd_momentum_step(float *const *grads, float *const *weights,
+                              float *velocity, int P, size_t n, int root,
+                              float lr, float mu)
+{
+    if (bad_args(grads, P, root) || bad_args(weights, P, root) || velocity == NULL)
+        return LPO_EINVAL;
+    const float invP = 1.0f / (float)P;
+    for (size_t i = 0; i < n; ++i) {
+        float s = grads[0][i];
+        for (int r = 1; r < P; ++r)
+            s = s + grads[r][i];
+        float g = s * invP;
+        float t = lr * g;
+        float m = mu * velocity[i];
+        float v = m + t;
+        float w = weights[root][i] - v;
+        velocity[i] = v;
+        for (int r = 0; r < P; ++r)
+            weights[r][i] = w;
+    }
+    return LPO_OK;
+}
+
+/* BSP-SGD step the Alg. 2 way (PAPER.md:140-168 as reconstructed in reading
+ * U9, prose PAPER.md:178): "The master GPU reconstructs grad by reducing all
+ * grad_sub.  Then, GPUs synchronize latest weight w by broadcasting."
+ *   1. grad = reduce(grad_sub) to the root       -> grads[root] holds S (in place, MPI style)
+ *   2. if root: w = GradientUpdate()             -> weights[root] updated from grads[root]
+ *   3. broadcast(w) from the root                -> every replica = weights[root]
+ * Written as those three steps, each calling the definition above it.  The
+ * update arithmetic is that of lpo_bsp_sgd_step (velocity == NULL) or of
+ * lpo_bsp_sgd_momentum_step, so the weights agree bit for bit with Alg. 3's
+ * fused step (tests pin that); the difference is the side effect on
+ * grads[root] and the number of passes over memory. */
+int lpo_bsp_sgd_alg2_step(float *const *grads, float *const *weights,
+                          float *velocity, int P, size_t n, int root,
+                          float lr, float mu)
+{
+    if (bad_args(grads, P, root) || bad_args(weights, P, root))
+        return LPO_EINVAL;
+    int rc = lpo_reduce(grads, P, n, root);                 /* step 1 */
+    if (rc != LPO_OK)
+        return rc;
+    const float invP = 1.0f / (float)P;
+    float *w = weights[root];
+    const float *S = grads[root];
+    for (size_t i = 0; i < n; ++i) {                        /* step 2, root only */
+        float g = S[i] * invP;
+        float t = lr * g;
+        if (velocity != NULL) {
+            float m = mu * velocity[i];
+            float v = m + t;
+            velocity[i] = v;
+            w[i] = w[i] - v;
+        } else {
+            w[i] = w[i] - t;
+        }
+    }
+    return lpo_broadcast(weights, P, n, root);              /* step 3 */
+}
+
 /* The same two definitions with the element loop spread over host threads.
  * Element i never depends on element j != i, so the bits are those of the
  * serial loops above (tests assert it).  These are the versions bench.py times

@@ -235,3 +235,127 @@ def test_sgd_step_fp64_bound_and_iterations(oracle):
         assert all(w.tobytes() == weights[0].tobytes() for w in weights)
         ref = w64 - it * lr * gbar
         assert np.max(np.abs(weights[0] - ref)) <= it * (2.0 ** -23) * 0.3
+
+
+# ----------------------------------------------------------------------------
+# SGD + momentum (reading U18) and the Alg. 2 step (U9)
+# ----------------------------------------------------------------------------
+
+def test_momentum_step_is_the_five_op_composition(oracle):
+    # written out with numpy float32 ops, one RN op each: g = S*invP, t = lr*g, m = mu*v, v' = m+t, w' = w_root-v'
+    P, n, lr, mu, root = 5, 4099, np.float32(0.015), np.float32(0.9), 3
+    grads, weights = inputs.sgd_inputs(71, P, n)
+    for r in range(P):
+        weights[r] = weights[r] + np.float32(r)
+    vel = inputs.normal(71, 99, n, 0.01)
+    g0 = _copy(grads)
+    S = grads[0].copy()
+    for r in range(1, P):
+        S = S + grads[r]
+    invP = np.float32(1.0) / np.float32(P)
+    t = lr * (S * invP)
+    m = mu * vel
+    v_want = m + t
+    w_want = weights[root] - v_want
+    assert v_want.dtype == np.float32 and w_want.dtype == np.float32
+    oracle.bsp_sgd_momentum_step(grads, weights, vel, root=root, lr=float(lr), mu=float(mu))
+    assert vel.tobytes() == v_want.tobytes()
+    for r in range(P):
+        assert weights[r].tobytes() == w_want.tobytes()
+        assert grads[r].tobytes() == g0[r].tobytes()
+
+
+def test_momentum_closed_forms(oracle):
+    n = 96
+    # mu = 0, v = 0: exactly the plain step (m = 0*0 = 0, v' = 0 + t = t)
+    grads, weights = inputs.sgd_inputs(72, 4, n)
+    w_plain = _copy(weights)
+    oracle.bsp_sgd_step(grads, w_plain, root=1, lr=0.01)
+    vel = np.zeros(n, np.float32)
+    oracle.bsp_sgd_momentum_step(grads, weights, vel, root=1, lr=0.01, mu=0.0)
+    assert all(a.tobytes() == b.tobytes() for a, b in zip(weights, w_plain))
+    # lr = 0: v' = mu*v, w' = w - mu*v  (dyadic values: exact)
+    P = 2
+    grads = [inputs.small_integers(73, r, n) for r in range(P)]
+    w = inputs.small_integers(73, 7, n, -100, 100)
+    weights = [w.copy() for _ in range(P)]
+    v = inputs.small_integers(73, 8, n, -64, 64)
+    vel = v.copy()
+    oracle.bsp_sgd_momentum_step(grads, weights, vel, root=0, lr=0.0, mu=0.5)
+    assert vel.tolist() == (0.5 * v.astype(np.float64)).tolist()
+    assert weights[1].tolist() == (w.astype(np.float64) - 0.5 * v.astype(np.float64)).tolist()
+    # constant small-integer gradient g on P = 4 ranks, lr = 0.25, mu = 0.5, v0 = 0: everything stays dyadic, so
+    # the geometric recurrence holds EXACTLY:  v_k = lr*g*(1 - mu^k)/(1 - mu),  w_k = w_0 - sum_{j<=k} v_j
+    P, lr, mu = 4, 0.25, 0.5
+    g = inputs.small_integers(74, 0, n, -8, 8)
+    grads = [g.copy() for _ in range(P)]
+    w0 = inputs.small_integers(74, 1, n, -100, 100)
+    weights = [w0.copy() for _ in range(P)]
+    vel = np.zeros(n, np.float32)
+    g64, w64, acc = g.astype(np.float64), w0.astype(np.float64), np.zeros(n)
+    for k in range(1, 9):
+        oracle.bsp_sgd_momentum_step(grads, weights, vel, root=k % P, lr=lr, mu=mu)
+        vk = lr * g64 * (1.0 - mu ** k) / (1.0 - mu)
+        acc = acc + vk
+        assert vel.tolist() == vk.tolist(), k
+        assert all(x.tolist() == (w64 - acc).tolist() for x in weights), k
+    # sign: positive gradient, positive velocity both decrease w
+    grads = [np.ones(4, np.float32) for _ in range(2)]
+    weights = [np.zeros(4, np.float32) for _ in range(2)]
+    vel = np.full(4, 2.0, np.float32)
+    oracle.bsp_sgd_momentum_step(grads, weights, vel, root=0, lr=0.25, mu=0.5)
+    assert vel.tolist() == [1.25] * 4 and weights[1].tolist() == [-1.25] * 4
+
+
+def test_momentum_tracks_fp64_recurrence(oracle):
+    P, n, lr, mu = 8, 2048, 0.01, 0.9
+    grads, weights = inputs.sgd_inputs(2, P, n)
+    vel = np.zeros(n, np.float32)
+    w64, v64 = weights[0].astype(np.float64), np.zeros(n)
+    gbar = np.stack([g.astype(np.float64) for g in grads]).mean(axis=0)
+    for it in range(1, 21):
+        oracle.bsp_sgd_momentum_step(grads, weights, vel, root=0, lr=lr, mu=mu)
+        v64 = mu * v64 + lr * gbar
+        w64 = w64 - v64
+        assert all(w.tobytes() == weights[0].tobytes() for w in weights)
+        assert np.max(np.abs(vel - v64)) <= it * 2.0 ** -23 * 0.02
+        assert np.max(np.abs(weights[0] - w64)) <= it * 2.0 ** -23 * 0.5
+
+
+@pytest.mark.parametrize("with_momentum", [False, True])
+def test_alg2_step_is_reduce_update_broadcast(oracle, with_momentum):
+    # Alg. 2 written with the oracle's OTHER entry points and numpy: reduce (grads[root] <- S), numpy update of
+    # the root replica, broadcast.  Its weights equal the fused Alg. 3 step bit for bit (same arithmetic on the same S).
+    P, n, lr, mu, root = 6, 3001, np.float32(0.02), np.float32(0.9), 4
+    grads, weights = inputs.sgd_inputs(75, P, n)
+    for r in range(P):
+        weights[r] = weights[r] + np.float32(r)
+    vel = inputs.normal(75, 99, n, 0.01) if with_momentum else None
+    g_a, w_a, v_a = _copy(grads), _copy(weights), (vel.copy() if with_momentum else None)
+    g_b, w_b, v_b = _copy(grads), _copy(weights), (vel.copy() if with_momentum else None)
+    # (a) by hand
+    oracle.reduce(g_a, root=root)
+    S = g_a[root]
+    t = lr * (S * (np.float32(1.0) / np.float32(P)))
+    if with_momentum:
+        v_a = mu * v_a + t
+        w_a[root] = w_a[root] - v_a
+    else:
+        w_a[root] = w_a[root] - t
+    oracle.broadcast(w_a, root=root)
+    # (b) the oracle's Alg. 2 step
+    oracle.bsp_sgd_alg2_step(g_b, w_b, v_b, root=root, lr=float(lr), mu=float(mu))
+    for r in range(P):
+        assert w_b[r].tobytes() == w_a[r].tobytes()
+        assert g_b[r].tobytes() == g_a[r].tobytes()       # grads[root] = S, others untouched
+    assert g_b[root].tobytes() == oracle.chain_sum(grads).tobytes()
+    if with_momentum:
+        assert v_b.tobytes() == v_a.tobytes()
+    # (c) Alg. 3's fused step gives the same weights (the two differ in synchronisation points only)
+    w_c, v_c = _copy(weights), (vel.copy() if with_momentum else None)
+    if with_momentum:
+        oracle.bsp_sgd_momentum_step(grads, w_c, v_c, root=root, lr=float(lr), mu=float(mu))
+        assert v_c.tobytes() == v_b.tobytes()
+    else:
+        oracle.bsp_sgd_step(grads, w_c, root=root, lr=float(lr))
+    assert all(a.tobytes() == b.tobytes() for a, b in zip(w_c, w_b))
