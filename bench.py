@@ -386,6 +386,19 @@ def secondary(torch, lp, dev, pristine, work, P, n, block, peak):
                                           restore_fn=restore2)
     out["mst_allreduce_cfg2_P8"] = measure(lambda: lp.lp_mst_allreduce(g), mb(lp.OP_ALLREDUCE, P2, n2),
                                            restore_fn=restore2)
+    # momentum and Alg. 2 (reduce, root update, broadcast) against the fused Alg. 3
+    # step on the same configs[2] vectors; the Alg. 2 rows are quoted on the FUSED step's minimum bytes so that
+    # the rows compare (Alg. 2 itself moves (2P+4) n 4 bytes in three launches)
+    vel = torch.zeros(n2, device=dev)
+    out["lp_bsp_sgd_momentum_step_cfg2"] = measure(
+        lambda: lp.lp_bsp_sgd_momentum_step(g, w, vel, c2["block"], root=0, lr=c2["lr"], mu=0.9),
+        mb(lp.OP_BSP_SGD_MOM, P2, n2), restore_fn=restore2)
+    out["lp_bsp_sgd_alg2_step_cfg2"] = measure(
+        lambda: lp.lp_bsp_sgd_alg2_step(g, w, c2["block"], root=0, lr=c2["lr"]),
+        mb(lp.OP_BSP_SGD, P2, n2), restore_fn=restore2)
+    out["lp_bsp_sgd_alg2_momentum_step_cfg2"] = measure(
+        lambda: lp.lp_bsp_sgd_alg2_step(g, w, c2["block"], velocity=vel, root=0, lr=c2["lr"], mu=0.9),
+        mb(lp.OP_BSP_SGD_MOM, P2, n2), restore_fn=restore2)
     return out
 
 

@@ -65,6 +65,7 @@ extern "C" {
 #define LP_OP_REDUCE 1
 #define LP_OP_ALLREDUCE 2
 #define LP_OP_BSP_SGD 3
+#define LP_OP_BSP_SGD_MOM 4  /* Alg. 3 step with momentum; for lp_plan_query / lp_min_bytes */
 
 /* realisation of the LP pipeline used by lp_broadcast/lp_reduce/lp_allreduce/lp_bsp_sgd_step */
 #define LP_VARIANT_PIPELINE 0    /* default: one persistent kernel; per CTA a TMA-bulk shared-memory ring
@@ -115,6 +116,23 @@ LP_API int lp_allreduce(float *const *bufs, int P, size_t n, size_t block, void 
  * grads[] and weights[] are 2P distinct buffers. */
 LP_API int lp_bsp_sgd_step(float *const *grads, float *const *weights, int P, size_t n, size_t block, int root,
                     float lr, void *cuda_stream);
+
+/* Fused BSP-SGD step with momentum.  PAPER.md:216: "The solver is SGD + momentum" (no formula printed; reading
+ * U18 = the solver of the system the paper modifies, Caffe): per element, five separately rounded fp32 ops,
+ *   g = S * invP;  t = lr * g;  m = mu * velocity[i];  v' = m + t;  w' = weights[root][i] - v';
+ *   velocity[i] <- v';  weights[r][i] <- w' for every r.
+ * velocity is ONE device vector of n floats (16-byte aligned, distinct from the 2P others): it lives where the
+ * update is computed.  grads are only read.  mu = 0 with a zero velocity is lp_bsp_sgd_step. */
+LP_API int lp_bsp_sgd_momentum_step(float *const *grads, float *const *weights, float *velocity, int P, size_t n,
+                                    size_t block, int root, float lr, float mu, void *cuda_stream);
+
+/* BSP-SGD step the Alg. 2 way (reading U9; prose PAPER.md:178): lp_reduce of the sub-gradients to
+ * the root (grads[root] <- S, as lp_reduce does), GradientUpdate on weights[root] (the same rounded operations as
+ * the fused steps; with velocity != NULL the momentum form, else mu is ignored), lp_broadcast of weights from the
+ * root.  Three launches on the stream -- two synchronisation points where Alg. 3 has one.  The weights (and
+ * velocity) it leaves are bit-identical to lp_bsp_sgd_step / lp_bsp_sgd_momentum_step. */
+LP_API int lp_bsp_sgd_alg2_step(float *const *grads, float *const *weights, float *velocity, int P, size_t n,
+                                size_t block, int root, float lr, float mu, void *cuda_stream);
 
 /* ---- MST (binomial tree) and BE (recursive halving / doubling) baselines ------ */
 /* PAPER.md:93 (MST: "balanced tree of height ceil(log p)", whole-message steps) and
@@ -169,7 +187,7 @@ typedef struct lp_plan_info {
 LP_API int lp_plan_query(int op, int P, size_t n, size_t block, lp_plan_info *out);
 
 /* Minimum HBM bytes of one call (each input read once, each output written once):
- * broadcast P*n*4, reduce (P+1)*n*4, allreduce 2*P*n*4, bsp_sgd (2P+1)*n*4. */
+ * broadcast P*n*4, reduce (P+1)*n*4, allreduce 2*P*n*4, bsp_sgd (2P+1)*n*4, bsp_sgd with momentum (2P+3)*n*4. */
 LP_API uint64_t lp_min_bytes(int op, int P, size_t n);
 
 /* ---- control ------------------------------------------------------------------ */

@@ -14,7 +14,7 @@ from . import build as _build
 # enums of include/lp_collectives.h
 LP_OK, LP_ERR_INVALID_ARG, LP_ERR_UNSUPPORTED, LP_ERR_CUDA = 0, 1, 2, 3
 LP_MAX_P = 32
-OP_BROADCAST, OP_REDUCE, OP_ALLREDUCE, OP_BSP_SGD = 0, 1, 2, 3
+OP_BROADCAST, OP_REDUCE, OP_ALLREDUCE, OP_BSP_SGD, OP_BSP_SGD_MOM = 0, 1, 2, 3, 4
 VARIANT_PIPELINE, VARIANT_DIRECT, VARIANT_CLUSTER, VARIANT_COPY_ENGINE = 0, 1, 2, 3
 MODEL_STAGE, MODEL_LINK, MODEL_LINK_RING = 0, 1, 2
 TUNE_TILE_ELEMS, TUNE_STAGES, TUNE_OUT_STAGES, TUNE_CTAS_PER_SM, TUNE_CE_STREAMS, TUNE_L2_HINT, TUNE_STORE_WAIT, \
@@ -61,6 +61,8 @@ def lib() -> ctypes.CDLL:
     L.lp_reduce.argtypes = [pp, i32, sz, sz, i32, vp]
     L.lp_allreduce.argtypes = [pp, i32, sz, sz, vp]
     L.lp_bsp_sgd_step.argtypes = [pp, pp, i32, sz, sz, i32, f32, vp]
+    L.lp_bsp_sgd_momentum_step.argtypes = [pp, pp, vp, i32, sz, sz, i32, f32, f32, vp]
+    L.lp_bsp_sgd_alg2_step.argtypes = [pp, pp, vp, i32, sz, sz, i32, f32, f32, vp]
     for name in ("lp_mst_broadcast", "lp_mst_reduce", "lp_be_broadcast", "lp_be_reduce"):
         getattr(L, name).argtypes = [pp, i32, sz, i32, vp]
     for name in ("lp_mst_allreduce", "lp_be_allreduce"):
@@ -175,6 +177,36 @@ def lp_bsp_sgd_step(grads, weights, block, root=0, lr=0.01, stream=None):
         raise ValueError("grads and weights must match in P and n")
     _check(lib().lp_bsp_sgd_step(ga, wa, len(grads), n, block, root, ctypes.c_float(lr), _stream_ptr(stream)),
            "lp_bsp_sgd_step")
+
+
+def _velocity_ptr(velocity, n):
+    if velocity is None:
+        return None
+    import torch
+    if not (isinstance(velocity, torch.Tensor) and velocity.is_cuda and velocity.dtype == torch.float32
+            and velocity.is_contiguous() and velocity.numel() == n):
+        raise TypeError("velocity must be a contiguous CUDA float32 tensor of n elements")
+    return ctypes.c_void_p(velocity.data_ptr())
+
+
+def lp_bsp_sgd_momentum_step(grads, weights, velocity, block, root=0, lr=0.01, mu=0.9, stream=None):
+    ga, n = _dev_ptrs(grads)
+    wa, nw = _dev_ptrs(weights)
+    if n != nw or len(grads) != len(weights):
+        raise ValueError("grads and weights must match in P and n")
+    _check(lib().lp_bsp_sgd_momentum_step(ga, wa, _velocity_ptr(velocity, n), len(grads), n, block, root,
+                                          ctypes.c_float(lr), ctypes.c_float(mu), _stream_ptr(stream)),
+           "lp_bsp_sgd_momentum_step")
+
+
+def lp_bsp_sgd_alg2_step(grads, weights, block, velocity=None, root=0, lr=0.01, mu=0.0, stream=None):
+    ga, n = _dev_ptrs(grads)
+    wa, nw = _dev_ptrs(weights)
+    if n != nw or len(grads) != len(weights):
+        raise ValueError("grads and weights must match in P and n")
+    _check(lib().lp_bsp_sgd_alg2_step(ga, wa, _velocity_ptr(velocity, n), len(grads), n, block, root,
+                                      ctypes.c_float(lr), ctypes.c_float(mu), _stream_ptr(stream)),
+           "lp_bsp_sgd_alg2_step")
 
 
 # ---- MST / BE baselines --------------------------------------------------------------------------------

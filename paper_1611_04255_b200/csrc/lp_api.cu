@@ -11,8 +11,9 @@
 
 cudaError_t lp_mst_run(int op, float *const *bufs, int P, size_t n, int root, int sm_count, cudaStream_t stream);
 cudaError_t lp_be_run(int op, float *const *bufs, int P, size_t n, int root, int sm_count, cudaStream_t stream);
-cudaError_t lp_copy_engine_run(int op, float *const *bufs, float *const *weights, int P, size_t n, size_t block,
-                               int root, float lr, const LpTuning &t, int sm_count, cudaStream_t stream);
+cudaError_t lp_copy_engine_run(int op, float *const *bufs, float *const *weights, float *velocity, int P, size_t n,
+                               size_t block, int root, float lr, float mu, const LpTuning &t, int sm_count,
+                               cudaStream_t stream);
 void lp_copy_engine_shutdown();
 
 namespace {
@@ -73,23 +74,30 @@ int check_buffers(const float *const *ptrs, int count, size_t n) {
     return LP_OK;
 }
 
-int validate(int op, float *const *bufs, float *const *weights, int P, size_t n, size_t block, int root) {
+bool is_sgd(int op) { return op == LP_OP_BSP_SGD || op == LP_OP_BSP_SGD_MOM; }
+
+int validate(int op, float *const *bufs, float *const *weights, const float *velocity, int P, size_t n, size_t block,
+             int root) {
     if (P < 1 || P > LP_MAX_P || bufs == nullptr || block == 0) return LP_ERR_INVALID_ARG;
     if (root < 0 || root >= P) return LP_ERR_INVALID_ARG;
-    if (op == LP_OP_BSP_SGD && weights == nullptr) return LP_ERR_INVALID_ARG;
-    const float *all[2 * LP_MAX_P];
+    if (is_sgd(op) && weights == nullptr) return LP_ERR_INVALID_ARG;
+    if (op == LP_OP_BSP_SGD_MOM && velocity == nullptr) return LP_ERR_INVALID_ARG;
+    const float *all[2 * LP_MAX_P + 1];
     int m = 0;
     for (int r = 0; r < P; ++r) all[m++] = bufs[r];
-    if (op == LP_OP_BSP_SGD)
+    if (is_sgd(op))
         for (int r = 0; r < P; ++r) all[m++] = weights[r];
+    if (velocity) all[m++] = velocity;
     return check_buffers(all, m, n);
 }
 
 // The kernel argument block of one collective (which vectors are folded, in which order; where the finished
 // tile goes).  The fold order is ALWAYS rank 0 -> P-1 (U4); `root` only selects sources / destinations.
-void fill_args(LpArgs &a, int op, float *const *bufs, float *const *weights, int P, int root, float lr) {
+void fill_args(LpArgs &a, int op, float *const *bufs, float *const *weights, float *velocity, int P, int root, float lr,
+               float mu) {
     memset(&a, 0, sizeof(a));
     a.lr = lr;
+    a.mu = mu;
     a.invP = 1.0f / (float)P;  // one RN division on the host (U7)
     a.l2_hint = g_tuning.v[LP_TUNE_L2_HINT];
     a.store_wait = g_tuning.v[LP_TUNE_STORE_WAIT];
@@ -113,12 +121,17 @@ void fill_args(LpArgs &a, int op, float *const *bufs, float *const *weights, int
                 for (int r = 0; r < P; ++r) a.out[a.n_out++] = bufs[r];
             }
             break;
-        default:  // LP_OP_BSP_SGD
-            a.epilogue = LP_EPI_SGD;
+        default:  // LP_OP_BSP_SGD, LP_OP_BSP_SGD_MOM
+            a.epilogue = op == LP_OP_BSP_SGD_MOM ? LP_EPI_SGD_MOM : LP_EPI_SGD;
             a.n_sum = P;
             a.n_in = P + 1;
             for (int r = 0; r < P; ++r) a.in[r] = bufs[r];
             a.in[P] = weights[root];
+            if (op == LP_OP_BSP_SGD_MOM) {
+                a.in[P + 1] = velocity;  // read and rewritten in place, tile by tile
+                a.vel_out = velocity;
+                a.n_in = P + 2;
+            }
             for (int r = 0; r < P; ++r) a.out[a.n_out++] = weights[r];
             break;
     }
@@ -134,18 +147,19 @@ int effective_variant(int variant, size_t n, size_t block) {
 }
 
 // Plans (and unless dry_run, enqueues) one LP collective on device buffers.
-int plan_and_run(int op, float *const *bufs, float *const *weights, int P, size_t n, size_t block, int root, float lr,
-                 int sm_count, lp_plan_info *info, bool dry_run, cudaStream_t stream) {
+int plan_and_run(int op, float *const *bufs, float *const *weights, float *velocity, int P, size_t n, size_t block,
+                 int root, float lr, float mu, int sm_count, lp_plan_info *info, bool dry_run, cudaStream_t stream) {
     const int variant = effective_variant(g_variant, n, block);
     LpArgs a;
     LpLaunch cfg = {0, 0, 0, 0, 0};
     if (!dry_run)
-        fill_args(a, op, bufs, weights, P, root, lr);
+        fill_args(a, op, bufs, weights, velocity, P, root, lr, mu);
     else {
         memset(&a, 0, sizeof(a));
-        a.epilogue = op == LP_OP_BROADCAST ? LP_EPI_COPY : (op == LP_OP_BSP_SGD ? LP_EPI_SGD : LP_EPI_SUM);
+        a.epilogue = op == LP_OP_BROADCAST ? LP_EPI_COPY
+                     : (op == LP_OP_BSP_SGD ? LP_EPI_SGD : (op == LP_OP_BSP_SGD_MOM ? LP_EPI_SGD_MOM : LP_EPI_SUM));
         a.n_sum = op == LP_OP_BROADCAST ? 1 : P;
-        a.n_in = a.n_sum + (op == LP_OP_BSP_SGD ? 1 : 0);
+        a.n_in = a.n_sum + (op == LP_OP_BSP_SGD ? 1 : (op == LP_OP_BSP_SGD_MOM ? 2 : 0));
         a.n_out = op == LP_OP_BROADCAST ? P - 1 : (op == LP_OP_REDUCE ? 1 : P);
     }
     uint32_t tile;
@@ -160,11 +174,12 @@ int plan_and_run(int op, float *const *bufs, float *const *weights, int P, size_
         if (es != cudaSuccess) return cuda_fail(es, "tile-claim counters");
     }
     // identity collectives: nothing to move (P == 1 broadcast/reduce/allreduce; n == 0)
-    const bool noop = (n == 0) || (P == 1 && op != LP_OP_BSP_SGD);
+    const bool noop = (n == 0) || (P == 1 && !is_sgd(op));
     cudaError_t e = cudaSuccess;
     if (variant == LP_VARIANT_COPY_ENGINE) {
         cfg.grid = cfg.threads = 0;
-        if (!dry_run && !noop) e = lp_copy_engine_run(op, bufs, weights, P, n, block, root, lr, g_tuning, sm_count, stream);
+        if (!dry_run && !noop)
+            e = lp_copy_engine_run(op, bufs, weights, velocity, P, n, block, root, lr, mu, g_tuning, sm_count, stream);
     } else if (variant == LP_VARIANT_DIRECT) {
         e = lp_direct_launch(a, g_tuning, sm_count, &cfg, dry_run || noop, stream);
     } else if (variant == LP_VARIANT_CLUSTER) {
@@ -189,9 +204,9 @@ int plan_and_run(int op, float *const *bufs, float *const *weights, int P, size_
     return LP_OK;
 }
 
-int run_device(int op, float *const *bufs, float *const *weights, int P, size_t n, size_t block, int root, float lr,
-               void *cuda_stream) {
-    int rc = validate(op, bufs, weights, P, n, block, root);
+int run_device(int op, float *const *bufs, float *const *weights, float *velocity, int P, size_t n, size_t block, int root,
+               float lr, float mu, void *cuda_stream) {
+    int rc = validate(op, bufs, weights, velocity, P, n, block, root);
     if (rc != LP_OK) return rc;
     std::lock_guard<std::mutex> lock(g_mu);
     if (g_variant == LP_VARIANT_CLUSTER && P > 16) return LP_ERR_UNSUPPORTED;
@@ -200,11 +215,34 @@ int run_device(int op, float *const *bufs, float *const *weights, int P, size_t 
         snprintf(g_err, sizeof(g_err), "no CUDA device: liblp_b200 has no CPU fallback");
         return LP_ERR_CUDA;
     }
-    return plan_and_run(op, bufs, weights, P, n, block, root, lr, sms, nullptr, false, (cudaStream_t)cuda_stream);
+    return plan_and_run(op, bufs, weights, velocity, P, n, block, root, lr, mu, sms, nullptr, false,
+                        (cudaStream_t)cuda_stream);
+}
+
+// Alg. 2 (PAPER.md:140-168 as read in U9; prose PAPER.md:178): reduce the sub-gradients to the root, the root
+// applies GradientUpdate, the new weights are broadcast.  Three launches over the same virtual ranks -- the
+// two-synchronisation-point counterpart of the fused Alg. 3 step.
+int run_alg2(float *const *grads, float *const *weights, float *velocity, int P, size_t n, size_t block, int root, float lr,
+             float mu, void *cuda_stream) {
+    int rc = validate(velocity ? LP_OP_BSP_SGD_MOM : LP_OP_BSP_SGD, grads, weights, velocity, P, n, block, root);
+    if (rc != LP_OK) return rc;
+    std::lock_guard<std::mutex> lock(g_mu);
+    if (g_variant == LP_VARIANT_CLUSTER && P > 16) return LP_ERR_UNSUPPORTED;
+    const int sms = sm_count_or_fail();
+    if (sms <= 0) {
+        snprintf(g_err, sizeof(g_err), "no CUDA device: liblp_b200 has no CPU fallback");
+        return LP_ERR_CUDA;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    rc = plan_and_run(LP_OP_REDUCE, grads, nullptr, nullptr, P, n, block, root, 0.f, 0.f, sms, nullptr, false, st);
+    if (rc != LP_OK) return rc;
+    cudaError_t e = lp_update_launch(weights[root], grads[root], velocity, n, lr, 1.0f / (float)P, mu, st);
+    if (e != cudaSuccess) return cuda_fail(e, "Alg. 2 GradientUpdate");
+    return plan_and_run(LP_OP_BROADCAST, weights, nullptr, nullptr, P, n, block, root, 0.f, 0.f, sms, nullptr, false, st);
 }
 
 int run_baseline(bool be, int op, float *const *bufs, int P, size_t n, int root, void *cuda_stream) {
-    int rc = validate(op, bufs, nullptr, P, n, 1, root);
+    int rc = validate(op, bufs, nullptr, nullptr, P, n, 1, root);
     if (rc != LP_OK) return rc;
     if (be && (P & (P - 1)) != 0) return LP_ERR_UNSUPPORTED;  // U14
     std::lock_guard<std::mutex> lock(g_mu);
@@ -337,7 +375,7 @@ int run_host(int op, float *const *hbufs, float *const *hweights, int P, size_t 
         LP_TRYC(cudaEventRecord(g_ev_up[s], g_up), "host path");
         // LP kernel
         LP_TRYC(cudaStreamWaitEvent(g_mid, g_ev_up[s], 0), "host path");
-        rc = plan_and_run(op, dg, sgd ? dw : nullptr, P, len, block, root, lr, sms, nullptr, false, g_mid);
+        rc = plan_and_run(op, dg, sgd ? dw : nullptr, nullptr, P, len, block, root, lr, 0.f, sms, nullptr, false, g_mid);
         if (rc != LP_OK) return rc;
         LP_TRYC(cudaEventRecord(g_ev_done[s], g_mid), "host path");
         // download
@@ -360,17 +398,25 @@ int run_host(int op, float *const *hbufs, float *const *hweights, int P, size_t 
 extern "C" {
 
 int lp_broadcast(float *const *bufs, int P, size_t n, size_t block, int root, void *cuda_stream) {
-    return run_device(LP_OP_BROADCAST, bufs, nullptr, P, n, block, root, 0.f, cuda_stream);
+    return run_device(LP_OP_BROADCAST, bufs, nullptr, nullptr, P, n, block, root, 0.f, 0.f, cuda_stream);
 }
 int lp_reduce(float *const *bufs, int P, size_t n, size_t block, int root, void *cuda_stream) {
-    return run_device(LP_OP_REDUCE, bufs, nullptr, P, n, block, root, 0.f, cuda_stream);
+    return run_device(LP_OP_REDUCE, bufs, nullptr, nullptr, P, n, block, root, 0.f, 0.f, cuda_stream);
 }
 int lp_allreduce(float *const *bufs, int P, size_t n, size_t block, void *cuda_stream) {
-    return run_device(LP_OP_ALLREDUCE, bufs, nullptr, P, n, block, 0, 0.f, cuda_stream);
+    return run_device(LP_OP_ALLREDUCE, bufs, nullptr, nullptr, P, n, block, 0, 0.f, 0.f, cuda_stream);
 }
 int lp_bsp_sgd_step(float *const *grads, float *const *weights, int P, size_t n, size_t block, int root, float lr,
                     void *cuda_stream) {
-    return run_device(LP_OP_BSP_SGD, grads, weights, P, n, block, root, lr, cuda_stream);
+    return run_device(LP_OP_BSP_SGD, grads, weights, nullptr, P, n, block, root, lr, 0.f, cuda_stream);
+}
+int lp_bsp_sgd_momentum_step(float *const *grads, float *const *weights, float *velocity, int P, size_t n, size_t block,
+                             int root, float lr, float mu, void *cuda_stream) {
+    return run_device(LP_OP_BSP_SGD_MOM, grads, weights, velocity, P, n, block, root, lr, mu, cuda_stream);
+}
+int lp_bsp_sgd_alg2_step(float *const *grads, float *const *weights, float *velocity, int P, size_t n, size_t block,
+                         int root, float lr, float mu, void *cuda_stream) {
+    return run_alg2(grads, weights, velocity, P, n, block, root, lr, mu, cuda_stream);
 }
 
 int lp_mst_broadcast(float *const *bufs, int P, size_t n, int root, void *s) {
@@ -402,12 +448,12 @@ int lp_bsp_sgd_step_host(float *const *host_grads, float *const *host_weights, i
 
 int lp_plan_query(int op, int P, size_t n, size_t block, lp_plan_info *out) {
     if (out == nullptr || P < 1 || P > LP_MAX_P || block == 0) return LP_ERR_INVALID_ARG;
-    if (op < LP_OP_BROADCAST || op > LP_OP_BSP_SGD) return LP_ERR_INVALID_ARG;
+    if (op < LP_OP_BROADCAST || op > LP_OP_BSP_SGD_MOM) return LP_ERR_INVALID_ARG;
     std::lock_guard<std::mutex> lock(g_mu);
     int sms = sm_count_or_fail();
     if (sms <= 0) sms = 148;  // planning works without a device: a B200 has 148 SMs
     memset(out, 0, sizeof(*out));
-    return plan_and_run(op, nullptr, nullptr, P, n, block, 0, 0.f, sms, out, true, nullptr);
+    return plan_and_run(op, nullptr, nullptr, nullptr, P, n, block, 0, 0.f, 0.f, sms, out, true, nullptr);
 }
 
 uint64_t lp_min_bytes(int op, int P, size_t n) {
@@ -417,6 +463,7 @@ uint64_t lp_min_bytes(int op, int P, size_t n) {
         case LP_OP_REDUCE: return (uint64_t)(P + 1) * v;
         case LP_OP_ALLREDUCE: return 2u * (uint64_t)P * v;
         case LP_OP_BSP_SGD: return (2u * (uint64_t)P + 1u) * v;
+        case LP_OP_BSP_SGD_MOM: return (2u * (uint64_t)P + 3u) * v;
         default: return 0;
     }
 }

@@ -7,15 +7,17 @@
 #include "../../include/lp_collectives.h"
 #include "lp_schedule.h"
 
-#define LP_MAX_IN (LP_MAX_P + 1)  // P gradient vectors + the root's weight vector
+#define LP_MAX_IN (LP_MAX_P + 2)  // P gradient vectors + the root's weight vector + the velocity
 
 // Epilogues of the chain fold.
 #define LP_EPI_SUM 0   // out = ((in0 + in1) + ...) + in[n_sum-1]
 #define LP_EPI_SGD 1   // out = in[n_sum] - lr * (S * invP), three RN ops      PAPER.md:172,174 (U7)
 #define LP_EPI_COPY 2  // out = in0 (broadcast)
+#define LP_EPI_SGD_MOM 3  // v' = mu * in[n_sum+1] + lr * (S * invP); out = in[n_sum] - v'; vel_out = v'   PAPER.md:216 (U18)
 
 // One launch = one collective.  in[0..n_sum) are folded in that order (rank 0 -> P-1); for LP_EPI_SGD
-// in[n_sum] is weights[root]; out[0..n_out) all receive the finished tile.
+// in[n_sum] is weights[root]; for LP_EPI_SGD_MOM in[n_sum + 1] is the velocity as well and vel_out receives
+// the new velocity; out[0..n_out) all receive the finished tile.
 struct LpArgs {
     const float *in[LP_MAX_IN];
     float *out[LP_MAX_P];
@@ -23,7 +25,8 @@ struct LpArgs {
     int n_in;      // n_sum (+1 for SGD)
     int n_out;
     int epilogue;
-    float lr, invP;
+    float lr, invP, mu;
+    float *vel_out;
     int l2_hint;
     int store_wait;  // LP_TUNE_STORE_WAIT
     // Dynamic tile claims (LP_TUNE_SCHED 0): sched[0] = tiles claimed beyond the first grid-full, sched[1] = CTAs
@@ -62,6 +65,10 @@ struct LpSegJob {
 };
 #define LP_MAX_JOBS 32
 cudaError_t lp_seg_launch(const LpSegJob *jobs, int n_jobs, int sm_count, cudaStream_t stream);
+// Alg. 2's GradientUpdate on the root: w <- w - lr * (S * invP), or with velocity != NULL the
+// momentum form (U18), element-wise over n floats.
+cudaError_t lp_update_launch(float *w, const float *S, float *velocity, uint64_t n, float lr, float invP, float mu,
+                             cudaStream_t stream);
 
 // Launch counter (kernels + async copies enqueued by the library).
 void lp_count_launch(uint64_t k);
@@ -166,6 +173,19 @@ __device__ __forceinline__ float4 lp_add4(const float4 &a, const float4 &b) {
 __device__ __forceinline__ float lp_sgd1(float s, float w, float lr, float invP) {
     return __fsub_rn(w, __fmul_rn(lr, __fmul_rn(s, invP)));
 }
+// momentum (U18): g = s * invP; t = lr * g; m = mu * v; v' = m + t; w' = w - v' -- five separately rounded operations
+__device__ __forceinline__ void lp_mom1(float s, float w, float v, float lr, float invP, float mu, float &v_new,
+                                        float &w_new) {
+    v_new = __fadd_rn(__fmul_rn(mu, v), __fmul_rn(lr, __fmul_rn(s, invP)));
+    w_new = __fsub_rn(w, v_new);
+}
+__device__ __forceinline__ void lp_mom4(const float4 &s, const float4 &w, const float4 &v, float lr, float invP, float mu,
+                                        float4 &v_new, float4 &w_new) {
+    lp_mom1(s.x, w.x, v.x, lr, invP, mu, v_new.x, w_new.x);
+    lp_mom1(s.y, w.y, v.y, lr, invP, mu, v_new.y, w_new.y);
+    lp_mom1(s.z, w.z, v.z, lr, invP, mu, v_new.z, w_new.z);
+    lp_mom1(s.w, w.w, v.w, lr, invP, mu, v_new.w, w_new.w);
+}
 __device__ __forceinline__ float4 lp_sgd4(const float4 &s, const float4 &w, float lr, float invP) {
     return make_float4(lp_sgd1(s.x, w.x, lr, invP), lp_sgd1(s.y, w.y, lr, invP), lp_sgd1(s.z, w.z, lr, invP),
                        lp_sgd1(s.w, w.w, lr, invP));
@@ -204,6 +224,12 @@ __device__ __forceinline__ void lp_scalar_element(const LpArgs &a, uint64_t i) {
     float s = a.in[0][i];
     for (int r = 1; r < a.n_sum; ++r) s = __fadd_rn(s, a.in[r][i]);
     if (a.epilogue == LP_EPI_SGD) s = lp_sgd1(s, a.in[a.n_sum][i], a.lr, a.invP);
+    if (a.epilogue == LP_EPI_SGD_MOM) {
+        float v_new, w_new;
+        lp_mom1(s, a.in[a.n_sum][i], a.in[a.n_sum + 1][i], a.lr, a.invP, a.mu, v_new, w_new);
+        a.vel_out[i] = v_new;
+        s = w_new;
+    }
     for (int q = 0; q < a.n_out; ++q) a.out[q][i] = s;
 }
 #endif  // __CUDACC__

@@ -39,10 +39,20 @@ cudaError_t ensure_streams(int S) {
     return cudaSuccess;
 }
 
-// dst = w - lr * (s * invP), three RN ops (U7); element-wise, any alignment.
-__global__ void lp_ce_sgd_kernel(float *dst, const float *s, const float *w, uint64_t len, float lr, float invP) {
-    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < len; i += (uint64_t)gridDim.x * blockDim.x)
-        dst[i] = lp_sgd1(s[i], w[i], lr, invP);
+// dst = w - lr * (s * invP), three RN ops (U7), or with vel != NULL the momentum form (U18: vel updated in place);
+// element-wise, any alignment.
+__global__ void lp_ce_sgd_kernel(float *dst, const float *s, const float *w, float *vel, uint64_t len, float lr, float invP,
+                                 float mu) {
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < len; i += (uint64_t)gridDim.x * blockDim.x) {
+        if (vel) {
+            float vn, wn;
+            lp_mom1(s[i], w[i], vel[i], lr, invP, mu, vn, wn);
+            vel[i] = vn;
+            dst[i] = wn;
+        } else {
+            dst[i] = lp_sgd1(s[i], w[i], lr, invP);
+        }
+    }
 }
 
 cudaError_t copy_block(float *dst, const float *src, uint64_t len, cudaStream_t st) {
@@ -63,10 +73,12 @@ void lp_copy_engine_shutdown() {
 }
 
 // op: LP_OP_*.  For LP_OP_BSP_SGD `bufs` are the gradients and `weights` the replicas.
-cudaError_t lp_copy_engine_run(int op, float *const *bufs, float *const *weights, int P, size_t n, size_t block,
-                               int root, float lr, const LpTuning &t, int sm_count, cudaStream_t stream) {
+cudaError_t lp_copy_engine_run(int op, float *const *bufs, float *const *weights, float *velocity, int P, size_t n,
+                               size_t block, int root, float lr, float mu, const LpTuning &t, int sm_count,
+                               cudaStream_t stream) {
+    const bool sgd = (op == LP_OP_BSP_SGD || op == LP_OP_BSP_SGD_MOM);
     if (n == 0) return cudaSuccess;
-    if (P == 1 && op != LP_OP_BSP_SGD) return cudaSuccess;
+    if (P == 1 && !sgd) return cudaSuccess;
     int S = t.v[LP_TUNE_CE_STREAMS] ? t.v[LP_TUNE_CE_STREAMS] : 2;
     if (S > kMaxStreams) S = kMaxStreams;
     if (block > n) block = n;
@@ -110,7 +122,7 @@ cudaError_t lp_copy_engine_run(int op, float *const *bufs, float *const *weights
         if (op == LP_OP_ALLREDUCE) {
             // finished block flows back P-1 -> P-2 -> ... -> 0 ("a'' is broadcast"; U3-A)
             for (int r = P - 1; r > 0; --r) LP_TRY(copy_block(bufs[r - 1] + off, bufs[r] + off, len, st));
-        } else if (op == LP_OP_BSP_SGD) {
+        } else if (sgd) {
             // last rank: w' = w_root - lr * (S / P), then w' to every replica
             float *s_ptr;
             if (P == 1) {
@@ -122,7 +134,8 @@ cudaError_t lp_copy_engine_run(int op, float *const *bufs, float *const *weights
             unsigned grid = (unsigned)((len + 255) / 256);
             if (grid > (unsigned)sm_count * 8u) grid = (unsigned)sm_count * 8u;
             lp_count_launch(1);
-            lp_ce_sgd_kernel<<<grid, 256, 0, st>>>(weights[P - 1] + off, s_ptr, weights[root] + off, len, lr, invP);
+            lp_ce_sgd_kernel<<<grid, 256, 0, st>>>(weights[P - 1] + off, s_ptr, weights[root] + off,
+                                                   op == LP_OP_BSP_SGD_MOM ? velocity + off : nullptr, len, lr, invP, mu);
             LP_TRY(cudaGetLastError());
             for (int r = P - 1; r > 0; --r) LP_TRY(copy_block(weights[r - 1] + off, weights[r] + off, len, st));
         }

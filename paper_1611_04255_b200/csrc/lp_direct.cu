@@ -41,10 +41,16 @@ __global__ void __launch_bounds__(kThreads) lp_direct_kernel(const __grid_consta
         bool live[V];
 #pragma unroll
         for (int v = 0; v < V; ++v) live[v] = (uint32_t)(tid + v * kThreads) < nvec;
-        if (a.epilogue == LP_EPI_SGD) {
+        float4 vel[V];
+        if (a.epilogue == LP_EPI_SGD || a.epilogue == LP_EPI_SGD_MOM) {
 #pragma unroll
             for (int v = 0; v < V; ++v)
                 if (live[v]) w[v] = lp_ldg_stream(a.in[n_sum] + a0 + 4 * (uint64_t)(tid + v * kThreads));
+        }
+        if (a.epilogue == LP_EPI_SGD_MOM) {
+#pragma unroll
+            for (int v = 0; v < V; ++v)
+                if (live[v]) vel[v] = lp_ldg_stream(a.in[n_sum + 1] + a0 + 4 * (uint64_t)(tid + v * kThreads));
         }
         for (int r0 = 0; r0 < n_sum; r0 += kRankChunk) {
             float4 x[V][kRankChunk];
@@ -67,6 +73,13 @@ __global__ void __launch_bounds__(kThreads) lp_direct_kernel(const __grid_consta
         if (a.epilogue == LP_EPI_SGD) {
 #pragma unroll
             for (int v = 0; v < V; ++v) acc[v] = lp_sgd4(acc[v], w[v], a.lr, a.invP);
+        }
+        if (a.epilogue == LP_EPI_SGD_MOM) {  // v' to the velocity vector, w' goes on as the finished tile
+#pragma unroll
+            for (int v = 0; v < V; ++v) {
+                lp_mom4(acc[v], w[v], vel[v], a.lr, a.invP, a.mu, vel[v], acc[v]);
+                if (live[v]) lp_stg_stream(a.vel_out + a0 + 4 * (uint64_t)(tid + v * kThreads), vel[v]);
+            }
         }
         for (int q = 0; q < a.n_out; ++q) {
 #pragma unroll

@@ -43,6 +43,11 @@ __device__ __forceinline__ void wait_read_lag(int lag, bool complete) {
     }
 }
 
+// Tags of a store-ring slot (otile_of): the tile index, optionally marked as the momentum step's velocity tile;
+// kEndTag ends the store thread.
+constexpr uint64_t kVelocityTag = 1ull << 62;
+constexpr uint64_t kEndTag = ~0ull;
+
 struct Ring {
     int slot;
     uint32_t phase;
@@ -140,19 +145,25 @@ __global__ void __launch_bounds__((CW + 2) * 32) lp_pipeline_kernel(const __grid
             int free_slot = 0;  // oldest slot not yet handed back
             for (;;) {
                 lp_mbar_wait(&ofull[ring.slot], ring.phase);
-                const uint64_t t = otile_of[ring.slot];
-                if (t >= part.n_tiles) break;
+                const uint64_t tag = otile_of[ring.slot];
+                if (tag == kEndTag) break;
+                const bool to_velocity = (tag & kVelocityTag) != 0;  // momentum: the tile of new velocities
+                const uint64_t t = tag & ~kVelocityTag;
                 uint64_t off;
                 uint32_t len;
                 lp_tile_range(part, t, off, len);
                 const uint32_t bytes = (len & ~3u) * 4u;
                 if (bytes) {
                     const float *src = out_ring + (size_t)ring.slot * TILE;
-                    for (int q = 0; q < a.n_out; ++q) {
-                        if (hint)
-                            lp_bulk_s2g_hint(a.out[q] + off, src, bytes, pol);
-                        else
-                            lp_bulk_s2g(a.out[q] + off, src, bytes);
+                    if (to_velocity) {
+                        lp_bulk_s2g(a.vel_out + off, src, bytes);
+                    } else {
+                        for (int q = 0; q < a.n_out; ++q) {
+                            if (hint)
+                                lp_bulk_s2g_hint(a.out[q] + off, src, bytes, pol);
+                            else
+                                lp_bulk_s2g(a.out[q] + off, src, bytes);
+                        }
                     }
                 }
                 lp_bulk_commit();
@@ -176,7 +187,7 @@ __global__ void __launch_bounds__((CW + 2) * 32) lp_pipeline_kernel(const __grid
             const uint64_t t = tile_of[ring.slot];
             if (t >= part.n_tiles) {  // end marker: pass it on to the store thread
                 lp_mbar_wait(&oempty[oring.slot], oring.phase ^ 1u);
-                if (ctid == 0) otile_of[oring.slot] = t;
+                if (ctid == 0) otile_of[oring.slot] = kEndTag;
                 __syncwarp();
                 if (lane == 0) lp_mbar_arrive(&ofull[oring.slot]);
                 break;
@@ -213,6 +224,38 @@ __global__ void __launch_bounds__((CW + 2) * 32) lp_pipeline_kernel(const __grid
                 __syncwarp();
                 if (lane == 0) lp_mbar_arrive(&empty[ring.slot]);
                 ring.advance();
+            }
+            if (a.epilogue == LP_EPI_SGD_MOM) {  // v' = mu v + lr g, w' = w_root - v'  (U18)
+                float4 w[V];
+                lp_mbar_wait(&full[ring.slot], ring.phase);
+                {
+                    const float4 *s = reinterpret_cast<const float4 *>(in_ring + (size_t)ring.slot * TILE);
+#pragma unroll
+                    for (int v = 0; v < V; ++v) w[v] = s[ctid + v * CT];
+                }
+                __syncwarp();
+                if (lane == 0) lp_mbar_arrive(&empty[ring.slot]);
+                ring.advance();
+                lp_mbar_wait(&full[ring.slot], ring.phase);
+                float4 vel[V];
+                {
+                    const float4 *s = reinterpret_cast<const float4 *>(in_ring + (size_t)ring.slot * TILE);
+#pragma unroll
+                    for (int v = 0; v < V; ++v) lp_mom4(acc[v], w[v], s[ctid + v * CT], a.lr, a.invP, a.mu, vel[v], acc[v]);
+                }
+                __syncwarp();
+                if (lane == 0) lp_mbar_arrive(&empty[ring.slot]);
+                ring.advance();
+                // the tile of new velocities goes through the store ring first, tagged for its own destination
+                lp_mbar_wait(&oempty[oring.slot], oring.phase ^ 1u);
+                float4 *ov = reinterpret_cast<float4 *>(out_ring + (size_t)oring.slot * TILE);
+#pragma unroll
+                for (int v = 0; v < V; ++v) ov[ctid + v * CT] = vel[v];
+                if (ctid == 0) otile_of[oring.slot] = t | kVelocityTag;
+                lp_fence_proxy_async();
+                __syncwarp();
+                if (lane == 0) lp_mbar_arrive(&ofull[oring.slot]);
+                oring.advance();
             }
             // finished tile -> store ring
             lp_mbar_wait(&oempty[oring.slot], oring.phase ^ 1u);

@@ -60,7 +60,49 @@ __global__ void __launch_bounds__(kSegThreads) lp_seg_kernel(const __grid_consta
     }
 }
 
+// GradientUpdate of Alg. 2 on the root replica: one thread per 16-byte vector (hardware-scheduled CTAs), scalar
+// path for misaligned ends.  Same rounded operations as the fused epilogues (lp_sgd1 / lp_mom1).
+__global__ void __launch_bounds__(kSegThreads) lp_update_kernel(float *w, const float *S, float *vel, uint64_t n, float lr,
+                                                                float invP, float mu) {
+    const uint64_t nvec = n >> 2;
+    const uint64_t v = (uint64_t)blockIdx.x * kSegThreads + threadIdx.x;
+    if (v < nvec) {
+        const float4 s4 = lp_ldg_stream(S + 4 * v);
+        const float4 w4 = lp_ldg_stream(w + 4 * v);
+        if (vel) {
+            const float4 v4 = lp_ldg_stream(vel + 4 * v);
+            float4 vn, wn;
+            lp_mom4(s4, w4, v4, lr, invP, mu, vn, wn);
+            lp_stg_stream(vel + 4 * v, vn);
+            lp_stg_stream(w + 4 * v, wn);
+        } else {
+            lp_stg_stream(w + 4 * v, lp_sgd4(s4, w4, lr, invP));
+        }
+    }
+    if (blockIdx.x == 0 && threadIdx.x < (n & 3u)) {
+        const uint64_t i = (nvec << 2) + threadIdx.x;
+        if (vel) {
+            float vn, wn;
+            lp_mom1(S[i], w[i], vel[i], lr, invP, mu, vn, wn);
+            vel[i] = vn;
+            w[i] = wn;
+        } else {
+            w[i] = lp_sgd1(S[i], w[i], lr, invP);
+        }
+    }
+}
+
 }  // namespace
+
+cudaError_t lp_update_launch(float *w, const float *S, float *velocity, uint64_t n, float lr, float invP, float mu,
+                             cudaStream_t stream) {
+    if (n == 0) return cudaSuccess;
+    const uint64_t blocks = ((n >> 2) + kSegThreads - 1) / kSegThreads + ((n >> 2) == 0 ? 1 : 0);
+    if (blocks > 0x7fffffffull) return cudaErrorInvalidValue;
+    lp_count_launch(1);
+    lp_update_kernel<<<(unsigned)blocks, kSegThreads, 0, stream>>>(w, S, velocity, n, lr, invP, mu);
+    return cudaGetLastError();
+}
 
 cudaError_t lp_seg_launch(const LpSegJob *jobs, int n_jobs, int sm_count, cudaStream_t stream) {
     LpSegArgs s;

@@ -275,6 +275,78 @@ def test_config2_sgd_100_iterations(oracle):
 
 
 # ---------------------------------------------------------------------------------------------------
+# SGD + momentum (U18) and the Alg. 2 step (U9)  -- SURVEY 8(f)-1
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("P,n,block,root", [(1, 1000, 256, 0), (2, 4099, 1024, 1), (6, 70_001, 1001, 2),
+                                            (8, 150_003, 16_384, 0), (16, 33_333, 4096, 15)])
+def test_momentum_step_bit_exact(oracle, variant, P, n, block, root):
+    lp.lp_set_variant(variant)
+    grads, weights = inputs.sgd_inputs([6, n], P, n)
+    weights[root] += np.float32(0.125)
+    vel = inputs.normal([6, n], 99, n, 0.01)
+    hg, hw, hv = copies(grads), copies(weights), vel.copy()
+    dg, dw, dv = up(grads), up(weights), torch.from_numpy(vel).cuda()
+    for it in range(4):
+        oracle.bsp_sgd_momentum_step(hg, hw, hv, root=root, lr=0.01, mu=0.9)
+        lp.lp_bsp_sgd_momentum_step(dg, dw, dv, block, root=root, lr=0.01, mu=0.9)
+        gw = down(dw)
+        for r in range(P):
+            assert same(gw[r], hw[r]), (it, r)
+        assert same(dv.cpu().numpy(), hv), it
+    assert all(same(g, s) for g, s in zip(down(dg), grads))  # grads only read
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("with_momentum", [False, True])
+@pytest.mark.parametrize("P,n,block,root", [(1, 1000, 256, 0), (3, 4099, 1024, 1), (6, 70_003, 1001, 5),
+                                            (8, 150_001, 16_384, 2)])
+def test_alg2_step_bit_exact_and_equals_alg3(oracle, variant, with_momentum, P, n, block, root):
+    lp.lp_set_variant(variant)
+    grads, weights = inputs.sgd_inputs([7, n], P, n)
+    weights[root] += np.float32(0.25)
+    vel = inputs.normal([7, n], 99, n, 0.01) if with_momentum else None
+    hg, hw, hv = copies(grads), copies(weights), (vel.copy() if with_momentum else None)
+    dg, dw = up(grads), up(weights)
+    dv = torch.from_numpy(vel).cuda() if with_momentum else None
+    oracle.bsp_sgd_alg2_step(hg, hw, hv, root=root, lr=0.02, mu=0.9)
+    lp.lp_bsp_sgd_alg2_step(dg, dw, block, velocity=dv, root=root, lr=0.02, mu=0.9)
+    gw, gg = down(dw), down(dg)
+    for r in range(P):
+        assert same(gw[r], hw[r]), ("w", r)
+        assert same(gg[r], hg[r]), ("g", r)  # grads[root] = S, the others untouched
+    if with_momentum:
+        assert same(dv.cpu().numpy(), hv)
+    # the fused Alg. 3 step on the same inputs leaves the same weights (and velocity)
+    dg3, dw3 = up(grads), up(weights)
+    if with_momentum:
+        dv3 = torch.from_numpy(vel).cuda()
+        lp.lp_bsp_sgd_momentum_step(dg3, dw3, dv3, block, root=root, lr=0.02, mu=0.9)
+        assert same(dv3.cpu().numpy(), hv)
+    else:
+        lp.lp_bsp_sgd_step(dg3, dw3, block, root=root, lr=0.02)
+    assert all(same(a, b) for a, b in zip(down(dw3), hw))
+
+
+def test_config2_momentum_20_iterations_all_tiles(oracle):
+    # configs[2]'s vectors (P=8, n=7,000,000) through the momentum step, every tile size of the pipeline
+    c = inputs.CONFIGS[2]
+    P, n = c["P"], c["n"]
+    grads, weights = inputs.sgd_inputs(2, P, n, c["sigma"], c["w_sigma"])
+    hw, hv = copies(weights), np.zeros(n, np.float32)
+    dg, dw, dv = up(grads), up(weights), torch.zeros(n, device="cuda")
+    tiles = (0, 1024, 2048, 4096, 8192)
+    for it in range(1, 21):
+        lp.lp_set_tuning(lp.TUNE_TILE_ELEMS, tiles[it % len(tiles)])
+        oracle.bsp_sgd_momentum_step(grads, hw, hv, root=it % P, lr=c["lr"], mu=0.9)
+        lp.lp_bsp_sgd_momentum_step(dg, dw, dv, c["block"], root=it % P, lr=c["lr"], mu=0.9)
+        if it in (1, 2, 5, 20):
+            gw = down(dw)
+            assert all(same(gw[r], hw[r]) for r in range(P)), it
+            assert same(dv.cpu().numpy(), hv), it
+
+
+# ---------------------------------------------------------------------------------------------------
 # MST / BE baselines (a7, a8)
 # ---------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("P,n", [(2, 1001), (3, 70_001), (4, 65_536), (5, 4099), (6, 300_003), (8, 100_001),

@@ -91,6 +91,7 @@ def test_min_bytes():
     assert lp.lp_min_bytes(REDUCE, 4, n) == 5 * n * 4
     assert lp.lp_min_bytes(ALLREDUCE, 6, n) == 2 * 6 * n * 4
     assert lp.lp_min_bytes(SGD, 8, n) == 17 * n * 4
+    assert lp.lp_min_bytes(lp.OP_BSP_SGD_MOM, 8, n) == 19 * n * 4
 
 
 @pytest.mark.parametrize("variant", [lp.VARIANT_PIPELINE, lp.VARIANT_DIRECT])
