@@ -62,6 +62,7 @@ def lib() -> ctypes.CDLL:
             getattr(L, name).argtypes = [pp, pp, i32, sz, i32, f32]
         for name in ("lpo_bsp_sgd_momentum_step", "lpo_bsp_sgd_alg2_step"):
             getattr(L, name).argtypes = [pp, pp, ctypes.c_void_p, i32, sz, i32, f32, f32]
+        L.lpo_collective_segments.argtypes = [i32, pp, i32, sz, ctypes.POINTER(sz), ctypes.POINTER(sz), i32, i32]
         L.lpo_lp_blocked.argtypes = [pp, i32, sz, sz, i32, i32, pu64]
         L.lpo_num_blocks.argtypes = [sz, sz]
         L.lpo_num_blocks.restype = u64
@@ -158,6 +159,15 @@ def bsp_sgd_alg2_step(grads, weights, velocity=None, root=0, lr=0.01, mu=0.0):
         raise ValueError("grads and weights must match in P and n")
     _check(lib().lpo_bsp_sgd_alg2_step(ga, wa, _velocity_ptr(velocity, n), len(grads), n, root,
                                        ctypes.c_float(lr), ctypes.c_float(mu)), "lpo_bsp_sgd_alg2_step")
+
+
+def collective_segments(op, bufs, segments, root=0):
+    """Layer-wise collective (Alg. 1): `op` (0 broadcast, 1 reduce, 2 allreduce) on every (offset, length) slice."""
+    arr, n = _ptrs(bufs)
+    k = len(segments)
+    off = (ctypes.c_size_t * max(k, 1))(*[int(o) for o, _ in segments])
+    ln = (ctypes.c_size_t * max(k, 1))(*[int(l) for _, l in segments])
+    _check(lib().lpo_collective_segments(op, arr, len(bufs), n, off, ln, k, root), "lpo_collective_segments")
 
 
 def lp_blocked(bufs, block, op, root=0) -> int:

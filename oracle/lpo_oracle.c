@@ -214,6 +214,44 @@ int lpo_bsp_sgd_alg2_step(float *const *grads, float *const *weights,
     return lpo_broadcast(weights, P, n, root);              /* step 3 */
 }
 
+/* Layer-wise collectives.  Alg. 1 (prose
+ * PAPER.md:182): "GPUs broadcast network parameters of layer t+1 amid forward
+ * computations at layer t ... all-reduce or reduce sub-gradients of layer t+1
+ * amidst backward computations at layer t": one collective PER LAYER, i.e. per
+ * slice [seg_off[s], seg_off[s] + seg_len[s]) of the flat rank vectors.  The
+ * definition is just that: the whole-message definition above applied to each
+ * slice in list order; elements outside every slice are not touched.
+ * op: 0 broadcast, 1 reduce, 2 allreduce.  Slices must lie inside [0, n). */
+int lpo_collective_segments(int op, float *const *bufs, int P, size_t n,
+                            const size_t *seg_off, const size_t *seg_len,
+                            int n_seg, int root)
+{
+    if (bad_args(bufs, P, root) || n_seg < 0 || (n_seg > 0 && (!seg_off || !seg_len)))
+        return LPO_EINVAL;
+    if (P > 64)
+        return LPO_EINVAL;
+    for (int s = 0; s < n_seg; ++s)
+        if (seg_off[s] > n || seg_len[s] > n - seg_off[s])
+            return LPO_EINVAL;
+    for (int s = 0; s < n_seg; ++s) {
+        float *slice[64];
+        for (int r = 0; r < P; ++r)
+            slice[r] = bufs[r] + seg_off[s];
+        int rc;
+        if (op == 0)
+            rc = lpo_broadcast(slice, P, seg_len[s], root);
+        else if (op == 1)
+            rc = lpo_reduce(slice, P, seg_len[s], root);
+        else if (op == 2)
+            rc = lpo_allreduce(slice, P, seg_len[s]);
+        else
+            rc = LPO_EINVAL;
+        if (rc != LPO_OK)
+            return rc;
+    }
+    return LPO_OK;
+}
+
 /* The same two definitions with the element loop spread over host threads.
  * Element i never depends on element j != i, so the bits are those of the
  * serial loops above (tests assert it).  These are the versions bench.py times

@@ -203,3 +203,42 @@ def test_omp_versions_bit_identical(oracle):
     oracle.bsp_sgd_step(g, w, root=2, lr=0.01)
     oracle.bsp_sgd_step(g, w2, root=2, lr=0.01, omp=True)
     assert all(x.tobytes() == y.tobytes() for x, y in zip(w, w2))
+
+
+# ----------------------------------------------------------------------------
+# layer-wise collectives (Alg. 1): one collective per slice
+# ----------------------------------------------------------------------------
+
+@pytest.mark.parametrize("op", [BCAST, REDUCE, ALLREDUCE])
+def test_segments_equal_whole_message_on_their_union(oracle, op):
+    # element-wise ops: a collective per slice touches exactly the slices' elements and gives them the values
+    # the whole-message collective gives; everything else keeps its bytes.  Slices unordered, ragged, some empty.
+    P, n, root = 5, 10_007, 3
+    segs = [(9000, 1007), (0, 1), (5, 3), (100, 0), (4096, 2048), (1001, 999), (8999, 1)]
+    src = inputs.rank_vectors(81, P, n, "uniform")
+    whole = _copy(src)
+    {BCAST: oracle.broadcast, REDUCE: oracle.reduce}.get(op, None)(whole, root=root) if op != ALLREDUCE \
+        else oracle.allreduce(whole)
+    got = _copy(src)
+    oracle.collective_segments(op, got, segs, root=root)
+    mask = np.zeros(n, bool)
+    for o, l in segs:
+        mask[o:o + l] = True
+    for r in range(P):
+        assert got[r][mask].tobytes() == whole[r][mask].tobytes()
+        assert got[r][~mask].tobytes() == src[r][~mask].tobytes()
+
+
+def test_segments_brute_force_small_integers(oracle):
+    P, n = 4, 64
+    src = [inputs.small_integers(82, r, n) for r in range(P)]
+    segs = [(60, 4), (0, 7), (31, 2)]
+    got = _copy(src)
+    oracle.collective_segments(ALLREDUCE, got, segs)
+    total = np.sum(np.stack(src).astype(np.int64), axis=0)
+    for r in range(P):
+        for i in range(n):
+            inside = any(o <= i < o + l for o, l in segs)
+            assert got[r][i] == (total[i] if inside else src[r][i])
+    with pytest.raises(RuntimeError):
+        oracle.collective_segments(ALLREDUCE, got, [(60, 5)])      # runs past n
