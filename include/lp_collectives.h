@@ -134,6 +134,26 @@ LP_API int lp_bsp_sgd_momentum_step(float *const *grads, float *const *weights, 
 LP_API int lp_bsp_sgd_alg2_step(float *const *grads, float *const *weights, float *velocity, int P, size_t n,
                                 size_t block, int root, float lr, float mu, void *cuda_stream);
 
+/* ---- layer-wise collectives (Alg. 1) ------------------------------------------ */
+/* Alg. 1 (prose PAPER.md:182) issues one collective PER LAYER: "GPUs broadcast network parameters
+ * of layer t+1 amid forward computations at layer t ... all-reduce or reduce sub-gradients of layer t+1 amidst
+ * backward computations at layer t".  These calls run the collective on a LIST of slices of the rank vectors in
+ * one launch: slice s is elements [seg_off[s], seg_off[s] + seg_len[s]) of every bufs[r] (r's copy of layer s).
+ * Every slice is its own LP message (cut into its own blocks of `block` elements, a1), the slices are worked on in
+ * list order (earlier slices finish first), elements outside every slice are not touched.  Results per slice are
+ * those of lp_broadcast / lp_reduce / lp_allreduce on that slice (bit-exact, chain order).
+ * seg_off / seg_len are HOST arrays of n_seg entries, read during the call; slices may start at any element
+ * (no alignment rule), may be empty, must lie inside [0, n) and must not overlap (else LP_ERR_INVALID_ARG);
+ * 0 <= n_seg <= LP_MAX_SEGMENTS; lists longer than 96 slices take one launch per 96.  Not available in the
+ * cluster variant (LP_ERR_UNSUPPORTED). */
+#define LP_MAX_SEGMENTS 65536
+LP_API int lp_broadcast_segments(float *const *bufs, int P, size_t n, const size_t *seg_off, const size_t *seg_len,
+                                 int n_seg, size_t block, int root, void *cuda_stream);
+LP_API int lp_reduce_segments(float *const *bufs, int P, size_t n, const size_t *seg_off, const size_t *seg_len,
+                              int n_seg, size_t block, int root, void *cuda_stream);
+LP_API int lp_allreduce_segments(float *const *bufs, int P, size_t n, const size_t *seg_off, const size_t *seg_len,
+                                 int n_seg, size_t block, void *cuda_stream);
+
 /* ---- MST (binomial tree) and BE (recursive halving / doubling) baselines ------ */
 /* PAPER.md:93 (MST: "balanced tree of height ceil(log p)", whole-message steps) and
  * PAPER.md:95 (BE: broadcast = MST scatter + BE allgather, reduce = reduce-scatter + gather, allreduce =
@@ -180,8 +200,7 @@ typedef struct lp_plan_info {
     uint32_t smem_bytes;      /* dynamic shared memory per CTA */
     uint32_t stages;          /* load-ring depth */
     uint32_t out_stages;      /* store-ring depth */
-    uint32_t variant;         /* variant that will actually run (PIPELINE falls back to DIRECT when
-                                 block % 4 != 0 and nb > 1) */
+    uint32_t variant;         /* variant that will run */
     uint32_t sm_count;        /* SMs assumed (device query, 148 when no device) */
 } lp_plan_info;
 LP_API int lp_plan_query(int op, int P, size_t n, size_t block, lp_plan_info *out);

@@ -61,6 +61,10 @@ def lib() -> ctypes.CDLL:
     L.lp_reduce.argtypes = [pp, i32, sz, sz, i32, vp]
     L.lp_allreduce.argtypes = [pp, i32, sz, sz, vp]
     L.lp_bsp_sgd_step.argtypes = [pp, pp, i32, sz, sz, i32, f32, vp]
+    psz = ctypes.POINTER(sz)
+    L.lp_broadcast_segments.argtypes = [pp, i32, sz, psz, psz, i32, sz, i32, vp]
+    L.lp_reduce_segments.argtypes = [pp, i32, sz, psz, psz, i32, sz, i32, vp]
+    L.lp_allreduce_segments.argtypes = [pp, i32, sz, psz, psz, i32, sz, vp]
     L.lp_bsp_sgd_momentum_step.argtypes = [pp, pp, vp, i32, sz, sz, i32, f32, f32, vp]
     L.lp_bsp_sgd_alg2_step.argtypes = [pp, pp, vp, i32, sz, sz, i32, f32, f32, vp]
     for name in ("lp_mst_broadcast", "lp_mst_reduce", "lp_be_broadcast", "lp_be_reduce"):
@@ -177,6 +181,41 @@ def lp_bsp_sgd_step(grads, weights, block, root=0, lr=0.01, stream=None):
         raise ValueError("grads and weights must match in P and n")
     _check(lib().lp_bsp_sgd_step(ga, wa, len(grads), n, block, root, ctypes.c_float(lr), _stream_ptr(stream)),
            "lp_bsp_sgd_step")
+
+
+# ---- layer-wise collectives (Alg. 1): one LP message per (offset, length) slice, one launch --------------
+class Segments:
+    """A list of (offset, length) slices marshalled once into the two host arrays the C ABI takes."""
+
+    def __init__(self, segments):
+        self.k = len(segments)
+        self.off = (ctypes.c_size_t * max(self.k, 1))(*[int(o) for o, _ in segments])
+        self.len = (ctypes.c_size_t * max(self.k, 1))(*[int(l) for _, l in segments])
+
+
+def _segments(segments):
+    return segments if isinstance(segments, Segments) else Segments(segments)
+
+
+def lp_broadcast_segments(bufs, segments, block, root=0, stream=None):
+    arr, n = _dev_ptrs(bufs)
+    sg = _segments(segments)
+    _check(lib().lp_broadcast_segments(arr, len(bufs), n, sg.off, sg.len, sg.k, block, root, _stream_ptr(stream)),
+           "lp_broadcast_segments")
+
+
+def lp_reduce_segments(bufs, segments, block, root=0, stream=None):
+    arr, n = _dev_ptrs(bufs)
+    sg = _segments(segments)
+    _check(lib().lp_reduce_segments(arr, len(bufs), n, sg.off, sg.len, sg.k, block, root, _stream_ptr(stream)),
+           "lp_reduce_segments")
+
+
+def lp_allreduce_segments(bufs, segments, block, stream=None):
+    arr, n = _dev_ptrs(bufs)
+    sg = _segments(segments)
+    _check(lib().lp_allreduce_segments(arr, len(bufs), n, sg.off, sg.len, sg.k, block, _stream_ptr(stream)),
+           "lp_allreduce_segments")
 
 
 def _velocity_ptr(velocity, n):

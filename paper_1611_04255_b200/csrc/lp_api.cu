@@ -4,8 +4,11 @@
 #include <stdio.h>
 #include <string.h>
 
+#include <algorithm>
 #include <atomic>
 #include <mutex>
+#include <utility>
+#include <vector>
 
 #include "lp_common.cuh"
 
@@ -137,19 +140,20 @@ void fill_args(LpArgs &a, int op, float *const *bufs, float *const *weights, flo
     }
 }
 
-// Variant that will really run: the TMA pipeline needs every tile to start on a 16-byte boundary.
-int effective_variant(int variant, size_t n, size_t block) {
-    if (variant == LP_VARIANT_PIPELINE || variant == LP_VARIANT_CLUSTER) {
-        const uint64_t nb = lp_num_blocks(n, block);
-        if (nb > 1 && (block % 4) != 0) return LP_VARIANT_DIRECT;
-    }
-    return variant;
-}
+// A list of slices of the rank vectors, each its own LP message (layer-wise collectives, Alg. 1); n == 0: the
+// whole vector is the one message.
+struct SegList {
+    const size_t *off;
+    const size_t *len;
+    int n;  // <= LP_MAX_SEGS, every len > 0
+};
 
 // Plans (and unless dry_run, enqueues) one LP collective on device buffers.
 int plan_and_run(int op, float *const *bufs, float *const *weights, float *velocity, int P, size_t n, size_t block,
-                 int root, float lr, float mu, int sm_count, lp_plan_info *info, bool dry_run, cudaStream_t stream) {
-    const int variant = effective_variant(g_variant, n, block);
+                 int root, float lr, float mu, int sm_count, lp_plan_info *info, bool dry_run, cudaStream_t stream,
+                 const SegList *segl = nullptr) {
+    const int variant = g_variant;
+    const bool layered = segl != nullptr && segl->n > 0;
     LpArgs a;
     LpLaunch cfg = {0, 0, 0, 0, 0};
     if (!dry_run)
@@ -162,31 +166,64 @@ int plan_and_run(int op, float *const *bufs, float *const *weights, float *veloc
         a.n_in = a.n_sum + (op == LP_OP_BSP_SGD ? 1 : (op == LP_OP_BSP_SGD_MOM ? 2 : 0));
         a.n_out = op == LP_OP_BROADCAST ? P - 1 : (op == LP_OP_REDUCE ? 1 : P);
     }
+    size_t n_work = n;  // elements the launch touches per rank
+    if (layered) {
+        n_work = 0;
+        for (int s = 0; s < segl->n; ++s) n_work += segl->len[s];
+    }
     uint32_t tile;
     switch (variant) {
         case LP_VARIANT_DIRECT: tile = lp_direct_tile(g_tuning, a.n_in); break;
         case LP_VARIANT_CLUSTER: tile = lp_cluster_tile(g_tuning); break;
-        default: tile = lp_pipeline_tile(g_tuning, a, n, block); break;
+        default: tile = lp_pipeline_tile(g_tuning, a, n_work, block); break;
     }
-    a.part = lp_make_partition(n, block, tile);
+    a.part = lp_make_partition(n_work, block, tile);
+    lp_seg_table table;
+    if (layered) {  // a1 per slice; tiles numbered slice by slice
+        table.n_seg = (uint32_t)segl->n;
+        uint64_t tiles = 0, blocks = 0;
+        for (int s = 0; s < segl->n; ++s) {
+            const lp_partition ps = lp_make_partition(segl->len[s], block, tile);
+            table.off[s] = segl->off[s];
+            table.len[s] = segl->len[s];
+            table.tile_start[s] = tiles;
+            tiles += ps.n_tiles;
+            blocks += ps.nb;
+        }
+        table.tile_start[segl->n] = tiles;
+        a.part.block = block;  // per-slice partitions are rebuilt from (block, tile) in the kernel
+        a.part.nb = blocks;
+        a.part.n_tiles = tiles;
+    }
     if (!dry_run && g_tuning.v[LP_TUNE_SCHED] == 0 && variant != LP_VARIANT_COPY_ENGINE && a.part.n_tiles > 0) {
         cudaError_t es = lp_sched_acquire(&a.sched);
         if (es != cudaSuccess) return cuda_fail(es, "tile-claim counters");
     }
     // identity collectives: nothing to move (P == 1 broadcast/reduce/allreduce; n == 0)
-    const bool noop = (n == 0) || (P == 1 && !is_sgd(op));
+    const bool noop = (n_work == 0) || (P == 1 && !is_sgd(op));
+    const lp_seg_table *tp = layered ? &table : nullptr;
     cudaError_t e = cudaSuccess;
     if (variant == LP_VARIANT_COPY_ENGINE) {
         cfg.grid = cfg.threads = 0;
-        if (!dry_run && !noop)
-            e = lp_copy_engine_run(op, bufs, weights, velocity, P, n, block, root, lr, mu, g_tuning, sm_count, stream);
+        if (!dry_run && !noop) {
+            if (!layered) {
+                e = lp_copy_engine_run(op, bufs, weights, velocity, P, n, block, root, lr, mu, g_tuning, sm_count, stream);
+            } else {  // one chain of copies + adds per slice
+                for (int s = 0; s < segl->n && e == cudaSuccess; ++s) {
+                    float *sb[LP_MAX_P];
+                    for (int r = 0; r < P; ++r) sb[r] = bufs[r] + segl->off[s];
+                    e = lp_copy_engine_run(op, sb, nullptr, nullptr, P, segl->len[s], block, root, lr, mu, g_tuning,
+                                           sm_count, stream);
+                }
+            }
+        }
     } else if (variant == LP_VARIANT_DIRECT) {
-        e = lp_direct_launch(a, g_tuning, sm_count, &cfg, dry_run || noop, stream);
+        e = lp_direct_launch(a, tp, g_tuning, sm_count, &cfg, dry_run || noop, stream);
     } else if (variant == LP_VARIANT_CLUSTER) {
         e = lp_cluster_launch(a, g_tuning, sm_count, &cfg, dry_run || noop, stream);
         if (e == cudaErrorNotSupported) return LP_ERR_UNSUPPORTED;
     } else {
-        e = lp_pipeline_launch(a, g_tuning, sm_count, &cfg, dry_run || noop, stream);
+        e = lp_pipeline_launch(a, tp, g_tuning, sm_count, &cfg, dry_run || noop, stream);
     }
     if (info) {
         info->nb = a.part.nb;
@@ -239,6 +276,50 @@ int run_alg2(float *const *grads, float *const *weights, float *velocity, int P,
     cudaError_t e = lp_update_launch(weights[root], grads[root], velocity, n, lr, 1.0f / (float)P, mu, st);
     if (e != cudaSuccess) return cuda_fail(e, "Alg. 2 GradientUpdate");
     return plan_and_run(LP_OP_BROADCAST, weights, nullptr, nullptr, P, n, block, root, 0.f, 0.f, sms, nullptr, false, st);
+}
+
+// Layer-wise collective (Alg. 1): `op` on every slice [seg_off[s], seg_off[s] + seg_len[s]) of the rank vectors,
+// each slice its own LP message, tiles handed out slice by slice in list order; LP_MAX_SEGS slices per launch.
+int run_segments(int op, float *const *bufs, int P, size_t n, const size_t *seg_off, const size_t *seg_len, int n_seg,
+                 size_t block, int root, void *cuda_stream) {
+    int rc = validate(op, bufs, nullptr, nullptr, P, n, block, root);
+    if (rc != LP_OK) return rc;
+    if (n_seg < 0 || n_seg > LP_MAX_SEGMENTS || (n_seg > 0 && (seg_off == nullptr || seg_len == nullptr)))
+        return LP_ERR_INVALID_ARG;
+    // slices inside [0, n) and pairwise disjoint (an in-place allreduce of overlapping slices would sum twice)
+    std::vector<std::pair<size_t, size_t>> sorted;
+    sorted.reserve((size_t)n_seg);
+    for (int s = 0; s < n_seg; ++s) {
+        if (seg_off[s] > n || seg_len[s] > n - seg_off[s]) return LP_ERR_INVALID_ARG;
+        if (seg_len[s]) sorted.emplace_back(seg_off[s], seg_len[s]);
+    }
+    std::sort(sorted.begin(), sorted.end());
+    for (size_t i = 1; i < sorted.size(); ++i)
+        if (sorted[i - 1].first + sorted[i - 1].second > sorted[i].first) return LP_ERR_INVALID_ARG;
+    std::lock_guard<std::mutex> lock(g_mu);
+    if (g_variant == LP_VARIANT_CLUSTER) return LP_ERR_UNSUPPORTED;
+    const int sms = sm_count_or_fail();
+    if (sms <= 0) {
+        snprintf(g_err, sizeof(g_err), "no CUDA device: liblp_b200 has no CPU fallback");
+        return LP_ERR_CUDA;
+    }
+    size_t off[LP_MAX_SEGS], len[LP_MAX_SEGS];
+    int m = 0;
+    for (int s = 0; s <= n_seg; ++s) {
+        if (s < n_seg && seg_len[s] > 0) {  // list order is kept: earlier slices finish first
+            off[m] = seg_off[s];
+            len[m] = seg_len[s];
+            ++m;
+        }
+        if (m == LP_MAX_SEGS || (s == n_seg && m > 0)) {
+            const SegList sl{off, len, m};
+            rc = plan_and_run(op, bufs, nullptr, nullptr, P, n, block, root, 0.f, 0.f, sms, nullptr, false,
+                              (cudaStream_t)cuda_stream, &sl);
+            if (rc != LP_OK) return rc;
+            m = 0;
+        }
+    }
+    return LP_OK;
 }
 
 int run_baseline(bool be, int op, float *const *bufs, int P, size_t n, int root, void *cuda_stream) {
@@ -417,6 +498,19 @@ int lp_bsp_sgd_momentum_step(float *const *grads, float *const *weights, float *
 int lp_bsp_sgd_alg2_step(float *const *grads, float *const *weights, float *velocity, int P, size_t n, size_t block,
                          int root, float lr, float mu, void *cuda_stream) {
     return run_alg2(grads, weights, velocity, P, n, block, root, lr, mu, cuda_stream);
+}
+
+int lp_broadcast_segments(float *const *bufs, int P, size_t n, const size_t *seg_off, const size_t *seg_len, int n_seg,
+                          size_t block, int root, void *cuda_stream) {
+    return run_segments(LP_OP_BROADCAST, bufs, P, n, seg_off, seg_len, n_seg, block, root, cuda_stream);
+}
+int lp_reduce_segments(float *const *bufs, int P, size_t n, const size_t *seg_off, const size_t *seg_len, int n_seg,
+                       size_t block, int root, void *cuda_stream) {
+    return run_segments(LP_OP_REDUCE, bufs, P, n, seg_off, seg_len, n_seg, block, root, cuda_stream);
+}
+int lp_allreduce_segments(float *const *bufs, int P, size_t n, const size_t *seg_off, const size_t *seg_len, int n_seg,
+                          size_t block, void *cuda_stream) {
+    return run_segments(LP_OP_ALLREDUCE, bufs, P, n, seg_off, seg_len, n_seg, block, 0, cuda_stream);
 }
 
 int lp_mst_broadcast(float *const *bufs, int P, size_t n, int root, void *s) {

@@ -35,6 +35,19 @@ struct LpArgs {
     lp_partition part;
 };
 
+// Second kernel parameter: the segment table of a layer-wise launch, or nothing.
+struct LpNoSegs {
+    int unused;
+};
+template <bool SEG>
+struct LpSegParam {
+    typedef LpNoSegs type;
+};
+template <>
+struct LpSegParam<true> {
+    typedef lp_seg_table type;
+};
+
 struct LpLaunch {
     uint32_t grid, threads, smem_bytes, stages, out_stages;
 };
@@ -46,10 +59,11 @@ struct LpTuning {
 
 // ---- launchers implemented in the kernel translation units ----------------------------------------
 // Each fills `cfg` (always) and, unless dry_run, enqueues the kernel(s) on `stream`.  Return cudaError_t.
-cudaError_t lp_pipeline_launch(const LpArgs &a, const LpTuning &t, int sm_count, LpLaunch *cfg, bool dry_run,
-                               cudaStream_t stream);
-cudaError_t lp_direct_launch(const LpArgs &a, const LpTuning &t, int sm_count, LpLaunch *cfg, bool dry_run,
-                             cudaStream_t stream);
+// `segs` != NULL: a layer-wise launch; a.part then holds block, tile and the TOTAL tile count only.
+cudaError_t lp_pipeline_launch(const LpArgs &a, const lp_seg_table *segs, const LpTuning &t, int sm_count, LpLaunch *cfg,
+                               bool dry_run, cudaStream_t stream);
+cudaError_t lp_direct_launch(const LpArgs &a, const lp_seg_table *segs, const LpTuning &t, int sm_count, LpLaunch *cfg,
+                             bool dry_run, cudaStream_t stream);
 cudaError_t lp_cluster_launch(const LpArgs &a, const LpTuning &t, int sm_count, LpLaunch *cfg, bool dry_run,
                               cudaStream_t stream);
 uint32_t lp_pipeline_tile(const LpTuning &t, const LpArgs &a, uint64_t n, uint64_t block);
@@ -215,6 +229,37 @@ struct LpTileClaimer {
             ctr[1] = 0ull;
             __threadfence();
         }
+    }
+};
+
+// a1/a2: tile index -> element range, for a single message (a.part) or a layer-wise launch (segment table).
+template <bool SEG>
+__device__ __forceinline__ void lp_lookup_tile(const LpArgs &a, const typename LpSegParam<SEG>::type &segs, uint64_t t,
+                                               uint64_t &off, uint32_t &len) {
+    if constexpr (SEG)
+        lp_seg_tile_range(segs, a.part.block, a.part.tile, t, off, len);
+    else
+        lp_tile_range(a.part, t, off, len);
+}
+
+// A tile [off, off + len) of 16-byte aligned vectors splits into a 16-byte aligned body [a0, a1) that the bulk
+// copies move and at most 3 + 3 head / tail elements that take the scalar path (tiles of a slice that does not
+// start on a 16-byte boundary, and the last tile of a message).
+struct LpTileSpan {
+    uint64_t a0;
+    uint32_t body;  // elements in [a0, a1): a multiple of 4
+    uint32_t head;  // elements in [off, a0)
+    uint32_t tail;  // elements in [a1, off + len)
+    __device__ __forceinline__ LpTileSpan(uint64_t off, uint32_t len) {
+        const uint64_t end = off + len;
+        uint64_t b0 = (off + 3) & ~(uint64_t)3;
+        if (b0 > end) b0 = end;
+        uint64_t b1 = end & ~(uint64_t)3;
+        if (b1 < b0) b1 = b0;
+        a0 = b0;
+        body = (uint32_t)(b1 - b0);
+        head = (uint32_t)(b0 - off);
+        tail = (uint32_t)(end - b1);
     }
 };
 

@@ -12,21 +12,31 @@ constexpr int kThreads = 256;
 constexpr int kRankChunk = 8;  // ranks whose loads are in flight together
 
 // NS > 0: number of folded inputs known at compile time (loops fully unrolled); NS == 0: runtime a.n_sum.
-template <int NS, int V>
-__global__ void __launch_bounds__(kThreads) lp_direct_kernel(const __grid_constant__ LpArgs a) {
-    const lp_partition &part = a.part;
+template <int NS, int V, bool SEG>
+__global__ void __launch_bounds__(kThreads)
+    lp_direct_kernel(const __grid_constant__ LpArgs a, const __grid_constant__ typename LpSegParam<SEG>::type segs) {
     const int n_sum = NS > 0 ? NS : a.n_sum;
     const int tid = threadIdx.x;
-    // a2: thread 0 claims the CTA's next tile one tile ahead (LpTileClaimer) and hands it over through shared memory
-    __shared__ unsigned long long s_tile[2];
-    LpTileClaimer claimer(a.sched, part.n_tiles);
-    uint64_t t = blockIdx.x;
-    if (tid == 0) claimer.claim();  // consumes blockIdx.x, prefetches the following tile
-    for (int it = 0; t < part.n_tiles; ++it) {
-        if (tid == 0) s_tile[it & 1] = claimer.claim();
-        uint64_t off;
-        uint32_t len;
-        lp_tile_range(part, t, off, len);
+    // a2: thread 0 claims the CTA's next tile one tile ahead (LpTileClaimer), turns it into an element range
+    // (single message or layer-wise list) and hands the range over through shared memory; len 0 = no tile left
+    __shared__ unsigned long long s_off[2];
+    __shared__ unsigned int s_len[2];
+    LpTileClaimer claimer(a.sched, a.part.n_tiles);
+    auto publish = [&](int slot) {
+        const uint64_t t = claimer.claim();
+        uint64_t off = 0;
+        uint32_t len = 0;
+        if (t < a.part.n_tiles) lp_lookup_tile<SEG>(a, segs, t, off, len);
+        s_off[slot] = off;
+        s_len[slot] = len;
+    };
+    if (tid == 0) publish(0);
+    __syncthreads();
+    for (int it = 0;; ++it) {
+        const uint64_t off = s_off[it & 1];
+        const uint32_t len = s_len[it & 1];
+        if (len == 0) break;
+        if (tid == 0) publish((it + 1) & 1);
         const uint64_t end = off + len;
         uint64_t a0 = (off + 3) & ~(uint64_t)3;  // first 16-byte aligned element (all buffers are 16-byte aligned)
         if (a0 > end) a0 = end;
@@ -86,34 +96,37 @@ __global__ void __launch_bounds__(kThreads) lp_direct_kernel(const __grid_consta
             for (int v = 0; v < V; ++v)
                 if (live[v]) lp_stg_stream(a.out[q] + a0 + 4 * (uint64_t)(tid + v * kThreads), acc[v]);
         }
-        __syncthreads();
-        t = s_tile[it & 1];
+        __syncthreads();  // the next range is published; everyone is done reading this one
     }
     if (tid == 0) claimer.finish();
 }
 
-template <int V>
-cudaError_t launch_v(const LpArgs &a, const LpLaunch &cfg, cudaStream_t stream) {
-#define LP_DIRECT_CASE(NS)                                                         \
-    case NS:                                                                       \
-        lp_direct_kernel<NS, V><<<cfg.grid, cfg.threads, 0, stream>>>(a);         \
+template <int V, bool SEG>
+cudaError_t launch_v(const LpArgs &a, const typename LpSegParam<SEG>::type &segs, const LpLaunch &cfg, cudaStream_t stream) {
+#define LP_DIRECT_CASE(NS)                                                                  \
+    case NS:                                                                                \
+        lp_direct_kernel<NS, V, SEG><<<cfg.grid, cfg.threads, 0, stream>>>(a, segs);       \
         break;
     switch (a.n_sum) {
         LP_DIRECT_CASE(1)
         LP_DIRECT_CASE(2)
         LP_DIRECT_CASE(3)
         LP_DIRECT_CASE(4)
-        LP_DIRECT_CASE(5)
         LP_DIRECT_CASE(6)
-        LP_DIRECT_CASE(7)
         LP_DIRECT_CASE(8)
         LP_DIRECT_CASE(16)
         default:
-            lp_direct_kernel<0, V><<<cfg.grid, cfg.threads, 0, stream>>>(a);
+            lp_direct_kernel<0, V, SEG><<<cfg.grid, cfg.threads, 0, stream>>>(a, segs);
             break;
     }
 #undef LP_DIRECT_CASE
     return cudaGetLastError();
+}
+
+template <int V>
+cudaError_t launch_seg(const LpArgs &a, const lp_seg_table *segs, const LpLaunch &cfg, cudaStream_t stream) {
+    if (segs) return launch_v<V, true>(a, *segs, cfg, stream);
+    return launch_v<V, false>(a, LpNoSegs{0}, cfg, stream);
 }
 
 }  // namespace
@@ -124,8 +137,8 @@ uint32_t lp_direct_tile(const LpTuning &t, int /*n_in*/) {
     return tile;
 }
 
-cudaError_t lp_direct_launch(const LpArgs &a, const LpTuning &t, int sm_count, LpLaunch *cfg, bool dry_run,
-                             cudaStream_t stream) {
+cudaError_t lp_direct_launch(const LpArgs &a, const lp_seg_table *segs, const LpTuning &t, int sm_count, LpLaunch *cfg,
+                             bool dry_run, cudaStream_t stream) {
     const uint32_t ctas = t.v[LP_TUNE_CTAS_PER_SM] ? (uint32_t)t.v[LP_TUNE_CTAS_PER_SM] : 4u;
     uint64_t grid = (uint64_t)sm_count * ctas;
     if (grid > a.part.n_tiles) grid = a.part.n_tiles;
@@ -137,9 +150,9 @@ cudaError_t lp_direct_launch(const LpArgs &a, const LpTuning &t, int sm_count, L
     if (dry_run || grid == 0) return cudaSuccess;
     lp_count_launch(1);
     switch (a.part.tile) {
-        case 1024: return launch_v<1>(a, *cfg, stream);
-        case 2048: return launch_v<2>(a, *cfg, stream);
-        case 4096: return launch_v<4>(a, *cfg, stream);
+        case 1024: return launch_seg<1>(a, segs, *cfg, stream);
+        case 2048: return launch_seg<2>(a, segs, *cfg, stream);
+        case 4096: return launch_seg<4>(a, segs, *cfg, stream);
         default: return cudaErrorInvalidValue;
     }
 }

@@ -17,7 +17,8 @@
 //                   (the paper's DMA2, outbound engine)
 //
 // so loads of later tiles/ranks, adds and stores of earlier tiles overlap (reduction math overlaps
-// transfer), and the grid of 148 x k persistent CTAs walks the tile list round-robin (lp_schedule.h).
+// transfer), and the grid of 148 x k persistent CTAs claims tiles from the launch's tile list (lp_schedule.h; the
+// list is one message cut into blocks, or -- layer-wise launches, Alg. 1 -- a list of messages).
 // Broadcast has no math: its kernel is the producer and the store thread alone.
 #include "lp_common.cuh"
 
@@ -43,10 +44,10 @@ __device__ __forceinline__ void wait_read_lag(int lag, bool complete) {
     }
 }
 
-// Tags of a store-ring slot (otile_of): the tile index, optionally marked as the momentum step's velocity tile;
-// kEndTag ends the store thread.
+// A ring slot's meta_len: the tile length (low 32 bits), in the store ring optionally marked as the momentum step's
+// velocity tile; kEndLen is the end marker.
 constexpr uint64_t kVelocityTag = 1ull << 62;
-constexpr uint64_t kEndTag = ~0ull;
+constexpr uint64_t kEndLen = ~0ull;
 
 struct Ring {
     int slot;
@@ -62,12 +63,14 @@ struct Ring {
 };
 
 // V float4 per add thread per tile, CW add warps: TILE = V * 4 * CW * 32 elements.
-// Every ring slot carries the index of the tile it belongs to (tile_of / otile_of): the producer claims tiles
-// (LpTileClaimer) and the other two roles learn the tile from the slot; an index >= n_tiles is the end marker
-// that travels producer -> add warps -> store thread.
-template <int V, int CW>
-__global__ void __launch_bounds__((CW + 2) * 32) lp_pipeline_kernel(const __grid_constant__ LpArgs a, int stages,
-                                                                     int out_stages) {
+// Every ring slot carries the element range of its tile (meta_off / meta_len): the producer claims tiles
+// (LpTileClaimer), turns the index into a range (lp_lookup_tile: a1/a2, single message or layer-wise list) and
+// the other two roles learn the range from the slot; kEndLen in meta_len is the end marker that travels
+// producer -> add warps -> store thread.
+template <int V, int CW, bool SEG>
+__global__ void __launch_bounds__((CW + 2) * 32)
+    lp_pipeline_kernel(const __grid_constant__ LpArgs a, const __grid_constant__ typename LpSegParam<SEG>::type segs,
+                       int stages, int out_stages) {
     constexpr int CT = CW * 32;
     constexpr int TILE = V * 4 * CT;
     extern __shared__ __align__(128) unsigned char lp_smem[];
@@ -77,8 +80,10 @@ __global__ void __launch_bounds__((CW + 2) * 32) lp_pipeline_kernel(const __grid
     uint64_t *empty = full + stages;
     uint64_t *ofull = empty + stages;
     uint64_t *oempty = ofull + out_stages;
-    uint64_t *tile_of = oempty + out_stages;  // [stages]
-    uint64_t *otile_of = tile_of + stages;    // [out_stages]
+    uint64_t *meta_off = oempty + out_stages;  // [stages]
+    uint64_t *meta_len = meta_off + stages;    // [stages]
+    uint64_t *ometa_off = meta_len + stages;   // [out_stages]
+    uint64_t *ometa_len = ometa_off + out_stages;
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < stages; ++s) {
@@ -95,7 +100,6 @@ __global__ void __launch_bounds__((CW + 2) * 32) lp_pipeline_kernel(const __grid
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
-    const lp_partition &part = a.part;
 
     if (warp == 0) {
         // ---------------- producer: claims tiles, TMA bulk loads in chain order ---------------------------
@@ -103,29 +107,31 @@ __global__ void __launch_bounds__((CW + 2) * 32) lp_pipeline_kernel(const __grid
             const uint64_t pol = lp_policy_evict_first();
             const bool hint = a.l2_hint >= 1;
             Ring ring(stages);
-            LpTileClaimer claimer(a.sched, part.n_tiles);
+            LpTileClaimer claimer(a.sched, a.part.n_tiles);
             for (;;) {
                 const uint64_t t = claimer.claim();
-                if (t >= part.n_tiles) {  // end marker
+                if (t >= a.part.n_tiles) {  // end marker
                     lp_mbar_wait(&empty[ring.slot], ring.phase ^ 1u);
-                    tile_of[ring.slot] = t;
+                    meta_len[ring.slot] = kEndLen;
                     lp_mbar_arrive(&full[ring.slot]);
                     break;
                 }
                 uint64_t off;
                 uint32_t len;
-                lp_tile_range(part, t, off, len);
-                const uint32_t bytes = (len & ~3u) * 4u;
+                lp_lookup_tile<SEG>(a, segs, t, off, len);
+                const LpTileSpan span(off, len);
+                const uint32_t bytes = span.body * 4u;
                 for (int r = 0; r < a.n_in; ++r) {
                     lp_mbar_wait(&empty[ring.slot], ring.phase ^ 1u);
-                    tile_of[ring.slot] = t;
+                    meta_off[ring.slot] = off;
+                    meta_len[ring.slot] = len;
                     if (bytes) {
                         lp_mbar_expect_tx(&full[ring.slot], bytes);
                         float *dst = in_ring + (size_t)ring.slot * TILE;
                         if (hint)
-                            lp_bulk_g2s_hint(dst, a.in[r] + off, bytes, &full[ring.slot], pol);
+                            lp_bulk_g2s_hint(dst, a.in[r] + span.a0, bytes, &full[ring.slot], pol);
                         else
-                            lp_bulk_g2s(dst, a.in[r] + off, bytes, &full[ring.slot]);
+                            lp_bulk_g2s(dst, a.in[r] + span.a0, bytes, &full[ring.slot]);
                     } else {
                         lp_mbar_arrive(&full[ring.slot]);
                     }
@@ -145,24 +151,21 @@ __global__ void __launch_bounds__((CW + 2) * 32) lp_pipeline_kernel(const __grid
             int free_slot = 0;  // oldest slot not yet handed back
             for (;;) {
                 lp_mbar_wait(&ofull[ring.slot], ring.phase);
-                const uint64_t tag = otile_of[ring.slot];
-                if (tag == kEndTag) break;
+                const uint64_t tag = ometa_len[ring.slot];
+                if (tag == kEndLen) break;
                 const bool to_velocity = (tag & kVelocityTag) != 0;  // momentum: the tile of new velocities
-                const uint64_t t = tag & ~kVelocityTag;
-                uint64_t off;
-                uint32_t len;
-                lp_tile_range(part, t, off, len);
-                const uint32_t bytes = (len & ~3u) * 4u;
+                const LpTileSpan span(ometa_off[ring.slot], (uint32_t)(tag & 0xffffffffull));
+                const uint32_t bytes = span.body * 4u;
                 if (bytes) {
                     const float *src = out_ring + (size_t)ring.slot * TILE;
                     if (to_velocity) {
-                        lp_bulk_s2g(a.vel_out + off, src, bytes);
+                        lp_bulk_s2g(a.vel_out + span.a0, src, bytes);
                     } else {
                         for (int q = 0; q < a.n_out; ++q) {
                             if (hint)
-                                lp_bulk_s2g_hint(a.out[q] + off, src, bytes, pol);
+                                lp_bulk_s2g_hint(a.out[q] + span.a0, src, bytes, pol);
                             else
-                                lp_bulk_s2g(a.out[q] + off, src, bytes);
+                                lp_bulk_s2g(a.out[q] + span.a0, src, bytes);
                         }
                     }
                 }
@@ -184,17 +187,16 @@ __global__ void __launch_bounds__((CW + 2) * 32) lp_pipeline_kernel(const __grid
         Ring oring(out_stages);
         for (;;) {
             lp_mbar_wait(&full[ring.slot], ring.phase);
-            const uint64_t t = tile_of[ring.slot];
-            if (t >= part.n_tiles) {  // end marker: pass it on to the store thread
+            const uint64_t len64 = meta_len[ring.slot];
+            if (len64 == kEndLen) {  // end marker: pass it on to the store thread
                 lp_mbar_wait(&oempty[oring.slot], oring.phase ^ 1u);
-                if (ctid == 0) otile_of[oring.slot] = kEndTag;
+                if (ctid == 0) ometa_len[oring.slot] = kEndLen;
                 __syncwarp();
                 if (lane == 0) lp_mbar_arrive(&ofull[oring.slot]);
                 break;
             }
-            uint64_t off;
-            uint32_t len;
-            lp_tile_range(part, t, off, len);
+            const uint64_t off = meta_off[ring.slot];
+            const uint32_t len = (uint32_t)len64;
             float4 acc[V];
             {  // rank 0: the partial starts as its block ("writing block a0 to a buffer on GPU1")
                 const float4 *s = reinterpret_cast<const float4 *>(in_ring + (size_t)ring.slot * TILE);
@@ -251,7 +253,10 @@ __global__ void __launch_bounds__((CW + 2) * 32) lp_pipeline_kernel(const __grid
                 float4 *ov = reinterpret_cast<float4 *>(out_ring + (size_t)oring.slot * TILE);
 #pragma unroll
                 for (int v = 0; v < V; ++v) ov[ctid + v * CT] = vel[v];
-                if (ctid == 0) otile_of[oring.slot] = t | kVelocityTag;
+                if (ctid == 0) {
+                    ometa_off[oring.slot] = off;
+                    ometa_len[oring.slot] = (uint64_t)len | kVelocityTag;
+                }
                 lp_fence_proxy_async();
                 __syncwarp();
                 if (lane == 0) lp_mbar_arrive(&ofull[oring.slot]);
@@ -262,27 +267,35 @@ __global__ void __launch_bounds__((CW + 2) * 32) lp_pipeline_kernel(const __grid
             float4 *o = reinterpret_cast<float4 *>(out_ring + (size_t)oring.slot * TILE);
 #pragma unroll
             for (int v = 0; v < V; ++v) o[ctid + v * CT] = acc[v];
-            if (ctid == 0) otile_of[oring.slot] = t;
+            if (ctid == 0) {
+                ometa_off[oring.slot] = off;
+                ometa_len[oring.slot] = len;
+            }
             lp_fence_proxy_async();
             __syncwarp();
             if (lane == 0) lp_mbar_arrive(&ofull[oring.slot]);
             oring.advance();
-            // elements past the 16-byte body of the message's last tile
-            const uint32_t rem = len & 3u;
-            if ((uint32_t)ctid < rem) lp_scalar_element(a, off + (len & ~3u) + ctid);
+            // the <= 3 + 3 elements outside the 16-byte aligned body of the tile
+            const LpTileSpan span(off, len);
+            if ((uint32_t)ctid < span.head) lp_scalar_element(a, off + ctid);
+            if ((uint32_t)ctid >= 32u && (uint32_t)ctid - 32u < span.tail) lp_scalar_element(a, span.a0 + span.body + (ctid - 32));
         }
     }
 }
 
 // Broadcast: the root's tile is loaded once into the ring and stored to the P-1 other ranks
 // straight from the same slot.  Warp 0 lane 0 claims tiles and loads, warp 1 lane 0 stores (and copies the
-// <= 3 elements past the 16-byte body of the message's last tile).
-__global__ void __launch_bounds__(64) lp_bcast_kernel(const __grid_constant__ LpArgs a, int stages, int tile) {
+// <= 3 + 3 elements outside the 16-byte aligned body of a tile).
+template <bool SEG>
+__global__ void __launch_bounds__(64)
+    lp_bcast_kernel(const __grid_constant__ LpArgs a, const __grid_constant__ typename LpSegParam<SEG>::type segs, int stages,
+                    int tile) {
     extern __shared__ __align__(128) unsigned char lp_smem[];
     float *ring_buf = reinterpret_cast<float *>(lp_smem);
     uint64_t *full = reinterpret_cast<uint64_t *>(ring_buf + (size_t)stages * tile);
     uint64_t *empty = full + stages;
-    uint64_t *tile_of = empty + stages;
+    uint64_t *meta_off = empty + stages;
+    uint64_t *meta_len = meta_off + stages;
     if (threadIdx.x == 0) {
         for (int s = 0; s < stages; ++s) {
             lp_mbar_init(&full[s], 1);
@@ -293,31 +306,33 @@ __global__ void __launch_bounds__(64) lp_bcast_kernel(const __grid_constant__ Lp
     __syncthreads();
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
-    const lp_partition &part = a.part;
     if (warp == 0 && lane == 0) {
         const uint64_t pol = lp_policy_evict_first();
         const bool hint = a.l2_hint >= 1;
         Ring ring(stages);
-        LpTileClaimer claimer(a.sched, part.n_tiles);
+        LpTileClaimer claimer(a.sched, a.part.n_tiles);
         for (;;) {
             const uint64_t t = claimer.claim();
             lp_mbar_wait(&empty[ring.slot], ring.phase ^ 1u);
-            tile_of[ring.slot] = t;
-            if (t >= part.n_tiles) {  // end marker
+            if (t >= a.part.n_tiles) {  // end marker
+                meta_len[ring.slot] = kEndLen;
                 lp_mbar_arrive(&full[ring.slot]);
                 break;
             }
             uint64_t off;
             uint32_t len;
-            lp_tile_range(part, t, off, len);
-            const uint32_t bytes = (len & ~3u) * 4u;
+            lp_lookup_tile<SEG>(a, segs, t, off, len);
+            meta_off[ring.slot] = off;
+            meta_len[ring.slot] = len;
+            const LpTileSpan span(off, len);
+            const uint32_t bytes = span.body * 4u;
             if (bytes) {
                 lp_mbar_expect_tx(&full[ring.slot], bytes);
                 float *dst = ring_buf + (size_t)ring.slot * tile;
                 if (hint)
-                    lp_bulk_g2s_hint(dst, a.in[0] + off, bytes, &full[ring.slot], pol);
+                    lp_bulk_g2s_hint(dst, a.in[0] + span.a0, bytes, &full[ring.slot], pol);
                 else
-                    lp_bulk_g2s(dst, a.in[0] + off, bytes, &full[ring.slot]);
+                    lp_bulk_g2s(dst, a.in[0] + span.a0, bytes, &full[ring.slot]);
             } else {
                 lp_mbar_arrive(&full[ring.slot]);
             }
@@ -333,22 +348,22 @@ __global__ void __launch_bounds__(64) lp_bcast_kernel(const __grid_constant__ Lp
         int free_slot = 0;
         for (;;) {
             lp_mbar_wait(&full[ring.slot], ring.phase);
-            const uint64_t t = tile_of[ring.slot];
-            if (t >= part.n_tiles) break;
-            uint64_t off;
-            uint32_t len;
-            lp_tile_range(part, t, off, len);
-            const uint32_t bytes = (len & ~3u) * 4u;
+            const uint64_t len64 = meta_len[ring.slot];
+            if (len64 == kEndLen) break;
+            const uint64_t off = meta_off[ring.slot];
+            const LpTileSpan span(off, (uint32_t)len64);
+            const uint32_t bytes = span.body * 4u;
             if (bytes) {
                 const float *src = ring_buf + (size_t)ring.slot * tile;
                 for (int q = 0; q < a.n_out; ++q) {
                     if (hint)
-                        lp_bulk_s2g_hint(a.out[q] + off, src, bytes, pol);
+                        lp_bulk_s2g_hint(a.out[q] + span.a0, src, bytes, pol);
                     else
-                        lp_bulk_s2g(a.out[q] + off, src, bytes);
+                        lp_bulk_s2g(a.out[q] + span.a0, src, bytes);
                 }
             }
-            for (uint32_t e = len & ~3u; e < len; ++e) lp_scalar_element(a, off + e);
+            for (uint32_t e = 0; e < span.head; ++e) lp_scalar_element(a, off + e);
+            for (uint32_t e = 0; e < span.tail; ++e) lp_scalar_element(a, span.a0 + span.body + e);
             lp_bulk_commit();
             ++issued;
             wait_read_lag(lag, a.store_wait != 0);
@@ -362,19 +377,38 @@ __global__ void __launch_bounds__(64) lp_bcast_kernel(const __grid_constant__ Lp
     }
 }
 
-template <int V, int CW>
-cudaError_t launch_fold(const LpArgs &a, const LpLaunch &cfg, cudaStream_t stream) {
-    static bool attr_set = false;  // per instantiation
-    static int attr_bytes = 0;
-    if (!attr_set || (int)cfg.smem_bytes > attr_bytes) {
-        cudaError_t e = cudaFuncSetAttribute(lp_pipeline_kernel<V, CW>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+template <int V, int CW, bool SEG>
+cudaError_t launch_fold_t(const LpArgs &a, const typename LpSegParam<SEG>::type &segs, const LpLaunch &cfg,
+                          cudaStream_t stream) {
+    static int attr_bytes = 0;  // per instantiation
+    if ((int)cfg.smem_bytes > attr_bytes) {
+        cudaError_t e = cudaFuncSetAttribute(lp_pipeline_kernel<V, CW, SEG>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              (int)cfg.smem_bytes);
         if (e != cudaSuccess) return e;
-        attr_set = true;
         attr_bytes = (int)cfg.smem_bytes;
     }
-    lp_pipeline_kernel<V, CW><<<cfg.grid, cfg.threads, cfg.smem_bytes, stream>>>(a, (int)cfg.stages,
-                                                                                  (int)cfg.out_stages);
+    lp_pipeline_kernel<V, CW, SEG><<<cfg.grid, cfg.threads, cfg.smem_bytes, stream>>>(a, segs, (int)cfg.stages,
+                                                                                       (int)cfg.out_stages);
+    return cudaGetLastError();
+}
+
+template <int V, int CW>
+cudaError_t launch_fold(const LpArgs &a, const lp_seg_table *segs, const LpLaunch &cfg, cudaStream_t stream) {
+    if (segs) return launch_fold_t<V, CW, true>(a, *segs, cfg, stream);
+    return launch_fold_t<V, CW, false>(a, LpNoSegs{0}, cfg, stream);
+}
+
+template <bool SEG>
+cudaError_t launch_bcast_t(const LpArgs &a, const typename LpSegParam<SEG>::type &segs, const LpLaunch &cfg, uint32_t tile,
+                           cudaStream_t stream) {
+    static int attr_bytes = 0;
+    if ((int)cfg.smem_bytes > attr_bytes) {
+        cudaError_t e = cudaFuncSetAttribute(lp_bcast_kernel<SEG>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             (int)cfg.smem_bytes);
+        if (e != cudaSuccess) return e;
+        attr_bytes = (int)cfg.smem_bytes;
+    }
+    lp_bcast_kernel<SEG><<<cfg.grid, cfg.threads, cfg.smem_bytes, stream>>>(a, segs, (int)cfg.stages, (int)tile);
     return cudaGetLastError();
 }
 
@@ -401,8 +435,8 @@ uint32_t lp_pipeline_tile(const LpTuning &t, const LpArgs &a, uint64_t n, uint64
     return tile;
 }
 
-cudaError_t lp_pipeline_launch(const LpArgs &a, const LpTuning &t, int sm_count, LpLaunch *cfg, bool dry_run,
-                               cudaStream_t stream) {
+cudaError_t lp_pipeline_launch(const LpArgs &a, const lp_seg_table *segs, const LpTuning &t, int sm_count, LpLaunch *cfg,
+                               bool dry_run, cudaStream_t stream) {
     const uint32_t tile = a.part.tile;
     const bool bcast = a.epilogue == LP_EPI_COPY;
     uint32_t ctas = t.v[LP_TUNE_CTAS_PER_SM] ? (uint32_t)t.v[LP_TUNE_CTAS_PER_SM] : (bcast && a.n_out <= 2 ? 3u : 2u);
@@ -416,7 +450,7 @@ cudaError_t lp_pipeline_launch(const LpArgs &a, const LpTuning &t, int sm_count,
         if (!t.v[LP_TUNE_STAGES] && !bcast && stages < (uint32_t)a.n_in) stages = a.n_in < 24 ? (uint32_t)a.n_in : 24u;
     }
     auto smem_of = [&](uint32_t st, uint32_t ost) {
-        return (st + ost) * tile * 4u + (3u * st + 3u * ost) * 8u;  // rings + full/empty barriers + tile indices
+        return (st + ost) * tile * 4u + (4u * st + 4u * ost) * 8u;  // rings + full/empty barriers + tile ranges
     };
     // shrink the rings until `ctas` CTAs fit one SM; if even the shallowest rings do not, take fewer CTAs
     const uint32_t want_stages = stages, want_out = out_stages;
@@ -464,20 +498,13 @@ cudaError_t lp_pipeline_launch(const LpArgs &a, const LpTuning &t, int sm_count,
         ap = &a_static;
     }
     if (bcast) {
-        static int attr_bytes = 0;
-        if ((int)cfg->smem_bytes > attr_bytes) {
-            cudaError_t e = cudaFuncSetAttribute(lp_bcast_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                 (int)cfg->smem_bytes);
-            if (e != cudaSuccess) return e;
-            attr_bytes = (int)cfg->smem_bytes;
-        }
-        lp_bcast_kernel<<<cfg->grid, cfg->threads, cfg->smem_bytes, stream>>>(*ap, (int)stages, (int)tile);
-        return cudaGetLastError();
+        if (segs) return launch_bcast_t<true>(*ap, *segs, *cfg, tile, stream);
+        return launch_bcast_t<false>(*ap, LpNoSegs{0}, *cfg, tile, stream);
     }
     switch (tile) {
-        case 1024: return launch_fold<2, 4>(*ap, *cfg, stream);
-        case 2048: return launch_fold<4, 4>(*ap, *cfg, stream);
-        case 4096: return launch_fold<4, 8>(*ap, *cfg, stream);
-        default: return launch_fold<8, 8>(*ap, *cfg, stream);
+        case 1024: return launch_fold<2, 4>(*ap, segs, *cfg, stream);
+        case 2048: return launch_fold<4, 4>(*ap, segs, *cfg, stream);
+        case 4096: return launch_fold<4, 8>(*ap, segs, *cfg, stream);
+        default: return launch_fold<8, 8>(*ap, segs, *cfg, stream);
     }
 }

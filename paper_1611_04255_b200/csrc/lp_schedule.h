@@ -56,3 +56,31 @@ LP_HD void lp_tile_range(const lp_partition &p, uint64_t idx, uint64_t &off, uin
     uint64_t rem = bend - off;
     len = rem < p.tile ? (uint32_t)rem : p.tile;
 }
+
+// ---- layer-wise messages (Alg. 1) -----------------------------------------------------
+// One launch can carry a LIST of messages: slices [off[s], off[s] + len[s]) of the rank vectors, e.g. the
+// layers of a network.  Every slice is its own LP message (own block partition, a1) and the tiles of the launch
+// are numbered slice by slice in list order, so earlier slices finish first.  tile_start[s] is the index of
+// slice s's first tile, tile_start[n_seg] the total.  The table travels as a kernel parameter (<= 4 KB).
+#define LP_MAX_SEGS 96
+
+struct lp_seg_table {
+    uint64_t off[LP_MAX_SEGS];
+    uint64_t len[LP_MAX_SEGS];
+    uint64_t tile_start[LP_MAX_SEGS + 1];
+    uint32_t n_seg;
+};
+
+// Tile idx of a segmented launch -> element range [off, off + len) in the rank vectors.
+LP_HD void lp_seg_tile_range(const lp_seg_table &st, uint64_t block, uint32_t tile, uint64_t idx, uint64_t &off,
+                             uint32_t &len) {
+    uint32_t lo = 0, hi = st.n_seg;  // tile_start[lo] <= idx < tile_start[hi]
+    while (hi - lo > 1) {
+        const uint32_t mid = (lo + hi) >> 1;
+        if (st.tile_start[mid] <= idx) lo = mid;
+        else hi = mid;
+    }
+    const lp_partition p = lp_make_partition(st.len[lo], block, tile);
+    lp_tile_range(p, idx - st.tile_start[lo], off, len);
+    off += st.off[lo];
+}

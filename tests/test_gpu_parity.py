@@ -347,6 +347,69 @@ def test_config2_momentum_20_iterations_all_tiles(oracle):
 
 
 # ---------------------------------------------------------------------------------------------------
+# layer-wise collectives (Alg. 1): a list of slices in one launch  -- SURVEY 8(f)-2
+# ---------------------------------------------------------------------------------------------------
+def _layer_slices(n, rng, k):
+    """k ragged, unordered, non-overlapping slices of [0, n) with gaps; offsets deliberately off 16-byte boundaries."""
+    cuts = np.sort(rng.choice(np.arange(1, n), size=2 * k - 1, replace=False))
+    bounds = np.concatenate([[0], cuts, [n]])
+    segs = [(int(bounds[2 * i]), int(bounds[2 * i + 1] - bounds[2 * i])) for i in range(k)]   # every other gap is a hole
+    order = rng.permutation(k)
+    return [segs[i] for i in order]
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("op", ["broadcast", "reduce", "allreduce"])
+@pytest.mark.parametrize("P,n,k,block", [(4, 300_007, 9, 16_384), (6, 1_000_003, 40, 65_536), (3, 5_000, 17, 100),
+                                         (16, 200_001, 5, 4096)])
+def test_segments_bit_exact(oracle, variant, op, P, n, k, block):
+    if variant == lp.VARIANT_COPY_ENGINE and k > 20:
+        pytest.skip("copy-engine variant: thousands of tiny copies, covered by the smaller cases")
+    lp.lp_set_variant(variant)
+    rng = np.random.default_rng([91, P, n])
+    segs = _layer_slices(n, rng, k) + [(n // 2, 0)]          # plus an empty slice
+    src = inputs.rank_vectors([9, n], P, n, "uniform")
+    root = P - 1
+    want = copies(src)
+    oracle.collective_segments({"broadcast": 0, "reduce": 1, "allreduce": 2}[op], want, segs, root=root)
+    dev = up(src)
+    if op == "allreduce":
+        lp.lp_allreduce_segments(dev, segs, block)
+    elif op == "reduce":
+        lp.lp_reduce_segments(dev, segs, block, root=root)
+    else:
+        lp.lp_broadcast_segments(dev, segs, block, root=root)
+    got = down(dev)
+    for r in range(P):
+        assert same(got[r], want[r]), (op, r)
+
+
+def test_segments_many_layers_and_all_tiles(oracle):
+    # more slices than one launch carries (96), every pipeline tile size, 1-element and 3-element slices included
+    P, n, block = 5, 2_000_003, 32_768
+    rng = np.random.default_rng(92)
+    segs = _layer_slices(n, rng, 230) + [(n - 1, 1)]
+    src = inputs.rank_vectors(93, P, n, "normal", 1e-3)
+    want = copies(src)
+    oracle.collective_segments(2, want, segs)
+    for tile in (0, 1024, 2048, 4096, 8192):
+        lp.lp_set_tuning(lp.TUNE_TILE_ELEMS, tile)
+        dev = up(src)
+        lp.lp_allreduce_segments(dev, segs, block)
+        assert all(same(g, w) for g, w in zip(down(dev), want)), tile
+
+
+def test_segments_validation():
+    dev = [torch.zeros(1000, device="cuda") for _ in range(3)]
+    for bad in ([(990, 11)], [(0, 10), (9, 5)], [(5, 10), (0, 6)]):     # past n; overlapping (either order)
+        with pytest.raises(lp.LpError) as e:
+            lp.lp_allreduce_segments(dev, bad, 64)
+        assert e.value.status == lp.LP_ERR_INVALID_ARG
+    lp.lp_allreduce_segments(dev, [], 64)                                # empty list: a no-op
+    lp.lp_allreduce_segments(dev, [(0, 0), (1000, 0)], 64)               # empty slices too
+
+
+# ---------------------------------------------------------------------------------------------------
 # MST / BE baselines (a7, a8)
 # ---------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("P,n", [(2, 1001), (3, 70_001), (4, 65_536), (5, 4099), (6, 300_003), (8, 100_001),
