@@ -93,7 +93,10 @@ extern "C" {
 #define LP_TUNE_SCHED 7         /* how persistent CTAs pick tiles: 0 (default) dynamic -- each CTA claims its next tile
                                    from a device-side counter, so SMs that get more HBM bandwidth take more tiles
                                    and all finish together; 1 static round robin (tile t -> CTA t mod grid) */
-#define LP_TUNE_COUNT 8
+#define LP_TUNE_GRID_LIMIT 8    /* at most this many persistent CTAs per launch (0 = one grid-full: SMs x CTAs per SM).
+                                   A collective that runs beside compute kernels (lp_comm_*) can be confined to a
+                                   few SMs' worth of CTAs, the way NCCL confines itself to a few channels */
+#define LP_TUNE_COUNT 9
 
 /* ---- LP collectives (the hot path) ----------------------------------------- */
 
@@ -153,6 +156,25 @@ LP_API int lp_reduce_segments(float *const *bufs, int P, size_t n, const size_t 
                               int n_seg, size_t block, int root, void *cuda_stream);
 LP_API int lp_allreduce_segments(float *const *bufs, int P, size_t n, const size_t *seg_off, const size_t *seg_len,
                                  int n_seg, size_t block, void *cuda_stream);
+
+/* ---- non-blocking use (Alg. 1's nonblocking_* / sync_*) ------------------------- */
+/* Every lp_* call above is already asynchronous to the host; "non-blocking" in the sense of Alg. 1 (PAPER.md:117-138:
+ * nonblocking_broadcast / nonblocking_reduce ... sync_broadcast() / sync_reduce(), "We use the nonblocking
+ * collective to achieve the overlapping") means asynchronous to the COMPUTE stream.  An lp_comm is a
+ * high-priority CUDA stream owned by the library plus the two events that tie it to the caller's streams:
+ *   lp_comm_after(c, s)   collectives enqueued on c from now on start after everything s holds now (the layer's
+ *                         gradient is ready), without blocking s;
+ *   lp_xxx(..., lp_comm_stream(c))   any collective of this library, enqueued on the comm stream;
+ *   lp_comm_wait(c, s)    s waits (on the device, no host sync) for everything enqueued on c so far: sync_reduce();
+ *   lp_comm_test(c, &done) host-side poll, done = 1 when the comm stream is idle.
+ * lp_comm_create fails with LP_ERR_CUDA without a device.  A comm may be used from one host thread at a time. */
+typedef struct lp_comm lp_comm;
+LP_API int lp_comm_create(lp_comm **comm);
+LP_API int lp_comm_destroy(lp_comm *comm);              /* synchronises the comm stream first */
+LP_API void *lp_comm_stream(lp_comm *comm);             /* the cudaStream_t, as void* */
+LP_API int lp_comm_after(lp_comm *comm, void *cuda_stream);
+LP_API int lp_comm_wait(lp_comm *comm, void *cuda_stream);
+LP_API int lp_comm_test(lp_comm *comm, int *done);
 
 /* ---- MST (binomial tree) and BE (recursive halving / doubling) baselines ------ */
 /* PAPER.md:93 (MST: "balanced tree of height ceil(log p)", whole-message steps) and

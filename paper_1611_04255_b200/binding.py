@@ -18,8 +18,8 @@ OP_BROADCAST, OP_REDUCE, OP_ALLREDUCE, OP_BSP_SGD, OP_BSP_SGD_MOM = 0, 1, 2, 3, 
 VARIANT_PIPELINE, VARIANT_DIRECT, VARIANT_CLUSTER, VARIANT_COPY_ENGINE = 0, 1, 2, 3
 MODEL_STAGE, MODEL_LINK, MODEL_LINK_RING = 0, 1, 2
 TUNE_TILE_ELEMS, TUNE_STAGES, TUNE_OUT_STAGES, TUNE_CTAS_PER_SM, TUNE_CE_STREAMS, TUNE_L2_HINT, TUNE_STORE_WAIT, \
-    TUNE_SCHED = range(8)
-TUNE_COUNT = 8
+    TUNE_SCHED, TUNE_GRID_LIMIT = range(9)
+TUNE_COUNT = 9
 VARIANT_NAMES = {0: "pipeline", 1: "direct", 2: "cluster", 3: "copy_engine"}
 
 
@@ -65,6 +65,13 @@ def lib() -> ctypes.CDLL:
     L.lp_broadcast_segments.argtypes = [pp, i32, sz, psz, psz, i32, sz, i32, vp]
     L.lp_reduce_segments.argtypes = [pp, i32, sz, psz, psz, i32, sz, i32, vp]
     L.lp_allreduce_segments.argtypes = [pp, i32, sz, psz, psz, i32, sz, vp]
+    L.lp_comm_create.argtypes = [ctypes.POINTER(vp)]
+    L.lp_comm_destroy.argtypes = [vp]
+    L.lp_comm_stream.argtypes = [vp]
+    L.lp_comm_stream.restype = vp
+    L.lp_comm_after.argtypes = [vp, vp]
+    L.lp_comm_wait.argtypes = [vp, vp]
+    L.lp_comm_test.argtypes = [vp, ctypes.POINTER(i32)]
     L.lp_bsp_sgd_momentum_step.argtypes = [pp, pp, vp, i32, sz, sz, i32, f32, f32, vp]
     L.lp_bsp_sgd_alg2_step.argtypes = [pp, pp, vp, i32, sz, sz, i32, f32, f32, vp]
     for name in ("lp_mst_broadcast", "lp_mst_reduce", "lp_be_broadcast", "lp_be_reduce"):
@@ -216,6 +223,41 @@ def lp_allreduce_segments(bufs, segments, block, stream=None):
     sg = _segments(segments)
     _check(lib().lp_allreduce_segments(arr, len(bufs), n, sg.off, sg.len, sg.k, block, _stream_ptr(stream)),
            "lp_allreduce_segments")
+
+
+# ---- lp_comm: Alg. 1's non-blocking collectives (a library-owned high-priority stream) --------------------
+class Comm:
+    """lp_comm handle.  `comm.stream` is a torch ExternalStream over the library's comm stream: pass it as
+    `stream=` to any collective; `after(s)` / `wait(s)` tie it to a compute stream (default: the current one)."""
+
+    def __init__(self):
+        import torch
+        h = ctypes.c_void_p()
+        _check(lib().lp_comm_create(ctypes.byref(h)), "lp_comm_create")
+        self.handle = h
+        self.stream = torch.cuda.ExternalStream(lib().lp_comm_stream(h))
+
+    def after(self, stream=None):
+        _check(lib().lp_comm_after(self.handle, _stream_ptr(stream)), "lp_comm_after")
+
+    def wait(self, stream=None):
+        _check(lib().lp_comm_wait(self.handle, _stream_ptr(stream)), "lp_comm_wait")
+
+    def test(self) -> bool:
+        done = ctypes.c_int(0)
+        _check(lib().lp_comm_test(self.handle, ctypes.byref(done)), "lp_comm_test")
+        return bool(done.value)
+
+    def close(self):
+        if self.handle is not None:
+            _check(lib().lp_comm_destroy(self.handle), "lp_comm_destroy")
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
 
 
 def _velocity_ptr(velocity, n):

@@ -23,7 +23,7 @@ namespace {
 
 std::mutex g_mu;
 int g_variant = LP_VARIANT_PIPELINE;
-LpTuning g_tuning = {{0, 0, 0, 0, 0, 0, 0, 0}};
+LpTuning g_tuning = {{0, 0, 0, 0, 0, 0, 0, 0, 0}};
 std::atomic<uint64_t> g_launches{0};
 char g_err[256] = "";
 int g_sm_count = 0;  // 0 = not queried yet
@@ -540,6 +540,78 @@ int lp_bsp_sgd_step_host(float *const *host_grads, float *const *host_weights, i
     return run_host(LP_OP_BSP_SGD, host_grads, host_weights, P, n, block, root, lr);
 }
 
+// ---- lp_comm: the comm stream of Alg. 1's non-blocking collectives ----------------------------------------
+struct lp_comm {
+    cudaStream_t stream;
+    cudaEvent_t after, done;
+};
+
+int lp_comm_create(lp_comm **comm) {
+    if (comm == nullptr) return LP_ERR_INVALID_ARG;
+    *comm = nullptr;
+    std::lock_guard<std::mutex> lock(g_mu);
+    if (sm_count_or_fail() <= 0) {
+        snprintf(g_err, sizeof(g_err), "no CUDA device: liblp_b200 has no CPU fallback");
+        return LP_ERR_CUDA;
+    }
+    int lo = 0, hi = 0;  // hi = numerically lowest = highest priority
+    LP_TRYC(cudaDeviceGetStreamPriorityRange(&lo, &hi), "lp_comm_create");
+    lp_comm *c = new lp_comm{nullptr, nullptr, nullptr};
+    cudaError_t e = cudaStreamCreateWithPriority(&c->stream, cudaStreamNonBlocking, hi);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->after, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->done, cudaEventDisableTiming);
+    if (e != cudaSuccess) {
+        if (c->done) cudaEventDestroy(c->done);
+        if (c->after) cudaEventDestroy(c->after);
+        if (c->stream) cudaStreamDestroy(c->stream);
+        delete c;
+        return cuda_fail(e, "lp_comm_create");
+    }
+    *comm = c;
+    return LP_OK;
+}
+
+int lp_comm_destroy(lp_comm *comm) {
+    if (comm == nullptr) return LP_ERR_INVALID_ARG;
+    cudaStreamSynchronize(comm->stream);
+    cudaEventDestroy(comm->after);
+    cudaEventDestroy(comm->done);
+    cudaStreamDestroy(comm->stream);
+    cudaGetLastError();
+    delete comm;
+    return LP_OK;
+}
+
+void *lp_comm_stream(lp_comm *comm) { return comm ? (void *)comm->stream : nullptr; }
+
+int lp_comm_after(lp_comm *comm, void *cuda_stream) {
+    if (comm == nullptr) return LP_ERR_INVALID_ARG;
+    LP_TRYC(cudaEventRecord(comm->after, (cudaStream_t)cuda_stream), "lp_comm_after");
+    LP_TRYC(cudaStreamWaitEvent(comm->stream, comm->after, 0), "lp_comm_after");
+    return LP_OK;
+}
+
+int lp_comm_wait(lp_comm *comm, void *cuda_stream) {
+    if (comm == nullptr) return LP_ERR_INVALID_ARG;
+    LP_TRYC(cudaEventRecord(comm->done, comm->stream), "lp_comm_wait");
+    LP_TRYC(cudaStreamWaitEvent((cudaStream_t)cuda_stream, comm->done, 0), "lp_comm_wait");
+    return LP_OK;
+}
+
+int lp_comm_test(lp_comm *comm, int *done) {
+    if (comm == nullptr || done == nullptr) return LP_ERR_INVALID_ARG;
+    const cudaError_t e = cudaStreamQuery(comm->stream);
+    if (e == cudaSuccess) {
+        *done = 1;
+    } else if (e == cudaErrorNotReady) {
+        cudaGetLastError();
+        *done = 0;
+    } else {
+        return cuda_fail(e, "lp_comm_test");
+    }
+    return LP_OK;
+}
+
 int lp_plan_query(int op, int P, size_t n, size_t block, lp_plan_info *out) {
     if (out == nullptr || P < 1 || P > LP_MAX_P || block == 0) return LP_ERR_INVALID_ARG;
     if (op < LP_OP_BROADCAST || op > LP_OP_BSP_SGD_MOM) return LP_ERR_INVALID_ARG;
@@ -590,6 +662,9 @@ int lp_set_tuning(int key, int value) {
         case LP_TUNE_STORE_WAIT:
         case LP_TUNE_SCHED:
             if (value > 1) return LP_ERR_INVALID_ARG;
+            break;
+        case LP_TUNE_GRID_LIMIT:
+            if (value > 65535) return LP_ERR_INVALID_ARG;
             break;
     }
     std::lock_guard<std::mutex> lock(g_mu);

@@ -141,6 +141,7 @@ cudaError_t lp_direct_launch(const LpArgs &a, const lp_seg_table *segs, const Lp
                              bool dry_run, cudaStream_t stream) {
     const uint32_t ctas = t.v[LP_TUNE_CTAS_PER_SM] ? (uint32_t)t.v[LP_TUNE_CTAS_PER_SM] : 4u;
     uint64_t grid = (uint64_t)sm_count * ctas;
+    if (t.v[LP_TUNE_GRID_LIMIT] && grid > (uint64_t)t.v[LP_TUNE_GRID_LIMIT]) grid = (uint64_t)t.v[LP_TUNE_GRID_LIMIT];
     if (grid > a.part.n_tiles) grid = a.part.n_tiles;
     cfg->grid = (uint32_t)grid;
     cfg->threads = kThreads;

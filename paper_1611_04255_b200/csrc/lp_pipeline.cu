@@ -426,8 +426,9 @@ static bool read_dominated(const LpArgs &a) { return a.epilogue != LP_EPI_COPY &
 // Tile size: the tuned or default size, halved while a whole block still fits in the half (a block is never
 // split finer than it has to be), floor 1024.
 uint32_t lp_pipeline_tile(const LpTuning &t, const LpArgs &a, uint64_t n, uint64_t block) {
+    const bool confined = t.v[LP_TUNE_GRID_LIMIT] > 0 && t.v[LP_TUNE_GRID_LIMIT] <= 148;  // see lp_pipeline_launch
     uint32_t tile = t.v[LP_TUNE_TILE_ELEMS] ? (uint32_t)t.v[LP_TUNE_TILE_ELEMS]
-                    : (a.epilogue == LP_EPI_COPY && a.n_out >= 9 ? 1024u : 2048u);
+                    : (confined ? 4096u : (a.epilogue == LP_EPI_COPY && a.n_out >= 9 ? 1024u : 2048u));
     uint64_t blk = block < n ? block : n;
     while (tile > 1024u && (uint64_t)(tile / 2) >= blk) tile /= 2;
     // latency regime: fewer tiles than SMs -> halve the tile so that twice as many SMs share the message
@@ -448,6 +449,14 @@ cudaError_t lp_pipeline_launch(const LpArgs &a, const lp_seg_table *segs, const 
     if (a.part.n_tiles <= (uint64_t)sm_count) {
         if (!t.v[LP_TUNE_CTAS_PER_SM]) ctas = 1u;
         if (!t.v[LP_TUNE_STAGES] && !bcast && stages < (uint32_t)a.n_in) stages = a.n_in < 24 ? (uint32_t)a.n_in : 24u;
+    }
+    // confined to fewer CTAs than SMs (LP_TUNE_GRID_LIMIT: a collective running beside compute kernels): one CTA per
+    // SM, 16 KB tiles (8 add warps) and a 12-deep load ring -- ~100 GB/s per CTA, so 64 CTAs already move 6.3 TB/s
+    // (profiles/r1_alg1_overlap.md)
+    if (t.v[LP_TUNE_GRID_LIMIT] && t.v[LP_TUNE_GRID_LIMIT] <= sm_count) {
+        if (!t.v[LP_TUNE_CTAS_PER_SM]) ctas = 1u;
+        if (!t.v[LP_TUNE_STAGES]) stages = 12u;
+        if (!t.v[LP_TUNE_OUT_STAGES] && !bcast) out_stages = 2u;
     }
     auto smem_of = [&](uint32_t st, uint32_t ost) {
         return (st + ost) * tile * 4u + (4u * st + 4u * ost) * 8u;  // rings + full/empty barriers + tile ranges
@@ -481,6 +490,7 @@ cudaError_t lp_pipeline_launch(const LpArgs &a, const lp_seg_table *segs, const 
         threads = (uint32_t)(CW + 2) * 32u;
     }
     uint64_t grid = (uint64_t)sm_count * ctas;
+    if (t.v[LP_TUNE_GRID_LIMIT] && grid > (uint64_t)t.v[LP_TUNE_GRID_LIMIT]) grid = (uint64_t)t.v[LP_TUNE_GRID_LIMIT];
     if (grid > a.part.n_tiles) grid = a.part.n_tiles;
     cfg->grid = (uint32_t)grid;
     cfg->threads = threads;

@@ -409,6 +409,57 @@ def test_segments_validation():
     lp.lp_allreduce_segments(dev, [(0, 0), (1000, 0)], 64)               # empty slices too
 
 
+def test_comm_nonblocking_alg1_backward_pass(oracle):
+    # Alg. 1's backward loop: nonblocking_reduce(layer i+1) on the comm stream while
+    # "Backward(i)" (here: a kernel that WRITES layer i's gradient on the compute stream) runs; sync_reduce() at
+    # the end.  The gradient of a layer only exists once its Backward has run, so a collective that did not wait
+    # for lp_comm_after would sum stale zeros.
+    P, block = 4, 16_384
+    layers = [(0, 70_001), (70_001, 300_000), (370_001, 13), (370_014, 1_000_003)]   # (offset, length), flat layout
+    n = layers[-1][0] + layers[-1][1]
+    src = inputs.rank_vectors(95, P, n, "normal", 1e-2)
+    want = copies(src)
+    oracle.collective_segments(2, want, layers)
+    staged = up(src)
+    grads = [torch.zeros(n, device="cuda") for _ in range(P)]
+    comm = lp.Comm()
+    compute = torch.cuda.Stream()
+    for limit in (0, 24):
+        lp.lp_set_tuning(lp.TUNE_GRID_LIMIT, limit)
+        for g in grads:
+            g.zero_()
+        torch.cuda.synchronize()
+        with torch.cuda.stream(compute):
+            for i in reversed(range(len(layers))):
+                o, l = layers[i]
+                torch.cuda._sleep(200_000)                    # Backward(i) takes a while ...
+                for g, s in zip(grads, staged):
+                    g[o:o + l].copy_(s[o:o + l])              # ... and produces layer i's sub-gradients
+                comm.after(compute)                           # nonblocking_allreduce(grad of layer i)
+                lp.lp_allreduce_segments(grads, [layers[i]], block, stream=comm.stream)
+            comm.wait(compute)                                # sync_reduce()
+            check = [g.clone() for g in grads]                # on the compute stream: must see the reduced values
+        torch.cuda.synchronize()
+        assert comm.test()
+        for r in range(P):
+            assert same(check[r].cpu().numpy(), want[r]), (limit, r)
+    comm.close()
+
+
+def test_grid_limit_bit_exact(oracle):
+    P, n, block = 6, 900_001, 65_536
+    src = inputs.rank_vectors(96, P, n, "uniform")
+    want = oracle.chain_sum(src)
+    for variant in (lp.VARIANT_PIPELINE, lp.VARIANT_DIRECT):
+        lp.lp_set_variant(variant)
+        for limit in (1, 7, 148):
+            lp.lp_set_tuning(lp.TUNE_GRID_LIMIT, limit)
+            dev = up(src)
+            lp.lp_allreduce(dev, block)
+            assert all(same(g, want) for g in down(dev)), (variant, limit)
+            assert lp.lp_plan_query(lp.OP_ALLREDUCE, P, n, block)["grid"] <= limit
+
+
 # ---------------------------------------------------------------------------------------------------
 # MST / BE baselines (a7, a8)
 # ---------------------------------------------------------------------------------------------------
