@@ -211,6 +211,19 @@ LP_API int lp_schedule_steps(int P, size_t n, size_t block, int op, int model, u
 /* Number of whole-message levels of the MST baseline, ceil(log2 P). */
 LP_API int lp_mst_levels(int P);
 
+/* Cost model of Sec. 3.2 (Eq. 1: T = alpha + beta n + gamma n per exchange; Table 1), in
+ * seconds: algo LP_ALGO_LP / MST / BE, op LP_OP_BROADCAST / REDUCE / ALLREDUCE, p ranks, message and block size in
+ * BYTES (the paper's unit here), alpha s, beta and gamma s/byte.  log p = log2 p without ceiling.
+ * b_bytes is ignored for MST / BE.  Returns -1 on bad arguments. */
+#define LP_ALGO_LP 0
+#define LP_ALGO_MST 1
+#define LP_ALGO_BE 2
+LP_API double lp_cost_model(int algo, int op, double p, double n_bytes, double b_bytes, double alpha, double beta,
+                            double gamma);
+/* The block size (bytes) that minimises lp_cost_model(LP_ALGO_LP, op, ...): sqrt(n a / ((p-1) w)), a and w the latency
+ * and per-byte cost of one block exchange of `op`; clamped to n_bytes.  -1 on bad arguments. */
+LP_API double lp_optimal_block(int op, double p, double n_bytes, double alpha, double beta, double gamma);
+
 /* How the persistent kernel will cut and spread the work for (op, P, n, block) under the current variant
  * and tuning: tile size, tile count, grid, threads, dynamic shared memory, ring depths. */
 typedef struct lp_plan_info {

@@ -86,6 +86,11 @@ def lib() -> ctypes.CDLL:
     L.lp_stage_block.restype = ctypes.c_int64
     L.lp_schedule_steps.argtypes = [i32, sz, sz, i32, i32, ctypes.POINTER(u64)]
     L.lp_mst_levels.argtypes = [i32]
+    f64 = ctypes.c_double
+    L.lp_cost_model.argtypes = [i32, i32, f64, f64, f64, f64, f64, f64]
+    L.lp_cost_model.restype = f64
+    L.lp_optimal_block.argtypes = [i32, f64, f64, f64, f64, f64]
+    L.lp_optimal_block.restype = f64
     L.lp_plan_query.argtypes = [i32, i32, sz, sz, ctypes.POINTER(PlanInfo)]
     L.lp_min_bytes.argtypes = [i32, i32, sz]
     L.lp_min_bytes.restype = u64
@@ -97,6 +102,17 @@ def lib() -> ctypes.CDLL:
     L.lp_status_string.restype = ctypes.c_char_p
     _lib = L
     return L
+
+
+ALGO_LP, ALGO_MST, ALGO_BE = 0, 1, 2
+
+
+def lp_cost_model(algo, op, p, n_bytes, b_bytes, alpha, beta, gamma=0.0) -> float:
+    return float(lib().lp_cost_model(algo, op, p, n_bytes, b_bytes, alpha, beta, gamma))
+
+
+def lp_optimal_block(op, p, n_bytes, alpha, beta, gamma=0.0) -> float:
+    return float(lib().lp_optimal_block(op, p, n_bytes, alpha, beta, gamma))
 
 
 def status_string(status: int) -> str:

@@ -10,6 +10,8 @@
 // reduce traffic has priority over redistribution traffic, lower blocks first.
 #include <stdint.h>
 
+#include <math.h>
+
 #include <vector>
 
 #include "../../include/lp_collectives.h"
@@ -118,4 +120,50 @@ extern "C" int lp_schedule_steps(int P, size_t n, size_t block, int op, int mode
     else
         *steps_out = link_steps(P, nb, op, model);
     return LP_OK;
+}
+
+// ---- cost model of Sec. 3.2 (Eq. 1, Table 1) -----------------------------------------
+// A block exchange costs alpha + beta b (+ gamma b with a reduce); LP pays it over a pipeline of p - 1 + n/b
+// blocks, MST pays a whole-message exchange per tree level (log2 p, ceiling omitted as in PAPER.md:93), BE pays
+// the scatter / reduce-scatter + gather / allgather sums of PAPER.md:95.  Table 1 read as in DESIGN.md U10/U11.
+extern "C" double lp_cost_model(int algo, int op, double p, double n_bytes, double b_bytes, double alpha, double beta,
+                                double gamma) {
+    if (p < 1.0 || n_bytes < 0.0 || alpha < 0.0 || beta < 0.0 || gamma < 0.0) return -1.0;
+    if (op != LP_OP_BROADCAST && op != LP_OP_REDUCE && op != LP_OP_ALLREDUCE) return -1.0;
+    const double levels = log2(p);
+    const double share = (p - 1.0) / p;
+    switch (algo) {
+        case LP_ALGO_LP: {
+            if (b_bytes <= 0.0) return -1.0;
+            const double exchanges = p - 1.0 + n_bytes / b_bytes;
+            const double per_exchange_bw = op == LP_OP_BROADCAST ? beta : (op == LP_OP_REDUCE ? beta + gamma : 2.0 * beta + gamma);
+            const double per_exchange_lat = op == LP_OP_ALLREDUCE ? 2.0 * alpha : alpha;
+            return exchanges * (per_exchange_lat + b_bytes * per_exchange_bw);
+        }
+        case LP_ALGO_MST: {
+            const double per_level = op == LP_OP_BROADCAST ? alpha + n_bytes * beta
+                                     : (op == LP_OP_REDUCE ? alpha + n_bytes * (beta + gamma)
+                                                           : 2.0 * alpha + n_bytes * (2.0 * beta + gamma));
+            return levels * per_level;
+        }
+        case LP_ALGO_BE: {
+            const double moved = share * n_bytes;
+            if (op == LP_OP_BROADCAST) return (levels + p - 1.0) * alpha + 2.0 * moved * beta;
+            return 2.0 * levels * alpha + 2.0 * moved * beta + moved * gamma;
+        }
+        default: return -1.0;
+    }
+}
+
+// Block size that minimises the LP cost above: d/db [(p - 1 + n/b)(a + b w)] = (p - 1) w - n a / b^2 = 0, with a the
+// latency and w the bandwidth cost of one exchange  =>  b* = sqrt(n a / ((p - 1) w)).  (The paper picks "around
+// 64 KB" by hand; this is the closed form its own model implies.)  p <= 1 or a == 0: any block does,
+// returns n.
+extern "C" double lp_optimal_block(int op, double p, double n_bytes, double alpha, double beta, double gamma) {
+    if (p < 1.0 || n_bytes <= 0.0 || alpha < 0.0 || beta < 0.0 || gamma < 0.0) return -1.0;
+    const double w = op == LP_OP_BROADCAST ? beta : (op == LP_OP_REDUCE ? beta + gamma : 2.0 * beta + gamma);
+    const double a = op == LP_OP_ALLREDUCE ? 2.0 * alpha : alpha;
+    if (p <= 1.0 || a == 0.0 || w == 0.0) return n_bytes;
+    const double b = sqrt(n_bytes * a / ((p - 1.0) * w));
+    return b < n_bytes ? b : n_bytes;
 }

@@ -162,3 +162,39 @@ def test_compute_entry_fails_loudly_without_device():
     # valid arguments, no GPU: the library must refuse (LP_ERR_CUDA), never compute on the CPU
     assert L.lp_allreduce(ptrs, 2, 64, 16, ctypes.c_void_p(0)) == lp.LP_ERR_CUDA
     assert not raw[0].any() and not raw[1].any()
+
+
+# ---- cost model of Sec. 3.2 (host only) --------------------------------------------------------------------
+def test_cost_model_matches_oracle_table1():
+    # the library's Table 1 (own code) against the oracle's, over a grid of p, n, b, alpha, beta, gamma
+    from oracle import lpo
+    for algo in (lp.ALGO_LP, lp.ALGO_MST, lp.ALGO_BE):
+        for op in (BCAST, REDUCE, ALLREDUCE):
+            for p in (2, 3, 6, 8, 16):
+                for n in (4096.0, 2.44e8, 5.5e8):
+                    for b in (4096.0, 65536.0, 1.0e6):
+                        for alpha, beta, gamma in ((1e-7, 1e-9, 0.0), (3e-6, 1.5e-13, 2e-14), (0.0, 1e-9, 1e-10)):
+                            got = lp.lp_cost_model(algo, op, p, n, b, alpha, beta, gamma)
+                            want = lpo.cost(algo, op, p, n, b, alpha, beta, gamma)
+                            assert got == pytest.approx(want, rel=1e-12), (algo, op, p, n, b)
+    assert lp.lp_cost_model(lp.ALGO_LP, BCAST, 4, 1e6, 0.0, 1e-7, 1e-9) == -1.0      # LP needs a block size
+    assert lp.lp_cost_model(7, BCAST, 4, 1e6, 1e4, 1e-7, 1e-9) == -1.0
+
+
+def test_optimal_block_minimises_the_lp_cost():
+    # b* against a brute-force scan of the ORACLE's cost function; and the paper's own numbers: alpha = 1e-7 s,
+    # beta = 1e-9 s/byte, AlexNet-sized 244 MB message on 6 GPUs -> tens of KB ("around 64 KB")
+    from oracle import lpo
+    for op in (BCAST, REDUCE, ALLREDUCE):
+        for p, n, alpha, beta, gamma in ((6, 2.44e8, 1e-7, 1e-9, 0.0), (16, 5.52e8, 2.5e-6, 1.4e-13, 1e-14),
+                                         (2, 1e6, 1e-6, 1e-10, 1e-10)):
+            b_star = lp.lp_optimal_block(op, p, n, alpha, beta, gamma)
+            scan = np.geomspace(64.0, n, 4000)
+            costs = [lpo.cost(0, op, p, n, b, alpha, beta, gamma) for b in scan]
+            best = scan[int(np.argmin(costs))]
+            assert abs(np.log(b_star / best)) < 0.01, (op, p, b_star, best)
+            assert lpo.cost(0, op, p, n, b_star, alpha, beta, gamma) <= min(costs) * (1 + 1e-9)
+    b = lp.lp_optimal_block(BCAST, 6, 2.44e8, 1e-7, 1e-9)
+    assert 32e3 < b < 128e3                                   # sqrt(2.44e8 * 1e-7 / (5 * 1e-9)) = 69.9 KB
+    assert lp.lp_optimal_block(BCAST, 1, 1e6, 1e-7, 1e-9) == 1e6
+    assert lp.lp_optimal_block(BCAST, 4, 1e6, 0.0, 1e-9) == 1e6
