@@ -45,7 +45,7 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json configs (1 or 4 for allreduce)")
     ap.add_argument("--block", type=int, default=0, help="LP block in elements (0 = the config's)")
-    ap.add_argument("--variant", default="pipeline", choices=["pipeline", "direct", "cluster", "copy_engine"])
+    ap.add_argument("--variant", default="auto", choices=["auto", "pipeline", "direct", "cluster", "copy_engine"])
     ap.add_argument("--no-detail", action="store_true", help="skip the secondary measurements")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
@@ -225,7 +225,7 @@ def run_ours(args, c, rank, world, local):
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     lp.lib()
-    variant = {"pipeline": 0, "direct": 1, "cluster": 2, "copy_engine": 3}[args.variant]
+    variant = {"pipeline": 0, "direct": 1, "cluster": 2, "copy_engine": 3, "auto": 4}[args.variant]
     lp.lp_set_variant(variant)
     P, n = c["P"], c["n"]
     block = args.block or c["block"]
@@ -271,6 +271,7 @@ def run_ours(args, c, rank, world, local):
     hbm = min_bytes / (ms_per_step * 1e-3) / 1e9  # per GPU
     peak, peak_src = measured_peak()
     plan = lp.lp_plan_query(lp.OP_ALLREDUCE, P, n, block)
+    ran = ["pipeline", "direct", "cluster", "copy_engine"][plan["variant"]]  # what LP_VARIANT_AUTO resolved to
 
     # e2e: host buffers through lp_allreduce_host, copies inside the timed region
     e2e = None
@@ -311,11 +312,11 @@ def run_ours(args, c, rank, world, local):
         "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": f"BASELINE.json configs[{args.config}]: {c['name']}", "P": P, "n": n, "block": block,
-                   "variant": args.variant, "plan": plan, "parallelism": f"replicas x{world} (no collective)",
+                   "variant": ran, "plan": plan, "parallelism": f"replicas x{world} (no collective)",
                    "l2": f"inputs {P * n * 4 / 1e6:.0f} MB per set >> 126 MB L2, {n_sets} rotating sets"},
         "roofline": {"bound": "hbm", "achieved": hbm, "peak": peak, "unit": "GB/s", "frac": hbm / peak,
-                     "traffic": NCU_TRAFFIC_BYTES.get((P, n, args.variant)), "peak_source": peak_src, "frac_of_nominal_8TBs": hbm / 8000.0,
-                     "kernel": "lp_pipeline_kernel" if variant == 0 else args.variant,
+                     "traffic": NCU_TRAFFIC_BYTES.get((P, n, ran)), "peak_source": peak_src, "frac_of_nominal_8TBs": hbm / 8000.0,
+                     "kernel": "lp_pipeline_kernel" if ran == "pipeline" else ran,
                      "algorithmic_bytes_per_launch": min_bytes},
         "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "detail": detail,
     }

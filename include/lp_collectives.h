@@ -68,13 +68,17 @@ extern "C" {
 #define LP_OP_BSP_SGD_MOM 4  /* Alg. 3 step with momentum; for lp_plan_query / lp_min_bytes */
 
 /* realisation of the LP pipeline used by lp_broadcast/lp_reduce/lp_allreduce/lp_bsp_sgd_step */
-#define LP_VARIANT_PIPELINE 0    /* default: one persistent kernel; per CTA a TMA-bulk shared-memory ring
+#define LP_VARIANT_PIPELINE 0    /* one persistent kernel; per CTA a TMA-bulk shared-memory ring
                                     with mbarrier full/empty flags handed producer warp -> add warps -> store warp */
-#define LP_VARIANT_DIRECT 1      /* one persistent kernel, 128-bit register loads/stores, chain fold in registers */
+#define LP_VARIANT_DIRECT 1      /* one kernel, one CTA per tile, 128-bit register loads/stores, chain fold in registers */
 #define LP_VARIANT_CLUSTER 2     /* stage-per-rank: a thread-block cluster of P CTAs, CTA r owns rank r and hands
                                     the running partial to CTA r+1 through distributed shared memory (P <= 16) */
 #define LP_VARIANT_COPY_ENGINE 3 /* the paper's own design: one cudaMemcpyAsync + one add kernel per (hop, block)
                                     on two streams */
+
+#define LP_VARIANT_AUTO 4        /* default: DIRECT below ~384 MB of HBM traffic per call (latency regime), PIPELINE
+                                    above and whenever LP_TUNE_GRID_LIMIT confines the grid; lp_plan_query reports the
+                                    variant that will run */
 
 /* schedule models of lp_schedule_steps (U2, U3) */
 #define LP_MODEL_STAGE 0        /* stages = the P ranks; pipeline length P - 1 + nb */

@@ -82,7 +82,7 @@ def main(argv=None):
                              t_at_b_star_ms=lp.lp_cost_model(lp.ALGO_LP, lp.OP_ALLREDUCE, P, nbytes, b_star, A / 2, W / 2, 0.0) * 1e3,
                              best_block_bytes=float(bb[i_best]), best_ms=ts[i_best] * 1e3,
                              max_rel_err=float(np.max(np.abs(pred - np.array(ts)) / np.array(ts))), pred_ms=(pred * 1e3).tolist())
-    lp.lp_set_variant(lp.VARIANT_PIPELINE)
+    lp.lp_set_variant(lp.VARIANT_AUTO)
     os.makedirs(os.path.dirname(os.path.abspath(args.out)), exist_ok=True)
     with open(args.out + ".jsonl", "w") as f:
         for r in rows:

@@ -22,7 +22,7 @@ void lp_copy_engine_shutdown();
 namespace {
 
 std::mutex g_mu;
-int g_variant = LP_VARIANT_PIPELINE;
+int g_variant = LP_VARIANT_AUTO;
 LpTuning g_tuning = {{0, 0, 0, 0, 0, 0, 0, 0, 0}};
 std::atomic<uint64_t> g_launches{0};
 char g_err[256] = "";
@@ -152,7 +152,6 @@ struct SegList {
 int plan_and_run(int op, float *const *bufs, float *const *weights, float *velocity, int P, size_t n, size_t block,
                  int root, float lr, float mu, int sm_count, lp_plan_info *info, bool dry_run, cudaStream_t stream,
                  const SegList *segl = nullptr) {
-    const int variant = g_variant;
     const bool layered = segl != nullptr && segl->n > 0;
     LpArgs a;
     LpLaunch cfg = {0, 0, 0, 0, 0};
@@ -171,9 +170,19 @@ int plan_and_run(int op, float *const *bufs, float *const *weights, float *veloc
         n_work = 0;
         for (int s = 0; s < segl->n; ++s) n_work += segl->len[s];
     }
+    // LP_VARIANT_AUTO: below ~384 MB of HBM traffic (192 MB for reduce, 64 MB for a copy to one or two ranks) the one-CTA-per-tile
+    // register kernel is ahead (no per-CTA pipeline to fill: 1.3-3 us against 2-6 us for a 4 KB message); above,
+    // the persistent TMA pipeline (profiles/r1_tuning.md section 6).  A confined grid always takes the pipeline.
+    int variant = g_variant;
+    if (variant == LP_VARIANT_AUTO) {
+        const uint64_t traffic = lp_min_bytes(op, P, n_work);
+        const uint64_t cut = (op == LP_OP_BROADCAST && P <= 3) ? (64ull << 20)
+                             : (op == LP_OP_REDUCE ? (192ull << 20) : (384ull << 20));
+        variant = (traffic < cut && g_tuning.v[LP_TUNE_GRID_LIMIT] == 0) ? LP_VARIANT_DIRECT : LP_VARIANT_PIPELINE;
+    }
     uint32_t tile;
     switch (variant) {
-        case LP_VARIANT_DIRECT: tile = lp_direct_tile(g_tuning, a.n_in); break;
+        case LP_VARIANT_DIRECT: tile = lp_direct_tile(g_tuning, a.n_in, n_work); break;
         case LP_VARIANT_CLUSTER: tile = lp_cluster_tile(g_tuning); break;
         default: tile = lp_pipeline_tile(g_tuning, a, n_work, block); break;
     }
@@ -195,7 +204,7 @@ int plan_and_run(int op, float *const *bufs, float *const *weights, float *veloc
         a.part.nb = blocks;
         a.part.n_tiles = tiles;
     }
-    if (!dry_run && g_tuning.v[LP_TUNE_SCHED] == 0 && variant != LP_VARIANT_COPY_ENGINE && a.part.n_tiles > 0) {
+    if (!dry_run && g_tuning.v[LP_TUNE_SCHED] == 0 && variant == LP_VARIANT_PIPELINE && a.part.n_tiles > 0) {
         cudaError_t es = lp_sched_acquire(&a.sched);
         if (es != cudaSuccess) return cuda_fail(es, "tile-claim counters");
     }
@@ -635,7 +644,7 @@ uint64_t lp_min_bytes(int op, int P, size_t n) {
 }
 
 int lp_set_variant(int variant) {
-    if (variant < LP_VARIANT_PIPELINE || variant > LP_VARIANT_COPY_ENGINE) return LP_ERR_INVALID_ARG;
+    if (variant < LP_VARIANT_PIPELINE || variant > LP_VARIANT_AUTO) return LP_ERR_INVALID_ARG;
     std::lock_guard<std::mutex> lock(g_mu);
     g_variant = variant;
     return LP_OK;

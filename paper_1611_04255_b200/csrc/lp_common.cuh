@@ -67,7 +67,7 @@ cudaError_t lp_direct_launch(const LpArgs &a, const lp_seg_table *segs, const Lp
 cudaError_t lp_cluster_launch(const LpArgs &a, const LpTuning &t, int sm_count, LpLaunch *cfg, bool dry_run,
                               cudaStream_t stream);
 uint32_t lp_pipeline_tile(const LpTuning &t, const LpArgs &a, uint64_t n, uint64_t block);
-uint32_t lp_direct_tile(const LpTuning &t, int n_in);
+uint32_t lp_direct_tile(const LpTuning &t, int n_in, uint64_t n_work);
 uint32_t lp_cluster_tile(const LpTuning &t);
 
 // Segment jobs of the MST / BE baselines: dst[i] = a[i] + b[i] (b != NULL) or dst[i] = a[i], i in [0, len).

@@ -1,4 +1,4 @@
-// lp_direct.cu -- LP_VARIANT_DIRECT: the LP collective as one persistent kernel that keeps the running
+// lp_direct.cu -- LP_VARIANT_DIRECT: the LP collective as one kernel (one CTA per tile) that keeps the running
 // partial of the chain (a0 -> a' = a0 + a1 -> a'' = a' + a2) in registers.  Each thread owns V
 // 16-byte vectors of a tile, issues the 128-bit streaming loads of up to 8 ranks at once (memory-level
 // parallelism replaces the paper's two DMA engines), folds them in rank order 0 -> P-1 with RN adds and
@@ -17,26 +17,14 @@ __global__ void __launch_bounds__(kThreads)
     lp_direct_kernel(const __grid_constant__ LpArgs a, const __grid_constant__ typename LpSegParam<SEG>::type segs) {
     const int n_sum = NS > 0 ? NS : a.n_sum;
     const int tid = threadIdx.x;
-    // a2: thread 0 claims the CTA's next tile one tile ahead (LpTileClaimer), turns it into an element range
-    // (single message or layer-wise list) and hands the range over through shared memory; len 0 = no tile left
-    __shared__ unsigned long long s_off[2];
-    __shared__ unsigned int s_len[2];
-    LpTileClaimer claimer(a.sched, a.part.n_tiles);
-    auto publish = [&](int slot) {
-        const uint64_t t = claimer.claim();
-        uint64_t off = 0;
-        uint32_t len = 0;
-        if (t < a.part.n_tiles) lp_lookup_tile<SEG>(a, segs, t, off, len);
-        s_off[slot] = off;
-        s_len[slot] = len;
-    };
-    if (tid == 0) publish(0);
-    __syncthreads();
-    for (int it = 0;; ++it) {
-        const uint64_t off = s_off[it & 1];
-        const uint32_t len = s_len[it & 1];
-        if (len == 0) break;
-        if (tid == 0) publish((it + 1) & 1);
+    // a2: one CTA per tile by default (grid == n_tiles): the hardware block scheduler hands the next tile to
+    // whichever SM frees up first -- the same balance the pipeline kernel gets from its tile claims, with no
+    // per-CTA setup at all, which is what the latency regime wants.  A confined grid (LP_TUNE_GRID_LIMIT /
+    // LP_TUNE_CTAS_PER_SM) walks the tile list round robin.
+    for (uint64_t t = blockIdx.x; t < a.part.n_tiles; t += gridDim.x) {
+        uint64_t off;
+        uint32_t len;
+        lp_lookup_tile<SEG>(a, segs, t, off, len);
         const uint64_t end = off + len;
         uint64_t a0 = (off + 3) & ~(uint64_t)3;  // first 16-byte aligned element (all buffers are 16-byte aligned)
         if (a0 > end) a0 = end;
@@ -96,9 +84,7 @@ __global__ void __launch_bounds__(kThreads)
             for (int v = 0; v < V; ++v)
                 if (live[v]) lp_stg_stream(a.out[q] + a0 + 4 * (uint64_t)(tid + v * kThreads), acc[v]);
         }
-        __syncthreads();  // the next range is published; everyone is done reading this one
     }
-    if (tid == 0) claimer.finish();
 }
 
 template <int V, bool SEG>
@@ -131,18 +117,25 @@ cudaError_t launch_seg(const LpArgs &a, const lp_seg_table *segs, const LpLaunch
 
 }  // namespace
 
-uint32_t lp_direct_tile(const LpTuning &t, int /*n_in*/) {
-    uint32_t tile = t.v[LP_TUNE_TILE_ELEMS] ? (uint32_t)t.v[LP_TUNE_TILE_ELEMS] : 2048u;
-    if (tile != 1024u && tile != 2048u && tile != 4096u) tile = 2048u;
+// 8 KB tiles (2 vectors per thread and rank); 4 KB when the message has fewer tiles than two grid-fulls of SMs
+// (latency regime: spread it over more SMs).
+uint32_t lp_direct_tile(const LpTuning &t, int /*n_in*/, uint64_t n_work) {
+    if (t.v[LP_TUNE_TILE_ELEMS]) {
+        const uint32_t tile = (uint32_t)t.v[LP_TUNE_TILE_ELEMS];
+        return (tile == 1024u || tile == 2048u || tile == 4096u) ? tile : 2048u;
+    }
+    uint32_t tile = 2048u;
+    if ((n_work + tile - 1) / tile < 2u * 148u) tile = 1024u;
     return tile;
 }
 
 cudaError_t lp_direct_launch(const LpArgs &a, const lp_seg_table *segs, const LpTuning &t, int sm_count, LpLaunch *cfg,
                              bool dry_run, cudaStream_t stream) {
-    const uint32_t ctas = t.v[LP_TUNE_CTAS_PER_SM] ? (uint32_t)t.v[LP_TUNE_CTAS_PER_SM] : 4u;
-    uint64_t grid = (uint64_t)sm_count * ctas;
+    uint64_t grid = a.part.n_tiles;  // one CTA per tile
+    if (t.v[LP_TUNE_CTAS_PER_SM]) grid = (uint64_t)sm_count * (uint32_t)t.v[LP_TUNE_CTAS_PER_SM];
     if (t.v[LP_TUNE_GRID_LIMIT] && grid > (uint64_t)t.v[LP_TUNE_GRID_LIMIT]) grid = (uint64_t)t.v[LP_TUNE_GRID_LIMIT];
     if (grid > a.part.n_tiles) grid = a.part.n_tiles;
+    if (grid > 0x7fffffffull) grid = 0x7fffffffull;
     cfg->grid = (uint32_t)grid;
     cfg->threads = kThreads;
     cfg->smem_bytes = 0;

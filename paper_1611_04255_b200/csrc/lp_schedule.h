@@ -47,8 +47,15 @@ LP_HD lp_partition lp_make_partition(uint64_t n, uint64_t block, uint32_t tile) 
 
 // Tile idx -> element range [off, off + len).
 LP_HD void lp_tile_range(const lp_partition &p, uint64_t idx, uint64_t &off, uint32_t &len) {
-    uint64_t k = idx / p.tiles_per_block;       // block index
-    uint64_t j = idx - k * p.tiles_per_block;   // tile within the block
+    uint64_t k, j;  // block index, tile within the block
+    if (((idx | p.tiles_per_block) >> 32) == 0) {  // the common case: a 32-bit division (64-bit ones are emulated on the GPU)
+        const uint32_t k32 = (uint32_t)idx / (uint32_t)p.tiles_per_block;
+        k = k32;
+        j = (uint32_t)idx - k32 * (uint32_t)p.tiles_per_block;
+    } else {
+        k = idx / p.tiles_per_block;
+        j = idx - k * p.tiles_per_block;
+    }
     uint64_t bstart = k * p.block;
     uint64_t bend = bstart + p.block;
     if (bend > p.n) bend = p.n;

@@ -51,14 +51,14 @@ def main(argv=None):
     ap.add_argument("--max-exp", type=int, default=27)
     ap.add_argument("--P", default="2,4,8,16")
     ap.add_argument("--block", type=int, default=65_536)
-    ap.add_argument("--variant", default="pipeline", choices=["pipeline", "direct"],
+    ap.add_argument("--variant", default="auto", choices=["auto", "pipeline", "direct"],
                     help="LP realisation timed in the LP column (default: the library default)")
     ap.add_argument("--algos", default="lp,mst,be")
     args = ap.parse_args(argv)
     assert torch.cuda.is_available(), "the sweep needs a CUDA device"
     dev = torch.device("cuda", 0)
     lp.lib()
-    lp.lp_set_variant({"pipeline": lp.VARIANT_PIPELINE, "direct": lp.VARIANT_DIRECT}[args.variant])
+    lp.lp_set_variant({"auto": lp.VARIANT_AUTO, "pipeline": lp.VARIANT_PIPELINE, "direct": lp.VARIANT_DIRECT}[args.variant])
     algos = tuple(a for a in ALGOS if a in args.algos.split(","))
     peak = 6553.3
     try:

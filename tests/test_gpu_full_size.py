@@ -15,7 +15,7 @@ torch = pytest.importorskip("torch")
 @pytest.fixture(autouse=True)
 def _defaults():
     assert torch.cuda.is_available()
-    lp.lp_set_variant(lp.VARIANT_PIPELINE)
+    lp.lp_set_variant(lp.VARIANT_AUTO)
     for k in range(lp.TUNE_COUNT):
         lp.lp_set_tuning(k, 0)
     yield

@@ -12,19 +12,19 @@ pytestmark = pytest.mark.gpu
 torch = pytest.importorskip("torch")
 
 LP, MST, BE = 0, 1, 2
-VARIANTS = [lp.VARIANT_PIPELINE, lp.VARIANT_DIRECT, lp.VARIANT_COPY_ENGINE]
+VARIANTS = [lp.VARIANT_PIPELINE, lp.VARIANT_DIRECT, lp.VARIANT_COPY_ENGINE, lp.VARIANT_AUTO]
 
 
 @pytest.fixture(autouse=True)
 def _device_and_defaults():
     assert torch.cuda.is_available(), "gpu tests need a CUDA device"
     lp.lib()
-    lp.lp_set_variant(lp.VARIANT_PIPELINE)
+    lp.lp_set_variant(lp.VARIANT_AUTO)
     for k in range(lp.TUNE_COUNT):
         lp.lp_set_tuning(k, 0)
     yield
     torch.cuda.synchronize()
-    lp.lp_set_variant(lp.VARIANT_PIPELINE)
+    lp.lp_set_variant(lp.VARIANT_AUTO)
 
 
 def up(arrs):

@@ -103,7 +103,7 @@ def test_plan_partition_covers_message_exactly(variant, P, n, block):
     try:
         info = lp.lp_plan_query(ALLREDUCE, P, n, block)
     finally:
-        lp.lp_set_variant(lp.VARIANT_PIPELINE)
+        lp.lp_set_variant(lp.VARIANT_AUTO)
     nb = -(-n // block)
     assert info["nb"] == nb
     tile = info["tile_elems"]
@@ -112,7 +112,10 @@ def test_plan_partition_covers_message_exactly(variant, P, n, block):
     last = n - (nb - 1) * blk
     assert info["n_tiles"] == (nb - 1) * tpb + -(-last // tile)
     assert 1 <= info["grid"] <= info["n_tiles"]
-    assert info["grid"] <= info["sm_count"] * 8
+    if variant == lp.VARIANT_PIPELINE:
+        assert info["grid"] <= info["sm_count"] * 8     # persistent CTAs
+    else:
+        assert info["grid"] == info["n_tiles"]           # register variant: one CTA per tile
     assert info["variant"] == variant
     if variant == lp.VARIANT_PIPELINE:  # any block size: tiles that start off a 16-byte boundary get a scalar head / tail
         assert info["smem_bytes"] <= 227 * 1024 and info["stages"] >= 2 and info["out_stages"] >= 1
@@ -198,3 +201,23 @@ def test_optimal_block_minimises_the_lp_cost():
     assert 32e3 < b < 128e3                                   # sqrt(2.44e8 * 1e-7 / (5 * 1e-9)) = 69.9 KB
     assert lp.lp_optimal_block(BCAST, 1, 1e6, 1e-7, 1e-9) == 1e6
     assert lp.lp_optimal_block(BCAST, 4, 1e6, 0.0, 1e-9) == 1e6
+
+
+def test_auto_variant_resolution():
+    # LP_VARIANT_AUTO (the default): register kernel in the latency regime, TMA pipeline for long messages and
+    # whenever the grid is confined
+    L = lp.lib()
+    assert lp.lp_get_variant() == lp.VARIANT_AUTO
+    small = lp.lp_plan_query(ALLREDUCE, 4, 1 << 20, 65_536)          # 32 MB of traffic
+    big = lp.lp_plan_query(ALLREDUCE, 6, 61_000_000, 65_536)         # 2.9 GB
+    assert small["variant"] == lp.VARIANT_DIRECT and small["grid"] == small["n_tiles"]
+    assert big["variant"] == lp.VARIANT_PIPELINE and big["grid"] == 2 * big["sm_count"]
+    assert lp.lp_plan_query(BCAST, 2, 1 << 23, 65_536)["variant"] == lp.VARIANT_PIPELINE      # 64 MB of copy traffic
+    assert lp.lp_plan_query(BCAST, 2, 1 << 22, 65_536)["variant"] == lp.VARIANT_DIRECT
+    assert lp.lp_plan_query(REDUCE, 2, 1 << 24, 65_536)["variant"] == lp.VARIANT_PIPELINE     # 192 MB
+    try:
+        lp.lp_set_tuning(lp.TUNE_GRID_LIMIT, 32)
+        conf = lp.lp_plan_query(ALLREDUCE, 4, 1 << 20, 65_536)
+        assert conf["variant"] == lp.VARIANT_PIPELINE and conf["grid"] <= 32
+    finally:
+        lp.lp_set_tuning(lp.TUNE_GRID_LIMIT, 0)
