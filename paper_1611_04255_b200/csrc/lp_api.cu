@@ -229,7 +229,7 @@ int plan_and_run(int op, float *const *bufs, float *const *weights, float *veloc
     } else if (variant == LP_VARIANT_DIRECT) {
         e = lp_direct_launch(a, tp, g_tuning, sm_count, &cfg, dry_run || noop, stream);
     } else if (variant == LP_VARIANT_CLUSTER) {
-        e = lp_cluster_launch(a, g_tuning, sm_count, &cfg, dry_run || noop, stream);
+        e = layered ? cudaErrorNotSupported : lp_cluster_launch(a, P, root, g_tuning, sm_count, &cfg, dry_run || noop, stream);
         if (e == cudaErrorNotSupported) return LP_ERR_UNSUPPORTED;
     } else {
         e = lp_pipeline_launch(a, tp, g_tuning, sm_count, &cfg, dry_run || noop, stream);

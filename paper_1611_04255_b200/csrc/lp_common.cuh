@@ -64,8 +64,8 @@ cudaError_t lp_pipeline_launch(const LpArgs &a, const lp_seg_table *segs, const 
                                bool dry_run, cudaStream_t stream);
 cudaError_t lp_direct_launch(const LpArgs &a, const lp_seg_table *segs, const LpTuning &t, int sm_count, LpLaunch *cfg,
                              bool dry_run, cudaStream_t stream);
-cudaError_t lp_cluster_launch(const LpArgs &a, const LpTuning &t, int sm_count, LpLaunch *cfg, bool dry_run,
-                              cudaStream_t stream);
+cudaError_t lp_cluster_launch(const LpArgs &a, int P, int root, const LpTuning &t, int sm_count, LpLaunch *cfg,
+                              bool dry_run, cudaStream_t stream);
 uint32_t lp_pipeline_tile(const LpTuning &t, const LpArgs &a, uint64_t n, uint64_t block);
 uint32_t lp_direct_tile(const LpTuning &t, int n_in, uint64_t n_work);
 uint32_t lp_cluster_tile(const LpTuning &t);

@@ -461,6 +461,53 @@ def test_grid_limit_bit_exact(oracle):
 
 
 # ---------------------------------------------------------------------------------------------------
+# stage-per-rank cluster variant: CTA r of a thread-block cluster plays GPU r of Fig. 2
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("P,n,block", [(2, 100_003, 16_384), (3, 70_001, 4096), (4, 1 << 20, 65_536), (6, 300_007, 1001),
+                                       (8, 150_003, 16_384), (16, 200_001, 65_536), (5, 7, 64), (6, 2_000_003, 65_536)])
+def test_cluster_variant_bit_exact(oracle, P, n, block):
+    lp.lp_set_variant(lp.VARIANT_CLUSTER)
+    src = inputs.rank_vectors([13, n], P, n, "uniform")
+    chain = oracle.chain_sum(src)
+    dev = up(src)
+    lp.lp_allreduce(dev, block)
+    assert all(same(g, chain) for g in down(dev)), "allreduce"
+    for root in sorted({0, P // 2, P - 1}):
+        dev = up(src)
+        lp.lp_reduce(dev, block, root=root)
+        got = down(dev)
+        for r in range(P):
+            assert same(got[r], chain if r == root else src[r]), ("reduce", root, r)
+        dev = up(src)
+        lp.lp_broadcast(dev, block, root=root)
+        assert all(same(g, src[root]) for g in down(dev)), ("broadcast", root)
+    grads, weights = inputs.sgd_inputs([14, n], P, n)
+    root = P - 1
+    weights[root] += np.float32(0.5)
+    hw = copies(weights)
+    dg, dw = up(grads), up(weights)
+    for it in range(2):
+        oracle.bsp_sgd_step(grads, hw, root=root, lr=0.01)
+        lp.lp_bsp_sgd_step(dg, dw, block, root=root, lr=0.01)
+        assert all(same(a, b) for a, b in zip(down(dw), hw)), ("sgd", it)
+
+
+def test_cluster_variant_limits():
+    lp.lp_set_variant(lp.VARIANT_CLUSTER)
+    dev = [torch.zeros(4096, device="cuda") for _ in range(17)]
+    with pytest.raises(lp.LpError) as e:
+        lp.lp_allreduce(dev, 1024)                           # P > 16: no cluster that large
+    assert e.value.status == lp.LP_ERR_UNSUPPORTED
+    with pytest.raises(lp.LpError) as e:
+        lp.lp_allreduce_segments(dev[:4], [(0, 100)], 1024)  # layer-wise launches are a pipeline / direct feature
+    assert e.value.status == lp.LP_ERR_UNSUPPORTED
+    vel = torch.zeros(4096, device="cuda")
+    with pytest.raises(lp.LpError) as e:
+        lp.lp_bsp_sgd_momentum_step(dev[:4], dev[4:8], vel, 1024)
+    assert e.value.status == lp.LP_ERR_UNSUPPORTED
+
+
+# ---------------------------------------------------------------------------------------------------
 # MST / BE baselines (a7, a8)
 # ---------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("P,n", [(2, 1001), (3, 70_001), (4, 65_536), (5, 4099), (6, 300_003), (8, 100_001),
