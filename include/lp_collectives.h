@@ -72,7 +72,8 @@ extern "C" {
                                     with mbarrier full/empty flags handed producer warp -> add warps -> store warp */
 #define LP_VARIANT_DIRECT 1      /* one kernel, one CTA per tile, 128-bit register loads/stores, chain fold in registers */
 #define LP_VARIANT_CLUSTER 2     /* stage-per-rank: a thread-block cluster of P CTAs, CTA r owns rank r and hands
-                                    the running partial to CTA r+1 through distributed shared memory (P <= 16) */
+                                    the running partial to CTA r+1 through distributed shared memory (P <= 16;
+                                    broadcast, reduce, allreduce, bsp_sgd_step; no momentum, no layer-wise lists) */
 #define LP_VARIANT_COPY_ENGINE 3 /* the paper's own design: one cudaMemcpyAsync + one add kernel per (hop, block)
                                     on two streams */
 

@@ -5,8 +5,8 @@
 //   reduce half   CTA r loads ITS rank's tile from HBM (TMA bulk load, its "local block"), receives the
 //                               running partial from CTA r-1 in a receive slot of its own shared memory ("writing
 //                               block a0 to a buffer on GPU1"), adds, and writes the new partial into a receive slot
-//                               of CTA r+1 through distributed shared memory (st.shared::cluster + a remote mbarrier
-//                               arrive: the block-ready flag).  The last CTA holds the finished tile a''.
+//                               of CTA r+1 through distributed shared memory (st.async: the store itself completes
+//                               transaction bytes on CTA r+1's mbarrier, the block-ready flag).  The last CTA holds a''.
 //   broadcast half  the finished tile flows back down the chain, CTA x -> CTA x-1 (U3 reading A,
 //                               reverse flow); every CTA on the way stores it to its own rank's buffer (TMA bulk
 //                               store) -- so each rank's HBM traffic is issued by "its" CTA, as on the real machine.
@@ -24,12 +24,12 @@
 
 namespace {
 
-constexpr int kFoldWarps = 4;
-constexpr int kRetWarps = 4;
+constexpr int kFoldWarps = 8;
+constexpr int kRetWarps = 8;
 constexpr int kClThreads = (2 + kFoldWarps + kRetWarps) * 32;  // producer, store, fold, return
 constexpr int kV = 4;                                          // float4 per fold / return thread
-constexpr int kClTile = kV * 4 * kFoldWarps * 32;              // 2048 elements
-constexpr int kSIn = 6, kSRv = 3, kSFin = 4;
+constexpr int kClTile = kV * 4 * kFoldWarps * 32;              // 4096 elements
+constexpr int kSIn = 6, kSRv = 4, kSFin = 4;
 
 struct LpClusterArgs {
     const float *in_of[16];  // what cluster CTA x loads (NULL: nothing)
@@ -52,29 +52,18 @@ __device__ __forceinline__ uint32_t cl_map(const void *local, uint32_t cta) {  /
     asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(lp_smem_u32(local)), "r"(cta));
     return r;
 }
+// Signals between neighbours.  Data goes by st.async: a 16-byte store into the neighbour's shared memory that
+// completes 16 transaction bytes on the neighbour's mbarrier -- the hardware's own "block ready" flag, no fences.
+// Credits ("I am done reading your slot") are plain remote arrives.  Cluster-scope acquire / release on every wait
+// and arrive would be correct too and was the first version: it compiles to MEMBAR.ALL.GPU + CCTL.IVALL per hop.
 __device__ __forceinline__ void cl_arrive(uint64_t *bar, uint32_t cta) {  // arrive on `bar` of CTA `cta` (may be me)
-    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cl_map(bar, cta)) : "memory");
+    asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cl_map(bar, cta)) : "memory");
 }
-__device__ __forceinline__ void cl_wait(uint64_t *bar, uint32_t parity) {  // local barrier, cluster-scope acquire
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "CL_WAIT_%=:\n"
-        "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra CL_DONE_%=;\n"
-        "bra CL_WAIT_%=;\n"
-        "CL_DONE_%=:\n"
-        "}\n" ::"r"(lp_smem_u32(bar)),
-        "r"(parity)
-        : "memory");
-}
-__device__ __forceinline__ void cl_store4(uint32_t remote, const float4 &v) {
-    asm volatile("st.shared::cluster.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(remote), "f"(v.x), "f"(v.y), "f"(v.z),
-                 "f"(v.w)
+__device__ __forceinline__ void cl_store4_async(uint32_t remote, const float4 &v, uint32_t remote_bar) {
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v4.f32 [%0], {%1, %2, %3, %4}, [%5];" ::"r"(remote),
+                 "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w), "r"(remote_bar)
                  : "memory");
 }
-__device__ __forceinline__ void cl_fence() { asm volatile("fence.acq_rel.cluster;" ::: "memory"); }
-__device__ __forceinline__ void cl_fence_proxy_async_all() { asm volatile("fence.proxy.async;" ::: "memory"); }
 
 struct ClRing {
     int slot;
@@ -116,16 +105,21 @@ __global__ void __launch_bounds__(kClThreads)
             lp_mbar_init(&in_empty[s], kFoldWarps);
         }
         for (int s = 0; s < kSRv; ++s) {
-            lp_mbar_init(&rv_full[s], kFoldWarps);
+            lp_mbar_init(&rv_full[s], 1);  // my own arrive.expect_tx; the bytes come from CTA x-1's st.async
             lp_mbar_init(&send_credit[s], kFoldWarps);
         }
         const int dn = x > 0 ? consumers(x - 1) : 0, own = consumers(x);
         for (int s = 0; s < kSFin; ++s) {
-            lp_mbar_init(&fin_full[s], head ? (c.head_tma ? 1 : kFoldWarps) : kRetWarps);
+            lp_mbar_init(&fin_full[s], head ? (c.head_tma ? 1 : kFoldWarps) : 1);
             lp_mbar_init(&dn_credit[s], dn > 0 ? dn : 1);
             lp_mbar_init(&own_credit[s], own > 0 ? own : 1);
         }
         lp_fence_mbar_init();
+        // arm the rings my neighbours write into: one tile of transaction bytes per slot and phase
+        if (c.fold && x > 0)
+            for (int s = 0; s < kSRv; ++s) lp_mbar_expect_tx(&rv_full[s], kClTile * 4u);
+        if (c.ret && !head)
+            for (int s = 0; s < kSFin; ++s) lp_mbar_expect_tx(&fin_full[s], kClTile * 4u);
     }
     cooperative_groups::this_cluster().sync();  // every barrier of the cluster exists before anyone signals remotely
 
@@ -160,7 +154,7 @@ __global__ void __launch_bounds__(kClThreads)
                         in.advance();
                     }
                 } else if (head) {  // broadcast: the root's tile is the finished tile
-                    cl_wait(&own_credit[fin.slot], fin.phase ^ 1u);
+                    lp_mbar_wait(&own_credit[fin.slot], fin.phase ^ 1u);
                     if (bytes) {
                         lp_mbar_expect_tx(&fin_full[fin.slot], bytes);
                         lp_bulk_g2s(fin_ring + fin.slot * kClTile, c.in_of[x] + span.a0, bytes, &fin_full[fin.slot]);
@@ -182,11 +176,12 @@ __global__ void __launch_bounds__(kClThreads)
                 uint32_t len;
                 lp_tile_range(part, t, off, len);
                 const LpTileSpan span(off, len);
-                cl_wait(&fin_full[fin.slot], fin.phase);
+                lp_mbar_wait(&fin_full[fin.slot], fin.phase);
                 lp_fence_proxy_async();
                 if (span.body) lp_bulk_s2g(c.out_of[x] + span.a0, fin_ring + fin.slot * kClTile, span.body * 4u);
                 lp_bulk_commit();
                 lp_bulk_wait_read<0>();
+                if (!head && !fwd_me) lp_mbar_expect_tx(&fin_full[fin.slot], kClTile * 4u);  // CTA 0: nobody else re-arms
                 if (head)
                     lp_mbar_arrive(&own_credit[fin.slot]);
                 else
@@ -212,26 +207,31 @@ __global__ void __launch_bounds__(kClThreads)
 #pragma unroll
                     for (int v = 0; v < kV; ++v) acc[v] = s[ftid + v * FT];
                 }
+                // A slot is handed back only after the shared-memory reads of it have RETURNED: this SM's load/store
+                // queue is busy with the neighbours' st.async traffic, and an mbarrier arrive does not wait for
+                // loads that are still queued -- without the fence the refill of the slot overtook them (seen as
+                // "rank r's term taken from the tile kSIn rounds ahead" in ~1 of 10 runs at P >= 3).
+                __threadfence_block();
                 __syncwarp();
                 if (lane == 0) lp_mbar_arrive(&in_empty[in.slot]);
                 in.advance();
                 if (x > 0) {  // a' = (what GPU x-1 sent) + my block, in that order (chain order)
-                    cl_wait(&rv_full[rv.slot], rv.phase);
+                    lp_mbar_wait(&rv_full[rv.slot], rv.phase);
                     const float4 *s = reinterpret_cast<const float4 *>(rv_ring + rv.slot * kClTile);
 #pragma unroll
                     for (int v = 0; v < kV; ++v) acc[v] = lp_add4(s[ftid + v * FT], acc[v]);
+                    __threadfence_block();  // my reads of the slot have returned before the credit leaves (see below)
                     __syncwarp();
+                    if (ftid == 0) lp_mbar_expect_tx(&rv_full[rv.slot], kClTile * 4u);  // re-arm for the slot's next use
                     if (lane == 0) cl_arrive(&send_credit[rv.slot], (uint32_t)x - 1u);
                     rv.advance();
                 }
                 if (!head) {
-                    cl_wait(&send_credit[snd.slot], snd.phase ^ 1u);
+                    lp_mbar_wait(&send_credit[snd.slot], snd.phase ^ 1u);
                     const uint32_t dst = cl_map(rv_ring + snd.slot * kClTile, (uint32_t)x + 1u);
+                    const uint32_t flag = cl_map(&rv_full[snd.slot], (uint32_t)x + 1u);
 #pragma unroll
-                    for (int v = 0; v < kV; ++v) cl_store4(dst + (uint32_t)(ftid + v * FT) * 16u, acc[v]);
-                    cl_fence();
-                    __syncwarp();
-                    if (lane == 0) cl_arrive(&rv_full[snd.slot], (uint32_t)x + 1u);
+                    for (int v = 0; v < kV; ++v) cl_store4_async(dst + (uint32_t)(ftid + v * FT) * 16u, acc[v], flag);
                     snd.advance();
                 } else {
                     if (sgd) {  // g = S/P, w' = w_root - lr g, applied where the chain ends
@@ -239,11 +239,12 @@ __global__ void __launch_bounds__(kClThreads)
                         const float4 *s = reinterpret_cast<const float4 *>(in_ring + in.slot * kClTile);
 #pragma unroll
                         for (int v = 0; v < kV; ++v) acc[v] = lp_sgd4(acc[v], s[ftid + v * FT], a.lr, a.invP);
+                        __threadfence_block();
                         __syncwarp();
                         if (lane == 0) lp_mbar_arrive(&in_empty[in.slot]);
                         in.advance();
                     }
-                    cl_wait(&own_credit[fin.slot], fin.phase ^ 1u);
+                    lp_mbar_wait(&own_credit[fin.slot], fin.phase ^ 1u);
                     float4 *o = reinterpret_cast<float4 *>(fin_ring + fin.slot * kClTile);
 #pragma unroll
                     for (int v = 0; v < kV; ++v) o[ftid + v * FT] = acc[v];
@@ -266,13 +267,15 @@ __global__ void __launch_bounds__(kClThreads)
             ClRing fin(kSFin), dn(kSFin);
             for (uint64_t t = cid; t < part.n_tiles; t += n_clusters) {
                 float4 r4[kV];
-                cl_wait(&fin_full[fin.slot], fin.phase);
+                lp_mbar_wait(&fin_full[fin.slot], fin.phase);
                 {
                     const float4 *s = reinterpret_cast<const float4 *>(fin_ring + fin.slot * kClTile);
 #pragma unroll
                     for (int v = 0; v < kV; ++v) r4[v] = s[rtid + v * RT];
                 }
+                __threadfence_block();  // my reads of the slot have returned before the credit leaves (see below)
                 __syncwarp();
+                if (!head && rtid == 0) lp_mbar_expect_tx(&fin_full[fin.slot], kClTile * 4u);  // re-arm (I am the one who does)
                 if (lane == 0) {
                     if (head)
                         lp_mbar_arrive(&own_credit[fin.slot]);
@@ -280,14 +283,11 @@ __global__ void __launch_bounds__(kClThreads)
                         cl_arrive(&dn_credit[fin.slot], (uint32_t)x + 1u);
                 }
                 fin.advance();
-                cl_wait(&dn_credit[dn.slot], dn.phase ^ 1u);
+                lp_mbar_wait(&dn_credit[dn.slot], dn.phase ^ 1u);
                 const uint32_t dst = cl_map(fin_ring + dn.slot * kClTile, (uint32_t)x - 1u);
+                const uint32_t flag = cl_map(&fin_full[dn.slot], (uint32_t)x - 1u);
 #pragma unroll
-                for (int v = 0; v < kV; ++v) cl_store4(dst + (uint32_t)(rtid + v * RT) * 16u, r4[v]);
-                cl_fence();
-                cl_fence_proxy_async_all();  // CTA x-1's bulk store (async proxy) will read what these generic stores wrote
-                __syncwarp();
-                if (lane == 0) cl_arrive(&fin_full[dn.slot], (uint32_t)x - 1u);
+                for (int v = 0; v < kV; ++v) cl_store4_async(dst + (uint32_t)(rtid + v * RT) * 16u, r4[v], flag);
                 dn.advance();
             }
         }

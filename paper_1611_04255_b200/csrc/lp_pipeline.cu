@@ -202,6 +202,9 @@ __global__ void __launch_bounds__((CW + 2) * 32)
                 const float4 *s = reinterpret_cast<const float4 *>(in_ring + (size_t)ring.slot * TILE);
 #pragma unroll
                 for (int v = 0; v < V; ++v) acc[v] = s[ctid + v * CT];
+                // nothing consumes these loads before the slot is handed back: make sure they have returned (an
+                // mbarrier arrive does not wait for queued shared-memory loads; lp_cluster.cu has the measured case)
+                __threadfence_block();
                 __syncwarp();
                 if (lane == 0) lp_mbar_arrive(&empty[ring.slot]);
                 ring.advance();
@@ -235,6 +238,7 @@ __global__ void __launch_bounds__((CW + 2) * 32)
 #pragma unroll
                     for (int v = 0; v < V; ++v) w[v] = s[ctid + v * CT];
                 }
+                __threadfence_block();
                 __syncwarp();
                 if (lane == 0) lp_mbar_arrive(&empty[ring.slot]);
                 ring.advance();

@@ -492,6 +492,22 @@ def test_cluster_variant_bit_exact(oracle, P, n, block):
         assert all(same(a, b) for a, b in zip(down(dw), hw)), ("sgd", it)
 
 
+@pytest.mark.parametrize("P,n", [(3, 3_000_003), (6, 2_000_003), (16, 1_000_003)])
+def test_cluster_variant_under_backpressure(oracle, P, n):
+    # many tiles per cluster: the rings wrap dozens of times and the middle CTAs of the chain run back-pressured by
+    # both halves of the allreduce.  This is the case that exposed a slot handed back before its shared-memory
+    # reads had returned (one warp row of one tile wrong in ~1 of 10 runs): repeat it.
+    lp.lp_set_variant(lp.VARIANT_CLUSTER)
+    src = inputs.rank_vectors([15, n], P, n, "uniform")
+    want = oracle.chain_sum(src)
+    pristine = up(src)
+    for it in range(15):
+        dev = [p.clone() for p in pristine]
+        lp.lp_allreduce(dev, 65_536)
+        for r, g in enumerate(down(dev)):
+            assert same(g, want), (it, r, int(np.count_nonzero(g != want)))
+
+
 def test_cluster_variant_limits():
     lp.lp_set_variant(lp.VARIANT_CLUSTER)
     dev = [torch.zeros(4096, device="cuda") for _ in range(17)]
