@@ -34,7 +34,7 @@ UNIT = "GB/s (algbw = n*4 bytes per rank / time; roofline on min bytes 2*P*n*4)"
 FALLBACK_HBM_GBS = 6650.0  # B200_PROFILING.md fallback, used only if MEASURED_PEAKS.json is absent
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` capture (profiles/r1_ncu_lp_pipeline.md); keyed by (P, n, variant)
-NCU_TRAFFIC_BYTES = {(6, 61_000_000, "pipeline"): 2_868_976_000}
+NCU_TRAFFIC_BYTES = {(6, 61_000_000, "pipeline"): 2_869_976_000}
 
 
 def parse_args():
@@ -353,7 +353,7 @@ def secondary(torch, lp, dev, pristine, work, P, n, block, peak):
     out["lp_reduce_root0"] = measure(lambda: lp.lp_reduce(work, block, root=0), mb(lp.OP_REDUCE))
     out["lp_broadcast_root0"] = measure(lambda: lp.lp_broadcast(work, block, root=0), mb(lp.OP_BROADCAST))
     cur = lp.lp_get_variant()
-    for name, v in (("pipeline", lp.VARIANT_PIPELINE), ("direct", lp.VARIANT_DIRECT)):
+    for name, v in (("pipeline", lp.VARIANT_PIPELINE), ("direct", lp.VARIANT_DIRECT), ("cluster", lp.VARIANT_CLUSTER)):
         lp.lp_set_variant(v)
         out[f"lp_allreduce_{name}"] = measure(lambda: lp.lp_allreduce(work, block), mb(lp.OP_ALLREDUCE))
     lp.lp_set_variant(cur)
