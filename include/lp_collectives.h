@@ -101,7 +101,9 @@ extern "C" {
 #define LP_TUNE_GRID_LIMIT 8    /* at most this many persistent CTAs per launch (0 = one grid-full: SMs x CTAs per SM).
                                    A collective that runs beside compute kernels (lp_comm_*) can be confined to a
                                    few SMs' worth of CTAs, the way NCCL confines itself to a few channels */
-#define LP_TUNE_COUNT 9
+#define LP_TUNE_NO_PDL 9        /* 1: launch kernels without programmatic dependent launch (default 0: back-to-back
+                                   collectives overlap launch latency and prologue with their predecessor's tail) */
+#define LP_TUNE_COUNT 10
 
 /* ---- LP collectives (the hot path) ----------------------------------------- */
 

@@ -18,8 +18,8 @@ OP_BROADCAST, OP_REDUCE, OP_ALLREDUCE, OP_BSP_SGD, OP_BSP_SGD_MOM = 0, 1, 2, 3, 
 VARIANT_PIPELINE, VARIANT_DIRECT, VARIANT_CLUSTER, VARIANT_COPY_ENGINE, VARIANT_AUTO = 0, 1, 2, 3, 4
 MODEL_STAGE, MODEL_LINK, MODEL_LINK_RING = 0, 1, 2
 TUNE_TILE_ELEMS, TUNE_STAGES, TUNE_OUT_STAGES, TUNE_CTAS_PER_SM, TUNE_CE_STREAMS, TUNE_L2_HINT, TUNE_STORE_WAIT, \
-    TUNE_SCHED, TUNE_GRID_LIMIT = range(9)
-TUNE_COUNT = 9
+    TUNE_SCHED, TUNE_GRID_LIMIT, TUNE_NO_PDL = range(10)
+TUNE_COUNT = 10
 VARIANT_NAMES = {0: "pipeline", 1: "direct", 2: "cluster", 3: "copy_engine"}
 
 

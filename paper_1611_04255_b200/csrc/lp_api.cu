@@ -23,7 +23,7 @@ namespace {
 
 std::mutex g_mu;
 int g_variant = LP_VARIANT_AUTO;
-LpTuning g_tuning = {{0, 0, 0, 0, 0, 0, 0, 0, 0}};
+LpTuning g_tuning = {{0, 0, 0, 0, 0, 0, 0, 0, 0, 0}};
 std::atomic<uint64_t> g_launches{0};
 char g_err[256] = "";
 int g_sm_count = 0;  // 0 = not queried yet
@@ -349,6 +349,8 @@ int run_baseline(bool be, int op, float *const *bufs, int P, size_t n, int root,
 
 }  // namespace
 
+bool lp_pdl_enabled() { return g_tuning.v[LP_TUNE_NO_PDL] == 0; }
+
 void lp_count_launch(uint64_t k) { g_launches.fetch_add(k, std::memory_order_relaxed); }
 
 // Called with g_mu held.  The ring is allocated and zeroed once (synchronously: before any launch that uses it).
@@ -670,6 +672,7 @@ int lp_set_tuning(int key, int value) {
             break;
         case LP_TUNE_STORE_WAIT:
         case LP_TUNE_SCHED:
+        case LP_TUNE_NO_PDL:
             if (value > 1) return LP_ERR_INVALID_ARG;
             break;
         case LP_TUNE_GRID_LIMIT:

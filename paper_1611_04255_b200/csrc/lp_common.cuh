@@ -3,6 +3,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <string.h>
 
 #include "../../include/lp_collectives.h"
 #include "lp_schedule.h"
@@ -50,6 +51,7 @@ struct LpSegParam<true> {
 
 struct LpLaunch {
     uint32_t grid, threads, smem_bytes, stages, out_stages;
+    bool pdl;
 };
 
 // Tuning state resolved by the API layer (0 = default).
@@ -84,12 +86,40 @@ cudaError_t lp_seg_launch(const LpSegJob *jobs, int n_jobs, int sm_count, cudaSt
 cudaError_t lp_update_launch(float *w, const float *S, float *velocity, uint64_t n, float lr, float invP, float mu,
                              cudaStream_t stream);
 
+// Programmatic dependent launch: every kernel of the library is launched with the "programmatic stream
+// serialization" attribute, tells the runtime when its CTAs have nothing left to claim (lp_pdl_trigger) and waits
+// for its predecessor in the stream before touching global memory (lp_pdl_wait).  Back-to-back collectives (layer-wise
+// lists, MST / BE levels, reduce -> update -> broadcast) then overlap their launch latency and prologue with the
+// predecessor's tail; a predecessor that never triggers (any other kernel) simply completes first, as always.
+// `pdl` = false (LP_TUNE_NO_PDL) launches the classic way.
+template <typename... KArgs, typename... Args>
+cudaError_t lp_launch(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream, bool pdl,
+                      Args &&...args) {
+    cudaLaunchConfig_t lc;
+    memset(&lc, 0, sizeof(lc));
+    lc.gridDim = grid;
+    lc.blockDim = block;
+    lc.dynamicSmemBytes = smem;
+    lc.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    lc.attrs = attr;
+    lc.numAttrs = pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&lc, kernel, static_cast<KArgs>(args)...);
+}
+
+bool lp_pdl_enabled();  // LP_TUNE_NO_PDL == 0 (read by launchers that do not get the tuning block)
+
 // Launch counter (kernels + async copies enqueued by the library).
 void lp_count_launch(uint64_t k);
 // A zeroed, self-resetting {claimed, finished} counter pair for one launch (see LpArgs::sched).
 cudaError_t lp_sched_acquire(unsigned long long **pair);
 
 #if defined(__CUDACC__)
+__device__ __forceinline__ void lp_pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void lp_pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 // ---- PTX wrappers ------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t lp_smem_u32(const void *p) {
     return (uint32_t)__cvta_generic_to_shared(p);

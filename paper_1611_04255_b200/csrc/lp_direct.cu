@@ -21,6 +21,10 @@ __global__ void __launch_bounds__(kThreads)
     // whichever SM frees up first -- the same balance the pipeline kernel gets from its tile claims, with no
     // per-CTA setup at all, which is what the latency regime wants.  A confined grid (LP_TUNE_GRID_LIMIT /
     // LP_TUNE_CTAS_PER_SM) walks the tile list round robin.
+    // wait first, then trigger: at most ONE successor waits behind a running kernel (triggering before the wait lets
+    // a whole queue of short kernels pile up on the SMs, each blocked on its predecessor: measured 2x slower at 256 KB)
+    lp_pdl_wait();
+    lp_pdl_trigger();  // every CTA of this grid is resident or done once the last one gets here
     for (uint64_t t = blockIdx.x; t < a.part.n_tiles; t += gridDim.x) {
         uint64_t off;
         uint32_t len;
@@ -91,8 +95,7 @@ template <int V, bool SEG>
 cudaError_t launch_v(const LpArgs &a, const typename LpSegParam<SEG>::type &segs, const LpLaunch &cfg, cudaStream_t stream) {
 #define LP_DIRECT_CASE(NS)                                                                  \
     case NS:                                                                                \
-        lp_direct_kernel<NS, V, SEG><<<cfg.grid, cfg.threads, 0, stream>>>(a, segs);       \
-        break;
+        return lp_launch(lp_direct_kernel<NS, V, SEG>, dim3(cfg.grid), dim3(cfg.threads), 0, stream, cfg.pdl, a, segs);
     switch (a.n_sum) {
         LP_DIRECT_CASE(1)
         LP_DIRECT_CASE(2)
@@ -102,11 +105,9 @@ cudaError_t launch_v(const LpArgs &a, const typename LpSegParam<SEG>::type &segs
         LP_DIRECT_CASE(8)
         LP_DIRECT_CASE(16)
         default:
-            lp_direct_kernel<0, V, SEG><<<cfg.grid, cfg.threads, 0, stream>>>(a, segs);
-            break;
+            return lp_launch(lp_direct_kernel<0, V, SEG>, dim3(cfg.grid), dim3(cfg.threads), 0, stream, cfg.pdl, a, segs);
     }
 #undef LP_DIRECT_CASE
-    return cudaGetLastError();
 }
 
 template <int V>
@@ -141,6 +142,7 @@ cudaError_t lp_direct_launch(const LpArgs &a, const lp_seg_table *segs, const Lp
     cfg->smem_bytes = 0;
     cfg->stages = 0;
     cfg->out_stages = 0;
+    cfg->pdl = t.v[LP_TUNE_NO_PDL] == 0;
     if (dry_run || grid == 0) return cudaSuccess;
     lp_count_launch(1);
     switch (a.part.tile) {

@@ -97,6 +97,7 @@ __global__ void __launch_bounds__((CW + 2) * 32)
         lp_fence_mbar_init();
     }
     __syncthreads();
+    lp_pdl_wait();  // the predecessor in the stream has completed and its writes are visible (no-op without PDL)
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
@@ -111,6 +112,7 @@ __global__ void __launch_bounds__((CW + 2) * 32)
             for (;;) {
                 const uint64_t t = claimer.claim();
                 if (t >= a.part.n_tiles) {  // end marker
+                    lp_pdl_trigger();  // nothing left to claim here: the next kernel's CTAs may start their prologue
                     lp_mbar_wait(&empty[ring.slot], ring.phase ^ 1u);
                     meta_len[ring.slot] = kEndLen;
                     lp_mbar_arrive(&full[ring.slot]);
@@ -308,6 +310,7 @@ __global__ void __launch_bounds__(64)
         lp_fence_mbar_init();
     }
     __syncthreads();
+    lp_pdl_wait();
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
     if (warp == 0 && lane == 0) {
@@ -317,6 +320,7 @@ __global__ void __launch_bounds__(64)
         LpTileClaimer claimer(a.sched, a.part.n_tiles);
         for (;;) {
             const uint64_t t = claimer.claim();
+            if (t >= a.part.n_tiles) lp_pdl_trigger();
             lp_mbar_wait(&empty[ring.slot], ring.phase ^ 1u);
             if (t >= a.part.n_tiles) {  // end marker
                 meta_len[ring.slot] = kEndLen;
@@ -391,9 +395,8 @@ cudaError_t launch_fold_t(const LpArgs &a, const typename LpSegParam<SEG>::type 
         if (e != cudaSuccess) return e;
         attr_bytes = (int)cfg.smem_bytes;
     }
-    lp_pipeline_kernel<V, CW, SEG><<<cfg.grid, cfg.threads, cfg.smem_bytes, stream>>>(a, segs, (int)cfg.stages,
-                                                                                       (int)cfg.out_stages);
-    return cudaGetLastError();
+    return lp_launch(lp_pipeline_kernel<V, CW, SEG>, dim3(cfg.grid), dim3(cfg.threads), cfg.smem_bytes, stream, cfg.pdl, a,
+                     segs, (int)cfg.stages, (int)cfg.out_stages);
 }
 
 template <int V, int CW>
@@ -412,8 +415,8 @@ cudaError_t launch_bcast_t(const LpArgs &a, const typename LpSegParam<SEG>::type
         if (e != cudaSuccess) return e;
         attr_bytes = (int)cfg.smem_bytes;
     }
-    lp_bcast_kernel<SEG><<<cfg.grid, cfg.threads, cfg.smem_bytes, stream>>>(a, segs, (int)cfg.stages, (int)tile);
-    return cudaGetLastError();
+    return lp_launch(lp_bcast_kernel<SEG>, dim3(cfg.grid), dim3(cfg.threads), cfg.smem_bytes, stream, cfg.pdl, a, segs,
+                     (int)cfg.stages, (int)tile);
 }
 
 constexpr uint32_t kSmemPerSm = 228u * 1024u;   // sm_100: 228 KB per SM, 227 KB max per CTA, 1 KB reserved per CTA
@@ -501,6 +504,7 @@ cudaError_t lp_pipeline_launch(const LpArgs &a, const lp_seg_table *segs, const 
     cfg->smem_bytes = smem_of(stages, out_stages);
     cfg->stages = stages;
     cfg->out_stages = out_stages;
+    cfg->pdl = t.v[LP_TUNE_NO_PDL] == 0;
     if (dry_run || grid == 0) return cudaSuccess;
 
     lp_count_launch(1);

@@ -15,6 +15,8 @@ constexpr int kSegThreads = 256;
 constexpr int kSegUnroll = 4;
 
 __global__ void __launch_bounds__(kSegThreads) lp_seg_kernel(const __grid_constant__ LpSegArgs s) {
+    lp_pdl_wait();     // the previous level (or whatever precedes in the stream) has completed
+    lp_pdl_trigger();  // one chunk per CTA: once the last CTA is resident the next level's kernel may be scheduled
     const LpSegJob &job = s.j[blockIdx.y];
     float *dst = job.dst;
     const float *a = job.a;
@@ -64,6 +66,8 @@ __global__ void __launch_bounds__(kSegThreads) lp_seg_kernel(const __grid_consta
 // path for misaligned ends.  Same rounded operations as the fused epilogues (lp_sgd1 / lp_mom1).
 __global__ void __launch_bounds__(kSegThreads) lp_update_kernel(float *w, const float *S, float *vel, uint64_t n, float lr,
                                                                 float invP, float mu) {
+    lp_pdl_wait();
+    lp_pdl_trigger();
     const uint64_t nvec = n >> 2;
     const uint64_t v = (uint64_t)blockIdx.x * kSegThreads + threadIdx.x;
     if (v < nvec) {
@@ -100,8 +104,8 @@ cudaError_t lp_update_launch(float *w, const float *S, float *velocity, uint64_t
     const uint64_t blocks = ((n >> 2) + kSegThreads - 1) / kSegThreads + ((n >> 2) == 0 ? 1 : 0);
     if (blocks > 0x7fffffffull) return cudaErrorInvalidValue;
     lp_count_launch(1);
-    lp_update_kernel<<<(unsigned)blocks, kSegThreads, 0, stream>>>(w, S, velocity, n, lr, invP, mu);
-    return cudaGetLastError();
+    return lp_launch(lp_update_kernel, dim3((unsigned)blocks), dim3(kSegThreads), 0, stream, lp_pdl_enabled(), w, S, velocity,
+                     (uint64_t)n, lr, invP, mu);
 }
 
 cudaError_t lp_seg_launch(const LpSegJob *jobs, int n_jobs, int sm_count, cudaStream_t stream) {
@@ -122,6 +126,5 @@ cudaError_t lp_seg_launch(const LpSegJob *jobs, int n_jobs, int sm_count, cudaSt
     if (per_job > 0x7fffffffull) return cudaErrorInvalidValue;
     dim3 grid((unsigned)per_job, (unsigned)m, 1);
     lp_count_launch(1);
-    lp_seg_kernel<<<grid, kSegThreads, 0, stream>>>(s);
-    return cudaGetLastError();
+    return lp_launch(lp_seg_kernel, grid, dim3(kSegThreads), 0, stream, lp_pdl_enabled(), s);
 }
