@@ -32,6 +32,9 @@
  *     allocated lazily and freed by lp_shutdown().
  *   - There is no CPU fallback: without a CUDA device the compute entry points
  *     return LP_ERR_CUDA.
+ *   * One device per process: the library binds to the CUDA device that is current at its first compute call
+ *     (scratch, tile-claim counters and streams live there); a call with another device current returns
+ *     LP_ERR_UNSUPPORTED; lp_shutdown() unbinds.  Calls are serialised by one library-wide mutex.
  */
 #ifndef LP_COLLECTIVES_H
 #define LP_COLLECTIVES_H
@@ -54,7 +57,8 @@ extern "C" {
 #define LP_OK 0
 #define LP_ERR_INVALID_ARG 1 /* P<1, P>LP_MAX_P, NULL pointer, block==0, root out of range,
                                 misaligned or overlapping buffers, unknown enum value */
-#define LP_ERR_UNSUPPORTED 2 /* BE with non-power-of-two P (U14); cluster variant with P it cannot hold */
+#define LP_ERR_UNSUPPORTED 2 /* BE with non-power-of-two P (U14); cluster variant: P > 16, momentum, slice lists;
+                                a call from a device other than the one the library is bound to */
 #define LP_ERR_CUDA 3        /* launch / allocation / copy failure, or no device */
 
 #define LP_MAX_P 32

@@ -45,20 +45,35 @@ int cuda_fail(cudaError_t e, const char *where) {
     return LP_ERR_CUDA;
 }
 
-// SM count of the current device; <= 0 when there is no usable device.
+// SM count of the current device; <= 0 when there is no usable device.  The library binds to the device that is
+// current at its first call (its scratch, tile-claim counters and streams live there: one process per GPU); a call
+// made with another device current is refused (-1) rather than allowed to touch the wrong device's memory.
+int g_device = -1;
 int sm_count_or_fail() {
-    if (g_sm_count > 0) return g_sm_count;
     int dev = 0, sms = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) {
         cudaGetLastError();
         return 0;
     }
+    if (g_sm_count > 0) return dev == g_device ? g_sm_count : -1;
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
         cudaGetLastError();
         return 0;
     }
     g_sm_count = sms;
+    g_device = dev;
     return sms;
+}
+
+// Message for a failed sm_count_or_fail().
+int no_device(int sms) {
+    if (sms < 0) {
+        snprintf(g_err, sizeof(g_err), "liblp_b200 is bound to CUDA device %d (one process per GPU); call lp_shutdown() before using another",
+                 g_device);
+        return LP_ERR_UNSUPPORTED;
+    }
+    snprintf(g_err, sizeof(g_err), "no CUDA device: liblp_b200 has no CPU fallback");
+    return LP_ERR_CUDA;
 }
 
 bool aligned16(const void *p) { return ((uintptr_t)p & 15u) == 0; }
@@ -257,10 +272,7 @@ int run_device(int op, float *const *bufs, float *const *weights, float *velocit
     std::lock_guard<std::mutex> lock(g_mu);
     if (g_variant == LP_VARIANT_CLUSTER && P > 16) return LP_ERR_UNSUPPORTED;
     const int sms = sm_count_or_fail();
-    if (sms <= 0) {
-        snprintf(g_err, sizeof(g_err), "no CUDA device: liblp_b200 has no CPU fallback");
-        return LP_ERR_CUDA;
-    }
+    if (sms <= 0) return no_device(sms);
     return plan_and_run(op, bufs, weights, velocity, P, n, block, root, lr, mu, sms, nullptr, false,
                         (cudaStream_t)cuda_stream);
 }
@@ -275,10 +287,7 @@ int run_alg2(float *const *grads, float *const *weights, float *velocity, int P,
     std::lock_guard<std::mutex> lock(g_mu);
     if (g_variant == LP_VARIANT_CLUSTER && P > 16) return LP_ERR_UNSUPPORTED;
     const int sms = sm_count_or_fail();
-    if (sms <= 0) {
-        snprintf(g_err, sizeof(g_err), "no CUDA device: liblp_b200 has no CPU fallback");
-        return LP_ERR_CUDA;
-    }
+    if (sms <= 0) return no_device(sms);
     cudaStream_t st = (cudaStream_t)cuda_stream;
     rc = plan_and_run(LP_OP_REDUCE, grads, nullptr, nullptr, P, n, block, root, 0.f, 0.f, sms, nullptr, false, st);
     if (rc != LP_OK) return rc;
@@ -308,10 +317,7 @@ int run_segments(int op, float *const *bufs, int P, size_t n, const size_t *seg_
     std::lock_guard<std::mutex> lock(g_mu);
     if (g_variant == LP_VARIANT_CLUSTER) return LP_ERR_UNSUPPORTED;
     const int sms = sm_count_or_fail();
-    if (sms <= 0) {
-        snprintf(g_err, sizeof(g_err), "no CUDA device: liblp_b200 has no CPU fallback");
-        return LP_ERR_CUDA;
-    }
+    if (sms <= 0) return no_device(sms);
     size_t off[LP_MAX_SEGS], len[LP_MAX_SEGS];
     int m = 0;
     for (int s = 0; s <= n_seg; ++s) {
@@ -337,10 +343,7 @@ int run_baseline(bool be, int op, float *const *bufs, int P, size_t n, int root,
     if (be && (P & (P - 1)) != 0) return LP_ERR_UNSUPPORTED;  // U14
     std::lock_guard<std::mutex> lock(g_mu);
     const int sms = sm_count_or_fail();
-    if (sms <= 0) {
-        snprintf(g_err, sizeof(g_err), "no CUDA device: liblp_b200 has no CPU fallback");
-        return LP_ERR_CUDA;
-    }
+    if (sms <= 0) return no_device(sms);
     cudaError_t e = be ? lp_be_run(op, bufs, P, n, root, sms, (cudaStream_t)cuda_stream)
                        : lp_mst_run(op, bufs, P, n, root, sms, (cudaStream_t)cuda_stream);
     if (e != cudaSuccess) return cuda_fail(e, be ? "BE baseline" : "MST baseline");
@@ -428,10 +431,7 @@ int run_host(int op, float *const *hbufs, float *const *hweights, int P, size_t 
     }
     std::lock_guard<std::mutex> lock(g_mu);
     const int sms = sm_count_or_fail();
-    if (sms <= 0) {
-        snprintf(g_err, sizeof(g_err), "no CUDA device: liblp_b200 has no CPU fallback");
-        return LP_ERR_CUDA;
-    }
+    if (sms <= 0) return no_device(sms);
     if (n == 0) return LP_OK;
     int rc = host_init();
     if (rc != LP_OK) return rc;
@@ -561,9 +561,9 @@ int lp_comm_create(lp_comm **comm) {
     if (comm == nullptr) return LP_ERR_INVALID_ARG;
     *comm = nullptr;
     std::lock_guard<std::mutex> lock(g_mu);
-    if (sm_count_or_fail() <= 0) {
-        snprintf(g_err, sizeof(g_err), "no CUDA device: liblp_b200 has no CPU fallback");
-        return LP_ERR_CUDA;
+    {
+        const int sms = sm_count_or_fail();
+        if (sms <= 0) return no_device(sms);
     }
     int lo = 0, hi = 0;  // hi = numerically lowest = highest priority
     LP_TRYC(cudaDeviceGetStreamPriorityRange(&lo, &hi), "lp_comm_create");
@@ -695,6 +695,8 @@ int lp_shutdown(void) {
     if (g_sched) cudaFree(g_sched);
     g_sched = nullptr;
     g_sched_next = 0;
+    g_sm_count = 0;  // unbind: the next call binds to whatever device is current then
+    g_device = -1;
     for (int s = 0; s < kScratchSlots; ++s) {
         if (g_scratch[s]) cudaFree(g_scratch[s]);
         g_scratch[s] = nullptr;
@@ -720,7 +722,10 @@ const char *lp_status_string(int status) {
     switch (status) {
         case LP_OK: return "LP_OK";
         case LP_ERR_INVALID_ARG: return "LP_ERR_INVALID_ARG: bad P / pointer / block / root / alignment / overlap";
-        case LP_ERR_UNSUPPORTED: return "LP_ERR_UNSUPPORTED: BE needs a power-of-two P; cluster variant needs P <= 16";
+        case LP_ERR_UNSUPPORTED:
+            return g_err[0] && strstr(g_err, "bound to CUDA device")
+                       ? g_err
+                       : "LP_ERR_UNSUPPORTED: BE needs a power-of-two P; cluster variant: P <= 16, no momentum, no slice lists";
         case LP_ERR_CUDA: return g_err[0] ? g_err : "LP_ERR_CUDA";
         default: return "unknown status";
     }
