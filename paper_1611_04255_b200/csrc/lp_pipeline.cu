@@ -483,15 +483,15 @@ cudaError_t lp_pipeline_launch(const LpArgs &a, const lp_seg_table *segs, const 
     }
 
     uint32_t threads;
-    int V = 0, CW = 0;
     if (bcast) {
         threads = 64;
     } else {
+        int CW;  // add warps: tile = V * 4 * CW * 32 elements with (V, CW) = (2,4) (4,4) (4,8) (8,8)
         switch (tile) {
-            case 1024: V = 2, CW = 4; break;
-            case 2048: V = 4, CW = 4; break;
-            case 4096: V = 4, CW = 8; break;
-            case 8192: V = 8, CW = 8; break;
+            case 1024:
+            case 2048: CW = 4; break;
+            case 4096:
+            case 8192: CW = 8; break;
             default: return cudaErrorInvalidValue;
         }
         threads = (uint32_t)(CW + 2) * 32u;
