@@ -24,12 +24,12 @@
 
 namespace {
 
-constexpr int kFoldWarps = 8;
-constexpr int kRetWarps = 8;
+constexpr int kFoldWarps = 4;
+constexpr int kRetWarps = 4;
 constexpr int kClThreads = (2 + kFoldWarps + kRetWarps) * 32;  // producer, store, fold, return
 constexpr int kV = 4;                                          // float4 per fold / return thread
-constexpr int kClTile = kV * 4 * kFoldWarps * 32;              // 4096 elements
-constexpr int kSIn = 6, kSRv = 4, kSFin = 4;
+constexpr int kClTile = kV * 4 * kFoldWarps * 32;              // 2048 elements: 11 slots = 88 KB, two CTAs per SM
+constexpr int kSIn = 5, kSRv = 3, kSFin = 3;
 
 struct LpClusterArgs {
     const float *in_of[16];  // what cluster CTA x loads (NULL: nothing)
@@ -202,36 +202,46 @@ __global__ void __launch_bounds__(kClThreads)
                 lp_tile_range(part, t, off, len);
                 float4 acc[kV];
                 lp_mbar_wait(&in_full[in.slot], in.phase);
-                {
-                    const float4 *s = reinterpret_cast<const float4 *>(in_ring + in.slot * kClTile);
-#pragma unroll
-                    for (int v = 0; v < kV; ++v) acc[v] = s[ftid + v * FT];
-                }
                 // A slot is handed back only after the shared-memory reads of it have RETURNED: this SM's load/store
-                // queue is busy with the neighbours' st.async traffic, and an mbarrier arrive does not wait for
-                // loads that are still queued -- without the fence the refill of the slot overtook them (seen as
-                // "rank r's term taken from the tile kSIn rounds ahead" in ~1 of 10 runs at P >= 3).
-                __threadfence_block();
-                __syncwarp();
-                if (lane == 0) lp_mbar_arrive(&in_empty[in.slot]);
-                in.advance();
+                // queue is busy with the neighbours' st.async traffic, and an mbarrier arrive does not wait for loads
+                // that are still queued (without this the refill of a slot overtook them: "rank r's term taken from
+                // the tile kSIn rounds ahead" in ~1 of 10 runs at P >= 3).  So every arrive that releases a slot comes
+                // after the instruction that consumes the loaded values (the add, the st.async) AND a CTA-scope fence
+                // (the fence costs nothing measurable here; the instruction order alone is at the scheduler's mercy).
+                const float4 *mine = reinterpret_cast<const float4 *>(in_ring + in.slot * kClTile);
                 if (x > 0) {  // a' = (what GPU x-1 sent) + my block, in that order (chain order)
                     lp_mbar_wait(&rv_full[rv.slot], rv.phase);
                     const float4 *s = reinterpret_cast<const float4 *>(rv_ring + rv.slot * kClTile);
 #pragma unroll
-                    for (int v = 0; v < kV; ++v) acc[v] = lp_add4(s[ftid + v * FT], acc[v]);
-                    __threadfence_block();  // my reads of the slot have returned before the credit leaves (see below)
+                    for (int v = 0; v < kV; ++v) acc[v] = lp_add4(s[ftid + v * FT], mine[ftid + v * FT]);
+                    __threadfence_block();
                     __syncwarp();
+                    if (lane == 0) lp_mbar_arrive(&in_empty[in.slot]);
                     if (ftid == 0) lp_mbar_expect_tx(&rv_full[rv.slot], kClTile * 4u);  // re-arm for the slot's next use
                     if (lane == 0) cl_arrive(&send_credit[rv.slot], (uint32_t)x - 1u);
                     rv.advance();
+                } else {
+#pragma unroll
+                    for (int v = 0; v < kV; ++v) acc[v] = mine[ftid + v * FT];
+                    if (head) {  // a cluster of one (P = 1): nothing consumes the loads before the slot goes back
+                        __threadfence_block();
+                        __syncwarp();
+                        if (lane == 0) lp_mbar_arrive(&in_empty[in.slot]);
+                    }
                 }
+                const int my_in_slot = in.slot;
+                in.advance();
                 if (!head) {
                     lp_mbar_wait(&send_credit[snd.slot], snd.phase ^ 1u);
                     const uint32_t dst = cl_map(rv_ring + snd.slot * kClTile, (uint32_t)x + 1u);
                     const uint32_t flag = cl_map(&rv_full[snd.slot], (uint32_t)x + 1u);
 #pragma unroll
                     for (int v = 0; v < kV; ++v) cl_store4_async(dst + (uint32_t)(ftid + v * FT) * 16u, acc[v], flag);
+                    if (x == 0) {  // rank 0's tile went out as it was: the stores above consumed the loads
+                        __threadfence_block();
+                        __syncwarp();
+                        if (lane == 0) lp_mbar_arrive(&in_empty[my_in_slot]);
+                    }
                     snd.advance();
                 } else {
                     if (sgd) {  // g = S/P, w' = w_root - lr g, applied where the chain ends
@@ -268,13 +278,18 @@ __global__ void __launch_bounds__(kClThreads)
             for (uint64_t t = cid; t < part.n_tiles; t += n_clusters) {
                 float4 r4[kV];
                 lp_mbar_wait(&fin_full[fin.slot], fin.phase);
+                lp_mbar_wait(&dn_credit[dn.slot], dn.phase ^ 1u);
                 {
                     const float4 *s = reinterpret_cast<const float4 *>(fin_ring + fin.slot * kClTile);
 #pragma unroll
                     for (int v = 0; v < kV; ++v) r4[v] = s[rtid + v * RT];
                 }
-                __threadfence_block();  // my reads of the slot have returned before the credit leaves (see below)
-                __syncwarp();
+                const uint32_t dst = cl_map(fin_ring + dn.slot * kClTile, (uint32_t)x - 1u);
+                const uint32_t flag = cl_map(&fin_full[dn.slot], (uint32_t)x - 1u);
+#pragma unroll
+                for (int v = 0; v < kV; ++v) cl_store4_async(dst + (uint32_t)(rtid + v * RT) * 16u, r4[v], flag);
+                __threadfence_block();
+                __syncwarp();  // the stores consumed the loads: my slot may go back (see the fold warps)
                 if (!head && rtid == 0) lp_mbar_expect_tx(&fin_full[fin.slot], kClTile * 4u);  // re-arm (I am the one who does)
                 if (lane == 0) {
                     if (head)
@@ -283,11 +298,6 @@ __global__ void __launch_bounds__(kClThreads)
                         cl_arrive(&dn_credit[fin.slot], (uint32_t)x + 1u);
                 }
                 fin.advance();
-                lp_mbar_wait(&dn_credit[dn.slot], dn.phase ^ 1u);
-                const uint32_t dst = cl_map(fin_ring + dn.slot * kClTile, (uint32_t)x - 1u);
-                const uint32_t flag = cl_map(&fin_full[dn.slot], (uint32_t)x - 1u);
-#pragma unroll
-                for (int v = 0; v < kV; ++v) cl_store4_async(dst + (uint32_t)(rtid + v * RT) * 16u, r4[v], flag);
                 dn.advance();
             }
         }
