@@ -524,6 +524,48 @@ def test_cluster_variant_limits():
 
 
 # ---------------------------------------------------------------------------------------------------
+# IEEE corner values (U16): no flush-to-zero, inf and NaN propagate
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("variant", [lp.VARIANT_AUTO, lp.VARIANT_PIPELINE, lp.VARIANT_DIRECT, lp.VARIANT_CLUSTER])
+def test_denormals_inf_nan(oracle, variant):
+    # subnormal inputs and subnormal sums must survive bit for bit (nvcc default -ftz=false, oracle without DAZ/FTZ);
+    # +-inf propagate exactly; NaN propagates as NaN (payload bits are not compared: x86 keeps the operand's
+    # payload, the GPU returns the canonical NaN)
+    lp.lp_set_variant(variant)
+    P, n = 4, 40_003
+    rng = np.random.default_rng(97)
+    tiny = np.float32(1e-45)                                   # smallest subnormal
+    src = [(rng.integers(-2000, 2000, n).astype(np.float32) * tiny) for _ in range(P)]   # all subnormal or zero
+    src[1][::7] = np.float32(1.17549435e-38)                   # smallest normal: sums cross the normal boundary
+    src[2][::7] = np.float32(-1.17549435e-38)
+    src[0][5::101] = np.inf
+    src[3][6::101] = -np.inf
+    src[0][7::101] = np.inf
+    src[3][7::101] = -np.inf                                   # inf + -inf = NaN
+    src[2][8::101] = np.nan
+    want = oracle.chain_sum(src)
+    assert np.any((want != 0) & (np.abs(want) < np.float32(1.17549435e-38)))      # subnormal results exist
+    dev = up(src)
+    lp.lp_allreduce(dev, 4096)
+    got = down(dev)
+    nan = np.isnan(want)
+    assert nan.any() and np.isinf(want).any()
+    for r in range(P):
+        assert np.array_equal(np.isnan(got[r]), nan), r
+        assert got[r][~nan].tobytes() == want[~nan].tobytes(), r
+    # SGD epilogue on subnormal sums: products that underflow must round the same way
+    weights = [np.full(n, np.float32(3e-39)) for _ in range(P)]
+    grads = [s.copy() for s in src]
+    for g in grads:
+        g[~np.isfinite(g)] = 0
+    hw = copies(weights)
+    oracle.bsp_sgd_step(grads, hw, root=0, lr=0.5)
+    dg, dw = up(grads), up(weights)
+    lp.lp_bsp_sgd_step(dg, dw, 4096, root=0, lr=0.5)
+    assert all(same(a, b) for a, b in zip(down(dw), hw))
+
+
+# ---------------------------------------------------------------------------------------------------
 # MST / BE baselines (a7, a8)
 # ---------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("P,n", [(2, 1001), (3, 70_001), (4, 65_536), (5, 4099), (6, 300_003), (8, 100_001),
