@@ -63,6 +63,7 @@ def lib() -> ctypes.CDLL:
         for name in ("lpo_bsp_sgd_momentum_step", "lpo_bsp_sgd_alg2_step"):
             getattr(L, name).argtypes = [pp, pp, ctypes.c_void_p, i32, sz, i32, f32, f32]
         L.lpo_collective_segments.argtypes = [i32, pp, i32, sz, ctypes.POINTER(sz), ctypes.POINTER(sz), i32, i32]
+        L.lpo_bsp_sgd_step_segments.argtypes = [pp, pp, i32, sz, ctypes.POINTER(sz), ctypes.POINTER(sz), i32, i32, f32]
         L.lpo_lp_blocked.argtypes = [pp, i32, sz, sz, i32, i32, pu64]
         L.lpo_num_blocks.argtypes = [sz, sz]
         L.lpo_num_blocks.restype = u64
@@ -168,6 +169,19 @@ def collective_segments(op, bufs, segments, root=0):
     off = (ctypes.c_size_t * max(k, 1))(*[int(o) for o, _ in segments])
     ln = (ctypes.c_size_t * max(k, 1))(*[int(l) for _, l in segments])
     _check(lib().lpo_collective_segments(op, arr, len(bufs), n, off, ln, k, root), "lpo_collective_segments")
+
+
+def bsp_sgd_step_segments(grads, weights, segments, root=0, lr=0.01):
+    """Layer-wise fused BSP-SGD step: bsp_sgd_step on every (offset, length) slice."""
+    ga, n = _ptrs(grads)
+    wa, nw = _ptrs(weights)
+    if n != nw or len(grads) != len(weights):
+        raise ValueError("grads and weights must match in P and n")
+    k = len(segments)
+    off = (ctypes.c_size_t * max(k, 1))(*[int(o) for o, _ in segments])
+    ln = (ctypes.c_size_t * max(k, 1))(*[int(l) for _, l in segments])
+    _check(lib().lpo_bsp_sgd_step_segments(ga, wa, len(grads), n, off, ln, k, root, ctypes.c_float(lr)),
+           "lpo_bsp_sgd_step_segments")
 
 
 def lp_blocked(bufs, block, op, root=0) -> int:

@@ -252,6 +252,32 @@ int lpo_collective_segments(int op, float *const *bufs, int P, size_t n,
     return LPO_OK;
 }
 
+/* Layer-wise fused BSP-SGD step: Alg. 1's per-layer communication with Alg. 3's update
+ * applied to each layer as soon as its gradient has been allreduced: lpo_bsp_sgd_step on
+ * every slice, in list order; elements outside every slice keep their weights. */
+int lpo_bsp_sgd_step_segments(float *const *grads, float *const *weights, int P, size_t n,
+                              const size_t *seg_off, const size_t *seg_len, int n_seg,
+                              int root, float lr)
+{
+    if (bad_args(grads, P, root) || bad_args(weights, P, root) || P > 64 ||
+        n_seg < 0 || (n_seg > 0 && (!seg_off || !seg_len)))
+        return LPO_EINVAL;
+    for (int s = 0; s < n_seg; ++s)
+        if (seg_off[s] > n || seg_len[s] > n - seg_off[s])
+            return LPO_EINVAL;
+    for (int s = 0; s < n_seg; ++s) {
+        float *g[64], *w[64];
+        for (int r = 0; r < P; ++r) {
+            g[r] = grads[r] + seg_off[s];
+            w[r] = weights[r] + seg_off[s];
+        }
+        int rc = lpo_bsp_sgd_step(g, w, P, seg_len[s], root, lr);
+        if (rc != LPO_OK)
+            return rc;
+    }
+    return LPO_OK;
+}
+
 /* The same two definitions with the element loop spread over host threads.
  * Element i never depends on element j != i, so the bits are those of the
  * serial loops above (tests assert it).  These are the versions bench.py times

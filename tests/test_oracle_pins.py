@@ -242,3 +242,26 @@ def test_segments_brute_force_small_integers(oracle):
             assert got[r][i] == (total[i] if inside else src[r][i])
     with pytest.raises(RuntimeError):
         oracle.collective_segments(ALLREDUCE, got, [(60, 5)])      # runs past n
+
+
+def test_sgd_segments_equal_whole_step_on_their_union(oracle):
+    # the update is element-wise: per-slice steps give the whole-vector step's weights inside the slices and leave
+    # every other weight (and every gradient) alone; written against the numpy composition, not the oracle's own step
+    P, n, root, lr = 4, 5003, 2, np.float32(0.05)
+    segs = [(4000, 1003), (0, 2), (17, 900), (2000, 0)]
+    grads, weights = inputs.sgd_inputs(83, P, n)
+    for r in range(P):
+        weights[r] = weights[r] + np.float32(r)
+    S = grads[0].copy()
+    for r in range(1, P):
+        S = S + grads[r]
+    w_new = weights[root] - lr * (S * (np.float32(1.0) / np.float32(P)))
+    g0, w0 = _copy(grads), _copy(weights)
+    oracle.bsp_sgd_step_segments(grads, weights, segs, root=root, lr=float(lr))
+    mask = np.zeros(n, bool)
+    for o, l in segs:
+        mask[o:o + l] = True
+    for r in range(P):
+        assert weights[r][mask].tobytes() == w_new[mask].tobytes()
+        assert weights[r][~mask].tobytes() == w0[r][~mask].tobytes()
+        assert grads[r].tobytes() == g0[r].tobytes()
