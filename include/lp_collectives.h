@@ -167,6 +167,12 @@ LP_API int lp_reduce_segments(float *const *bufs, int P, size_t n, const size_t 
                               int n_seg, size_t block, int root, void *cuda_stream);
 LP_API int lp_allreduce_segments(float *const *bufs, int P, size_t n, const size_t *seg_off, const size_t *seg_len,
                                  int n_seg, size_t block, void *cuda_stream);
+/* The fused BSP-SGD step of lp_bsp_sgd_step on every slice (a layer's weights are updated as soon as its gradient
+ * has been allreduced: Alg. 1's per-layer communication with Alg. 3's update); weights outside every slice keep
+ * their values, grads are only read. */
+LP_API int lp_bsp_sgd_step_segments(float *const *grads, float *const *weights, int P, size_t n, const size_t *seg_off,
+                                    const size_t *seg_len, int n_seg, size_t block, int root, float lr,
+                                    void *cuda_stream);
 
 /* ---- non-blocking use (Alg. 1's nonblocking_* / sync_*) ------------------------- */
 /* Every lp_* call above is already asynchronous to the host; "non-blocking" in the sense of Alg. 1 (PAPER.md:117-138:

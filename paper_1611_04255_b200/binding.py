@@ -65,6 +65,7 @@ def lib() -> ctypes.CDLL:
     L.lp_broadcast_segments.argtypes = [pp, i32, sz, psz, psz, i32, sz, i32, vp]
     L.lp_reduce_segments.argtypes = [pp, i32, sz, psz, psz, i32, sz, i32, vp]
     L.lp_allreduce_segments.argtypes = [pp, i32, sz, psz, psz, i32, sz, vp]
+    L.lp_bsp_sgd_step_segments.argtypes = [pp, pp, i32, sz, psz, psz, i32, sz, i32, f32, vp]
     L.lp_comm_create.argtypes = [ctypes.POINTER(vp)]
     L.lp_comm_destroy.argtypes = [vp]
     L.lp_comm_stream.argtypes = [vp]
@@ -274,6 +275,16 @@ class Comm:
             self.close()
         except Exception:
             pass
+
+
+def lp_bsp_sgd_step_segments(grads, weights, segments, block, root=0, lr=0.01, stream=None):
+    ga, n = _dev_ptrs(grads)
+    wa, nw = _dev_ptrs(weights)
+    if n != nw or len(grads) != len(weights):
+        raise ValueError("grads and weights must match in P and n")
+    sg = _segments(segments)
+    _check(lib().lp_bsp_sgd_step_segments(ga, wa, len(grads), n, sg.off, sg.len, sg.k, block, root, ctypes.c_float(lr),
+                                          _stream_ptr(stream)), "lp_bsp_sgd_step_segments")
 
 
 def _velocity_ptr(velocity, n):

@@ -234,10 +234,13 @@ int plan_and_run(int op, float *const *bufs, float *const *weights, float *veloc
                 e = lp_copy_engine_run(op, bufs, weights, velocity, P, n, block, root, lr, mu, g_tuning, sm_count, stream);
             } else {  // one chain of copies + adds per slice
                 for (int s = 0; s < segl->n && e == cudaSuccess; ++s) {
-                    float *sb[LP_MAX_P];
-                    for (int r = 0; r < P; ++r) sb[r] = bufs[r] + segl->off[s];
-                    e = lp_copy_engine_run(op, sb, nullptr, nullptr, P, segl->len[s], block, root, lr, mu, g_tuning,
-                                           sm_count, stream);
+                    float *sb[LP_MAX_P], *sw[LP_MAX_P];
+                    for (int r = 0; r < P; ++r) {
+                        sb[r] = bufs[r] + segl->off[s];
+                        sw[r] = weights ? weights[r] + segl->off[s] : nullptr;
+                    }
+                    e = lp_copy_engine_run(op, sb, weights ? sw : nullptr, nullptr, P, segl->len[s], block, root, lr, mu,
+                                           g_tuning, sm_count, stream);
                 }
             }
         }
@@ -298,9 +301,9 @@ int run_alg2(float *const *grads, float *const *weights, float *velocity, int P,
 
 // Layer-wise collective (Alg. 1): `op` on every slice [seg_off[s], seg_off[s] + seg_len[s]) of the rank vectors,
 // each slice its own LP message, tiles handed out slice by slice in list order; LP_MAX_SEGS slices per launch.
-int run_segments(int op, float *const *bufs, int P, size_t n, const size_t *seg_off, const size_t *seg_len, int n_seg,
-                 size_t block, int root, void *cuda_stream) {
-    int rc = validate(op, bufs, nullptr, nullptr, P, n, block, root);
+int run_segments(int op, float *const *bufs, float *const *weights, int P, size_t n, const size_t *seg_off,
+                 const size_t *seg_len, int n_seg, size_t block, int root, float lr, void *cuda_stream) {
+    int rc = validate(op, bufs, weights, nullptr, P, n, block, root);
     if (rc != LP_OK) return rc;
     if (n_seg < 0 || n_seg > LP_MAX_SEGMENTS || (n_seg > 0 && (seg_off == nullptr || seg_len == nullptr)))
         return LP_ERR_INVALID_ARG;
@@ -328,7 +331,7 @@ int run_segments(int op, float *const *bufs, int P, size_t n, const size_t *seg_
         }
         if (m == LP_MAX_SEGS || (s == n_seg && m > 0)) {
             const SegList sl{off, len, m};
-            rc = plan_and_run(op, bufs, nullptr, nullptr, P, n, block, root, 0.f, 0.f, sms, nullptr, false,
+            rc = plan_and_run(op, bufs, weights, nullptr, P, n, block, root, lr, 0.f, sms, nullptr, false,
                               (cudaStream_t)cuda_stream, &sl);
             if (rc != LP_OK) return rc;
             m = 0;
@@ -513,15 +516,20 @@ int lp_bsp_sgd_alg2_step(float *const *grads, float *const *weights, float *velo
 
 int lp_broadcast_segments(float *const *bufs, int P, size_t n, const size_t *seg_off, const size_t *seg_len, int n_seg,
                           size_t block, int root, void *cuda_stream) {
-    return run_segments(LP_OP_BROADCAST, bufs, P, n, seg_off, seg_len, n_seg, block, root, cuda_stream);
+    return run_segments(LP_OP_BROADCAST, bufs, nullptr, P, n, seg_off, seg_len, n_seg, block, root, 0.f, cuda_stream);
 }
 int lp_reduce_segments(float *const *bufs, int P, size_t n, const size_t *seg_off, const size_t *seg_len, int n_seg,
                        size_t block, int root, void *cuda_stream) {
-    return run_segments(LP_OP_REDUCE, bufs, P, n, seg_off, seg_len, n_seg, block, root, cuda_stream);
+    return run_segments(LP_OP_REDUCE, bufs, nullptr, P, n, seg_off, seg_len, n_seg, block, root, 0.f, cuda_stream);
 }
 int lp_allreduce_segments(float *const *bufs, int P, size_t n, const size_t *seg_off, const size_t *seg_len, int n_seg,
                           size_t block, void *cuda_stream) {
-    return run_segments(LP_OP_ALLREDUCE, bufs, P, n, seg_off, seg_len, n_seg, block, 0, cuda_stream);
+    return run_segments(LP_OP_ALLREDUCE, bufs, nullptr, P, n, seg_off, seg_len, n_seg, block, 0, 0.f, cuda_stream);
+}
+int lp_bsp_sgd_step_segments(float *const *grads, float *const *weights, int P, size_t n, const size_t *seg_off,
+                             const size_t *seg_len, int n_seg, size_t block, int root, float lr, void *cuda_stream) {
+    if (weights == nullptr) return LP_ERR_INVALID_ARG;
+    return run_segments(LP_OP_BSP_SGD, grads, weights, P, n, seg_off, seg_len, n_seg, block, root, lr, cuda_stream);
 }
 
 int lp_mst_broadcast(float *const *bufs, int P, size_t n, int root, void *s) {

@@ -399,6 +399,25 @@ def test_segments_many_layers_and_all_tiles(oracle):
         assert all(same(g, w) for g, w in zip(down(dev), want)), tile
 
 
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_sgd_step_segments_bit_exact(oracle, variant):
+    lp.lp_set_variant(variant)
+    P, n, block, root = 6, 500_009, 16_384, 4
+    rng = np.random.default_rng(98)
+    segs = _layer_slices(n, rng, 12) + [(7, 0)]
+    grads, weights = inputs.sgd_inputs([16, n], P, n)
+    weights[root] += np.float32(0.125)
+    hw = copies(weights)
+    dg, dw = up(grads), up(weights)
+    for it in range(2):
+        oracle.bsp_sgd_step_segments(grads, hw, segs, root=root, lr=0.01)
+        lp.lp_bsp_sgd_step_segments(dg, dw, segs, block, root=root, lr=0.01)
+        gw = down(dw)
+        for r in range(P):
+            assert same(gw[r], hw[r]), (it, r)
+    assert all(same(g, s) for g, s in zip(down(dg), grads))
+
+
 def test_segments_validation():
     dev = [torch.zeros(1000, device="cuda") for _ in range(3)]
     for bad in ([(990, 11)], [(0, 10), (9, 5)], [(5, 10), (0, 6)]):     # past n; overlapping (either order)
