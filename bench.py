@@ -34,7 +34,7 @@ UNIT = "GB/s (algbw = n*4 bytes per rank / time; roofline on min bytes 2*P*n*4)"
 FALLBACK_HBM_GBS = 6650.0  # B200_PROFILING.md fallback, used only if MEASURED_PEAKS.json is absent
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` capture (profiles/r1_ncu_lp_pipeline.md); keyed by (P, n, variant)
-NCU_TRAFFIC_BYTES = {(6, 61_000_000, "pipeline"): 2_869_976_000}
+NCU_TRAFFIC_BYTES = {(6, 61_000_000, "pipeline"): 2_869_606_000}
 
 
 def parse_args():
