@@ -94,12 +94,13 @@ extern "C" {
 #define LP_TUNE_TILE_ELEMS 0    /* tile (sub-block) size in elements: 1024, 2048, 4096 or 8192 */
 #define LP_TUNE_STAGES 1        /* depth of the load ring (2..32) */
 #define LP_TUNE_OUT_STAGES 2    /* depth of the store ring (1..8) */
-#define LP_TUNE_CTAS_PER_SM 3   /* persistent CTAs per SM (1..8) */
+#define LP_TUNE_CTAS_PER_SM 3   /* persistent CTAs per SM (1..8); the direct variant launches one CTA per tile
+                                   unless this (or LP_TUNE_GRID_LIMIT) is set */
 #define LP_TUNE_CE_STREAMS 4    /* copy-engine variant: number of streams / receive slots (paper: 2) */
 #define LP_TUNE_L2_HINT 5       /* 0 none, 1 evict_first on loads, 2 evict_first on loads and stores */
 #define LP_TUNE_STORE_WAIT 6    /* 0: a store-ring slot is reused once its bulk stores have READ it (default);
                                    1: only once they have COMPLETED (bounds the store bytes in flight) */
-#define LP_TUNE_SCHED 7         /* how persistent CTAs pick tiles: 0 (default) dynamic -- each CTA claims its next tile
+#define LP_TUNE_SCHED 7         /* pipeline variant: how persistent CTAs pick tiles: 0 (default) dynamic -- each CTA claims its next tile
                                    from a device-side counter, so SMs that get more HBM bandwidth take more tiles
                                    and all finish together; 1 static round robin (tile t -> CTA t mod grid) */
 #define LP_TUNE_GRID_LIMIT 8    /* at most this many persistent CTAs per launch (0 = one grid-full: SMs x CTAs per SM).
