@@ -57,6 +57,10 @@ def main(argv=None):
     ap.add_argument("--ratios", default="0.5,1,2")
     ap.add_argument("--limits", default="0,64,32,16")
     ap.add_argument("--compute", default="matmul,spin")
+    ap.add_argument("--mode", default="allreduce", choices=["allreduce", "sgd", "broadcast"],
+                    help="allreduce: backward pass, layer-wise allreduce of the gradients (default); sgd: backward "
+                         "pass, layer-wise fused BSP-SGD step (lp_bsp_sgd_step_segments); broadcast: forward pass, "
+                         "layer-wise broadcast of the weights from rank 0 (Alg. 1 lines 2-6)")
     args = ap.parse_args(argv)
     assert torch.cuda.is_available(), "needs a CUDA device"
     dev = torch.device("cuda", 0)
@@ -69,8 +73,18 @@ def main(argv=None):
     segs = {name: lp.Segments([(off, cnt)]) for name, off, cnt in slices}
     comm = lp.Comm()
     compute = torch.cuda.Stream()
-    back = list(reversed(slices))  # backward order: fc8 ... conv1
-    min_bytes = lp.lp_min_bytes(lp.OP_ALLREDUCE, P, n)
+    back = list(reversed(slices)) if args.mode != "broadcast" else list(slices)  # backward: fc8 ... conv1; forward: conv1 ... fc8
+    op = {"allreduce": lp.OP_ALLREDUCE, "sgd": lp.OP_BSP_SGD, "broadcast": lp.OP_BROADCAST}[args.mode]
+    min_bytes = lp.lp_min_bytes(op, P, n)
+    weights = lp.Ranks([torch.from_numpy(inputs.normal(1, 100, n, 0.05)).to(dev) for _ in range(P)]) if args.mode == "sgd" else None
+
+    def collective(name, stream):
+        if args.mode == "allreduce":
+            lp.lp_allreduce_segments(ranks, segs[name], args.block, stream=stream)
+        elif args.mode == "sgd":
+            lp.lp_bsp_sgd_step_segments(ranks, weights, segs[name], args.block, root=0, lr=0.01, stream=stream)
+        else:
+            lp.lp_broadcast_segments(ranks, segs[name], args.block, root=0, stream=stream)
 
     a = torch.randn(2048, 2048, device=dev, dtype=torch.bfloat16)
     b = torch.randn(2048, 2048, device=dev, dtype=torch.bfloat16)
@@ -97,7 +111,7 @@ def main(argv=None):
 
     def comm_only():
         for name, _, _ in back:
-            lp.lp_allreduce_segments(ranks, segs[name], args.block, stream=compute)
+            collective(name, compute)
 
     def unit_ms(kind):
         """Milliseconds of one unit of the compute stand-in (one matmul / 100k spin cycles)."""
@@ -131,13 +145,22 @@ def main(argv=None):
             def serial():
                 for name, _, _ in back:
                     backward(name)
-                    lp.lp_allreduce_segments(ranks, segs[name], args.block, stream=compute)
+                    collective(name, compute)
 
             def overlapped():
+                if args.mode == "broadcast":            # Alg. 1 lines 1-6: broadcast(w^0); nonblocking_broadcast(w^{i+1}); Forward(i)
+                    comm.after(compute)
+                    collective(back[0][0], comm.stream)
+                    for i, (name, _, _) in enumerate(back):
+                        comm.wait(compute)              # layer i's weights have arrived
+                        if i + 1 < len(back):
+                            collective(back[i + 1][0], comm.stream)
+                        backward(name)                  # Forward(i) on the compute stream
+                    return
                 for name, _, _ in back:
                     backward(name)                      # Backward(i) on the compute stream
                     comm.after(compute)                 # its gradient is ready: nonblocking_allreduce(layer i)
-                    lp.lp_allreduce_segments(ranks, segs[name], args.block, stream=comm.stream)
+                    collective(name, comm.stream)
                 comm.wait(compute)                      # sync_reduce()
 
             t_comp = timed(compute_only)
@@ -146,7 +169,7 @@ def main(argv=None):
                 t_comm = timed(comm_only)
                 t_ser = timed(serial)
                 t_ovl = timed(overlapped)
-                row = dict(compute=kind, ratio=ratio, grid_limit=limit, P=P, n=n, layers=len(LAYERS),
+                row = dict(mode=args.mode, compute=kind, ratio=ratio, grid_limit=limit, P=P, n=n, layers=len(LAYERS),
                            comm_ms=round(t_comm, 4), compute_ms=round(t_comp, 4), serial_ms=round(t_ser, 4),
                            overlapped_ms=round(t_ovl, 4), max_ms=round(max(t_comm, t_comp), 4),
                            sum_ms=round(t_comm + t_comp, 4),
@@ -163,9 +186,10 @@ def main(argv=None):
     with open(args.out + ".md", "w") as f:
         f.write("# Alg. 1 on one B200: layer-wise LP allreduce overlapped with the backward computation\n\n")
         f.write(f"Command: `python -m paper_1611_04255_b200.alg1_overlap --out {args.out} --P {P} --block {args.block} "
-                f"--ratios {args.ratios} --limits {args.limits} --compute {args.compute}`\n\n")
+                f"--ratios {args.ratios} --limits {args.limits} --compute {args.compute} --mode {args.mode}`\n\n")
         f.write(f"AlexNet-shaped layer list ({len(LAYERS)} messages, {n:,} fp32 per rank), P={P} virtual ranks; one "
-                "`lp_allreduce_segments` per layer in backward order.  PAPER.md:192: the overlapped iteration should cost "
+                f"`{ {'allreduce': 'lp_allreduce_segments', 'sgd': 'lp_bsp_sgd_step_segments', 'broadcast': 'lp_broadcast_segments'}[args.mode] }` "
+                f"per layer in {'forward' if args.mode == 'broadcast' else 'backward'} order.  PAPER.md:192: the overlapped iteration should cost "
                 "max(comm, compt), the serial one comm + compt.  `hidden` = (serial - overlapped) / min(comm, compt): "
                 "the fraction of the shorter of the two that the overlap hides.  grid limit 0 = the collective takes "
                 "its usual 2 CTAs on every SM.\n\n")
