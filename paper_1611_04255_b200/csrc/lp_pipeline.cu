@@ -435,7 +435,7 @@ static bool read_dominated(const LpArgs &a) { return a.epilogue != LP_EPI_COPY &
 uint32_t lp_pipeline_tile(const LpTuning &t, const LpArgs &a, uint64_t n, uint64_t block) {
     const bool confined = t.v[LP_TUNE_GRID_LIMIT] > 0 && t.v[LP_TUNE_GRID_LIMIT] <= 148;  // see lp_pipeline_launch
     uint32_t tile = t.v[LP_TUNE_TILE_ELEMS] ? (uint32_t)t.v[LP_TUNE_TILE_ELEMS]
-                    : (confined ? (a.epilogue == LP_EPI_COPY ? 4096u : 8192u)
+                    : (confined ? (read_dominated(a) ? 8192u : 4096u)
                                 : (a.epilogue == LP_EPI_COPY && a.n_out >= 9 ? 1024u : 2048u));
     uint64_t blk = block < n ? block : n;
     while (tile > 1024u && (uint64_t)(tile / 2) >= blk) tile /= 2;
@@ -459,13 +459,13 @@ cudaError_t lp_pipeline_launch(const LpArgs &a, const lp_seg_table *segs, const 
         if (!t.v[LP_TUNE_STAGES] && !bcast && stages < (uint32_t)a.n_in) stages = a.n_in < 24 ? (uint32_t)a.n_in : 24u;
     }
     // confined to fewer CTAs than SMs (LP_TUNE_GRID_LIMIT: a collective running beside compute kernels): one CTA per
-    // SM with all of its shared memory -- folds take 32 KB tiles (8 add warps, 8 vectors each) in a 6-deep load ring:
-    // 100 GB/s per CTA for allreduce and 130 GB/s for reduce, so 64 CTAs move 6.3 / 7.1 TB/s; broadcast takes 16 KB
-    // tiles x 12 slots and is bounded by ~60 GB/s of bulk stores per SM (profiles/r1_tuning.md section 6)
+    // SM with all of its shared memory -- 16 KB tiles in a 12-deep load ring (~100 GB/s per CTA for allreduce: 64 CTAs
+    // move 6.3 TB/s), 32 KB tiles x 6 for the read-dominated reduce (~130 GB/s per CTA: 7.1 TB/s); broadcast is
+    // bounded by ~60 GB/s of bulk stores per SM whatever the ring (profiles/r1_tuning.md section 6)
     if (t.v[LP_TUNE_GRID_LIMIT] && t.v[LP_TUNE_GRID_LIMIT] <= sm_count) {
         if (!t.v[LP_TUNE_CTAS_PER_SM]) ctas = 1u;
-        if (!t.v[LP_TUNE_STAGES]) stages = bcast ? 12u : 6u;
-        if (!t.v[LP_TUNE_OUT_STAGES] && !bcast) out_stages = 1u;
+        if (!t.v[LP_TUNE_STAGES]) stages = read_dominated(a) ? 6u : 12u;
+        if (!t.v[LP_TUNE_OUT_STAGES] && !bcast) out_stages = read_dominated(a) ? 1u : 2u;
     }
     auto smem_of = [&](uint32_t st, uint32_t ost) {
         return (st + ost) * tile * 4u + (4u * st + 4u * ost) * 8u;  // rings + full/empty barriers + tile ranges
