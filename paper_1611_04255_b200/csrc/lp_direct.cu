@@ -9,7 +9,12 @@
 namespace {
 
 constexpr int kThreads = 256;
-constexpr int kRankChunk = 8;  // ranks whose loads are in flight together
+// ranks whose loads are in flight together: 8, or 16 for the one-vector-per-thread kernels of the latency regime (a
+// 16-rank chain then costs one HBM latency, not two)
+template <int V>
+struct LpRankChunk {
+    static constexpr int value = V == 1 ? 16 : 8;
+};
 
 // NS > 0: number of folded inputs known at compile time (loops fully unrolled); NS == 0: runtime a.n_sum.
 template <int NS, int V, bool SEG>
@@ -54,6 +59,7 @@ __global__ void __launch_bounds__(kThreads)
             for (int v = 0; v < V; ++v)
                 if (live[v]) vel[v] = lp_ldg_stream(a.in[n_sum + 1] + a0 + 4 * (uint64_t)(tid + v * kThreads));
         }
+        constexpr int kRankChunk = LpRankChunk<V>::value;
         for (int r0 = 0; r0 < n_sum; r0 += kRankChunk) {
             float4 x[V][kRankChunk];
 #pragma unroll
