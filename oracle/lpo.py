@@ -25,6 +25,7 @@ GCC_FLAGS = ["-O2", "-std=c11", "-ffp-contract=off", "-fno-fast-math", "-fopenmp
              "-fPIC", "-shared"]
 
 OP_BROADCAST, OP_REDUCE, OP_ALLREDUCE = 0, 1, 2
+RED_SUM, RED_PROD = 0, 1  # PAPER.md:59 "summations and multiplications"
 ALGO_LP, ALGO_MST, ALGO_BE = 0, 1, 2
 READING_A_REVERSE, READING_B_RING = 0, 1
 
@@ -64,6 +65,12 @@ def lib() -> ctypes.CDLL:
             getattr(L, name).argtypes = [pp, pp, ctypes.c_void_p, i32, sz, i32, f32, f32]
         L.lpo_collective_segments.argtypes = [i32, pp, i32, sz, ctypes.POINTER(sz), ctypes.POINTER(sz), i32, i32]
         L.lpo_bsp_sgd_step_segments.argtypes = [pp, pp, i32, sz, ctypes.POINTER(sz), ctypes.POINTER(sz), i32, i32, f32]
+        L.lpo_chain_fold.argtypes = [pp, i32, sz, i32, ctypes.c_void_p]
+        for name in ("lpo_reduce_op", "lpo_mst_reduce_op", "lpo_be_reduce_op"):
+            getattr(L, name).argtypes = [pp, i32, sz, i32, i32]
+        for name in ("lpo_allreduce_op", "lpo_mst_allreduce_op", "lpo_be_allreduce_op"):
+            getattr(L, name).argtypes = [pp, i32, sz, i32]
+        L.lpo_collective_segments_op.argtypes = [i32, i32, pp, i32, sz, ctypes.POINTER(sz), ctypes.POINTER(sz), i32, i32]
         L.lpo_lp_blocked.argtypes = [pp, i32, sz, sz, i32, i32, pu64]
         L.lpo_num_blocks.argtypes = [sz, sz]
         L.lpo_num_blocks.restype = u64
@@ -122,6 +129,36 @@ def allreduce(bufs, algo=ALGO_LP, omp=False):
     f = {ALGO_LP: "lpo_allreduce_omp" if omp else "lpo_allreduce",
          ALGO_MST: "lpo_mst_allreduce", ALGO_BE: "lpo_be_allreduce"}[algo]
     _check(getattr(lib(), f)(arr, len(bufs), n), f)
+
+
+def chain_fold(bufs, red=RED_SUM) -> np.ndarray:
+    """Left fold in rank order with the reduce operator `red`."""
+    arr, n = _ptrs(bufs)
+    out = np.empty(n, dtype=np.float32)
+    _check(lib().lpo_chain_fold(arr, len(bufs), n, red, out.ctypes.data), "lpo_chain_fold")
+    return out
+
+
+def reduce_op(bufs, red, root=0, algo=ALGO_LP):
+    arr, n = _ptrs(bufs)
+    f = {ALGO_LP: "lpo_reduce_op", ALGO_MST: "lpo_mst_reduce_op", ALGO_BE: "lpo_be_reduce_op"}[algo]
+    _check(getattr(lib(), f)(arr, len(bufs), n, root, red), f)
+
+
+def allreduce_op(bufs, red, algo=ALGO_LP):
+    arr, n = _ptrs(bufs)
+    f = {ALGO_LP: "lpo_allreduce_op", ALGO_MST: "lpo_mst_allreduce_op", ALGO_BE: "lpo_be_allreduce_op"}[algo]
+    _check(getattr(lib(), f)(arr, len(bufs), n, red), f)
+
+
+def collective_segments_op(op, red, bufs, segments, root=0):
+    """Layer-wise reduce (op 1) / allreduce (op 2) with operator `red` on every (offset, length) slice."""
+    arr, n = _ptrs(bufs)
+    k = len(segments)
+    off = (ctypes.c_size_t * max(k, 1))(*[int(o) for o, _ in segments])
+    ln = (ctypes.c_size_t * max(k, 1))(*[int(l) for _, l in segments])
+    _check(lib().lpo_collective_segments_op(op, red, arr, len(bufs), n, off, ln, k, root),
+           "lpo_collective_segments_op")
 
 
 def bsp_sgd_step(grads, weights, root=0, lr=0.01, omp=False):

@@ -833,6 +833,208 @@ int lpo_be_broadcast(float *const *bufs, int P, size_t n, int root)
 }
 
 /* ------------------------------------------------------------------------ */
+/* 5b. Reduce / allreduce with an operator                        */
+/* ------------------------------------------------------------------------ */
+
+/* PAPER.md:59 (Sec. 3, Reduce): "It supports basic arithmetic operations such
+ * as summations and multiplications."  red: 0 = sum, 1 = product.  Everything
+ * else is as in sections 1, 4 and 5: the LP result is the left fold in rank
+ * order 0 -> P-1 (a0, a' = a0 (op) a1, a'' = a' (op) a2), MST and BE combine
+ * along their own trees; one fp32 RN operation per combine, no FMA. */
+#define LPO_RED_SUM 0
+#define LPO_RED_PROD 1
+
+static float combine(float a, float b, int red)
+{
+    return red == LPO_RED_PROD ? a * b : a + b;
+}
+
+static int bad_red(int red) { return red != LPO_RED_SUM && red != LPO_RED_PROD; }
+
+/* F[i] = (((x_0[i] op x_1[i]) op x_2[i]) op ...) op x_{P-1}[i].  out may not alias inputs. */
+int lpo_chain_fold(const float *const *in, int P, size_t n, int red, float *out)
+{
+    if (in == NULL || out == NULL || P < 1 || bad_red(red))
+        return LPO_EINVAL;
+    for (size_t i = 0; i < n; ++i) {
+        float s = in[0][i];
+        for (int r = 1; r < P; ++r)
+            s = combine(s, in[r][i], red);
+        out[i] = s;
+    }
+    return LPO_OK;
+}
+
+/* Reduce with operator: root <- F, the other vectors unchanged (U5). */
+int lpo_reduce_op(float *const *bufs, int P, size_t n, int root, int red)
+{
+    if (bad_args(bufs, P, root) || bad_red(red))
+        return LPO_EINVAL;
+    for (size_t i = 0; i < n; ++i) {
+        float s = bufs[0][i];
+        for (int r = 1; r < P; ++r)
+            s = combine(s, bufs[r][i], red);
+        bufs[root][i] = s;
+    }
+    return LPO_OK;
+}
+
+/* Allreduce with operator: every rank <- F, the same bits everywhere. */
+int lpo_allreduce_op(float *const *bufs, int P, size_t n, int red)
+{
+    if (bad_args(bufs, P, 0) || bad_red(red))
+        return LPO_EINVAL;
+    for (size_t i = 0; i < n; ++i) {
+        float s = bufs[0][i];
+        for (int r = 1; r < P; ++r)
+            s = combine(s, bufs[r][i], red);
+        for (int r = 0; r < P; ++r)
+            bufs[r][i] = s;
+    }
+    return LPO_OK;
+}
+
+/* MST tree (section 4) with operator: x_v = x_v op x_{v+d}, d = 1, 2, 4, ... */
+static void mst_reduce_virtual_op(float **work, int P, size_t n, int red)
+{
+    for (int d = 1; d < P; d *= 2)
+        for (int v = 0; v + d < P; v += 2 * d)
+            for (size_t i = 0; i < n; ++i)
+                work[v][i] = combine(work[v][i], work[v + d][i], red);
+}
+
+int lpo_mst_reduce_op(float *const *bufs, int P, size_t n, int root, int red)
+{
+    if (bad_args(bufs, P, root) || bad_red(red))
+        return LPO_EINVAL;
+    float **work = (float **)malloc((size_t)P * sizeof(float *));
+    if (!work)
+        return LPO_ENOMEM;
+    for (int v = 0; v < P; ++v) {
+        work[v] = (float *)malloc((n ? n : 1) * sizeof(float));
+        if (!work[v])
+            return LPO_ENOMEM;
+        memcpy(work[v], bufs[vrank_to_rank(v, root, P)], n * sizeof(float));
+    }
+    mst_reduce_virtual_op(work, P, n, red);
+    memcpy(bufs[root], work[0], n * sizeof(float));
+    for (int v = 0; v < P; ++v)
+        free(work[v]);
+    free(work);
+    return LPO_OK;
+}
+
+int lpo_mst_allreduce_op(float *const *bufs, int P, size_t n, int red)
+{
+    int rc = lpo_mst_reduce_op(bufs, P, n, 0, red);
+    if (rc != LPO_OK)
+        return rc;
+    return lpo_mst_broadcast(bufs, P, n, 0);
+}
+
+/* BE reduce-scatter (section 5) with operator: own_half = own_half op partner's copy of that half. */
+static void be_reduce_scatter_op(float **work, int P, size_t n, size_t *seg_lo,
+                                 size_t *seg_hi, int red)
+{
+    for (int r = 0; r < P; ++r) {
+        seg_lo[r] = 0;
+        seg_hi[r] = n;
+    }
+    for (int d = P / 2; d >= 1; d /= 2) {
+        for (int r = 0; r < P; ++r) {
+            int q = r ^ d;
+            size_t lo = seg_lo[r], hi = seg_hi[r];
+            size_t mid = lo + (hi - lo) / 2;
+            size_t klo = (r & d) ? mid : lo;
+            size_t khi = (r & d) ? hi : mid;
+            for (size_t i = klo; i < khi; ++i)
+                work[r][i] = combine(work[r][i], work[q][i], red);
+        }
+        for (int r = 0; r < P; ++r) {
+            size_t lo = seg_lo[r], hi = seg_hi[r];
+            size_t mid = lo + (hi - lo) / 2;
+            if (r & d)
+                seg_lo[r] = mid;
+            else
+                seg_hi[r] = mid;
+        }
+    }
+}
+
+int lpo_be_allreduce_op(float *const *bufs, int P, size_t n, int red)
+{
+    if (bad_args(bufs, P, 0) || bad_red(red))
+        return LPO_EINVAL;
+    if (!is_pow2(P))
+        return LPO_EUNSUPPORTED;
+    size_t *lo = (size_t *)malloc((size_t)P * sizeof(size_t));
+    size_t *hi = (size_t *)malloc((size_t)P * sizeof(size_t));
+    float **work = (float **)malloc((size_t)P * sizeof(float *));
+    if (!lo || !hi || !work)
+        return LPO_ENOMEM;
+    for (int r = 0; r < P; ++r)
+        work[r] = bufs[r];
+    be_reduce_scatter_op(work, P, n, lo, hi, red);
+    be_allgather(work, P, lo, hi);
+    free(lo);
+    free(hi);
+    free(work);
+    return LPO_OK;
+}
+
+int lpo_be_reduce_op(float *const *bufs, int P, size_t n, int root, int red)
+{
+    if (bad_args(bufs, P, root) || bad_red(red))
+        return LPO_EINVAL;
+    if (!is_pow2(P))
+        return LPO_EUNSUPPORTED;
+    size_t *lo = (size_t *)malloc((size_t)P * sizeof(size_t));
+    size_t *hi = (size_t *)malloc((size_t)P * sizeof(size_t));
+    float **work = (float **)malloc((size_t)P * sizeof(float *));
+    if (!lo || !hi || !work)
+        return LPO_ENOMEM;
+    for (int r = 0; r < P; ++r) {
+        work[r] = (float *)malloc((n ? n : 1) * sizeof(float));
+        if (!work[r])
+            return LPO_ENOMEM;
+        memcpy(work[r], bufs[r], n * sizeof(float));
+    }
+    be_reduce_scatter_op(work, P, n, lo, hi, red);
+    for (int r = 0; r < P; ++r)
+        memcpy(bufs[root] + lo[r], work[r] + lo[r], (hi[r] - lo[r]) * sizeof(float));
+    for (int r = 0; r < P; ++r)
+        free(work[r]);
+    free(lo);
+    free(hi);
+    free(work);
+    return LPO_OK;
+}
+
+/* Layer-wise reduce / allreduce with operator: the definitions above on every
+ * slice, in list order (Alg. 1).  op: 1 reduce, 2 allreduce. */
+int lpo_collective_segments_op(int op, int red, float *const *bufs, int P, size_t n,
+                               const size_t *seg_off, const size_t *seg_len,
+                               int n_seg, int root)
+{
+    if (bad_args(bufs, P, root) || bad_red(red) || n_seg < 0 ||
+        (n_seg > 0 && (!seg_off || !seg_len)) || P > 64 || (op != 1 && op != 2))
+        return LPO_EINVAL;
+    for (int s = 0; s < n_seg; ++s)
+        if (seg_off[s] > n || seg_len[s] > n - seg_off[s])
+            return LPO_EINVAL;
+    for (int s = 0; s < n_seg; ++s) {
+        float *slice[64];
+        for (int r = 0; r < P; ++r)
+            slice[r] = bufs[r] + seg_off[s];
+        int rc = op == 1 ? lpo_reduce_op(slice, P, seg_len[s], root, red)
+                         : lpo_allreduce_op(slice, P, seg_len[s], red);
+        if (rc != LPO_OK)
+            return rc;
+    }
+    return LPO_OK;
+}
+
+/* ------------------------------------------------------------------------ */
 /* 6. Cost model, Table 1, fp64                        */
 /* ------------------------------------------------------------------------ */
 
