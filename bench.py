@@ -9,7 +9,11 @@ seed 1 -- through the C ABI (lp_allreduce) with the inputs already resident in H
 n*4 bytes / t (nccl-tests convention) summed over the N replicas; `roofline.achieved` = minimum HBM bytes
 2*P*n*4 / t against the measured copy peak of MEASURED_PEAKS.json.  `e2e` = the same metric through
 lp_allreduce_host with pinned HOST buffers (H2D + kernel + D2H inside the timed region).  `cpu_baseline` /
-`--impl reference` time the CPU oracle as it stands on the box's host cores.  Prints ONE JSON line (rank 0).
+`--impl reference` time the CPU oracle as it stands on the box's host cores, on the FULL vectors of the workload.
+`detail` carries the other BASELINE.json configs, driver-measured in the same run: configs[3] from 64 MB up at
+P = 2, 3, 4, 5, 6, 8, 16 (LP vs MST vs BE, three collectives, with the HBM ceiling of the same read : write mix from a
+plain streaming kernel beside every cell), configs[4] (P=16, 138 M), configs[2] (fused BSP-SGD step, 100 iterations),
+the other ops / variants / block sizes of configs[1], and the pure-stream HBM ceilings.  Prints ONE JSON line (rank 0).
 """
 from __future__ import annotations
 
@@ -32,9 +36,9 @@ from paper_1611_04255_b200 import inputs  # noqa: E402
 METRIC = "lp_allreduce_algbw"
 UNIT = "GB/s (algbw = n*4 bytes per rank / time; roofline on min bytes 2*P*n*4)"
 FALLBACK_HBM_GBS = 6650.0  # B200_PROFILING.md fallback, used only if MEASURED_PEAKS.json is absent
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-# `ncu --set full` capture (profiles/r1_ncu_lp_pipeline.md); keyed by (P, n, variant)
-NCU_TRAFFIC_BYTES = {(6, 61_000_000, "pipeline"): 2_869_606_000}
+# roofline.traffic (dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel) cannot be measured inside
+# this program (it needs ncu's replays): the line carries null and names the committed capture of the same command
+TRAFFIC_PROFILE = "profiles/r2_ncu_lp_pipeline.md (ncu --set full of this command: read + write = 0.98 x algorithmic)"
 
 
 def parse_args():
@@ -47,6 +51,8 @@ def parse_args():
     ap.add_argument("--block", type=int, default=0, help="LP block in elements (0 = the config's)")
     ap.add_argument("--variant", default="auto", choices=["auto", "pipeline", "direct", "cluster", "copy_engine"])
     ap.add_argument("--no-detail", action="store_true", help="skip the secondary measurements")
+    ap.add_argument("--detail", default="configs1,configs2,configs4,sweep,ceilings",
+                    help="comma list of detail sections to run")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     return ap.parse_args()
@@ -154,40 +160,68 @@ def sum_over_ranks(value, world, device=None):
 
 
 # ---- the oracle on the host cores (cpu_baseline leg and --impl reference) ------------------------------
-def time_oracle(P, n_sample, dist_kind, sigma, seed, passes):
-    """Times oracle.lpo.allreduce(omp=True) as it stands on a bounded sample: the first n_sample elements of every
-    rank's vector.  Returns (seconds per pass list, cores)."""
+def time_oracle(P, n, dist_kind, sigma, seed, passes, warm=2, single_thread_passes=0):
+    """Times the oracle's allreduce as it stands on the FULL vectors of the workload (no sample): `passes` timed passes
+    of lpo_allreduce_omp (element loop over all host cores) after `warm` untimed ones, and optionally a few passes of
+    the canonical single-thread loop lpo_allreduce.  The allreduce is in place (|x| grows ~P per pass): inputs are
+    restored outside the timed region before magnitudes could overflow.  Returns (omp seconds list, cores,
+    single-thread seconds list)."""
     from oracle import lpo
-    src = inputs.rank_vectors(seed, P, n_sample, dist_kind, sigma)
+    src = inputs.rank_vectors(seed, P, n, dist_kind, sigma)
     work = [s.copy() for s in src]
-    lpo.allreduce(work, omp=True)  # warm-up (page faults, thread pool)
-    times = []
-    for _ in range(passes):
-        for w, s in zip(work, src):
-            np.copyto(w, s)
-        t0 = time.perf_counter()
-        lpo.allreduce(work, omp=True)
-        times.append(time.perf_counter() - t0)
-    return times, lpo.num_threads()
+    vmax = max(float(np.abs(h).max()) for h in src)
+    safe = max(1, int(np.floor(np.log(1e30 / max(vmax, 1e-30)) / np.log(max(P, 2)))))
+
+    def run(fn_omp, count):
+        out, used = [], 0
+        for _ in range(count):
+            if used >= safe:
+                for w, s_ in zip(work, src):
+                    np.copyto(w, s_)
+                used = 0
+            t0 = time.perf_counter()
+            lpo.allreduce(work, omp=fn_omp)
+            out.append(time.perf_counter() - t0)
+            used += 1
+        return out
+
+    run(True, warm)  # page faults, thread pool
+    omp = run(True, passes)
+    single = run(False, single_thread_passes) if single_thread_passes else []
+    return omp, lpo.num_threads(), single
+
+
+def oracle_baseline(c, cfg_idx, passes, single_thread_passes):
+    P, n = c["P"], c["n"]
+    omp, cores, single = time_oracle(P, n, c["dist"], c.get("sigma", 1.0), cfg_idx, passes,
+                                     single_thread_passes=single_thread_passes)
+    t = sum(omp) / len(omp)
+    out = {"value": n * 4 / t / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
+           "sample": f"the full workload: all {n} elements of each of the P={P} vectors ({P * n * 4 / 1e9:.2f} GB), "
+                     f"lpo_allreduce_omp, {len(omp)} timed passes after 2 warm-up passes, {t * 1e3:.1f} ms per pass "
+                     f"(min {min(omp) * 1e3:.1f})"}
+    if single:
+        ts = sum(single) / len(single)
+        out["single_thread"] = {"value": n * 4 / ts / 1e9, "unit": UNIT, "cores": 1, "ms_per_pass": ts * 1e3,
+                                "passes": len(single), "what": "lpo_allreduce: the canonical plain loop, one host thread"}
+    return out, t
 
 
 def run_reference(args, c, rank, world):
-    """--impl reference: the CPU oracle, unmodified, on the host cores.  Rank 0 only."""
+    """--impl reference: the CPU oracle, unmodified, on the host cores, on the whole workload.  Rank 0 only."""
     if rank != 0:
         return
     P, n = c["P"], c["n"]
-    n_sample = min(n, 16_000_000)
-    times, cores = time_oracle(P, n_sample, c["dist"], c.get("sigma", 1.0), args.config, args.warmup + args.steps)
-    timed = times[args.warmup:]
-    t = sum(timed) / len(timed)
-    value = n_sample * 4 / t / 1e9
-    sample = f"first {n_sample} of {n} elements per rank, P={P}, oracle lpo_allreduce_omp, {len(timed)} passes"
+    omp, cores, _ = time_oracle(P, n, c["dist"], c.get("sigma", 1.0), args.config, args.steps, warm=max(args.warmup, 1))
+    t = sum(omp) / len(omp)
+    value = n * 4 / t / 1e9
+    sample = (f"the full workload: all {n} elements of each of the P={P} vectors, oracle lpo_allreduce_omp, "
+              f"{len(omp)} timed passes after {max(args.warmup, 1)} warm-up passes")
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": t * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": f"BASELINE.json configs[{args.config}]: {c['name']}", "P": P, "n": n,
-                   "sample_n": n_sample},
+        "config": {"workload": f"BASELINE.json configs[{args.config}]: {c['name']}", "P": P, "n": n},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -294,16 +328,24 @@ def run_ours(args, c, rank, world, local):
 
     detail = None
     if rank == 0 and not args.no_detail:
-        detail = secondary(torch, lp, dev, pristine, sets[0], P, n, block, peak)
+        want = set(args.detail.split(","))
+        detail = {}
+        if "configs1" in want:
+            detail["configs1"] = cfg1_more(torch, lp, dev, pristine, sets[0], P, n, block, peak)
+        del pristine, sets
+        torch.cuda.empty_cache()
+        if "configs2" in want:
+            detail["configs2"] = cfg2_steps(torch, lp, dev, peak)
+        if "configs4" in want:
+            detail["configs4"] = cfg4_row(torch, lp, dev, peak)
+        if "sweep" in want:
+            detail["sweep"] = sweep_cfg3(torch, lp, dev, peak)
+        if "ceilings" in want:
+            detail["ceilings"] = ceilings(torch, lp, dev, peak)
 
     cpu = None
     if rank == 0 and not args.no_cpu:
-        n_sample = min(n, 16_000_000)
-        times, cores = time_oracle(P, n_sample, c["dist"], sigma, args.config, 5)
-        t = sum(times) / len(times)
-        cpu = {"value": n_sample * 4 / t / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
-               "sample": f"first {n_sample} of {n} elements per rank, P={P}, lpo_allreduce_omp, 5 passes, "
-                         f"{t * 1e3:.1f} ms per pass"}
+        cpu, _ = oracle_baseline(c, args.config, passes=20, single_thread_passes=3)
 
     if rank != 0:
         return
@@ -315,7 +357,12 @@ def run_ours(args, c, rank, world, local):
                    "variant": ran, "plan": plan, "parallelism": f"replicas x{world} (no collective)",
                    "l2": f"inputs {P * n * 4 / 1e6:.0f} MB per set >> 126 MB L2, {n_sets} rotating sets"},
         "roofline": {"bound": "hbm", "achieved": hbm, "peak": peak, "unit": "GB/s", "frac": hbm / peak,
-                     "traffic": NCU_TRAFFIC_BYTES.get((P, n, ran)), "peak_source": peak_src, "frac_of_nominal_8TBs": hbm / 8000.0,
+                     "traffic": None, "traffic_source": TRAFFIC_PROFILE, "peak_source": peak_src,
+                     "peak_note": "the measured peak is a 1 read : 1 write copy; a fraction above 1 is possible for this "
+                                  "kernel (pure write streams reach 7.4 TB/s here: detail.ceilings) and is not a ceiling "
+                                  "claim -- detail.configs1.allreduce.lp_over_ceiling compares with a plain kernel of "
+                                  "the same mix",
+                     "frac_of_nominal_8TBs": hbm / 8000.0,
                      "kernel": "lp_pipeline_kernel" if ran == "pipeline" else ran,
                      "algorithmic_bytes_per_launch": min_bytes},
         "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "detail": detail,
@@ -323,83 +370,276 @@ def run_ours(args, c, rank, world, local):
     print(json.dumps(line), flush=True)
 
 
-def secondary(torch, lp, dev, pristine, work, P, n, block, peak):
-    """Secondary measurements reported under "detail" (same inputs, same timing method, 5 timed calls each):
-    the other LP ops, the other variants, the MST baseline, the block sweep of configs[1], and the fused
-    BSP-SGD step + BE baseline on configs[2] (P=8, n=7,000,000)."""
+# ---- detail: the rest of BASELINE.json's configs, driver-measured ---------------------------------------
+L2_BYTES = 126 << 20
+SWEEP_PS = (2, 3, 4, 5, 6, 8, 16)          # 3, 5, 6: the paper's own Fig. 4 points
+SWEEP_EXPS = (24, 25, 26, 27)             # 64, 128, 256, 512 MB per rank: where north_star's 80 % bar applies
+
+
+def graph_time(torch, fn_of_set, n_sets, restore, traffic_bytes, reps=3, target_ms=2.0, k_max=400):
+    """Device time per call: K back-to-back calls captured in one CUDA graph (the host's call overhead is not billed,
+    consecutive calls overlap their launches as they do in a training loop), call i on buffer set i mod n_sets,
+    inputs restored outside the event pair; median of `reps` replays after one warm-up replay.  Returns (us, K)."""
+    est = max(traffic_bytes / 3e12, 4e-6)
+    K = int(min(max(target_ms * 1e-3 / est, 3), 20 * n_sets, k_max))
+    fn_of_set(0)  # outside capture: function attributes, scratch, claim counters
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        for i in range(K):
+            fn_of_set(i % n_sets)
+    ms = []
+    for rep in range(reps + 1):
+        restore()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        g.replay()
+        e1.record()
+        torch.cuda.synchronize()
+        if rep:
+            ms.append(e0.elapsed_time(e1) / K)
+    del g
+    return float(np.median(ms)) * 1e3, K
+
+
+def lp_call(lp, algo, op, bufs, block):
+    if algo == "lp":
+        if op == "allreduce":
+            lp.lp_allreduce(bufs, block)
+        elif op == "reduce":
+            lp.lp_reduce(bufs, block, root=0)
+        else:
+            lp.lp_broadcast(bufs, block, root=0)
+    else:
+        f = getattr(lp, f"lp_{algo}_{op}")
+        f(bufs) if op == "allreduce" else f(bufs, root=0)
+
+
+def probe_call(lp, op, bufs):
+    """The same read : write mix as `op` over the same buffers, from the plain streaming kernel (lp_hbm_probe)."""
+    if op == "allreduce":
+        lp.lp_hbm_probe(bufs, bufs)          # P reads, P writes, in place like the collective
+    elif op == "reduce":
+        lp.lp_hbm_probe(bufs, bufs[:1])      # P reads, 1 write (root 0)
+    else:
+        lp.lp_hbm_probe(bufs[:1], bufs[1:])  # 1 read, P-1 writes
+
+
+def cell(lp, torch, op, P, n, block, sets, restore, peak, algos=("lp", "mst", "be")):
+    op_id = {"broadcast": lp.OP_BROADCAST, "reduce": lp.OP_REDUCE, "allreduce": lp.OP_ALLREDUCE}[op]
+    mb = lp.lp_min_bytes(op_id, P, n)
+    row = {"P": P, "msg_MB": n * 4 / 2 ** 20, "op": op, "min_bytes": mb}
+    for algo in algos:
+        if algo == "be" and P & (P - 1):
+            continue
+        us, K = graph_time(torch, lambda s, a=algo: lp_call(lp, a, op, sets[s], block), len(sets), restore, mb)
+        row[f"{algo}_us"] = round(us, 2)
+        row[f"{algo}_GBps"] = round(mb / us / 1e3, 1)
+        row["calls_per_graph"] = K
+    # the same LP calls with stream chaining off (LP_TUNE_CHAIN 2): every call waits for its predecessor to finish
+    # before it starts, as in round 1 -- what one call costs when the NEXT one depends on it
+    lp.lp_set_tuning(lp.TUNE_CHAIN, 2)
+    us, _ = graph_time(torch, lambda s: lp_call(lp, "lp", op, sets[s], block), len(sets), restore, mb)
+    lp.lp_set_tuning(lp.TUNE_CHAIN, 0)
+    row["lp_us_unchained"] = round(us, 2)
+    row["lp_GBps_unchained"] = round(mb / us / 1e3, 1)
+    us, _ = graph_time(torch, lambda s: probe_call(lp, op, sets[s]), len(sets), restore, mb)
+    row["ceiling_GBps"] = round(mb / us / 1e3, 1)      # plain streaming kernel, same mix, same buffers, same method
+    g = row["lp_GBps"]
+    row["lp_frac_8TBs"] = round(g / 8000.0, 4)
+    row["lp_frac_8TBs_unchained"] = round(row["lp_GBps_unchained"] / 8000.0, 4)
+    row["lp_frac_measured_copy_peak"] = round(g / peak, 4)
+    row["lp_over_ceiling"] = round(g / row["ceiling_GBps"], 4)
+    if "mst_us" in row:
+        row["lp_vs_mst"] = round(row["mst_us"] / row["lp_us"], 3)
+    if "be_us" in row:
+        row["lp_vs_be"] = round(row["be_us"] / row["lp_us"], 3)
+    row["lp_variant"] = ["pipeline", "direct", "cluster", "copy_engine"][lp.lp_plan_query(op_id, P, n, block)["variant"]]
+    return row
+
+
+def sweep_cfg3(torch, lp, dev, peak, ps=SWEEP_PS, exps=SWEEP_EXPS, block=65_536):
+    """BASELINE.json configs[3] at the sizes north_star's bar applies to (>= 64 MB), plus the paper's Fig. 4 rank counts
+    3, 5, 6: LP vs MST vs BE, three collectives, uniform[-1,1] from seed [3, r]."""
+    n_max = 1 << max(exps)
+    host = [inputs.uniform(3, r, n_max) for r in range(max(ps))]
+    pristine_all = [torch.from_numpy(h).to(dev) for h in host]
+    del host
+    rows = []
+    for P in ps:
+        pristine = pristine_all[:P]
+        work = [torch.empty_like(p) for p in pristine]
+        for e in exps:
+            n = 1 << e
+            n_sets = int(max(1, min(n_max // n, 64, -(-8 * L2_BYTES // (P * n * 4)))))  # rotate through >= 1 GB
+            sets = [lp.Ranks([w[s * n:(s + 1) * n] for w in work]) for s in range(n_sets)]
+
+            def restore(n_sets=n_sets, n=n):
+                for w, p in zip(work, pristine):
+                    w[:n_sets * n].copy_(p[:n_sets * n])
+
+            for op in ("broadcast", "reduce", "allreduce"):
+                row = cell(lp, torch, op, P, n, block, sets, restore, peak)
+                row["rotating_sets"] = n_sets
+                rows.append(row)
+        del work, sets
+        torch.cuda.empty_cache()
+    del pristine_all
+    torch.cuda.empty_cache()
+    lp_rows = [r for r in rows]
+    summary = {
+        "cells": len(rows),
+        "lp_min_frac_8TBs": min(r["lp_frac_8TBs"] for r in lp_rows),
+        "lp_cells_below_0.80_of_8TBs": [f"{r['op']} P={r['P']} {int(r['msg_MB'])}MB: {r['lp_frac_8TBs']}" for r in lp_rows
+                                        if r["lp_frac_8TBs"] < 0.80],
+        "lp_min_frac_8TBs_unchained": min(r["lp_frac_8TBs_unchained"] for r in lp_rows),
+        "lp_cells_below_0.80_of_8TBs_unchained": [f"{r['op']} P={r['P']} {int(r['msg_MB'])}MB: {r['lp_frac_8TBs_unchained']}"
+                                                  for r in lp_rows if r["lp_frac_8TBs_unchained"] < 0.80],
+        "lp_min_over_ceiling": min(r["lp_over_ceiling"] for r in lp_rows),
+        "lp_min_vs_mst": min(r["lp_vs_mst"] for r in lp_rows if "lp_vs_mst" in r),
+        "lp_min_vs_be": min(r["lp_vs_be"] for r in lp_rows if "lp_vs_be" in r),
+        "lp_cells_slower_than_mst_or_be": [f"{r['op']} P={r['P']} {int(r['msg_MB'])}MB" for r in lp_rows
+                                           if r.get("lp_vs_mst", 9) < 1.0 or r.get("lp_vs_be", 9) < 1.0],
+    }
+    return {"note": "us per call = CUDA-graph replay of K back-to-back calls / K, median of 3, buffer sets rotating through "
+                    ">= 1 GB (8 x L2), inputs restored outside the event pair; GB/s on the op's minimum HBM bytes for every "
+                    "algorithm so rows compare; ceiling = lp_hbm_probe (plain streaming kernel, same read:write mix, same "
+                    "buffers); block 65,536.  Consecutive calls of a graph work on different buffer sets wherever "
+                    "rotating_sets > 1, so a call may start while its predecessor drains (LP_TUNE_CHAIN, also applied to "
+                    "MST / BE); *_unchained = the same with every call waiting for its predecessor first (round 1's method)",
+            "summary": summary, "rows": rows}
+
+
+def cfg4_row(torch, lp, dev, peak):
+    """BASELINE.json configs[4]: P=16, n=138,000,000 (VGG-16-sized), N(0,1e-3) seed 4, b=262,144 -- the largest config."""
+    c = inputs.CONFIGS[4]
+    P, n, block = c["P"], c["n"], c["block"]
+    pristine = [torch.from_numpy(inputs.normal(4, r, n, c["sigma"])).to(dev) for r in range(P)]
+    work = [torch.empty_like(p) for p in pristine]
+    sets = [lp.Ranks(work)]
+
+    def restore():
+        for w, p in zip(work, pristine):
+            w.copy_(p)
+
+    out = {"P": P, "n": n, "block": block, "footprint_GB": round(P * n * 4 / 1e9, 2)}
+    for op in ("allreduce", "reduce", "broadcast"):
+        out[op] = cell(lp, torch, op, P, n, block, sets, restore, peak)
+    del pristine, work, sets
+    torch.cuda.empty_cache()
+    return out
+
+
+def cfg2_steps(torch, lp, dev, peak):
+    """BASELINE.json configs[2]: fused BSP-SGD step, P=8, n=7,000,000, 100 iterations back to back (one CUDA graph of
+    100 steps over 3 rotating sets of gradients + weight replicas = 1.3 GB), and the f1 steps beside it."""
+    c2 = inputs.CONFIGS[2]
+    P, n, block, lr = c2["P"], c2["n"], c2["block"], c2["lr"]
+    g_h, w_h = inputs.sgd_inputs(2, P, n, c2["sigma"], c2["w_sigma"])
+    n_sets = 3
+    g0 = [torch.from_numpy(x).to(dev) for x in g_h]
+    w0 = [torch.from_numpy(x).to(dev) for x in w_h]
+    gs = [lp.Ranks([x.clone() for x in g0]) for _ in range(n_sets)]
+    ws = [lp.Ranks([x.clone() for x in w0]) for _ in range(n_sets)]
+    vel = [torch.zeros(n, device=dev) for _ in range(n_sets)]
+
+    def restore():
+        for s in range(n_sets):
+            for d, p in zip(ws[s], w0):
+                d.copy_(p)
+            for d, p in zip(gs[s], g0):
+                d.copy_(p)
+            vel[s].zero_()
+
+    out = {"P": P, "n": n, "block": block, "iterations_per_graph": 100, "rotating_sets": n_sets}
+
+    def add(name, fn, op_id):
+        mb = lp.lp_min_bytes(op_id, P, n)
+        us, K = graph_time(torch, fn, n_sets, restore, mb, k_max=100, target_ms=1e9)
+        out[name] = {"us_per_step": round(us, 2), "hbm_GBps_min_bytes": round(mb / us / 1e3, 1),
+                     "frac_8TBs": round(mb / us / 1e3 / 8000, 4), "frac_measured_copy_peak": round(mb / us / 1e3 / peak, 4),
+                     "steps_per_graph": K}
+
+    add("lp_bsp_sgd_step", lambda s: lp.lp_bsp_sgd_step(gs[s], ws[s], block, root=0, lr=lr), lp.OP_BSP_SGD)
+    add("lp_bsp_sgd_momentum_step", lambda s: lp.lp_bsp_sgd_momentum_step(gs[s], ws[s], vel[s], block, root=0, lr=lr, mu=0.9),
+        lp.OP_BSP_SGD_MOM)
+    # Alg. 2 (reduce, root update, broadcast: three launches), quoted on the FUSED step's minimum bytes so rows compare
+    add("lp_bsp_sgd_alg2_step", lambda s: lp.lp_bsp_sgd_alg2_step(gs[s], ws[s], block, root=0, lr=lr), lp.OP_BSP_SGD)
+    add("lp_allreduce_P8_7M", lambda s: lp.lp_allreduce(gs[s], block), lp.OP_ALLREDUCE)
+    add("mst_allreduce_P8_7M", lambda s: lp.lp_mst_allreduce(gs[s]), lp.OP_ALLREDUCE)
+    add("be_allreduce_P8_7M", lambda s: lp.lp_be_allreduce(gs[s]), lp.OP_ALLREDUCE)
+    us, _ = graph_time(torch, lambda s: lp.lp_hbm_probe(list(gs[s]) + [ws[s][0]], list(ws[s])), n_sets, restore,
+                       lp.lp_min_bytes(lp.OP_BSP_SGD, P, n), k_max=100, target_ms=1e9)
+    out["ceiling_GBps_same_mix"] = round(lp.lp_min_bytes(lp.OP_BSP_SGD, P, n) / us / 1e3, 1)
+    out["bar_80pct_of_8TBs_us"] = round(lp.lp_min_bytes(lp.OP_BSP_SGD, P, n) / 6400e9 * 1e6, 2)
+    return out
+
+
+def cfg1_more(torch, lp, dev, pristine, work, P, n, block, peak):
+    """configs[1] beyond the headline: reduce / broadcast, every LP variant, the block sweep (16K = the paper's 64 KB),
+    MST.  Same graph timing; one working set (1.46 GB >> L2)."""
+    sets = [lp.Ranks(work)]
+
     def restore():
         for d, p in zip(work, pristine):
             d.copy_(p)
 
-    def measure(fn, min_bytes, iters=5, restore_fn=restore):
-        ms = []
-        for it in range(iters + 2):
-            restore_fn()
-            torch.cuda.synchronize()
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            torch.cuda._sleep(200_000)  # ~0.1 ms of GPU spin: the launch below is queued before e0 fires,
-            e0.record()                 # so host-side call overhead is not billed to a 50-100 us kernel
-            fn()
-            e1.record()
-            torch.cuda.synchronize()
-            if it >= 2:
-                ms.append(e0.elapsed_time(e1))
-        t = float(np.median(ms))
-        gbs = min_bytes / (t * 1e-3) / 1e9
-        return {"ms": round(t, 4), "hbm_GBps_min_bytes": round(gbs, 1), "frac_of_measured_peak": round(gbs / peak, 4)}
-
-    out = {"note": "median of 5 single calls, inputs restored before each; min bytes per SURVEY 8(d)"}
-    mb = lambda op, p=P, m=n: lp.lp_min_bytes(op, p, m)  # noqa: E731
-    out["lp_reduce_root0"] = measure(lambda: lp.lp_reduce(work, block, root=0), mb(lp.OP_REDUCE))
-    out["lp_broadcast_root0"] = measure(lambda: lp.lp_broadcast(work, block, root=0), mb(lp.OP_BROADCAST))
+    out = {}
+    for op in ("allreduce", "reduce", "broadcast"):
+        out[op] = cell(lp, torch, op, P, n, block, sets, restore, peak, algos=("lp", "mst"))
+    mb = lp.lp_min_bytes(lp.OP_ALLREDUCE, P, n)
     cur = lp.lp_get_variant()
+    var = {}
     for name, v in (("pipeline", lp.VARIANT_PIPELINE), ("direct", lp.VARIANT_DIRECT), ("cluster", lp.VARIANT_CLUSTER)):
         lp.lp_set_variant(v)
-        out[f"lp_allreduce_{name}"] = measure(lambda: lp.lp_allreduce(work, block), mb(lp.OP_ALLREDUCE))
+        us, _ = graph_time(torch, lambda s: lp.lp_allreduce(sets[s], block), 1, restore, mb)
+        var[name] = {"us": round(us, 2), "hbm_GBps_min_bytes": round(mb / us / 1e3, 1)}
+    lp.lp_set_variant(lp.VARIANT_COPY_ENGINE)  # the paper's own design: at the paper's 64 KB block and at block = 0 (fitted optimum)
+    for label, b in (("copy_engine_block_auto", 0), ("copy_engine_block_262144", 262_144)):
+        lp.lp_allreduce(sets[0], b)  # scratch
+        torch.cuda.synchronize()
+        restore()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        lp.lp_allreduce(sets[0], b)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1)
+        var[label] = {"us": round(ms * 1e3, 1), "hbm_GBps_min_bytes": round(mb / ms / 1e6, 1),
+                      "block": int(lp.lp_auto_block(lp.OP_ALLREDUCE, P, n, lp.VARIANT_COPY_ENGINE)) if b == 0 else b}
     lp.lp_set_variant(cur)
+    out["allreduce_variants"] = var
     sweep = {}
     for b in (16_384, 65_536, 131_072, 262_144, 524_288, 1_048_576):
-        sweep[str(b)] = measure(lambda b=b: lp.lp_allreduce(work, b), mb(lp.OP_ALLREDUCE))
-    out["lp_allreduce_block_sweep"] = sweep
-    # MST moves 5(P-1)n*4 bytes; its GB/s is still quoted on the ALGORITHM's minimum bytes so rows compare
-    out["mst_allreduce"] = measure(lambda: lp.lp_mst_allreduce(work), mb(lp.OP_ALLREDUCE))
-    out["mst_reduce_root0"] = measure(lambda: lp.lp_mst_reduce(work, root=0), mb(lp.OP_REDUCE))
-    out["mst_broadcast_root0"] = measure(lambda: lp.lp_mst_broadcast(work, root=0), mb(lp.OP_BROADCAST))
-    # configs[2]: fused BSP-SGD step, P=8, n=7,000,000; BE baseline on the same 8 vectors
-    c2 = inputs.CONFIGS[2]
-    P2, n2 = c2["P"], c2["n"]
-    g_h, w_h = inputs.sgd_inputs(2, P2, n2, c2["sigma"], c2["w_sigma"])
-    g = [torch.from_numpy(x).to(dev) for x in g_h]
-    w = [torch.from_numpy(x).to(dev) for x in w_h]
-    g0 = [x.clone() for x in g]
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)  # 256 MB > L2: written between calls
+        us, _ = graph_time(torch, lambda s, b=b: lp.lp_allreduce(sets[s], b), 1, restore, mb)
+        sweep[str(b)] = {"us": round(us, 2), "hbm_GBps_min_bytes": round(mb / us / 1e3, 1)}
+    out["allreduce_block_sweep"] = sweep
+    return out
 
-    def restore2():
-        for d, p in zip(g, g0):
-            d.copy_(p)
-        flush.fill_(1)
 
-    out["lp_bsp_sgd_step_cfg2"] = measure(lambda: lp.lp_bsp_sgd_step(g, w, c2["block"], root=0, lr=c2["lr"]),
-                                          mb(lp.OP_BSP_SGD, P2, n2), restore_fn=restore2)
-    out["lp_allreduce_cfg2_P8"] = measure(lambda: lp.lp_allreduce(g, c2["block"]), mb(lp.OP_ALLREDUCE, P2, n2),
-                                          restore_fn=restore2)
-    out["be_allreduce_cfg2_P8"] = measure(lambda: lp.lp_be_allreduce(g), mb(lp.OP_ALLREDUCE, P2, n2),
-                                          restore_fn=restore2)
-    out["mst_allreduce_cfg2_P8"] = measure(lambda: lp.lp_mst_allreduce(g), mb(lp.OP_ALLREDUCE, P2, n2),
-                                           restore_fn=restore2)
-    # SURVEY 8(f)-1: momentum (PAPER.md:216) and Alg. 2 (reduce, root update, broadcast) against the fused Alg. 3
-    # step on the same configs[2] vectors; the Alg. 2 rows are quoted on the FUSED step's minimum bytes so that
-    # the rows compare (Alg. 2 itself moves (2P+4) n 4 bytes in three launches)
-    vel = torch.zeros(n2, device=dev)
-    out["lp_bsp_sgd_momentum_step_cfg2"] = measure(
-        lambda: lp.lp_bsp_sgd_momentum_step(g, w, vel, c2["block"], root=0, lr=c2["lr"], mu=0.9),
-        mb(lp.OP_BSP_SGD_MOM, P2, n2), restore_fn=restore2)
-    out["lp_bsp_sgd_alg2_step_cfg2"] = measure(
-        lambda: lp.lp_bsp_sgd_alg2_step(g, w, c2["block"], root=0, lr=c2["lr"]),
-        mb(lp.OP_BSP_SGD, P2, n2), restore_fn=restore2)
-    out["lp_bsp_sgd_alg2_momentum_step_cfg2"] = measure(
-        lambda: lp.lp_bsp_sgd_alg2_step(g, w, c2["block"], velocity=vel, root=0, lr=c2["lr"], mu=0.9),
-        mb(lp.OP_BSP_SGD_MOM, P2, n2), restore_fn=restore2)
+def ceilings(torch, lp, dev, peak):
+    """HBM ceilings of this GPU for pure and mixed streams, 512 MB per stream, lp_hbm_probe (plain kernel) and torch."""
+    n = 1 << 27
+    bufs = [torch.empty(n, device=dev) for _ in range(6)]
+    for b in bufs:
+        b.normal_()
+    out = {}
+
+    def t(fn, nbytes):
+        us, _ = graph_time(torch, lambda s: fn(), 1, lambda: None, nbytes)
+        return round(nbytes / us / 1e3, 1)
+
+    out["probe_read_only_4_streams"] = t(lambda: lp.lp_hbm_probe(bufs[:4], []), 4 * n * 4)
+    out["probe_write_only_4_streams"] = t(lambda: lp.lp_hbm_probe([], bufs[:4]), 4 * n * 4)
+    out["probe_copy_1r_1w"] = t(lambda: lp.lp_hbm_probe(bufs[:1], bufs[1:2]), 2 * n * 4)
+    out["probe_1r_5w"] = t(lambda: lp.lp_hbm_probe(bufs[:1], bufs[1:6]), 6 * n * 4)
+    out["probe_5r_1w"] = t(lambda: lp.lp_hbm_probe(bufs[:5], bufs[5:6]), 6 * n * 4)
+    out["torch_copy_1r_1w"] = t(lambda: bufs[1].copy_(bufs[0]), 2 * n * 4)
+    out["torch_fill_write_only"] = t(lambda: bufs[0].fill_(1.0), n * 4)
+    out["measured_peaks_json_hbm_gbs"] = peak
+    out["unit"] = "GB/s"
     return out
 
 

@@ -15,7 +15,10 @@
  *     and does not overlap another buffer of the same call.
  *   - `block` is the LP block size b ("we dissect a long message into
  *     fine-grained blocks"): nb = ceil(n / block), last block short (U6).
- *     Results never depend on `block`; speed does.
+ *     Results never depend on `block`; speed does only in the copy-engine variant
+ *     (profiles/r2_cost_model_fit.md).  block == 0 lets the library choose: the block
+ *     that minimises the fitted cost model of PAPER.md:81-89 (lp_optimal_block) for the
+ *     copy-engine variant, LP_DEFAULT_BLOCK elements for the others.
  *   - `cuda_stream` is a cudaStream_t (NULL = legacy default stream).  Work is
  *     enqueued on it and the call returns without a host sync; results are valid
  *     once the stream reaches that point.  `_host` entry points are synchronous.
@@ -32,9 +35,21 @@
  *     allocated lazily and freed by lp_shutdown().
  *   - There is no CPU fallback: without a CUDA device the compute entry points
  *     return LP_ERR_CUDA.
- *   * One device per process: the library binds to the CUDA device that is current at its first compute call
+ *   - One device per process: the library binds to the CUDA device that is current at its first compute call
  *     (scratch, tile-claim counters and streams live there); a call with another device current returns
- *     LP_ERR_UNSUPPORTED; lp_shutdown() unbinds.  Calls are serialised by one library-wide mutex.
+ *     LP_ERR_UNSUPPORTED; lp_shutdown() unbinds.
+ *   - Threads and streams: every entry point may be called from any host thread; calls on different streams run
+ *     concurrently on the device.  The library's lock covers only its own tables (defaults, scratch, tile-claim
+ *     counters), never a launch or a copy.  Tile-claim counters belong to the stream a call is enqueued on (launches
+ *     of one stream are ordered); a launch recorded during CUDA-graph capture gets a counter pair of its own for the
+ *     life of the process, out of LP_CAPTURE_PAIRS, after which captured launches fall back to the static schedule
+ *     (LP_TUNE_SCHED 1: same results, a few per cent slower).  MST / BE reduce scratch is per stream as well.
+ *   - Stream order: results are those of calls executed one after the other in stream order.  Internally a call may
+ *     START before its predecessors on the stream have finished when it touches none of their buffers (LP_TUNE_CHAIN);
+ *     it never COMPLETES before them, so whatever follows in the stream (or waits on an event) sees all of them done.
+ *     lp_set_variant / lp_set_tuning change process-wide DEFAULTS, read once at the start of each call; a caller that
+ *     needs its own settings (a confined comm-stream collective beside unconfined ones) uses an lp_plan.
+ *     The last-error text of lp_status_string is per thread.
  */
 #ifndef LP_COLLECTIVES_H
 #define LP_COLLECTIVES_H
@@ -55,13 +70,15 @@ extern "C" {
 
 /* ---- status codes ------------------------------------------------------- */
 #define LP_OK 0
-#define LP_ERR_INVALID_ARG 1 /* P<1, P>LP_MAX_P, NULL pointer, block==0, root out of range,
+#define LP_ERR_INVALID_ARG 1 /* P<1, P>LP_MAX_P, NULL pointer, root out of range,
                                 misaligned or overlapping buffers, unknown enum value */
-#define LP_ERR_UNSUPPORTED 2 /* BE with non-power-of-two P (U14); cluster variant: P > 16, momentum, slice lists;
+#define LP_ERR_UNSUPPORTED 2 /* BE with non-power-of-two P (U14); cluster variant: P > 16;
                                 a call from a device other than the one the library is bound to */
 #define LP_ERR_CUDA 3        /* launch / allocation / copy failure, or no device */
 
 #define LP_MAX_P 32
+#define LP_DEFAULT_BLOCK 65536 /* elements; what block == 0 means outside the copy-engine variant (BASELINE.json configs) */
+#define LP_CAPTURE_PAIRS 8192  /* tile-claim counter pairs available to launches recorded under CUDA-graph capture */
 
 /* ---- enums ---------------------------------------------------------------- */
 /* collective, PAPER.md:57 (broadcast), :59 (reduce), :61,71 (allreduce), :144-180 (BSP-SGD Alg. 3) */
@@ -71,13 +88,17 @@ extern "C" {
 #define LP_OP_BSP_SGD 3
 #define LP_OP_BSP_SGD_MOM 4  /* Alg. 3 step with momentum; for lp_plan_query / lp_min_bytes */
 
+/* reduce operator of reduce / allreduce, PAPER.md:59 (Sec. 3, Reduce): "It supports basic arithmetic operations
+ * such as summations and multiplications."  One fp32 RN operation per combine, in chain order. */
+#define LP_REDUCE_SUM 0
+#define LP_REDUCE_PROD 1
+
 /* realisation of the LP pipeline used by lp_broadcast/lp_reduce/lp_allreduce/lp_bsp_sgd_step */
 #define LP_VARIANT_PIPELINE 0    /* one persistent kernel; per CTA a TMA-bulk shared-memory ring
                                     with mbarrier full/empty flags handed producer warp -> add warps -> store warp */
 #define LP_VARIANT_DIRECT 1      /* one kernel, one CTA per tile, 128-bit register loads/stores, chain fold in registers */
 #define LP_VARIANT_CLUSTER 2     /* stage-per-rank: a thread-block cluster of P CTAs, CTA r owns rank r and hands
-                                    the running partial to CTA r+1 through distributed shared memory (P <= 16;
-                                    broadcast, reduce, allreduce, bsp_sgd_step; no momentum, no layer-wise lists) */
+                                    the running partial to CTA r+1 through distributed shared memory (P <= 16) */
 #define LP_VARIANT_COPY_ENGINE 3 /* the paper's own design: one cudaMemcpyAsync + one add kernel per (hop, block)
                                     on two streams */
 
@@ -108,7 +129,21 @@ extern "C" {
                                    few SMs' worth of CTAs, the way NCCL confines itself to a few channels */
 #define LP_TUNE_NO_PDL 9        /* 1: launch kernels without programmatic dependent launch (default 0: back-to-back
                                    collectives overlap launch latency and prologue with their predecessor's tail) */
-#define LP_TUNE_COUNT 10
+#define LP_TUNE_GRANULE_DIV 10  /* pipeline variant: a claim counts GRANULES of tile / div elements (1 (default), 2, 4, 8);
+                                   a ring slot holds a run of up to div granules.  Claims shrink from LP_TUNE_CLAIM_SLOTS
+                                   slots to one granule as the tile list runs out ("guided self-scheduling") */
+#define LP_TUNE_CLAIM_SLOTS 11  /* pipeline variant: ring slots' worth of granules per claim while the list is long (1..16, default 1) */
+#define LP_TUNE_PREFETCH 12     /* pipeline variant: 0/1 a CTA prefetches its first loads into L2 before it waits for the
+                                   predecessor kernel (programmatic dependent launch), 2 = off */
+#define LP_TUNE_CLUSTER_TILE 13 /* cluster variant: tile elements, 1024 / 2048 (default) / 4096 */
+#define LP_TUNE_CHAIN 14        /* 0/1: a call whose buffers overlap none of the calls still in flight ahead of it on its stream
+                                   does not wait for them before it starts (it waits before it ENDS, so completion order
+                                   on the stream is kept): back-to-back collectives on different buffers -- the layers of
+                                   Alg. 1, rotating buffer sets -- run into each other without a bubble; 2 = off, every
+                                   call waits for its predecessor first */
+#define LP_TUNE_DIRECT_OCC 15   /* direct variant: at most this many CTAs resident per SM (1..8; 0 = the library's choice by
+                                   collective: write-heavy launches run best with few stores in flight) */
+#define LP_TUNE_COUNT 16
 
 /* ---- LP collectives (the hot path) ----------------------------------------- */
 
@@ -124,6 +159,13 @@ LP_API int lp_reduce(float *const *bufs, int P, size_t n, size_t block, int root
 /* Allreduce, PAPER.md:61,71 (Fig. 2c): "equivalent to a reduce followed by a broadcast", pipeline filled
  * once.  bufs[r][i] <- S[i] for every r; the same bits on every rank. */
 LP_API int lp_allreduce(float *const *bufs, int P, size_t n, size_t block, void *cuda_stream);
+
+/* Reduce / allreduce with an operator: "It supports basic arithmetic operations such as summations and
+ * multiplications."  As lp_reduce / lp_allreduce with F[i] = ((bufs[0][i] op bufs[1][i]) op ...) op bufs[P-1][i],
+ * op = + (LP_REDUCE_SUM, identical to the calls above) or * (LP_REDUCE_PROD); one RN operation per combine, chain
+ * order whatever the root (U4).  Unknown reduce_op: LP_ERR_INVALID_ARG. */
+LP_API int lp_reduce_op(float *const *bufs, int P, size_t n, size_t block, int root, int reduce_op, void *cuda_stream);
+LP_API int lp_allreduce_op(float *const *bufs, int P, size_t n, size_t block, int reduce_op, void *cuda_stream);
 
 /* Fused BSP-SGD step = Alg. 3's communication + update (Eq. 5, 174, 180):
  *   S = chain sum of grads;  g = S * invP, invP = fl(1.0f / P) (U7);  t = lr * g;  w' = weights[root][i] - t;
@@ -159,8 +201,8 @@ LP_API int lp_bsp_sgd_alg2_step(float *const *grads, float *const *weights, floa
  * those of lp_broadcast / lp_reduce / lp_allreduce on that slice (bit-exact, chain order).
  * seg_off / seg_len are HOST arrays of n_seg entries, read during the call; slices may start at any element
  * (no alignment rule), may be empty, must lie inside [0, n) and must not overlap (else LP_ERR_INVALID_ARG);
- * 0 <= n_seg <= LP_MAX_SEGMENTS; lists longer than 96 slices take one launch per 96.  Not available in the
- * cluster variant (LP_ERR_UNSUPPORTED). */
+ * 0 <= n_seg <= LP_MAX_SEGMENTS; lists longer than 96 slices take one launch per 96 (the cluster variant: one launch
+ * per slice). */
 #define LP_MAX_SEGMENTS 65536
 LP_API int lp_broadcast_segments(float *const *bufs, int P, size_t n, const size_t *seg_off, const size_t *seg_len,
                                  int n_seg, size_t block, int root, void *cuda_stream);
@@ -206,12 +248,18 @@ LP_API int lp_mst_allreduce(float *const *bufs, int P, size_t n, void *cuda_stre
 LP_API int lp_be_broadcast(float *const *bufs, int P, size_t n, int root, void *cuda_stream);
 LP_API int lp_be_reduce(float *const *bufs, int P, size_t n, int root, void *cuda_stream);
 LP_API int lp_be_allreduce(float *const *bufs, int P, size_t n, void *cuda_stream);
+/* The same trees with the operator of lp_reduce_op. */
+LP_API int lp_mst_reduce_op(float *const *bufs, int P, size_t n, int root, int reduce_op, void *cuda_stream);
+LP_API int lp_mst_allreduce_op(float *const *bufs, int P, size_t n, int reduce_op, void *cuda_stream);
+LP_API int lp_be_reduce_op(float *const *bufs, int P, size_t n, int root, int reduce_op, void *cuda_stream);
+LP_API int lp_be_allreduce_op(float *const *bufs, int P, size_t n, int reduce_op, void *cuda_stream);
 
 /* ---- host-buffer entry points (end-to-end path) ------------------------------- */
 /* Same results as lp_allreduce / lp_bsp_sgd_step, but the P (2P) buffers live in HOST memory (pinned for
  * full speed; pageable works).  The message is cut into chunks that flow host -> device -> kernel -> host
  * on three streams, so the upload of chunk c+1, the LP kernel on chunk c and the download of chunk c-1
- * overlap.  Synchronous: returns when every host buffer holds its result. */
+ * overlap.  Synchronous: returns when every host buffer holds its result.  Host-buffer calls are serialised among
+ * themselves (they share the staging chunks) but do not block device-buffer calls of other threads. */
 LP_API int lp_allreduce_host(float *const *host_bufs, int P, size_t n, size_t block);
 LP_API int lp_bsp_sgd_step_host(float *const *host_grads, float *const *host_weights, int P, size_t n, size_t block,
                          int root, float lr);
@@ -241,6 +289,17 @@ LP_API double lp_cost_model(int algo, int op, double p, double n_bytes, double b
 /* The block size (bytes) that minimises lp_cost_model(LP_ALGO_LP, op, ...): sqrt(n a / ((p-1) w)), a and w the latency
  * and per-byte cost of one block exchange of `op`; clamped to n_bytes.  -1 on bad arguments. */
 LP_API double lp_optimal_block(int op, double p, double n_bytes, double alpha, double beta, double gamma);
+/* The block (ELEMENTS, a multiple of 4, in [4, n]) that block == 0 resolves to for `variant` (LP_VARIANT_AUTO: the
+ * variant that would run): lp_optimal_block with the constants fitted on B200 (profiles/r2_cost_model_fit.md; Eq. 1
+ * with A = 2 alpha per pipeline step and W = 2 beta + gamma per byte, both measured for the copy-engine variant) for
+ * LP_VARIANT_COPY_ENGINE, LP_DEFAULT_BLOCK (clamped to n) otherwise -- the persistent kernels are flat in `block`.
+ * 0 on bad arguments. */
+LP_API size_t lp_auto_block(int op, int P, size_t n, int variant);
+/* The fitted constants behind lp_auto_block, for tests and reports: alpha (s per block exchange) and beta (s/byte),
+ * gamma = 0 (folded into beta), of the copy-engine variant's allreduce over P ranks on B200.  Eq. 1
+ * takes them as independent of p -- every hop has its own link; on one GPU the p-1 hops of a block share two streams
+ * and one HBM, so both grow with p - 1 (profiles/r2_cost_model_fit.md); their ratio, all that b* needs, does not. */
+LP_API void lp_fitted_constants(int P, double *alpha, double *beta);
 
 /* How the persistent kernel will cut and spread the work for (op, P, n, block) under the current variant
  * and tuning: tile size, tile count, grid, threads, dynamic shared memory, ring depths. */
@@ -255,21 +314,65 @@ typedef struct lp_plan_info {
     uint32_t out_stages;      /* store-ring depth */
     uint32_t variant;         /* variant that will run */
     uint32_t sm_count;        /* SMs assumed (device query, 148 when no device) */
+    uint64_t block;           /* LP block in elements after block == 0 has been resolved */
+    uint32_t granule_elems;   /* pipeline variant: elements per claim granule (tile_elems for the others) */
+    uint32_t claim_granules;  /* pipeline variant: granules per claim while the list is long */
 } lp_plan_info;
 LP_API int lp_plan_query(int op, int P, size_t n, size_t block, lp_plan_info *out);
+
+/* ---- plans: per-call settings instead of process-wide defaults ------------------- */
+/* An lp_plan fixes WHAT is run (collective, operator, P, n, block, root) and HOW (variant, tuning) once; lp_plan_run
+ * enqueues it on any stream with any buffers.  Two plans with different settings (say, a comm-stream allreduce
+ * confined to 64 CTAs by LP_TUNE_GRID_LIMIT and an unconfined broadcast) run concurrently from different threads and
+ * streams without touching each other or the process defaults.  A plan is immutable after creation and may be used
+ * from several threads at once.  Results are those of the matching lp_* call (bit-exact, chain order). */
+typedef struct lp_plan lp_plan;
+typedef struct lp_plan_desc {
+    int op;                     /* LP_OP_BROADCAST / REDUCE / ALLREDUCE / BSP_SGD / BSP_SGD_MOM */
+    int reduce_op;              /* LP_REDUCE_*; must be LP_REDUCE_SUM for the SGD steps (the average) */
+    int P;
+    int root;                   /* ignored by allreduce */
+    size_t n;                   /* elements per rank vector */
+    size_t block;               /* LP block in elements, 0 = library chooses */
+    int variant;                /* LP_VARIANT_* */
+    int tuning[16];             /* indexed by LP_TUNE_*; 0 = library default */
+} lp_plan_desc;
+/* Fills *desc with defaults: allreduce, sum, variant LP_VARIANT_AUTO, block 0, tuning all 0; P, n left 0. */
+LP_API int lp_plan_desc_init(lp_plan_desc *desc);
+/* Validates the descriptor (LP_ERR_INVALID_ARG / LP_ERR_UNSUPPORTED as the matching call would) and creates the plan;
+ * no device needed. */
+LP_API int lp_plan_create(const lp_plan_desc *desc, lp_plan **plan);
+LP_API int lp_plan_destroy(lp_plan *plan);
+/* Enqueues the plan's collective on `cuda_stream`.  bufs: the P rank vectors (gradients for the SGD steps); weights:
+ * the P replicas (SGD steps, else NULL); velocity: LP_OP_BSP_SGD_MOM only, else NULL; lr, mu: SGD steps. */
+LP_API int lp_plan_run(const lp_plan *plan, float *const *bufs, float *const *weights, float *velocity, float lr,
+                       float mu, void *cuda_stream);
+/* The plan's collective on a list of slices (as lp_*_segments; not for LP_OP_BSP_SGD_MOM). */
+LP_API int lp_plan_run_segments(const lp_plan *plan, float *const *bufs, float *const *weights, const size_t *seg_off,
+                                const size_t *seg_len, int n_seg, float lr, void *cuda_stream);
+/* What lp_plan_run will launch (as lp_plan_query, under the plan's own variant and tuning). */
+LP_API int lp_plan_get_info(const lp_plan *plan, struct lp_plan_info *out);
+
+/* HBM ceiling probe (measurement aid, used by bench.py): a plain streaming kernel, no schedule and no fold, that reads
+ * n_read device vectors of n floats and writes n_write others (every thread: one 16-byte vector of each; values are
+ * summed so no load can be dropped).  It puts the same read : write mix on HBM as a collective does and so measures
+ * the ceiling that mix allows.  bufs: HOST array of n_read + n_write DEVICE pointers (reads first), 16-byte aligned;
+ * outputs may alias inputs (the in-place mix of an allreduce). */
+LP_API int lp_hbm_probe(float *const *bufs, int n_read, int n_write, size_t n, void *cuda_stream);
 
 /* Minimum HBM bytes of one call (each input read once, each output written once):
  * broadcast P*n*4, reduce (P+1)*n*4, allreduce 2*P*n*4, bsp_sgd (2P+1)*n*4, bsp_sgd with momentum (2P+3)*n*4. */
 LP_API uint64_t lp_min_bytes(int op, int P, size_t n);
 
 /* ---- control ------------------------------------------------------------------ */
-LP_API int lp_set_variant(int variant);             /* LP_VARIANT_*; affects the four LP calls */
+LP_API int lp_set_variant(int variant);             /* LP_VARIANT_*; process-wide default of the LP calls (not of plans) */
 LP_API int lp_get_variant(void);
-LP_API int lp_set_tuning(int key, int value);       /* LP_TUNE_*; value 0 restores the default */
+LP_API int lp_set_tuning(int key, int value);       /* LP_TUNE_*; process-wide default; value 0 restores the library's */
 LP_API int lp_get_tuning(int key);
 LP_API uint64_t lp_launch_count(void);              /* kernels + async copies enqueued by this library so far */
 LP_API int lp_shutdown(void);                       /* frees library scratch; safe to call twice */
-LP_API const char *lp_status_string(int status);    /* static string; appends the last CUDA error for LP_ERR_CUDA */
+LP_API const char *lp_status_string(int status);    /* static or per-thread string; carries the calling thread's last CUDA
+                                                       error for LP_ERR_CUDA */
 LP_API int lp_version(void);                        /* 10000*major + 100*minor + patch */
 
 #ifdef __cplusplus

@@ -18,8 +18,11 @@ OP_BROADCAST, OP_REDUCE, OP_ALLREDUCE, OP_BSP_SGD, OP_BSP_SGD_MOM = 0, 1, 2, 3, 
 VARIANT_PIPELINE, VARIANT_DIRECT, VARIANT_CLUSTER, VARIANT_COPY_ENGINE, VARIANT_AUTO = 0, 1, 2, 3, 4
 MODEL_STAGE, MODEL_LINK, MODEL_LINK_RING = 0, 1, 2
 TUNE_TILE_ELEMS, TUNE_STAGES, TUNE_OUT_STAGES, TUNE_CTAS_PER_SM, TUNE_CE_STREAMS, TUNE_L2_HINT, TUNE_STORE_WAIT, \
-    TUNE_SCHED, TUNE_GRID_LIMIT, TUNE_NO_PDL = range(10)
-TUNE_COUNT = 10
+    TUNE_SCHED, TUNE_GRID_LIMIT, TUNE_NO_PDL, TUNE_GRANULE_DIV, TUNE_CLAIM_SLOTS, TUNE_PREFETCH, \
+    TUNE_CLUSTER_TILE, TUNE_CHAIN, TUNE_DIRECT_OCC = range(16)
+TUNE_COUNT = 16
+REDUCE_SUM, REDUCE_PROD = 0, 1
+DEFAULT_BLOCK = 65536
 VARIANT_NAMES = {0: "pipeline", 1: "direct", 2: "cluster", 3: "copy_engine"}
 
 
@@ -33,10 +36,17 @@ class PlanInfo(ctypes.Structure):
     _fields_ = [("nb", ctypes.c_uint64), ("n_tiles", ctypes.c_uint64), ("tile_elems", ctypes.c_uint32),
                 ("grid", ctypes.c_uint32), ("threads", ctypes.c_uint32), ("smem_bytes", ctypes.c_uint32),
                 ("stages", ctypes.c_uint32), ("out_stages", ctypes.c_uint32), ("variant", ctypes.c_uint32),
-                ("sm_count", ctypes.c_uint32)]
+                ("sm_count", ctypes.c_uint32), ("block", ctypes.c_uint64), ("granule_elems", ctypes.c_uint32),
+                ("claim_granules", ctypes.c_uint32)]
 
     def as_dict(self):
         return {k: int(getattr(self, k)) for k, _ in self._fields_}
+
+
+class PlanDesc(ctypes.Structure):
+    _fields_ = [("op", ctypes.c_int), ("reduce_op", ctypes.c_int), ("P", ctypes.c_int), ("root", ctypes.c_int),
+                ("n", ctypes.c_size_t), ("block", ctypes.c_size_t), ("variant", ctypes.c_int),
+                ("tuning", ctypes.c_int * 16)]
 
 
 _lib = None
@@ -79,6 +89,23 @@ def lib() -> ctypes.CDLL:
         getattr(L, name).argtypes = [pp, i32, sz, i32, vp]
     for name in ("lp_mst_allreduce", "lp_be_allreduce"):
         getattr(L, name).argtypes = [pp, i32, sz, vp]
+    L.lp_reduce_op.argtypes = [pp, i32, sz, sz, i32, i32, vp]
+    L.lp_allreduce_op.argtypes = [pp, i32, sz, sz, i32, vp]
+    for name in ("lp_mst_reduce_op", "lp_be_reduce_op"):
+        getattr(L, name).argtypes = [pp, i32, sz, i32, i32, vp]
+    for name in ("lp_mst_allreduce_op", "lp_be_allreduce_op"):
+        getattr(L, name).argtypes = [pp, i32, sz, i32, vp]
+    L.lp_plan_desc_init.argtypes = [ctypes.POINTER(PlanDesc)]
+    L.lp_plan_create.argtypes = [ctypes.POINTER(PlanDesc), ctypes.POINTER(vp)]
+    L.lp_plan_destroy.argtypes = [vp]
+    L.lp_plan_run.argtypes = [vp, pp, pp, vp, f32, f32, vp]
+    L.lp_plan_run_segments.argtypes = [vp, pp, pp, psz, psz, i32, f32, vp]
+    L.lp_plan_get_info.argtypes = [vp, ctypes.POINTER(PlanInfo)]
+    L.lp_hbm_probe.argtypes = [pp, i32, i32, sz, vp]
+    L.lp_auto_block.argtypes = [i32, i32, sz, i32]
+    L.lp_auto_block.restype = sz
+    L.lp_fitted_constants.argtypes = [i32, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
+    L.lp_fitted_constants.restype = None
     L.lp_allreduce_host.argtypes = [pp, i32, sz, sz]
     L.lp_bsp_sgd_step_host.argtypes = [pp, pp, i32, sz, sz, i32, f32]
     L.lp_num_blocks.argtypes = [sz, sz]
@@ -207,6 +234,83 @@ def lp_bsp_sgd_step(grads, weights, block, root=0, lr=0.01, stream=None):
            "lp_bsp_sgd_step")
 
 
+def lp_reduce_op(bufs, block, reduce_op, root=0, stream=None):
+    arr, n = _dev_ptrs(bufs)
+    _check(lib().lp_reduce_op(arr, len(bufs), n, block, root, reduce_op, _stream_ptr(stream)), "lp_reduce_op")
+
+
+def lp_allreduce_op(bufs, block, reduce_op, stream=None):
+    arr, n = _dev_ptrs(bufs)
+    _check(lib().lp_allreduce_op(arr, len(bufs), n, block, reduce_op, _stream_ptr(stream)), "lp_allreduce_op")
+
+
+# ---- plans: per-call settings (variant, tuning) instead of the process-wide defaults -----------------------
+class Plan:
+    """lp_plan handle: `Plan(op, P, n, block=0, root=0, reduce_op=REDUCE_SUM, variant=VARIANT_AUTO, tuning={key: value})`;
+    `run(bufs, ...)` enqueues it on a stream.  Immutable; usable from several threads at once."""
+
+    def __init__(self, op, P, n, block=0, root=0, reduce_op=REDUCE_SUM, variant=VARIANT_AUTO, tuning=None):
+        d = PlanDesc()
+        _check(lib().lp_plan_desc_init(ctypes.byref(d)), "lp_plan_desc_init")
+        d.op, d.reduce_op, d.P, d.root, d.n, d.block, d.variant = op, reduce_op, P, root, n, block, variant
+        for k, v in (tuning or {}).items():
+            d.tuning[k] = v
+        h = ctypes.c_void_p()
+        _check(lib().lp_plan_create(ctypes.byref(d), ctypes.byref(h)), "lp_plan_create")
+        self.handle, self.op, self.P, self.n = h, op, P, n
+
+    def _ranks(self, bufs):
+        arr, n = _dev_ptrs(bufs)
+        if n != self.n or len(bufs) != self.P:
+            raise ValueError("buffers do not match the plan's P and n")
+        return arr
+
+    def run(self, bufs, weights=None, velocity=None, lr=0.0, mu=0.0, stream=None):
+        ba = self._ranks(bufs)
+        wa = self._ranks(weights) if weights is not None else None
+        _check(lib().lp_plan_run(self.handle, ba, wa, _velocity_ptr(velocity, self.n), ctypes.c_float(lr),
+                                 ctypes.c_float(mu), _stream_ptr(stream)), "lp_plan_run")
+
+    def run_segments(self, bufs, segments, weights=None, lr=0.0, stream=None):
+        ba = self._ranks(bufs)
+        wa = self._ranks(weights) if weights is not None else None
+        sg = _segments(segments)
+        _check(lib().lp_plan_run_segments(self.handle, ba, wa, sg.off, sg.len, sg.k, ctypes.c_float(lr),
+                                          _stream_ptr(stream)), "lp_plan_run_segments")
+
+    def info(self) -> dict:
+        info = PlanInfo()
+        _check(lib().lp_plan_get_info(self.handle, ctypes.byref(info)), "lp_plan_get_info")
+        return info.as_dict()
+
+    def close(self):
+        if self.handle is not None:
+            _check(lib().lp_plan_destroy(self.handle), "lp_plan_destroy")
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def lp_hbm_probe(read_bufs, write_bufs, stream=None):
+    """HBM ceiling probe: stream len(read_bufs) reads and len(write_bufs) writes of n floats each (no schedule, no fold)."""
+    arr, n = _dev_ptrs(list(read_bufs) + list(write_bufs))
+    _check(lib().lp_hbm_probe(arr, len(read_bufs), len(write_bufs), n, _stream_ptr(stream)), "lp_hbm_probe")
+
+
+def lp_auto_block(op, P, n, variant=VARIANT_AUTO) -> int:
+    return lib().lp_auto_block(op, P, n, variant)
+
+
+def lp_fitted_constants(P=6):
+    a, b = ctypes.c_double(0), ctypes.c_double(0)
+    lib().lp_fitted_constants(P, ctypes.byref(a), ctypes.byref(b))
+    return a.value, b.value
+
+
 # ---- layer-wise collectives (Alg. 1): one LP message per (offset, length) slice, one launch --------------
 class Segments:
     """A list of (offset, length) slices marshalled once into the two host arrays the C ABI takes."""
@@ -318,13 +422,27 @@ def lp_bsp_sgd_alg2_step(grads, weights, block, velocity=None, root=0, lr=0.01, 
 
 
 # ---- MST / BE baselines --------------------------------------------------------------------------------
-def _baseline(name, bufs, root, stream):
+def _baseline(name, bufs, root, stream, reduce_op=None):
     arr, n = _dev_ptrs(bufs)
     f = getattr(lib(), name)
-    if root is None:
-        _check(f(arr, len(bufs), n, _stream_ptr(stream)), name)
-    else:
-        _check(f(arr, len(bufs), n, root, _stream_ptr(stream)), name)
+    args = [arr, len(bufs), n] + ([] if root is None else [root]) + ([] if reduce_op is None else [reduce_op])
+    _check(f(*args, _stream_ptr(stream)), name)
+
+
+def lp_mst_reduce_op(bufs, reduce_op, root=0, stream=None):
+    _baseline("lp_mst_reduce_op", bufs, root, stream, reduce_op)
+
+
+def lp_mst_allreduce_op(bufs, reduce_op, stream=None):
+    _baseline("lp_mst_allreduce_op", bufs, None, stream, reduce_op)
+
+
+def lp_be_reduce_op(bufs, reduce_op, root=0, stream=None):
+    _baseline("lp_be_reduce_op", bufs, root, stream, reduce_op)
+
+
+def lp_be_allreduce_op(bufs, reduce_op, stream=None):
+    _baseline("lp_be_allreduce_op", bufs, None, stream, reduce_op)
 
 
 def lp_mst_broadcast(bufs, root=0, stream=None):

@@ -11,7 +11,6 @@
 // Reduce leaves the non-root buffers unchanged (U5): partial results of non-root ranks live in library scratch.
 #include "lp_common.cuh"
 
-cudaError_t lp_scratch_get(int slot, size_t bytes, float **ptr);  // lp_api.cu
 
 namespace {
 
@@ -25,7 +24,8 @@ inline float *rank_buf(float *const *bufs, int v, int root, int P) { return bufs
 
 }  // namespace
 
-cudaError_t lp_mst_run(int op, float *const *bufs, int P, size_t n, int root, int sm_count, cudaStream_t stream) {
+cudaError_t lp_mst_run(int op, int red_op, float *const *bufs, int P, size_t n, int root, int sm_count, bool pdl,
+                       bool chain, cudaStream_t stream) {
     if (P == 1 || n == 0) return cudaSuccess;
     LpSegJob jobs[LP_MAX_JOBS];
     float *cur[LP_MAX_P];
@@ -37,17 +37,17 @@ cudaError_t lp_mst_run(int op, float *const *bufs, int P, size_t n, int root, in
             for (int d = 1; d < P; d *= 2)
                 for (int v = 2 * d; v + d < P; v += 2 * d) {
                     float *s;
-                    LP_TRY(lp_scratch_get(v, n * sizeof(float), &s));
+                    LP_TRY(lp_scratch_get(stream, v, n * sizeof(float), &s));
                 }
         for (int d = 1; d < P; d *= 2) {
             int m = 0;
             for (int v = 0; v + d < P; v += 2 * d) {
                 float *out = cur[v];
-                if (keep_others && v != 0) LP_TRY(lp_scratch_get(v, n * sizeof(float), &out));
+                if (keep_others && v != 0) LP_TRY(lp_scratch_get(stream, v, n * sizeof(float), &out));
                 jobs[m++] = LpSegJob{out, cur[v], cur[v + d], n};
                 cur[v] = out;
             }
-            LP_TRY(lp_seg_launch(jobs, m, sm_count, stream));
+            LP_TRY(lp_seg_launch(jobs, m, sm_count, stream, pdl, red_op, chain));
         }
     }
     if (op == LP_OP_BROADCAST || op == LP_OP_ALLREDUCE) {
@@ -56,13 +56,14 @@ cudaError_t lp_mst_run(int op, float *const *bufs, int P, size_t n, int root, in
         for (int d = dmax; d >= 1; d /= 2) {
             int m = 0;
             for (int v = 0; v + d < P; v += 2 * d) jobs[m++] = LpSegJob{cur[v + d], cur[v], nullptr, n};
-            LP_TRY(lp_seg_launch(jobs, m, sm_count, stream));
+            LP_TRY(lp_seg_launch(jobs, m, sm_count, stream, pdl, red_op, chain));
         }
     }
     return cudaSuccess;
 }
 
-cudaError_t lp_be_run(int op, float *const *bufs, int P, size_t n, int root, int sm_count, cudaStream_t stream) {
+cudaError_t lp_be_run(int op, int red_op, float *const *bufs, int P, size_t n, int root, int sm_count, bool pdl,
+                      bool chain, cudaStream_t stream) {
     if (P == 1 || n == 0) return cudaSuccess;
     LpSegJob jobs[LP_MAX_JOBS];
     size_t lo[LP_MAX_P], hi[LP_MAX_P];
@@ -83,7 +84,7 @@ cudaError_t lp_be_run(int op, float *const *bufs, int P, size_t n, int root, int
                 hi[v + d] = hi[v];
                 hi[v] = mid;
             }
-            LP_TRY(lp_seg_launch(jobs, m, sm_count, stream));
+            LP_TRY(lp_seg_launch(jobs, m, sm_count, stream, pdl, red_op, chain));
         }
         for (int d = 1; d < P; d *= 2) {
             int m = 0;
@@ -91,7 +92,7 @@ cudaError_t lp_be_run(int op, float *const *bufs, int P, size_t n, int root, int
                 int q = v ^ d;
                 jobs[m++] = LpSegJob{work[v] + lo[q], work[q] + lo[q], nullptr, hi[q] - lo[q]};
             }
-            LP_TRY(lp_seg_launch(jobs, m, sm_count, stream));
+            LP_TRY(lp_seg_launch(jobs, m, sm_count, stream, pdl, red_op, chain));
             for (int v = 0; v < P; ++v) {
                 int q = v ^ d;
                 if (q < v) continue;
@@ -121,7 +122,7 @@ cudaError_t lp_be_run(int op, float *const *bufs, int P, size_t n, int root, int
             if (r == root) continue;
             size_t klo = (r & d0) ? mid : 0, khi = (r & d0) ? n : mid;
             float *s;
-            LP_TRY(lp_scratch_get(r, (khi - klo + 4) * sizeof(float), &s));
+            LP_TRY(lp_scratch_get(stream, r, (khi - klo + 4) * sizeof(float), &s));
             outp[r] = s + (klo & 3) - klo;
         }
     }
@@ -134,7 +135,7 @@ cudaError_t lp_be_run(int op, float *const *bufs, int P, size_t n, int root, int
             size_t khi = (r & d) ? hi[r] : mid;
             jobs[m++] = LpSegJob{outp[r] + klo, cur[r] + klo, cur[q] + klo, khi - klo};
         }
-        LP_TRY(lp_seg_launch(jobs, m, sm_count, stream));
+        LP_TRY(lp_seg_launch(jobs, m, sm_count, stream, pdl, red_op, chain));
         for (int r = 0; r < P; ++r) {
             size_t mid = lo[r] + (hi[r] - lo[r]) / 2;
             if (r & d)
@@ -148,7 +149,7 @@ cudaError_t lp_be_run(int op, float *const *bufs, int P, size_t n, int root, int
         int m = 0;
         for (int r = 0; r < P; ++r)
             if (r != root) jobs[m++] = LpSegJob{bufs[root] + lo[r], cur[r] + lo[r], nullptr, hi[r] - lo[r]};
-        LP_TRY(lp_seg_launch(jobs, m, sm_count, stream));
+        LP_TRY(lp_seg_launch(jobs, m, sm_count, stream, pdl, red_op, chain));
         return cudaSuccess;
     }
     for (int d = 1; d < P; d *= 2) {  // allgather by recursive doubling
@@ -157,7 +158,7 @@ cudaError_t lp_be_run(int op, float *const *bufs, int P, size_t n, int root, int
             int q = r ^ d;
             jobs[m++] = LpSegJob{cur[r] + lo[q], cur[q] + lo[q], nullptr, hi[q] - lo[q]};
         }
-        LP_TRY(lp_seg_launch(jobs, m, sm_count, stream));
+        LP_TRY(lp_seg_launch(jobs, m, sm_count, stream, pdl, red_op, chain));
         for (int r = 0; r < P; ++r) {
             int q = r ^ d;
             if (q < r) continue;

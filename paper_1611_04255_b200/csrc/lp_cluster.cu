@@ -20,6 +20,8 @@
 #include <cooperative_groups.h>
 #include <string.h>
 
+#include <atomic>
+
 #include "lp_common.cuh"
 
 namespace {
@@ -27,18 +29,21 @@ namespace {
 constexpr int kFoldWarps = 4;
 constexpr int kRetWarps = 4;
 constexpr int kClThreads = (2 + kFoldWarps + kRetWarps) * 32;  // producer, store, fold, return
-constexpr int kV = 4;                                          // float4 per fold / return thread
-constexpr int kClTile = kV * 4 * kFoldWarps * 32;              // 2048 elements: 11 slots = 88 KB, two CTAs per SM
-constexpr int kSIn = 5, kSRv = 3, kSFin = 3;
+// Tile = KV float4 per fold / return thread: KV = 2, 4, 8 -> 1024, 2048 (default), 4096 elements (LP_TUNE_CLUSTER_TILE).
+// Ring depths are launch parameters: s_in local-block slots (LP_TUNE_STAGES, default 5), s_rv receive slots for
+// partials and as many for finished tiles (LP_TUNE_OUT_STAGES, default 3).  2048 x (5 + 3 + 3) = 88 KB: two CTAs per SM.
 
 struct LpClusterArgs {
     const float *in_of[16];  // what cluster CTA x loads (NULL: nothing)
     float *out_of[16];       // where cluster CTA x stores the finished tile (NULL: nowhere)
     const float *w_root;     // SGD: weights[root], loaded by the last CTA
+    const float *vel_in;     // SGD + momentum: the velocity, loaded by the last CTA
+    uint64_t base;           // element offset of the message inside the rank vectors (slice of a layer-wise list)
     int C;
     int fold;      // reduce half active
     int ret;       // broadcast half active
     int head_tma;  // broadcast: the head's finished tile comes straight from HBM
+    int s_in, s_rv, s_fin;
 };
 
 // ---- cluster-scope PTX ------------------------------------------------------------------------------------
@@ -78,8 +83,11 @@ struct ClRing {
     }
 };
 
+template <int kV>
 __global__ void __launch_bounds__(kClThreads)
     lp_cluster_kernel(const __grid_constant__ LpArgs a, const __grid_constant__ LpClusterArgs c) {
+    constexpr int kClTile = kV * 4 * kFoldWarps * 32;
+    const int kSIn = c.s_in, kSRv = c.s_rv, kSFin = c.s_fin;
     extern __shared__ __align__(128) unsigned char lp_smem[];
     float *in_ring = reinterpret_cast<float *>(lp_smem);   // my rank's tiles (and, on the last CTA, the weight tiles)
     float *rv_ring = in_ring + kSIn * kClTile;              // partials written by CTA x-1
@@ -128,7 +136,9 @@ __global__ void __launch_bounds__(kClThreads)
     const uint64_t cid = blockIdx.x / (unsigned)C;
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
-    const bool sgd = a.epilogue == LP_EPI_SGD;
+    const bool mom = a.epilogue == LP_EPI_SGD_MOM;
+    const bool sgd = a.epilogue == LP_EPI_SGD || mom;
+    const bool prod = a.red_op == LP_REDUCE_PROD;
 
     if (warp == 0) {
         // ---------------- producer: my rank's tiles from HBM ("local block") ------------------------------------
@@ -138,12 +148,13 @@ __global__ void __launch_bounds__(kClThreads)
                 uint64_t off;
                 uint32_t len;
                 lp_tile_range(part, t, off, len);
+                off += c.base;
                 const LpTileSpan span(off, len);
                 const uint32_t bytes = span.body * 4u;
                 if (c.fold) {
-                    const int loads = (head && sgd) ? 2 : 1;
+                    const int loads = (head && sgd) ? (mom ? 3 : 2) : 1;
                     for (int k = 0; k < loads; ++k) {
-                        const float *src = k == 0 ? c.in_of[x] : c.w_root;
+                        const float *src = k == 0 ? c.in_of[x] : (k == 1 ? c.w_root : c.vel_in);
                         lp_mbar_wait(&in_empty[in.slot], in.phase ^ 1u);
                         if (bytes) {
                             lp_mbar_expect_tx(&in_full[in.slot], bytes);
@@ -175,6 +186,7 @@ __global__ void __launch_bounds__(kClThreads)
                 uint64_t off;
                 uint32_t len;
                 lp_tile_range(part, t, off, len);
+                off += c.base;
                 const LpTileSpan span(off, len);
                 lp_mbar_wait(&fin_full[fin.slot], fin.phase);
                 lp_fence_proxy_async();
@@ -200,6 +212,7 @@ __global__ void __launch_bounds__(kClThreads)
                 uint64_t off;
                 uint32_t len;
                 lp_tile_range(part, t, off, len);
+                off += c.base;
                 float4 acc[kV];
                 lp_mbar_wait(&in_full[in.slot], in.phase);
                 // A slot is handed back only after the shared-memory reads of it have RETURNED: this SM's load/store
@@ -213,7 +226,7 @@ __global__ void __launch_bounds__(kClThreads)
                     lp_mbar_wait(&rv_full[rv.slot], rv.phase);
                     const float4 *s = reinterpret_cast<const float4 *>(rv_ring + rv.slot * kClTile);
 #pragma unroll
-                    for (int v = 0; v < kV; ++v) acc[v] = lp_add4(s[ftid + v * FT], mine[ftid + v * FT]);
+                    for (int v = 0; v < kV; ++v) acc[v] = lp_combine4(s[ftid + v * FT], mine[ftid + v * FT], prod);
                     __threadfence_block();
                     __syncwarp();
                     if (lane == 0) lp_mbar_arrive(&in_empty[in.slot]);
@@ -244,11 +257,40 @@ __global__ void __launch_bounds__(kClThreads)
                     }
                     snd.advance();
                 } else {
-                    if (sgd) {  // g = S/P, w' = w_root - lr g, applied where the chain ends
+                    if (sgd && !mom) {  // g = S/P, w' = w_root - lr g, applied where the chain ends
                         lp_mbar_wait(&in_full[in.slot], in.phase);
                         const float4 *s = reinterpret_cast<const float4 *>(in_ring + in.slot * kClTile);
 #pragma unroll
                         for (int v = 0; v < kV; ++v) acc[v] = lp_sgd4(acc[v], s[ftid + v * FT], a.lr, a.invP);
+                        __threadfence_block();
+                        __syncwarp();
+                        if (lane == 0) lp_mbar_arrive(&in_empty[in.slot]);
+                        in.advance();
+                    }
+                    if (mom) {  // v' = mu v + lr g, w' = w_root - v' (U18); v' goes straight to the velocity vector
+                        float4 w[kV];
+                        lp_mbar_wait(&in_full[in.slot], in.phase);
+                        {
+                            const float4 *s = reinterpret_cast<const float4 *>(in_ring + in.slot * kClTile);
+#pragma unroll
+                            for (int v = 0; v < kV; ++v) w[v] = s[ftid + v * FT];
+                        }
+                        __threadfence_block();
+                        __syncwarp();
+                        if (lane == 0) lp_mbar_arrive(&in_empty[in.slot]);
+                        in.advance();
+                        lp_mbar_wait(&in_full[in.slot], in.phase);
+                        const LpTileSpan vspan(off, len);
+                        {
+                            const float4 *s = reinterpret_cast<const float4 *>(in_ring + in.slot * kClTile);
+#pragma unroll
+                            for (int v = 0; v < kV; ++v) {
+                                float4 vel;
+                                lp_mom4(acc[v], w[v], s[ftid + v * FT], a.lr, a.invP, a.mu, vel, acc[v]);
+                                const uint32_t e = (uint32_t)(ftid + v * FT) * 4u;
+                                if (e < vspan.body) lp_stg_stream(a.vel_out + vspan.a0 + e, vel);
+                            }
+                        }
                         __threadfence_block();
                         __syncwarp();
                         if (lane == 0) lp_mbar_arrive(&in_empty[in.slot]);
@@ -305,24 +347,86 @@ __global__ void __launch_bounds__(kClThreads)
     cooperative_groups::this_cluster().sync();  // nobody leaves while a neighbour may still write into it
 }
 
-constexpr uint32_t kClSmem = (kSIn + kSRv + kSFin) * kClTile * 4u + (2u * kSIn + 2u * kSRv + 3u * kSFin) * 8u;
+uint32_t cl_smem(uint32_t tile, int s_in, int s_rv, int s_fin) {
+    return (uint32_t)(s_in + s_rv + s_fin) * tile * 4u + (2u * s_in + 2u * s_rv + 3u * s_fin) * 8u;
+}
+
+// per kernel instantiation and device binding (lp_attr_epoch): dynamic shared memory limit + non-portable cluster size
+struct ClAttrCache {
+    std::atomic<int> bytes{0};
+    std::atomic<unsigned> epoch{0};
+};
+
+template <int KV>
+cudaError_t cl_set_attrs(uint32_t smem) {
+    static ClAttrCache cache;
+    if (cache.epoch.load() == lp_attr_epoch() && (int)smem <= cache.bytes.load()) return cudaSuccess;
+    cudaError_t e = cudaFuncSetAttribute(lp_cluster_kernel<KV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(lp_cluster_kernel<KV>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+    if (e != cudaSuccess) return e;
+    cache.epoch.store(lp_attr_epoch());
+    cache.bytes.store((int)smem);
+    return cudaSuccess;
+}
+
+template <int KV>
+cudaError_t cl_launch_t(const LpArgs &a, const LpClusterArgs &c, int P, const LpTuning &t, LpLaunch *cfg, cudaStream_t stream) {
+    cudaError_t e = cl_set_attrs<KV>(cfg->smem_bytes);
+    if (e != cudaSuccess) return e;
+    cudaLaunchConfig_t lc;
+    memset(&lc, 0, sizeof(lc));
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = (unsigned)P;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    lc.gridDim = dim3((unsigned)P, 1, 1);
+    lc.blockDim = dim3(kClThreads, 1, 1);
+    lc.dynamicSmemBytes = cfg->smem_bytes;
+    lc.stream = stream;
+    lc.attrs = attr;
+    lc.numAttrs = 1;
+    int max_clusters = 0;
+    e = cudaOccupancyMaxActiveClusters(&max_clusters, lp_cluster_kernel<KV>, &lc);
+    if (e != cudaSuccess) return e;
+    if (max_clusters <= 0) return cudaErrorNotSupported;  // a cluster of P CTAs does not fit this device
+    uint64_t clusters = (uint64_t)max_clusters;
+    if (t.v[LP_TUNE_GRID_LIMIT] && clusters > (uint64_t)t.v[LP_TUNE_GRID_LIMIT] / P)
+        clusters = (uint64_t)t.v[LP_TUNE_GRID_LIMIT] / P ? (uint64_t)t.v[LP_TUNE_GRID_LIMIT] / P : 1;
+    if (clusters > a.part.n_tiles) clusters = a.part.n_tiles;
+    cfg->grid = (uint32_t)(clusters * P);
+    lc.gridDim = dim3(cfg->grid, 1, 1);
+    lp_count_launch(1);
+    return cudaLaunchKernelEx(&lc, lp_cluster_kernel<KV>, a, c);
+}
 
 }  // namespace
 
-uint32_t lp_cluster_tile(const LpTuning &) { return (uint32_t)kClTile; }
+uint32_t lp_cluster_tile(const LpTuning &t) { return t.v[LP_TUNE_CLUSTER_TILE] ? (uint32_t)t.v[LP_TUNE_CLUSTER_TILE] : 2048u; }
 
 // `root` is needed for the broadcast chain (position j plays rank (root + j) mod P); P = number of virtual ranks.
-cudaError_t lp_cluster_launch(const LpArgs &a, int P, int root, const LpTuning &t, int sm_count, LpLaunch *cfg, bool dry_run,
-                              cudaStream_t stream) {
+cudaError_t lp_cluster_launch(const LpArgs &a, int P, int root, uint64_t base_off, const LpTuning &t, int sm_count,
+                              LpLaunch *cfg, bool dry_run, cudaStream_t stream) {
     cfg->grid = cfg->threads = cfg->smem_bytes = cfg->stages = cfg->out_stages = 0;
+    cfg->pdl = false;
+    cfg->claim = 1;
     const bool bcast = a.epilogue == LP_EPI_COPY;
-    if (P > 16 || a.epilogue == LP_EPI_SGD_MOM) return cudaErrorNotSupported;
+    if (P > 16) return cudaErrorNotSupported;
     LpClusterArgs c;
     memset(&c, 0, sizeof(c));
     c.C = P;
+    c.base = base_off;
     c.fold = bcast ? 0 : 1;
     c.ret = (bcast || a.n_out > 1) ? 1 : 0;  // allreduce / SGD / broadcast send the finished tile back down the chain
     c.head_tma = bcast ? 1 : 0;
+    const uint32_t tile = a.part.tile;
+    c.s_in = t.v[LP_TUNE_STAGES] ? t.v[LP_TUNE_STAGES] : 5;
+    c.s_rv = c.s_fin = t.v[LP_TUNE_OUT_STAGES] ? t.v[LP_TUNE_OUT_STAGES] : 3;
+    if (c.s_in < 3) c.s_in = 3;  // the head of a momentum step has three loads per tile
+    if (c.s_rv < 2) c.s_rv = c.s_fin = 2;
+    while (cl_smem(tile, c.s_in, c.s_rv, c.s_fin) > 227u * 1024u && c.s_in > 3) --c.s_in;
+    while (cl_smem(tile, c.s_in, c.s_rv, c.s_fin) > 227u * 1024u && c.s_rv > 2) c.s_fin = --c.s_rv;
+    if (cl_smem(tile, c.s_in, c.s_rv, c.s_fin) > 227u * 1024u) return cudaErrorInvalidConfiguration;
     if (!dry_run) {
         if (bcast) {  // CTA x is chain position j = C-1-x and plays rank (root + j) mod P; the head plays the root
             const float *src = a.in[0];
@@ -341,50 +445,25 @@ cudaError_t lp_cluster_launch(const LpArgs &a, int P, int root, const LpTuning &
                 c.in_of[x] = a.in[x];
                 c.out_of[x] = a.n_out > 1 ? a.out[x] : (x == P - 1 ? a.out[0] : nullptr);
             }
-            c.w_root = a.epilogue == LP_EPI_SGD ? a.in[a.n_sum] : nullptr;
+            const bool sgd = a.epilogue == LP_EPI_SGD || a.epilogue == LP_EPI_SGD_MOM;
+            c.w_root = sgd ? a.in[a.n_sum] : nullptr;
+            c.vel_in = a.epilogue == LP_EPI_SGD_MOM ? a.in[a.n_sum + 1] : nullptr;
         }
     }
     cfg->threads = kClThreads;
-    cfg->smem_bytes = kClSmem;
-    cfg->stages = kSIn;
-    cfg->out_stages = kSFin;
-    uint64_t clusters = (uint64_t)(sm_count / P);  // planning figure; the launch asks the occupancy calculator
+    cfg->smem_bytes = cl_smem(tile, c.s_in, c.s_rv, c.s_fin);
+    cfg->stages = (uint32_t)c.s_in;
+    cfg->out_stages = (uint32_t)c.s_fin;
+    uint64_t clusters = (uint64_t)(sm_count / P) * (228u * 1024u / (cfg->smem_bytes + 1024u));  // planning figure; the launch asks the occupancy calculator
     if (t.v[LP_TUNE_GRID_LIMIT] && clusters > (uint64_t)t.v[LP_TUNE_GRID_LIMIT] / P)
         clusters = (uint64_t)t.v[LP_TUNE_GRID_LIMIT] / P ? (uint64_t)t.v[LP_TUNE_GRID_LIMIT] / P : 1;
     if (clusters > a.part.n_tiles) clusters = a.part.n_tiles;
     cfg->grid = (uint32_t)(clusters * P);
     if (dry_run || a.part.n_tiles == 0) return cudaSuccess;
-
-    static bool attrs_set = false;
-    if (!attrs_set) {
-        cudaError_t e = cudaFuncSetAttribute(lp_cluster_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kClSmem);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(lp_cluster_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
-        if (e != cudaSuccess) return e;
-        attrs_set = true;
+    switch (tile) {
+        case 1024: return cl_launch_t<2>(a, c, P, t, cfg, stream);
+        case 2048: return cl_launch_t<4>(a, c, P, t, cfg, stream);
+        case 4096: return cl_launch_t<8>(a, c, P, t, cfg, stream);
+        default: return cudaErrorInvalidValue;
     }
-    cudaLaunchConfig_t lc;
-    memset(&lc, 0, sizeof(lc));
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = (unsigned)P;
-    attr[0].val.clusterDim.y = 1;
-    attr[0].val.clusterDim.z = 1;
-    lc.gridDim = dim3((unsigned)P, 1, 1);
-    lc.blockDim = dim3(kClThreads, 1, 1);
-    lc.dynamicSmemBytes = kClSmem;
-    lc.stream = stream;
-    lc.attrs = attr;
-    lc.numAttrs = 1;
-    int max_clusters = 0;
-    cudaError_t e = cudaOccupancyMaxActiveClusters(&max_clusters, lp_cluster_kernel, &lc);
-    if (e != cudaSuccess) return e;
-    if (max_clusters <= 0) return cudaErrorNotSupported;  // a cluster of P CTAs does not fit this device
-    clusters = (uint64_t)max_clusters;
-    if (t.v[LP_TUNE_GRID_LIMIT] && clusters > (uint64_t)t.v[LP_TUNE_GRID_LIMIT] / P)
-        clusters = (uint64_t)t.v[LP_TUNE_GRID_LIMIT] / P ? (uint64_t)t.v[LP_TUNE_GRID_LIMIT] / P : 1;
-    if (clusters > a.part.n_tiles) clusters = a.part.n_tiles;
-    cfg->grid = (uint32_t)(clusters * P);
-    lc.gridDim = dim3(cfg->grid, 1, 1);
-    lp_count_launch(1);
-    return cudaLaunchKernelEx(&lc, lp_cluster_kernel, a, c);
 }

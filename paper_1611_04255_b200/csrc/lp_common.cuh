@@ -11,7 +11,7 @@
 #define LP_MAX_IN (LP_MAX_P + 2)  // P gradient vectors + the root's weight vector + the velocity
 
 // Epilogues of the chain fold.
-#define LP_EPI_SUM 0   // out = ((in0 + in1) + ...) + in[n_sum-1]
+#define LP_EPI_SUM 0   // out = ((in0 op in1) op ...) op in[n_sum-1], op = a.red_op
 #define LP_EPI_SGD 1   // out = in[n_sum] - lr * (S * invP), three RN ops      PAPER.md:172,174 (U7)
 #define LP_EPI_COPY 2  // out = in0 (broadcast)
 #define LP_EPI_SGD_MOM 3  // v' = mu * in[n_sum+1] + lr * (S * invP); out = in[n_sum] - v'; vel_out = v'   PAPER.md:216 (U18)
@@ -26,6 +26,7 @@ struct LpArgs {
     int n_in;      // n_sum (+1 for SGD)
     int n_out;
     int epilogue;
+    int red_op;    // LP_REDUCE_SUM / LP_REDUCE_PROD: the operator of the fold
     float lr, invP, mu;
     float *vel_out;
     int l2_hint;
@@ -33,6 +34,18 @@ struct LpArgs {
     // Dynamic tile claims (LP_TUNE_SCHED 0): sched[0] = tiles claimed beyond the first grid-full, sched[1] = CTAs
     // that have finished claiming; the last CTA to finish zeroes both for the next launch.  NULL = static round robin.
     unsigned long long *sched;
+    // Pipeline kernels: part.tile is the GRANULE (the unit of a claim); a ring slot holds a run of up to slot_gran
+    // consecutive granules of one block; a claim takes claim_max granules, fewer towards the end of the list
+    // (remaining >> claim_shift, at least one) so that all CTAs run dry together.  Other kernels: one tile per claim.
+    uint32_t slot_gran;
+    uint32_t claim_max;
+    uint32_t claim_shift;
+    int prefetch;  // LP_TUNE_PREFETCH: L2 prefetch of a CTA's first loads before it waits for the predecessor kernel
+    // Stream chaining (LP_TUNE_CHAIN, lp_chain_admit): 1 = this launch touches no buffer of the launches that may still
+    // be running ahead of it on its stream, so it does not wait for them before it starts; one thread per CTA waits
+    // before the CTA EXITS instead, which keeps completion order on the stream.
+    int late_wait;
+    uint64_t span_elems;  // elements per rank vector (the whole vector, also for a layer-wise launch): chain ranges
     lp_partition part;
 };
 
@@ -52,6 +65,7 @@ struct LpSegParam<true> {
 struct LpLaunch {
     uint32_t grid, threads, smem_bytes, stages, out_stages;
     bool pdl;
+    uint32_t claim;  // pipeline variant: granules per claim while the list is long
 };
 
 // Tuning state resolved by the API layer (0 = default).
@@ -66,13 +80,24 @@ cudaError_t lp_pipeline_launch(const LpArgs &a, const lp_seg_table *segs, const 
                                bool dry_run, cudaStream_t stream);
 cudaError_t lp_direct_launch(const LpArgs &a, const lp_seg_table *segs, const LpTuning &t, int sm_count, LpLaunch *cfg,
                              bool dry_run, cudaStream_t stream);
-cudaError_t lp_cluster_launch(const LpArgs &a, int P, int root, const LpTuning &t, int sm_count, LpLaunch *cfg,
-                              bool dry_run, cudaStream_t stream);
-uint32_t lp_pipeline_tile(const LpTuning &t, const LpArgs &a, uint64_t n, uint64_t block);
-uint32_t lp_direct_tile(const LpTuning &t, int n_in, uint64_t n_work);
+// base_off: element offset of the message inside the rank vectors (a slice of a layer-wise list; 0 = whole vectors)
+cudaError_t lp_cluster_launch(const LpArgs &a, int P, int root, uint64_t base_off, const LpTuning &t, int sm_count,
+                              LpLaunch *cfg, bool dry_run, cudaStream_t stream);
+uint32_t lp_pipeline_tile(const LpTuning &t, const LpArgs &a, uint64_t n, uint64_t block, int sm_count);
+uint32_t lp_pipeline_granule(const LpTuning &t, uint32_t tile);
+uint32_t lp_direct_tile(const LpTuning &t, int n_sum, bool sgd, uint64_t n_work, int sm_count);
 uint32_t lp_cluster_tile(const LpTuning &t);
+// LP_TUNE_GRID_LIMIT confines the launch to fewer CTAs than the device has SMs (a collective beside compute kernels):
+// the one predicate tile choice, ring choice and variant choice share.
+inline bool lp_grid_confined(const LpTuning &t, int sm_count) {
+    return t.v[LP_TUNE_GRID_LIMIT] > 0 && t.v[LP_TUNE_GRID_LIMIT] <= sm_count;
+}
+// Function attributes (dynamic shared memory limit, non-portable cluster size) are per device: the launchers cache
+// "already set" against this epoch, which lp_shutdown() advances when it unbinds the library from its device.
+unsigned lp_attr_epoch();
 
-// Segment jobs of the MST / BE baselines: dst[i] = a[i] + b[i] (b != NULL) or dst[i] = a[i], i in [0, len).
+// Segment jobs of the MST / BE baselines: dst[i] = a[i] op b[i] (b != NULL; op = red_op of the launch) or
+// dst[i] = a[i], i in [0, len).
 struct LpSegJob {
     float *dst;
     const float *a;
@@ -80,11 +105,12 @@ struct LpSegJob {
     uint64_t len;
 };
 #define LP_MAX_JOBS 32
-cudaError_t lp_seg_launch(const LpSegJob *jobs, int n_jobs, int sm_count, cudaStream_t stream);
+cudaError_t lp_seg_launch(const LpSegJob *jobs, int n_jobs, int sm_count, cudaStream_t stream, bool pdl,
+                          int red_op = LP_REDUCE_SUM, bool chain = false);
 // Alg. 2's GradientUpdate on the root: w <- w - lr * (S * invP), or with velocity != NULL the
 // momentum form (U18), element-wise over n floats.
 cudaError_t lp_update_launch(float *w, const float *S, float *velocity, uint64_t n, float lr, float invP, float mu,
-                             cudaStream_t stream);
+                             cudaStream_t stream, bool pdl);
 
 // Programmatic dependent launch: every kernel of the library is launched with the "programmatic stream
 // serialization" attribute, tells the runtime when its CTAs have nothing left to claim (lp_pdl_trigger) and waits
@@ -109,12 +135,41 @@ cudaError_t lp_launch(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t sm
     return cudaLaunchKernelEx(&lc, kernel, static_cast<KArgs>(args)...);
 }
 
-bool lp_pdl_enabled();  // LP_TUNE_NO_PDL == 0 (read by launchers that do not get the tuning block)
+// ---- stream chaining -------------------------------------------------------------------------------------------
+// With programmatic dependent launch a kernel starts when its predecessor has TRIGGERED, not when it has finished; a
+// kernel of this library triggers once it has nothing left to claim and normally waits (griddepcontrol.wait) before it
+// touches memory.  lp_chain_admit keeps, per stream, the byte ranges of the launches that may still be running when the
+// next one starts (everything since the last launch that waited FIRST: that one cannot trigger before all its
+// predecessors have completed).  A launch that overlaps none of them may defer its wait to its end -- "late": its
+// fill overlaps their drain, yet it cannot complete before they do, so anything later in the stream still sees stream
+// order.  Returns true for late.  A launch without PDL, an overlap, an unknown predecessor (lp_chain_reset) or a
+// full table make the launch wait first, and the table restarts with it.
+struct LpRange {
+    uintptr_t lo, hi;  // bytes [lo, hi)
+};
+bool lp_chain_admit(cudaStream_t stream, const LpRange *ranges, int n, bool pdl, bool allowed);
+void lp_chain_reset(cudaStream_t stream);  // something the table does not track went into the stream
+// The ranges a launch described by LpArgs touches (whole rank vectors); returns their number (<= 2 * LP_MAX_IN).
+inline int lp_args_ranges(const LpArgs &a, LpRange *r) {
+    int m = 0;
+    const uintptr_t bytes = (uintptr_t)a.span_elems * 4u;
+    for (int i = 0; i < a.n_in; ++i) r[m++] = LpRange{(uintptr_t)a.in[i], (uintptr_t)a.in[i] + bytes};
+    for (int i = 0; i < a.n_out; ++i) r[m++] = LpRange{(uintptr_t)a.out[i], (uintptr_t)a.out[i] + bytes};
+    if (a.vel_out) r[m++] = LpRange{(uintptr_t)a.vel_out, (uintptr_t)a.vel_out + bytes};
+    return m;
+}
 
 // Launch counter (kernels + async copies enqueued by the library).
 void lp_count_launch(uint64_t k);
-// A zeroed, self-resetting {claimed, finished} counter pair for one launch (see LpArgs::sched).
-cudaError_t lp_sched_acquire(unsigned long long **pair);
+// A zeroed, self-resetting {claimed, finished} counter pair for a launch on `stream` (see LpArgs::sched): the
+// stream's own pair (launches of one stream are ordered), or a pair of its own when the stream is being captured
+// into a CUDA graph.  *pair = NULL (static schedule) when none can be had.
+cudaError_t lp_sched_acquire(cudaStream_t stream, unsigned long long **pair);
+// Library scratch for (stream, slot): grows on demand; per stream so that calls on different streams never share it.
+cudaError_t lp_scratch_get(cudaStream_t stream, int slot, size_t bytes, float **ptr);
+// key of scratch that is not tied to a caller's stream (host-path staging sets, copy-engine receive slots: both are
+// used under a lock of their own, on streams the library owns)
+#define LP_SCRATCH_SHARED ((cudaStream_t)(intptr_t)-1)
 
 #if defined(__CUDACC__)
 __device__ __forceinline__ void lp_pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
@@ -213,6 +268,14 @@ __device__ __forceinline__ void lp_stg_stream(float *p, const float4 &v) {
 __device__ __forceinline__ float4 lp_add4(const float4 &a, const float4 &b) {
     return make_float4(__fadd_rn(a.x, b.x), __fadd_rn(a.y, b.y), __fadd_rn(a.z, b.z), __fadd_rn(a.w, b.w));
 }
+__device__ __forceinline__ float4 lp_mul4(const float4 &a, const float4 &b) {
+    return make_float4(__fmul_rn(a.x, b.x), __fmul_rn(a.y, b.y), __fmul_rn(a.z, b.z), __fmul_rn(a.w, b.w));
+}
+// partial op local block ("summations and multiplications"); `prod` is uniform over the launch
+__device__ __forceinline__ float4 lp_combine4(const float4 &a, const float4 &b, bool prod) {
+    return prod ? lp_mul4(a, b) : lp_add4(a, b);
+}
+__device__ __forceinline__ float lp_combine1(float a, float b, bool prod) { return prod ? __fmul_rn(a, b) : __fadd_rn(a, b); }
 // w' = w - lr * (s * invP): three separately rounded operations (U7)
 __device__ __forceinline__ float lp_sgd1(float s, float w, float lr, float invP) {
     return __fsub_rn(w, __fmul_rn(lr, __fmul_rn(s, invP)));
@@ -235,28 +298,56 @@ __device__ __forceinline__ float4 lp_sgd4(const float4 &s, const float4 &w, floa
                        lp_sgd1(s.w, w.w, lr, invP));
 }
 
-// The a2 schedule of one persistent CTA (lp_schedule.h): which tile it works on next.  Its first tile is
-// blockIdx.x; after that either the next unclaimed tile of the launch (dynamic: one atomicAdd per tile, issued
-// one tile ahead so its latency hides behind the current tile's loads) or blockIdx.x + k * gridDim.x (static).
-// SMs do not get equal shares of HBM bandwidth when the memory system is saturated; with static shares the
-// slow SMs finish last and alone, with claims every SM is busy until the tile list is empty.
+// The a2 schedule of one persistent CTA (lp_schedule.h): which tiles it works on next.  A claim is a range of
+// consecutive tile indices.  The first claim is static (claim_max tiles from blockIdx.x * claim_max); every further
+// one comes from the launch's device counter (one atomicAdd per claim, issued one claim ahead so its latency hides
+// behind the current loads), or -- static schedule -- lies gridDim.x * claim_max further on.
+// Why claims: SMs do not get equal shares of HBM bandwidth when the memory system is saturated; with static shares
+// the slow SMs finish last and alone.  Why they shrink ("guided self-scheduling"): a CTA's ring holds work it has
+// claimed but not finished, and what it claims last it finishes last; with claims of remaining / (2 * grid) tiles
+// the work in hand shrinks with the list and all CTAs run dry within one small tile of each other -- on a 64 MB
+// message the fixed-size tail was 2-6 us of a 20-90 us call.
+struct LpClaim {
+    uint64_t g0, g1;  // tiles [g0, g1); g0 >= n_tiles: none left
+};
 struct LpTileClaimer {
     unsigned long long *ctr;
-    uint64_t next, n_tiles;
-    __device__ __forceinline__ LpTileClaimer(unsigned long long *c, uint64_t nt) : ctr(c), next(blockIdx.x), n_tiles(nt) {}
-    // tile to work on now (>= n_tiles: none left)
-    __device__ __forceinline__ uint64_t claim() {
-        const uint64_t t = next;
-        if (t < n_tiles) next = ctr ? (uint64_t)gridDim.x + atomicAdd(ctr, 1ull) : t + gridDim.x;
-        return t;
+    uint64_t n_tiles, next0, next1;
+    uint32_t cmax, shift;
+    __device__ __forceinline__ LpTileClaimer(unsigned long long *c, uint64_t nt, uint32_t claim_max, uint32_t claim_shift)
+        : ctr(c), n_tiles(nt), cmax(claim_max ? claim_max : 1u), shift(claim_shift) {
+        next0 = (uint64_t)blockIdx.x * cmax;
+        next1 = next0 + cmax;
     }
-    // after the last claim: count this CTA out; the last one re-arms the pair for the next launch
+    // the first claim, without consuming it (for prefetching)
+    __device__ __forceinline__ LpClaim peek() const {
+        LpClaim c{next0, next1 < n_tiles ? next1 : n_tiles};
+        return c;
+    }
+    __device__ __forceinline__ LpClaim claim() {
+        LpClaim c{next0, next1 < n_tiles ? next1 : n_tiles};
+        if (c.g0 < n_tiles) {
+            if (ctr) {
+                const uint64_t rem = n_tiles > next1 ? n_tiles - next1 : 0;  // tiles nobody has claimed yet, at most
+                uint64_t size = rem >> shift;
+                size = size < 1 ? 1 : (size > cmax ? cmax : size);
+                next0 = (uint64_t)gridDim.x * cmax + atomicAdd(ctr, (unsigned long long)size);
+                next1 = next0 + size;
+            } else {
+                next0 += (uint64_t)gridDim.x * cmax;
+                next1 = next0 + cmax;
+            }
+        }
+        return c;
+    }
+    // after the last claim and BEFORE griddepcontrol.launch_dependents: count this CTA out; the last one re-arms the
+    // pair for the next launch (which starts only once every CTA of this one has triggered)
     __device__ __forceinline__ void finish() {
         if (!ctr) return;
         __threadfence();
         if (atomicAdd(ctr + 1, 1ull) == (unsigned long long)gridDim.x - 1ull) {
-            ctr[0] = 0ull;
-            ctr[1] = 0ull;
+            atomicExch(ctr, 0ull);  // at L2, where the next launch's claims are served (it may start without waiting
+            atomicExch(ctr + 1, 0ull);  // for this kernel to END, but not before every CTA has got past this point)
             __threadfence();
         }
     }
@@ -270,6 +361,31 @@ __device__ __forceinline__ void lp_lookup_tile(const LpArgs &a, const typename L
         lp_seg_tile_range(segs, a.part.block, a.part.tile, t, off, len);
     else
         lp_tile_range(a.part, t, off, len);
+}
+
+// The run of tiles that starts at tile g and ends before g1, at the end of g's block or after `max_run` tiles,
+// whichever comes first: one contiguous element range [off, off + len); returns the number of tiles in it.
+template <bool SEG>
+__device__ __forceinline__ uint64_t lp_lookup_run(const LpArgs &a, const typename LpSegParam<SEG>::type &segs, uint64_t g,
+                                                  uint64_t g1, uint32_t max_run, uint64_t &off, uint32_t &len) {
+    uint64_t left, bend;
+    uint32_t len1;
+    if constexpr (SEG)
+        lp_seg_tile_range_ex(segs, a.part.block, a.part.tile, g, off, len1, left, bend);
+    else
+        lp_tile_range_ex(a.part, g, off, len1, left, bend);
+    uint64_t run = g1 - g;
+    if (run > left) run = left;
+    if (run > max_run) run = max_run;
+    const uint64_t span = run * (uint64_t)a.part.tile;
+    len = off + span <= bend ? (uint32_t)span : (uint32_t)(bend - off);
+    return run;
+}
+
+// L2 prefetch of [p, p + bytes) (a hint: L2 is the point of coherence, so it is safe even while the predecessor
+// kernel is still writing); bytes a multiple of 16.
+__device__ __forceinline__ void lp_prefetch_l2(const void *p, uint32_t bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
 }
 
 // A tile [off, off + len) of 16-byte aligned vectors splits into a 16-byte aligned body [a0, a1) that the bulk
@@ -297,7 +413,8 @@ struct LpTileSpan {
 // epilogue and fan-out for element i, straight from and to global memory.
 __device__ __forceinline__ void lp_scalar_element(const LpArgs &a, uint64_t i) {
     float s = a.in[0][i];
-    for (int r = 1; r < a.n_sum; ++r) s = __fadd_rn(s, a.in[r][i]);
+    const bool prod = a.red_op == LP_REDUCE_PROD;
+    for (int r = 1; r < a.n_sum; ++r) s = lp_combine1(s, a.in[r][i], prod);
     if (a.epilogue == LP_EPI_SGD) s = lp_sgd1(s, a.in[a.n_sum][i], a.lr, a.invP);
     if (a.epilogue == LP_EPI_SGD_MOM) {
         float v_new, w_new;

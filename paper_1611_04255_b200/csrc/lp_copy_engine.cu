@@ -8,12 +8,15 @@
 // back down the chain (U3 reading A); the fused SGD step applies the update at the last rank and sends w'.
 // On one B200 this is bound by launch / copy-submission overhead (2-3 operations per hop per block), which
 // is exactly why the product path is the persistent kernel.
-#include "lp_common.cuh"
+#include <mutex>
 
-cudaError_t lp_scratch_get(int slot, size_t bytes, float **ptr);  // lp_api.cu
+#include "lp_common.cuh"
 
 namespace {
 
+// The side streams, their events and the receive slots are one set per process: calls of this variant are enqueued
+// one at a time (g_ce_mu) and run one after the other on the side streams, whatever streams the callers use.
+std::mutex g_ce_mu;
 constexpr int kMaxStreams = 8;
 cudaStream_t g_side[kMaxStreams];
 cudaEvent_t g_fork, g_join[kMaxStreams];
@@ -63,6 +66,7 @@ cudaError_t copy_block(float *dst, const float *src, uint64_t len, cudaStream_t 
 }  // namespace
 
 void lp_copy_engine_shutdown() {
+    std::lock_guard<std::mutex> lock(g_ce_mu);
     for (int s = 0; s < g_n_side; ++s) cudaStreamDestroy(g_side[s]);
     g_n_side = 0;
     if (g_events) {
@@ -73,9 +77,10 @@ void lp_copy_engine_shutdown() {
 }
 
 // op: LP_OP_*.  For LP_OP_BSP_SGD `bufs` are the gradients and `weights` the replicas.
-cudaError_t lp_copy_engine_run(int op, float *const *bufs, float *const *weights, float *velocity, int P, size_t n,
-                               size_t block, int root, float lr, float mu, const LpTuning &t, int sm_count,
+cudaError_t lp_copy_engine_run(int op, int red_op, float *const *bufs, float *const *weights, float *velocity, int P,
+                               size_t n, size_t block, int root, float lr, float mu, const LpTuning &t, int sm_count,
                                cudaStream_t stream) {
+    std::lock_guard<std::mutex> lock(g_ce_mu);
     const bool sgd = (op == LP_OP_BSP_SGD || op == LP_OP_BSP_SGD_MOM);
     if (n == 0) return cudaSuccess;
     if (P == 1 && !sgd) return cudaSuccess;
@@ -90,7 +95,7 @@ cudaError_t lp_copy_engine_run(int op, float *const *bufs, float *const *weights
     const bool reduces = (op != LP_OP_BROADCAST);
     if (reduces)
         for (int r = (P == 1 ? 0 : 1); r < P; ++r)
-            LP_TRY(lp_scratch_get(LP_MAX_P + r, (size_t)S * (block + 4) * sizeof(float), &recv[r]));
+            LP_TRY(lp_scratch_get(LP_SCRATCH_SHARED, LP_MAX_P + r, (size_t)S * (block + 4) * sizeof(float), &recv[r]));
 
     LP_TRY(cudaEventRecord(g_fork, stream));
     for (int s = 0; s < S; ++s) LP_TRY(cudaStreamWaitEvent(g_side[s], g_fork, 0));
@@ -115,8 +120,8 @@ cudaError_t lp_copy_engine_run(int op, float *const *bufs, float *const *weights
             float *dst = slot;
             if (r == P - 1 && op == LP_OP_REDUCE) dst = bufs[root] + off;  // "returns the combined value ... to a specific GPU"
             if (r == P - 1 && op == LP_OP_ALLREDUCE) dst = bufs[P - 1] + off;
-            LpSegJob job{dst, slot, bufs[r] + off, len};  // partial + local block, RN
-            LP_TRY(lp_seg_launch(&job, 1, sm_count, st));
+            LpSegJob job{dst, slot, bufs[r] + off, len};  // partial op local block, RN
+            LP_TRY(lp_seg_launch(&job, 1, sm_count, st, false, red_op));
             partial = dst;
         }
         if (op == LP_OP_ALLREDUCE) {

@@ -4,11 +4,21 @@
 // parallelism replaces the paper's two DMA engines), folds them in rank order 0 -> P-1 with RN adds and
 // writes the finished vector to every destination rank.  It is also the path that takes any alignment:
 // a tile whose start is not a multiple of 4 elements (block % 4 != 0) gets a scalar head and tail.
+#include <atomic>
+
 #include "lp_common.cuh"
 
 namespace {
 
 constexpr int kThreads = 256;
+
+// CTAs per SM the launch is capped at (8 = no cap: 2048 threads).  A thread's stores are fire-and-forget, so a
+// write-heavy launch (broadcast to several ranks) keeps far more bytes in flight per CTA than it has loaded; beyond a
+// few CTAs per SM the extra stores only queue up in front of the L2 (profiles/r2_tuning.md).
+uint32_t lp_direct_occupancy(const LpArgs &a) {
+    if (a.epilogue == LP_EPI_COPY && a.n_out >= 2) return 3u;
+    return 8u;
+}
 // ranks whose loads are in flight together: 8, or 16 for the one-vector-per-thread kernels of the latency regime (a
 // 16-rank chain then costs one HBM latency, not two)
 template <int V>
@@ -17,18 +27,23 @@ struct LpRankChunk {
 };
 
 // NS > 0: number of folded inputs known at compile time (loops fully unrolled); NS == 0: runtime a.n_sum.
-template <int NS, int V, bool SEG>
+// SGD: the launch has an SGD epilogue (plain or momentum, a.epilogue); false keeps the weight / velocity registers
+// out of the copy / fold kernels (a broadcast thread then needs 8 V + ~20 registers: 4 CTAs of 8 vectors per thread
+// = 128 KB of loads in flight per SM).
+template <int NS, int V, bool SEG, bool SGD>
 __global__ void __launch_bounds__(kThreads)
     lp_direct_kernel(const __grid_constant__ LpArgs a, const __grid_constant__ typename LpSegParam<SEG>::type segs) {
     const int n_sum = NS > 0 ? NS : a.n_sum;
     const int tid = threadIdx.x;
+    const bool prod = a.red_op == LP_REDUCE_PROD;
     // a2: one CTA per tile by default (grid == n_tiles): the hardware block scheduler hands the next tile to
     // whichever SM frees up first -- the same balance the pipeline kernel gets from its tile claims, with no
     // per-CTA setup at all, which is what the latency regime wants.  A confined grid (LP_TUNE_GRID_LIMIT /
     // LP_TUNE_CTAS_PER_SM) walks the tile list round robin.
     // wait first, then trigger: at most ONE successor waits behind a running kernel (triggering before the wait lets
     // a whole queue of short kernels pile up on the SMs, each blocked on its predecessor: measured 2x slower at 256 KB)
-    lp_pdl_wait();
+    // A launch that touches none of the buffers of the launches ahead of it (a.late_wait) waits before it exits instead.
+    if (!a.late_wait) lp_pdl_wait();
     lp_pdl_trigger();  // every CTA of this grid is resident or done once the last one gets here
     for (uint64_t t = blockIdx.x; t < a.part.n_tiles; t += gridDim.x) {
         uint64_t off;
@@ -42,22 +57,23 @@ __global__ void __launch_bounds__(kThreads)
         const uint32_t nvec = (uint32_t)((a1 - a0) >> 2);
         if ((uint64_t)tid < a0 - off) lp_scalar_element(a, off + tid);
         if ((uint64_t)tid < end - a1) lp_scalar_element(a, a1 + tid);
+        const uint64_t e0 = a0 + 4 * (uint64_t)tid;  // this thread's first element; vector v is v * 4 * kThreads further on
 
         float4 acc[V];
-        float4 w[V];
+        float4 w[SGD ? V : 1];
+        float4 vel[SGD ? V : 1];
         bool live[V];
 #pragma unroll
         for (int v = 0; v < V; ++v) live[v] = (uint32_t)(tid + v * kThreads) < nvec;
-        float4 vel[V];
-        if (a.epilogue == LP_EPI_SGD || a.epilogue == LP_EPI_SGD_MOM) {
+        if constexpr (SGD) {
 #pragma unroll
             for (int v = 0; v < V; ++v)
-                if (live[v]) w[v] = lp_ldg_stream(a.in[n_sum] + a0 + 4 * (uint64_t)(tid + v * kThreads));
-        }
-        if (a.epilogue == LP_EPI_SGD_MOM) {
+                if (live[v]) w[v] = lp_ldg_stream(a.in[n_sum] + e0 + (uint64_t)(v * 4 * kThreads));
+            if (a.epilogue == LP_EPI_SGD_MOM) {
 #pragma unroll
-            for (int v = 0; v < V; ++v)
-                if (live[v]) vel[v] = lp_ldg_stream(a.in[n_sum + 1] + a0 + 4 * (uint64_t)(tid + v * kThreads));
+                for (int v = 0; v < V; ++v)
+                    if (live[v]) vel[v] = lp_ldg_stream(a.in[n_sum + 1] + e0 + (uint64_t)(v * 4 * kThreads));
+            }
         }
         constexpr int kRankChunk = LpRankChunk<V>::value;
         for (int r0 = 0; r0 < n_sum; r0 += kRankChunk) {
@@ -67,51 +83,81 @@ __global__ void __launch_bounds__(kThreads)
                 if (NS > 0 ? (r0 + j < NS) : (r0 + j < n_sum)) {
 #pragma unroll
                     for (int v = 0; v < V; ++v)
-                        if (live[v]) x[v][j] = lp_ldg_stream(a.in[r0 + j] + a0 + 4 * (uint64_t)(tid + v * kThreads));
+                        if (live[v]) x[v][j] = lp_ldg_stream(a.in[r0 + j] + e0 + (uint64_t)(v * 4 * kThreads));
                 }
             }
 #pragma unroll
             for (int j = 0; j < kRankChunk; ++j) {
                 if (NS > 0 ? (r0 + j < NS) : (r0 + j < n_sum)) {
 #pragma unroll
-                    for (int v = 0; v < V; ++v) acc[v] = (r0 + j == 0) ? x[v][j] : lp_add4(acc[v], x[v][j]);
+                    for (int v = 0; v < V; ++v) acc[v] = (r0 + j == 0) ? x[v][j] : lp_combine4(acc[v], x[v][j], prod);
                 }
             }
         }
-        if (a.epilogue == LP_EPI_SGD) {
+        if constexpr (SGD) {
+            if (a.epilogue == LP_EPI_SGD) {
 #pragma unroll
-            for (int v = 0; v < V; ++v) acc[v] = lp_sgd4(acc[v], w[v], a.lr, a.invP);
-        }
-        if (a.epilogue == LP_EPI_SGD_MOM) {  // v' to the velocity vector, w' goes on as the finished tile
+                for (int v = 0; v < V; ++v) acc[v] = lp_sgd4(acc[v], w[v], a.lr, a.invP);
+            } else {  // momentum: v' to the velocity vector, w' goes on as the finished tile
 #pragma unroll
-            for (int v = 0; v < V; ++v) {
-                lp_mom4(acc[v], w[v], vel[v], a.lr, a.invP, a.mu, vel[v], acc[v]);
-                if (live[v]) lp_stg_stream(a.vel_out + a0 + 4 * (uint64_t)(tid + v * kThreads), vel[v]);
+                for (int v = 0; v < V; ++v) {
+                    lp_mom4(acc[v], w[v], vel[v], a.lr, a.invP, a.mu, vel[v], acc[v]);
+                    if (live[v]) lp_stg_stream(a.vel_out + e0 + (uint64_t)(v * 4 * kThreads), vel[v]);
+                }
             }
         }
         for (int q = 0; q < a.n_out; ++q) {
 #pragma unroll
             for (int v = 0; v < V; ++v)
-                if (live[v]) lp_stg_stream(a.out[q] + a0 + 4 * (uint64_t)(tid + v * kThreads), acc[v]);
+                if (live[v]) lp_stg_stream(a.out[q] + e0 + (uint64_t)(v * 4 * kThreads), acc[v]);
         }
     }
+    if (a.late_wait && tid == 0) lp_pdl_wait();  // this CTA does not exit before the launches ahead of it have completed
+}
+
+// One instantiation's launch.  cfg.smem_bytes > 0 is dynamic shared memory the kernel never touches: it caps how many
+// CTAs an SM holds (LP_TUNE_DIRECT_OCC), i.e. how many stores the SM keeps in flight.
+template <int NS, int V, bool SEG, bool SGD>
+cudaError_t launch_k(const LpArgs &a, const typename LpSegParam<SEG>::type &segs, const LpLaunch &cfg, cudaStream_t stream) {
+    if (cfg.smem_bytes > 48u * 1024u) {
+        static std::atomic<int> bytes{0};
+        static std::atomic<unsigned> epoch{0};
+        if (epoch.load() != lp_attr_epoch() || (int)cfg.smem_bytes > bytes.load()) {
+            cudaError_t e = cudaFuncSetAttribute(lp_direct_kernel<NS, V, SEG, SGD>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                 (int)cfg.smem_bytes);
+            if (e != cudaSuccess) return e;
+            epoch.store(lp_attr_epoch());
+            bytes.store((int)cfg.smem_bytes);
+        }
+    }
+    return lp_launch(lp_direct_kernel<NS, V, SEG, SGD>, dim3(cfg.grid), dim3(cfg.threads), cfg.smem_bytes, stream, cfg.pdl, a,
+                     segs);
 }
 
 template <int V, bool SEG>
 cudaError_t launch_v(const LpArgs &a, const typename LpSegParam<SEG>::type &segs, const LpLaunch &cfg, cudaStream_t stream) {
-#define LP_DIRECT_CASE(NS)                                                                  \
-    case NS:                                                                                \
-        return lp_launch(lp_direct_kernel<NS, V, SEG>, dim3(cfg.grid), dim3(cfg.threads), 0, stream, cfg.pdl, a, segs);
+    const bool sgd = a.epilogue == LP_EPI_SGD || a.epilogue == LP_EPI_SGD_MOM;
+#define LP_DIRECT_CASE(NS, SGD) \
+    case NS: return launch_k<NS, V, SEG, SGD>(a, segs, cfg, stream);
+    if (sgd) {
+        switch (a.n_sum) {
+            LP_DIRECT_CASE(2, true)
+            LP_DIRECT_CASE(4, true)
+            LP_DIRECT_CASE(8, true)
+            LP_DIRECT_CASE(16, true)
+            default: return launch_k<0, V, SEG, true>(a, segs, cfg, stream);
+        }
+    }
     switch (a.n_sum) {
-        LP_DIRECT_CASE(1)
-        LP_DIRECT_CASE(2)
-        LP_DIRECT_CASE(3)
-        LP_DIRECT_CASE(4)
-        LP_DIRECT_CASE(6)
-        LP_DIRECT_CASE(8)
-        LP_DIRECT_CASE(16)
-        default:
-            return lp_launch(lp_direct_kernel<0, V, SEG>, dim3(cfg.grid), dim3(cfg.threads), 0, stream, cfg.pdl, a, segs);
+        LP_DIRECT_CASE(1, false)
+        LP_DIRECT_CASE(2, false)
+        LP_DIRECT_CASE(3, false)
+        LP_DIRECT_CASE(4, false)
+        LP_DIRECT_CASE(5, false)
+        LP_DIRECT_CASE(6, false)
+        LP_DIRECT_CASE(8, false)
+        LP_DIRECT_CASE(16, false)
+        default: return launch_k<0, V, SEG, false>(a, segs, cfg, stream);
     }
 #undef LP_DIRECT_CASE
 }
@@ -124,20 +170,25 @@ cudaError_t launch_seg(const LpArgs &a, const lp_seg_table *segs, const LpLaunch
 
 }  // namespace
 
-// 8 KB tiles (2 vectors per thread and rank); 4 KB when the message has fewer tiles than two grid-fulls of SMs
-// (latency regime: spread it over more SMs).
-uint32_t lp_direct_tile(const LpTuning &t, int /*n_in*/, uint64_t n_work) {
+// Tile = V * 1024 elements, V 16-byte vectors per thread and input stream.  What the kernel needs is enough load bytes
+// in flight per SM (HBM latency x the SM's share of the bandwidth: ~100 KB): a thread has V * n_sum loads outstanding
+// and the registers they take decide how many CTAs an SM holds, so few streams want long tiles and many streams short
+// ones -- 16 KB (V = 4, 32 / 64 registers: 8 / 4 CTAs) for a copy and a 2-rank fold, 8 KB from 3 to 8 ranks, 4 KB
+// (16 ranks' loads at once, 2 CTAs) above: ~128 KB in flight in every case (profiles/r2_tuning.md).  4 KB also when
+// the message has fewer tiles than two grid-fulls of SMs (latency regime: spread it over more SMs).
+uint32_t lp_direct_tile(const LpTuning &t, int n_sum, bool sgd, uint64_t n_work, int sm_count) {
     if (t.v[LP_TUNE_TILE_ELEMS]) {
         const uint32_t tile = (uint32_t)t.v[LP_TUNE_TILE_ELEMS];
-        return (tile == 1024u || tile == 2048u || tile == 4096u) ? tile : 2048u;
+        return tile <= 4096u ? tile : 4096u;
     }
-    uint32_t tile = 2048u;
-    if ((n_work + tile - 1) / tile < 2u * 148u) tile = 1024u;
+    uint32_t tile = (!sgd && n_sum <= 2) ? 4096u : (n_sum <= 8 ? 2048u : 1024u);
+    while (tile > 1024u && (n_work + tile - 1) / tile < 2ull * (uint64_t)sm_count) tile /= 2u;
     return tile;
 }
 
-cudaError_t lp_direct_launch(const LpArgs &a, const lp_seg_table *segs, const LpTuning &t, int sm_count, LpLaunch *cfg,
+cudaError_t lp_direct_launch(const LpArgs &a_in, const lp_seg_table *segs, const LpTuning &t, int sm_count, LpLaunch *cfg,
                              bool dry_run, cudaStream_t stream) {
+    LpArgs a = a_in;
     uint64_t grid = a.part.n_tiles;  // one CTA per tile
     if (t.v[LP_TUNE_CTAS_PER_SM]) grid = (uint64_t)sm_count * (uint32_t)t.v[LP_TUNE_CTAS_PER_SM];
     if (t.v[LP_TUNE_GRID_LIMIT] && grid > (uint64_t)t.v[LP_TUNE_GRID_LIMIT]) grid = (uint64_t)t.v[LP_TUNE_GRID_LIMIT];
@@ -145,12 +196,20 @@ cudaError_t lp_direct_launch(const LpArgs &a, const lp_seg_table *segs, const Lp
     if (grid > 0x7fffffffull) grid = 0x7fffffffull;
     cfg->grid = (uint32_t)grid;
     cfg->threads = kThreads;
-    cfg->smem_bytes = 0;
+    // residency cap: unused dynamic shared memory sized so that `occ` CTAs fill an SM's 228 KB
+    const uint32_t occ = t.v[LP_TUNE_DIRECT_OCC] ? (uint32_t)t.v[LP_TUNE_DIRECT_OCC] : lp_direct_occupancy(a);
+    cfg->smem_bytes = occ >= 8u ? 0u : (228u * 1024u / occ - 1024u) / 1024u * 1024u - (occ == 1u ? 1024u : 0u);
     cfg->stages = 0;
     cfg->out_stages = 0;
     cfg->pdl = t.v[LP_TUNE_NO_PDL] == 0;
+    cfg->claim = 1;
     if (dry_run || grid == 0) return cudaSuccess;
     lp_count_launch(1);
+    {
+        LpRange ranges[2 * LP_MAX_IN];
+        const int nr = lp_args_ranges(a, ranges);
+        a.late_wait = lp_chain_admit(stream, ranges, nr, cfg->pdl, t.v[LP_TUNE_CHAIN] != 2) ? 1 : 0;
+    }
     switch (a.part.tile) {
         case 1024: return launch_seg<1>(a, segs, *cfg, stream);
         case 2048: return launch_seg<2>(a, segs, *cfg, stream);

@@ -4,9 +4,11 @@
 // the last one short (U6).  On one GPU a block is further cut into TILES of `tile` elements (the unit
 // one CTA keeps on chip while it walks the chain rank 0 -> P-1); a tile never straddles a block
 // boundary, so `block` stays the unit the pipeline is built from and small blocks really cost more
-// (the alpha term of PAPER.md:89).  Tiles are numbered block by block, and tile idx is handled by
-// persistent CTA (idx mod grid): at any moment the whole grid works on neighbouring tiles of the same
-// few blocks, the analogue of "the entire network is fully utilized once the pipeline is filled".
+// (the alpha term of PAPER.md:89).  Tiles are numbered block by block and handed to the persistent CTAs in
+// increasing order (lp_common.cuh, LpTileClaimer): at any moment the whole grid works on neighbouring tiles of
+// the same few blocks, the analogue of "the entire network is fully utilized once the pipeline is filled".
+// The pipeline kernels partition into small tiles ("granules") and move RUNS of consecutive granules of one block
+// through their ring slots, so the unit of work can shrink towards the end of the list.
 #pragma once
 #include <stdint.h>
 
@@ -45,8 +47,10 @@ LP_HD lp_partition lp_make_partition(uint64_t n, uint64_t block, uint32_t tile) 
     return p;
 }
 
-// Tile idx -> element range [off, off + len).
-LP_HD void lp_tile_range(const lp_partition &p, uint64_t idx, uint64_t &off, uint32_t &len) {
+// Tile idx -> element range [off, off + len); `left` = tiles from idx to the end of its block (>= 1), so that
+// idx .. idx + left - 1 are contiguous in memory and lie in one block (the last one may be short).
+LP_HD void lp_tile_range_ex(const lp_partition &p, uint64_t idx, uint64_t &off, uint32_t &len, uint64_t &left,
+                            uint64_t &block_end) {
     uint64_t k, j;  // block index, tile within the block
     if (((idx | p.tiles_per_block) >> 32) == 0) {  // the common case: a 32-bit division (64-bit ones are emulated on the GPU)
         const uint32_t k32 = (uint32_t)idx / (uint32_t)p.tiles_per_block;
@@ -62,6 +66,13 @@ LP_HD void lp_tile_range(const lp_partition &p, uint64_t idx, uint64_t &off, uin
     off = bstart + j * (uint64_t)p.tile;
     uint64_t rem = bend - off;
     len = rem < p.tile ? (uint32_t)rem : p.tile;
+    left = (rem + p.tile - 1) / p.tile;  // <= tiles_per_block - j (fewer in the short last block)
+    block_end = bend;
+}
+
+LP_HD void lp_tile_range(const lp_partition &p, uint64_t idx, uint64_t &off, uint32_t &len) {
+    uint64_t left, bend;
+    lp_tile_range_ex(p, idx, off, len, left, bend);
 }
 
 // ---- layer-wise messages (Alg. 1) -----------------------------------------------------
@@ -78,9 +89,10 @@ struct lp_seg_table {
     uint32_t n_seg;
 };
 
-// Tile idx of a segmented launch -> element range [off, off + len) in the rank vectors.
-LP_HD void lp_seg_tile_range(const lp_seg_table &st, uint64_t block, uint32_t tile, uint64_t idx, uint64_t &off,
-                             uint32_t &len) {
+// Tile idx of a segmented launch -> element range [off, off + len) in the rank vectors (+ `left`, `block_end` as in
+// lp_tile_range_ex; a run of tiles never leaves its slice because a slice ends where its last block ends).
+LP_HD void lp_seg_tile_range_ex(const lp_seg_table &st, uint64_t block, uint32_t tile, uint64_t idx, uint64_t &off,
+                                uint32_t &len, uint64_t &left, uint64_t &block_end) {
     uint32_t lo = 0, hi = st.n_seg;  // tile_start[lo] <= idx < tile_start[hi]
     while (hi - lo > 1) {
         const uint32_t mid = (lo + hi) >> 1;
@@ -88,6 +100,13 @@ LP_HD void lp_seg_tile_range(const lp_seg_table &st, uint64_t block, uint32_t ti
         else hi = mid;
     }
     const lp_partition p = lp_make_partition(st.len[lo], block, tile);
-    lp_tile_range(p, idx - st.tile_start[lo], off, len);
+    lp_tile_range_ex(p, idx - st.tile_start[lo], off, len, left, block_end);
     off += st.off[lo];
+    block_end += st.off[lo];
+}
+
+LP_HD void lp_seg_tile_range(const lp_seg_table &st, uint64_t block, uint32_t tile, uint64_t idx, uint64_t &off,
+                             uint32_t &len) {
+    uint64_t left, bend;
+    lp_seg_tile_range_ex(st, block, tile, idx, off, len, left, bend);
 }

@@ -9,15 +9,25 @@ namespace {
 
 struct LpSegArgs {
     LpSegJob j[LP_MAX_JOBS];
+    int red_op;  // LP_REDUCE_*: the operator of dst = a op b
+    int late_wait;  // lp_chain_admit: wait for the launches ahead at the end of the CTA instead of at its start
 };
 
 constexpr int kSegThreads = 256;
 constexpr int kSegUnroll = 4;
 
+__device__ __forceinline__ void lp_seg_body(const LpSegArgs &s);
+
 __global__ void __launch_bounds__(kSegThreads) lp_seg_kernel(const __grid_constant__ LpSegArgs s) {
-    lp_pdl_wait();     // the previous level (or whatever precedes in the stream) has completed
+    if (!s.late_wait) lp_pdl_wait();  // the previous level (or whatever precedes in the stream) has completed
     lp_pdl_trigger();  // one chunk per CTA: once the last CTA is resident the next level's kernel may be scheduled
+    lp_seg_body(s);
+    if (s.late_wait && threadIdx.x == 0) lp_pdl_wait();
+}
+
+__device__ __forceinline__ void lp_seg_body(const LpSegArgs &s) {
     const LpSegJob &job = s.j[blockIdx.y];
+    const bool prod = s.red_op == LP_REDUCE_PROD;
     float *dst = job.dst;
     const float *a = job.a;
     const float *b = job.b;
@@ -30,7 +40,7 @@ __global__ void __launch_bounds__(kSegThreads) lp_seg_kernel(const __grid_consta
         const uint64_t per = (uint64_t)kSegThreads * kSegUnroll * 4;
         const uint64_t lo = (uint64_t)blockIdx.x * per;
         const uint64_t hi = lo + per < len ? lo + per : len;
-        for (uint64_t i = lo + threadIdx.x; i < hi; i += kSegThreads) dst[i] = b ? __fadd_rn(a[i], b[i]) : a[i];
+        for (uint64_t i = lo + threadIdx.x; i < hi; i += kSegThreads) dst[i] = b ? lp_combine1(a[i], b[i], prod) : a[i];
         return;
     }
     uint64_t head = ((16u - mis) & 15u) >> 2;
@@ -39,8 +49,8 @@ __global__ void __launch_bounds__(kSegThreads) lp_seg_kernel(const __grid_consta
     const uint64_t tail0 = head + (nvec << 2);
     if (blockIdx.x == 0) {
         const uint64_t i = threadIdx.x;
-        if (i < head) dst[i] = b ? __fadd_rn(a[i], b[i]) : a[i];
-        if (i < len - tail0) dst[tail0 + i] = b ? __fadd_rn(a[tail0 + i], b[tail0 + i]) : a[tail0 + i];
+        if (i < head) dst[i] = b ? lp_combine1(a[i], b[i], prod) : a[i];
+        if (i < len - tail0) dst[tail0 + i] = b ? lp_combine1(a[tail0 + i], b[tail0 + i], prod) : a[tail0 + i];
     }
     float *d4 = dst + head;
     const float *a4 = a + head;
@@ -58,7 +68,7 @@ __global__ void __launch_bounds__(kSegThreads) lp_seg_kernel(const __grid_consta
 #pragma unroll
     for (int u = 0; u < kSegUnroll; ++u) {
         const uint64_t v = v0 + (uint64_t)u * kSegThreads;
-        if (v < nvec) lp_stg_stream(d4 + 4 * v, b4 ? lp_add4(x[u], y[u]) : x[u]);
+        if (v < nvec) lp_stg_stream(d4 + 4 * v, b4 ? lp_combine4(x[u], y[u], prod) : x[u]);
     }
 }
 
@@ -99,17 +109,20 @@ __global__ void __launch_bounds__(kSegThreads) lp_update_kernel(float *w, const 
 }  // namespace
 
 cudaError_t lp_update_launch(float *w, const float *S, float *velocity, uint64_t n, float lr, float invP, float mu,
-                             cudaStream_t stream) {
+                             cudaStream_t stream, bool pdl) {
     if (n == 0) return cudaSuccess;
     const uint64_t blocks = ((n >> 2) + kSegThreads - 1) / kSegThreads + ((n >> 2) == 0 ? 1 : 0);
     if (blocks > 0x7fffffffull) return cudaErrorInvalidValue;
     lp_count_launch(1);
-    return lp_launch(lp_update_kernel, dim3((unsigned)blocks), dim3(kSegThreads), 0, stream, lp_pdl_enabled(), w, S, velocity,
+    lp_chain_reset(stream);  // waits first, reads and rewrites what its neighbours in the stream touch
+    return lp_launch(lp_update_kernel, dim3((unsigned)blocks), dim3(kSegThreads), 0, stream, pdl, w, S, velocity,
                      (uint64_t)n, lr, invP, mu);
 }
 
-cudaError_t lp_seg_launch(const LpSegJob *jobs, int n_jobs, int sm_count, cudaStream_t stream) {
+cudaError_t lp_seg_launch(const LpSegJob *jobs, int n_jobs, int sm_count, cudaStream_t stream, bool pdl, int red_op,
+                          bool chain) {
     LpSegArgs s;
+    s.red_op = red_op;
     int m = 0;
     uint64_t longest = 0;
     for (int i = 0; i < n_jobs; ++i) {
@@ -126,5 +139,16 @@ cudaError_t lp_seg_launch(const LpSegJob *jobs, int n_jobs, int sm_count, cudaSt
     if (per_job > 0x7fffffffull) return cudaErrorInvalidValue;
     dim3 grid((unsigned)per_job, (unsigned)m, 1);
     lp_count_launch(1);
-    return lp_launch(lp_seg_kernel, grid, dim3(kSegThreads), 0, stream, lp_pdl_enabled(), s);
+    {
+        LpRange ranges[3 * LP_MAX_JOBS];
+        int nr = 0;
+        for (int i = 0; i < m; ++i) {
+            const uintptr_t bytes = (uintptr_t)s.j[i].len * 4u;
+            ranges[nr++] = LpRange{(uintptr_t)s.j[i].dst, (uintptr_t)s.j[i].dst + bytes};
+            ranges[nr++] = LpRange{(uintptr_t)s.j[i].a, (uintptr_t)s.j[i].a + bytes};
+            if (s.j[i].b) ranges[nr++] = LpRange{(uintptr_t)s.j[i].b, (uintptr_t)s.j[i].b + bytes};
+        }
+        s.late_wait = lp_chain_admit(stream, ranges, nr, pdl, chain) ? 1 : 0;
+    }
+    return lp_launch(lp_seg_kernel, grid, dim3(kSegThreads), 0, stream, pdl, s);
 }

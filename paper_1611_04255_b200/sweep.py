@@ -1,8 +1,11 @@
 """Message-size sweep of BASELINE.json configs[3] (the shape of the paper's Fig. 3 / Fig. 4):
-n = 2^10 .. 2^27 fp32 (4 KB .. 512 MB per rank), P in {2, 4, 8, 16}, broadcast / reduce / allreduce, LP vs MST
-(binomial tree) vs BE (recursive halving-doubling) on the same GPU, uniform[-1,1] inputs from seed [3, r].
+n = 2^10 .. 2^27 fp32 (4 KB .. 512 MB per rank), P in {2, 4, 8, 16} (plus the paper's own 3, 5, 6 by default),
+broadcast / reduce / allreduce, LP vs MST (binomial tree) vs BE (recursive halving-doubling) on the same GPU,
+uniform[-1,1] inputs from seed [3, r].
 
-    python -m paper_1611_04255_b200.sweep --out gpurun_out/sweep_cfg3 [--min-exp 10] [--max-exp 27] [--P 2,4,8,16]
+    python -m paper_1611_04255_b200.sweep --out gpurun_out/sweep_cfg3 [--min-exp 10] [--max-exp 27] [--P 2,3,4,5,6,8,16]
+                                          [--ops broadcast,reduce,allreduce] [--algos lp,mst,be] [--variant auto]
+                                          [--tune CHAIN=2,TILE_ELEMS=4096]
 
 Writes <out>.jsonl (one row per cell) and <out>.md (tables).  GB/s is quoted on the ALGORITHM-independent minimum
 bytes of the op (broadcast P*n*4, reduce (P+1)*n*4, allreduce 2*P*n*4) so LP, MST and BE rows compare directly;
@@ -49,16 +52,23 @@ def main(argv=None):
     ap.add_argument("--out", default="gpurun_out/sweep_cfg3")
     ap.add_argument("--min-exp", type=int, default=10)
     ap.add_argument("--max-exp", type=int, default=27)
-    ap.add_argument("--P", default="2,4,8,16")
+    ap.add_argument("--P", default="2,3,4,5,6,8,16")
+    ap.add_argument("--ops", default="broadcast,reduce,allreduce")
+    ap.add_argument("--tune", default="", help="comma list of LP_TUNE key=value (names as in binding.TUNE_*), e.g. CHAIN=2")
     ap.add_argument("--block", type=int, default=65_536)
-    ap.add_argument("--variant", default="auto", choices=["auto", "pipeline", "direct"],
+    ap.add_argument("--variant", default="auto", choices=["auto", "pipeline", "direct", "cluster"],
                     help="LP realisation timed in the LP column (default: the library default)")
     ap.add_argument("--algos", default="lp,mst,be")
     args = ap.parse_args(argv)
     assert torch.cuda.is_available(), "the sweep needs a CUDA device"
     dev = torch.device("cuda", 0)
     lp.lib()
-    lp.lp_set_variant({"auto": lp.VARIANT_AUTO, "pipeline": lp.VARIANT_PIPELINE, "direct": lp.VARIANT_DIRECT}[args.variant])
+    lp.lp_set_variant({"auto": lp.VARIANT_AUTO, "pipeline": lp.VARIANT_PIPELINE, "direct": lp.VARIANT_DIRECT,
+                       "cluster": lp.VARIANT_CLUSTER}[args.variant])
+    for kv in filter(None, args.tune.split(",")):
+        k, v = kv.split("=")
+        lp.lp_set_tuning(getattr(lp, "TUNE_" + k.strip().upper()), int(v))
+    ops = tuple(o for o in OPS if o in args.ops.split(","))
     algos = tuple(a for a in ALGOS if a in args.algos.split(","))
     peak = 6553.3
     try:
@@ -76,7 +86,7 @@ def main(argv=None):
             n = 1 << e
             n_sets = int(max(1, min(n_max // n, 64, -(-8 * L2_BYTES // (P * n * 4)))))
             sets = [[w[s * n:(s + 1) * n] for w in work] for s in range(n_sets)]
-            for op in OPS:
+            for op in ops:
                 mb = lp.lp_min_bytes(OP_ID[op], P, n)
                 est = max(mb / 3e12, 4e-6)  # seconds per call, rough
                 K = int(min(max(2e-3 / est, 3), 20 * n_sets, 400))
@@ -129,7 +139,8 @@ def write_markdown(rows, path, peak, Ps, args):
     with open(path, "w") as f:
         f.write("# Message-size sweep (BASELINE.json configs[3]) — LP vs MST vs BE on one B200\n\n")
         f.write(f"Command: `python -m paper_1611_04255_b200.sweep --out {args.out} --min-exp {args.min_exp} "
-                f"--max-exp {args.max_exp} --P {args.P} --block {args.block} --variant {args.variant} --algos {args.algos}`\n\n")
+                f"--max-exp {args.max_exp} --P {args.P} --block {args.block} --variant {args.variant} --algos {args.algos} "
+                f"--ops {args.ops}" + (f" --tune {args.tune}" if args.tune else "") + "`\n\n")
         f.write(f"Cells: GB/s on the op's minimum HBM bytes (fraction of the measured copy peak {peak} GB/s); "
                 "LP block 65,536 elements; uniform[-1,1], seed [3, r]. North-star bar: LP >= 80 % of 8 TB/s = 6400 GB/s "
                 "for messages >= 64 MB, and LP faster than MST and BE.\n")

@@ -1,7 +1,7 @@
 """GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times (default variant and
-tuning).  configs[1] (P=6, 61 M floats) is compared in full; configs[4] (P=16, 138 M floats, 8.8 GB) on sampled
-slices -- the path is element-wise, so the oracle evaluated on a slice is exact for that slice -- plus the
-properties that hold at any size (all ranks bit-identical)."""
+tuning), element for element and unsampled: configs[1] (P=6, 61 M floats), configs[4] (P=16, 138 M floats, 8.8 GB:
+rank 0 against the oracle's chain sum over all 138 M elements, every other rank against rank 0 on the device) and
+the configs[3] sweep cells the headline numbers come from (2^24 .. 2^27 floats = 64 .. 512 MB per rank)."""
 import numpy as np
 import pytest
 
@@ -48,34 +48,65 @@ def test_config1_alexnet_allreduce_full_compare(oracle):
     assert all(torch.equal(dev[r], dev[4]) for r in range(P))
 
 
-def test_config4_vgg16_allreduce_sampled(oracle):
+def _full_compare(oracle, src, block, ops=("allreduce", "reduce", "broadcast"), root=None):
+    """LP collectives on device copies of `src` against the oracle on ALL n elements: rank 0 (the root) byte for
+    byte on the host, the other ranks against it on the device (torch.equal), non-root buffers of reduce against
+    the inputs."""
+    P = len(src)
+    root = P - 1 if root is None else root
+    want = oracle.chain_sum(src)
+    pristine = [torch.from_numpy(s_).cuda() for s_ in src]
+    dev = [p.clone() for p in pristine]
+    if "allreduce" in ops:
+        lp.lp_allreduce(dev, block)
+        torch.cuda.synchronize()
+        assert dev[0].cpu().numpy().tobytes() == want.tobytes(), "allreduce rank 0"
+        for r in range(1, P):  # PAPER.md:71: the reduced block is forwarded, every rank holds the same bits
+            assert torch.equal(dev[r], dev[0]), ("allreduce", r)
+    if "reduce" in ops:
+        for d, p in zip(dev, pristine):
+            d.copy_(p)
+        lp.lp_reduce(dev, block, root=root)
+        torch.cuda.synchronize()
+        assert dev[root].cpu().numpy().tobytes() == want.tobytes(), "reduce root"
+        for r in range(P):
+            if r != root:
+                assert torch.equal(dev[r], pristine[r]), ("reduce left rank", r)   # U5
+    if "broadcast" in ops:
+        for d, p in zip(dev, pristine):
+            d.copy_(p)
+        lp.lp_broadcast(dev, block, root=root)
+        torch.cuda.synchronize()
+        assert dev[root].cpu().numpy().tobytes() == src[root].tobytes(), "broadcast root"
+        for r in range(P):
+            assert torch.equal(dev[r], dev[root]), ("broadcast", r)
+    del dev, pristine
+    torch.cuda.empty_cache()
+
+
+def test_config4_vgg16_full_compare(oracle):
+    # BASELINE.json configs[4], the largest single-GPU config: P=16, n=138,000,000 (8.83 GB), b=262,144 (527 blocks,
+    # ragged tail of 112,256).  Host: 8.8 GB of inputs + 0.55 GB of oracle output.
     c = inputs.CONFIGS[4]
     P, n, block = c["P"], c["n"], c["block"]
-    # sampled slices: message head, a block boundary, a window in the middle, the ragged tail of the last block
-    last_block = (n // block) * block
-    windows = [(0, 200_000), (block - 4100, block + 4100), (n // 2 - 50_000, n // 2 + 50_000),
-               (last_block - 5000, n)]
-    dev, slices = [], []
-    for r in range(P):
-        x = inputs.normal(4, r, n, c["sigma"])
-        slices.append([x[a:b].copy() for a, b in windows])
-        dev.append(torch.from_numpy(x).cuda())
-        del x
-    lp.lp_allreduce(dev, block)
-    torch.cuda.synchronize()
-    for w, (a, b) in enumerate(windows):
-        want = oracle.chain_sum([slices[r][w] for r in range(P)])
-        for r in (0, 7, 15):
-            assert dev[r][a:b].cpu().numpy().tobytes() == want.tobytes(), (w, r)
-    for r in range(1, P):   # every rank holds the same bits (the reduced block is forwarded)
-        assert torch.equal(dev[r], dev[0]), r
+    src = [inputs.normal(4, r, n, c["sigma"]) for r in range(P)]
+    _full_compare(oracle, src, block, root=5)
+
+
+@pytest.mark.parametrize("P,e", [(4, 27), (3, 26), (2, 26), (8, 25), (16, 25)])
+def test_config3_large_cells_full_compare(oracle, P, e):
+    # the 128 .. 512 MB cells of the sweep (P=4 at 512 MB; 3 ranks -- a Fig. 4 point -- and 2 at 256 MB; 8 and 16 at
+    # 128 MB), all three collectives, every element
+    n = 1 << e
+    src = [inputs.uniform(3, r, n) for r in range(P)]
+    _full_compare(oracle, src, 65_536)
 
 
 @pytest.mark.parametrize("P", [2, 4, 8, 16])
 def test_config3_sweep_cells(oracle, P):
     # BASELINE.json configs[3]: uniform[-1,1] from seed [3, r], n = 2^10 .. 2^27, LP vs MST vs BE.  Cells up to 2^20
-    # are compared in full for every op and algorithm; 2^24 (the 64 MB message of the bar: AUTO takes the pipeline
-    # there, the register kernel below) on sampled windows, the path being element-wise.
+    # are compared in full for every op and algorithm, 2^24 in full for the LP collectives; 2^25 .. 2^27 in
+    # test_config3_large_cells_full_compare.
     for e in (10, 13, 16, 20):
         n = 1 << e
         src = [inputs.uniform(3, r, n) for r in range(P)]
@@ -106,15 +137,7 @@ def test_config3_sweep_cells(oracle, P):
                 torch.cuda.synchronize()
                 for r in range(P):
                     assert dev[r].cpu().numpy().tobytes() == want[r].tobytes(), (e, name, op, r)
+    # 2^24 (the 64 MB message of the bar; AUTO takes the pipeline there, the register kernel below): every element
     n = 1 << 24
-    windows = [(0, 70_000), (65_536 - 3000, 65_536 + 3000), (n // 2, n // 2 + 100_000), (n - 50_000, n)]
     src = [inputs.uniform(3, r, n) for r in range(P)]
-    dev = [torch.from_numpy(s).cuda() for s in src]
-    lp.lp_allreduce(dev, 65_536)
-    torch.cuda.synchronize()
-    for a, b in windows:
-        want = oracle.chain_sum([s[a:b].copy() for s in src])
-        for r in (0, P - 1):
-            assert dev[r][a:b].cpu().numpy().tobytes() == want.tobytes(), (a, r)
-    for r in range(1, P):
-        assert torch.equal(dev[r], dev[0]), r
+    _full_compare(oracle, src, 65_536)

@@ -44,6 +44,13 @@ def copies(arrs):
     return [a.copy() for a in arrs]
 
 
+def same_but_nan_payload(a, b):
+    """Bit-exact except that a NaN may carry any payload (IEEE-754 leaves it open; x86 keeps an operand's, the GPU
+    returns the canonical quiet NaN): NaNs in the same places, every other element the same bytes."""
+    na, nb = np.isnan(a), np.isnan(b)
+    return a.shape == b.shape and np.array_equal(na, nb) and a[~na].tobytes() == b[~nb].tobytes()
+
+
 def run_lp(op, dev, block, root=0, stream=None):
     if op == "allreduce":
         lp.lp_allreduce(dev, block, stream=stream)
@@ -533,13 +540,410 @@ def test_cluster_variant_limits():
     with pytest.raises(lp.LpError) as e:
         lp.lp_allreduce(dev, 1024)                           # P > 16: no cluster that large
     assert e.value.status == lp.LP_ERR_UNSUPPORTED
-    with pytest.raises(lp.LpError) as e:
-        lp.lp_allreduce_segments(dev[:4], [(0, 100)], 1024)  # layer-wise launches are a pipeline / direct feature
-    assert e.value.status == lp.LP_ERR_UNSUPPORTED
-    vel = torch.zeros(4096, device="cuda")
-    with pytest.raises(lp.LpError) as e:
-        lp.lp_bsp_sgd_momentum_step(dev[:4], dev[4:8], vel, 1024)
-    assert e.value.status == lp.LP_ERR_UNSUPPORTED
+
+
+@pytest.mark.parametrize("tile,stages,out_stages", [(0, 0, 0), (1024, 0, 0), (4096, 0, 0), (2048, 3, 2), (2048, 8, 6), (4096, 5, 4)])
+def test_cluster_variant_tiles_rings_momentum_slices(oracle, tile, stages, out_stages):
+    # tile size and ring depths of the stage-per-rank kernel are launch parameters; momentum and slice lists run in
+    # it too (one launch per slice)
+    lp.lp_set_variant(lp.VARIANT_CLUSTER)
+    lp.lp_set_tuning(lp.TUNE_CLUSTER_TILE, tile)
+    lp.lp_set_tuning(lp.TUNE_STAGES, stages)
+    lp.lp_set_tuning(lp.TUNE_OUT_STAGES, out_stages)
+    P, n, block = 6, 700_003, 65_536
+    src = inputs.rank_vectors([16, n], P, n, "uniform")
+    chain = oracle.chain_sum(src)
+    dev = up(src)
+    lp.lp_allreduce(dev, block)
+    assert all(same(g, chain) for g in down(dev))
+    dev = up(src)
+    lp.lp_broadcast(dev, block, root=4)
+    assert all(same(g, src[4]) for g in down(dev))
+    # momentum (U18): 3 iterations, weights and velocity bit-exact
+    grads, weights = inputs.sgd_inputs([17, n], P, n)
+    hw, hv = copies(weights), np.zeros(n, np.float32)
+    dg, dw, dv = up(grads), up(weights), torch.zeros(n, device="cuda")
+    for it in range(3):
+        oracle.bsp_sgd_momentum_step(grads, hw, hv, root=2, lr=0.01, mu=0.9)
+        lp.lp_bsp_sgd_momentum_step(dg, dw, dv, block, root=2, lr=0.01, mu=0.9)
+        assert all(same(a, b) for a, b in zip(down(dw), hw)), ("momentum w", it)
+        assert same(down([dv])[0], hv), ("momentum v", it)
+    # slices that start off the 16-byte grid
+    segs = [(5, 1000), (70_001, 123_457), (200_000, 3), (300_002, 250_001)]
+    for op, opid in (("broadcast", 0), ("reduce", 1), ("allreduce", 2)):
+        want = copies(src)
+        oracle.collective_segments(opid, want, segs, root=1)
+        dev = up(src)
+        if op == "allreduce":
+            lp.lp_allreduce_segments(dev, segs, block)
+        elif op == "reduce":
+            lp.lp_reduce_segments(dev, segs, block, root=1)
+        else:
+            lp.lp_broadcast_segments(dev, segs, block, root=1)
+        assert all(same(a, b) for a, b in zip(down(dev), want)), op
+
+
+# ---------------------------------------------------------------------------------------------------
+# reduce operator ("summations and multiplications"): every LP variant and the MST / BE trees
+# ---------------------------------------------------------------------------------------------------
+OP_SHAPES = [(1, 1000, 256), (2, 4099, 1024), (3, 70_001, 1001), (4, 1 << 20, 65_536), (6, 300_007, 16_384), (8, 100_001, 4096),
+             (16, 250_003, 65_536), (5, 3, 64)]
+
+
+def product_inputs(seed, P, n):
+    # factors around 1 (|x| in [0.5, 1.5), random sign): 16 of them stay far from overflow / underflow
+    out = []
+    for r in range(P):
+        rng = np.random.default_rng([seed, r])
+        out.append((rng.random(n, dtype=np.float32) + np.float32(0.5)) * rng.choice(np.array([-1, 1], np.float32), n))
+    return out
+
+
+@pytest.mark.parametrize("variant", VARIANTS + [lp.VARIANT_CLUSTER])
+@pytest.mark.parametrize("P,n,block", OP_SHAPES)
+def test_product_bit_exact(oracle, variant, P, n, block):
+    if variant == lp.VARIANT_COPY_ENGINE and (n // block) * P > 400:
+        pytest.skip("copy-engine variant: thousands of tiny operations")
+    lp.lp_set_variant(variant)
+    src = product_inputs([18, n], P, n)
+    fold = oracle.chain_fold(src, oracle.RED_PROD)
+    dev = up(src)
+    lp.lp_allreduce_op(dev, block, lp.REDUCE_PROD)
+    assert all(same(g, fold) for g in down(dev)), "allreduce prod"
+    for root in sorted({0, P - 1}):
+        dev = up(src)
+        lp.lp_reduce_op(dev, block, lp.REDUCE_PROD, root=root)
+        got = down(dev)
+        for r in range(P):
+            assert same(got[r], fold if r == root else src[r]), ("reduce prod", root, r)
+    dev = up(src)   # red = sum through the operator entry point is lp_allreduce
+    lp.lp_allreduce_op(dev, block, lp.REDUCE_SUM)
+    assert all(same(g, oracle.chain_sum(src)) for g in down(dev))
+
+
+def test_product_overflow_order_and_specials(oracle):
+    # (1e30 * 1e30) * 1e-30 = inf in chain order, ~1e30 in any other; NaN / inf / denormal factors as the oracle's
+    P, n = 4, 5000
+    src = [np.full(n, v, np.float32) for v in (1e30, 1e30, 1e-30, 1e-30)]
+    src[0][::7] = np.float32("nan")
+    src[1][1::7] = np.float32("-inf")
+    src[2][2::7] = np.float32(1e-42)
+    src[3][3::7] = 0.0
+    for variant in (lp.VARIANT_PIPELINE, lp.VARIANT_DIRECT, lp.VARIANT_CLUSTER):
+        lp.lp_set_variant(variant)
+        want = oracle.chain_fold(src, oracle.RED_PROD)
+        dev = up(src)
+        lp.lp_allreduce_op(dev, 1024, lp.REDUCE_PROD)
+        for g in down(dev):
+            assert same_but_nan_payload(g, want), variant
+    assert np.isinf(want[4]) and np.isnan(want[0])
+    for algo, fn in ((MST, lp.lp_mst_allreduce_op), (BE, lp.lp_be_allreduce_op)):
+        h = copies(src)
+        oracle.allreduce_op(h, oracle.RED_PROD, algo=algo)
+        dev = up(src)
+        fn(dev, lp.REDUCE_PROD)
+        assert all(same_but_nan_payload(a, b) for a, b in zip(down(dev), h)), algo
+
+
+@pytest.mark.parametrize("P,n", [(2, 1001), (3, 70_001), (4, 65_536), (5, 4099), (6, 300_003), (8, 100_001), (16, 50_001)])
+def test_mst_be_product_against_same_tree_oracle(oracle, P, n):
+    src = product_inputs([19, n], P, n)
+    for algo, red_fn, all_fn in ((MST, lp.lp_mst_reduce_op, lp.lp_mst_allreduce_op), (BE, lp.lp_be_reduce_op, lp.lp_be_allreduce_op)):
+        if algo == BE and P & (P - 1):
+            continue
+        h = copies(src)
+        oracle.allreduce_op(h, oracle.RED_PROD, algo=algo)
+        dev = up(src)
+        all_fn(dev, lp.REDUCE_PROD)
+        assert all(same(a, b) for a, b in zip(down(dev), h)), ("allreduce", algo)
+        root = P - 1
+        h = copies(src)
+        oracle.reduce_op(h, oracle.RED_PROD, root=root, algo=algo)
+        dev = up(src)
+        red_fn(dev, lp.REDUCE_PROD, root=root)
+        assert all(same(a, b) for a, b in zip(down(dev), h)), ("reduce", algo)
+
+
+def test_product_segments_through_a_plan(oracle):
+    P, n, block = 4, 300_007, 16_384
+    src = product_inputs([20, n], P, n)
+    segs = [(5, 1000), (70_001, 123_457), (200_000, 3)]
+    for variant in (lp.VARIANT_PIPELINE, lp.VARIANT_DIRECT, lp.VARIANT_CLUSTER):
+        for op, opid in ((lp.OP_REDUCE, 1), (lp.OP_ALLREDUCE, 2)):
+            want = copies(src)
+            oracle.collective_segments_op(opid, oracle.RED_PROD, want, segs, root=3)
+            dev = up(src)
+            plan = lp.Plan(op, P, n, block=block, root=3, reduce_op=lp.REDUCE_PROD, variant=variant)
+            plan.run_segments(dev, segs)
+            assert all(same(a, b) for a, b in zip(down(dev), want)), (variant, op)
+            plan.close()
+
+
+# ---------------------------------------------------------------------------------------------------
+# plans: per-call settings; two threads / streams with different settings at once
+# ---------------------------------------------------------------------------------------------------
+def test_plans_bit_exact_every_op(oracle):
+    P, n, block = 6, 500_003, 65_536
+    src = inputs.rank_vectors([21, n], P, n, "uniform")
+    chain = oracle.chain_sum(src)
+    for variant in (lp.VARIANT_AUTO, lp.VARIANT_PIPELINE, lp.VARIANT_DIRECT, lp.VARIANT_CLUSTER):
+        for tuning in ({}, {lp.TUNE_GRID_LIMIT: 24}, {lp.TUNE_GRANULE_DIV: 8, lp.TUNE_CLAIM_SLOTS: 1}):
+            dev = up(src)
+            lp.Plan(lp.OP_ALLREDUCE, P, n, block=block, variant=variant, tuning=tuning).run(dev)
+            assert all(same(g, chain) for g in down(dev)), (variant, tuning)
+            dev = up(src)
+            lp.Plan(lp.OP_REDUCE, P, n, root=4, variant=variant, tuning=tuning).run(dev)     # block 0: library chooses
+            got = down(dev)
+            assert all(same(got[r], chain if r == 4 else src[r]) for r in range(P))
+            dev = up(src)
+            lp.Plan(lp.OP_BROADCAST, P, n, block=block, root=5, variant=variant, tuning=tuning).run(dev)
+            assert all(same(g, src[5]) for g in down(dev))
+    grads, weights = inputs.sgd_inputs([22, n], P, n)
+    hw, hv = copies(weights), np.zeros(n, np.float32)
+    oracle.bsp_sgd_momentum_step(grads, hw, hv, root=1, lr=0.02, mu=0.8)
+    dg, dw, dv = up(grads), up(weights), torch.zeros(n, device="cuda")
+    lp.Plan(lp.OP_BSP_SGD_MOM, P, n, block=block, root=1).run(dg, weights=dw, velocity=dv, lr=0.02, mu=0.8)
+    assert all(same(a, b) for a, b in zip(down(dw), hw)) and same(down([dv])[0], hv)
+    hw = copies(weights)
+    oracle.bsp_sgd_step(grads, hw, root=1, lr=0.02)
+    dw = up(weights)
+    lp.Plan(lp.OP_BSP_SGD, P, n, block=block, root=1, tuning={lp.TUNE_GRID_LIMIT: 64}).run(dg, weights=dw, lr=0.02)
+    assert all(same(a, b) for a, b in zip(down(dw), hw))
+    # the process-wide defaults were never touched
+    assert lp.lp_get_variant() == lp.VARIANT_AUTO and all(lp.lp_get_tuning(k) == 0 for k in range(lp.TUNE_COUNT))
+
+
+def test_two_threads_two_streams_different_grid_limits(oracle):
+    # a confined comm-stream collective must not confine anyone else.  Two host threads, two
+    # streams, two plans (64 CTAs / unconfined), 40 launches each, running concurrently; both bit-exact every time.
+    import threading
+    P, n, block = 6, 4_000_003, 65_536
+    src_a = inputs.rank_vectors([23, 0], P, n, "uniform")
+    src_b = inputs.rank_vectors([23, 1], P, n, "uniform")
+    want_a, want_b = oracle.chain_sum(src_a), oracle.chain_sum(src_b)
+    plan_a = lp.Plan(lp.OP_ALLREDUCE, P, n, block=block, variant=lp.VARIANT_PIPELINE, tuning={lp.TUNE_GRID_LIMIT: 64})
+    plan_b = lp.Plan(lp.OP_ALLREDUCE, P, n, block=block, variant=lp.VARIANT_PIPELINE)
+    assert plan_a.info()["grid"] == 64 and plan_b.info()["grid"] > 64
+    pa, pb = up(src_a), up(src_b)
+    bad = []
+
+    def worker(plan, pristine, want, tag):
+        try:
+            torch.cuda.set_device(0)
+            st = torch.cuda.Stream()
+            with torch.cuda.stream(st):
+                for it in range(40):
+                    dev = [p.clone() for p in pristine]
+                    plan.run(dev, stream=st)
+                    st.synchronize()
+                    for r, d in enumerate(dev):
+                        if not same(d.cpu().numpy(), want):
+                            bad.append((tag, it, r))
+        except Exception as ex:  # noqa: BLE001
+            bad.append((tag, repr(ex)))
+
+    ts = [threading.Thread(target=worker, args=(plan_a, pa, want_a, "a")),
+          threading.Thread(target=worker, args=(plan_b, pb, want_b, "b"))]
+    for t in ts:
+        t.start()
+    for t in ts:
+        t.join()
+    assert not bad, bad[:5]
+
+
+def test_many_launches_in_flight_on_many_streams(oracle):
+    # tile-claim counters belong to the stream (the old ring of 1024 pairs was shared by launch k
+    # and launch k + 1024): 2100 pipeline launches spread over 3 streams without a host sync in between, then 40
+    # captured in one CUDA graph replayed twice beside eager launches on another stream
+    P, n, block = 4, 600_003, 65_536
+    lp.lp_set_variant(lp.VARIANT_PIPELINE)
+    src = inputs.rank_vectors([24, n], P, n, "uniform")
+    streams = [torch.cuda.Stream() for _ in range(3)]
+    pristine = up(src)
+    work = [[p.clone() for p in pristine] for _ in streams]
+    torch.cuda.synchronize()
+    for it in range(700):
+        for st, w in zip(streams, work):
+            lp.lp_broadcast(w, block, root=it % P, stream=st)    # idempotent after the first: every rank = src[0]
+    torch.cuda.synchronize()
+    for w in work:
+        assert all(same(g, src[0]) for g in down(w))
+    chain = oracle.chain_sum(src)
+    gsets = [[p.clone() for p in pristine] for _ in range(40)]
+    side = [p.clone() for p in pristine]
+    lp.lp_allreduce(gsets[0], block)
+    torch.cuda.synchronize()
+    for d, p_ in zip(gsets[0], pristine):
+        d.copy_(p_)
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        for d in gsets:
+            lp.lp_allreduce(d, block)
+    for rep in range(2):
+        for d in gsets:
+            for x, p_ in zip(d, pristine):
+                x.copy_(p_)
+        torch.cuda.synchronize()
+        g.replay()
+        for it in range(20):
+            for x, p_ in zip(side, pristine):
+                x.copy_(p_, non_blocking=True)
+            lp.lp_allreduce(side, block, stream=streams[0])
+        torch.cuda.synchronize()
+        for d in gsets:
+            assert all(same(x, chain) for x in down(d)), rep
+        assert all(same(x, chain) for x in down(side))
+
+
+def test_stream_chaining_keeps_stream_order(oracle):
+    # LP_TUNE_CHAIN (default on): a call that touches none of the buffers of the calls still in flight ahead of it starts
+    # without waiting for them.  Everything that DOES depend on an earlier call -- same buffers, a sub-range of them,
+    # a foreign kernel in between -- must still see stream order.  No host sync inside a sequence; 30 repetitions.
+    P, n, block = 4, 1_500_012, 65_536    # a multiple of 4 (the views below must start 16-byte aligned), not of a tile
+    rng = np.random.default_rng(27)
+    base = [rng.integers(-3, 4, 3 * n).astype(np.float32) for _ in range(P)]   # small integers: sums stay exact, no overflow
+    for variant in (lp.VARIANT_PIPELINE, lp.VARIANT_DIRECT, lp.VARIANT_AUTO):
+        lp.lp_set_variant(variant)
+        for rep in range(10):
+            big = up(base)                                    # each rank: one tensor of 3n, used through views
+            A = [b[0:n] for b in big]
+            B = [b[n:2 * n] for b in big]
+            C = [b[2 * n:3 * n] for b in big]
+            off = (n // 2) & ~3                               # a 16-byte aligned start
+            AB = [b[off:off + n] for b in big]                # straddles A and B
+            h = copies(base)
+            hA, hB, hC = [x[0:n] for x in h], [x[n:2 * n] for x in h], [x[2 * n:3 * n] for x in h]
+            hAB = [x[off:off + n] for x in h]
+            lp.lp_allreduce(A, block)          # 1
+            lp.lp_allreduce(B, block)          # 2: disjoint from 1 -> may start early
+            lp.lp_broadcast(C, block, root=1)  # 3: disjoint from 1, 2
+            lp.lp_reduce(A, block, root=2)     # 4: depends on 1
+            big[0].mul_(2.0)                   # a foreign kernel on the stream, touching everything of rank 0
+            lp.lp_allreduce(AB, block)         # 5: depends on 1, 2, 4 and on the foreign kernel
+            lp.lp_broadcast(B, block, root=0)  # 6: depends on 2, 5
+            lp.lp_allreduce(C, block)          # 7: depends on 3
+            lp.lp_mst_allreduce(A)             # 8: the baselines are chained too
+            lp.lp_be_allreduce(C)              # 9
+            for fn, args in ((oracle.allreduce, (hA,)), (oracle.allreduce, (hB,))):
+                fn(*args)
+            oracle.broadcast(hC, root=1)
+            oracle.reduce(hA, root=2)
+            h[0] *= np.float32(2.0)
+            oracle.allreduce(hAB)
+            oracle.broadcast(hB, root=0)
+            oracle.allreduce(hC)
+            oracle.allreduce(hA, algo=MST)
+            oracle.allreduce(hC, algo=BE)
+            got = down(big)
+            for r in range(P):
+                assert same(got[r], h[r]), (variant, rep, r, int(np.count_nonzero(got[r] != h[r])))
+    # the same with chaining off gives the same bits
+    lp.lp_set_tuning(lp.TUNE_CHAIN, 2)
+    lp.lp_set_variant(lp.VARIANT_PIPELINE)
+    big = up(base)
+    A, B = [b[0:n] for b in big], [b[n:2 * n] for b in big]
+    lp.lp_allreduce(A, block)
+    lp.lp_allreduce(B, block)
+    lp.lp_reduce(A, block, root=2)
+    h = copies(base)
+    hA, hB = [x[0:n] for x in h], [x[n:2 * n] for x in h]
+    oracle.allreduce(hA)
+    oracle.allreduce(hB)
+    oracle.reduce(hA, root=2)
+    assert all(same(g, w) for g, w in zip(down(big), h))
+
+
+def test_stream_chaining_long_runs_and_graphs(oracle):
+    # many independent calls back to back (rotating buffer sets, as bench.py times them), eagerly and as a CUDA graph:
+    # every set must hold the chain sum; then a dependent tail (an SGD loop on ONE set, which may never be chained)
+    P, n, block = 6, 800_003, 65_536
+    src = inputs.rank_vectors([28, n], P, n, "uniform")
+    chain = oracle.chain_sum(src)
+    pristine = up(src)
+    n_sets = 12
+    for variant in (lp.VARIANT_PIPELINE, lp.VARIANT_DIRECT):
+        lp.lp_set_variant(variant)
+        sets = [lp.Ranks([p.clone() for p in pristine]) for _ in range(n_sets)]
+        torch.cuda.synchronize()
+        for s_ in sets:
+            lp.lp_allreduce(s_, block)
+        torch.cuda.synchronize()
+        for k, s_ in enumerate(sets):
+            assert all(same(g, chain) for g in down(s_.bufs)), (variant, "eager", k)
+        for s_ in sets:
+            for d, p in zip(s_.bufs, pristine):
+                d.copy_(p)
+        lp.lp_allreduce(sets[0], block)
+        torch.cuda.synchronize()
+        for d, p in zip(sets[0].bufs, pristine):
+            d.copy_(p)
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            for s_ in sets:
+                lp.lp_reduce(s_, block, root=3)
+            for s_ in sets:
+                lp.lp_broadcast(s_, block, root=3)
+        for rep in range(3):
+            for s_ in sets:
+                for d, p in zip(s_.bufs, pristine):
+                    d.copy_(p)
+            torch.cuda.synchronize()
+            g.replay()
+            torch.cuda.synchronize()
+            for k, s_ in enumerate(sets):
+                assert all(same(x, chain) for x in down(s_.bufs)), (variant, "graph", rep, k)
+        del g
+    grads, weights = inputs.sgd_inputs([29, n], P, n)
+    hw = copies(weights)
+    dg, dw = up(grads), up(weights)
+    for it in range(25):   # step k + 1 reads the weights step k wrote: never chained
+        lp.lp_bsp_sgd_step(dg, dw, block, root=it % P, lr=0.01)
+    for it in range(25):
+        oracle.bsp_sgd_step(grads, hw, root=it % P, lr=0.01)
+    assert all(same(a, b) for a, b in zip(down(dw), hw))
+
+
+def test_shutdown_and_rebind(oracle):
+    # function attributes are per device; lp_shutdown() unbinds the library, and the launchers
+    # must set them again afterwards (the pipeline's 49 KB and the cluster kernel's ring need the opt-in limit)
+    P, n, block = 4, 300_003, 65_536
+    src = inputs.rank_vectors([25, n], P, n, "uniform")
+    chain = oracle.chain_sum(src)
+    for rounds in range(2):
+        for variant in (lp.VARIANT_PIPELINE, lp.VARIANT_CLUSTER, lp.VARIANT_DIRECT):
+            lp.lp_set_variant(variant)
+            dev = up(src)
+            lp.lp_allreduce(dev, block)
+            assert all(same(g, chain) for g in down(dev)), (rounds, variant)
+            dev = up(src)
+            lp.lp_broadcast(dev, block, root=1)
+            assert all(same(g, src[1]) for g in down(dev))
+        h = [torch.from_numpy(s.copy()).pin_memory() for s in src]
+        lp.lp_allreduce_host(h, block)
+        assert all(same(x.numpy(), chain) for x in h)
+        torch.cuda.synchronize()
+        lp.lp_shutdown()
+
+
+def test_guided_claims_cover_every_element_once(oracle):
+    # the shrinking claims (LpTileClaimer): every granule exactly once for any granule / claim size, odd block sizes
+    # (runs that end at block boundaries), and a message short for the grid
+    lp.lp_set_variant(lp.VARIANT_PIPELINE)
+    for P, n, block in ((3, 5_000_011, 65_536), (2, 3_000_001, 1001), (5, 40_003, 4099), (4, 2_500_000, 300_000)):
+        src = inputs.rank_vectors([26, n], P, n, "uniform")
+        chain = oracle.chain_sum(src)
+        for div, claim, tile in ((0, 0, 0), (1, 1, 0), (8, 16, 0), (2, 3, 4096), (4, 2, 1024), (8, 8, 8192)):
+            lp.lp_set_tuning(lp.TUNE_GRANULE_DIV, div)
+            lp.lp_set_tuning(lp.TUNE_CLAIM_SLOTS, claim)
+            lp.lp_set_tuning(lp.TUNE_TILE_ELEMS, tile)
+            for sched in (0, 1):
+                lp.lp_set_tuning(lp.TUNE_SCHED, sched)
+                dev = up(src)
+                lp.lp_allreduce(dev, block)
+                assert all(same(g, chain) for g in down(dev)), (P, n, block, div, claim, tile, sched)
+                dev = up(src)
+                lp.lp_broadcast(dev, block, root=P - 1)
+                assert all(same(g, src[P - 1]) for g in down(dev)), (P, n, block, div, claim, tile, sched)
 
 
 # ---------------------------------------------------------------------------------------------------

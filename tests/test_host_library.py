@@ -105,13 +105,18 @@ def test_plan_partition_covers_message_exactly(variant, P, n, block):
     finally:
         lp.lp_set_variant(lp.VARIANT_AUTO)
     nb = -(-n // block)
-    assert info["nb"] == nb
-    tile = info["tile_elems"]
+    assert info["nb"] == nb and info["block"] == min(block, n)
+    # the pipeline variant counts GRANULES (the unit of a claim; a ring slot holds a run of tile / granule of them)
+    tile = info["granule_elems"]
+    assert info["tile_elems"] % tile == 0 and info["tile_elems"] // tile in (1, 2, 4, 8)
+    if variant == lp.VARIANT_DIRECT:
+        assert tile == info["tile_elems"]
     blk = min(block, n)
     tpb = -(-blk // tile)
     last = n - (nb - 1) * blk
     assert info["n_tiles"] == (nb - 1) * tpb + -(-last // tile)
     assert 1 <= info["grid"] <= info["n_tiles"]
+    assert 1 <= info["claim_granules"] and info["grid"] * info["claim_granules"] < info["n_tiles"] + info["claim_granules"]
     if variant == lp.VARIANT_PIPELINE:
         assert info["grid"] <= info["sm_count"] * 8     # persistent CTAs
     else:
@@ -134,7 +139,13 @@ def test_argument_validation_needs_no_device():
     null_stream = ctypes.c_void_p(0)
     assert L.lp_allreduce(ptrs, 0, n, 16, null_stream) == lp.LP_ERR_INVALID_ARG          # P < 1
     assert L.lp_allreduce(ptrs, 33, n, 16, null_stream) == lp.LP_ERR_INVALID_ARG         # P > LP_MAX_P
-    assert L.lp_allreduce(ptrs, 4, n, 0, null_stream) == lp.LP_ERR_INVALID_ARG           # block == 0
+    # block == 0 is valid since 0.2.0 ("library chooses"): with good arguments and no device the call gets as far as
+    # the device check (test_compute_entry_fails_loudly_without_device); with bad ones it is still refused first
+    assert L.lp_allreduce(ptrs, 0, n, 0, null_stream) == lp.LP_ERR_INVALID_ARG
+    assert L.lp_reduce_op(ptrs, 4, n, 16, 0, 2, null_stream) == lp.LP_ERR_INVALID_ARG    # unknown reduce operator
+    assert L.lp_allreduce_op(ptrs, 4, n, 16, -1, null_stream) == lp.LP_ERR_INVALID_ARG
+    assert L.lp_mst_allreduce_op(ptrs, 4, n, 7, null_stream) == lp.LP_ERR_INVALID_ARG
+    assert L.lp_be_reduce_op(ptrs, 3, n, 0, 1, null_stream) == lp.LP_ERR_UNSUPPORTED     # U14 holds for every operator
     assert L.lp_reduce(ptrs, 4, n, 16, 4, null_stream) == lp.LP_ERR_INVALID_ARG          # root out of range
     assert L.lp_broadcast(ptrs, 4, n, 16, -1, null_stream) == lp.LP_ERR_INVALID_ARG
     assert L.lp_allreduce(None, 4, n, 16, null_stream) == lp.LP_ERR_INVALID_ARG          # NULL array
@@ -164,7 +175,74 @@ def test_compute_entry_fails_loudly_without_device():
     ptrs = (ctypes.c_void_p * 2)(*[a.ctypes.data + ((-a.ctypes.data) % 16) for a in raw])
     # valid arguments, no GPU: the library must refuse (LP_ERR_CUDA), never compute on the CPU
     assert L.lp_allreduce(ptrs, 2, 64, 16, ctypes.c_void_p(0)) == lp.LP_ERR_CUDA
+    assert L.lp_allreduce(ptrs, 2, 64, 0, ctypes.c_void_p(0)) == lp.LP_ERR_CUDA        # block == 0: library chooses
+    assert L.lp_allreduce_op(ptrs, 2, 64, 16, lp.REDUCE_PROD, ctypes.c_void_p(0)) == lp.LP_ERR_CUDA
+    assert L.lp_hbm_probe(ptrs, 1, 1, 64, ctypes.c_void_p(0)) == lp.LP_ERR_CUDA
+    plan = lp.Plan(ALLREDUCE, 2, 64)
+    with pytest.raises(lp.LpError) as ei:
+        L_ = ctypes.c_void_p(0)
+        rc = L.lp_plan_run(plan.handle, ptrs, None, None, ctypes.c_float(0), ctypes.c_float(0), L_)
+        if rc:
+            raise lp.LpError(rc, "lp_plan_run")
+    assert ei.value.status == lp.LP_ERR_CUDA
+    assert "no CUDA device" in lp.status_string(lp.LP_ERR_CUDA)
     assert not raw[0].any() and not raw[1].any()
+
+
+def test_plan_validation_and_info_need_no_device():
+    # a plan carries its own variant and tuning; creating and querying it is host-only
+    with pytest.raises(lp.LpError):
+        lp.Plan(9, 4, 1000)                                           # unknown collective
+    with pytest.raises(lp.LpError):
+        lp.Plan(ALLREDUCE, 0, 1000)
+    with pytest.raises(lp.LpError):
+        lp.Plan(REDUCE, 4, 1000, root=4)
+    with pytest.raises(lp.LpError):
+        lp.Plan(ALLREDUCE, 4, 1000, reduce_op=5)
+    with pytest.raises(lp.LpError):
+        lp.Plan(lp.OP_BSP_SGD, 4, 1000, reduce_op=lp.REDUCE_PROD)     # the SGD steps average: sum only
+    with pytest.raises(lp.LpError):
+        lp.Plan(ALLREDUCE, 4, 1000, tuning={lp.TUNE_TILE_ELEMS: 1000})
+    with pytest.raises(lp.LpError) as ei:
+        lp.Plan(ALLREDUCE, 17, 1000, variant=lp.VARIANT_CLUSTER)
+    assert ei.value.status == lp.LP_ERR_UNSUPPORTED
+    n = 61_000_000
+    free = lp.Plan(ALLREDUCE, 6, n, block=65_536)
+    conf = lp.Plan(ALLREDUCE, 6, n, block=65_536, tuning={lp.TUNE_GRID_LIMIT: 64})
+    a, b = free.info(), conf.info()
+    assert a["variant"] == lp.VARIANT_PIPELINE and a["grid"] == 2 * a["sm_count"]
+    assert b["variant"] == lp.VARIANT_PIPELINE and b["grid"] == 64 and b["tile_elems"] == 4096
+    # the process-wide defaults are untouched by either plan
+    assert lp.lp_get_tuning(lp.TUNE_GRID_LIMIT) == 0 and lp.lp_get_variant() == lp.VARIANT_AUTO
+    d = lp.Plan(ALLREDUCE, 6, n, variant=lp.VARIANT_DIRECT).info()
+    assert d["variant"] == lp.VARIANT_DIRECT and d["block"] == lp.DEFAULT_BLOCK      # block 0 -> LP_DEFAULT_BLOCK
+
+
+def test_auto_block():
+    # block == 0: LP_DEFAULT_BLOCK for the persistent kernels (flat in block), the fitted model's optimum for the
+    # copy-engine variant (PAPER.md:81-89 with the B200 constants, profiles/r2_cost_model_fit.md)
+    n = 61_000_000
+    for v in (lp.VARIANT_AUTO, lp.VARIANT_PIPELINE, lp.VARIANT_DIRECT, lp.VARIANT_CLUSTER):
+        assert lp.lp_auto_block(ALLREDUCE, 6, n, v) == lp.DEFAULT_BLOCK
+        assert lp.lp_auto_block(ALLREDUCE, 6, 1000, v) == 1000                      # clamped to n
+    alpha, beta = lp.lp_fitted_constants(6)
+    assert 1e-6 < alpha < 1e-4 and 1e-13 < beta < 1e-11
+    a2, b2 = lp.lp_fitted_constants(2)
+    assert alpha / beta == pytest.approx(a2 / b2, rel=1e-12) and a2 == pytest.approx(alpha / 5, rel=1e-12)
+    for op in (BCAST, REDUCE, ALLREDUCE):
+        for P in (2, 6, 16):
+            alpha, beta = lp.lp_fitted_constants(P)
+            b = lp.lp_auto_block(op, P, n, lp.VARIANT_COPY_ENGINE)
+            want = lp.lp_optimal_block(op, P, n * 4.0, alpha, beta, 0.0) / 4.0
+            assert b % 4 == 0 and 4 <= b <= n and abs(b - want) <= 4, (op, P, b, want)
+            # and it does minimise the fitted model over the block sizes a caller might try
+            cost = lambda blk: lp.lp_cost_model(lp.ALGO_LP, op, P, n * 4.0, blk * 4.0, alpha, beta, 0.0)  # noqa: E731
+            assert all(cost(b) <= cost(x) * (1 + 1e-9) for x in (16_384, 65_536, 1 << 20, 1 << 22, 1 << 24, n))
+    assert lp.lp_auto_block(ALLREDUCE, 6, n, lp.VARIANT_COPY_ENGINE) > 100 * 16_384   # far from the paper's 64 KB
+    assert lp.lp_auto_block(ALLREDUCE, 1, n, lp.VARIANT_COPY_ENGINE) == n
+    assert lp.lp_auto_block(7, 6, n, lp.VARIANT_AUTO) == 0 and lp.lp_auto_block(ALLREDUCE, 0, n, lp.VARIANT_AUTO) == 0
+    info = lp.Plan(ALLREDUCE, 6, n, variant=lp.VARIANT_COPY_ENGINE).info()
+    assert info["block"] == lp.lp_auto_block(ALLREDUCE, 6, n, lp.VARIANT_COPY_ENGINE)
 
 
 # ---- cost model of Sec. 3.2 (host only) --------------------------------------------------------------------
