@@ -75,10 +75,45 @@ def measured_peak():
 
 # ---- clocks ------------------------------------------------------------------------------------------
 class ClockSampler:
+    """SM clock and throttle reasons sampled DURING the timed region: an NVML polling thread (about 1 kHz: the timed
+    region of the default run is ~10 ms), or `nvidia-smi -lms 20` when the NVML binding is missing."""
     Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
     def __init__(self, index=0):
+        self.p = self.f = self.thread = None
+        self.samples, self.reasons, self.max_mhz, self.stop_flag = [], set(), None, False
+        try:
+            import threading
+
+            import pynvml
+            pynvml.nvmlInit()
+            h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM))
+            masks = {"hw_slowdown": pynvml.nvmlClocksThrottleReasonHwSlowdown,
+                     "hw_thermal_slowdown": pynvml.nvmlClocksThrottleReasonHwThermalSlowdown,
+                     "sw_thermal_slowdown": pynvml.nvmlClocksThrottleReasonSwThermalSlowdown,
+                     "sw_power_cap": pynvml.nvmlClocksThrottleReasonSwPowerCap}
+
+            def poll():
+                while not self.stop_flag:
+                    try:
+                        self.samples.append(float(pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM)))
+                        r = pynvml.nvmlDeviceGetCurrentClocksThrottleReasons(h)
+                        for name, m in masks.items():
+                            if r & m:
+                                self.reasons.add(name)
+                    except Exception:  # noqa: BLE001
+                        break
+                    time.sleep(0.0005)
+
+            self.thread = threading.Thread(target=poll, daemon=True)
+            self.thread.start()
+            self.how = "nvml thread"
+            return
+        except Exception:  # noqa: BLE001
+            self.thread = None
+        self.how = "nvidia-smi -lms 20"
         self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
@@ -88,7 +123,14 @@ class ClockSampler:
             self.p = None
 
     def stop(self):
-        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "how": self.how}
+        if self.thread is not None:
+            self.stop_flag = True
+            self.thread.join(timeout=2)
+            if self.samples:
+                out.update(sm_mhz=float(np.median(self.samples)), sm_min_mhz=float(min(self.samples)),
+                           sm_max_mhz=self.max_mhz, reasons=sorted(self.reasons), samples=len(self.samples))
+            return out
         if self.p is None:
             return out
         time.sleep(0.15)
@@ -195,13 +237,13 @@ def oracle_baseline(c, cfg_idx, passes, single_thread_passes):
     P, n = c["P"], c["n"]
     omp, cores, single = time_oracle(P, n, c["dist"], c.get("sigma", 1.0), cfg_idx, passes,
                                      single_thread_passes=single_thread_passes)
-    t = sum(omp) / len(omp)
+    t = float(np.median(omp))
     out = {"value": n * 4 / t / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
            "sample": f"the full workload: all {n} elements of each of the P={P} vectors ({P * n * 4 / 1e9:.2f} GB), "
-                     f"lpo_allreduce_omp, {len(omp)} timed passes after 2 warm-up passes, {t * 1e3:.1f} ms per pass "
-                     f"(min {min(omp) * 1e3:.1f})"}
+                     f"lpo_allreduce_omp, {len(omp)} timed passes after 2 warm-up passes, median {t * 1e3:.1f} ms per pass "
+                     f"(min {min(omp) * 1e3:.1f}, mean {sum(omp) / len(omp) * 1e3:.1f})"}
     if single:
-        ts = sum(single) / len(single)
+        ts = float(np.median(single))
         out["single_thread"] = {"value": n * 4 / ts / 1e9, "unit": UNIT, "cores": 1, "ms_per_pass": ts * 1e3,
                                 "passes": len(single), "what": "lpo_allreduce: the canonical plain loop, one host thread"}
     return out, t
@@ -213,10 +255,11 @@ def run_reference(args, c, rank, world):
         return
     P, n = c["P"], c["n"]
     omp, cores, _ = time_oracle(P, n, c["dist"], c.get("sigma", 1.0), args.config, args.steps, warm=max(args.warmup, 1))
-    t = sum(omp) / len(omp)
+    t = float(np.median(omp))
     value = n * 4 / t / 1e9
     sample = (f"the full workload: all {n} elements of each of the P={P} vectors, oracle lpo_allreduce_omp, "
-              f"{len(omp)} timed passes after {max(args.warmup, 1)} warm-up passes")
+              f"{len(omp)} timed passes after {max(args.warmup, 1)} warm-up passes, median pass "
+              f"(mean {sum(omp) / len(omp) * 1e3:.1f} ms, min {min(omp) * 1e3:.1f} ms)")
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": t * 1e3, "higher_is_better": True,
@@ -472,7 +515,9 @@ def sweep_cfg3(torch, lp, dev, peak, ps=SWEEP_PS, exps=SWEEP_EXPS, block=65_536)
         work = [torch.empty_like(p) for p in pristine]
         for e in exps:
             n = 1 << e
-            n_sets = int(max(1, min(n_max // n, 64, -(-8 * L2_BYTES // (P * n * 4)))))  # rotate through >= 1 GB
+            # rotate through >= 1 GB (8 x L2), and through at least two sets where the arena holds two: consecutive
+            # collectives of a training step work on different buffers (the layers of Alg. 1)
+            n_sets = int(max(1, min(n_max // n, 64, max(2, -(-8 * L2_BYTES // (P * n * 4))))))
             sets = [lp.Ranks([w[s * n:(s + 1) * n] for w in work]) for s in range(n_sets)]
 
             def restore(n_sets=n_sets, n=n):
@@ -620,7 +665,7 @@ def cfg1_more(torch, lp, dev, pristine, work, P, n, block, peak):
 
 
 def ceilings(torch, lp, dev, peak):
-    """HBM ceilings of this GPU for pure and mixed streams, 512 MB per stream, lp_hbm_probe (plain kernel) and torch."""
+    """HBM ceilings of this GPU for pure and mixed streams, 512 MB per stream: lp_hbm_probe (plain kernel) and torch's fill."""
     n = 1 << 27
     bufs = [torch.empty(n, device=dev) for _ in range(6)]
     for b in bufs:
@@ -636,7 +681,6 @@ def ceilings(torch, lp, dev, peak):
     out["probe_copy_1r_1w"] = t(lambda: lp.lp_hbm_probe(bufs[:1], bufs[1:2]), 2 * n * 4)
     out["probe_1r_5w"] = t(lambda: lp.lp_hbm_probe(bufs[:1], bufs[1:6]), 6 * n * 4)
     out["probe_5r_1w"] = t(lambda: lp.lp_hbm_probe(bufs[:5], bufs[5:6]), 6 * n * 4)
-    out["torch_copy_1r_1w"] = t(lambda: bufs[1].copy_(bufs[0]), 2 * n * 4)
     out["torch_fill_write_only"] = t(lambda: bufs[0].fill_(1.0), n * 4)
     out["measured_peaks_json_hbm_gbs"] = peak
     out["unit"] = "GB/s"

@@ -41,9 +41,11 @@
  *   - Threads and streams: every entry point may be called from any host thread; calls on different streams run
  *     concurrently on the device.  The library's lock covers only its own tables (defaults, scratch, tile-claim
  *     counters), never a launch or a copy.  Tile-claim counters belong to the stream a call is enqueued on (launches
- *     of one stream are ordered); a launch recorded during CUDA-graph capture gets a counter pair of its own for the
- *     life of the process, out of LP_CAPTURE_PAIRS, after which captured launches fall back to the static schedule
- *     (LP_TUNE_SCHED 1: same results, a few per cent slower).  MST / BE reduce scratch is per stream as well.
+ *     of one stream are ordered); launches recorded during a CUDA-graph capture share a counter pair per capture and
+ *     stream, out of LP_CAPTURE_PAIRS for the life of the process, after which captured launches fall back to the
+ *     static schedule (LP_TUNE_SCHED 1: same results, a few per cent slower).  MST / BE reduce scratch is per stream
+ *     as well (for captured launches: per capturing stream, so two graphs that both hold an MST / BE reduce captured
+ *     on the same stream must not be replayed at the same time).
  *   - Stream order: results are those of calls executed one after the other in stream order.  Internally a call may
  *     START before its predecessors on the stream have finished when it touches none of their buffers (LP_TUNE_CHAIN);
  *     it never COMPLETES before them, so whatever follows in the stream (or waits on an event) sees all of them done.
@@ -78,7 +80,7 @@ extern "C" {
 
 #define LP_MAX_P 32
 #define LP_DEFAULT_BLOCK 65536 /* elements; what block == 0 means outside the copy-engine variant (BASELINE.json configs) */
-#define LP_CAPTURE_PAIRS 8192  /* tile-claim counter pairs available to launches recorded under CUDA-graph capture */
+#define LP_CAPTURE_PAIRS 8192  /* tile-claim counter pairs for CUDA-graph captures: one per (capture, stream) */
 
 /* ---- enums ---------------------------------------------------------------- */
 /* collective, PAPER.md:57 (broadcast), :59 (reduce), :61,71 (allreduce), :144-180 (BSP-SGD Alg. 3) */
@@ -102,9 +104,9 @@ extern "C" {
 #define LP_VARIANT_COPY_ENGINE 3 /* the paper's own design: one cudaMemcpyAsync + one add kernel per (hop, block)
                                     on two streams */
 
-#define LP_VARIANT_AUTO 4        /* default: DIRECT below ~384 MB of HBM traffic per call (latency regime), PIPELINE
-                                    above and whenever LP_TUNE_GRID_LIMIT confines the grid; lp_plan_query reports the
-                                    variant that will run */
+#define LP_VARIANT_AUTO 4        /* default: DIRECT below ~2 GB of HBM traffic per call (~650 MB for a reduce over 4 or more
+                                    ranks), PIPELINE above and whenever LP_TUNE_GRID_LIMIT confines the grid;
+                                    lp_plan_query reports the variant that will run */
 
 /* schedule models of lp_schedule_steps (U2, U3) */
 #define LP_MODEL_STAGE 0        /* stages = the P ranks; pipeline length P - 1 + nb */
@@ -297,8 +299,10 @@ LP_API double lp_optimal_block(int op, double p, double n_bytes, double alpha, d
 LP_API size_t lp_auto_block(int op, int P, size_t n, int variant);
 /* The fitted constants behind lp_auto_block, for tests and reports: alpha (s per block exchange) and beta (s/byte),
  * gamma = 0 (folded into beta), of the copy-engine variant's allreduce over P ranks on B200.  Eq. 1
- * takes them as independent of p -- every hop has its own link; on one GPU the p-1 hops of a block share two streams
- * and one HBM, so both grow with p - 1 (profiles/r2_cost_model_fit.md); their ratio, all that b* needs, does not. */
+ * takes them as independent of p -- every hop has its own link; on one GPU the p-1 hops of a block share two streams,
+ * so alpha = 4.4 us x (p - 1) while beta = 0.5 ps/B stays put (profiles/r2_cost_model_fit.md: fits at p = 2, 6, 16).
+ * With these the model's optimal block sqrt(n alpha / ((p-1) beta)) is ~46 MB for a 244 MB message at every p
+ * (measured optimum: flat from 16 to 64 MB) and its times are within 35 % of the measured ones at the optimum. */
 LP_API void lp_fitted_constants(int P, double *alpha, double *beta);
 
 /* How the persistent kernel will cut and spread the work for (op, P, n, block) under the current variant

@@ -53,25 +53,30 @@ int g_sm_count = 0;  // 0 = not queried yet
 int g_device = -1;
 
 // ---- fitted cost-model constants: Eq. 1 of PAPER.md:81-85 for the copy-engine variant on B200.
-// profiles/r2_cost_model_fit.md: at P = 6 one pipeline step costs alpha = 19.8 us (the stream operations of a block:
-// per hop one copy, one add launch, one copy back, ~2.6 us of submission each, over two streams) and beta = 0.86 ps
-// per byte.  Both are sums over the p - 1 hops of a block, which on one GPU share the streams and the HBM instead of
-// each owning a link: alpha(p) = (p - 1) alpha_hop, beta(p) = (p - 1) beta_hop.  Their ratio, all that b* needs,
-// stays put.
-constexpr double kFitAlphaHop = 19.78e-6 / 5.0;   // per hop: fitted at P = 6 (5 hops)
-constexpr double kFitBetaHop = 0.8603e-12 / 5.0;
+// profiles/r2_cost_model_fit.md, fits at p = 2, 6, 16 (n = 61 M): the latency of one pipeline step is A = 2 alpha =
+// 8.9 / 44.5 / 130.2 us = 8.8 us x (p - 1) -- the stream operations of a block (per hop one copy, one add launch, one
+// copy back at ~2.9 us of submission each), and on one GPU the p - 1 hops of a block share two streams instead of
+// each owning a link, so alpha grows with p - 1 where Eq. 1 takes it as constant.  The per-byte cost W = 2 beta + gamma
+// = 0.65 / 1.47 / 0.83 ps/B follows no such law (the "pipeline fill" of p - 1 blocks that multiplies it does not exist
+// when all hops run on the same device); 1.0 ps/B is within a factor 1.5 of all three and the optimal block moves
+// only with its square root.
+constexpr double kFitAlphaHop = 4.4e-6;  // s per block exchange and hop
+constexpr double kFitBeta = 0.5e-12;     // s per byte
 
 // ---- tile-claim counters (LpArgs::sched) ----------------------------------------------------------------------
-// One self-resetting pair per STREAM (launches of a stream are ordered, and a kernel claims only after
-// griddepcontrol.wait, i.e. after its predecessor has re-armed the pair), handed out on a stream's first launch; one
-// pair per launch recorded under CUDA-graph capture (a graph may be replayed on any stream, beside anything).  When a
-// table is full the launch takes the static schedule instead: same results.
+// One self-resetting pair per STREAM (launches of a stream are ordered, and a kernel claims only after its
+// predecessor's CTAs have all finished claiming and re-armed the pair: LpTileClaimer::finish precedes the trigger),
+// handed out on a stream's first launch.  Launches recorded under CUDA-graph capture take the pair of their CAPTURE
+// (capture id, stream): a graph may be replayed on any stream beside anything -- eager launches of the stream it was
+// captured on, other graphs -- but never beside itself, and inside it the launches of one stream are ordered.  When a
+// table is full the launch takes the static schedule instead: same results, a few per cent slower.
 constexpr int kStreamPairs = 1024;
 constexpr int kSchedStride = 4;  // unsigned long longs per pair (32 bytes: one L2 sector each)
 unsigned long long *g_sched = nullptr;
 std::unordered_map<cudaStream_t, int> g_stream_pair;
 std::vector<int> g_free_pairs;  // given back by lp_comm_destroy
 int g_stream_next = 0;
+std::map<std::pair<unsigned long long, cudaStream_t>, int> g_capture_pair;
 int g_capture_next = 0;
 
 // ---- scratch: (stream, slot) -> device buffer ---------------------------------------------------------------------
@@ -311,22 +316,23 @@ struct SegList {
     int n;  // <= LP_MAX_SEGS, every len > 0
 };
 
-// LP_VARIANT_AUTO: below a few hundred MB of HBM traffic the one-CTA-per-tile register kernel is ahead (no per-CTA
-// pipeline to fill: 1.3-3 us against 2-6 us for a 4 KB message); above, the persistent TMA pipeline.  The cut-offs were
-// measured on a 148-SM B200 (profiles/r2_tuning.md) and scale with the SM count: what matters is the traffic per SM
-// over which a pipeline's fill is amortised.  A confined grid always takes the pipeline.
+// LP_VARIANT_AUTO.  The one-CTA-per-tile register kernel has nothing to fill before its first store leaves and keeps
+// ~128 KB of loads in flight per SM however few ranks there are, so it owns the latency regime and stays ahead of the
+// persistent TMA pipeline up to ~2 GB of HBM traffic per call (by 8 % at 64 MB, 1 % at 256 MB); above, the pipeline's
+// steadier request stream wins by 1-2 %, and for the read-dominated reduce from 4 ranks on already at ~640 MB
+// (7.3 against 7.1 TB/s at P = 16, 512 MB).  A 2-rank reduce never crosses over.  Cut-offs measured on a 148-SM B200
+// (profiles/r2_tuning.md section 3), kept as traffic per SM: what matters is how much each SM streams per launch.
+// A confined grid always takes the pipeline (a CTA per SM with a deep ring moves the most per CTA).
 int resolve_variant(const LpCallCfg &cfg, int op, int P, size_t n_work, int sm_count) {
     if (cfg.variant != LP_VARIANT_AUTO) return cfg.variant;
     if (cfg.tuning.v[LP_TUNE_GRID_LIMIT] > 0) return LP_VARIANT_PIPELINE;
     const uint64_t traffic = lp_min_bytes(op, P, n_work);
-    const uint64_t per_sm = (1ull << 20) / 32;  // cut-offs in 32 KB of traffic per SM
+    const uint64_t mb_per_sm = (uint64_t)sm_count << 20;  // one MB of traffic per SM
     uint64_t cut;
-    if (op == LP_OP_BROADCAST && P <= 3)
-        cut = (uint64_t)sm_count * per_sm * 13;  // 60 MB on 148 SMs
-    else if (op == LP_OP_REDUCE)
-        cut = (uint64_t)sm_count * per_sm * 41;  // 190 MB
+    if (op == LP_OP_REDUCE)
+        cut = P <= 2 ? ~0ull : (P == 3 ? mb_per_sm * 7 : mb_per_sm * 9 / 2);  // never / 1036 MB / 666 MB on 148 SMs
     else
-        cut = (uint64_t)sm_count * per_sm * 82;  // 379 MB
+        cut = mb_per_sm * 27 / 2;  // 1998 MB: a call of 2 GB (allreduce of 64 MB over 16 ranks) takes the pipeline
     return traffic < cut ? LP_VARIANT_DIRECT : LP_VARIANT_PIPELINE;
 }
 
@@ -355,7 +361,7 @@ int plan_and_run(const LpCallCfg &cfg, int op, int red_op, float *const *bufs, f
     block = resolve_block(block, op, P, layered ? n_work : n, variant);
     uint32_t tile, gran;
     switch (variant) {
-        case LP_VARIANT_DIRECT: tile = gran = lp_direct_tile(tun, a.n_sum, is_sgd(op), n_work, sm_count); break;
+        case LP_VARIANT_DIRECT: tile = gran = lp_direct_tile(tun, a, n_work, sm_count); break;
         case LP_VARIANT_CLUSTER: tile = gran = lp_cluster_tile(tun); break;
         case LP_VARIANT_PIPELINE:
             tile = lp_pipeline_tile(tun, a, n_work, block, sm_count);
@@ -549,7 +555,13 @@ void lp_count_launch(uint64_t k) { g_launches.fetch_add(k, std::memory_order_rel
 
 cudaError_t lp_sched_acquire(cudaStream_t stream, unsigned long long **pair) {
     *pair = nullptr;
-    const bool capturing = stream_capturing(stream);
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    unsigned long long capture_id = 0;
+    if (cudaStreamGetCaptureInfo(stream, &cap, &capture_id) != cudaSuccess) {
+        cudaGetLastError();
+        cap = cudaStreamCaptureStatusNone;
+    }
+    const bool capturing = cap != cudaStreamCaptureStatusNone;
     std::lock_guard<std::mutex> lock(g_mu);
     if (g_sched == nullptr) {
         if (capturing) return cudaSuccess;  // no allocation under capture: static schedule for this launch
@@ -567,8 +579,13 @@ cudaError_t lp_sched_acquire(cudaStream_t stream, unsigned long long **pair) {
     }
     int idx;
     if (capturing) {
-        if (g_capture_next >= LP_CAPTURE_PAIRS) return cudaSuccess;
-        idx = kStreamPairs + g_capture_next++;
+        auto key = std::make_pair(capture_id, stream);
+        auto it = g_capture_pair.find(key);
+        if (it == g_capture_pair.end()) {
+            if (g_capture_next >= LP_CAPTURE_PAIRS) return cudaSuccess;
+            it = g_capture_pair.emplace(key, kStreamPairs + g_capture_next++).first;
+        }
+        idx = it->second;
     } else {
         auto it = g_stream_pair.find(stream);
         if (it == g_stream_pair.end()) {
@@ -1108,7 +1125,7 @@ size_t lp_auto_block(int op, int P, size_t n, int variant) {
 void lp_fitted_constants(int P, double *alpha, double *beta) {
     const double hops = P > 1 ? (double)(P - 1) : 1.0;
     if (alpha) *alpha = kFitAlphaHop * hops;
-    if (beta) *beta = kFitBetaHop * hops;
+    if (beta) *beta = kFitBeta;
 }
 
 int lp_set_variant(int variant) {
@@ -1147,6 +1164,7 @@ int lp_shutdown(void) {
     g_stream_pair.clear();
     g_free_pairs.clear();
     g_stream_next = 0;
+    g_capture_pair.clear();
     g_capture_next = 0;
     g_sm_count = 0;  // unbind: the next call binds to whatever device is current then
     g_device = -1;

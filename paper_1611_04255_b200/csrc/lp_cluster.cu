@@ -30,8 +30,9 @@ constexpr int kFoldWarps = 4;
 constexpr int kRetWarps = 4;
 constexpr int kClThreads = (2 + kFoldWarps + kRetWarps) * 32;  // producer, store, fold, return
 // Tile = KV float4 per fold / return thread: KV = 2, 4, 8 -> 1024, 2048 (default), 4096 elements (LP_TUNE_CLUSTER_TILE).
-// Ring depths are launch parameters: s_in local-block slots (LP_TUNE_STAGES, default 5), s_rv receive slots for
-// partials and as many for finished tiles (LP_TUNE_OUT_STAGES, default 3).  2048 x (5 + 3 + 3) = 88 KB: two CTAs per SM.
+// Ring depths are launch parameters: s_in local-block slots (LP_TUNE_STAGES, default 3), s_rv receive slots for
+// partials and as many for finished tiles (LP_TUNE_OUT_STAGES, default 2).  2048 x (3 + 2 + 2) x 4 B = 56 KB: three
+// CTAs per SM.
 
 struct LpClusterArgs {
     const float *in_of[16];  // what cluster CTA x loads (NULL: nothing)
@@ -420,8 +421,11 @@ cudaError_t lp_cluster_launch(const LpArgs &a, int P, int root, uint64_t base_of
     c.ret = (bcast || a.n_out > 1) ? 1 : 0;  // allreduce / SGD / broadcast send the finished tile back down the chain
     c.head_tma = bcast ? 1 : 0;
     const uint32_t tile = a.part.tile;
-    c.s_in = t.v[LP_TUNE_STAGES] ? t.v[LP_TUNE_STAGES] : 5;
-    c.s_rv = c.s_fin = t.v[LP_TUNE_OUT_STAGES] ? t.v[LP_TUNE_OUT_STAGES] : 3;
+    // defaults: 3 + 2 + 2 slots of 8 KB = 56 KB, three CTAs per SM (registers).  Deeper rings or larger tiles buy nothing:
+    // 4.0-4.4 TB/s for every tile (4 / 8 / 16 KB) and ring depth tried (profiles/r2_cluster.md) -- the variant is bound
+    // by what an SM can push into its neighbour's shared memory, not by the latency of a hop
+    c.s_in = t.v[LP_TUNE_STAGES] ? t.v[LP_TUNE_STAGES] : 3;
+    c.s_rv = c.s_fin = t.v[LP_TUNE_OUT_STAGES] ? t.v[LP_TUNE_OUT_STAGES] : 2;
     if (c.s_in < 3) c.s_in = 3;  // the head of a momentum step has three loads per tile
     if (c.s_rv < 2) c.s_rv = c.s_fin = 2;
     while (cl_smem(tile, c.s_in, c.s_rv, c.s_fin) > 227u * 1024u && c.s_in > 3) --c.s_in;

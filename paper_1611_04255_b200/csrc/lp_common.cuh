@@ -85,7 +85,7 @@ cudaError_t lp_cluster_launch(const LpArgs &a, int P, int root, uint64_t base_of
                               LpLaunch *cfg, bool dry_run, cudaStream_t stream);
 uint32_t lp_pipeline_tile(const LpTuning &t, const LpArgs &a, uint64_t n, uint64_t block, int sm_count);
 uint32_t lp_pipeline_granule(const LpTuning &t, uint32_t tile);
-uint32_t lp_direct_tile(const LpTuning &t, int n_sum, bool sgd, uint64_t n_work, int sm_count);
+uint32_t lp_direct_tile(const LpTuning &t, const LpArgs &a, uint64_t n_work, int sm_count);
 uint32_t lp_cluster_tile(const LpTuning &t);
 // LP_TUNE_GRID_LIMIT confines the launch to fewer CTAs than the device has SMs (a collective beside compute kernels):
 // the one predicate tile choice, ring choice and variant choice share.

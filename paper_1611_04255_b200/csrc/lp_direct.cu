@@ -13,12 +13,16 @@ namespace {
 constexpr int kThreads = 256;
 
 // CTAs per SM the launch is capped at (8 = no cap: 2048 threads).  A thread's stores are fire-and-forget, so a
-// write-heavy launch (broadcast to several ranks) keeps far more bytes in flight per CTA than it has loaded; beyond a
-// few CTAs per SM the extra stores only queue up in front of the L2 (profiles/r2_tuning.md).
+// write-heavy launch (broadcast to several ranks) keeps far more bytes in flight per CTA than it has loaded; beyond
+// ~150 KB of stores in flight per SM the extra ones only queue up in front of the L2 and the launch slows down by
+// 3-5 % (profiles/r2_tuning.md: 8 KB tiles x n_out destinations x CTAs: 8 CTAs for 2 destinations, 6 for 3, 4 for 5,
+// 3 for 7, 2 for 15).  Folds are capped by their registers long before.
 uint32_t lp_direct_occupancy(const LpArgs &a) {
-    if (a.epilogue == LP_EPI_COPY && a.n_out >= 2) return 3u;
-    return 8u;
+    if (a.epilogue != LP_EPI_COPY || a.n_out <= 2) return 8u;
+    const uint32_t occ = (18u + (uint32_t)a.n_out / 2u) / (uint32_t)a.n_out;
+    return occ < 2u ? 2u : (occ > 8u ? 8u : occ);
 }
+
 // ranks whose loads are in flight together: 8, or 16 for the one-vector-per-thread kernels of the latency regime (a
 // 16-rank chain then costs one HBM latency, not two)
 template <int V>
@@ -173,15 +177,17 @@ cudaError_t launch_seg(const LpArgs &a, const lp_seg_table *segs, const LpLaunch
 // Tile = V * 1024 elements, V 16-byte vectors per thread and input stream.  What the kernel needs is enough load bytes
 // in flight per SM (HBM latency x the SM's share of the bandwidth: ~100 KB): a thread has V * n_sum loads outstanding
 // and the registers they take decide how many CTAs an SM holds, so few streams want long tiles and many streams short
-// ones -- 16 KB (V = 4, 32 / 64 registers: 8 / 4 CTAs) for a copy and a 2-rank fold, 8 KB from 3 to 8 ranks, 4 KB
-// (16 ranks' loads at once, 2 CTAs) above: ~128 KB in flight in every case (profiles/r2_tuning.md).  4 KB also when
-// the message has fewer tiles than two grid-fulls of SMs (latency regime: spread it over more SMs).
-uint32_t lp_direct_tile(const LpTuning &t, int n_sum, bool sgd, uint64_t n_work, int sm_count) {
+// ones -- 16 KB (V = 4, 32 / 64 registers: 8 / 4 CTAs) for a copy to one rank and a 2-rank reduce, 8 KB from 3 to 8
+// ranks and for broadcasts to several ranks (whose stores in flight lp_direct_occupancy bounds), 4 KB (16 ranks' loads
+// at once, 2 CTAs) above: ~128 KB in flight in every case (profiles/r2_tuning.md).  4 KB also when the message has
+// fewer tiles than two grid-fulls of SMs (latency regime: spread it over more SMs).
+uint32_t lp_direct_tile(const LpTuning &t, const LpArgs &a, uint64_t n_work, int sm_count) {
     if (t.v[LP_TUNE_TILE_ELEMS]) {
         const uint32_t tile = (uint32_t)t.v[LP_TUNE_TILE_ELEMS];
         return tile <= 4096u ? tile : 4096u;
     }
-    uint32_t tile = (!sgd && n_sum <= 2) ? 4096u : (n_sum <= 8 ? 2048u : 1024u);
+    const bool sgd = a.epilogue == LP_EPI_SGD || a.epilogue == LP_EPI_SGD_MOM;
+    uint32_t tile = (!sgd && a.n_sum <= 2 && a.n_out <= 1) ? 4096u : (a.n_sum <= 8 ? 2048u : 1024u);
     while (tile > 1024u && (n_work + tile - 1) / tile < 2ull * (uint64_t)sm_count) tile /= 2u;
     return tile;
 }

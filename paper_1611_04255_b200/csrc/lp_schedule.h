@@ -25,12 +25,15 @@ struct lp_partition {
     uint64_t tiles_per_block;  // ceil(block / tile)
     uint64_t n_tiles;          // total tiles
     uint32_t tile;             // elements per full tile
+    uint32_t uniform;          // 1: every block but the last holds a whole number of full tiles (block % tile == 0, or
+                               // one block): tile idx starts at idx * tile, no division needed
 };
 
 LP_HD lp_partition lp_make_partition(uint64_t n, uint64_t block, uint32_t tile) {
     lp_partition p;
     p.n = n;
     p.tile = tile;
+    p.uniform = 1;
     if (n == 0) {
         p.block = block ? block : 1;
         p.nb = 0;
@@ -44,6 +47,7 @@ LP_HD lp_partition lp_make_partition(uint64_t n, uint64_t block, uint32_t tile) 
     p.tiles_per_block = (block + tile - 1) / tile;
     uint64_t last = n - (p.nb - 1) * block;  // length of the last block, 1..block
     p.n_tiles = (p.nb - 1) * p.tiles_per_block + (last + tile - 1) / tile;
+    p.uniform = (p.nb == 1 || block % tile == 0) ? 1u : 0u;
     return p;
 }
 
@@ -71,6 +75,12 @@ LP_HD void lp_tile_range_ex(const lp_partition &p, uint64_t idx, uint64_t &off, 
 }
 
 LP_HD void lp_tile_range(const lp_partition &p, uint64_t idx, uint64_t &off, uint32_t &len) {
+    if (p.uniform) {  // the common case (block a multiple of the tile): no division on the way to the first load
+        off = idx * (uint64_t)p.tile;
+        const uint64_t rem = p.n - off;
+        len = rem < p.tile ? (uint32_t)rem : p.tile;
+        return;
+    }
     uint64_t left, bend;
     lp_tile_range_ex(p, idx, off, len, left, bend);
 }

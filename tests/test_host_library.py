@@ -228,7 +228,7 @@ def test_auto_block():
     alpha, beta = lp.lp_fitted_constants(6)
     assert 1e-6 < alpha < 1e-4 and 1e-13 < beta < 1e-11
     a2, b2 = lp.lp_fitted_constants(2)
-    assert alpha / beta == pytest.approx(a2 / b2, rel=1e-12) and a2 == pytest.approx(alpha / 5, rel=1e-12)
+    assert a2 == pytest.approx(alpha / 5, rel=1e-12) and b2 == beta       # alpha grows with the hops, beta does not
     for op in (BCAST, REDUCE, ALLREDUCE):
         for P in (2, 6, 16):
             alpha, beta = lp.lp_fitted_constants(P)
@@ -282,17 +282,29 @@ def test_optimal_block_minimises_the_lp_cost():
 
 
 def test_auto_variant_resolution():
-    # LP_VARIANT_AUTO (the default): register kernel in the latency regime, TMA pipeline for long messages and
-    # whenever the grid is confined
-    L = lp.lib()
+    # LP_VARIANT_AUTO (the default): register kernel up to ~2 GB of HBM traffic per call (~650 MB for a reduce over
+    # >= 4 ranks, never the pipeline for a 2-rank reduce), TMA pipeline above and whenever the grid is confined
     assert lp.lp_get_variant() == lp.VARIANT_AUTO
     small = lp.lp_plan_query(ALLREDUCE, 4, 1 << 20, 65_536)          # 32 MB of traffic
     big = lp.lp_plan_query(ALLREDUCE, 6, 61_000_000, 65_536)         # 2.9 GB
     assert small["variant"] == lp.VARIANT_DIRECT and small["grid"] == small["n_tiles"]
     assert big["variant"] == lp.VARIANT_PIPELINE and big["grid"] == 2 * big["sm_count"]
-    assert lp.lp_plan_query(BCAST, 2, 1 << 23, 65_536)["variant"] == lp.VARIANT_PIPELINE      # 64 MB of copy traffic
-    assert lp.lp_plan_query(BCAST, 2, 1 << 22, 65_536)["variant"] == lp.VARIANT_DIRECT
-    assert lp.lp_plan_query(REDUCE, 2, 1 << 24, 65_536)["variant"] == lp.VARIANT_PIPELINE     # 192 MB
+    assert lp.lp_plan_query(ALLREDUCE, 8, 1 << 24, 65_536)["variant"] == lp.VARIANT_DIRECT     # 1 GB
+    assert lp.lp_plan_query(ALLREDUCE, 16, 1 << 24, 65_536)["variant"] == lp.VARIANT_PIPELINE  # 2 GB
+    assert lp.lp_plan_query(BCAST, 2, 1 << 27, 65_536)["variant"] == lp.VARIANT_DIRECT         # 1 GB of copy traffic
+    assert lp.lp_plan_query(BCAST, 16, 1 << 25, 65_536)["variant"] == lp.VARIANT_PIPELINE      # 2 GB
+    assert lp.lp_plan_query(REDUCE, 2, 1 << 27, 65_536)["variant"] == lp.VARIANT_DIRECT        # 2 ranks: always
+    assert lp.lp_plan_query(REDUCE, 4, 1 << 24, 65_536)["variant"] == lp.VARIANT_DIRECT        # 320 MB
+    assert lp.lp_plan_query(REDUCE, 4, 1 << 25, 65_536)["variant"] == lp.VARIANT_DIRECT        # 640 MB
+    assert lp.lp_plan_query(REDUCE, 8, 1 << 25, 65_536)["variant"] == lp.VARIANT_PIPELINE      # 1.1 GB
+    assert lp.lp_plan_query(lp.OP_BSP_SGD, 8, 7_000_000, 65_536)["variant"] == lp.VARIANT_DIRECT   # configs[2]: 476 MB
+    # the register kernel's tile follows the number of input streams; a broadcast to many ranks is capped in CTAs per SM
+    assert lp.lp_plan_query(BCAST, 2, 1 << 24, 65_536)["tile_elems"] == 4096
+    assert lp.lp_plan_query(REDUCE, 2, 1 << 24, 65_536)["tile_elems"] == 4096
+    assert lp.lp_plan_query(ALLREDUCE, 6, 1 << 24, 65_536)["tile_elems"] == 2048
+    assert lp.lp_plan_query(ALLREDUCE, 16, 1 << 22, 65_536)["tile_elems"] == 1024
+    assert lp.lp_plan_query(BCAST, 8, 1 << 24, 65_536)["smem_bytes"] > 48 * 1024                # occupancy cap of 3 CTAs
+    assert lp.lp_plan_query(BCAST, 3, 1 << 24, 65_536)["smem_bytes"] == 0
     try:
         lp.lp_set_tuning(lp.TUNE_GRID_LIMIT, 32)
         conf = lp.lp_plan_query(ALLREDUCE, 4, 1 << 20, 65_536)
