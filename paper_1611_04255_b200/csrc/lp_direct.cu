@@ -16,9 +16,10 @@ constexpr int kThreads = 256;
 // write-heavy launch (broadcast to several ranks) keeps far more bytes in flight per CTA than it has loaded; beyond
 // ~150 KB of stores in flight per SM the extra ones only queue up in front of the L2 and the launch slows down by
 // 3-5 % (profiles/r2_tuning.md: 8 KB tiles x n_out destinations x CTAs: 8 CTAs for 2 destinations, 6 for 3, 4 for 5,
-// 3 for 7, 2 for 15).  Folds are capped by their registers long before.
+// 3 for 7; 3 CTAs of 4 KB tiles from 12 destinations on).  Folds are capped by their registers long before.
 uint32_t lp_direct_occupancy(const LpArgs &a) {
     if (a.epilogue != LP_EPI_COPY || a.n_out <= 2) return 8u;
+    if (a.n_out >= 12) return 3u;  // with 4 KB tiles (lp_direct_tile)
     const uint32_t occ = (18u + (uint32_t)a.n_out / 2u) / (uint32_t)a.n_out;
     return occ < 2u ? 2u : (occ > 8u ? 8u : occ);
 }
@@ -187,7 +188,7 @@ uint32_t lp_direct_tile(const LpTuning &t, const LpArgs &a, uint64_t n_work, int
         return tile <= 4096u ? tile : 4096u;
     }
     const bool sgd = a.epilogue == LP_EPI_SGD || a.epilogue == LP_EPI_SGD_MOM;
-    uint32_t tile = (!sgd && a.n_sum <= 2 && a.n_out <= 1) ? 4096u : (a.n_sum <= 8 ? 2048u : 1024u);
+    uint32_t tile = (!sgd && a.n_sum <= 2 && a.n_out <= 1) ? 4096u : ((a.n_sum <= 8 && a.n_out < 12) ? 2048u : 1024u);
     while (tile > 1024u && (n_work + tile - 1) / tile < 2ull * (uint64_t)sm_count) tile /= 2u;
     return tile;
 }

@@ -55,6 +55,8 @@ def main(argv=None):
     ap.add_argument("--P", default="2,3,4,5,6,8,16")
     ap.add_argument("--ops", default="broadcast,reduce,allreduce")
     ap.add_argument("--tune", default="", help="comma list of LP_TUNE key=value (names as in binding.TUNE_*), e.g. CHAIN=2")
+    ap.add_argument("--tune-grid", default="", help="several named tunings to compare, LP only: 'name:K=V,K=V;name2:K=V' "
+                                                     "(an empty list after the colon = library defaults); writes one column per name")
     ap.add_argument("--block", type=int, default=65_536)
     ap.add_argument("--variant", default="auto", choices=["auto", "pipeline", "direct", "cluster"],
                     help="LP realisation timed in the LP column (default: the library default)")
@@ -70,21 +72,23 @@ def main(argv=None):
         lp.lp_set_tuning(getattr(lp, "TUNE_" + k.strip().upper()), int(v))
     ops = tuple(o for o in OPS if o in args.ops.split(","))
     algos = tuple(a for a in ALGOS if a in args.algos.split(","))
+    if args.tune_grid:
+        return tune_grid(torch, dev, args, ops)
     peak = 6553.3
     try:
         peak = float(json.load(open(os.path.join(os.path.dirname(__file__), "..", "MEASURED_PEAKS.json")))["hbm_gbs"])
     except Exception:
         pass
     Ps = [int(x) for x in args.P.split(",")]
-    n_max = 1 << args.max_exp
     rows = []
     for P in Ps:
         # pristine vectors (seed [3, r]) and the working arena, both P x n_max
-        pristine = [torch.from_numpy(inputs.uniform(3, r, n_max)).to(dev) for r in range(P)]
-        work = [torch.empty_like(p) for p in pristine]
+        n_max = arena_elems(P, args.max_exp)
+        pristine = [torch.from_numpy(inputs.uniform(3, r, 1 << args.max_exp)).to(dev) for r in range(P)]
+        work = [torch.empty(n_max, dtype=torch.float32, device=dev) for _ in range(P)]
         for e in range(args.min_exp, args.max_exp + 1):
             n = 1 << e
-            n_sets = int(max(1, min(n_max // n, 64, -(-8 * L2_BYTES // (P * n * 4)))))
+            n_sets = int(max(1, min(n_max // n, 64, max(2, -(-8 * L2_BYTES // (P * n * 4))))))
             sets = [[w[s * n:(s + 1) * n] for w in work] for s in range(n_sets)]
             for op in ops:
                 mb = lp.lp_min_bytes(OP_ID[op], P, n)
@@ -103,8 +107,9 @@ def main(argv=None):
                             call(algo, op, rsets[i % n_sets], args.block)
                     ms = []
                     for rep in range(4):
-                        for w, p in zip(work, pristine):
-                            w[:n_sets * n].copy_(p[:n_sets * n])
+                        for w, p in zip(work, pristine):   # every set starts from the same seeded vectors
+                            for s_ in range(n_sets):
+                                w[s_ * n:(s_ + 1) * n].copy_(p[:n])
                         torch.cuda.synchronize()
                         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                         e0.record()
@@ -128,6 +133,98 @@ def main(argv=None):
         for r in rows:
             f.write(json.dumps(r) + "\n")
     write_markdown(rows, args.out + ".md", peak, Ps, args)
+
+
+def arena_elems(P, max_exp):
+    """Elements per rank of the working arena: the largest message, and at least two buffer sets of it or 1 GB over the
+    P ranks (8 x the 126 MB L2), whichever is more -- so that no cell is timed on an L2-resident working set."""
+    n_max = 1 << max_exp
+    need = -(-8 * L2_BYTES // (P * 4))
+    return max(2 * n_max if 2 * n_max * P * 4 <= (48 << 30) else n_max, -(-need // n_max) * n_max)
+
+
+def parse_tuning(text):
+    out = {}
+    for kv in filter(None, text.split(",")):
+        k, v = kv.split("=")
+        out[getattr(lp, "TUNE_" + k.strip().upper())] = int(v)
+    return out
+
+
+def tune_grid(torch, dev, args, ops):
+    """LP only: the same cells under several named tunings (one column each), same timing method as the sweep."""
+    grid = []
+    for item in filter(None, args.tune_grid.split(";")):
+        name, _, text = item.partition(":")
+        grid.append((name.strip(), parse_tuning(text)))
+    base = parse_tuning(args.tune)
+    Ps = [int(x) for x in args.P.split(",")]
+    rows = []
+    for P in Ps:
+        n_max = arena_elems(P, args.max_exp)
+        pristine = [torch.from_numpy(inputs.uniform(3, r, 1 << args.max_exp)).to(dev) for r in range(P)]
+        work = [torch.empty(n_max, dtype=torch.float32, device=dev) for _ in range(P)]
+        for e in range(args.min_exp, args.max_exp + 1):
+            n = 1 << e
+            n_sets = int(max(1, min(n_max // n, 64, max(2, -(-8 * L2_BYTES // (P * n * 4))))))
+            sets = [lp.Ranks([w[s * n:(s + 1) * n] for w in work]) for s in range(n_sets)]
+            for op in ops:
+                mb = lp.lp_min_bytes(OP_ID[op], P, n)
+                K = int(min(max(2e-3 / max(mb / 3e12, 4e-6), 3), 20 * n_sets, 400))
+                row = dict(op=op, P=P, n=n, msg_bytes=n * 4, min_bytes=mb, calls=K, sets=n_sets, us={})
+                for name, tuning in grid:
+                    for k in range(lp.TUNE_COUNT):
+                        lp.lp_set_tuning(k, base.get(k, 0))
+                    for k, v in tuning.items():
+                        lp.lp_set_tuning(k, v)
+                    call("lp", op, sets[0], args.block)
+                    torch.cuda.synchronize()
+                    graph = torch.cuda.CUDAGraph()
+                    with torch.cuda.graph(graph):
+                        for i in range(K):
+                            call("lp", op, sets[i % n_sets], args.block)
+                    ms = []
+                    for rep in range(4):
+                        for w, p in zip(work, pristine):   # every set starts from the same seeded vectors
+                            for s_ in range(n_sets):
+                                w[s_ * n:(s_ + 1) * n].copy_(p[:n])
+                        torch.cuda.synchronize()
+                        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                        e0.record()
+                        graph.replay()
+                        e1.record()
+                        torch.cuda.synchronize()
+                        if rep:
+                            ms.append(e0.elapsed_time(e1) / K)
+                    del graph
+                    row["us"][name] = round(float(np.median(ms)) * 1e3, 2)
+                rows.append(row)
+                print(json.dumps(row), flush=True)
+        del pristine, work
+        torch.cuda.empty_cache()
+    for k in range(lp.TUNE_COUNT):
+        lp.lp_set_tuning(k, 0)
+    os.makedirs(os.path.dirname(os.path.abspath(args.out)), exist_ok=True)
+    with open(args.out + ".jsonl", "w") as f:
+        for r in rows:
+            f.write(json.dumps(r) + "\n")
+    with open(args.out + ".md", "w") as f:
+        f.write(f"Command: `python -m paper_1611_04255_b200.sweep --out {args.out} --min-exp {args.min_exp} --max-exp {args.max_exp} "
+                f"--P {args.P} --ops {args.ops} --variant {args.variant}" + (f" --tune {args.tune}" if args.tune else "")
+                + f" --tune-grid '{args.tune_grid}'`\n\n")
+        f.write("us per call (CUDA-graph replay of K back-to-back calls / K, median of 3, rotating buffer sets); in brackets the "
+                "fraction of 8 TB/s on the op's minimum HBM bytes.\n\n")
+        names = [g[0] for g in grid]
+        f.write("| op | P | message | " + " | ".join(names) + " |\n|---|---|---|" + "---|" * len(names) + "\n")
+        for r in rows:
+            best = min(r["us"].values())
+            cells = []
+            for nme in names:
+                u = r["us"][nme]
+                txt = f"{u:.2f} ({r['min_bytes'] / u / 1e3 / 8000:.3f})"
+                cells.append(f"**{txt}**" if u == best else txt)
+            f.write(f"| {r['op']} | {r['P']} | {r['msg_bytes'] >> 20} MB | " + " | ".join(cells) + " |\n")
+    return 0
 
 
 def write_markdown(rows, path, peak, Ps, args):
