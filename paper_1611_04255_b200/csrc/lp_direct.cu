@@ -178,17 +178,18 @@ cudaError_t launch_seg(const LpArgs &a, const lp_seg_table *segs, const LpLaunch
 // Tile = V * 1024 elements, V 16-byte vectors per thread and input stream.  What the kernel needs is enough load bytes
 // in flight per SM (HBM latency x the SM's share of the bandwidth: ~100 KB): a thread has V * n_sum loads outstanding
 // and the registers they take decide how many CTAs an SM holds, so few streams want long tiles and many streams short
-// ones -- 16 KB (V = 4, 32 / 64 registers: 8 / 4 CTAs) for a copy to one rank and a 2-rank reduce, 8 KB from 3 to 8
-// ranks and for broadcasts to several ranks (whose stores in flight lp_direct_occupancy bounds), 4 KB (16 ranks' loads
-// at once, 2 CTAs) above: ~128 KB in flight in every case (profiles/r2_tuning.md).  4 KB also when the message has
-// fewer tiles than two grid-fulls of SMs (latency regime: spread it over more SMs).
+// ones -- 16 KB (V = 4, 64 registers: 4 CTAs) for a 2-rank reduce, 8 KB from 3 to 8 ranks and for broadcasts (a copy to
+// one rank: 8 CTAs x 8 KB beat 8 x 16 KB by 1.5 % from 64 to 512 MB and equal the MST baseline's plain copy, which is
+// the same operation at P = 2; broadcasts to several ranks: their stores in flight are what lp_direct_occupancy
+// bounds), 4 KB (16 ranks' loads at once, 2 CTAs) above: ~64-128 KB in flight in every case (profiles/r2_tuning.md).
+// 4 KB also when the message has fewer tiles than two grid-fulls of SMs (latency regime: spread it over more SMs).
 uint32_t lp_direct_tile(const LpTuning &t, const LpArgs &a, uint64_t n_work, int sm_count) {
     if (t.v[LP_TUNE_TILE_ELEMS]) {
         const uint32_t tile = (uint32_t)t.v[LP_TUNE_TILE_ELEMS];
         return tile <= 4096u ? tile : 4096u;
     }
     const bool sgd = a.epilogue == LP_EPI_SGD || a.epilogue == LP_EPI_SGD_MOM;
-    uint32_t tile = (!sgd && a.n_sum <= 2 && a.n_out <= 1) ? 4096u : ((a.n_sum <= 8 && a.n_out < 12) ? 2048u : 1024u);
+    uint32_t tile = (!sgd && a.n_sum == 2 && a.n_out <= 1) ? 4096u : ((a.n_sum <= 8 && a.n_out < 12) ? 2048u : 1024u);
     while (tile > 1024u && (n_work + tile - 1) / tile < 2ull * (uint64_t)sm_count) tile /= 2u;
     return tile;
 }
