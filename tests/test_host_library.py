@@ -299,7 +299,7 @@ def test_auto_variant_resolution():
     assert lp.lp_plan_query(REDUCE, 8, 1 << 25, 65_536)["variant"] == lp.VARIANT_PIPELINE      # 1.1 GB
     assert lp.lp_plan_query(lp.OP_BSP_SGD, 8, 7_000_000, 65_536)["variant"] == lp.VARIANT_DIRECT   # configs[2]: 476 MB
     # the register kernel's tile follows the number of input streams; a broadcast to many ranks is capped in CTAs per SM
-    assert lp.lp_plan_query(BCAST, 2, 1 << 24, 65_536)["tile_elems"] == 4096
+    assert lp.lp_plan_query(BCAST, 2, 1 << 24, 65_536)["tile_elems"] == 2048  # one-destination copy: 8 CTAs x 8 KB (profiles/r2_tuning.md 2b)
     assert lp.lp_plan_query(REDUCE, 2, 1 << 24, 65_536)["tile_elems"] == 4096
     assert lp.lp_plan_query(ALLREDUCE, 6, 1 << 24, 65_536)["tile_elems"] == 2048
     assert lp.lp_plan_query(ALLREDUCE, 16, 1 << 22, 65_536)["tile_elems"] == 1024
