@@ -28,6 +28,10 @@ OP_BROADCAST, OP_REDUCE, OP_ALLREDUCE = 0, 1, 2
 RED_SUM, RED_PROD = 0, 1  # PAPER.md:59 "summations and multiplications"
 ALGO_LP, ALGO_MST, ALGO_BE = 0, 1, 2
 READING_A_REVERSE, READING_B_RING = 0, 1
+# element types (lpo_oracle.c section 7, U21); f16 vectors are numpy float16 arrays, bf16 vectors are numpy
+# uint16 arrays of bit patterns (numpy has no bfloat16), f64 / f32 the native types
+DT_F32, DT_F16, DT_BF16, DT_F64 = 0, 1, 2, 3
+NP_OF_DT = {DT_F32: np.float32, DT_F16: np.float16, DT_BF16: np.uint16, DT_F64: np.float64}
 
 
 def build(force: bool = False) -> str:
@@ -71,6 +75,16 @@ def lib() -> ctypes.CDLL:
         for name in ("lpo_allreduce_op", "lpo_mst_allreduce_op", "lpo_be_allreduce_op"):
             getattr(L, name).argtypes = [pp, i32, sz, i32]
         L.lpo_collective_segments_op.argtypes = [i32, i32, pp, i32, sz, ctypes.POINTER(sz), ctypes.POINTER(sz), i32, i32]
+        L.lpo_chain_fold_dt.argtypes = [pp, i32, sz, i32, i32, ctypes.c_void_p]
+        L.lpo_broadcast_dt.argtypes = [pp, i32, sz, i32, i32]
+        L.lpo_reduce_dt.argtypes = [pp, i32, sz, i32, i32, i32]
+        L.lpo_allreduce_dt.argtypes = [pp, i32, sz, i32, i32]
+        for name in ("lpo_f16_from_f64", "lpo_bf16_from_f64"):
+            getattr(L, name).argtypes = [ctypes.c_double]
+            getattr(L, name).restype = ctypes.c_uint16
+        for name in ("lpo_f16_to_f64", "lpo_bf16_to_f64"):
+            getattr(L, name).argtypes = [ctypes.c_uint16]
+            getattr(L, name).restype = ctypes.c_double
         L.lpo_lp_blocked.argtypes = [pp, i32, sz, sz, i32, i32, pu64]
         L.lpo_num_blocks.argtypes = [sz, sz]
         L.lpo_num_blocks.restype = u64
@@ -149,6 +163,56 @@ def allreduce_op(bufs, red, algo=ALGO_LP):
     arr, n = _ptrs(bufs)
     f = {ALGO_LP: "lpo_allreduce_op", ALGO_MST: "lpo_mst_allreduce_op", ALGO_BE: "lpo_be_allreduce_op"}[algo]
     _check(getattr(lib(), f)(arr, len(bufs), n, red), f)
+
+
+def _ptrs_dt(bufs, dt):
+    want = np.dtype(NP_OF_DT[dt])
+    for b in bufs:
+        if not (isinstance(b, np.ndarray) and b.dtype == want and b.flags.c_contiguous and b.flags.writeable):
+            raise TypeError(f"oracle buffers of element type {dt} must be writable C-contiguous {want} numpy arrays")
+    n = bufs[0].size if bufs else 0
+    if any(b.size != n for b in bufs):
+        raise ValueError("all ranks must hold vectors of the same length")
+    return (ctypes.c_void_p * len(bufs))(*[b.ctypes.data for b in bufs]), n
+
+
+def chain_fold_dt(bufs, dt, red=RED_SUM) -> np.ndarray:
+    """Left fold in rank order, one RN operation in the element type per combine (U21)."""
+    arr, n = _ptrs_dt(bufs, dt)
+    out = np.empty(n, dtype=NP_OF_DT[dt])
+    _check(lib().lpo_chain_fold_dt(arr, len(bufs), n, dt, red, out.ctypes.data), "lpo_chain_fold_dt")
+    return out
+
+
+def broadcast_dt(bufs, dt, root=0):
+    arr, n = _ptrs_dt(bufs, dt)
+    _check(lib().lpo_broadcast_dt(arr, len(bufs), n, dt, root), "lpo_broadcast_dt")
+
+
+def reduce_dt(bufs, dt, red=RED_SUM, root=0):
+    arr, n = _ptrs_dt(bufs, dt)
+    _check(lib().lpo_reduce_dt(arr, len(bufs), n, dt, root, red), "lpo_reduce_dt")
+
+
+def allreduce_dt(bufs, dt, red=RED_SUM):
+    arr, n = _ptrs_dt(bufs, dt)
+    _check(lib().lpo_allreduce_dt(arr, len(bufs), n, dt, red), "lpo_allreduce_dt")
+
+
+def f16_from_f64(x: float) -> int:
+    return int(lib().lpo_f16_from_f64(float(x)))
+
+
+def bf16_from_f64(x: float) -> int:
+    return int(lib().lpo_bf16_from_f64(float(x)))
+
+
+def f16_to_f64(bits: int) -> float:
+    return float(lib().lpo_f16_to_f64(int(bits)))
+
+
+def bf16_to_f64(bits: int) -> float:
+    return float(lib().lpo_bf16_to_f64(int(bits)))
 
 
 def collective_segments_op(op, red, bufs, segments, root=0):

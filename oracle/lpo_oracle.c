@@ -1068,3 +1068,198 @@ double lpo_cost(int algo, int op, double p, double n, double b, double alpha,
         return (lg + p - 1.0) * alpha + 2.0 * f * n * beta;
     return 2.0 * lg * alpha + 2.0 * f * n * beta + f * n * gamma;
 }
+
+/* ------------------------------------------------------------------------ */
+/* 7. Element types other than fp32 (SURVEY 8(f)-4 "other reduce ops /        */
+/*    dtypes"; reading U21)                                         */
+/* ------------------------------------------------------------------------ */
+
+/* The paper's messages are fp32 (Caffe).  This section extends the result
+ * definitions of sections 1 and 5b to vectors of IEEE binary16 (f16), bfloat16
+ * (bf16: 1 sign, 8 exponent, 7 fraction bits) and binary64 (f64).  Reading U21:
+ * the chain forwards the running partial as a block of the message itself
+ * ("GPU1 reduces the received block a0 with a1 to yield a'", and
+ * a' then travels to GPU2 like any block), so the partial HAS the message's
+ * element type: every combine is ONE round-to-nearest-even operation in that
+ * type,
+ *     F[i] = (((x_0[i] op x_1[i]) op x_2[i]) op ...) op x_{P-1}[i],
+ * op = + or *, no wider accumulator, no flush-to-zero.  f16 and bf16 values are
+ * passed as their 16-bit patterns (uint16_t).
+ *
+ * How one RN operation in a 16-bit type is computed here: both operands are
+ * converted to double (exact), the operation is done in double, and the result
+ * is rounded ONCE more to the narrow type by round_to_narrow() below.
+ *  - products: 11 x 11 (f16) or 8 x 8 (bf16) significand bits -> exact in double;
+ *  - sums: exact in double whenever the operands' exponents differ by less
+ *    than 53 - p bits (p = 11 / 8 significand bits); beyond that the smaller
+ *    operand is below 2^-40 ulp of the larger and neither rounding moves the
+ *    result off the larger operand.  (In general a second rounding from a
+ *    format with at least 2p + 2 significand bits is innocuous for + and *.)
+ * So the value is the correctly rounded result of the exact operation.       */
+
+#define LPO_DT_F32 0
+#define LPO_DT_F16 1
+#define LPO_DT_BF16 2
+#define LPO_DT_F64 3
+
+/* Round a double to the nearest value of a binary format with `p` significand
+ * bits (hidden bit included), minimum normal exponent emin (value 2^emin) and
+ * largest finite value (2 - 2^(1-p)) * 2^emax; ties to even; overflow to
+ * infinity; gradual underflow.  Returns sign, biased exponent field and
+ * fraction field packed as (sign << (ebits + p - 1)) | (E << (p - 1)) | frac.
+ * NaN -> quiet NaN with the top fraction bit set.                            */
+static uint32_t round_to_narrow(double x, int p, int ebits)
+{
+    const int bias = (1 << (ebits - 1)) - 1;
+    const int emin = 1 - bias;            /* exponent of the smallest normal */
+    const int emax = bias;                /* exponent of the largest binade  */
+    const uint32_t sign = signbit(x) ? 1u << (ebits + p - 1) : 0u;
+    const uint32_t inf = ((1u << ebits) - 1u) << (p - 1);
+    if (isnan(x))
+        return sign | inf | (1u << (p - 2));
+    double ax = fabs(x);
+    if (isinf(ax))
+        return sign | inf;
+    if (ax == 0.0)
+        return sign;
+    if (ax < ldexp(1.0, emin)) {
+        /* subnormal range: spacing 2^(emin - (p-1)); the scaling is exact     */
+        double q = nearbyint(ldexp(ax, (p - 1) - emin));   /* ties to even     */
+        return sign | (uint32_t)q;       /* q == 2^(p-1) is the smallest normal */
+    }
+    int e;
+    double m = frexp(ax, &e);            /* ax = m * 2^e, 0.5 <= m < 1         */
+    double q = nearbyint(ldexp(m, p));   /* p-bit integer significand, RNE    */
+    if (q == ldexp(1.0, p)) {            /* rounded up into the next binade   */
+        q = ldexp(1.0, p - 1);
+        e += 1;
+    }
+    int E = (e - 1) + bias;              /* ax = (q / 2^(p-1)) * 2^(e-1)       */
+    if (e - 1 > emax)
+        return sign | inf;               /* overflow: RN gives infinity       */
+    return sign | ((uint32_t)E << (p - 1)) | ((uint32_t)q - (1u << (p - 1)));
+}
+
+/* Exact widening of a narrow pattern (p significand bits, ebits exponent bits). */
+static double widen_narrow(uint32_t bits, int p, int ebits)
+{
+    const int bias = (1 << (ebits - 1)) - 1;
+    const uint32_t frac = bits & ((1u << (p - 1)) - 1u);
+    const uint32_t E = (bits >> (p - 1)) & ((1u << ebits) - 1u);
+    const int neg = (bits >> (ebits + p - 1)) & 1u;
+    double v;
+    if (E == (1u << ebits) - 1u)
+        v = frac ? NAN : INFINITY;
+    else if (E == 0)
+        v = ldexp((double)frac, (1 - bias) - (p - 1));
+    else
+        v = ldexp((double)(frac | (1u << (p - 1))), (int)E - bias - (p - 1));
+    return neg ? -v : v;
+}
+
+uint16_t lpo_f16_from_f64(double x) { return (uint16_t)round_to_narrow(x, 11, 5); }
+uint16_t lpo_bf16_from_f64(double x) { return (uint16_t)round_to_narrow(x, 8, 8); }
+double lpo_f16_to_f64(uint16_t h) { return widen_narrow(h, 11, 5); }
+double lpo_bf16_to_f64(uint16_t h) { return widen_narrow(h, 8, 8); }
+
+static size_t dt_size(int dt)
+{
+    return dt == LPO_DT_F64 ? 8 : (dt == LPO_DT_F32 ? 4 : 2);
+}
+static int bad_dt(int dt) { return dt < LPO_DT_F32 || dt > LPO_DT_F64; }
+
+/* element i of a vector of type dt, as a double (exact for every dt) */
+static double dt_load(const void *v, size_t i, int dt)
+{
+    switch (dt) {
+    case LPO_DT_F16: return lpo_f16_to_f64(((const uint16_t *)v)[i]);
+    case LPO_DT_BF16: return lpo_bf16_to_f64(((const uint16_t *)v)[i]);
+    case LPO_DT_F64: return ((const double *)v)[i];
+    default: return (double)((const float *)v)[i];
+    }
+}
+
+/* one RN operation in type dt on two values of type dt (held exactly in doubles) */
+static double dt_combine(double a, double b, int dt, int red)
+{
+    switch (dt) {
+    case LPO_DT_F16: {
+        double r = red == LPO_RED_PROD ? a * b : a + b;
+        return lpo_f16_to_f64(lpo_f16_from_f64(r));
+    }
+    case LPO_DT_BF16: {
+        double r = red == LPO_RED_PROD ? a * b : a + b;
+        return lpo_bf16_to_f64(lpo_bf16_from_f64(r));
+    }
+    case LPO_DT_F64:
+        return red == LPO_RED_PROD ? a * b : a + b;
+    default: {
+        float fa = (float)a, fb = (float)b;      /* exact: a, b are fp32 values */
+        return (double)(red == LPO_RED_PROD ? fa * fb : fa + fb);
+    }
+    }
+}
+
+static void dt_store(void *v, size_t i, int dt, double x)
+{
+    switch (dt) {
+    case LPO_DT_F16: ((uint16_t *)v)[i] = lpo_f16_from_f64(x); break;   /* x is already an f16 value: exact */
+    case LPO_DT_BF16: ((uint16_t *)v)[i] = lpo_bf16_from_f64(x); break;
+    case LPO_DT_F64: ((double *)v)[i] = x; break;
+    default: ((float *)v)[i] = (float)x; break;
+    }
+}
+
+/* F = left fold in rank order of P vectors of n elements of type dt; out may not alias inputs. */
+int lpo_chain_fold_dt(const void *const *in, int P, size_t n, int dt, int red, void *out)
+{
+    if (in == NULL || out == NULL || P < 1 || bad_red(red) || bad_dt(dt))
+        return LPO_EINVAL;
+    for (size_t i = 0; i < n; ++i) {
+        double s = dt_load(in[0], i, dt);
+        for (int r = 1; r < P; ++r)
+            s = dt_combine(s, dt_load(in[r], i, dt), dt, red);
+        dt_store(out, i, dt, s);
+    }
+    return LPO_OK;
+}
+
+/* Broadcast: every rank's vector <- the root's, byte for byte. */
+int lpo_broadcast_dt(void *const *bufs, int P, size_t n, int dt, int root)
+{
+    if (bufs == NULL || P < 1 || root < 0 || root >= P || bad_dt(dt))
+        return LPO_EINVAL;
+    for (int r = 0; r < P; ++r)
+        if (r != root)
+            memcpy(bufs[r], bufs[root], n * dt_size(dt));
+    return LPO_OK;
+}
+
+/* Reduce: root <- F, the other vectors unchanged (U5). */
+int lpo_reduce_dt(void *const *bufs, int P, size_t n, int dt, int root, int red)
+{
+    if (bufs == NULL || P < 1 || root < 0 || root >= P || bad_red(red) || bad_dt(dt))
+        return LPO_EINVAL;
+    for (size_t i = 0; i < n; ++i) {
+        double s = dt_load(bufs[0], i, dt);
+        for (int r = 1; r < P; ++r)
+            s = dt_combine(s, dt_load(bufs[r], i, dt), dt, red);
+        dt_store(bufs[root], i, dt, s);
+    }
+    return LPO_OK;
+}
+
+/* Allreduce: every rank <- F, the same bits everywhere. */
+int lpo_allreduce_dt(void *const *bufs, int P, size_t n, int dt, int red)
+{
+    if (bufs == NULL || P < 1 || bad_red(red) || bad_dt(dt))
+        return LPO_EINVAL;
+    for (size_t i = 0; i < n; ++i) {
+        double s = dt_load(bufs[0], i, dt);
+        for (int r = 1; r < P; ++r)
+            s = dt_combine(s, dt_load(bufs[r], i, dt), dt, red);
+        for (int r = 0; r < P; ++r)
+            dt_store(bufs[r], i, dt, s);
+    }
+    return LPO_OK;
+}

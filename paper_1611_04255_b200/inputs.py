@@ -70,3 +70,47 @@ def small_integers(seed, rank: int, n: int, lo: int = -8, hi: int = 8) -> np.nda
     """Small-integer-valued float32 vector: every summation order is exact."""
     rng = np.random.default_rng([*np.atleast_1d(seed).tolist(), rank])
     return rng.integers(lo, hi + 1, size=n).astype(np.float32)
+
+
+# ---- element types other than fp32 (DESIGN.md U21) --------------------------------------------------------
+# f16 vectors are numpy float16 arrays, bf16 vectors numpy uint16 arrays of bit patterns (numpy has no bfloat16),
+# f64 vectors numpy float64.  The 16-bit values are drawn as BIT PATTERNS (random sign, exponent field in a band,
+# random fraction), so nothing here rounds or converts a floating-point value.
+DT_F32, DT_F16, DT_BF16, DT_F64 = 0, 1, 2, 3
+DT_NAMES = {DT_F32: "f32", DT_F16: "f16", DT_BF16: "bf16", DT_F64: "f64"}
+DT_NUMPY = {DT_F32: np.float32, DT_F16: np.float16, DT_BF16: np.uint16, DT_F64: np.float64}
+_FRAC_BITS = {DT_F16: 10, DT_BF16: 7}
+_EXP_BIAS = {DT_F16: 15, DT_BF16: 127}
+
+
+def typed_vector(seed, rank: int, n: int, dt: int, kind: str = "sum") -> np.ndarray:
+    """One rank's vector of element type `dt`.  kind "sum": magnitudes in [2^-4, 2) (sums over 32 ranks stay finite
+    in every type); "prod": magnitudes in [0.5, 2) (products wander by a few binades, now and then out of f16's range
+    -- both sides then produce the same infinities or zeros); "wide": any finite exponent, subnormals included."""
+    rng = np.random.default_rng([*np.atleast_1d(seed).tolist(), rank, dt])
+    if dt == DT_F32 or dt == DT_F64:
+        ftype = np.float32 if dt == DT_F32 else np.float64
+        if kind == "prod":
+            x = rng.random(n, dtype=ftype) + ftype(0.5)          # [0.5, 1.5)
+            x *= rng.integers(0, 2, size=n).astype(ftype) * ftype(2) - ftype(1)
+            return x
+        x = rng.random(n, dtype=ftype)
+        x *= ftype(2.0)
+        x -= ftype(1.0)
+        return x
+    fb, bias = _FRAC_BITS[dt], _EXP_BIAS[dt]
+    if kind == "sum":
+        e = rng.integers(bias - 4, bias + 1, size=n)
+    elif kind == "prod":
+        e = rng.integers(bias - 1, bias + 1, size=n)
+    elif kind == "wide":
+        e = rng.integers(0, 2 * bias + 1, size=n)                # 0 = zero / subnormal ... 2 * bias = largest binade
+    else:
+        raise ValueError(kind)
+    bits = (rng.integers(0, 2, size=n) << 15) | (e << fb) | rng.integers(0, 1 << fb, size=n)
+    bits = bits.astype(np.uint16)
+    return bits.view(np.float16) if dt == DT_F16 else bits
+
+
+def typed_rank_vectors(seed, P: int, n: int, dt: int, kind: str = "sum"):
+    return [typed_vector(seed, r, n, dt, kind) for r in range(P)]
