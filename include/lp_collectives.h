@@ -95,6 +95,15 @@ extern "C" {
 #define LP_REDUCE_SUM 0
 #define LP_REDUCE_PROD 1
 
+/* element type of the lp_*_dt calls (SURVEY 8(f)-4 "other ... dtypes"; reading U21 in DESIGN.md).  The paper's messages
+ * are fp32; a chain forwards the running partial as a block of the message, so the partial has the
+ * message's element type: every combine is ONE round-to-nearest-even operation in that type, no wider accumulator,
+ * no flush-to-zero.  bf16 = 1 sign, 8 exponent, 7 fraction bits. */
+#define LP_DT_F32 0
+#define LP_DT_F16 1
+#define LP_DT_BF16 2
+#define LP_DT_F64 3
+
 /* realisation of the LP pipeline used by lp_broadcast/lp_reduce/lp_allreduce/lp_bsp_sgd_step */
 #define LP_VARIANT_PIPELINE 0    /* one persistent kernel; per CTA a TMA-bulk shared-memory ring
                                     with mbarrier full/empty flags handed producer warp -> add warps -> store warp */
@@ -168,6 +177,20 @@ LP_API int lp_allreduce(float *const *bufs, int P, size_t n, size_t block, void 
  * order whatever the root (U4).  Unknown reduce_op: LP_ERR_INVALID_ARG. */
 LP_API int lp_reduce_op(float *const *bufs, int P, size_t n, size_t block, int root, int reduce_op, void *cuda_stream);
 LP_API int lp_allreduce_op(float *const *bufs, int P, size_t n, size_t block, int reduce_op, void *cuda_stream);
+
+/* Broadcast / reduce / allreduce of vectors of element type `dtype` (LP_DT_*).  As lp_broadcast / lp_reduce_op /
+ * lp_allreduce_op with bufs[r] pointing at n elements of that type; n and block count ELEMENTS of that type; buffers
+ * are 16-byte aligned and disjoint.  F[i] = ((bufs[0][i] op bufs[1][i]) op ...) op bufs[P-1][i] with every op one RN
+ * operation IN THE ELEMENT TYPE (U21), chain order whatever the root (U4): bit-exact to that definition (NaN results are
+ * NaNs; their payload bits are the hardware's).  Every LP variant takes every type.  16-bit blocks are rounded up to an
+ * even number of elements (results never depend on the block).  LP_DT_F32 is the plain call.  Unknown dtype or
+ * reduce_op: LP_ERR_INVALID_ARG.  The SGD steps, slice lists, plans and the MST / BE baselines stay fp32 (the paper's). */
+LP_API int lp_broadcast_dt(void *const *bufs, int P, size_t n, size_t block, int root, int dtype, void *cuda_stream);
+LP_API int lp_reduce_dt(void *const *bufs, int P, size_t n, size_t block, int root, int dtype, int reduce_op,
+                        void *cuda_stream);
+LP_API int lp_allreduce_dt(void *const *bufs, int P, size_t n, size_t block, int dtype, int reduce_op, void *cuda_stream);
+/* bytes per element of LP_DT_*; 0 for an unknown type */
+LP_API size_t lp_dtype_size(int dtype);
 
 /* Fused BSP-SGD step = Alg. 3's communication + update (Eq. 5, 174, 180):
  *   S = chain sum of grads;  g = S * invP, invP = fl(1.0f / P) (U7);  t = lr * g;  w' = weights[root][i] - t;

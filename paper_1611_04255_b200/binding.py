@@ -22,6 +22,7 @@ TUNE_TILE_ELEMS, TUNE_STAGES, TUNE_OUT_STAGES, TUNE_CTAS_PER_SM, TUNE_CE_STREAMS
     TUNE_CLUSTER_TILE, TUNE_CHAIN, TUNE_DIRECT_OCC = range(16)
 TUNE_COUNT = 16
 REDUCE_SUM, REDUCE_PROD = 0, 1
+DT_F32, DT_F16, DT_BF16, DT_F64 = 0, 1, 2, 3
 DEFAULT_BLOCK = 65536
 VARIANT_NAMES = {0: "pipeline", 1: "direct", 2: "cluster", 3: "copy_engine"}
 
@@ -95,6 +96,11 @@ def lib() -> ctypes.CDLL:
         getattr(L, name).argtypes = [pp, i32, sz, i32, i32, vp]
     for name in ("lp_mst_allreduce_op", "lp_be_allreduce_op"):
         getattr(L, name).argtypes = [pp, i32, sz, i32, vp]
+    L.lp_broadcast_dt.argtypes = [pp, i32, sz, sz, i32, i32, vp]
+    L.lp_reduce_dt.argtypes = [pp, i32, sz, sz, i32, i32, i32, vp]
+    L.lp_allreduce_dt.argtypes = [pp, i32, sz, sz, i32, i32, vp]
+    L.lp_dtype_size.argtypes = [i32]
+    L.lp_dtype_size.restype = sz
     L.lp_plan_desc_init.argtypes = [ctypes.POINTER(PlanDesc)]
     L.lp_plan_create.argtypes = [ctypes.POINTER(PlanDesc), ctypes.POINTER(vp)]
     L.lp_plan_destroy.argtypes = [vp]
@@ -242,6 +248,54 @@ def lp_reduce_op(bufs, block, reduce_op, root=0, stream=None):
 def lp_allreduce_op(bufs, block, reduce_op, stream=None):
     arr, n = _dev_ptrs(bufs)
     _check(lib().lp_allreduce_op(arr, len(bufs), n, block, reduce_op, _stream_ptr(stream)), "lp_allreduce_op")
+
+
+# ---- element types other than fp32 (U21) ------------------------------------------------------------------
+def _torch_dt():
+    import torch
+    return {torch.float32: DT_F32, torch.float16: DT_F16, torch.bfloat16: DT_BF16, torch.float64: DT_F64}
+
+
+def _dev_ptrs_dt(bufs, dtype=None):
+    """Host array of device pointers from CUDA tensors of one element type; returns (array, n, LP_DT_*).  `dtype`
+    overrides the tensors' own type for tensors that only carry bit patterns (int16 / uint16 holding f16 or bf16)."""
+    import torch
+    n = bufs[0].numel() if len(bufs) else 0
+    table = _torch_dt()
+    dt = dtype
+    for b in bufs:
+        if not (isinstance(b, torch.Tensor) and b.is_cuda and b.is_contiguous()):
+            raise TypeError("buffers must be contiguous CUDA tensors")
+        if b.numel() != n:
+            raise ValueError("all ranks must hold vectors of the same length")
+        if dtype is None:
+            if b.dtype not in table:
+                raise TypeError(f"no LP element type for {b.dtype}")
+            if dt is not None and table[b.dtype] != dt:
+                raise TypeError("all ranks must hold the same element type")
+            dt = table[b.dtype]
+        elif b.element_size() != int(lib().lp_dtype_size(dtype)):
+            raise TypeError("tensor element size does not match the LP element type")
+    return (ctypes.c_void_p * len(bufs))(*[b.data_ptr() for b in bufs]), n, (DT_F32 if dt is None else dt)
+
+
+def lp_broadcast_dt(bufs, block, root=0, dtype=None, stream=None):
+    arr, n, dt = _dev_ptrs_dt(bufs, dtype)
+    _check(lib().lp_broadcast_dt(arr, len(bufs), n, block, root, dt, _stream_ptr(stream)), "lp_broadcast_dt")
+
+
+def lp_reduce_dt(bufs, block, root=0, dtype=None, reduce_op=REDUCE_SUM, stream=None):
+    arr, n, dt = _dev_ptrs_dt(bufs, dtype)
+    _check(lib().lp_reduce_dt(arr, len(bufs), n, block, root, dt, reduce_op, _stream_ptr(stream)), "lp_reduce_dt")
+
+
+def lp_allreduce_dt(bufs, block, dtype=None, reduce_op=REDUCE_SUM, stream=None):
+    arr, n, dt = _dev_ptrs_dt(bufs, dtype)
+    _check(lib().lp_allreduce_dt(arr, len(bufs), n, block, dt, reduce_op, _stream_ptr(stream)), "lp_allreduce_dt")
+
+
+def lp_dtype_size(dtype) -> int:
+    return int(lib().lp_dtype_size(dtype))
 
 
 # ---- plans: per-call settings (variant, tuning) instead of the process-wide defaults -----------------------

@@ -26,7 +26,8 @@ cudaError_t lp_be_run(int op, int red_op, float *const *bufs, int P, size_t n, i
                       bool chain, cudaStream_t stream);
 cudaError_t lp_copy_engine_run(int op, int red_op, float *const *bufs, float *const *weights, float *velocity, int P,
                                size_t n, size_t block, int root, float lr, float mu, const LpTuning &t, int sm_count,
-                               cudaStream_t stream);
+                               cudaStream_t stream, int dtype);
+cudaError_t lp_tail16_launch(const LpArgs &a, uint64_t elem, cudaStream_t stream, bool pdl);
 void lp_copy_engine_shutdown();
 cudaError_t lp_probe_launch(float *const *bufs, int n_read, int n_write, size_t n, cudaStream_t stream);
 
@@ -171,11 +172,10 @@ int begin_call(const LpCallCfg *cfg_in, LpCallCfg &cfg, int &sms) {
 
 bool aligned16(const void *p) { return ((uintptr_t)p & 15u) == 0; }
 
-// NULL, alignment and pairwise-overlap checks over `count` buffers of n floats.
-int check_buffers(const float *const *ptrs, int count, size_t n) {
+// NULL, alignment and pairwise-overlap checks over `count` buffers of `bytes` bytes.
+int check_buffers(const float *const *ptrs, int count, size_t bytes) {
     for (int i = 0; i < count; ++i)
         if (ptrs[i] == nullptr || !aligned16(ptrs[i])) return LP_ERR_INVALID_ARG;
-    const size_t bytes = n * sizeof(float);
     if (bytes == 0) return LP_OK;
     for (int i = 0; i < count; ++i)
         for (int j = i + 1; j < count; ++j) {
@@ -197,7 +197,7 @@ int validate_shape(int op, int red_op, int P, int root) {
 }
 
 int validate(int op, int red_op, float *const *bufs, float *const *weights, const float *velocity, int P, size_t n,
-             int root) {
+             int root, size_t elem_bytes = sizeof(float)) {
     int rc = validate_shape(op, red_op, P, root);
     if (rc != LP_OK || bufs == nullptr) return LP_ERR_INVALID_ARG;
     if (is_sgd(op) && weights == nullptr) return LP_ERR_INVALID_ARG;
@@ -208,7 +208,7 @@ int validate(int op, int red_op, float *const *bufs, float *const *weights, cons
     if (is_sgd(op))
         for (int r = 0; r < P; ++r) all[m++] = weights[r];
     if (velocity) all[m++] = velocity;
-    return check_buffers(all, m, n);
+    return check_buffers(all, m, n * elem_bytes);
 }
 
 int validate_tuning(int key, int value) {
@@ -255,8 +255,9 @@ int validate_tuning(int key, int value) {
 // The kernel argument block of one collective (which vectors are folded, in which order; where the finished
 // tile goes).  The fold order is ALWAYS rank 0 -> P-1 (U4); `root` only selects sources / destinations.
 void fill_args(LpArgs &a, int op, int red_op, float *const *bufs, float *const *weights, float *velocity, int P, int root,
-               float lr, float mu, const LpTuning &t) {
+               float lr, float mu, const LpTuning &t, int dtype) {
     memset(&a, 0, sizeof(a));
+    a.dtype = dtype;
     a.lr = lr;
     a.mu = mu;
     a.invP = 1.0f / (float)P;  // one RN division on the host (U7)
@@ -346,12 +347,13 @@ size_t resolve_block(size_t block, int op, int P, size_t n, int variant) {
 // Plans (and unless dry_run, enqueues) one LP collective on device buffers.
 int plan_and_run(const LpCallCfg &cfg, int op, int red_op, float *const *bufs, float *const *weights, float *velocity,
                  int P, size_t n, size_t block, int root, float lr, float mu, int sm_count, lp_plan_info *info,
-                 bool dry_run, cudaStream_t stream, const SegList *segl = nullptr) {
+                 bool dry_run, cudaStream_t stream, const SegList *segl = nullptr, int dtype = LP_DT_F32,
+                 LpArgs *args_out = nullptr) {
     const bool layered = segl != nullptr && segl->n > 0;
     const LpTuning &tun = cfg.tuning;
     LpArgs a;
     LpLaunch cfg_l = {0, 0, 0, 0, 0, false};
-    fill_args(a, op, red_op, dry_run ? nullptr : bufs, weights, velocity, P, root, lr, mu, tun);
+    fill_args(a, op, red_op, dry_run ? nullptr : bufs, weights, velocity, P, root, lr, mu, tun, dtype);
     size_t n_work = n;  // elements the launch touches per rank
     if (layered) {
         n_work = 0;
@@ -403,7 +405,8 @@ int plan_and_run(const LpCallCfg &cfg, int op, int red_op, float *const *bufs, f
         cfg_l.grid = cfg_l.threads = 0;
         if (!dry_run && !noop) {
             if (!layered) {
-                e = lp_copy_engine_run(op, red_op, bufs, weights, velocity, P, n, block, root, lr, mu, tun, sm_count, stream);
+                e = lp_copy_engine_run(op, red_op, bufs, weights, velocity, P, n, block, root, lr, mu, tun, sm_count, stream,
+                                       dtype);
             } else {  // one chain of copies + adds per slice
                 for (int s = 0; s < segl->n && e == cudaSuccess; ++s) {
                     float *sb[LP_MAX_P], *sw[LP_MAX_P];
@@ -412,7 +415,7 @@ int plan_and_run(const LpCallCfg &cfg, int op, int red_op, float *const *bufs, f
                         sw[r] = weights ? weights[r] + segl->off[s] : nullptr;
                     }
                     e = lp_copy_engine_run(op, red_op, sb, weights ? sw : nullptr, nullptr, P, segl->len[s], block, root, lr,
-                                           mu, tun, sm_count, stream);
+                                           mu, tun, sm_count, stream, dtype);
                 }
             }
         }
@@ -447,6 +450,7 @@ int plan_and_run(const LpCallCfg &cfg, int op, int red_op, float *const *bufs, f
         info->granule_elems = gran;
         info->claim_granules = cfg_l.claim;
     }
+    if (args_out) *args_out = a;
     if (e != cudaSuccess) return cuda_fail(e, "LP launch");
     return LP_OK;
 }
@@ -462,6 +466,47 @@ int run_device(const LpCallCfg *cfg_in, int op, int red_op, float *const *bufs, 
     if (cfg.variant == LP_VARIANT_CLUSTER && P > 16) return LP_ERR_UNSUPPORTED;
     return plan_and_run(cfg, op, red_op, bufs, weights, velocity, P, n, block, root, lr, mu, sms, nullptr, false,
                         (cudaStream_t)cuda_stream);
+}
+
+size_t dtype_bytes(int dtype) { return dtype == LP_DT_F64 ? 8 : (dtype == LP_DT_F32 ? 4 : 2); }
+
+// Collectives on vectors of element type `dtype` (U21).  The kernels address memory in 4-byte words (LpArgs::dtype):
+// an f64 element is two words, two f16 / bf16 elements share one.  n and block arrive in ELEMENTS; 16-bit blocks are
+// rounded up to whole words (results never depend on the block), and the odd last element of a 16-bit vector, which
+// fills only half a word, is folded by a one-thread kernel behind the main launch.
+int run_device_dt(int op, int red_op, int dtype, void *const *bufs, int P, size_t n, size_t block, int root,
+                  void *cuda_stream) {
+    if (dtype < LP_DT_F32 || dtype > LP_DT_F64) return LP_ERR_INVALID_ARG;
+    float *const *fb = reinterpret_cast<float *const *>(bufs);
+    if (dtype == LP_DT_F32)
+        return run_device(nullptr, op, red_op, fb, nullptr, nullptr, P, n, block, root, 0.f, 0.f, cuda_stream);
+    if (is_sgd(op)) return LP_ERR_INVALID_ARG;  // the SGD steps are the paper's fp32 solver
+    int rc = validate(op, red_op, fb, nullptr, nullptr, P, n, root, dtype_bytes(dtype));
+    if (rc != LP_OK) return rc;
+    if (n > (~(size_t)0) / 8) return LP_ERR_INVALID_ARG;
+    LpCallCfg cfg;
+    int sms;
+    rc = begin_call(nullptr, cfg, sms);
+    if (rc != LP_OK) return rc;
+    if (cfg.variant == LP_VARIANT_CLUSTER && P > 16) return LP_ERR_UNSUPPORTED;
+    size_t n_words, block_words;  // block == 0 (the library chooses) stays 0
+    bool odd = false;
+    if (dtype == LP_DT_F64) {
+        n_words = 2 * n;
+        block_words = block > (~(size_t)0) / 2 ? ~(size_t)1 : 2 * block;
+    } else {
+        n_words = n / 2;
+        odd = (n & 1u) != 0;
+        block_words = block / 2 + (block & 1u);
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    LpArgs a;
+    rc = plan_and_run(cfg, op, red_op, fb, nullptr, nullptr, P, n_words, block_words, root, 0.f, 0.f, sms, nullptr, false, st,
+                      nullptr, dtype, &a);
+    if (rc != LP_OK || !odd || (P == 1)) return rc;
+    const cudaError_t e = lp_tail16_launch(a, (uint64_t)n - 1, st, cfg.tuning.v[LP_TUNE_NO_PDL] == 0);
+    if (e != cudaSuccess) return cuda_fail(e, "16-bit tail element");
+    return LP_OK;
 }
 
 // Alg. 2 (PAPER.md:140-168 as read in U9; prose PAPER.md:178): reduce the sub-gradients to the root, the root
@@ -819,6 +864,16 @@ int lp_reduce_op(float *const *bufs, int P, size_t n, size_t block, int root, in
 int lp_allreduce_op(float *const *bufs, int P, size_t n, size_t block, int reduce_op, void *cuda_stream) {
     return run_device(nullptr, LP_OP_ALLREDUCE, reduce_op, bufs, nullptr, nullptr, P, n, block, 0, 0.f, 0.f, cuda_stream);
 }
+int lp_broadcast_dt(void *const *bufs, int P, size_t n, size_t block, int root, int dtype, void *cuda_stream) {
+    return run_device_dt(LP_OP_BROADCAST, LP_REDUCE_SUM, dtype, bufs, P, n, block, root, cuda_stream);
+}
+int lp_reduce_dt(void *const *bufs, int P, size_t n, size_t block, int root, int dtype, int reduce_op, void *cuda_stream) {
+    return run_device_dt(LP_OP_REDUCE, reduce_op, dtype, bufs, P, n, block, root, cuda_stream);
+}
+int lp_allreduce_dt(void *const *bufs, int P, size_t n, size_t block, int dtype, int reduce_op, void *cuda_stream) {
+    return run_device_dt(LP_OP_ALLREDUCE, reduce_op, dtype, bufs, P, n, block, 0, cuda_stream);
+}
+size_t lp_dtype_size(int dtype) { return dtype < LP_DT_F32 || dtype > LP_DT_F64 ? 0 : dtype_bytes(dtype); }
 int lp_bsp_sgd_step(float *const *grads, float *const *weights, int P, size_t n, size_t block, int root, float lr,
                     void *cuda_stream) {
     return run_device(nullptr, LP_OP_BSP_SGD, LP_REDUCE_SUM, grads, weights, nullptr, P, n, block, root, lr, 0.f, cuda_stream);
@@ -1203,6 +1258,6 @@ const char *lp_status_string(int status) {
     }
 }
 
-int lp_version(void) { return 200; }  // 0.2.0
+int lp_version(void) { return 300; }  // 0.3.0
 
 }  // extern "C"

@@ -139,7 +139,7 @@ __global__ void __launch_bounds__(kClThreads)
     const int lane = threadIdx.x & 31;
     const bool mom = a.epilogue == LP_EPI_SGD_MOM;
     const bool sgd = a.epilogue == LP_EPI_SGD || mom;
-    const bool prod = a.red_op == LP_REDUCE_PROD;
+    const int code = lp_fold_code(a.dtype, a.red_op);
 
     if (warp == 0) {
         // ---------------- producer: my rank's tiles from HBM ("local block") ------------------------------------
@@ -227,7 +227,7 @@ __global__ void __launch_bounds__(kClThreads)
                     lp_mbar_wait(&rv_full[rv.slot], rv.phase);
                     const float4 *s = reinterpret_cast<const float4 *>(rv_ring + rv.slot * kClTile);
 #pragma unroll
-                    for (int v = 0; v < kV; ++v) acc[v] = lp_combine4(s[ftid + v * FT], mine[ftid + v * FT], prod);
+                    for (int v = 0; v < kV; ++v) acc[v] = lp_combine4(s[ftid + v * FT], mine[ftid + v * FT], code);
                     __threadfence_block();
                     __syncwarp();
                     if (lane == 0) lp_mbar_arrive(&in_empty[in.slot]);

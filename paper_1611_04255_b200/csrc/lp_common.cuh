@@ -1,6 +1,8 @@
 // lp_common.cuh -- kernel argument block, PTX wrappers (mbarrier, TMA bulk copies) and the
 // internal launcher interface between lp_api.cu and the kernel translation units.  sm_100a only.
 #pragma once
+#include <cuda_bf16.h>
+#include <cuda_fp16.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <string.h>
@@ -27,6 +29,11 @@ struct LpArgs {
     int n_out;
     int epilogue;
     int red_op;    // LP_REDUCE_SUM / LP_REDUCE_PROD: the operator of the fold
+    // Element type of the vectors (LP_DT_*; U21).  Kernels address every vector in 4-byte WORDS whatever the type: an
+    // f32 element is one word, an f64 element two (every offset and length the planner hands out is then even), f16 /
+    // bf16 elements come two to a word (the planner rounds blocks up to whole words; an odd last element is folded by
+    // lp_tail16_launch).  Only the combine and the scalar head / tail path look at the type.  SGD epilogues: f32 only.
+    int dtype;
     float lr, invP, mu;
     float *vel_out;
     int l2_hint;
@@ -97,7 +104,7 @@ inline bool lp_grid_confined(const LpTuning &t, int sm_count) {
 unsigned lp_attr_epoch();
 
 // Segment jobs of the MST / BE baselines: dst[i] = a[i] op b[i] (b != NULL; op = red_op of the launch) or
-// dst[i] = a[i], i in [0, len).
+// dst[i] = a[i], i in [0, len); len counts 4-byte words of vectors of element type `dtype` (LpArgs::dtype).
 struct LpSegJob {
     float *dst;
     const float *a;
@@ -106,7 +113,7 @@ struct LpSegJob {
 };
 #define LP_MAX_JOBS 32
 cudaError_t lp_seg_launch(const LpSegJob *jobs, int n_jobs, int sm_count, cudaStream_t stream, bool pdl,
-                          int red_op = LP_REDUCE_SUM, bool chain = false);
+                          int red_op = LP_REDUCE_SUM, bool chain = false, int dtype = LP_DT_F32);
 // Alg. 2's GradientUpdate on the root: w <- w - lr * (S * invP), or with velocity != NULL the
 // momentum form (U18), element-wise over n floats.
 cudaError_t lp_update_launch(float *w, const float *S, float *velocity, uint64_t n, float lr, float invP, float mu,
@@ -271,11 +278,107 @@ __device__ __forceinline__ float4 lp_add4(const float4 &a, const float4 &b) {
 __device__ __forceinline__ float4 lp_mul4(const float4 &a, const float4 &b) {
     return make_float4(__fmul_rn(a.x, b.x), __fmul_rn(a.y, b.y), __fmul_rn(a.z, b.z), __fmul_rn(a.w, b.w));
 }
-// partial op local block ("summations and multiplications"); `prod` is uniform over the launch
-__device__ __forceinline__ float4 lp_combine4(const float4 &a, const float4 &b, bool prod) {
-    return prod ? lp_mul4(a, b) : lp_add4(a, b);
+// ---- partial op local block ("summations and multiplications") in the element type (U21) -----------
+// `code` = (dtype << 1) | red_op, uniform over the launch: 0 / 1 = f32 sum / product (the paper's case), then f16, bf16,
+// f64.  Every combine is ONE round-to-nearest-even operation in the element type: the partial travels as a block of the
+// message, so it has the message's type; no wider accumulator, no flush-to-zero, no contraction (__h*2_rn, __d*_rn).
+__device__ __forceinline__ int lp_fold_code(int dtype, int red_op) { return (dtype << 1) | red_op; }
+__device__ __forceinline__ __half2 lp_as_h2(float w) {
+    const uint32_t u = __float_as_uint(w);
+    return *reinterpret_cast<const __half2 *>(&u);
 }
-__device__ __forceinline__ float lp_combine1(float a, float b, bool prod) { return prod ? __fmul_rn(a, b) : __fadd_rn(a, b); }
+__device__ __forceinline__ float lp_from_h2(__half2 h) { return __uint_as_float(*reinterpret_cast<const uint32_t *>(&h)); }
+__device__ __forceinline__ __nv_bfloat162 lp_as_b2(float w) {
+    const uint32_t u = __float_as_uint(w);
+    return *reinterpret_cast<const __nv_bfloat162 *>(&u);
+}
+__device__ __forceinline__ float lp_from_b2(__nv_bfloat162 h) {
+    return __uint_as_float(*reinterpret_cast<const uint32_t *>(&h));
+}
+// one 4-byte word: an f32 element, or two f16 / bf16 elements (f64 never comes here: lp_combine_f64)
+template <int CODE>
+__device__ __forceinline__ float lp_word_op(float a, float b) {
+    if constexpr (CODE == 0) return __fadd_rn(a, b);
+    if constexpr (CODE == 1) return __fmul_rn(a, b);
+    if constexpr (CODE == 2) return lp_from_h2(__hadd2_rn(lp_as_h2(a), lp_as_h2(b)));
+    if constexpr (CODE == 3) return lp_from_h2(__hmul2_rn(lp_as_h2(a), lp_as_h2(b)));
+    if constexpr (CODE == 4) return lp_from_b2(__hadd2_rn(lp_as_b2(a), lp_as_b2(b)));
+    if constexpr (CODE == 5) return lp_from_b2(__hmul2_rn(lp_as_b2(a), lp_as_b2(b)));
+    return a;
+}
+__device__ __forceinline__ double lp_words_f64(float lo, float hi) {
+    return __hiloint2double(__float_as_int(hi), __float_as_int(lo));
+}
+__device__ __forceinline__ double lp_combine_f64(double a, double b, bool prod) { return prod ? __dmul_rn(a, b) : __dadd_rn(a, b); }
+template <int CODE>
+__device__ __forceinline__ float4 lp_vec_op(const float4 &a, const float4 &b) {
+    if constexpr (CODE >= 6) {  // two f64 elements
+        const double r0 = lp_combine_f64(lp_words_f64(a.x, a.y), lp_words_f64(b.x, b.y), CODE == 7);
+        const double r1 = lp_combine_f64(lp_words_f64(a.z, a.w), lp_words_f64(b.z, b.w), CODE == 7);
+        return make_float4(__int_as_float(__double2loint(r0)), __int_as_float(__double2hiint(r0)),
+                           __int_as_float(__double2loint(r1)), __int_as_float(__double2hiint(r1)));
+    } else {
+        return make_float4(lp_word_op<CODE>(a.x, b.x), lp_word_op<CODE>(a.y, b.y), lp_word_op<CODE>(a.z, b.z),
+                           lp_word_op<CODE>(a.w, b.w));
+    }
+}
+__device__ __forceinline__ float4 lp_combine4(const float4 &a, const float4 &b, int code) {
+    switch (code) {
+        case 0: return lp_vec_op<0>(a, b);
+        case 1: return lp_vec_op<1>(a, b);
+        case 2: return lp_vec_op<2>(a, b);
+        case 3: return lp_vec_op<3>(a, b);
+        case 4: return lp_vec_op<4>(a, b);
+        case 5: return lp_vec_op<5>(a, b);
+        case 6: return lp_vec_op<6>(a, b);
+        default: return lp_vec_op<7>(a, b);
+    }
+}
+// acc[v] <- acc[v] op x[v] for the first nv of V vectors: the switch on the launch's code sits outside the loop
+template <int V>
+__device__ __forceinline__ void lp_fold_vecs(float4 (&acc)[V], const float4 (&x)[V], int nv, int code) {
+#define LP_FOLD_CASE(C)                                       \
+    case C:                                                   \
+        _Pragma("unroll") for (int v = 0; v < V; ++v) {       \
+            if (v < nv) acc[v] = lp_vec_op<C>(acc[v], x[v]);  \
+        }                                                     \
+        break;
+    switch (code) {
+        LP_FOLD_CASE(0)
+        LP_FOLD_CASE(1)
+        LP_FOLD_CASE(2)
+        LP_FOLD_CASE(3)
+        LP_FOLD_CASE(4)
+        LP_FOLD_CASE(5)
+        LP_FOLD_CASE(6)
+        default:
+            LP_FOLD_CASE(7)
+    }
+#undef LP_FOLD_CASE
+}
+// one word of an f32 / f16 / bf16 vector (codes 0..5)
+__device__ __forceinline__ float lp_combine1(float a, float b, int code) {
+    switch (code) {
+        case 0: return lp_word_op<0>(a, b);
+        case 1: return lp_word_op<1>(a, b);
+        case 2: return lp_word_op<2>(a, b);
+        case 3: return lp_word_op<3>(a, b);
+        case 4: return lp_word_op<4>(a, b);
+        default: return lp_word_op<5>(a, b);
+    }
+}
+// dst[i] = a[i] op b[i] on WORD i of vectors of the code's element type, straight from and to global memory (the few
+// words of a segment outside its 16-byte aligned body).  f64: the element that starts at an even word; odd words are
+// their element's upper half and are skipped (offsets and lengths are even, so both halves lie in the same range).
+__device__ __forceinline__ void lp_word_combine_store(float *dst, const float *a, const float *b, uint64_t i, int code) {
+    if (code >= 6) {
+        if (i & 1u) return;
+        const double x = *reinterpret_cast<const double *>(a + i);
+        *reinterpret_cast<double *>(dst + i) = b ? lp_combine_f64(x, *reinterpret_cast<const double *>(b + i), code == 7) : x;
+        return;
+    }
+    dst[i] = b ? lp_combine1(a[i], b[i], code) : a[i];
+}
 // w' = w - lr * (s * invP): three separately rounded operations (U7)
 __device__ __forceinline__ float lp_sgd1(float s, float w, float lr, float invP) {
     return __fsub_rn(w, __fmul_rn(lr, __fmul_rn(s, invP)));
@@ -412,9 +515,16 @@ struct LpTileSpan {
 // Scalar path for the (at most a few) elements of a tile outside its 16-byte aligned body: the chain fold,
 // epilogue and fan-out for element i, straight from and to global memory.
 __device__ __forceinline__ void lp_scalar_element(const LpArgs &a, uint64_t i) {
+    const int code = lp_fold_code(a.dtype, a.red_op);
+    if (code >= 6) {  // f64: word i is the lower half of an element (i even) or its upper half (skipped)
+        if (i & 1u) return;
+        double s = *reinterpret_cast<const double *>(a.in[0] + i);
+        for (int r = 1; r < a.n_sum; ++r) s = lp_combine_f64(s, *reinterpret_cast<const double *>(a.in[r] + i), code == 7);
+        for (int q = 0; q < a.n_out; ++q) *reinterpret_cast<double *>(a.out[q] + i) = s;
+        return;
+    }
     float s = a.in[0][i];
-    const bool prod = a.red_op == LP_REDUCE_PROD;
-    for (int r = 1; r < a.n_sum; ++r) s = lp_combine1(s, a.in[r][i], prod);
+    for (int r = 1; r < a.n_sum; ++r) s = lp_combine1(s, a.in[r][i], code);
     if (a.epilogue == LP_EPI_SGD) s = lp_sgd1(s, a.in[a.n_sum][i], a.lr, a.invP);
     if (a.epilogue == LP_EPI_SGD_MOM) {
         float v_new, w_new;

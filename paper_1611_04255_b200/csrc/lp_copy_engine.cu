@@ -79,7 +79,7 @@ void lp_copy_engine_shutdown() {
 // op: LP_OP_*.  For LP_OP_BSP_SGD `bufs` are the gradients and `weights` the replicas.
 cudaError_t lp_copy_engine_run(int op, int red_op, float *const *bufs, float *const *weights, float *velocity, int P,
                                size_t n, size_t block, int root, float lr, float mu, const LpTuning &t, int sm_count,
-                               cudaStream_t stream) {
+                               cudaStream_t stream, int dtype) {
     std::lock_guard<std::mutex> lock(g_ce_mu);
     const bool sgd = (op == LP_OP_BSP_SGD || op == LP_OP_BSP_SGD_MOM);
     if (n == 0) return cudaSuccess;
@@ -121,7 +121,7 @@ cudaError_t lp_copy_engine_run(int op, int red_op, float *const *bufs, float *co
             if (r == P - 1 && op == LP_OP_REDUCE) dst = bufs[root] + off;  // "returns the combined value ... to a specific GPU"
             if (r == P - 1 && op == LP_OP_ALLREDUCE) dst = bufs[P - 1] + off;
             LpSegJob job{dst, slot, bufs[r] + off, len};  // partial op local block, RN
-            LP_TRY(lp_seg_launch(&job, 1, sm_count, st, false, red_op));
+            LP_TRY(lp_seg_launch(&job, 1, sm_count, st, false, red_op, false, dtype));
             partial = dst;
         }
         if (op == LP_OP_ALLREDUCE) {

@@ -40,7 +40,7 @@ __global__ void __launch_bounds__(kThreads)
     lp_direct_kernel(const __grid_constant__ LpArgs a, const __grid_constant__ typename LpSegParam<SEG>::type segs) {
     const int n_sum = NS > 0 ? NS : a.n_sum;
     const int tid = threadIdx.x;
-    const bool prod = a.red_op == LP_REDUCE_PROD;
+    const int code = lp_fold_code(a.dtype, a.red_op);
     // a2: one CTA per tile by default (grid == n_tiles): the hardware block scheduler hands the next tile to
     // whichever SM frees up first -- the same balance the pipeline kernel gets from its tile claims, with no
     // per-CTA setup at all, which is what the latency regime wants.  A confined grid (LP_TUNE_GRID_LIMIT /
@@ -95,7 +95,7 @@ __global__ void __launch_bounds__(kThreads)
             for (int j = 0; j < kRankChunk; ++j) {
                 if (NS > 0 ? (r0 + j < NS) : (r0 + j < n_sum)) {
 #pragma unroll
-                    for (int v = 0; v < V; ++v) acc[v] = (r0 + j == 0) ? x[v][j] : lp_combine4(acc[v], x[v][j], prod);
+                    for (int v = 0; v < V; ++v) acc[v] = (r0 + j == 0) ? x[v][j] : lp_combine4(acc[v], x[v][j], code);
                 }
             }
         }

@@ -203,7 +203,7 @@ __global__ void __launch_bounds__((CW + 2) * 32)
     } else {
         // ---------------- add warps: chain fold in registers ----------------------------------------------
         const int ctid = threadIdx.x - 64;
-        const bool prod = a.red_op == LP_REDUCE_PROD;
+        const int code = lp_fold_code(a.dtype, a.red_op);
         Ring ring(stages);
         Ring oring(out_stages);
         for (;;) {
@@ -240,9 +240,7 @@ __global__ void __launch_bounds__((CW + 2) * 32)
 #pragma unroll
                 for (int v = 0; v < V; ++v)
                     if (v < nv) x[v] = s[ctid + v * CT];
-#pragma unroll
-                for (int v = 0; v < V; ++v)
-                    if (v < nv) acc[v] = lp_combine4(acc[v], x[v], prod);
+                lp_fold_vecs<V>(acc, x, nv, code);
                 __syncwarp();
                 if (lane == 0) lp_mbar_arrive(&empty[ring.slot]);
                 ring.advance();

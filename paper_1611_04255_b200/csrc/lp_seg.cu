@@ -9,7 +9,7 @@ namespace {
 
 struct LpSegArgs {
     LpSegJob j[LP_MAX_JOBS];
-    int red_op;  // LP_REDUCE_*: the operator of dst = a op b
+    int code;  // (dtype << 1) | red_op: the operator of dst = a op b and the element type (lp_common.cuh)
     int late_wait;  // lp_chain_admit: wait for the launches ahead at the end of the CTA instead of at its start
 };
 
@@ -27,7 +27,7 @@ __global__ void __launch_bounds__(kSegThreads) lp_seg_kernel(const __grid_consta
 
 __device__ __forceinline__ void lp_seg_body(const LpSegArgs &s) {
     const LpSegJob &job = s.j[blockIdx.y];
-    const bool prod = s.red_op == LP_REDUCE_PROD;
+    const int code = s.code;
     float *dst = job.dst;
     const float *a = job.a;
     const float *b = job.b;
@@ -40,7 +40,7 @@ __device__ __forceinline__ void lp_seg_body(const LpSegArgs &s) {
         const uint64_t per = (uint64_t)kSegThreads * kSegUnroll * 4;
         const uint64_t lo = (uint64_t)blockIdx.x * per;
         const uint64_t hi = lo + per < len ? lo + per : len;
-        for (uint64_t i = lo + threadIdx.x; i < hi; i += kSegThreads) dst[i] = b ? lp_combine1(a[i], b[i], prod) : a[i];
+        for (uint64_t i = lo + threadIdx.x; i < hi; i += kSegThreads) lp_word_combine_store(dst, a, b, i, code);
         return;
     }
     uint64_t head = ((16u - mis) & 15u) >> 2;
@@ -49,8 +49,8 @@ __device__ __forceinline__ void lp_seg_body(const LpSegArgs &s) {
     const uint64_t tail0 = head + (nvec << 2);
     if (blockIdx.x == 0) {
         const uint64_t i = threadIdx.x;
-        if (i < head) dst[i] = b ? lp_combine1(a[i], b[i], prod) : a[i];
-        if (i < len - tail0) dst[tail0 + i] = b ? lp_combine1(a[tail0 + i], b[tail0 + i], prod) : a[tail0 + i];
+        if (i < head) lp_word_combine_store(dst, a, b, i, code);
+        if (i < len - tail0) lp_word_combine_store(dst, a, b, tail0 + i, code);
     }
     float *d4 = dst + head;
     const float *a4 = a + head;
@@ -68,7 +68,7 @@ __device__ __forceinline__ void lp_seg_body(const LpSegArgs &s) {
 #pragma unroll
     for (int u = 0; u < kSegUnroll; ++u) {
         const uint64_t v = v0 + (uint64_t)u * kSegThreads;
-        if (v < nvec) lp_stg_stream(d4 + 4 * v, b4 ? lp_combine4(x[u], y[u], prod) : x[u]);
+        if (v < nvec) lp_stg_stream(d4 + 4 * v, b4 ? lp_combine4(x[u], y[u], code) : x[u]);
     }
 }
 
@@ -106,7 +106,27 @@ __global__ void __launch_bounds__(kSegThreads) lp_update_kernel(float *w, const 
     }
 }
 
+// The odd last element of a 16-bit vector (it fills half a 4-byte word, so the word-addressed kernels stop before it):
+// one thread folds element e of every input in chain order and writes it to every output.  The element rides in the
+// low half of a two-element word whose high half is zero (0 op 0 raises nothing and is dropped).
+__global__ void lp_tail16_kernel(const __grid_constant__ LpArgs a, uint64_t e) {
+    lp_pdl_wait();
+    if (threadIdx.x != 0) return;
+    const int code = lp_fold_code(a.dtype, a.red_op);
+    float s = __uint_as_float((uint32_t) reinterpret_cast<const unsigned short *>(a.in[0])[e]);
+    for (int r = 1; r < a.n_sum; ++r)
+        s = lp_combine1(s, __uint_as_float((uint32_t) reinterpret_cast<const unsigned short *>(a.in[r])[e]), code);
+    for (int q = 0; q < a.n_out; ++q)
+        reinterpret_cast<unsigned short *>(a.out[q])[e] = (unsigned short)(__float_as_uint(s) & 0xffffu);
+}
+
 }  // namespace
+
+cudaError_t lp_tail16_launch(const LpArgs &a, uint64_t elem, cudaStream_t stream, bool pdl) {
+    lp_count_launch(1);
+    lp_chain_reset(stream);  // waits first; touches the last bytes of every vector of the launch ahead of it
+    return lp_launch(lp_tail16_kernel, dim3(1), dim3(32), 0, stream, pdl, a, elem);
+}
 
 cudaError_t lp_update_launch(float *w, const float *S, float *velocity, uint64_t n, float lr, float invP, float mu,
                              cudaStream_t stream, bool pdl) {
@@ -120,9 +140,9 @@ cudaError_t lp_update_launch(float *w, const float *S, float *velocity, uint64_t
 }
 
 cudaError_t lp_seg_launch(const LpSegJob *jobs, int n_jobs, int sm_count, cudaStream_t stream, bool pdl, int red_op,
-                          bool chain) {
+                          bool chain, int dtype) {
     LpSegArgs s;
-    s.red_op = red_op;
+    s.code = (dtype << 1) | red_op;
     int m = 0;
     uint64_t longest = 0;
     for (int i = 0; i < n_jobs; ++i) {
