@@ -279,6 +279,69 @@ LP_API int lp_mst_allreduce_op(float *const *bufs, int P, size_t n, int reduce_o
 LP_API int lp_be_reduce_op(float *const *bufs, int P, size_t n, int root, int reduce_op, void *cuda_stream);
 LP_API int lp_be_allreduce_op(float *const *bufs, int P, size_t n, int reduce_op, void *cuda_stream);
 
+/* ---- the chain over real GPUs: one rank per GPU, peer memory over NVLink / NVSwitch ------ */
+/* PAPER.md:55-59,71,77 (Sec. 3, Fig. 2): rank r receives a block from rank r-1 while it sends one to rank r+1; reduce
+ * adds the local block to the partial on its way up the chain 0 -> 1 -> ... -> P-1 (U4: that order whatever the root),
+ * allreduce sends the finished block back down (U3-A), broadcast runs root -> root+1 -> ... around the ring.  An
+ * lp_chain is ONE rank's endpoint: receive rings and counters in its own device memory that its two neighbours write
+ * through peer mappings (data pushed with plain stores, published with fence.acq_rel.sys + a counter in the
+ * receiver's memory; slots returned by a credit counter in the sender's memory; csrc/lp_chain.cu).
+ *   lp_chain_create(rank, P, channels, slots, tile, &ch)   on the rank's device (current device); 0 = defaults.  Every
+ *       rank must pass the same (P, channels, slots, tile).  channels: 1..LP_CHAIN_MAX_CHANNELS concurrent rings (2 CTAs
+ *       of 512 threads each); slots: ring depth 1..64; tile: 4096 / 8192 / 16384 elements per slot (16384 floats =
+ *       64 KB = the paper's block).
+ *   lp_chain_get_handle(ch, h)     LP_CHAIN_HANDLE_BYTES opaque bytes (a CUDA IPC handle) to all-gather over any
+ *       transport (paper_1611_04255_b200/chain.py uses torch.distributed);
+ *   lp_chain_connect(ch, handles)  handles = P x LP_CHAIN_HANDLE_BYTES in rank order; maps ranks (rank +- 1) mod P.
+ *   lp_chain_connect_ptrs(ch, up, down)  the same for endpoints of this process (lp_chain_endpoint of the neighbours'
+ *       chains; the caller enables peer access between the devices).
+ *   lp_chain_run(ch, op, buf, n, block, root, reduce_op, stream)   this rank's share of LP_OP_BROADCAST / REDUCE /
+ *       ALLREDUCE on its vector buf (n floats, 16-byte aligned, in place; same semantics and the same bits as
+ *       lp_broadcast / lp_reduce_op / lp_allreduce_op over P virtual ranks).  Every rank calls it with the same
+ *       arguments, in the same order as its other chain collectives, on one stream per endpoint.  `block` is rounded
+ *       up to a multiple of 4 elements (0 = one tile); a block is moved in pieces of at most one tile.
+ *   lp_chain_error(ch, &e)   synchronises; e != 0: a wait gave up (a neighbour never arrived) and the result is void.
+ * lp_chain_plan is the host-only part: what `rank` does in (op, P, root) -- its ring neighbours and which of the steps
+ * load / receive / store / send up / send down its forward and return CTAs take.  No device needed.
+ * This build's box has ONE GPU: kernels that wait for each other cannot be run there as separate launches, so what
+ * the GPU tests execute is lp_chain_emulate -- the same per-rank device code for all P ranks in ONE cooperative launch
+ * of P x 2 x channels co-resident CTAs over P endpoints in this device's memory, bufs = the P virtual ranks as
+ * everywhere else in this header (LP_ERR_UNSUPPORTED when that many CTAs do not fit the device). */
+#define LP_CHAIN_HANDLE_BYTES 64
+#define LP_CHAIN_MAX_CHANNELS 64
+#define LP_CHAIN_DEFAULT_CHANNELS 32
+#define LP_CHAIN_EMULATE_CHANNELS 8
+#define LP_CHAIN_DEFAULT_SLOTS 8
+#define LP_CHAIN_DEFAULT_TILE 16384
+typedef struct lp_chain lp_chain;
+typedef struct lp_chain_role {
+    int position;     /* place in the chain of this collective: rank for reduce / allreduce, (rank - root) mod P for broadcast */
+    int up, down;     /* ring neighbours: (rank + 1) mod P, (rank - 1) mod P */
+    int f_active;     /* forward CTAs run */
+    int f_load;       /* ... load the local block */
+    int f_recv;       /* ... receive a block from `down` (and combine it with the local one when both) */
+    int f_send_up;    /* ... push the result to `up` */
+    int f_store;      /* ... store it to the local vector */
+    int f_send_down;  /* ... chain end of allreduce / reduce to another root: push the finished block to `down` */
+    int r_active;     /* return CTAs run: receive finished blocks from `up` */
+    int r_store;      /* ... store them to the local vector */
+    int r_send_down;  /* ... pass them on to `down` */
+} lp_chain_role;
+LP_API int lp_chain_plan(int op, int P, int root, int rank, lp_chain_role *out);
+LP_API size_t lp_chain_endpoint_bytes(int channels, int slots, int tile);
+LP_API int lp_chain_create(int rank, int P, int channels, int slots, int tile, lp_chain **out);
+LP_API int lp_chain_get_handle(lp_chain *ch, void *handle_out);
+LP_API int lp_chain_connect(lp_chain *ch, const void *handles);
+LP_API int lp_chain_connect_ptrs(lp_chain *ch, void *up_endpoint, void *down_endpoint);
+LP_API void *lp_chain_endpoint(lp_chain *ch);
+LP_API int lp_chain_run(lp_chain *ch, int op, float *buf, size_t n, size_t block, int root, int reduce_op, void *cuda_stream);
+LP_API int lp_chain_error(lp_chain *ch, int *error_out);
+LP_API int lp_chain_destroy(lp_chain *ch);
+LP_API int lp_chain_emulate(int op, float *const *bufs, int P, size_t n, size_t block, int root, int reduce_op, int channels,
+                            int slots, int tile, void *cuda_stream);
+LP_API int lp_chain_emulate_channels(int P, int tile);
+LP_API int lp_chain_emulate_error(int P, int channels, int slots, int tile, int *error_out);
+
 /* ---- host-buffer entry points (end-to-end path) ------------------------------- */
 /* Same results as lp_allreduce / lp_bsp_sgd_step, but the P (2P) buffers live in HOST memory (pinned for
  * full speed; pageable works).  The message is cut into chunks that flow host -> device -> kernel -> host

@@ -44,6 +44,14 @@ class PlanInfo(ctypes.Structure):
         return {k: int(getattr(self, k)) for k, _ in self._fields_}
 
 
+class ChainRole(ctypes.Structure):
+    _fields_ = [(k, ctypes.c_int) for k in ("position", "up", "down", "f_active", "f_load", "f_recv", "f_send_up", "f_store",
+                                            "f_send_down", "r_active", "r_store", "r_send_down")]
+
+    def as_dict(self):
+        return {k: int(getattr(self, k)) for k, _ in self._fields_}
+
+
 class PlanDesc(ctypes.Structure):
     _fields_ = [("op", ctypes.c_int), ("reduce_op", ctypes.c_int), ("P", ctypes.c_int), ("root", ctypes.c_int),
                 ("n", ctypes.c_size_t), ("block", ctypes.c_size_t), ("variant", ctypes.c_int),
@@ -101,6 +109,21 @@ def lib() -> ctypes.CDLL:
     L.lp_allreduce_dt.argtypes = [pp, i32, sz, sz, i32, i32, vp]
     L.lp_dtype_size.argtypes = [i32]
     L.lp_dtype_size.restype = sz
+    L.lp_chain_plan.argtypes = [i32, i32, i32, i32, ctypes.POINTER(ChainRole)]
+    L.lp_chain_endpoint_bytes.argtypes = [i32, i32, i32]
+    L.lp_chain_endpoint_bytes.restype = sz
+    L.lp_chain_create.argtypes = [i32, i32, i32, i32, i32, ctypes.POINTER(vp)]
+    L.lp_chain_get_handle.argtypes = [vp, ctypes.c_char_p]
+    L.lp_chain_connect.argtypes = [vp, ctypes.c_char_p]
+    L.lp_chain_connect_ptrs.argtypes = [vp, vp, vp]
+    L.lp_chain_endpoint.argtypes = [vp]
+    L.lp_chain_endpoint.restype = vp
+    L.lp_chain_run.argtypes = [vp, i32, vp, sz, sz, i32, i32, vp]
+    L.lp_chain_error.argtypes = [vp, ctypes.POINTER(i32)]
+    L.lp_chain_destroy.argtypes = [vp]
+    L.lp_chain_emulate.argtypes = [i32, pp, i32, sz, sz, i32, i32, i32, i32, i32, vp]
+    L.lp_chain_emulate_channels.argtypes = [i32, i32]
+    L.lp_chain_emulate_error.argtypes = [i32, i32, i32, i32, ctypes.POINTER(i32)]
     L.lp_plan_desc_init.argtypes = [ctypes.POINTER(PlanDesc)]
     L.lp_plan_create.argtypes = [ctypes.POINTER(PlanDesc), ctypes.POINTER(vp)]
     L.lp_plan_destroy.argtypes = [vp]
@@ -296,6 +319,79 @@ def lp_allreduce_dt(bufs, block, dtype=None, reduce_op=REDUCE_SUM, stream=None):
 
 def lp_dtype_size(dtype) -> int:
     return int(lib().lp_dtype_size(dtype))
+
+
+# ---- the chain over real GPUs (one rank per GPU) and its one-GPU emulation ---------------------------------------
+CHAIN_HANDLE_BYTES = 64
+
+
+def lp_chain_plan(op, P, root, rank) -> dict:
+    """Host only: what `rank` does in collective `op` over P ranks (ring neighbours, forward / return steps)."""
+    role = ChainRole()
+    _check(lib().lp_chain_plan(op, P, root, rank, ctypes.byref(role)), "lp_chain_plan")
+    return role.as_dict()
+
+
+def lp_chain_emulate(op, bufs, block=0, root=0, reduce_op=REDUCE_SUM, channels=0, slots=0, tile=0, stream=None):
+    """All P ranks of the multi-GPU chain on this GPU in one cooperative launch (the same per-rank device code)."""
+    arr, n = _dev_ptrs(bufs)
+    _check(lib().lp_chain_emulate(op, arr, len(bufs), n, block, root, reduce_op, channels, slots, tile, _stream_ptr(stream)),
+           "lp_chain_emulate")
+
+
+def lp_chain_emulate_error(P, channels=0, slots=0, tile=0) -> int:
+    e = ctypes.c_int(0)
+    _check(lib().lp_chain_emulate_error(P, channels, slots, tile, ctypes.byref(e)), "lp_chain_emulate_error")
+    return int(e.value)
+
+
+def lp_chain_emulate_channels(P, tile=0) -> int:
+    return int(lib().lp_chain_emulate_channels(P, tile))
+
+
+class Chain:
+    """One rank's endpoint of the chain over real GPUs (lp_chain_*): create on the rank's device, exchange `handle()`
+    with all ranks (any transport; chain.py uses torch.distributed), `connect(handles)`, then `run(op, buf, ...)`."""
+
+    def __init__(self, rank, P, channels=0, slots=0, tile=0):
+        h = ctypes.c_void_p()
+        _check(lib().lp_chain_create(rank, P, channels, slots, tile, ctypes.byref(h)), "lp_chain_create")
+        self.h, self.rank, self.P = h, rank, P
+
+    def handle(self) -> bytes:
+        buf = ctypes.create_string_buffer(CHAIN_HANDLE_BYTES)
+        _check(lib().lp_chain_get_handle(self.h, buf), "lp_chain_get_handle")
+        return buf.raw
+
+    def endpoint(self) -> int:
+        return int(lib().lp_chain_endpoint(self.h) or 0)
+
+    def connect(self, handles):
+        blob = b"".join(handles)
+        if len(blob) != self.P * CHAIN_HANDLE_BYTES:
+            raise ValueError("need one handle per rank, in rank order")
+        _check(lib().lp_chain_connect(self.h, blob), "lp_chain_connect")
+
+    def connect_ptrs(self, up_endpoint, down_endpoint):
+        _check(lib().lp_chain_connect_ptrs(self.h, ctypes.c_void_p(up_endpoint), ctypes.c_void_p(down_endpoint)),
+               "lp_chain_connect_ptrs")
+
+    def run(self, op, buf, block=0, root=0, reduce_op=REDUCE_SUM, stream=None):
+        import torch
+        if not (isinstance(buf, torch.Tensor) and buf.is_cuda and buf.dtype == torch.float32 and buf.is_contiguous()):
+            raise TypeError("buf must be a contiguous float32 CUDA tensor")
+        _check(lib().lp_chain_run(self.h, op, ctypes.c_void_p(buf.data_ptr()), buf.numel(), block, root, reduce_op,
+                                  _stream_ptr(stream)), "lp_chain_run")
+
+    def error(self) -> int:
+        e = ctypes.c_int(0)
+        _check(lib().lp_chain_error(self.h, ctypes.byref(e)), "lp_chain_error")
+        return int(e.value)
+
+    def destroy(self):
+        if self.h:
+            lib().lp_chain_destroy(self.h)
+            self.h = None
 
 
 # ---- plans: per-call settings (variant, tuning) instead of the process-wide defaults -----------------------

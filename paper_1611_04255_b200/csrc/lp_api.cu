@@ -29,6 +29,7 @@ cudaError_t lp_copy_engine_run(int op, int red_op, float *const *bufs, float *co
                                cudaStream_t stream, int dtype);
 cudaError_t lp_tail16_launch(const LpArgs &a, uint64_t elem, cudaStream_t stream, bool pdl);
 void lp_copy_engine_shutdown();
+void lp_chain_shutdown();
 cudaError_t lp_probe_launch(float *const *bufs, int n_read, int n_write, size_t n, cudaStream_t stream);
 
 // The settings of one call: the process defaults at the time of the call, or a plan's own.
@@ -1213,6 +1214,7 @@ int lp_shutdown(void) {
     std::lock_guard<std::mutex> host_lock(g_host_mu);
     lp_copy_engine_shutdown();
     std::lock_guard<std::mutex> lock(g_mu);
+    lp_chain_shutdown();
     if (g_host_ready || g_sched != nullptr || !g_scratch.empty()) cudaDeviceSynchronize();
     if (g_sched) cudaFree(g_sched);
     g_sched = nullptr;

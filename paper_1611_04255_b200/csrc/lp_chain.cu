@@ -1,0 +1,692 @@
+// lp_chain.cu -- the paper's own setting: ONE RANK PER GPU, the chain GPU r -> r+1 over peer memory (NVLink 5 /
+// NVSwitch P2P), SURVEY 8(e) / 8(f)-4.  PAPER.md:55-59 (Sec. 3, Fig. 2): every GPU "receives a block from the prior
+// GPU ... while sending a block to the next one"; reduce: "GPU1 reduces the received block a0 with a1 to yield a'",
+// which travels on; allreduce sends the finished block back (U3 reading A, reverse flow).
+//
+// Each rank owns an ENDPOINT in its own HBM (one allocation, exported to its two neighbours): per channel a forward
+// receive ring (partials / broadcast blocks from rank r-1) and a backward receive ring (finished blocks from rank r+1)
+// of S slots of one tile, plus four monotonic 64-bit counters.  A transfer is a PUSH: the sender's SMs store the tile
+// into the receiver's ring through the peer mapping (stores are fire-and-forget over NVLink; loads would pay the
+// ~1 us round trip per tile), then one thread publishes it -- barrier, fence.acq_rel.sys, st.relaxed.sys of the ring's
+// tail counter in the RECEIVER's memory, which the receiver polls locally.  A slot goes back by a credit counter in
+// the SENDER's memory, written remotely by the receiver after it has consumed the slot's values.  Counters only ever
+// grow (slot = sequence mod S), so nothing is reset between calls and a rank may run ahead of its neighbours into the
+// next collective; the neighbours of a ring never change: rank r's forward ring is written by rank (r-1) mod P, its
+// backward ring by rank r+1 (broadcast runs root -> root+1 -> ... around the ring in the forward direction,
+// PAPER.md:77 "data always flow in one direction").
+//
+// The rank's kernel is 2 C CTAs: C forward CTAs (channel c takes tiles c, c + C, ...: load my block, wait for the
+// partial, combine in chain order, push up; the last rank stores / turns the finished tile around) and C return CTAs
+// (wait for a finished tile, store it to my vector, push it further down).  No CTA of a rank waits for another CTA of
+// the same rank; a channel advances whenever its CTAs are resident on every rank, and the grid never exceeds what
+// the device holds at once.
+//
+// ONE GPU (this build's box): kernels that wait on each other must not run as separate launches on one device, so
+// lp_chain_emulate runs the SAME per-rank code for all P ranks inside ONE cooperative launch (P x 2 C co-resident
+// CTAs), every "peer" pointer then being a local one.  That is what tests/ compare with the oracle bit for bit; the
+// multi-process plumbing (roles, handle exchange) is covered on the CPU.  Values: the chain order rank 0 -> P-1 (U4),
+// one RN operation per combine -- the same definition as every other LP variant.
+#include <cooperative_groups.h>
+#include <string.h>
+
+#include <mutex>
+#include <vector>
+
+#include "lp_common.cuh"
+
+namespace {
+
+constexpr int kChainThreads = 512;
+constexpr int kFlagStride = 16;           // unsigned long longs between two counters: one 128-byte line each
+constexpr int kFlagsPerChannel = 4 * kFlagStride;
+enum { F_FWD_TAIL = 0, F_BWD_TAIL = kFlagStride, F_UP_CREDIT = 2 * kFlagStride, F_DOWN_CREDIT = 3 * kFlagStride };
+enum { ST_RECV_FWD = 0, ST_SENT_UP = 1, ST_RECV_BWD = 2, ST_SENT_DOWN = 3 };
+
+// What one rank's CTAs need: its vector, its endpoint, its two neighbours' endpoints, its roles in this call.
+struct LpChainRank {
+    float *buf;
+    unsigned long long *flags;   // my counters: [C][kFlagsPerChannel]
+    unsigned long long *state;   // my private sequence numbers: [C][4]
+    float *fwd_ring, *bwd_ring;  // my receive rings: [C][S][tile]
+    unsigned long long *up_flags;    // endpoint of rank (r + 1) mod P
+    float *up_fwd_ring;
+    unsigned long long *down_flags;  // endpoint of rank (r - 1 + P) mod P
+    float *down_bwd_ring;
+    int *error;  // my error word (0 = fine)
+    // forward CTAs
+    unsigned char f_active, f_load, f_recv, f_send_up, f_store, f_send_down;
+    // return CTAs
+    unsigned char r_active, r_store, r_send_down;
+    unsigned char pad[3];
+};
+
+struct LpChainLaunch {
+    LpChainRank rank[LP_MAX_P];  // [0] alone for a real launch (one rank per GPU); all P for the one-GPU emulation
+    lp_partition part;
+    int n_local;  // ranks in this launch
+    int C, S;
+    int code;  // (dtype << 1) | red_op
+    unsigned long long spin_limit;  // polls before a wait gives up and flags an error: a missing peer never hangs the GPU
+};
+
+__device__ __forceinline__ unsigned long long ld_sys(const unsigned long long *p) {
+    unsigned long long v;
+    asm volatile("ld.relaxed.sys.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_sys(unsigned long long *p, unsigned long long v) {
+    asm volatile("st.relaxed.sys.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ void fence_sys() { asm volatile("fence.acq_rel.sys;" ::: "memory"); }
+// ring data is written by another GPU (or another SM): never from L1
+__device__ __forceinline__ float4 ld_ring(const float *p) {
+    float4 v;
+    asm volatile("ld.volatile.global.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ float ld_ring1(const float *p) {
+    float v;
+    asm volatile("ld.volatile.global.f32 %0, [%1];" : "=f"(v) : "l"(p) : "memory");
+    return v;
+}
+
+// Thread 0 polls *flag until it reaches `want`, then everybody passes the barrier.  Returns false (for every thread)
+// when the poll gave up or another CTA of this rank already failed: the caller leaves its loop.
+__device__ __forceinline__ bool wait_counter(const unsigned long long *flag, unsigned long long want, int *error, int *s_ok,
+                                             unsigned long long spin_limit) {
+    if (threadIdx.x == 0) {
+        int ok = 1;
+        unsigned long long spins = 0;
+        while (ld_sys(flag) < want) {
+            if (++spins > spin_limit || ((spins & 0xfffu) == 0 && *reinterpret_cast<volatile int *>(error) != 0)) {
+                ok = 0;
+                atomicCAS(error, 0, 1);
+                break;
+            }
+        }
+        fence_sys();  // acquire: the data published before the counter is visible to loads after the barrier
+        *s_ok = ok;
+    }
+    __syncthreads();
+    const bool ok = *s_ok != 0;
+    __syncthreads();  // s_ok may be rewritten by the next wait
+    return ok;
+}
+
+// After every thread's stores into the neighbour's ring: publish the new sequence number in the neighbour's memory.
+__device__ __forceinline__ void publish(unsigned long long *remote_flag, unsigned long long seq) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        fence_sys();  // release, cumulative over the barrier: the tile is visible before the counter
+        st_sys(remote_flag, seq);
+    }
+}
+// After every thread has CONSUMED the values it loaded from a slot (they went into an add or a store): credit.
+__device__ __forceinline__ void credit(unsigned long long *remote_flag, unsigned long long seq) {
+    __syncthreads();
+    if (threadIdx.x == 0) st_sys(remote_flag, seq);
+}
+
+// The tile as V vectors per thread; `nfull` whole 16-byte vectors, then `rem` (< 4) single elements (last tile only:
+// every tile starts on a 16-byte boundary because the chain rounds blocks up to a multiple of 4 elements).
+template <int V>
+struct TileRegs {
+    float4 v[V];
+};
+
+template <int V>
+__device__ __forceinline__ void load_tile(TileRegs<V> &t, const float *src, uint32_t len, bool ring) {
+    const uint32_t nfull = len >> 2, rem = len & 3u;
+#pragma unroll
+    for (int k = 0; k < V; ++k) {
+        const uint32_t j = threadIdx.x + (uint32_t)k * kChainThreads;
+        if (j < nfull) {
+            t.v[k] = ring ? ld_ring(src + 4 * j) : lp_ldg_stream(src + 4 * j);
+        } else if (j == nfull && rem) {
+            float e[3] = {0.f, 0.f, 0.f};
+            for (uint32_t q = 0; q < rem; ++q) e[q] = ring ? ld_ring1(src + 4 * j + q) : src[4 * j + q];
+            t.v[k] = make_float4(e[0], e[1], e[2], 0.f);
+        }
+    }
+}
+
+template <int V>
+__device__ __forceinline__ void store_tile(const TileRegs<V> &t, float *dst, uint32_t len) {
+    const uint32_t nfull = len >> 2, rem = len & 3u;
+#pragma unroll
+    for (int k = 0; k < V; ++k) {
+        const uint32_t j = threadIdx.x + (uint32_t)k * kChainThreads;
+        if (j < nfull) {
+            lp_stg_stream(dst + 4 * j, t.v[k]);
+        } else if (j == nfull && rem) {
+            const float e[3] = {t.v[k].x, t.v[k].y, t.v[k].z};
+            for (uint32_t q = 0; q < rem; ++q) dst[4 * j + q] = e[q];
+        }
+    }
+}
+
+// Forward CTA of channel c: the reduce half of Fig. 2b (and the whole of a broadcast, Fig. 2a).
+template <int V>
+__device__ void chain_forward(const LpChainRank &A, const LpChainLaunch &L, int c, int *s_ok) {
+    constexpr uint32_t kTile = V * 4 * kChainThreads;
+    unsigned long long *st = A.state + (size_t)c * 4;
+    unsigned long long recv = st[ST_RECV_FWD], sent_up = st[ST_SENT_UP], sent_down = st[ST_SENT_DOWN];
+    unsigned long long *my = A.flags + (size_t)c * kFlagsPerChannel;
+    unsigned long long *up = A.up_flags + (size_t)c * kFlagsPerChannel;
+    unsigned long long *down = A.down_flags + (size_t)c * kFlagsPerChannel;
+    const size_t ring_c = (size_t)c * L.S * kTile;
+    __syncthreads();  // everybody has read the sequence numbers before thread 0 may write them back
+    bool ok = true;
+    for (uint64_t t = (uint64_t)c; ok && t < L.part.n_tiles; t += (uint64_t)L.C) {
+        uint64_t off;
+        uint32_t len;
+        lp_tile_range(L.part, t, off, len);
+        TileRegs<V> acc, mine;
+        if (A.f_load) load_tile<V>(A.f_recv ? mine : acc, A.buf + off, len, false);  // my block: no flag to wait for
+        if (A.f_recv) {  // "GPU1 reduces the received block a0 with a1 to yield a'": partial op mine, in that order
+            ok = wait_counter(my + F_FWD_TAIL, recv + 1, A.error, s_ok, L.spin_limit);
+            if (!ok) break;
+            load_tile<V>(acc, A.fwd_ring + ring_c + (size_t)(recv % (unsigned)L.S) * kTile, len, true);
+            if (A.f_load) lp_fold_vecs<V>(acc.v, mine.v, V, L.code);
+            ++recv;
+        }
+        if (A.f_send_up) {
+            ok = wait_counter(my + F_UP_CREDIT, sent_up + 1 > (unsigned)L.S ? sent_up + 1 - (unsigned)L.S : 0, A.error, s_ok, L.spin_limit);
+            if (!ok) break;
+            store_tile<V>(acc, A.up_fwd_ring + ring_c + (size_t)(sent_up % (unsigned)L.S) * kTile, len);
+            publish(up + F_FWD_TAIL, ++sent_up);
+        }
+        if (A.f_store) store_tile<V>(acc, A.buf + off, len);
+        if (A.f_send_down) {  // the chain's end: the finished tile turns around
+            ok = wait_counter(my + F_DOWN_CREDIT, sent_down + 1 > (unsigned)L.S ? sent_down + 1 - (unsigned)L.S : 0, A.error,
+                              s_ok, L.spin_limit);
+            if (!ok) break;
+            store_tile<V>(acc, A.down_bwd_ring + ring_c + (size_t)(sent_down % (unsigned)L.S) * kTile, len);
+            publish(down + F_BWD_TAIL, ++sent_down);
+        }
+        // the slot's values have been consumed by the stores / the fold above: hand it back to rank r-1
+        if (A.f_recv) credit(down + F_UP_CREDIT, recv);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        st[ST_RECV_FWD] = recv;
+        st[ST_SENT_UP] = sent_up;
+        if (A.f_send_down) st[ST_SENT_DOWN] = sent_down;
+    }
+}
+
+// Return CTA of channel c: the broadcast half of allreduce (and the way a reduced tile reaches a root that is not
+// the chain's end): finished tiles flow rank r+1 -> r.
+template <int V>
+__device__ void chain_return(const LpChainRank &A, const LpChainLaunch &L, int c, int *s_ok) {
+    constexpr uint32_t kTile = V * 4 * kChainThreads;
+    unsigned long long *st = A.state + (size_t)c * 4;
+    unsigned long long recv = st[ST_RECV_BWD], sent_down = st[ST_SENT_DOWN];
+    unsigned long long *my = A.flags + (size_t)c * kFlagsPerChannel;
+    unsigned long long *up = A.up_flags + (size_t)c * kFlagsPerChannel;
+    unsigned long long *down = A.down_flags + (size_t)c * kFlagsPerChannel;
+    const size_t ring_c = (size_t)c * L.S * kTile;
+    __syncthreads();
+    bool ok = true;
+    for (uint64_t t = (uint64_t)c; ok && t < L.part.n_tiles; t += (uint64_t)L.C) {
+        uint64_t off;
+        uint32_t len;
+        lp_tile_range(L.part, t, off, len);
+        TileRegs<V> fin;
+        ok = wait_counter(my + F_BWD_TAIL, recv + 1, A.error, s_ok, L.spin_limit);
+        if (!ok) break;
+        load_tile<V>(fin, A.bwd_ring + ring_c + (size_t)(recv % (unsigned)L.S) * kTile, len, true);
+        ++recv;
+        if (A.r_store) store_tile<V>(fin, A.buf + off, len);
+        if (A.r_send_down) {
+            ok = wait_counter(my + F_DOWN_CREDIT, sent_down + 1 > (unsigned)L.S ? sent_down + 1 - (unsigned)L.S : 0, A.error,
+                              s_ok, L.spin_limit);
+            if (!ok) break;
+            store_tile<V>(fin, A.down_bwd_ring + ring_c + (size_t)(sent_down % (unsigned)L.S) * kTile, len);
+            publish(down + F_BWD_TAIL, ++sent_down);
+        }
+        credit(up + F_DOWN_CREDIT, recv);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        st[ST_RECV_BWD] = recv;
+        if (A.r_send_down) st[ST_SENT_DOWN] = sent_down;
+    }
+}
+
+// grid = n_local x 2 C: CTA b plays local rank b / (2 C); of a rank's 2 C CTAs the first C are forward, the rest return.
+template <int V>
+__global__ void __launch_bounds__(kChainThreads) lp_chain_kernel(const __grid_constant__ LpChainLaunch L) {
+    __shared__ int s_ok;
+    const int per_rank = 2 * L.C;
+    const int lr = (int)blockIdx.x / per_rank;
+    const int j = (int)blockIdx.x - lr * per_rank;
+    const LpChainRank &A = L.rank[lr];
+    if (j < L.C) {
+        if (A.f_active) chain_forward<V>(A, L, j, &s_ok);
+    } else {
+        if (A.r_active) chain_return<V>(A, L, j - L.C, &s_ok);
+    }
+}
+
+}  // namespace
+
+// ---- host side -------------------------------------------------------------------------------------------------
+
+// Roles of `rank` in a collective over P ranks (pure host logic: the part of the multi-process path that needs no GPU).
+extern "C" int lp_chain_plan(int op, int P, int root, int rank, lp_chain_role *out) {
+    if (out == nullptr || P < 1 || P > LP_MAX_P || rank < 0 || rank >= P) return LP_ERR_INVALID_ARG;
+    if (op != LP_OP_BROADCAST && op != LP_OP_REDUCE && op != LP_OP_ALLREDUCE) return LP_ERR_INVALID_ARG;
+    if (op != LP_OP_ALLREDUCE && (root < 0 || root >= P)) return LP_ERR_INVALID_ARG;
+    memset(out, 0, sizeof(*out));
+    out->up = (rank + 1) % P;
+    out->down = (rank + P - 1) % P;
+    if (P == 1) return LP_OK;  // nothing moves
+    if (op == LP_OP_BROADCAST) {  // root -> root+1 -> ... -> root-1 around the ring, forward direction only
+        const int j = (rank - root + P) % P;
+        out->position = j;
+        out->f_active = 1;
+        out->f_load = j == 0;
+        out->f_recv = j > 0;
+        out->f_store = j > 0;
+        out->f_send_up = j < P - 1;
+        return LP_OK;
+    }
+    // reduce / allreduce: the chain is rank 0 -> 1 -> ... -> P-1 whatever the root (U4)
+    const bool all = op == LP_OP_ALLREDUCE;
+    const bool head = rank == P - 1;
+    const int ret_lo = all ? 0 : root;  // the lowest rank a finished tile travels back to
+    out->position = rank;
+    out->f_active = 1;
+    out->f_load = 1;
+    out->f_recv = rank > 0;
+    out->f_send_up = !head;
+    out->f_store = head && (all || root == P - 1);
+    out->f_send_down = head && ret_lo < P - 1;
+    out->r_active = !head && rank >= ret_lo && ret_lo < P - 1;
+    out->r_store = out->r_active && (all || rank == root);
+    out->r_send_down = out->r_active && rank > ret_lo;
+    return LP_OK;
+}
+
+struct lp_chain {
+    int rank, P, C, S, tile;
+    int device;
+    void *base;        // my endpoint (cudaMalloc)
+    size_t bytes;
+    void *peer_up, *peer_down;  // mapped endpoints of the neighbours (== base of another lp_chain in the same process)
+    bool up_ipc, down_ipc;      // opened with cudaIpcOpenMemHandle (to be closed)
+    bool connected;
+};
+
+namespace {
+
+struct EndpointLayout {
+    size_t flags_off, state_off, error_off, fwd_off, bwd_off, bytes;
+};
+EndpointLayout layout_of(int C, int S, int tile) {
+    EndpointLayout l;
+    size_t o = 0;
+    l.flags_off = o;
+    o += (size_t)C * kFlagsPerChannel * sizeof(unsigned long long);
+    l.state_off = o;
+    o += (size_t)C * 4 * sizeof(unsigned long long);
+    l.error_off = o;
+    o += 256;
+    o = (o + 255) & ~(size_t)255;
+    l.fwd_off = o;
+    o += (size_t)C * S * tile * sizeof(float);
+    l.bwd_off = o;
+    o += (size_t)C * S * tile * sizeof(float);
+    l.bytes = o;
+    return l;
+}
+
+void fill_rank(LpChainRank &R, const EndpointLayout &l, float *buf, void *mine, void *up, void *down, const lp_chain_role &role) {
+    memset(&R, 0, sizeof(R));
+    char *m = (char *)mine, *u = (char *)up, *d = (char *)down;
+    R.buf = buf;
+    R.flags = (unsigned long long *)(m + l.flags_off);
+    R.state = (unsigned long long *)(m + l.state_off);
+    R.error = (int *)(m + l.error_off);
+    R.fwd_ring = (float *)(m + l.fwd_off);
+    R.bwd_ring = (float *)(m + l.bwd_off);
+    R.up_flags = (unsigned long long *)(u + l.flags_off);
+    R.up_fwd_ring = (float *)(u + l.fwd_off);
+    R.down_flags = (unsigned long long *)(d + l.flags_off);
+    R.down_bwd_ring = (float *)(d + l.bwd_off);
+    R.f_active = role.f_active;
+    R.f_load = role.f_load;
+    R.f_recv = role.f_recv;
+    R.f_send_up = role.f_send_up;
+    R.f_store = role.f_store;
+    R.f_send_down = role.f_send_down;
+    R.r_active = role.r_active;
+    R.r_store = role.r_store;
+    R.r_send_down = role.r_send_down;
+}
+
+// CTAs of the chain kernel the current device holds at once
+template <int V>
+cudaError_t resident_t(int *ctas) {
+    int per_sm = 0, dev = 0, sms = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, lp_chain_kernel<V>, kChainThreads, 0);
+    *ctas = per_sm * sms;
+    return e;
+}
+cudaError_t resident(int tile, int *ctas) {
+    switch (tile) {
+        case 4096: return resident_t<2>(ctas);
+        case 8192: return resident_t<4>(ctas);
+        default: return resident_t<8>(ctas);
+    }
+}
+
+template <int V>
+cudaError_t launch_t(const LpChainLaunch &L, bool cooperative, cudaStream_t stream) {
+    const unsigned grid = (unsigned)(L.n_local * 2 * L.C);
+    int cap = 0;
+    cudaError_t e = resident_t<V>(&cap);
+    if (e != cudaSuccess) return e;
+    if ((unsigned)cap < grid) return cudaErrorCooperativeLaunchTooLarge;  // every CTA must be resident
+    cudaLaunchConfig_t lc;
+    memset(&lc, 0, sizeof(lc));
+    lc.gridDim = dim3(grid);
+    lc.blockDim = dim3(kChainThreads);
+    lc.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeCooperative;
+    attr[0].val.cooperative = 1;
+    lc.attrs = attr;
+    lc.numAttrs = cooperative ? 1 : 0;
+    lp_count_launch(1);
+    lp_chain_reset(stream);
+    return cudaLaunchKernelEx(&lc, lp_chain_kernel<V>, L);
+}
+
+cudaError_t launch(const LpChainLaunch &L, int tile, bool cooperative, cudaStream_t stream) {
+    switch (tile) {
+        case 4096: return launch_t<2>(L, cooperative, stream);
+        case 8192: return launch_t<4>(L, cooperative, stream);
+        case 16384: return launch_t<8>(L, cooperative, stream);
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+// a1 for the chain: blocks of `block` elements rounded up to a multiple of 4 (every tile then starts on a 16-byte
+// boundary; results never depend on the block), cut into tiles of one ring slot.
+lp_partition chain_partition(size_t n, size_t block, int tile) {
+    if (block == 0) block = LP_CHAIN_DEFAULT_TILE;
+    if (block < ~(size_t)3) block = (block + 3) & ~(size_t)3;
+    return lp_make_partition(n, block, (uint32_t)tile);
+}
+
+bool valid_geometry(int C, int S, int tile) {
+    return C >= 1 && C <= LP_CHAIN_MAX_CHANNELS && S >= 1 && S <= 64 && (tile == 4096 || tile == 8192 || tile == 16384);
+}
+
+int chain_fail(cudaError_t e) {
+    cudaGetLastError();
+    return e == cudaErrorCooperativeLaunchTooLarge ? LP_ERR_UNSUPPORTED : LP_ERR_CUDA;
+}
+
+// emulation endpoints: (geometry, P) -> one allocation holding P endpoints, kept for the life of the library binding
+struct EmulEndpoints {
+    int P, C, S, tile;
+    void *base;
+};
+std::mutex g_emul_mu;
+std::vector<EmulEndpoints> g_emul;
+
+}  // namespace
+
+void lp_chain_shutdown() {
+    std::lock_guard<std::mutex> lock(g_emul_mu);
+    for (auto &e : g_emul) cudaFree(e.base);
+    g_emul.clear();
+}
+
+extern "C" {
+
+size_t lp_chain_endpoint_bytes(int channels, int slots, int tile) {
+    return valid_geometry(channels, slots, tile) ? layout_of(channels, slots, tile).bytes : 0;
+}
+
+int lp_chain_create(int rank, int P, int channels, int slots, int tile, lp_chain **out) {
+    if (out == nullptr) return LP_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (channels == 0) channels = LP_CHAIN_DEFAULT_CHANNELS;
+    if (slots == 0) slots = LP_CHAIN_DEFAULT_SLOTS;
+    if (tile == 0) tile = LP_CHAIN_DEFAULT_TILE;
+    if (P < 1 || P > LP_MAX_P || rank < 0 || rank >= P || !valid_geometry(channels, slots, tile)) return LP_ERR_INVALID_ARG;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) {
+        cudaGetLastError();
+        return LP_ERR_CUDA;
+    }
+    lp_chain *ch = new lp_chain;
+    memset(ch, 0, sizeof(*ch));
+    ch->rank = rank;
+    ch->P = P;
+    ch->C = channels;
+    ch->S = slots;
+    ch->tile = tile;
+    ch->device = dev;
+    ch->bytes = layout_of(channels, slots, tile).bytes;
+    cudaError_t e = cudaMalloc(&ch->base, ch->bytes);
+    if (e == cudaSuccess) e = cudaMemset(ch->base, 0, ch->bytes);
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    if (e != cudaSuccess) {
+        if (ch->base) cudaFree(ch->base);
+        delete ch;
+        return chain_fail(e);
+    }
+    *out = ch;
+    return LP_OK;
+}
+
+int lp_chain_get_handle(lp_chain *ch, void *handle_out) {
+    if (ch == nullptr || handle_out == nullptr) return LP_ERR_INVALID_ARG;
+    static_assert(sizeof(cudaIpcMemHandle_t) == LP_CHAIN_HANDLE_BYTES, "handle size");
+    cudaIpcMemHandle_t h;
+    const cudaError_t e = cudaIpcGetMemHandle(&h, ch->base);
+    if (e != cudaSuccess) return chain_fail(e);
+    memcpy(handle_out, &h, sizeof(h));
+    return LP_OK;
+}
+
+// handles: P x LP_CHAIN_HANDLE_BYTES, rank order (what an all-gather of lp_chain_get_handle leaves on every rank).
+int lp_chain_connect(lp_chain *ch, const void *handles) {
+    if (ch == nullptr || handles == nullptr || ch->connected) return LP_ERR_INVALID_ARG;
+    const int up = (ch->rank + 1) % ch->P, down = (ch->rank + ch->P - 1) % ch->P;
+    auto open = [&](int peer, void **ptr, bool *ipc) -> cudaError_t {
+        if (peer == ch->rank) {
+            *ptr = ch->base;
+            *ipc = false;
+            return cudaSuccess;
+        }
+        cudaIpcMemHandle_t h;
+        memcpy(&h, (const char *)handles + (size_t)peer * LP_CHAIN_HANDLE_BYTES, sizeof(h));
+        *ipc = true;
+        return cudaIpcOpenMemHandle(ptr, h, cudaIpcMemLazyEnablePeerAccess);
+    };
+    cudaError_t e = open(up, &ch->peer_up, &ch->up_ipc);
+    if (e != cudaSuccess) return chain_fail(e);
+    if (down == up) {
+        ch->peer_down = ch->peer_up;
+        ch->down_ipc = false;
+    } else {
+        e = open(down, &ch->peer_down, &ch->down_ipc);
+        if (e != cudaSuccess) {
+            if (ch->up_ipc) cudaIpcCloseMemHandle(ch->peer_up);
+            return chain_fail(e);
+        }
+    }
+    ch->connected = true;
+    return LP_OK;
+}
+
+// The same with raw device pointers: endpoints of other lp_chain objects of THIS process (one process driving several
+// GPUs with peer access enabled by the caller).
+int lp_chain_connect_ptrs(lp_chain *ch, void *up_endpoint, void *down_endpoint) {
+    if (ch == nullptr || up_endpoint == nullptr || down_endpoint == nullptr || ch->connected) return LP_ERR_INVALID_ARG;
+    ch->peer_up = up_endpoint;
+    ch->peer_down = down_endpoint;
+    ch->up_ipc = ch->down_ipc = false;
+    ch->connected = true;
+    return LP_OK;
+}
+
+void *lp_chain_endpoint(lp_chain *ch) { return ch ? ch->base : nullptr; }
+
+int lp_chain_destroy(lp_chain *ch) {
+    if (ch == nullptr) return LP_ERR_INVALID_ARG;
+    cudaDeviceSynchronize();
+    if (ch->connected) {
+        if (ch->up_ipc) cudaIpcCloseMemHandle(ch->peer_up);
+        if (ch->down_ipc) cudaIpcCloseMemHandle(ch->peer_down);
+    }
+    cudaFree(ch->base);
+    cudaGetLastError();
+    delete ch;
+    return LP_OK;
+}
+
+// One rank's share of the collective: every rank of the chain calls this with the same (op, n, block, root, reduce_op),
+// in the same order as its other chain collectives.
+int lp_chain_run(lp_chain *ch, int op, float *buf, size_t n, size_t block, int root, int reduce_op, void *cuda_stream) {
+    if (ch == nullptr || !ch->connected) return LP_ERR_INVALID_ARG;
+    if (reduce_op != LP_REDUCE_SUM && reduce_op != LP_REDUCE_PROD) return LP_ERR_INVALID_ARG;
+    if (op == LP_OP_ALLREDUCE) root = 0;
+    lp_chain_role role;
+    int rc = lp_chain_plan(op, ch->P, root, ch->rank, &role);
+    if (rc != LP_OK) return rc;
+    if (buf == nullptr || ((uintptr_t)buf & 15u)) return LP_ERR_INVALID_ARG;
+    if (n == 0 || ch->P == 1) return LP_OK;
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != ch->device) {
+        cudaGetLastError();
+        return LP_ERR_UNSUPPORTED;
+    }
+    LpChainLaunch L;
+    memset(&L, 0, sizeof(L));
+    L.n_local = 1;
+    L.C = ch->C;
+    L.S = ch->S;
+    L.code = reduce_op;  // fp32
+    L.spin_limit = 1ull << 28;  // ~a minute of polling: ranks of different processes start at different times
+    L.part = chain_partition(n, block, ch->tile);
+    fill_rank(L.rank[0], layout_of(ch->C, ch->S, ch->tile), buf, ch->base, ch->peer_up, ch->peer_down, role);
+    const cudaError_t e = launch(L, ch->tile, false, (cudaStream_t)cuda_stream);
+    return e == cudaSuccess ? LP_OK : chain_fail(e);
+}
+
+// 0 = no wait of this endpoint's kernels has given up so far (a peer that never arrived); synchronises the device.
+int lp_chain_error(lp_chain *ch, int *error_out) {
+    if (ch == nullptr || error_out == nullptr) return LP_ERR_INVALID_ARG;
+    cudaError_t e = cudaDeviceSynchronize();
+    if (e == cudaSuccess)
+        e = cudaMemcpy(error_out, (char *)ch->base + layout_of(ch->C, ch->S, ch->tile).error_off, sizeof(int), cudaMemcpyDeviceToHost);
+    return e == cudaSuccess ? LP_OK : chain_fail(e);
+}
+
+// Channels per rank the emulation takes by default: LP_CHAIN_EMULATE_CHANNELS, fewer when P x 2 x channels CTAs would
+// not all be resident on the current device (1 without a device).
+int lp_chain_emulate_channels(int P, int tile) {
+    if (tile == 0) tile = LP_CHAIN_DEFAULT_TILE;
+    if (P < 1 || P > LP_MAX_P || !valid_geometry(1, 1, tile)) return 0;
+    int cap = 0;
+    if (resident(tile, &cap) != cudaSuccess) {
+        cudaGetLastError();
+        return 1;
+    }
+    int c = cap / (2 * P);
+    if (c > LP_CHAIN_EMULATE_CHANNELS) c = LP_CHAIN_EMULATE_CHANNELS;
+    return c < 1 ? 1 : c;
+}
+
+// All P ranks of the chain on ONE device, in one cooperative launch: P x 2 x channels co-resident CTAs run the per-rank
+// code above against P endpoints in this device's memory.
+int lp_chain_emulate(int op, float *const *bufs, int P, size_t n, size_t block, int root, int reduce_op, int channels,
+                     int slots, int tile, void *cuda_stream) {
+    if (slots == 0) slots = LP_CHAIN_DEFAULT_SLOTS;
+    if (tile == 0) tile = LP_CHAIN_DEFAULT_TILE;
+    if (channels == 0) channels = lp_chain_emulate_channels(P, tile);
+    if (bufs == nullptr || P < 1 || P > LP_MAX_P || !valid_geometry(channels, slots, tile)) return LP_ERR_INVALID_ARG;
+    if (reduce_op != LP_REDUCE_SUM && reduce_op != LP_REDUCE_PROD) return LP_ERR_INVALID_ARG;
+    if (op == LP_OP_ALLREDUCE) root = 0;
+    lp_chain_role roles[LP_MAX_P];
+    for (int r = 0; r < P; ++r) {
+        const int rc = lp_chain_plan(op, P, root, r, &roles[r]);
+        if (rc != LP_OK) return rc;
+    }
+    const size_t bytes = n * sizeof(float);
+    for (int r = 0; r < P; ++r) {
+        if (bufs[r] == nullptr || ((uintptr_t)bufs[r] & 15u)) return LP_ERR_INVALID_ARG;
+        for (int q = 0; q < r; ++q) {
+            const uintptr_t a = (uintptr_t)bufs[r], b = (uintptr_t)bufs[q];
+            if (bytes && a < b + bytes && b < a + bytes) return LP_ERR_INVALID_ARG;
+        }
+    }
+    if (n == 0 || P == 1) return LP_OK;
+    const EndpointLayout l = layout_of(channels, slots, tile);
+    void *base = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(g_emul_mu);
+        for (auto &e : g_emul)
+            if (e.P == P && e.C == channels && e.S == slots && e.tile == tile) base = e.base;
+        if (base == nullptr) {
+            cudaError_t e = cudaMalloc(&base, l.bytes * (size_t)P);
+            if (e == cudaSuccess) e = cudaMemset(base, 0, l.bytes * (size_t)P);
+            if (e == cudaSuccess) e = cudaDeviceSynchronize();
+            if (e != cudaSuccess) {
+                if (base) cudaFree(base);
+                return chain_fail(e);
+            }
+            g_emul.push_back(EmulEndpoints{P, channels, slots, tile, base});
+        }
+    }
+    LpChainLaunch L;
+    memset(&L, 0, sizeof(L));
+    L.n_local = P;
+    L.C = channels;
+    L.S = slots;
+    L.code = reduce_op;
+    L.spin_limit = 1ull << 23;  // all ranks start together here: a few seconds mean a bug
+    L.part = chain_partition(n, block, tile);
+    for (int r = 0; r < P; ++r) {
+        char *b = (char *)base;
+        fill_rank(L.rank[r], l, bufs[r], b + l.bytes * (size_t)r, b + l.bytes * (size_t)roles[r].up,
+                  b + l.bytes * (size_t)roles[r].down, roles[r]);
+    }
+    const cudaError_t e = launch(L, tile, true, (cudaStream_t)cuda_stream);
+    return e == cudaSuccess ? LP_OK : chain_fail(e);
+}
+
+// error word of emulated rank `rank` for the geometry (P, channels, slots, tile); synchronises the device
+int lp_chain_emulate_error(int P, int channels, int slots, int tile, int *error_out) {
+    if (slots == 0) slots = LP_CHAIN_DEFAULT_SLOTS;
+    if (tile == 0) tile = LP_CHAIN_DEFAULT_TILE;
+    if (channels == 0) channels = lp_chain_emulate_channels(P, tile);
+    if (error_out == nullptr || !valid_geometry(channels, slots, tile)) return LP_ERR_INVALID_ARG;
+    *error_out = 0;
+    void *base = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(g_emul_mu);
+        for (auto &e : g_emul)
+            if (e.P == P && e.C == channels && e.S == slots && e.tile == tile) base = e.base;
+    }
+    if (base == nullptr) return LP_OK;
+    cudaError_t e = cudaDeviceSynchronize();
+    const EndpointLayout l = layout_of(channels, slots, tile);
+    for (int r = 0; r < P && e == cudaSuccess; ++r) {
+        int w = 0;
+        e = cudaMemcpy(&w, (char *)base + l.bytes * (size_t)r + l.error_off, sizeof(int), cudaMemcpyDeviceToHost);
+        if (w) *error_out = w;
+    }
+    return e == cudaSuccess ? LP_OK : chain_fail(e);
+}
+
+}  // extern "C"

@@ -1,0 +1,153 @@
+"""GPU parity of the multi-GPU chain's device code (csrc/lp_chain.cu) against the oracle.  The box
+has one GPU and kernels that wait on each other may not run there as separate launches, so the P ranks run as ONE
+cooperative launch (lp_chain_emulate: the same per-rank code, P endpoints in one device's memory).  Bit-exact: the
+chain folds in rank order 0 -> P-1 whatever the root (U4), one RN operation per combine.  Every test is marked gpu.
+"""
+import numpy as np
+import pytest
+
+from paper_1611_04255_b200 import inputs
+from paper_1611_04255_b200 import binding as lp
+
+pytestmark = pytest.mark.gpu
+torch = pytest.importorskip("torch")
+
+OPS = {"broadcast": lp.OP_BROADCAST, "reduce": lp.OP_REDUCE, "allreduce": lp.OP_ALLREDUCE}
+
+
+@pytest.fixture(autouse=True)
+def _device():
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    lp.lib()
+    yield
+    torch.cuda.synchronize()
+
+
+def up(arrs):
+    return [torch.from_numpy(a).cuda() for a in arrs]
+
+
+def down(tensors):
+    torch.cuda.synchronize()
+    return [t.cpu().numpy() for t in tensors]
+
+
+def run_oracle(oracle, op, host, root, red):
+    if op == "allreduce":
+        oracle.allreduce_op(host, red)
+    elif op == "reduce":
+        oracle.reduce_op(host, red, root=root)
+    else:
+        oracle.broadcast(host, root=root)
+
+
+def check(oracle, P, n, block, op, root=0, red=lp.REDUCE_SUM, kind="uniform", **geom):
+    src = inputs.rank_vectors([31, n, P], P, n, kind)
+    want = [a.copy() for a in src]
+    run_oracle(oracle, op, want, root, red)
+    dev = up(src)
+    lp.lp_chain_emulate(OPS[op], dev, block=block, root=root, reduce_op=red, **geom)
+    got = down(dev)
+    assert lp.lp_chain_emulate_error(P, **geom) == 0, "a wait of the chain gave up"
+    for r in range(P):
+        assert got[r].tobytes() == want[r].tobytes(), (op, P, n, block, root, red, geom, r)
+
+
+SHAPES = [
+    # P, n, block
+    (1, 1000, 64), (2, 1, 1), (2, 3, 64), (2, 5, 4), (3, 1001, 100), (3, 4097, 1000), (4, 70_001, 4096),
+    (5, 300_003, 65_536), (6, 70_001, 1001), (7, 12_345, 333), (8, 262_147, 16_384), (16, 100_003, 8192),
+    (32, 20_001, 5000), (4, 16384 * 3 + 5, 16384), (6, 1 << 20, 1 << 22),
+]
+
+
+@pytest.mark.parametrize("op", ["allreduce", "reduce", "broadcast"])
+@pytest.mark.parametrize("P,n,block", SHAPES)
+def test_chain_ragged_shapes_bit_exact(oracle, op, P, n, block):
+    check(oracle, P, n, block, op, root=P // 2)
+
+
+@pytest.mark.parametrize("op", ["reduce", "broadcast"])
+def test_chain_every_root(oracle, op):
+    for P in (2, 3, 5):
+        for root in range(P):
+            check(oracle, P, 50_001, 4096, op, root=root)
+
+
+@pytest.mark.parametrize("tile", [4096, 8192, 16384])
+@pytest.mark.parametrize("slots", [1, 2, 8])
+def test_chain_ring_geometry_and_back_pressure(oracle, tile, slots):
+    """Few channels and shallow rings: every slot is reused hundreds of times, so credits and sequence numbers wrap
+    the ring over and over (a one-slot ring is pure stop-and-wait)."""
+    for op in ("allreduce", "reduce", "broadcast"):
+        check(oracle, 6, 1_500_003, 65_536, op, root=2, channels=2, slots=slots, tile=tile)
+
+
+def test_chain_product(oracle):
+    src = inputs.typed_rank_vectors([32, 0], 6, 200_001, inputs.DT_F32, "prod")
+    want = [a.copy() for a in src]
+    oracle.allreduce_op(want, oracle.RED_PROD)
+    dev = up(src)
+    lp.lp_chain_emulate(lp.OP_ALLREDUCE, dev, block=8192, reduce_op=lp.REDUCE_PROD)
+    got = down(dev)
+    assert all(g.tobytes() == w.tobytes() for g, w in zip(got, want))
+
+
+def test_chain_back_to_back_collectives_share_the_rings(oracle):
+    """Counters only grow: a sequence of different collectives (different roots, so different senders into the same
+    rings) on one stream, no reset in between."""
+    P, n = 4, 300_007
+    src = inputs.rank_vectors([33, 0], P, n, "uniform")
+    host = [a.copy() for a in src]
+    dev = up(src)
+    seq = [("allreduce", 0), ("broadcast", 2), ("reduce", 1), ("broadcast", 0), ("allreduce", 0), ("reduce", 3),
+           ("broadcast", 3), ("reduce", 0)] * 3
+    for op, root in seq:
+        run_oracle(oracle, op, host, root, oracle.RED_SUM)
+        lp.lp_chain_emulate(OPS[op], dev, block=16_384, root=root)
+    got = down(dev)
+    assert lp.lp_chain_emulate_error(P) == 0
+    for r in range(P):
+        assert got[r].tobytes() == host[r].tobytes(), r
+
+
+def test_chain_large_message(oracle):
+    P, n = 4, (64 << 20) // 4 + 3          # 64 MB per rank: ~1000 tiles per rank, 8 channels
+    src = inputs.rank_vectors([34, 0], P, n, "normal", 1e-3)
+    want = [a.copy() for a in src]
+    oracle.allreduce(want, omp=True)
+    dev = up(src)
+    lp.lp_chain_emulate(lp.OP_ALLREDUCE, dev, block=65_536)
+    got = down(dev)
+    assert lp.lp_chain_emulate_error(P) == 0
+    for r in range(P):
+        assert got[r].tobytes() == want[r].tobytes(), r
+
+
+def test_chain_argument_errors():
+    dev = [torch.zeros(64, device="cuda") for _ in range(2)]
+    arr, n = lp._dev_ptrs(dev)
+    L = lp.lib()
+    s = lp._stream_ptr(None)
+    assert L.lp_chain_emulate(lp.OP_ALLREDUCE, arr, 2, n, 16, 0, 7, 0, 0, 0, s) == lp.LP_ERR_INVALID_ARG   # operator
+    assert L.lp_chain_emulate(lp.OP_REDUCE, arr, 2, n, 16, 2, 0, 0, 0, 0, s) == lp.LP_ERR_INVALID_ARG      # root
+    assert L.lp_chain_emulate(lp.OP_BSP_SGD, arr, 2, n, 16, 0, 0, 0, 0, 0, s) == lp.LP_ERR_INVALID_ARG     # collective
+    assert L.lp_chain_emulate(lp.OP_ALLREDUCE, arr, 2, n, 16, 0, 0, 0, 0, 1000, s) == lp.LP_ERR_INVALID_ARG  # tile
+    assert L.lp_chain_emulate(lp.OP_ALLREDUCE, arr, 2, n, 16, 0, 0, 64, 0, 0, s) == lp.LP_ERR_UNSUPPORTED   # 256 CTAs of 94 regs
+    assert L.lp_chain_emulate(lp.OP_ALLREDUCE, arr, 2, 0, 16, 0, 0, 0, 0, 0, s) == lp.LP_OK                 # n == 0
+
+
+def test_chain_endpoint_of_one_rank(oracle):
+    """The real entry points on the one GPU there is: create / handle / connect-to-self / run with P = 1 (a no-op by
+    definition), and a P = 2 endpoint refuses to run before it is connected."""
+    ch = lp.Chain(0, 1)
+    assert len(ch.handle()) == lp.CHAIN_HANDLE_BYTES and ch.endpoint() != 0
+    ch.connect([ch.handle()])
+    x = torch.arange(1000, dtype=torch.float32, device="cuda")
+    ch.run(lp.OP_ALLREDUCE, x)
+    assert ch.error() == 0 and torch.equal(x.cpu(), torch.arange(1000, dtype=torch.float32))
+    ch.destroy()
+    ch2 = lp.Chain(1, 2, channels=2, slots=2, tile=4096)
+    with pytest.raises(lp.LpError):
+        ch2.run(lp.OP_ALLREDUCE, x)
+    ch2.destroy()
