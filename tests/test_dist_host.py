@@ -49,6 +49,97 @@ def test_gloo_world2_max_and_sum_over_ranks():
     assert got == [(0, 11.0, 300.0), (1, 11.0, 300.0)]
 
 
+class _FakeEndpoint:
+    """Stand-in for binding.Chain on the CPU box (no CUDA IPC there): its handle is 64 bytes that name its rank."""
+    def __init__(self, rank, P, channels, slots, tile):
+        self.rank, self.P, self.connected = rank, P, None
+
+    def handle(self):
+        return bytes([self.rank]) * 64
+
+    def connect(self, handles):
+        self.connected = list(handles)
+
+    def destroy(self):
+        pass
+
+
+def _chain_worker(rank, world, port, q):
+    """One rank of the chain with gloo as the link: the per-rank steps csrc/lp_chain.cu takes (lp_chain_plan's roles),
+    one message per tile and ring, fp32 numpy adds -- the multi-process path of the chain on the CPU."""
+    os.environ.update(RANK=str(rank), WORLD_SIZE=str(world), LOCAL_RANK=str(rank), MASTER_ADDR="127.0.0.1",
+                      MASTER_PORT=str(port))
+    sys.path.insert(0, ROOT)
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_1611_04255_b200 import binding as lp
+    from paper_1611_04255_b200 import chain, inputs
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    grp = chain.ChainGroup(endpoint_factory=_FakeEndpoint)
+    ok_handles = grp.endpoint.connected == [bytes([r]) * 64 for r in range(world)]
+    n, tile = 10_003, 4096
+    results = {}
+    for op, root in ((lp.OP_ALLREDUCE, 0), (lp.OP_REDUCE, 0), (lp.OP_REDUCE, 1), (lp.OP_BROADCAST, 1)):
+        ro = grp.role(op, root)
+        x = inputs.uniform([41, 0], rank, n).copy()
+        for off in range(0, n, tile):                      # tiles in order, one channel
+            sl = slice(off, min(off + tile, n))
+            if ro["f_active"]:
+                v = x[sl].copy() if ro["f_load"] else None
+                if ro["f_recv"]:
+                    t = torch.empty(sl.stop - sl.start, dtype=torch.float32)
+                    dist.recv(t, src=ro["down"])
+                    v = (t.numpy() + v) if ro["f_load"] else t.numpy().copy()     # partial + mine, fp32 RN
+                if ro["f_send_up"]:
+                    dist.send(torch.from_numpy(v.copy()), dst=ro["up"])
+                if ro["f_store"]:
+                    x[sl] = v
+                if ro["f_send_down"]:
+                    dist.send(torch.from_numpy(v.copy()), dst=ro["down"])
+            if ro["r_active"]:
+                t = torch.empty(sl.stop - sl.start, dtype=torch.float32)
+                dist.recv(t, src=ro["up"])
+                if ro["r_store"]:
+                    x[sl] = t.numpy()
+                if ro["r_send_down"]:
+                    dist.send(t, dst=ro["down"])
+        results[(op, root)] = x.tobytes()
+    dist.barrier()
+    dist.destroy_process_group()
+    q.put((rank, ok_handles, results))
+
+
+def test_gloo_world2_chain_handles_and_roles(oracle):
+    import numpy as np
+    from paper_1611_04255_b200 import binding as lp
+    from paper_1611_04255_b200 import inputs
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_chain_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    got = sorted((q.get(timeout=180) for _ in procs), key=lambda t: t[0])
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert all(ok for _, ok, _ in got), "every rank must see every rank's handle, in rank order"
+    n = 10_003
+    src = [inputs.uniform([41, 0], r, n) for r in range(2)]
+    for (op, root), name in (((lp.OP_ALLREDUCE, 0), "allreduce"), ((lp.OP_REDUCE, 0), "reduce"),
+                             ((lp.OP_REDUCE, 1), "reduce"), ((lp.OP_BROADCAST, 1), "broadcast")):
+        want = [a.copy() for a in src]
+        if name == "allreduce":
+            oracle.allreduce(want)
+        elif name == "reduce":
+            oracle.reduce(want, root=root)
+        else:
+            oracle.broadcast(want, root=root)
+        for r in range(2):
+            assert got[r][2][(op, root)] == want[r].tobytes(), (name, root, r)
+
+
 def test_reference_arm_under_torchrun_prints_once():
     # --impl reference with N = 2: rank 0 alone runs the oracle and prints the line, rank 1 exits 0 silently
     port = _free_port()
