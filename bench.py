@@ -51,7 +51,7 @@ def parse_args():
     ap.add_argument("--block", type=int, default=0, help="LP block in elements (0 = the config's)")
     ap.add_argument("--variant", default="auto", choices=["auto", "pipeline", "direct", "cluster", "copy_engine"])
     ap.add_argument("--no-detail", action="store_true", help="skip the secondary measurements")
-    ap.add_argument("--detail", default="configs1,configs2,configs4,sweep,ceilings",
+    ap.add_argument("--detail", default="configs1,configs2,configs4,sweep,ceilings,dtypes,chain",
                     help="comma list of detail sections to run")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
@@ -385,6 +385,10 @@ def run_ours(args, c, rank, world, local):
             detail["sweep"] = sweep_cfg3(torch, lp, dev, peak)
         if "ceilings" in want:
             detail["ceilings"] = ceilings(torch, lp, dev, peak)
+        if "dtypes" in want:
+            detail["dtypes"] = dtype_rows(torch, lp, dev)
+        if "chain" in want:
+            detail["chain"] = chain_rows(torch, lp, dev)
 
     cpu = None
     if rank == 0 and not args.no_cpu:
@@ -684,6 +688,74 @@ def ceilings(torch, lp, dev, peak):
     out["torch_fill_write_only"] = t(lambda: bufs[0].fill_(1.0), n * 4)
     out["measured_peaks_json_hbm_gbs"] = peak
     out["unit"] = "GB/s"
+    return out
+
+
+def dtype_rows(torch, lp, dev, P=6, msg_bytes=256 << 20):
+    """SURVEY 8(f)-4 'dtypes': the typed collectives (lp_*_dt, reading U21) on messages of the SAME BYTES per rank in
+    every element type -- the path is HBM-bound, so the element type should not change the time.  Same graph timing as
+    the sweep; >= 1 GB of rotating buffer sets."""
+    types = (("f32", lp.DT_F32, torch.float32), ("f16", lp.DT_F16, torch.float16), ("bf16", lp.DT_BF16, torch.bfloat16),
+             ("f64", lp.DT_F64, torch.float64))
+    n_sets = max(2, -(-(8 * L2_BYTES) // (P * msg_bytes)))
+    out = {"P": P, "msg_MB": msg_bytes / 2 ** 20, "rotating_sets": n_sets,
+           "what": "us per call and GB/s on the op's minimum bytes (allreduce 2 P bytes, reduce (P+1) bytes, broadcast P bytes)"}
+    raw = [[torch.empty(msg_bytes, dtype=torch.uint8, device=dev) for _ in range(P)] for _ in range(n_sets)]
+    for name, dt, tdt in types:
+        sets = [[b.view(tdt) for b in s] for s in raw]
+        n = sets[0][0].numel()
+
+        def restore():
+            for s in sets:
+                for r, b in enumerate(s):
+                    b.fill_(0.001 * (r + 1))   # repeated in-place sums may reach inf in the 16-bit types: same cost
+
+        row = {"n_elements": n}
+        for op, mult in (("allreduce", 2 * P), ("reduce", P + 1), ("broadcast", P)):
+            if op == "allreduce":
+                fn = lambda s, dt=dt: lp.lp_allreduce_dt(sets[s], 65_536, dtype=dt)
+            elif op == "reduce":
+                fn = lambda s, dt=dt: lp.lp_reduce_dt(sets[s], 65_536, root=0, dtype=dt)
+            else:
+                fn = lambda s, dt=dt: lp.lp_broadcast_dt(sets[s], 65_536, root=0, dtype=dt)
+            us, _ = graph_time(torch, fn, n_sets, restore, mult * msg_bytes)
+            gbs = mult * msg_bytes / us / 1e3
+            row[op] = {"us": round(us, 2), "hbm_GBps_min_bytes": round(gbs, 1), "frac_of_8TBs": round(gbs / 8000.0, 4)}
+        out[name] = row
+    return out
+
+
+def chain_rows(torch, lp, dev, msg_bytes=64 << 20):
+    """the one-rank-per-GPU chain (csrc/lp_chain.cu) as far as ONE GPU can run it -- all P ranks in
+    one cooperative launch (lp_chain_emulate), every 'link' being this GPU's own HBM.  So this measures the PROTOCOL
+    (push + publish + credit per 256 KB tile), not NVLink: per_link_GBps = message bytes / time is what every emulated link
+    direction carried; hbm_GBps counts what the emulation really moves, (6P-4) n 4 bytes for an allreduce (P loads, P stores
+    and 2(P-1) ring writes + reads), (3P-2) n 4 for a broadcast.  Eager launches, K back to back between two events."""
+    n = msg_bytes // 4
+    out = {"msg_MB": msg_bytes / 2 ** 20, "tile_elems": 65_536, "slots": 8,
+           "what": "us per call, GB/s per emulated link direction, HBM GB/s of the emulation; NOT an NVLink measurement"}
+    for P in (2, 4, 8):
+        bufs = [torch.full((n,), 0.001 * (r + 1), device=dev) for r in range(P)]
+        row = {"channels": lp.lp_chain_emulate_channels(P)}
+        for op, op_id, moved in (("allreduce", lp.OP_ALLREDUCE, 6 * P - 4), ("broadcast", lp.OP_BROADCAST, 3 * P - 2)):
+            for _ in range(2):
+                lp.lp_chain_emulate(op_id, bufs, block=65_536)
+            torch.cuda.synchronize()
+            K = 10
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(K):
+                lp.lp_chain_emulate(op_id, bufs, block=65_536)
+            e1.record()
+            torch.cuda.synchronize()
+            us = e0.elapsed_time(e1) * 1e3 / K
+            row[op] = {"us": round(us, 1), "per_link_GBps": round(msg_bytes / us / 1e3, 1),
+                       "hbm_GBps": round(moved * msg_bytes / us / 1e3, 1)}
+            for r, b in enumerate(bufs):
+                b.fill_(0.001 * (r + 1))
+        row["error"] = lp.lp_chain_emulate_error(P)
+        out[f"P{P}"] = row
+        del bufs
     return out
 
 

@@ -288,8 +288,10 @@ LP_API int lp_be_allreduce_op(float *const *bufs, int P, size_t n, int reduce_op
  * receiver's memory; slots returned by a credit counter in the sender's memory; csrc/lp_chain.cu).
  *   lp_chain_create(rank, P, channels, slots, tile, &ch)   on the rank's device (current device); 0 = defaults.  Every
  *       rank must pass the same (P, channels, slots, tile).  channels: 1..LP_CHAIN_MAX_CHANNELS concurrent rings (2 CTAs
- *       of 512 threads each); slots: ring depth 1..64; tile: 4096 / 8192 / 16384 elements per slot (16384 floats =
- *       64 KB = the paper's block).
+ *       of 1024 threads each: an SM moves ~45 GB/s and a block costs three to four memory accesses on its way through a
+ *       rank, so filling a 900 GB/s NVLink direction takes ~60 forward and ~60 return SMs -- hence 64); slots: ring depth
+ *       1..64; tile: elements per slot = the unit of a flag exchange, a power of two from 4096 to 262144 (default 65536
+ *       floats = 256 KB = the LP block of BASELINE.json's configs; 16384 = the paper's 64 KB).
  *   lp_chain_get_handle(ch, h)     LP_CHAIN_HANDLE_BYTES opaque bytes (a CUDA IPC handle) to all-gather over any
  *       transport (paper_1611_04255_b200/chain.py uses torch.distributed);
  *   lp_chain_connect(ch, handles)  handles = P x LP_CHAIN_HANDLE_BYTES in rank order; maps ranks (rank +- 1) mod P.
@@ -309,10 +311,10 @@ LP_API int lp_be_allreduce_op(float *const *bufs, int P, size_t n, int reduce_op
  * everywhere else in this header (LP_ERR_UNSUPPORTED when that many CTAs do not fit the device). */
 #define LP_CHAIN_HANDLE_BYTES 64
 #define LP_CHAIN_MAX_CHANNELS 64
-#define LP_CHAIN_DEFAULT_CHANNELS 32
-#define LP_CHAIN_EMULATE_CHANNELS 8
+#define LP_CHAIN_DEFAULT_CHANNELS 64
+#define LP_CHAIN_EMULATE_CHANNELS 16
 #define LP_CHAIN_DEFAULT_SLOTS 8
-#define LP_CHAIN_DEFAULT_TILE 16384
+#define LP_CHAIN_DEFAULT_TILE 65536
 typedef struct lp_chain lp_chain;
 typedef struct lp_chain_role {
     int position;     /* place in the chain of this collective: rank for reduce / allreduce, (rank - root) mod P for broadcast */

@@ -36,7 +36,7 @@
 
 namespace {
 
-constexpr int kChainThreads = 512;
+constexpr int kChainThreads = 1024;
 constexpr int kFlagStride = 16;           // unsigned long longs between two counters: one 128-byte line each
 constexpr int kFlagsPerChannel = 4 * kFlagStride;
 enum { F_FWD_TAIL = 0, F_BWD_TAIL = kFlagStride, F_UP_CREDIT = 2 * kFlagStride, F_DOWN_CREDIT = 3 * kFlagStride };
@@ -65,6 +65,7 @@ struct LpChainLaunch {
     lp_partition part;
     int n_local;  // ranks in this launch
     int C, S;
+    uint32_t tile;  // elements per ring slot
     int code;  // (dtype << 1) | red_op
     unsigned long long spin_limit;  // polls before a wait gives up and flags an error: a missing peer never hangs the GPU
 };
@@ -127,18 +128,20 @@ __device__ __forceinline__ void credit(unsigned long long *remote_flag, unsigned
     if (threadIdx.x == 0) st_sys(remote_flag, seq);
 }
 
-// The tile as V vectors per thread; `nfull` whole 16-byte vectors, then `rem` (< 4) single elements (last tile only:
+// A slot (one tile of L.tile elements: the unit of a flag exchange) is worked through in STEPS of kStep elements, kV
+// 16-byte vectors per thread: between two flag exchanges nothing synchronises, so the loads of one step overlap the
+// stores of the step before.  `nfull` whole vectors, then `rem` (< 4) single elements (the message's last tile only:
 // every tile starts on a 16-byte boundary because the chain rounds blocks up to a multiple of 4 elements).
-template <int V>
-struct TileRegs {
-    float4 v[V];
+constexpr int kV = 4;
+constexpr uint32_t kStep = kV * 4 * kChainThreads;  // 16384 elements = 64 KB
+struct StepRegs {
+    float4 v[kV];
 };
 
-template <int V>
-__device__ __forceinline__ void load_tile(TileRegs<V> &t, const float *src, uint32_t len, bool ring) {
+__device__ __forceinline__ void load_step(StepRegs &t, const float *src, uint32_t len, bool ring) {
     const uint32_t nfull = len >> 2, rem = len & 3u;
 #pragma unroll
-    for (int k = 0; k < V; ++k) {
+    for (int k = 0; k < kV; ++k) {
         const uint32_t j = threadIdx.x + (uint32_t)k * kChainThreads;
         if (j < nfull) {
             t.v[k] = ring ? ld_ring(src + 4 * j) : lp_ldg_stream(src + 4 * j);
@@ -150,11 +153,10 @@ __device__ __forceinline__ void load_tile(TileRegs<V> &t, const float *src, uint
     }
 }
 
-template <int V>
-__device__ __forceinline__ void store_tile(const TileRegs<V> &t, float *dst, uint32_t len) {
+__device__ __forceinline__ void store_step(const StepRegs &t, float *dst, uint32_t len) {
     const uint32_t nfull = len >> 2, rem = len & 3u;
 #pragma unroll
-    for (int k = 0; k < V; ++k) {
+    for (int k = 0; k < kV; ++k) {
         const uint32_t j = threadIdx.x + (uint32_t)k * kChainThreads;
         if (j < nfull) {
             lp_stg_stream(dst + 4 * j, t.v[k]);
@@ -165,47 +167,48 @@ __device__ __forceinline__ void store_tile(const TileRegs<V> &t, float *dst, uin
     }
 }
 
+__device__ __forceinline__ unsigned long long slot_free_at(unsigned long long sent, int S) {
+    return sent + 1 > (unsigned)S ? sent + 1 - (unsigned)S : 0;  // send number sent + 1 reuses the slot of send sent + 1 - S
+}
+
 // Forward CTA of channel c: the reduce half of Fig. 2b (and the whole of a broadcast, Fig. 2a).
-template <int V>
 __device__ void chain_forward(const LpChainRank &A, const LpChainLaunch &L, int c, int *s_ok) {
-    constexpr uint32_t kTile = V * 4 * kChainThreads;
     unsigned long long *st = A.state + (size_t)c * 4;
     unsigned long long recv = st[ST_RECV_FWD], sent_up = st[ST_SENT_UP], sent_down = st[ST_SENT_DOWN];
     unsigned long long *my = A.flags + (size_t)c * kFlagsPerChannel;
     unsigned long long *up = A.up_flags + (size_t)c * kFlagsPerChannel;
     unsigned long long *down = A.down_flags + (size_t)c * kFlagsPerChannel;
-    const size_t ring_c = (size_t)c * L.S * kTile;
+    const size_t ring_c = (size_t)c * L.S * L.tile;
     __syncthreads();  // everybody has read the sequence numbers before thread 0 may write them back
     bool ok = true;
     for (uint64_t t = (uint64_t)c; ok && t < L.part.n_tiles; t += (uint64_t)L.C) {
         uint64_t off;
         uint32_t len;
         lp_tile_range(L.part, t, off, len);
-        TileRegs<V> acc, mine;
-        if (A.f_load) load_tile<V>(A.f_recv ? mine : acc, A.buf + off, len, false);  // my block: no flag to wait for
-        if (A.f_recv) {  // "GPU1 reduces the received block a0 with a1 to yield a'": partial op mine, in that order
-            ok = wait_counter(my + F_FWD_TAIL, recv + 1, A.error, s_ok, L.spin_limit);
-            if (!ok) break;
-            load_tile<V>(acc, A.fwd_ring + ring_c + (size_t)(recv % (unsigned)L.S) * kTile, len, true);
-            if (A.f_load) lp_fold_vecs<V>(acc.v, mine.v, V, L.code);
-            ++recv;
+        // every flag this tile needs, then the tile itself without a single barrier
+        if (A.f_recv) ok = wait_counter(my + F_FWD_TAIL, recv + 1, A.error, s_ok, L.spin_limit);
+        if (ok && A.f_send_up) ok = wait_counter(my + F_UP_CREDIT, slot_free_at(sent_up, L.S), A.error, s_ok, L.spin_limit);
+        if (ok && A.f_send_down) ok = wait_counter(my + F_DOWN_CREDIT, slot_free_at(sent_down, L.S), A.error, s_ok, L.spin_limit);
+        if (!ok) break;
+        const float *in_slot = A.fwd_ring + ring_c + (size_t)(recv % (unsigned)L.S) * L.tile;
+        float *up_slot = A.up_fwd_ring + ring_c + (size_t)(sent_up % (unsigned)L.S) * L.tile;
+        float *down_slot = A.down_bwd_ring + ring_c + (size_t)(sent_down % (unsigned)L.S) * L.tile;
+        for (uint32_t s0 = 0; s0 < len; s0 += kStep) {
+            const uint32_t sl = len - s0 < kStep ? len - s0 : kStep;
+            StepRegs acc, mine;
+            if (A.f_load) load_step(A.f_recv ? mine : acc, A.buf + off + s0, sl, false);
+            if (A.f_recv) {  // "GPU1 reduces the received block a0 with a1 to yield a'": partial op mine, in that order
+                load_step(acc, in_slot + s0, sl, true);
+                if (A.f_load) lp_fold_vecs<kV>(acc.v, mine.v, kV, L.code);
+            }
+            if (A.f_send_up) store_step(acc, up_slot + s0, sl);
+            if (A.f_store) store_step(acc, A.buf + off + s0, sl);
+            if (A.f_send_down) store_step(acc, down_slot + s0, sl);  // the chain's end: the tile turns around
         }
-        if (A.f_send_up) {
-            ok = wait_counter(my + F_UP_CREDIT, sent_up + 1 > (unsigned)L.S ? sent_up + 1 - (unsigned)L.S : 0, A.error, s_ok, L.spin_limit);
-            if (!ok) break;
-            store_tile<V>(acc, A.up_fwd_ring + ring_c + (size_t)(sent_up % (unsigned)L.S) * kTile, len);
-            publish(up + F_FWD_TAIL, ++sent_up);
-        }
-        if (A.f_store) store_tile<V>(acc, A.buf + off, len);
-        if (A.f_send_down) {  // the chain's end: the finished tile turns around
-            ok = wait_counter(my + F_DOWN_CREDIT, sent_down + 1 > (unsigned)L.S ? sent_down + 1 - (unsigned)L.S : 0, A.error,
-                              s_ok, L.spin_limit);
-            if (!ok) break;
-            store_tile<V>(acc, A.down_bwd_ring + ring_c + (size_t)(sent_down % (unsigned)L.S) * kTile, len);
-            publish(down + F_BWD_TAIL, ++sent_down);
-        }
+        if (A.f_send_up) publish(up + F_FWD_TAIL, ++sent_up);
+        if (A.f_send_down) publish(down + F_BWD_TAIL, ++sent_down);
         // the slot's values have been consumed by the stores / the fold above: hand it back to rank r-1
-        if (A.f_recv) credit(down + F_UP_CREDIT, recv);
+        if (A.f_recv) credit(down + F_UP_CREDIT, ++recv);
     }
     __syncthreads();
     if (threadIdx.x == 0) {
@@ -217,35 +220,33 @@ __device__ void chain_forward(const LpChainRank &A, const LpChainLaunch &L, int 
 
 // Return CTA of channel c: the broadcast half of allreduce (and the way a reduced tile reaches a root that is not
 // the chain's end): finished tiles flow rank r+1 -> r.
-template <int V>
 __device__ void chain_return(const LpChainRank &A, const LpChainLaunch &L, int c, int *s_ok) {
-    constexpr uint32_t kTile = V * 4 * kChainThreads;
     unsigned long long *st = A.state + (size_t)c * 4;
     unsigned long long recv = st[ST_RECV_BWD], sent_down = st[ST_SENT_DOWN];
     unsigned long long *my = A.flags + (size_t)c * kFlagsPerChannel;
     unsigned long long *up = A.up_flags + (size_t)c * kFlagsPerChannel;
     unsigned long long *down = A.down_flags + (size_t)c * kFlagsPerChannel;
-    const size_t ring_c = (size_t)c * L.S * kTile;
+    const size_t ring_c = (size_t)c * L.S * L.tile;
     __syncthreads();
     bool ok = true;
     for (uint64_t t = (uint64_t)c; ok && t < L.part.n_tiles; t += (uint64_t)L.C) {
         uint64_t off;
         uint32_t len;
         lp_tile_range(L.part, t, off, len);
-        TileRegs<V> fin;
         ok = wait_counter(my + F_BWD_TAIL, recv + 1, A.error, s_ok, L.spin_limit);
+        if (ok && A.r_send_down) ok = wait_counter(my + F_DOWN_CREDIT, slot_free_at(sent_down, L.S), A.error, s_ok, L.spin_limit);
         if (!ok) break;
-        load_tile<V>(fin, A.bwd_ring + ring_c + (size_t)(recv % (unsigned)L.S) * kTile, len, true);
-        ++recv;
-        if (A.r_store) store_tile<V>(fin, A.buf + off, len);
-        if (A.r_send_down) {
-            ok = wait_counter(my + F_DOWN_CREDIT, sent_down + 1 > (unsigned)L.S ? sent_down + 1 - (unsigned)L.S : 0, A.error,
-                              s_ok, L.spin_limit);
-            if (!ok) break;
-            store_tile<V>(fin, A.down_bwd_ring + ring_c + (size_t)(sent_down % (unsigned)L.S) * kTile, len);
-            publish(down + F_BWD_TAIL, ++sent_down);
+        const float *in_slot = A.bwd_ring + ring_c + (size_t)(recv % (unsigned)L.S) * L.tile;
+        float *down_slot = A.down_bwd_ring + ring_c + (size_t)(sent_down % (unsigned)L.S) * L.tile;
+        for (uint32_t s0 = 0; s0 < len; s0 += kStep) {
+            const uint32_t sl = len - s0 < kStep ? len - s0 : kStep;
+            StepRegs fin;
+            load_step(fin, in_slot + s0, sl, true);
+            if (A.r_store) store_step(fin, A.buf + off + s0, sl);
+            if (A.r_send_down) store_step(fin, down_slot + s0, sl);
         }
-        credit(up + F_DOWN_CREDIT, recv);
+        if (A.r_send_down) publish(down + F_BWD_TAIL, ++sent_down);
+        credit(up + F_DOWN_CREDIT, ++recv);
     }
     __syncthreads();
     if (threadIdx.x == 0) {
@@ -255,17 +256,16 @@ __device__ void chain_return(const LpChainRank &A, const LpChainLaunch &L, int c
 }
 
 // grid = n_local x 2 C: CTA b plays local rank b / (2 C); of a rank's 2 C CTAs the first C are forward, the rest return.
-template <int V>
-__global__ void __launch_bounds__(kChainThreads) lp_chain_kernel(const __grid_constant__ LpChainLaunch L) {
+__global__ void __launch_bounds__(kChainThreads, 1) lp_chain_kernel(const __grid_constant__ LpChainLaunch L) {
     __shared__ int s_ok;
     const int per_rank = 2 * L.C;
     const int lr = (int)blockIdx.x / per_rank;
     const int j = (int)blockIdx.x - lr * per_rank;
     const LpChainRank &A = L.rank[lr];
     if (j < L.C) {
-        if (A.f_active) chain_forward<V>(A, L, j, &s_ok);
+        if (A.f_active) chain_forward(A, L, j, &s_ok);
     } else {
-        if (A.r_active) chain_return<V>(A, L, j - L.C, &s_ok);
+        if (A.r_active) chain_return(A, L, j - L.C, &s_ok);
     }
 }
 
@@ -367,28 +367,19 @@ void fill_rank(LpChainRank &R, const EndpointLayout &l, float *buf, void *mine, 
 }
 
 // CTAs of the chain kernel the current device holds at once
-template <int V>
-cudaError_t resident_t(int *ctas) {
+cudaError_t resident(int *ctas) {
     int per_sm = 0, dev = 0, sms = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, lp_chain_kernel<V>, kChainThreads, 0);
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, lp_chain_kernel, kChainThreads, 0);
     *ctas = per_sm * sms;
     return e;
 }
-cudaError_t resident(int tile, int *ctas) {
-    switch (tile) {
-        case 4096: return resident_t<2>(ctas);
-        case 8192: return resident_t<4>(ctas);
-        default: return resident_t<8>(ctas);
-    }
-}
 
-template <int V>
-cudaError_t launch_t(const LpChainLaunch &L, bool cooperative, cudaStream_t stream) {
+cudaError_t launch(const LpChainLaunch &L, bool cooperative, cudaStream_t stream) {
     const unsigned grid = (unsigned)(L.n_local * 2 * L.C);
     int cap = 0;
-    cudaError_t e = resident_t<V>(&cap);
+    cudaError_t e = resident(&cap);
     if (e != cudaSuccess) return e;
     if ((unsigned)cap < grid) return cudaErrorCooperativeLaunchTooLarge;  // every CTA must be resident
     cudaLaunchConfig_t lc;
@@ -403,28 +394,20 @@ cudaError_t launch_t(const LpChainLaunch &L, bool cooperative, cudaStream_t stre
     lc.numAttrs = cooperative ? 1 : 0;
     lp_count_launch(1);
     lp_chain_reset(stream);
-    return cudaLaunchKernelEx(&lc, lp_chain_kernel<V>, L);
-}
-
-cudaError_t launch(const LpChainLaunch &L, int tile, bool cooperative, cudaStream_t stream) {
-    switch (tile) {
-        case 4096: return launch_t<2>(L, cooperative, stream);
-        case 8192: return launch_t<4>(L, cooperative, stream);
-        case 16384: return launch_t<8>(L, cooperative, stream);
-        default: return cudaErrorInvalidValue;
-    }
+    return cudaLaunchKernelEx(&lc, lp_chain_kernel, L);
 }
 
 // a1 for the chain: blocks of `block` elements rounded up to a multiple of 4 (every tile then starts on a 16-byte
 // boundary; results never depend on the block), cut into tiles of one ring slot.
 lp_partition chain_partition(size_t n, size_t block, int tile) {
-    if (block == 0) block = LP_CHAIN_DEFAULT_TILE;
+    if (block == 0) block = (size_t)tile;
     if (block < ~(size_t)3) block = (block + 3) & ~(size_t)3;
     return lp_make_partition(n, block, (uint32_t)tile);
 }
 
-bool valid_geometry(int C, int S, int tile) {
-    return C >= 1 && C <= LP_CHAIN_MAX_CHANNELS && S >= 1 && S <= 64 && (tile == 4096 || tile == 8192 || tile == 16384);
+bool valid_geometry(int C, int S, int tile) {  // tile: a power of two, 4096 .. 262144 elements (16 KB .. 1 MB)
+    return C >= 1 && C <= LP_CHAIN_MAX_CHANNELS && S >= 1 && S <= 64 && tile >= 4096 && tile <= 262144 &&
+           (tile & (tile - 1)) == 0;
 }
 
 int chain_fail(cudaError_t e) {
@@ -578,8 +561,9 @@ int lp_chain_run(lp_chain *ch, int op, float *buf, size_t n, size_t block, int r
     L.code = reduce_op;  // fp32
     L.spin_limit = 1ull << 28;  // ~a minute of polling: ranks of different processes start at different times
     L.part = chain_partition(n, block, ch->tile);
+    L.tile = (uint32_t)ch->tile;
     fill_rank(L.rank[0], layout_of(ch->C, ch->S, ch->tile), buf, ch->base, ch->peer_up, ch->peer_down, role);
-    const cudaError_t e = launch(L, ch->tile, false, (cudaStream_t)cuda_stream);
+    const cudaError_t e = launch(L, false, (cudaStream_t)cuda_stream);
     return e == cudaSuccess ? LP_OK : chain_fail(e);
 }
 
@@ -598,7 +582,7 @@ int lp_chain_emulate_channels(int P, int tile) {
     if (tile == 0) tile = LP_CHAIN_DEFAULT_TILE;
     if (P < 1 || P > LP_MAX_P || !valid_geometry(1, 1, tile)) return 0;
     int cap = 0;
-    if (resident(tile, &cap) != cudaSuccess) {
+    if (resident(&cap) != cudaSuccess) {
         cudaGetLastError();
         return 1;
     }
@@ -661,7 +645,8 @@ int lp_chain_emulate(int op, float *const *bufs, int P, size_t n, size_t block, 
         fill_rank(L.rank[r], l, bufs[r], b + l.bytes * (size_t)r, b + l.bytes * (size_t)roles[r].up,
                   b + l.bytes * (size_t)roles[r].down, roles[r]);
     }
-    const cudaError_t e = launch(L, tile, true, (cudaStream_t)cuda_stream);
+    L.tile = (uint32_t)tile;
+    const cudaError_t e = launch(L, true, (cudaStream_t)cuda_stream);
     return e == cudaSuccess ? LP_OK : chain_fail(e);
 }
 

@@ -74,7 +74,7 @@ def test_chain_every_root(oracle, op):
             check(oracle, P, 50_001, 4096, op, root=root)
 
 
-@pytest.mark.parametrize("tile", [4096, 8192, 16384])
+@pytest.mark.parametrize("tile", [4096, 16384, 65536, 262144])
 @pytest.mark.parametrize("slots", [1, 2, 8])
 def test_chain_ring_geometry_and_back_pressure(oracle, tile, slots):
     """Few channels and shallow rings: every slot is reused hundreds of times, so credits and sequence numbers wrap
@@ -133,7 +133,9 @@ def test_chain_argument_errors():
     assert L.lp_chain_emulate(lp.OP_REDUCE, arr, 2, n, 16, 2, 0, 0, 0, 0, s) == lp.LP_ERR_INVALID_ARG      # root
     assert L.lp_chain_emulate(lp.OP_BSP_SGD, arr, 2, n, 16, 0, 0, 0, 0, 0, s) == lp.LP_ERR_INVALID_ARG     # collective
     assert L.lp_chain_emulate(lp.OP_ALLREDUCE, arr, 2, n, 16, 0, 0, 0, 0, 1000, s) == lp.LP_ERR_INVALID_ARG  # tile
-    assert L.lp_chain_emulate(lp.OP_ALLREDUCE, arr, 2, n, 16, 0, 0, 64, 0, 0, s) == lp.LP_ERR_UNSUPPORTED   # 256 CTAs of 94 regs
+    dev4 = [torch.zeros(64, device="cuda") for _ in range(4)]
+    arr4, _ = lp._dev_ptrs(dev4)
+    assert L.lp_chain_emulate(lp.OP_ALLREDUCE, arr4, 4, n, 16, 0, 0, 64, 0, 0, s) == lp.LP_ERR_UNSUPPORTED  # 512 CTAs at once
     assert L.lp_chain_emulate(lp.OP_ALLREDUCE, arr, 2, 0, 16, 0, 0, 0, 0, 0, s) == lp.LP_OK                 # n == 0
 
 
