@@ -325,6 +325,7 @@ typedef struct lp_chain_role {
     int f_send_up;    /* ... push the result to `up` */
     int f_store;      /* ... store it to the local vector */
     int f_send_down;  /* ... chain end of allreduce / reduce to another root: push the finished block to `down` */
+    int f_update;     /* ... chain end of the SGD step: apply w' = w - lr * (S * invP) before the block turns around */
     int r_active;     /* return CTAs run: receive finished blocks from `up` */
     int r_store;      /* ... store them to the local vector */
     int r_send_down;  /* ... pass them on to `down` */
@@ -337,10 +338,24 @@ LP_API int lp_chain_connect(lp_chain *ch, const void *handles);
 LP_API int lp_chain_connect_ptrs(lp_chain *ch, void *up_endpoint, void *down_endpoint);
 LP_API void *lp_chain_endpoint(lp_chain *ch);
 LP_API int lp_chain_run(lp_chain *ch, int op, float *buf, size_t n, size_t block, int root, int reduce_op, void *cuda_stream);
+/* The same on vectors of element type `dtype` (LP_DT_*, U21; n, block in elements; an f16 / bf16 vector must hold an even
+ * number of elements here: a push moves whole 4-byte words). */
+LP_API int lp_chain_run_dt(lp_chain *ch, int op, void *buf, size_t n, size_t block, int root, int dtype, int reduce_op,
+                           void *cuda_stream);
+/* Alg. 3's communication + update over the chain: the sub-gradients `grad` are folded up the chain,
+ * the last rank forms w' = w - lr * (S * fl(1/P)) (three RN operations, U7) from ITS replica `weight` (all replicas hold
+ * the same bits, U8) and w' travels back down; every rank stores it into its `weight`.  grad is only read; fp32. */
+LP_API int lp_chain_bsp_sgd_step(lp_chain *ch, float *grad, float *weight, size_t n, size_t block, float lr,
+                                 void *cuda_stream);
 LP_API int lp_chain_error(lp_chain *ch, int *error_out);
 LP_API int lp_chain_destroy(lp_chain *ch);
 LP_API int lp_chain_emulate(int op, float *const *bufs, int P, size_t n, size_t block, int root, int reduce_op, int channels,
                             int slots, int tile, void *cuda_stream);
+LP_API int lp_chain_emulate_dt(int op, void *const *bufs, int P, size_t n, size_t block, int root, int dtype, int reduce_op,
+                               int channels, int slots, int tile, void *cuda_stream);
+/* grads[r], weights[r]: rank r's vectors; equals lp_bsp_sgd_step with root = P - 1 (the replica the chain's end reads) */
+LP_API int lp_chain_emulate_bsp_sgd_step(float *const *grads, float *const *weights, int P, size_t n, size_t block, float lr,
+                                         int channels, int slots, int tile, void *cuda_stream);
 LP_API int lp_chain_emulate_channels(int P, int tile);
 LP_API int lp_chain_emulate_error(int P, int channels, int slots, int tile, int *error_out);
 

@@ -46,7 +46,7 @@ class PlanInfo(ctypes.Structure):
 
 class ChainRole(ctypes.Structure):
     _fields_ = [(k, ctypes.c_int) for k in ("position", "up", "down", "f_active", "f_load", "f_recv", "f_send_up", "f_store",
-                                            "f_send_down", "r_active", "r_store", "r_send_down")]
+                                            "f_send_down", "f_update", "r_active", "r_store", "r_send_down")]
 
     def as_dict(self):
         return {k: int(getattr(self, k)) for k, _ in self._fields_}
@@ -119,6 +119,10 @@ def lib() -> ctypes.CDLL:
     L.lp_chain_endpoint.argtypes = [vp]
     L.lp_chain_endpoint.restype = vp
     L.lp_chain_run.argtypes = [vp, i32, vp, sz, sz, i32, i32, vp]
+    L.lp_chain_run_dt.argtypes = [vp, i32, vp, sz, sz, i32, i32, i32, vp]
+    L.lp_chain_bsp_sgd_step.argtypes = [vp, vp, vp, sz, sz, f32, vp]
+    L.lp_chain_emulate_dt.argtypes = [i32, pp, i32, sz, sz, i32, i32, i32, i32, i32, i32, vp]
+    L.lp_chain_emulate_bsp_sgd_step.argtypes = [pp, pp, i32, sz, sz, f32, i32, i32, i32, vp]
     L.lp_chain_error.argtypes = [vp, ctypes.POINTER(i32)]
     L.lp_chain_destroy.argtypes = [vp]
     L.lp_chain_emulate.argtypes = [i32, pp, i32, sz, sz, i32, i32, i32, i32, i32, vp]
@@ -339,6 +343,22 @@ def lp_chain_emulate(op, bufs, block=0, root=0, reduce_op=REDUCE_SUM, channels=0
            "lp_chain_emulate")
 
 
+def lp_chain_emulate_dt(op, bufs, block=0, root=0, dtype=None, reduce_op=REDUCE_SUM, channels=0, slots=0, tile=0, stream=None):
+    arr, n, dt = _dev_ptrs_dt(bufs, dtype)
+    _check(lib().lp_chain_emulate_dt(op, arr, len(bufs), n, block, root, dt, reduce_op, channels, slots, tile,
+                                     _stream_ptr(stream)), "lp_chain_emulate_dt")
+
+
+def lp_chain_emulate_bsp_sgd_step(grads, weights, block=0, lr=0.01, channels=0, slots=0, tile=0, stream=None):
+    """Alg. 3's step over the emulated chain; equals lp_bsp_sgd_step with root = P - 1."""
+    ga, n = _dev_ptrs(grads)
+    wa, nw = _dev_ptrs(weights)
+    if n != nw or len(grads) != len(weights):
+        raise ValueError("grads and weights must match in P and n")
+    _check(lib().lp_chain_emulate_bsp_sgd_step(ga, wa, len(grads), n, block, ctypes.c_float(lr), channels, slots, tile,
+                                               _stream_ptr(stream)), "lp_chain_emulate_bsp_sgd_step")
+
+
 def lp_chain_emulate_error(P, channels=0, slots=0, tile=0) -> int:
     e = ctypes.c_int(0)
     _check(lib().lp_chain_emulate_error(P, channels, slots, tile, ctypes.byref(e)), "lp_chain_emulate_error")
@@ -382,6 +402,22 @@ class Chain:
             raise TypeError("buf must be a contiguous float32 CUDA tensor")
         _check(lib().lp_chain_run(self.h, op, ctypes.c_void_p(buf.data_ptr()), buf.numel(), block, root, reduce_op,
                                   _stream_ptr(stream)), "lp_chain_run")
+
+    def run_dt(self, op, buf, block=0, root=0, reduce_op=REDUCE_SUM, dtype=None, stream=None):
+        _, n, dt = _dev_ptrs_dt([buf], dtype)
+        _check(lib().lp_chain_run_dt(self.h, op, ctypes.c_void_p(buf.data_ptr()), n, block, root, dt, reduce_op,
+                                     _stream_ptr(stream)), "lp_chain_run_dt")
+
+    def bsp_sgd_step(self, grad, weight, block=0, lr=0.01, stream=None):
+        import torch
+        for t in (grad, weight):
+            if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()):
+                raise TypeError("grad and weight must be contiguous float32 CUDA tensors")
+        if grad.numel() != weight.numel():
+            raise ValueError("grad and weight must have the same length")
+        _check(lib().lp_chain_bsp_sgd_step(self.h, ctypes.c_void_p(grad.data_ptr()), ctypes.c_void_p(weight.data_ptr()),
+                                           grad.numel(), block, ctypes.c_float(lr), _stream_ptr(stream)),
+               "lp_chain_bsp_sgd_step")
 
     def error(self) -> int:
         e = ctypes.c_int(0)

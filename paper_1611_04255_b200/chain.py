@@ -54,6 +54,10 @@ class ChainGroup:
     def broadcast(self, buf, root=0, block=0, stream=None):
         self.endpoint.run(lp.OP_BROADCAST, buf, block=block, root=root, stream=stream)
 
+    def bsp_sgd_step(self, grad, weight, lr, block=0, stream=None):
+        """Alg. 3: allreduce of the sub-gradients, w -= lr * mean gradient, fused; every rank's `weight` gets the new bits."""
+        self.endpoint.bsp_sgd_step(grad, weight, block=block, lr=lr, stream=stream)
+
     def error(self) -> int:
         return self.endpoint.error()
 

@@ -44,7 +44,9 @@ enum { ST_RECV_FWD = 0, ST_SENT_UP = 1, ST_RECV_BWD = 2, ST_SENT_DOWN = 3 };
 
 // What one rank's CTAs need: its vector, its endpoint, its two neighbours' endpoints, its roles in this call.
 struct LpChainRank {
-    float *buf;
+    float *buf;         // my vector: what the forward CTAs load
+    float *out;         // where finished blocks are stored: buf (in place), or my weight replica for the SGD step
+    const float *w_in;  // SGD step, chain end only: the weight replica the update reads
     unsigned long long *flags;   // my counters: [C][kFlagsPerChannel]
     unsigned long long *state;   // my private sequence numbers: [C][4]
     float *fwd_ring, *bwd_ring;  // my receive rings: [C][S][tile]
@@ -54,10 +56,10 @@ struct LpChainRank {
     float *down_bwd_ring;
     int *error;  // my error word (0 = fine)
     // forward CTAs
-    unsigned char f_active, f_load, f_recv, f_send_up, f_store, f_send_down;
+    unsigned char f_active, f_load, f_recv, f_send_up, f_store, f_send_down, f_update;
     // return CTAs
     unsigned char r_active, r_store, r_send_down;
-    unsigned char pad[3];
+    unsigned char pad[2];
 };
 
 struct LpChainLaunch {
@@ -67,6 +69,7 @@ struct LpChainLaunch {
     int C, S;
     uint32_t tile;  // elements per ring slot
     int code;  // (dtype << 1) | red_op
+    float lr, invP;  // SGD step (LpChainRank::f_update): w' = w - lr * (S * invP) where the chain ends (U7)
     unsigned long long spin_limit;  // polls before a wait gives up and flags an error: a missing peer never hangs the GPU
 };
 
@@ -201,8 +204,14 @@ __device__ void chain_forward(const LpChainRank &A, const LpChainLaunch &L, int 
                 load_step(acc, in_slot + s0, sl, true);
                 if (A.f_load) lp_fold_vecs<kV>(acc.v, mine.v, kV, L.code);
             }
+            if (A.f_update) {  // Alg. 3's update where the global gradient S is complete: three RN operations
+                StepRegs w;
+                load_step(w, A.w_in + off + s0, sl, false);
+#pragma unroll
+                for (int k = 0; k < kV; ++k) acc.v[k] = lp_sgd4(acc.v[k], w.v[k], L.lr, L.invP);
+            }
             if (A.f_send_up) store_step(acc, up_slot + s0, sl);
-            if (A.f_store) store_step(acc, A.buf + off + s0, sl);
+            if (A.f_store) store_step(acc, A.out + off + s0, sl);
             if (A.f_send_down) store_step(acc, down_slot + s0, sl);  // the chain's end: the tile turns around
         }
         if (A.f_send_up) publish(up + F_FWD_TAIL, ++sent_up);
@@ -242,7 +251,7 @@ __device__ void chain_return(const LpChainRank &A, const LpChainLaunch &L, int c
             const uint32_t sl = len - s0 < kStep ? len - s0 : kStep;
             StepRegs fin;
             load_step(fin, in_slot + s0, sl, true);
-            if (A.r_store) store_step(fin, A.buf + off + s0, sl);
+            if (A.r_store) store_step(fin, A.out + off + s0, sl);
             if (A.r_send_down) store_step(fin, down_slot + s0, sl);
         }
         if (A.r_send_down) publish(down + F_BWD_TAIL, ++sent_down);
@@ -276,12 +285,15 @@ __global__ void __launch_bounds__(kChainThreads, 1) lp_chain_kernel(const __grid
 // Roles of `rank` in a collective over P ranks (pure host logic: the part of the multi-process path that needs no GPU).
 extern "C" int lp_chain_plan(int op, int P, int root, int rank, lp_chain_role *out) {
     if (out == nullptr || P < 1 || P > LP_MAX_P || rank < 0 || rank >= P) return LP_ERR_INVALID_ARG;
-    if (op != LP_OP_BROADCAST && op != LP_OP_REDUCE && op != LP_OP_ALLREDUCE) return LP_ERR_INVALID_ARG;
-    if (op != LP_OP_ALLREDUCE && (root < 0 || root >= P)) return LP_ERR_INVALID_ARG;
+    if (op != LP_OP_BROADCAST && op != LP_OP_REDUCE && op != LP_OP_ALLREDUCE && op != LP_OP_BSP_SGD) return LP_ERR_INVALID_ARG;
+    if ((op == LP_OP_BROADCAST || op == LP_OP_REDUCE) && (root < 0 || root >= P)) return LP_ERR_INVALID_ARG;
     memset(out, 0, sizeof(*out));
     out->up = (rank + 1) % P;
     out->down = (rank + P - 1) % P;
-    if (P == 1) return LP_OK;  // nothing moves
+    if (P == 1) {  // nothing moves; the SGD step of a single rank is its own update
+        if (op == LP_OP_BSP_SGD) out->f_active = out->f_load = out->f_update = out->f_store = 1;
+        return LP_OK;
+    }
     if (op == LP_OP_BROADCAST) {  // root -> root+1 -> ... -> root-1 around the ring, forward direction only
         const int j = (rank - root + P) % P;
         out->position = j;
@@ -293,7 +305,7 @@ extern "C" int lp_chain_plan(int op, int P, int root, int rank, lp_chain_role *o
         return LP_OK;
     }
     // reduce / allreduce: the chain is rank 0 -> 1 -> ... -> P-1 whatever the root (U4)
-    const bool all = op == LP_OP_ALLREDUCE;
+    const bool all = op != LP_OP_REDUCE;  // allreduce, and the SGD step (the new weights go to every rank)
     const bool head = rank == P - 1;
     const int ret_lo = all ? 0 : root;  // the lowest rank a finished tile travels back to
     out->position = rank;
@@ -303,6 +315,7 @@ extern "C" int lp_chain_plan(int op, int P, int root, int rank, lp_chain_role *o
     out->f_send_up = !head;
     out->f_store = head && (all || root == P - 1);
     out->f_send_down = head && ret_lo < P - 1;
+    out->f_update = head && op == LP_OP_BSP_SGD;
     out->r_active = !head && rank >= ret_lo && ret_lo < P - 1;
     out->r_store = out->r_active && (all || rank == root);
     out->r_send_down = out->r_active && rank > ret_lo;
@@ -342,10 +355,13 @@ EndpointLayout layout_of(int C, int S, int tile) {
     return l;
 }
 
-void fill_rank(LpChainRank &R, const EndpointLayout &l, float *buf, void *mine, void *up, void *down, const lp_chain_role &role) {
+void fill_rank(LpChainRank &R, const EndpointLayout &l, float *buf, float *out, const float *w_in, void *mine, void *up,
+               void *down, const lp_chain_role &role) {
     memset(&R, 0, sizeof(R));
     char *m = (char *)mine, *u = (char *)up, *d = (char *)down;
     R.buf = buf;
+    R.out = out;
+    R.w_in = w_in;
     R.flags = (unsigned long long *)(m + l.flags_off);
     R.state = (unsigned long long *)(m + l.state_off);
     R.error = (int *)(m + l.error_off);
@@ -361,6 +377,7 @@ void fill_rank(LpChainRank &R, const EndpointLayout &l, float *buf, void *mine, 
     R.f_send_up = role.f_send_up;
     R.f_store = role.f_store;
     R.f_send_down = role.f_send_down;
+    R.f_update = role.f_update;
     R.r_active = role.r_active;
     R.r_store = role.r_store;
     R.r_send_down = role.r_send_down;
@@ -537,17 +554,35 @@ int lp_chain_destroy(lp_chain *ch) {
     return LP_OK;
 }
 
-// One rank's share of the collective: every rank of the chain calls this with the same (op, n, block, root, reduce_op),
-// in the same order as its other chain collectives.
-int lp_chain_run(lp_chain *ch, int op, float *buf, size_t n, size_t block, int root, int reduce_op, void *cuda_stream) {
+// Words per element and the operator code of a typed launch; false for an unknown type.  The chain addresses vectors
+// in 4-byte words like every other kernel (LpArgs::dtype): n and block arrive in elements and leave in words.  16-bit
+// vectors must hold an even number of elements here (a push moves whole words).
+static bool chain_words(int dtype, int reduce_op, size_t &n, size_t &block, int &code) {
+    if (dtype < LP_DT_F32 || dtype > LP_DT_F64) return false;
+    if (reduce_op != LP_REDUCE_SUM && reduce_op != LP_REDUCE_PROD) return false;
+    code = (dtype << 1) | reduce_op;
+    if (dtype == LP_DT_F64) {
+        if (n > (~(size_t)0) / 8) return false;
+        n *= 2;
+        block = block > (~(size_t)0) / 2 ? ~(size_t)3 : 2 * block;
+    } else if (dtype != LP_DT_F32) {
+        if (n & 1u) return false;
+        n /= 2;
+        block = block / 2 + (block & 1u);
+    }
+    return true;
+}
+
+static int chain_run_rank(lp_chain *ch, int op, float *buf, float *out, const float *w_in, size_t n, size_t block, int root,
+                          int code, float lr, void *cuda_stream) {
     if (ch == nullptr || !ch->connected) return LP_ERR_INVALID_ARG;
-    if (reduce_op != LP_REDUCE_SUM && reduce_op != LP_REDUCE_PROD) return LP_ERR_INVALID_ARG;
-    if (op == LP_OP_ALLREDUCE) root = 0;
+    if (op == LP_OP_ALLREDUCE || op == LP_OP_BSP_SGD) root = 0;
     lp_chain_role role;
     int rc = lp_chain_plan(op, ch->P, root, ch->rank, &role);
     if (rc != LP_OK) return rc;
-    if (buf == nullptr || ((uintptr_t)buf & 15u)) return LP_ERR_INVALID_ARG;
-    if (n == 0 || ch->P == 1) return LP_OK;
+    if (buf == nullptr || ((uintptr_t)buf & 15u) || out == nullptr || ((uintptr_t)out & 15u)) return LP_ERR_INVALID_ARG;
+    if (n == 0) return LP_OK;
+    if (ch->P == 1 && op != LP_OP_BSP_SGD) return LP_OK;
     int dev = -1;
     if (cudaGetDevice(&dev) != cudaSuccess || dev != ch->device) {
         cudaGetLastError();
@@ -558,13 +593,40 @@ int lp_chain_run(lp_chain *ch, int op, float *buf, size_t n, size_t block, int r
     L.n_local = 1;
     L.C = ch->C;
     L.S = ch->S;
-    L.code = reduce_op;  // fp32
+    L.code = code;
+    L.lr = lr;
+    L.invP = 1.0f / (float)ch->P;  // one RN division on the host (U7)
     L.spin_limit = 1ull << 28;  // ~a minute of polling: ranks of different processes start at different times
     L.part = chain_partition(n, block, ch->tile);
     L.tile = (uint32_t)ch->tile;
-    fill_rank(L.rank[0], layout_of(ch->C, ch->S, ch->tile), buf, ch->base, ch->peer_up, ch->peer_down, role);
+    fill_rank(L.rank[0], layout_of(ch->C, ch->S, ch->tile), buf, out, w_in, ch->base, ch->peer_up, ch->peer_down, role);
     const cudaError_t e = launch(L, false, (cudaStream_t)cuda_stream);
     return e == cudaSuccess ? LP_OK : chain_fail(e);
+}
+
+// One rank's share of the collective: every rank of the chain calls this with the same (op, n, block, root, reduce_op),
+// in the same order as its other chain collectives.
+int lp_chain_run(lp_chain *ch, int op, float *buf, size_t n, size_t block, int root, int reduce_op, void *cuda_stream) {
+    if (op != LP_OP_BROADCAST && op != LP_OP_REDUCE && op != LP_OP_ALLREDUCE) return LP_ERR_INVALID_ARG;
+    int code;
+    if (!chain_words(LP_DT_F32, reduce_op, n, block, code)) return LP_ERR_INVALID_ARG;
+    return chain_run_rank(ch, op, buf, buf, nullptr, n, block, root, code, 0.f, cuda_stream);
+}
+
+int lp_chain_run_dt(lp_chain *ch, int op, void *buf, size_t n, size_t block, int root, int dtype, int reduce_op,
+                    void *cuda_stream) {
+    if (op != LP_OP_BROADCAST && op != LP_OP_REDUCE && op != LP_OP_ALLREDUCE) return LP_ERR_INVALID_ARG;
+    int code;
+    if (!chain_words(dtype, reduce_op, n, block, code)) return LP_ERR_INVALID_ARG;
+    return chain_run_rank(ch, op, (float *)buf, (float *)buf, nullptr, n, block, root, code, 0.f, cuda_stream);
+}
+
+// Alg. 3's communication + update over the chain: the sub-gradients are folded up the chain, the
+// last rank forms w' = w - lr * (S * invP) from ITS weight replica (all replicas hold the same bits, U8) and the new
+// weights travel back down; every rank stores them into its replica.  grad is only read.
+int lp_chain_bsp_sgd_step(lp_chain *ch, float *grad, float *weight, size_t n, size_t block, float lr, void *cuda_stream) {
+    if (weight == nullptr || grad == weight) return LP_ERR_INVALID_ARG;
+    return chain_run_rank(ch, LP_OP_BSP_SGD, grad, weight, weight, n, block, 0, LP_REDUCE_SUM, lr, cuda_stream);
 }
 
 // 0 = no wait of this endpoint's kernels has given up so far (a peer that never arrived); synchronises the device.
@@ -593,28 +655,32 @@ int lp_chain_emulate_channels(int P, int tile) {
 
 // All P ranks of the chain on ONE device, in one cooperative launch: P x 2 x channels co-resident CTAs run the per-rank
 // code above against P endpoints in this device's memory.
-int lp_chain_emulate(int op, float *const *bufs, int P, size_t n, size_t block, int root, int reduce_op, int channels,
-                     int slots, int tile, void *cuda_stream) {
+static int chain_emulate(int op, float *const *bufs, float *const *outs, int P, size_t n, size_t block, int root, int code,
+                         size_t elem_bytes_total, float lr, int channels, int slots, int tile, void *cuda_stream) {
     if (slots == 0) slots = LP_CHAIN_DEFAULT_SLOTS;
     if (tile == 0) tile = LP_CHAIN_DEFAULT_TILE;
     if (channels == 0) channels = lp_chain_emulate_channels(P, tile);
     if (bufs == nullptr || P < 1 || P > LP_MAX_P || !valid_geometry(channels, slots, tile)) return LP_ERR_INVALID_ARG;
-    if (reduce_op != LP_REDUCE_SUM && reduce_op != LP_REDUCE_PROD) return LP_ERR_INVALID_ARG;
-    if (op == LP_OP_ALLREDUCE) root = 0;
+    if (op == LP_OP_ALLREDUCE || op == LP_OP_BSP_SGD) root = 0;
     lp_chain_role roles[LP_MAX_P];
     for (int r = 0; r < P; ++r) {
         const int rc = lp_chain_plan(op, P, root, r, &roles[r]);
         if (rc != LP_OK) return rc;
     }
-    const size_t bytes = n * sizeof(float);
-    for (int r = 0; r < P; ++r) {
-        if (bufs[r] == nullptr || ((uintptr_t)bufs[r] & 15u)) return LP_ERR_INVALID_ARG;
-        for (int q = 0; q < r; ++q) {
-            const uintptr_t a = (uintptr_t)bufs[r], b = (uintptr_t)bufs[q];
-            if (bytes && a < b + bytes && b < a + bytes) return LP_ERR_INVALID_ARG;
+    const float *all[2 * LP_MAX_P];
+    int m = 0;
+    for (int r = 0; r < P; ++r) all[m++] = bufs[r];
+    if (outs != bufs)
+        for (int r = 0; r < P; ++r) all[m++] = outs[r];
+    for (int i = 0; i < m; ++i) {
+        if (all[i] == nullptr || ((uintptr_t)all[i] & 15u)) return LP_ERR_INVALID_ARG;
+        for (int q = 0; q < i; ++q) {
+            const uintptr_t a = (uintptr_t)all[i], b = (uintptr_t)all[q];
+            if (elem_bytes_total && a < b + elem_bytes_total && b < a + elem_bytes_total) return LP_ERR_INVALID_ARG;
         }
     }
-    if (n == 0 || P == 1) return LP_OK;
+    if (n == 0) return LP_OK;
+    if (P == 1 && op != LP_OP_BSP_SGD) return LP_OK;
     const EndpointLayout l = layout_of(channels, slots, tile);
     void *base = nullptr;
     {
@@ -637,17 +703,45 @@ int lp_chain_emulate(int op, float *const *bufs, int P, size_t n, size_t block, 
     L.n_local = P;
     L.C = channels;
     L.S = slots;
-    L.code = reduce_op;
+    L.code = code;
+    L.lr = lr;
+    L.invP = 1.0f / (float)P;
     L.spin_limit = 1ull << 23;  // all ranks start together here: a few seconds mean a bug
     L.part = chain_partition(n, block, tile);
+    L.tile = (uint32_t)tile;
     for (int r = 0; r < P; ++r) {
         char *b = (char *)base;
-        fill_rank(L.rank[r], l, bufs[r], b + l.bytes * (size_t)r, b + l.bytes * (size_t)roles[r].up,
-                  b + l.bytes * (size_t)roles[r].down, roles[r]);
+        fill_rank(L.rank[r], l, bufs[r], outs[r], op == LP_OP_BSP_SGD ? outs[r] : nullptr, b + l.bytes * (size_t)r,
+                  b + l.bytes * (size_t)roles[r].up, b + l.bytes * (size_t)roles[r].down, roles[r]);
     }
-    L.tile = (uint32_t)tile;
     const cudaError_t e = launch(L, true, (cudaStream_t)cuda_stream);
     return e == cudaSuccess ? LP_OK : chain_fail(e);
+}
+
+int lp_chain_emulate(int op, float *const *bufs, int P, size_t n, size_t block, int root, int reduce_op, int channels,
+                     int slots, int tile, void *cuda_stream) {
+    if (op != LP_OP_BROADCAST && op != LP_OP_REDUCE && op != LP_OP_ALLREDUCE) return LP_ERR_INVALID_ARG;
+    int code;
+    const size_t bytes = n * sizeof(float);
+    if (!chain_words(LP_DT_F32, reduce_op, n, block, code)) return LP_ERR_INVALID_ARG;
+    return chain_emulate(op, bufs, bufs, P, n, block, root, code, bytes, 0.f, channels, slots, tile, cuda_stream);
+}
+
+int lp_chain_emulate_dt(int op, void *const *bufs, int P, size_t n, size_t block, int root, int dtype, int reduce_op,
+                        int channels, int slots, int tile, void *cuda_stream) {
+    if (op != LP_OP_BROADCAST && op != LP_OP_REDUCE && op != LP_OP_ALLREDUCE) return LP_ERR_INVALID_ARG;
+    int code;
+    const size_t bytes = n * (dtype == LP_DT_F64 ? 8 : (dtype == LP_DT_F32 ? 4 : 2));
+    if (!chain_words(dtype, reduce_op, n, block, code)) return LP_ERR_INVALID_ARG;
+    return chain_emulate(op, (float *const *)bufs, (float *const *)bufs, P, n, block, root, code, bytes, 0.f, channels, slots,
+                         tile, cuda_stream);
+}
+
+int lp_chain_emulate_bsp_sgd_step(float *const *grads, float *const *weights, int P, size_t n, size_t block, float lr,
+                                  int channels, int slots, int tile, void *cuda_stream) {
+    if (weights == nullptr) return LP_ERR_INVALID_ARG;
+    return chain_emulate(LP_OP_BSP_SGD, grads, weights, P, n, block, 0, LP_REDUCE_SUM, n * sizeof(float), lr, channels, slots,
+                         tile, cuda_stream);
 }
 
 // error word of emulated rank `rank` for the geometry (P, channels, slots, tile); synchronises the device

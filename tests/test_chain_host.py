@@ -91,6 +91,19 @@ def test_chain_ring_neighbours_never_change(P):
                 assert bool(ro["f_send_down"] or ro["r_send_down"]) == bool(down["r_active"]), (op, root, r)
 
 
+def test_chain_sgd_step_roles():
+    """The fused step is an allreduce whose end applies the update: same roles, plus f_update on the last rank only."""
+    for P in (1, 2, 6, 16):
+        for r in range(P):
+            a = lp.lp_chain_plan(lp.OP_ALLREDUCE, P, 0, r)
+            g = lp.lp_chain_plan(lp.OP_BSP_SGD, P, 0, r)
+            assert g["f_update"] == (1 if r == P - 1 else 0) and a["f_update"] == 0
+            if P > 1:
+                assert {k: v for k, v in g.items() if k != "f_update"} == {k: v for k, v in a.items() if k != "f_update"}
+    one = lp.lp_chain_plan(lp.OP_BSP_SGD, 1, 0, 0)
+    assert one["f_active"] and one["f_load"] and one["f_store"] and not one["f_send_up"] and not one["f_send_down"]
+
+
 def test_chain_link_traffic_is_invariant_to_p():
     """PAPER.md:106 "the cost of Linear Pipeline is invariant to GPU count p": per tile every rank pushes at most one
     block up and one block down, whatever P -- the busiest link of an allreduce carries 1 block per tile and direction."""
@@ -108,7 +121,7 @@ def test_chain_plan_argument_errors():
     assert L.lp_chain_plan(lp.OP_ALLREDUCE, 33, 0, 0, ref) == lp.LP_ERR_INVALID_ARG
     assert L.lp_chain_plan(lp.OP_ALLREDUCE, 4, 0, 4, ref) == lp.LP_ERR_INVALID_ARG
     assert L.lp_chain_plan(lp.OP_REDUCE, 4, 4, 0, ref) == lp.LP_ERR_INVALID_ARG
-    assert L.lp_chain_plan(lp.OP_BSP_SGD, 4, 0, 0, ref) == lp.LP_ERR_INVALID_ARG
+    assert L.lp_chain_plan(lp.OP_BSP_SGD_MOM, 4, 0, 0, ref) == lp.LP_ERR_INVALID_ARG
     assert L.lp_chain_plan(lp.OP_ALLREDUCE, 4, 99, 0, ref) == lp.LP_OK          # allreduce ignores the root
     assert L.lp_chain_endpoint_bytes(32, 8, 16384) == 32 * 64 * 8 + 32 * 4 * 8 + 256 + 2 * 32 * 8 * 16384 * 4 \
         or L.lp_chain_endpoint_bytes(32, 8, 16384) > 2 * 32 * 8 * 16384 * 4

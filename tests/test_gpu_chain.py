@@ -124,6 +124,50 @@ def test_chain_large_message(oracle):
         assert got[r].tobytes() == want[r].tobytes(), r
 
 
+@pytest.mark.parametrize("P,n,block", [(1, 5_001, 1024), (2, 70_001, 4096), (6, 300_003, 65_536), (8, 1_000_003, 65_536),
+                                       (16, 100_003, 8192)])
+def test_chain_fused_bsp_sgd_step(oracle, P, n, block):
+    """Alg. 3 over the chain: the chain's end applies the update from its own replica and the new
+    weights travel back down -- the oracle's fused step with root = P - 1, three RN operations, bit for bit; the
+    gradients are only read.  Replicas are made DIFFERENT on purpose so that reading any other one would show."""
+    grads, weights = inputs.sgd_inputs([35, n], P, n)
+    weights = [w + np.float32(r) for r, w in enumerate(weights)]
+    hw = [w.copy() for w in weights]
+    oracle.bsp_sgd_step(grads, hw, root=P - 1, lr=0.01)
+    dg, dw = up(grads), up(weights)
+    for it in range(3):                       # three steps back to back over the same rings
+        lp.lp_chain_emulate_bsp_sgd_step(dg, dw, block=block, lr=0.01)
+        if it < 2:
+            oracle.bsp_sgd_step(grads, hw, root=P - 1, lr=0.01)
+    got_w, got_g = down(dw), down(dg)
+    assert lp.lp_chain_emulate_error(P) == 0
+    for r in range(P):
+        assert got_w[r].tobytes() == hw[r].tobytes(), ("weights", r)
+        assert got_g[r].tobytes() == grads[r].tobytes(), ("grads must be untouched", r)
+
+
+@pytest.mark.parametrize("dt", [inputs.DT_F16, inputs.DT_BF16, inputs.DT_F64])
+def test_chain_element_types(oracle, dt):
+    P, n = 5, 200_002
+    for red, kind in ((lp.REDUCE_SUM, "sum"), (lp.REDUCE_PROD, "prod")):
+        src = inputs.typed_rank_vectors([36, dt], P, n, dt, kind)
+        for op in ("allreduce", "reduce", "broadcast"):
+            want = [a.copy() for a in src]
+            if op == "allreduce":
+                oracle.allreduce_dt(want, dt, red=red)
+            elif op == "reduce":
+                oracle.reduce_dt(want, dt, red=red, root=2)
+            else:
+                oracle.broadcast_dt(want, dt, root=2)
+            dev = [torch.from_numpy(a.view(np.int16) if dt == inputs.DT_BF16 else a).cuda() for a in src]
+            lp.lp_chain_emulate_dt(OPS[op], dev, block=8192, root=2, dtype=dt, reduce_op=red)
+            torch.cuda.synchronize()
+            assert lp.lp_chain_emulate_error(P) == 0
+            for r in range(P):
+                assert dev[r].cpu().numpy().tobytes() == want[r].view(np.int16 if dt == inputs.DT_BF16 else want[r].dtype).tobytes(), \
+                    (op, dt, red, r)
+
+
 def test_chain_argument_errors():
     dev = [torch.zeros(64, device="cuda") for _ in range(2)]
     arr, n = lp._dev_ptrs(dev)
