@@ -432,9 +432,11 @@ int chain_fail(cudaError_t e) {
     return e == cudaErrorCooperativeLaunchTooLarge ? LP_ERR_UNSUPPORTED : LP_ERR_CUDA;
 }
 
-// emulation endpoints: (geometry, P) -> one allocation holding P endpoints, kept for the life of the library binding
+// emulation endpoints: (geometry, P, stream) -> one allocation holding P endpoints, kept for the life of the library
+// binding.  Per stream: launches of one stream are ordered, launches of two streams may overlap and must not share rings.
 struct EmulEndpoints {
     int P, C, S, tile;
+    cudaStream_t stream;
     void *base;
 };
 std::mutex g_emul_mu;
@@ -686,7 +688,8 @@ static int chain_emulate(int op, float *const *bufs, float *const *outs, int P, 
     {
         std::lock_guard<std::mutex> lock(g_emul_mu);
         for (auto &e : g_emul)
-            if (e.P == P && e.C == channels && e.S == slots && e.tile == tile) base = e.base;
+            if (e.P == P && e.C == channels && e.S == slots && e.tile == tile && e.stream == (cudaStream_t)cuda_stream)
+                base = e.base;
         if (base == nullptr) {
             cudaError_t e = cudaMalloc(&base, l.bytes * (size_t)P);
             if (e == cudaSuccess) e = cudaMemset(base, 0, l.bytes * (size_t)P);
@@ -695,7 +698,7 @@ static int chain_emulate(int op, float *const *bufs, float *const *outs, int P, 
                 if (base) cudaFree(base);
                 return chain_fail(e);
             }
-            g_emul.push_back(EmulEndpoints{P, channels, slots, tile, base});
+            g_emul.push_back(EmulEndpoints{P, channels, slots, tile, (cudaStream_t)cuda_stream, base});
         }
     }
     LpChainLaunch L;
@@ -751,20 +754,21 @@ int lp_chain_emulate_error(int P, int channels, int slots, int tile, int *error_
     if (channels == 0) channels = lp_chain_emulate_channels(P, tile);
     if (error_out == nullptr || !valid_geometry(channels, slots, tile)) return LP_ERR_INVALID_ARG;
     *error_out = 0;
-    void *base = nullptr;
+    std::vector<void *> bases;  // the endpoints of this geometry on every stream they were used on
     {
         std::lock_guard<std::mutex> lock(g_emul_mu);
         for (auto &e : g_emul)
-            if (e.P == P && e.C == channels && e.S == slots && e.tile == tile) base = e.base;
+            if (e.P == P && e.C == channels && e.S == slots && e.tile == tile) bases.push_back(e.base);
     }
-    if (base == nullptr) return LP_OK;
+    if (bases.empty()) return LP_OK;
     cudaError_t e = cudaDeviceSynchronize();
     const EndpointLayout l = layout_of(channels, slots, tile);
-    for (int r = 0; r < P && e == cudaSuccess; ++r) {
-        int w = 0;
-        e = cudaMemcpy(&w, (char *)base + l.bytes * (size_t)r + l.error_off, sizeof(int), cudaMemcpyDeviceToHost);
-        if (w) *error_out = w;
-    }
+    for (void *base : bases)
+        for (int r = 0; r < P && e == cudaSuccess; ++r) {
+            int w = 0;
+            e = cudaMemcpy(&w, (char *)base + l.bytes * (size_t)r + l.error_off, sizeof(int), cudaMemcpyDeviceToHost);
+            if (w) *error_out = w;
+        }
     return e == cudaSuccess ? LP_OK : chain_fail(e);
 }
 
