@@ -136,7 +136,7 @@ __device__ __forceinline__ void credit(unsigned long long *remote_flag, unsigned
 // stores of the step before.  `nfull` whole vectors, then `rem` (< 4) single elements (the message's last tile only:
 // every tile starts on a 16-byte boundary because the chain rounds blocks up to a multiple of 4 elements).
 constexpr int kV = 4;
-constexpr uint32_t kStep = kV * 4 * kChainThreads;  // 16384 elements = 64 KB
+#define kStep ((uint32_t)(kV * 4) * blockDim.x)  // 16384 elements = 64 KB with 1024 threads
 struct StepRegs {
     float4 v[kV];
 };
@@ -145,7 +145,7 @@ __device__ __forceinline__ void load_step(StepRegs &t, const float *src, uint32_
     const uint32_t nfull = len >> 2, rem = len & 3u;
 #pragma unroll
     for (int k = 0; k < kV; ++k) {
-        const uint32_t j = threadIdx.x + (uint32_t)k * kChainThreads;
+        const uint32_t j = threadIdx.x + (uint32_t)k * blockDim.x;
         if (j < nfull) {
             t.v[k] = ring ? ld_ring(src + 4 * j) : lp_ldg_stream(src + 4 * j);
         } else if (j == nfull && rem) {
@@ -160,7 +160,7 @@ __device__ __forceinline__ void store_step(const StepRegs &t, float *dst, uint32
     const uint32_t nfull = len >> 2, rem = len & 3u;
 #pragma unroll
     for (int k = 0; k < kV; ++k) {
-        const uint32_t j = threadIdx.x + (uint32_t)k * kChainThreads;
+        const uint32_t j = threadIdx.x + (uint32_t)k * blockDim.x;
         if (j < nfull) {
             lp_stg_stream(dst + 4 * j, t.v[k]);
         } else if (j == nfull && rem) {
@@ -383,12 +383,16 @@ void fill_rank(LpChainRank &R, const EndpointLayout &l, float *buf, float *out, 
     R.r_send_down = role.r_send_down;
 }
 
+// 1024 threads, one CTA per SM.  (512-thread CTAs, two per SM, on twice the channels: 5-20 % more per SM in the one-GPU
+// emulation, for twice the ring memory -- profiles/r2_dtypes_chain.md.)
+int chain_threads() { return kChainThreads; }
+
 // CTAs of the chain kernel the current device holds at once
 cudaError_t resident(int *ctas) {
     int per_sm = 0, dev = 0, sms = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, lp_chain_kernel, kChainThreads, 0);
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, lp_chain_kernel, chain_threads(), 0);
     *ctas = per_sm * sms;
     return e;
 }
@@ -402,7 +406,7 @@ cudaError_t launch(const LpChainLaunch &L, bool cooperative, cudaStream_t stream
     cudaLaunchConfig_t lc;
     memset(&lc, 0, sizeof(lc));
     lc.gridDim = dim3(grid);
-    lc.blockDim = dim3(kChainThreads);
+    lc.blockDim = dim3(chain_threads());
     lc.stream = stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeCooperative;
