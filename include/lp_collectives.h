@@ -337,6 +337,9 @@ LP_API int lp_chain_get_handle(lp_chain *ch, void *handle_out);
 LP_API int lp_chain_connect(lp_chain *ch, const void *handles);
 LP_API int lp_chain_connect_ptrs(lp_chain *ch, void *up_endpoint, void *down_endpoint);
 LP_API void *lp_chain_endpoint(lp_chain *ch);
+/* How long a kernel of this endpoint polls a counter before it gives up and sets the endpoint's error word, in polls
+ * (~0.3-1 us each; default 2^28, about a minute: the ranks of a job start at different times). */
+LP_API int lp_chain_set_timeout(lp_chain *ch, unsigned long long polls);
 LP_API int lp_chain_run(lp_chain *ch, int op, float *buf, size_t n, size_t block, int root, int reduce_op, void *cuda_stream);
 /* The same on vectors of element type `dtype` (LP_DT_*, U21; n, block in elements; an f16 / bf16 vector must hold an even
  * number of elements here: a push moves whole 4-byte words). */

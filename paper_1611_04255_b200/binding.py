@@ -116,6 +116,7 @@ def lib() -> ctypes.CDLL:
     L.lp_chain_get_handle.argtypes = [vp, ctypes.c_char_p]
     L.lp_chain_connect.argtypes = [vp, ctypes.c_char_p]
     L.lp_chain_connect_ptrs.argtypes = [vp, vp, vp]
+    L.lp_chain_set_timeout.argtypes = [vp, ctypes.c_ulonglong]
     L.lp_chain_endpoint.argtypes = [vp]
     L.lp_chain_endpoint.restype = vp
     L.lp_chain_run.argtypes = [vp, i32, vp, sz, sz, i32, i32, vp]
@@ -385,6 +386,9 @@ class Chain:
 
     def endpoint(self) -> int:
         return int(lib().lp_chain_endpoint(self.h) or 0)
+
+    def set_timeout(self, polls: int):
+        _check(lib().lp_chain_set_timeout(self.h, polls), "lp_chain_set_timeout")
 
     def connect(self, handles):
         blob = b"".join(handles)

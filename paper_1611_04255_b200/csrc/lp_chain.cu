@@ -330,6 +330,7 @@ struct lp_chain {
     void *peer_up, *peer_down;  // mapped endpoints of the neighbours (== base of another lp_chain in the same process)
     bool up_ipc, down_ipc;      // opened with cudaIpcOpenMemHandle (to be closed)
     bool connected;
+    unsigned long long spin_limit;  // polls before a wait of this endpoint's kernels gives up
 };
 
 namespace {
@@ -481,6 +482,7 @@ int lp_chain_create(int rank, int P, int channels, int slots, int tile, lp_chain
     ch->tile = tile;
     ch->device = dev;
     ch->bytes = layout_of(channels, slots, tile).bytes;
+    ch->spin_limit = 1ull << 28;  // ~a minute of polling: ranks of different processes start at different times
     cudaError_t e = cudaMalloc(&ch->base, ch->bytes);
     if (e == cudaSuccess) e = cudaMemset(ch->base, 0, ch->bytes);
     if (e == cudaSuccess) e = cudaDeviceSynchronize();
@@ -547,6 +549,12 @@ int lp_chain_connect_ptrs(lp_chain *ch, void *up_endpoint, void *down_endpoint) 
 
 void *lp_chain_endpoint(lp_chain *ch) { return ch ? ch->base : nullptr; }
 
+int lp_chain_set_timeout(lp_chain *ch, unsigned long long polls) {
+    if (ch == nullptr || polls == 0) return LP_ERR_INVALID_ARG;
+    ch->spin_limit = polls;
+    return LP_OK;
+}
+
 int lp_chain_destroy(lp_chain *ch) {
     if (ch == nullptr) return LP_ERR_INVALID_ARG;
     cudaDeviceSynchronize();
@@ -602,7 +610,7 @@ static int chain_run_rank(lp_chain *ch, int op, float *buf, float *out, const fl
     L.code = code;
     L.lr = lr;
     L.invP = 1.0f / (float)ch->P;  // one RN division on the host (U7)
-    L.spin_limit = 1ull << 28;  // ~a minute of polling: ranks of different processes start at different times
+    L.spin_limit = ch->spin_limit;
     L.part = chain_partition(n, block, ch->tile);
     L.tile = (uint32_t)ch->tile;
     fill_rank(L.rank[0], layout_of(ch->C, ch->S, ch->tile), buf, out, w_in, ch->base, ch->peer_up, ch->peer_down, role);

@@ -183,6 +183,36 @@ def test_chain_argument_errors():
     assert L.lp_chain_emulate(lp.OP_ALLREDUCE, arr, 2, 0, 16, 0, 0, 0, 0, 0, s) == lp.LP_OK                 # n == 0
 
 
+def test_chain_real_entry_points_rank_after_rank(oracle):
+    """The REAL per-rank entry points (lp_chain_create / connect_ptrs / run: the launch a rank of a multi-GPU job makes,
+    not the cooperative emulation) on P endpoints of this one GPU.  Kernels that wait for each other may not run here as
+    separate launches, so only collectives whose data flows one way are run, rank after rank in chain order, with rings
+    that never wrap within a call (tiles per channel <= slots): every wait of a kernel is then already satisfied when
+    it starts, and the counters -- which are never reset -- carry over from call to call."""
+    P, C, S, tile = 4, 2, 8, 4096
+    n = 50_001                                            # 13 tiles over 2 channels: 7 <= 8 slots
+    chains = [lp.Chain(r, P, channels=C, slots=S, tile=tile) for r in range(P)]
+    for r, ch in enumerate(chains):
+        ch.set_timeout(1 << 22)
+        ch.connect_ptrs(chains[(r + 1) % P].endpoint(), chains[(r - 1) % P].endpoint())
+    src = inputs.rank_vectors([37, 0], P, n, "uniform")
+    host = [a.copy() for a in src]
+    dev = up(src)
+    calls = [("broadcast", 0), ("reduce", P - 1), ("broadcast", 2), ("reduce", P - 1), ("broadcast", 3), ("broadcast", 1)]
+    for op, root in calls:
+        run_oracle(oracle, op, host, root, oracle.RED_SUM)
+        order = [(root + j) % P for j in range(P)] if op == "broadcast" else list(range(P))
+        for r in order:
+            chains[r].run(OPS[op], dev[r], block=tile, root=root)
+            torch.cuda.synchronize()                      # rank after rank: nothing runs beside anything
+    got = down(dev)
+    assert all(ch.error() == 0 for ch in chains)
+    for r in range(P):
+        assert got[r].tobytes() == host[r].tobytes(), r
+    for ch in chains:
+        ch.destroy()
+
+
 def test_chain_endpoint_of_one_rank(oracle):
     """The real entry points on the one GPU there is: create / handle / connect-to-self / run with P = 1 (a no-op by
     definition), and a P = 2 endpoint refuses to run before it is connected."""
