@@ -13,7 +13,8 @@ lp_allreduce_host with pinned HOST buffers (H2D + kernel + D2H inside the timed 
 `detail` carries the other BASELINE.json configs, driver-measured in the same run: configs[3] from 64 MB up at
 P = 2, 3, 4, 5, 6, 8, 16 (LP vs MST vs BE, three collectives, with the HBM ceiling of the same read : write mix from a
 plain streaming kernel beside every cell), configs[4] (P=16, 138 M), configs[2] (fused BSP-SGD step, 100 iterations),
-the other ops / variants / block sizes of configs[1], and the pure-stream HBM ceilings.  Prints ONE JSON line (rank 0).
+the other ops / variants / block sizes of configs[1], the pure-stream HBM ceilings, the typed collectives (f16 / bf16 / f64 at
+the same bytes per rank as f32) and the multi-GPU chain's one-GPU emulation.  Prints ONE JSON line (rank 0).
 """
 from __future__ import annotations
 
