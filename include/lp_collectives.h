@@ -184,11 +184,21 @@ LP_API int lp_allreduce_op(float *const *bufs, int P, size_t n, size_t block, in
  * operation IN THE ELEMENT TYPE (U21), chain order whatever the root (U4): bit-exact to that definition (NaN results are
  * NaNs; their payload bits are the hardware's).  Every LP variant takes every type.  16-bit blocks are rounded up to an
  * even number of elements (results never depend on the block).  LP_DT_F32 is the plain call.  Unknown dtype or
- * reduce_op: LP_ERR_INVALID_ARG.  The SGD steps, slice lists, plans and the MST / BE baselines stay fp32 (the paper's). */
+ * reduce_op: LP_ERR_INVALID_ARG.  Slice lists: lp_*_segments_dt; plans: lp_plan_desc.dtype.  The SGD steps and the
+ * MST / BE baselines stay fp32 (the paper's). */
 LP_API int lp_broadcast_dt(void *const *bufs, int P, size_t n, size_t block, int root, int dtype, void *cuda_stream);
 LP_API int lp_reduce_dt(void *const *bufs, int P, size_t n, size_t block, int root, int dtype, int reduce_op,
                         void *cuda_stream);
 LP_API int lp_allreduce_dt(void *const *bufs, int P, size_t n, size_t block, int dtype, int reduce_op, void *cuda_stream);
+/* The layer-wise calls (Alg. 1, below) on vectors of element type `dtype`: seg_off / seg_len count elements of that type.
+ * A slice of 16-bit elements must start at an even element offset (on a 4-byte word; else LP_ERR_INVALID_ARG); any
+ * length is fine. */
+LP_API int lp_broadcast_segments_dt(void *const *bufs, int P, size_t n, const size_t *seg_off, const size_t *seg_len,
+                                    int n_seg, size_t block, int root, int dtype, void *cuda_stream);
+LP_API int lp_reduce_segments_dt(void *const *bufs, int P, size_t n, const size_t *seg_off, const size_t *seg_len, int n_seg,
+                                 size_t block, int root, int dtype, int reduce_op, void *cuda_stream);
+LP_API int lp_allreduce_segments_dt(void *const *bufs, int P, size_t n, const size_t *seg_off, const size_t *seg_len,
+                                    int n_seg, size_t block, int dtype, int reduce_op, void *cuda_stream);
 /* bytes per element of LP_DT_*; 0 for an unknown type */
 LP_API size_t lp_dtype_size(int dtype);
 
@@ -446,6 +456,8 @@ typedef struct lp_plan_desc {
     size_t block;               /* LP block in elements, 0 = library chooses */
     int variant;                /* LP_VARIANT_* */
     int tuning[16];             /* indexed by LP_TUNE_*; 0 = library default */
+    int dtype;                  /* LP_DT_*: element type of the vectors (n, block in elements of it); LP_DT_F32 for the SGD
+                                   steps.  lp_plan_run then takes the P pointers as they are (cast to float *const *) */
 } lp_plan_desc;
 /* Fills *desc with defaults: allreduce, sum, variant LP_VARIANT_AUTO, block 0, tuning all 0; P, n left 0. */
 LP_API int lp_plan_desc_init(lp_plan_desc *desc);

@@ -55,7 +55,7 @@ class ChainRole(ctypes.Structure):
 class PlanDesc(ctypes.Structure):
     _fields_ = [("op", ctypes.c_int), ("reduce_op", ctypes.c_int), ("P", ctypes.c_int), ("root", ctypes.c_int),
                 ("n", ctypes.c_size_t), ("block", ctypes.c_size_t), ("variant", ctypes.c_int),
-                ("tuning", ctypes.c_int * 16)]
+                ("tuning", ctypes.c_int * 16), ("dtype", ctypes.c_int)]
 
 
 _lib = None
@@ -107,6 +107,9 @@ def lib() -> ctypes.CDLL:
     L.lp_broadcast_dt.argtypes = [pp, i32, sz, sz, i32, i32, vp]
     L.lp_reduce_dt.argtypes = [pp, i32, sz, sz, i32, i32, i32, vp]
     L.lp_allreduce_dt.argtypes = [pp, i32, sz, sz, i32, i32, vp]
+    L.lp_broadcast_segments_dt.argtypes = [pp, i32, sz, psz, psz, i32, sz, i32, i32, vp]
+    L.lp_reduce_segments_dt.argtypes = [pp, i32, sz, psz, psz, i32, sz, i32, i32, i32, vp]
+    L.lp_allreduce_segments_dt.argtypes = [pp, i32, sz, psz, psz, i32, sz, i32, i32, vp]
     L.lp_dtype_size.argtypes = [i32]
     L.lp_dtype_size.restype = sz
     L.lp_chain_plan.argtypes = [i32, i32, i32, i32, ctypes.POINTER(ChainRole)]
@@ -439,18 +442,22 @@ class Plan:
     """lp_plan handle: `Plan(op, P, n, block=0, root=0, reduce_op=REDUCE_SUM, variant=VARIANT_AUTO, tuning={key: value})`;
     `run(bufs, ...)` enqueues it on a stream.  Immutable; usable from several threads at once."""
 
-    def __init__(self, op, P, n, block=0, root=0, reduce_op=REDUCE_SUM, variant=VARIANT_AUTO, tuning=None):
+    def __init__(self, op, P, n, block=0, root=0, reduce_op=REDUCE_SUM, variant=VARIANT_AUTO, tuning=None, dtype=DT_F32):
         d = PlanDesc()
         _check(lib().lp_plan_desc_init(ctypes.byref(d)), "lp_plan_desc_init")
         d.op, d.reduce_op, d.P, d.root, d.n, d.block, d.variant = op, reduce_op, P, root, n, block, variant
+        d.dtype = dtype
         for k, v in (tuning or {}).items():
             d.tuning[k] = v
         h = ctypes.c_void_p()
         _check(lib().lp_plan_create(ctypes.byref(d), ctypes.byref(h)), "lp_plan_create")
-        self.handle, self.op, self.P, self.n = h, op, P, n
+        self.handle, self.op, self.P, self.n, self.dtype = h, op, P, n, dtype
 
     def _ranks(self, bufs):
-        arr, n = _dev_ptrs(bufs)
+        if self.dtype != DT_F32:
+            arr, n, _ = _dev_ptrs_dt(bufs, self.dtype)
+        else:
+            arr, n = _dev_ptrs(bufs)
         if n != self.n or len(bufs) != self.P:
             raise ValueError("buffers do not match the plan's P and n")
         return arr
@@ -534,6 +541,27 @@ def lp_allreduce_segments(bufs, segments, block, stream=None):
     sg = _segments(segments)
     _check(lib().lp_allreduce_segments(arr, len(bufs), n, sg.off, sg.len, sg.k, block, _stream_ptr(stream)),
            "lp_allreduce_segments")
+
+
+def lp_broadcast_segments_dt(bufs, segments, block, root=0, dtype=None, stream=None):
+    arr, n, dt = _dev_ptrs_dt(bufs, dtype)
+    sg = _segments(segments)
+    _check(lib().lp_broadcast_segments_dt(arr, len(bufs), n, sg.off, sg.len, sg.k, block, root, dt, _stream_ptr(stream)),
+           "lp_broadcast_segments_dt")
+
+
+def lp_reduce_segments_dt(bufs, segments, block, root=0, dtype=None, reduce_op=REDUCE_SUM, stream=None):
+    arr, n, dt = _dev_ptrs_dt(bufs, dtype)
+    sg = _segments(segments)
+    _check(lib().lp_reduce_segments_dt(arr, len(bufs), n, sg.off, sg.len, sg.k, block, root, dt, reduce_op,
+                                       _stream_ptr(stream)), "lp_reduce_segments_dt")
+
+
+def lp_allreduce_segments_dt(bufs, segments, block, dtype=None, reduce_op=REDUCE_SUM, stream=None):
+    arr, n, dt = _dev_ptrs_dt(bufs, dtype)
+    sg = _segments(segments)
+    _check(lib().lp_allreduce_segments_dt(arr, len(bufs), n, sg.off, sg.len, sg.k, block, dt, reduce_op,
+                                          _stream_ptr(stream)), "lp_allreduce_segments_dt")
 
 
 # ---- lp_comm: Alg. 1's non-blocking collectives (a library-owned high-priority stream) --------------------

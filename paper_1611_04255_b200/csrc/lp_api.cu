@@ -475,31 +475,41 @@ size_t dtype_bytes(int dtype) { return dtype == LP_DT_F64 ? 8 : (dtype == LP_DT_
 // an f64 element is two words, two f16 / bf16 elements share one.  n and block arrive in ELEMENTS; 16-bit blocks are
 // rounded up to whole words (results never depend on the block), and the odd last element of a 16-bit vector, which
 // fills only half a word, is folded by a one-thread kernel behind the main launch.
-int run_device_dt(int op, int red_op, int dtype, void *const *bufs, int P, size_t n, size_t block, int root,
-                  void *cuda_stream) {
+// n and block of a typed call in 4-byte words (block == 0, "the library chooses", stays 0); *odd: a 16-bit vector
+// ends in half a word.
+void typed_words(int dtype, size_t n, size_t block, size_t &n_words, size_t &block_words, bool &odd) {
+    odd = false;
+    if (dtype == LP_DT_F64) {
+        n_words = 2 * n;
+        block_words = block > (~(size_t)0) / 2 ? ~(size_t)1 : 2 * block;
+    } else if (dtype == LP_DT_F32) {
+        n_words = n;
+        block_words = block;
+    } else {
+        n_words = n / 2;
+        odd = (n & 1u) != 0;
+        block_words = block / 2 + (block & 1u);
+    }
+}
+
+int run_device_dt(const LpCallCfg *cfg_in, int op, int red_op, int dtype, void *const *bufs, int P, size_t n, size_t block,
+                  int root, void *cuda_stream) {
     if (dtype < LP_DT_F32 || dtype > LP_DT_F64) return LP_ERR_INVALID_ARG;
     float *const *fb = reinterpret_cast<float *const *>(bufs);
     if (dtype == LP_DT_F32)
-        return run_device(nullptr, op, red_op, fb, nullptr, nullptr, P, n, block, root, 0.f, 0.f, cuda_stream);
+        return run_device(cfg_in, op, red_op, fb, nullptr, nullptr, P, n, block, root, 0.f, 0.f, cuda_stream);
     if (is_sgd(op)) return LP_ERR_INVALID_ARG;  // the SGD steps are the paper's fp32 solver
     int rc = validate(op, red_op, fb, nullptr, nullptr, P, n, root, dtype_bytes(dtype));
     if (rc != LP_OK) return rc;
     if (n > (~(size_t)0) / 8) return LP_ERR_INVALID_ARG;
     LpCallCfg cfg;
     int sms;
-    rc = begin_call(nullptr, cfg, sms);
+    rc = begin_call(cfg_in, cfg, sms);
     if (rc != LP_OK) return rc;
     if (cfg.variant == LP_VARIANT_CLUSTER && P > 16) return LP_ERR_UNSUPPORTED;
-    size_t n_words, block_words;  // block == 0 (the library chooses) stays 0
-    bool odd = false;
-    if (dtype == LP_DT_F64) {
-        n_words = 2 * n;
-        block_words = block > (~(size_t)0) / 2 ? ~(size_t)1 : 2 * block;
-    } else {
-        n_words = n / 2;
-        odd = (n & 1u) != 0;
-        block_words = block / 2 + (block & 1u);
-    }
+    size_t n_words, block_words;
+    bool odd;
+    typed_words(dtype, n, block, n_words, block_words, odd);
     cudaStream_t st = (cudaStream_t)cuda_stream;
     LpArgs a;
     rc = plan_and_run(cfg, op, red_op, fb, nullptr, nullptr, P, n_words, block_words, root, 0.f, 0.f, sms, nullptr, false, st,
@@ -537,10 +547,12 @@ int run_alg2(float *const *grads, float *const *weights, float *velocity, int P,
 // each slice its own LP message, tiles handed out slice by slice in list order; LP_MAX_SEGS slices per launch.
 int run_segments(const LpCallCfg *cfg_in, int op, int red_op, float *const *bufs, float *const *weights, int P, size_t n,
                  const size_t *seg_off, const size_t *seg_len, int n_seg, size_t block, int root, float lr,
-                 void *cuda_stream) {
+                 void *cuda_stream, int dtype = LP_DT_F32) {
     if (op == LP_OP_BSP_SGD_MOM) return LP_ERR_INVALID_ARG;
-    int rc = validate(op, red_op, bufs, weights, nullptr, P, n, root);
+    if (dtype < LP_DT_F32 || dtype > LP_DT_F64 || (dtype != LP_DT_F32 && is_sgd(op))) return LP_ERR_INVALID_ARG;
+    int rc = validate(op, red_op, bufs, weights, nullptr, P, n, root, dtype_bytes(dtype));
     if (rc != LP_OK) return rc;
+    const bool half = dtype == LP_DT_F16 || dtype == LP_DT_BF16;
     if (n_seg < 0 || n_seg > LP_MAX_SEGMENTS || (n_seg > 0 && (seg_off == nullptr || seg_len == nullptr)))
         return LP_ERR_INVALID_ARG;
     // slices inside [0, n) and pairwise disjoint (an in-place allreduce of overlapping slices would sum twice)
@@ -548,6 +560,7 @@ int run_segments(const LpCallCfg *cfg_in, int op, int red_op, float *const *bufs
     sorted.reserve((size_t)n_seg);
     for (int s = 0; s < n_seg; ++s) {
         if (seg_off[s] > n || seg_len[s] > n - seg_off[s]) return LP_ERR_INVALID_ARG;
+        if (half && seg_len[s] && (seg_off[s] & 1u)) return LP_ERR_INVALID_ARG;  // a 16-bit slice starts on a 4-byte word
         if (seg_len[s]) sorted.emplace_back(seg_off[s], seg_len[s]);
     }
     std::sort(sorted.begin(), sorted.end());
@@ -558,20 +571,39 @@ int run_segments(const LpCallCfg *cfg_in, int op, int red_op, float *const *bufs
     rc = begin_call(cfg_in, cfg, sms);
     if (rc != LP_OK) return rc;
     if (cfg.variant == LP_VARIANT_CLUSTER && P > 16) return LP_ERR_UNSUPPORTED;
+    // typed slices: offsets and lengths in 4-byte words (LpArgs::dtype); the odd last element of a 16-bit slice is
+    // folded by the one-thread tail kernel behind the launch that carries the slice
+    size_t n_words, block_words;
+    bool odd_n;
+    typed_words(dtype, n, block, n_words, block_words, odd_n);
+    if (odd_n) ++n_words;  // the span of the vectors, for the stream-chaining ranges
+    const size_t wmul = dtype == LP_DT_F64 ? 2 : 1, wdiv = half ? 2 : 1;
     size_t off[LP_MAX_SEGS], len[LP_MAX_SEGS];
+    std::vector<uint64_t> tails;
     int m = 0;
     for (int s = 0; s <= n_seg; ++s) {
         if (s < n_seg && seg_len[s] > 0) {  // list order is kept: earlier slices finish first
-            off[m] = seg_off[s];
-            len[m] = seg_len[s];
-            ++m;
+            if (half && (seg_len[s] & 1u)) tails.push_back((uint64_t)(seg_off[s] + seg_len[s] - 1));
+            if (seg_len[s] / wdiv > 0) {
+                off[m] = seg_off[s] * wmul / wdiv;
+                len[m] = seg_len[s] * wmul / wdiv;
+                ++m;
+            }
         }
         if (m == LP_MAX_SEGS || (s == n_seg && m > 0)) {
             const SegList sl{off, len, m};
-            rc = plan_and_run(cfg, op, red_op, bufs, weights, nullptr, P, n, block, root, lr, 0.f, sms, nullptr, false,
-                              (cudaStream_t)cuda_stream, &sl);
+            rc = plan_and_run(cfg, op, red_op, bufs, weights, nullptr, P, n_words, block_words, root, lr, 0.f, sms, nullptr,
+                              false, (cudaStream_t)cuda_stream, &sl, dtype);
             if (rc != LP_OK) return rc;
             m = 0;
+        }
+    }
+    if (!tails.empty() && P > 1) {
+        LpArgs a;
+        fill_args(a, op, red_op, bufs, nullptr, nullptr, P, root, 0.f, 0.f, cfg.tuning, dtype);
+        for (uint64_t e : tails) {
+            const cudaError_t ce = lp_tail16_launch(a, e, (cudaStream_t)cuda_stream, cfg.tuning.v[LP_TUNE_NO_PDL] == 0);
+            if (ce != cudaSuccess) return cuda_fail(ce, "16-bit tail element");
         }
     }
     return LP_OK;
@@ -866,13 +898,28 @@ int lp_allreduce_op(float *const *bufs, int P, size_t n, size_t block, int reduc
     return run_device(nullptr, LP_OP_ALLREDUCE, reduce_op, bufs, nullptr, nullptr, P, n, block, 0, 0.f, 0.f, cuda_stream);
 }
 int lp_broadcast_dt(void *const *bufs, int P, size_t n, size_t block, int root, int dtype, void *cuda_stream) {
-    return run_device_dt(LP_OP_BROADCAST, LP_REDUCE_SUM, dtype, bufs, P, n, block, root, cuda_stream);
+    return run_device_dt(nullptr, LP_OP_BROADCAST, LP_REDUCE_SUM, dtype, bufs, P, n, block, root, cuda_stream);
 }
 int lp_reduce_dt(void *const *bufs, int P, size_t n, size_t block, int root, int dtype, int reduce_op, void *cuda_stream) {
-    return run_device_dt(LP_OP_REDUCE, reduce_op, dtype, bufs, P, n, block, root, cuda_stream);
+    return run_device_dt(nullptr, LP_OP_REDUCE, reduce_op, dtype, bufs, P, n, block, root, cuda_stream);
 }
 int lp_allreduce_dt(void *const *bufs, int P, size_t n, size_t block, int dtype, int reduce_op, void *cuda_stream) {
-    return run_device_dt(LP_OP_ALLREDUCE, reduce_op, dtype, bufs, P, n, block, 0, cuda_stream);
+    return run_device_dt(nullptr, LP_OP_ALLREDUCE, reduce_op, dtype, bufs, P, n, block, 0, cuda_stream);
+}
+int lp_broadcast_segments_dt(void *const *bufs, int P, size_t n, const size_t *seg_off, const size_t *seg_len, int n_seg,
+                             size_t block, int root, int dtype, void *cuda_stream) {
+    return run_segments(nullptr, LP_OP_BROADCAST, LP_REDUCE_SUM, reinterpret_cast<float *const *>(bufs), nullptr, P, n, seg_off,
+                        seg_len, n_seg, block, root, 0.f, cuda_stream, dtype);
+}
+int lp_reduce_segments_dt(void *const *bufs, int P, size_t n, const size_t *seg_off, const size_t *seg_len, int n_seg,
+                          size_t block, int root, int dtype, int reduce_op, void *cuda_stream) {
+    return run_segments(nullptr, LP_OP_REDUCE, reduce_op, reinterpret_cast<float *const *>(bufs), nullptr, P, n, seg_off,
+                        seg_len, n_seg, block, root, 0.f, cuda_stream, dtype);
+}
+int lp_allreduce_segments_dt(void *const *bufs, int P, size_t n, const size_t *seg_off, const size_t *seg_len, int n_seg,
+                             size_t block, int dtype, int reduce_op, void *cuda_stream) {
+    return run_segments(nullptr, LP_OP_ALLREDUCE, reduce_op, reinterpret_cast<float *const *>(bufs), nullptr, P, n, seg_off,
+                        seg_len, n_seg, block, 0, 0.f, cuda_stream, dtype);
 }
 size_t lp_dtype_size(int dtype) { return dtype < LP_DT_F32 || dtype > LP_DT_F64 ? 0 : dtype_bytes(dtype); }
 int lp_bsp_sgd_step(float *const *grads, float *const *weights, int P, size_t n, size_t block, int root, float lr,
@@ -957,6 +1004,7 @@ int lp_plan_desc_init(lp_plan_desc *desc) {
     desc->op = LP_OP_ALLREDUCE;
     desc->reduce_op = LP_REDUCE_SUM;
     desc->variant = LP_VARIANT_AUTO;
+    desc->dtype = LP_DT_F32;
     return LP_OK;
 }
 
@@ -968,6 +1016,8 @@ int lp_plan_create(const lp_plan_desc *desc, lp_plan **plan) {
     int rc = validate_shape(desc->op, desc->reduce_op, desc->P, root);
     if (rc != LP_OK) return rc;
     if (desc->variant < LP_VARIANT_PIPELINE || desc->variant > LP_VARIANT_AUTO) return LP_ERR_INVALID_ARG;
+    if (desc->dtype < LP_DT_F32 || desc->dtype > LP_DT_F64 || (desc->dtype != LP_DT_F32 && is_sgd(desc->op)))
+        return LP_ERR_INVALID_ARG;
     for (int k = 0; k < 16; ++k) {
         if (k >= LP_TUNE_COUNT) {
             if (desc->tuning[k] != 0) return LP_ERR_INVALID_ARG;
@@ -998,6 +1048,9 @@ int lp_plan_run(const lp_plan *plan, float *const *bufs, float *const *weights, 
     const lp_plan_desc &d = plan->d;
     if (!is_sgd(d.op) && (weights != nullptr || velocity != nullptr)) return LP_ERR_INVALID_ARG;
     if (d.op == LP_OP_BSP_SGD && velocity != nullptr) return LP_ERR_INVALID_ARG;
+    if (d.dtype != LP_DT_F32)  // bufs then point at elements of the plan's type
+        return run_device_dt(&plan->cfg, d.op, d.reduce_op, d.dtype, reinterpret_cast<void *const *>(bufs), d.P, d.n, d.block,
+                             d.root, cuda_stream);
     return run_device(&plan->cfg, d.op, d.reduce_op, bufs, weights, velocity, d.P, d.n, d.block, d.root, lr, mu, cuda_stream);
 }
 
@@ -1007,7 +1060,7 @@ int lp_plan_run_segments(const lp_plan *plan, float *const *bufs, float *const *
     const lp_plan_desc &d = plan->d;
     if (d.op == LP_OP_BSP_SGD ? weights == nullptr : weights != nullptr) return LP_ERR_INVALID_ARG;
     return run_segments(&plan->cfg, d.op, d.reduce_op, bufs, weights, d.P, d.n, seg_off, seg_len, n_seg, d.block, d.root, lr,
-                        cuda_stream);
+                        cuda_stream, d.dtype);
 }
 
 int lp_plan_get_info(const lp_plan *plan, lp_plan_info *out) {
@@ -1020,8 +1073,11 @@ int lp_plan_get_info(const lp_plan *plan, lp_plan_info *out) {
     if (sms <= 0) sms = 148;  // planning works without a device: a B200 has 148 SMs
     memset(out, 0, sizeof(*out));
     const lp_plan_desc &d = plan->d;
-    return plan_and_run(plan->cfg, d.op, d.reduce_op, nullptr, nullptr, nullptr, d.P, d.n, d.block, d.root, 0.f, 0.f, sms, out,
-                        true, nullptr);
+    size_t n_words, block_words;  // a typed plan is laid out in 4-byte words (tile_elems, block then count words)
+    bool odd;
+    typed_words(d.dtype, d.n, d.block, n_words, block_words, odd);
+    return plan_and_run(plan->cfg, d.op, d.reduce_op, nullptr, nullptr, nullptr, d.P, n_words, block_words, d.root, 0.f, 0.f,
+                        sms, out, true, nullptr, nullptr, d.dtype);
 }
 
 int lp_hbm_probe(float *const *bufs, int n_read, int n_write, size_t n, void *cuda_stream) {

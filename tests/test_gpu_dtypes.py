@@ -165,6 +165,82 @@ def test_typed_large_message_pipeline_and_direct(oracle, dt):
             assert same_typed(got[r], want[r], dt), (variant, r)
 
 
+def _oracle_slices(oracle, op, host, segs, dt, red, root):
+    """The definition of a layer-wise call: the whole-message collective on every slice (Alg. 1), nothing elsewhere."""
+    for off, ln in segs:
+        if ln == 0:
+            continue
+        views = [h[off:off + ln] for h in host]           # contiguous views: the oracle works in place on them
+        run_oracle(oracle, op, views, dt, red=red, root=root)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("dt", DTS)
+def test_typed_slice_lists(oracle, variant, dt):
+    """Layer-wise collectives (Alg. 1) on typed vectors: slices of any length (odd ones end in half a word for the
+    16-bit types), empty slices, a slice of one element, gaps that must stay untouched."""
+    P, n = 4, 120_011
+    segs = [(10, 1001), (2000, 0), (5000, 1), (7002, 30_000), (40_000, 4097), (60_000, 2), (100_000, 20_011)]
+    lp.lp_set_variant(variant)
+    src = inputs.typed_rank_vectors([25, dt], P, n, dt, "sum")
+    for op, red in (("allreduce", SUM), ("reduce", PROD), ("broadcast", SUM)):
+        want = [a.copy() for a in src]
+        _oracle_slices(oracle, op, want, segs, dt, red, root=1)
+        dev = up(src, dt)
+        if op == "allreduce":
+            lp.lp_allreduce_segments_dt(dev, segs, 4096, dtype=dt, reduce_op=red)
+        elif op == "reduce":
+            lp.lp_reduce_segments_dt(dev, segs, 4096, root=1, dtype=dt, reduce_op=red)
+        else:
+            lp.lp_broadcast_segments_dt(dev, segs, 4096, root=1, dtype=dt)
+        got = down(dev, dt)
+        for r in range(P):
+            assert same_typed(got[r], want[r], dt), (op, variant, inputs.DT_NAMES[dt], r)
+
+
+def test_typed_slices_must_start_on_a_word():
+    dev = [torch.zeros(64, dtype=torch.float16, device="cuda") for _ in range(2)]
+    with pytest.raises(lp.LpError) as e:
+        lp.lp_allreduce_segments_dt(dev, [(3, 8)], 16)
+    assert e.value.status == lp.LP_ERR_INVALID_ARG
+    lp.lp_allreduce_segments_dt(dev, [(4, 7)], 16)                               # even offset, odd length: fine
+    dev64 = [torch.zeros(64, dtype=torch.float64, device="cuda") for _ in range(2)]
+    lp.lp_allreduce_segments_dt(dev64, [(3, 8)], 16)                             # f64: any offset
+
+
+@pytest.mark.parametrize("dt", DTS)
+def test_typed_plans(oracle, dt):
+    """A plan fixes the element type too: two typed plans with different variants and tunings, one confined to 32 CTAs."""
+    P, n = 6, 300_003
+    src = inputs.typed_rank_vectors([26, dt], P, n, dt, "sum")
+    want = [a.copy() for a in src]
+    oracle.allreduce_dt(want, dt)
+    plans = [lp.Plan(lp.OP_ALLREDUCE, P, n, block=8192, variant=lp.VARIANT_PIPELINE, dtype=dt,
+                     tuning={lp.TUNE_GRID_LIMIT: 32}),
+             lp.Plan(lp.OP_ALLREDUCE, P, n, block=0, variant=lp.VARIANT_DIRECT, dtype=dt)]
+    for plan in plans:
+        dev = up(src, dt)
+        plan.run(dev)
+        got = down(dev, dt)
+        for r in range(P):
+            assert same_typed(got[r], want[r], dt), (inputs.DT_NAMES[dt], r)
+        assert plan.info()["n_tiles"] > 0
+        plan.close()
+    with pytest.raises(lp.LpError):
+        lp.Plan(lp.OP_BSP_SGD, P, n, dtype=dt)                                    # the SGD steps are fp32
+    segs = [(0, 1001), (2000, 50_001)]
+    plan = lp.Plan(lp.OP_REDUCE, P, n, block=4096, root=2, reduce_op=PROD, dtype=dt)
+    psrc = inputs.typed_rank_vectors([27, dt], P, n, dt, "prod")
+    want = [a.copy() for a in psrc]
+    _oracle_slices(oracle, "reduce", want, segs, dt, PROD, root=2)
+    dev = up(psrc, dt)
+    plan.run_segments(dev, segs)
+    got = down(dev, dt)
+    for r in range(P):
+        assert same_typed(got[r], want[r], dt), (inputs.DT_NAMES[dt], r)
+    plan.close()
+
+
 def test_typed_f32_is_the_plain_call(oracle):
     P, n = 6, 70_001
     src = inputs.rank_vectors([24, 0], P, n, "uniform")
