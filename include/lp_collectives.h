@@ -311,7 +311,9 @@ LP_API int lp_be_allreduce_op(float *const *bufs, int P, size_t n, int reduce_op
  *       ALLREDUCE on its vector buf (n floats, 16-byte aligned, in place; same semantics and the same bits as
  *       lp_broadcast / lp_reduce_op / lp_allreduce_op over P virtual ranks).  Every rank calls it with the same
  *       arguments, in the same order as its other chain collectives, on one stream per endpoint.  `block` is rounded
- *       up to a multiple of 4 elements (0 = one tile); a block is moved in pieces of at most one tile.
+ *       up to a multiple of 4 elements and moved in pieces of at most one tile; 0 = the library chooses: one tile for
+ *       long messages, for short ones the power of two (>= 4096) that still gives every channel about four blocks, so
+ *       that the chain fills after a small block (the fill term of the pipeline is (p - 1) b).
  *   lp_chain_error(ch, &e)   synchronises; e != 0: a wait gave up (a neighbour never arrived) and the result is void.
  * lp_chain_plan is the host-only part: what `rank` does in (op, P, root) -- its ring neighbours and which of the steps
  * load / receive / store / send up / send down its forward and return CTAs take.  No device needed.

@@ -94,21 +94,30 @@ __device__ __forceinline__ float ld_ring1(const float *p) {
     return v;
 }
 
-// Thread 0 polls *flag until it reaches `want`, then everybody passes the barrier.  Returns false (for every thread)
-// when the poll gave up or another CTA of this rank already failed: the caller leaves its loop.
-__device__ __forceinline__ bool wait_counter(const unsigned long long *flag, unsigned long long want, int *error, int *s_ok,
-                                             unsigned long long spin_limit) {
+// Thread 0 polls up to three counters until each has reached its target (want == 0: nothing to wait for), then
+// everybody passes the barrier.  ONE acquire fence after the polls: it is what makes the data that was published
+// before the tail counter visible to the ring loads behind the barrier; the credit counters need none of their own
+// (what follows them are stores into the freed slot, and a store is never performed ahead of the load it depends on).
+// Returns false (for every thread) when a poll gave up or another CTA of this rank already failed.
+__device__ __forceinline__ bool wait_counters(const unsigned long long *f0, unsigned long long w0, const unsigned long long *f1,
+                                              unsigned long long w1, const unsigned long long *f2, unsigned long long w2,
+                                              int *error, int *s_ok, unsigned long long spin_limit) {
     if (threadIdx.x == 0) {
         int ok = 1;
-        unsigned long long spins = 0;
-        while (ld_sys(flag) < want) {
-            if (++spins > spin_limit || ((spins & 0xfffu) == 0 && *reinterpret_cast<volatile int *>(error) != 0)) {
-                ok = 0;
-                atomicCAS(error, 0, 1);
-                break;
+        const unsigned long long *f[3] = {f0, f1, f2};
+        const unsigned long long w[3] = {w0, w1, w2};
+        for (int i = 0; i < 3 && ok; ++i) {
+            if (w[i] == 0) continue;
+            unsigned long long spins = 0;
+            while (ld_sys(f[i]) < w[i]) {
+                if (++spins > spin_limit || ((spins & 0xfffu) == 0 && *reinterpret_cast<volatile int *>(error) != 0)) {
+                    ok = 0;
+                    atomicCAS(error, 0, 1);
+                    break;
+                }
             }
         }
-        fence_sys();  // acquire: the data published before the counter is visible to loads after the barrier
+        if (w0) fence_sys();  // f0 is the tail counter of a receive ring
         *s_ok = ok;
     }
     __syncthreads();
@@ -189,9 +198,9 @@ __device__ void chain_forward(const LpChainRank &A, const LpChainLaunch &L, int 
         uint32_t len;
         lp_tile_range(L.part, t, off, len);
         // every flag this tile needs, then the tile itself without a single barrier
-        if (A.f_recv) ok = wait_counter(my + F_FWD_TAIL, recv + 1, A.error, s_ok, L.spin_limit);
-        if (ok && A.f_send_up) ok = wait_counter(my + F_UP_CREDIT, slot_free_at(sent_up, L.S), A.error, s_ok, L.spin_limit);
-        if (ok && A.f_send_down) ok = wait_counter(my + F_DOWN_CREDIT, slot_free_at(sent_down, L.S), A.error, s_ok, L.spin_limit);
+        ok = wait_counters(my + F_FWD_TAIL, A.f_recv ? recv + 1 : 0, my + F_UP_CREDIT,
+                           A.f_send_up ? slot_free_at(sent_up, L.S) : 0, my + F_DOWN_CREDIT,
+                           A.f_send_down ? slot_free_at(sent_down, L.S) : 0, A.error, s_ok, L.spin_limit);
         if (!ok) break;
         const float *in_slot = A.fwd_ring + ring_c + (size_t)(recv % (unsigned)L.S) * L.tile;
         float *up_slot = A.up_fwd_ring + ring_c + (size_t)(sent_up % (unsigned)L.S) * L.tile;
@@ -242,8 +251,8 @@ __device__ void chain_return(const LpChainRank &A, const LpChainLaunch &L, int c
         uint64_t off;
         uint32_t len;
         lp_tile_range(L.part, t, off, len);
-        ok = wait_counter(my + F_BWD_TAIL, recv + 1, A.error, s_ok, L.spin_limit);
-        if (ok && A.r_send_down) ok = wait_counter(my + F_DOWN_CREDIT, slot_free_at(sent_down, L.S), A.error, s_ok, L.spin_limit);
+        ok = wait_counters(my + F_BWD_TAIL, recv + 1, my + F_DOWN_CREDIT, A.r_send_down ? slot_free_at(sent_down, L.S) : 0,
+                           nullptr, 0, A.error, s_ok, L.spin_limit);
         if (!ok) break;
         const float *in_slot = A.bwd_ring + ring_c + (size_t)(recv % (unsigned)L.S) * L.tile;
         float *down_slot = A.down_bwd_ring + ring_c + (size_t)(sent_down % (unsigned)L.S) * L.tile;
@@ -420,9 +429,16 @@ cudaError_t launch(const LpChainLaunch &L, bool cooperative, cudaStream_t stream
 }
 
 // a1 for the chain: blocks of `block` elements rounded up to a multiple of 4 (every tile then starts on a 16-byte
-// boundary; results never depend on the block), cut into tiles of one ring slot.
-lp_partition chain_partition(size_t n, size_t block, int tile) {
-    if (block == 0) block = (size_t)tile;
+// boundary; results never depend on the block), cut into tiles of at most one ring slot.  block == 0, "the library
+// chooses": one slot for long messages; for short ones the power of two that still gives every channel about four
+// blocks (floor 4096 elements), so that the pipeline over the ranks fills after a small block instead of after a
+// whole slot -- the paper's reason for small blocks, PAPER.md:89 ((p - 1 + n/b) steps: the fill term is (p - 1) b).
+lp_partition chain_partition(size_t n, size_t block, int tile, int channels) {
+    if (block == 0) {
+        size_t b = 4096;
+        while (b < (size_t)tile && b * 4u * (size_t)channels < n) b *= 2;
+        block = b;
+    }
     if (block < ~(size_t)3) block = (block + 3) & ~(size_t)3;
     return lp_make_partition(n, block, (uint32_t)tile);
 }
@@ -611,7 +627,7 @@ static int chain_run_rank(lp_chain *ch, int op, float *buf, float *out, const fl
     L.lr = lr;
     L.invP = 1.0f / (float)ch->P;  // one RN division on the host (U7)
     L.spin_limit = ch->spin_limit;
-    L.part = chain_partition(n, block, ch->tile);
+    L.part = chain_partition(n, block, ch->tile, ch->C);
     L.tile = (uint32_t)ch->tile;
     fill_rank(L.rank[0], layout_of(ch->C, ch->S, ch->tile), buf, out, w_in, ch->base, ch->peer_up, ch->peer_down, role);
     const cudaError_t e = launch(L, false, (cudaStream_t)cuda_stream);
@@ -722,7 +738,7 @@ static int chain_emulate(int op, float *const *bufs, float *const *outs, int P, 
     L.lr = lr;
     L.invP = 1.0f / (float)P;
     L.spin_limit = 1ull << 23;  // all ranks start together here: a few seconds mean a bug
-    L.part = chain_partition(n, block, tile);
+    L.part = chain_partition(n, block, tile, channels);
     L.tile = (uint32_t)tile;
     for (int r = 0; r < P; ++r) {
         char *b = (char *)base;
