@@ -320,7 +320,9 @@ LP_API int lp_be_allreduce_op(float *const *bufs, int P, size_t n, int reduce_op
  * This build's box has ONE GPU: kernels that wait for each other cannot be run there as separate launches, so what
  * the GPU tests execute is lp_chain_emulate -- the same per-rank device code for all P ranks in ONE cooperative launch
  * of P x 2 x channels co-resident CTAs over P endpoints in this device's memory, bufs = the P virtual ranks as
- * everywhere else in this header (LP_ERR_UNSUPPORTED when that many CTAs do not fit the device). */
+ * everywhere else in this header (LP_ERR_UNSUPPORTED when that many CTAs do not fit the device).  The emulated endpoints
+ * belong to (P, geometry, stream) and are allocated on first use -- a call that would have to allocate while its stream is
+ * being captured into a CUDA graph returns LP_ERR_UNSUPPORTED (call once outside the capture first). */
 #define LP_CHAIN_HANDLE_BYTES 64
 #define LP_CHAIN_MAX_CHANNELS 64
 #define LP_CHAIN_DEFAULT_CHANNELS 64

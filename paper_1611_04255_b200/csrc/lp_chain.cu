@@ -719,6 +719,10 @@ static int chain_emulate(int op, float *const *bufs, float *const *outs, int P, 
             if (e.P == P && e.C == channels && e.S == slots && e.tile == tile && e.stream == (cudaStream_t)cuda_stream)
                 base = e.base;
         if (base == nullptr) {
+            // the endpoints of a (geometry, stream) are allocated and zeroed on first use: not under stream capture
+            cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+            if (cudaStreamIsCapturing((cudaStream_t)cuda_stream, &cap) != cudaSuccess) cudaGetLastError();
+            if (cap != cudaStreamCaptureStatusNone) return LP_ERR_UNSUPPORTED;
             cudaError_t e = cudaMalloc(&base, l.bytes * (size_t)P);
             if (e == cudaSuccess) e = cudaMemset(base, 0, l.bytes * (size_t)P);
             if (e == cudaSuccess) e = cudaDeviceSynchronize();
