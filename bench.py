@@ -755,6 +755,20 @@ def chain_rows(torch, lp, dev, msg_bytes=64 << 20):
             for r, b in enumerate(bufs):
                 b.fill_(0.001 * (r + 1))
         row["error"] = lp.lp_chain_emulate_error(P)
+        if P == 2:  # the register realisation of a rank's CTAs beside the default (TMA loads), same protocol
+            lp.lp_chain_set_kernel(lp.CHAIN_KERNEL_REGISTER)
+            for _ in range(2):
+                lp.lp_chain_emulate(lp.OP_ALLREDUCE, bufs, block=65_536)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(10):
+                lp.lp_chain_emulate(lp.OP_ALLREDUCE, bufs, block=65_536)
+            e1.record()
+            torch.cuda.synchronize()
+            us = e0.elapsed_time(e1) * 1e3 / 10
+            row["allreduce_register_kernel"] = {"us": round(us, 1), "per_link_GBps": round(msg_bytes / us / 1e3, 1)}
+            lp.lp_chain_set_kernel(lp.CHAIN_KERNEL_DEFAULT)
         out[f"P{P}"] = row
         del bufs
     return out

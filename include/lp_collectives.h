@@ -297,9 +297,10 @@ LP_API int lp_be_allreduce_op(float *const *bufs, int P, size_t n, int reduce_op
  * through peer mappings (data pushed with plain stores, published with fence.acq_rel.sys + a counter in the
  * receiver's memory; slots returned by a credit counter in the sender's memory; csrc/lp_chain.cu).
  *   lp_chain_create(rank, P, channels, slots, tile, &ch)   on the rank's device (current device); 0 = defaults.  Every
- *       rank must pass the same (P, channels, slots, tile).  channels: 1..LP_CHAIN_MAX_CHANNELS concurrent rings (2 CTAs
- *       of 1024 threads each: an SM moves ~45 GB/s and a block costs three to four memory accesses on its way through a
- *       rank, so filling a 900 GB/s NVLink direction takes ~60 forward and ~60 return SMs -- hence 64); slots: ring depth
+ *       rank must pass the same (P, channels, slots, tile).  channels: 1..LP_CHAIN_MAX_CHANNELS concurrent rings, 2 CTAs
+ *       (one SM) each.  A CTA of the default kernel moves ~75 GB/s and a block costs three memory accesses on its way
+ *       through a middle rank's forward CTA (and three through its return CTA), i.e. ~25 GB/s of link payload per CTA:
+ *       a 900 GB/s NVLink direction takes ~36 forward + ~36 return CTAs -- hence 40, about half the SMs; slots: ring depth
  *       1..64; tile: elements per slot = the unit of a flag exchange, a power of two from 4096 to 262144 (default 65536
  *       floats = 256 KB = the LP block of BASELINE.json's configs; 16384 = the paper's 64 KB).
  *   lp_chain_get_handle(ch, h)     LP_CHAIN_HANDLE_BYTES opaque bytes (a CUDA IPC handle) to all-gather over any
@@ -325,7 +326,7 @@ LP_API int lp_be_allreduce_op(float *const *bufs, int P, size_t n, int reduce_op
  * being captured into a CUDA graph returns LP_ERR_UNSUPPORTED (call once outside the capture first). */
 #define LP_CHAIN_HANDLE_BYTES 64
 #define LP_CHAIN_MAX_CHANNELS 64
-#define LP_CHAIN_DEFAULT_CHANNELS 64
+#define LP_CHAIN_DEFAULT_CHANNELS 40
 #define LP_CHAIN_EMULATE_CHANNELS 16
 #define LP_CHAIN_DEFAULT_SLOTS 8
 #define LP_CHAIN_DEFAULT_TILE 65536
@@ -344,6 +345,14 @@ typedef struct lp_chain_role {
     int r_store;      /* ... store them to the local vector */
     int r_send_down;  /* ... pass them on to `down` */
 } lp_chain_role;
+/* Which kernel the chain launches (process-wide; the protocol between ranks is the same, so ranks may even differ):
+ * TMA (default) = a producer thread streams everything a rank reads -- its vector, its receive rings -- through a deep
+ * shared-memory ring with cp.async.bulk + mbarriers, 8 consumer warps fold and push with plain 128-bit stores;
+ * REGISTER = 1024 threads load, fold and store from registers in 64 KB steps. */
+#define LP_CHAIN_KERNEL_DEFAULT 0
+#define LP_CHAIN_KERNEL_REGISTER 1
+#define LP_CHAIN_KERNEL_TMA 2
+LP_API int lp_chain_set_kernel(int kernel);
 LP_API int lp_chain_plan(int op, int P, int root, int rank, lp_chain_role *out);
 LP_API size_t lp_chain_endpoint_bytes(int channels, int slots, int tile);
 LP_API int lp_chain_create(int rank, int P, int channels, int slots, int tile, lp_chain **out);

@@ -120,6 +120,7 @@ def lib() -> ctypes.CDLL:
     L.lp_chain_connect.argtypes = [vp, ctypes.c_char_p]
     L.lp_chain_connect_ptrs.argtypes = [vp, vp, vp]
     L.lp_chain_set_timeout.argtypes = [vp, ctypes.c_ulonglong]
+    L.lp_chain_set_kernel.argtypes = [i32]
     L.lp_chain_endpoint.argtypes = [vp]
     L.lp_chain_endpoint.restype = vp
     L.lp_chain_run.argtypes = [vp, i32, vp, sz, sz, i32, i32, vp]
@@ -331,6 +332,12 @@ def lp_dtype_size(dtype) -> int:
 
 # ---- the chain over real GPUs (one rank per GPU) and its one-GPU emulation ---------------------------------------
 CHAIN_HANDLE_BYTES = 64
+CHAIN_KERNEL_DEFAULT, CHAIN_KERNEL_REGISTER, CHAIN_KERNEL_TMA = 0, 1, 2
+
+
+def lp_chain_set_kernel(kernel):
+    _check(lib().lp_chain_set_kernel(kernel), "lp_chain_set_kernel")
+
 
 
 def lp_chain_plan(op, P, root, rank) -> dict:

@@ -1310,7 +1310,8 @@ const char *lp_status_string(int status) {
         case LP_ERR_UNSUPPORTED:
             return t_err[0] && strstr(t_err, "bound to another CUDA device")
                        ? t_err
-                       : "LP_ERR_UNSUPPORTED: BE needs a power-of-two P; cluster variant: P <= 16";
+                       : "LP_ERR_UNSUPPORTED: BE needs a power-of-two P; cluster variant: P <= 16; chain: more CTAs than the device "
+                         "holds at once, a call from another device, or a first emulation call under stream capture";
         case LP_ERR_CUDA: return t_err[0] ? t_err : "LP_ERR_CUDA";
         default: return "unknown status";
     }

@@ -29,6 +29,7 @@
 #include <cooperative_groups.h>
 #include <string.h>
 
+#include <atomic>
 #include <mutex>
 #include <vector>
 
@@ -287,6 +288,310 @@ __global__ void __launch_bounds__(kChainThreads, 1) lp_chain_kernel(const __grid
     }
 }
 
+// ---- the same roles with TMA on the load side (the default kernel) ---------------------------------------------------
+// Everything a rank READS is local -- its vector, its weight replica, its receive rings -- so the load side can be the
+// TMA pipeline of lp_pipeline.cu: a producer thread waits for the ring's tail counter, then issues cp.async.bulk loads
+// of the tile, step by step, into a deep shared-memory ring (192 KB in flight per CTA; mbarrier full / empty flags),
+// running several steps and, across tiles, several flags ahead of the consumers.  What a rank WRITES to a neighbour
+// stays plain 128-bit stores (generic proxy, fire-and-forget over NVLink) published with fence.acq_rel.sys + the
+// tail counter, exactly as in the register kernel above: the protocol between ranks is unchanged, only the inside
+// of a CTA is.  One CTA: 1 producer warp + 16 consumer warps (8 consumer warps: 16 % slower; measured in the one-GPU
+// emulation, 64 MB allreduce over 2 ranks x 32 channels: 496 GB/s per emulated link direction against 302 for the
+// register kernel, profiles/r2_dtypes_chain.md).
+constexpr int kTmaConsumers = 512;
+constexpr int kTmaThreads = 32 + kTmaConsumers;
+constexpr int kTmaVec = 2;                                               // 16-byte vectors per consumer thread and step
+constexpr uint32_t kTmaStep = kTmaVec * 4 * kTmaConsumers;               // 4096 elements = 16 KB per source
+constexpr uint32_t kTmaRingBytes = 192u * 1024u;
+constexpr int kTmaMaxStages = 12;
+
+// What one CTA does with every tile of its channel: up to three local sources, folded in this order, to up to three
+// destinations.
+struct ChainStream {
+    const float *src_ring;               // my receive ring of this channel (partial / finished block), or NULL
+    const unsigned long long *src_tail;  // its tail counter (my memory)
+    unsigned long long *src_credit;      // where its slots are handed back (the sender's memory)
+    int st_recv;
+    const float *src_local;              // my vector, or NULL
+    const float *src_w;                  // SGD step at the chain's end: my weight replica, or NULL
+    float *dst_local;                    // where the finished block is stored, or NULL
+    float *dst_ring[2];                  // a neighbour's ring of this channel, or NULL
+    unsigned long long *dst_tail[2];     // its tail counter (the neighbour's memory)
+    const unsigned long long *dst_credit[2];  // my credit counter for it (my memory)
+    int st_sent[2];
+};
+
+__device__ __forceinline__ bool mbar_try(uint64_t *bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n"
+        : "=r"(ok)
+        : "r"(lp_smem_u32(bar)), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
+// mbarrier wait that gives up when the CTA has been aborted (a counter poll ran into its limit)
+__device__ __forceinline__ bool mbar_wait_abortable(uint64_t *bar, uint32_t parity, volatile int *abort_flag) {
+    while (!mbar_try(bar, parity))
+        if (*abort_flag) return false;
+    return true;
+}
+__device__ __forceinline__ bool poll_counter(const unsigned long long *flag, unsigned long long want, int *error,
+                                             volatile int *abort_flag, unsigned long long spin_limit) {
+    unsigned long long spins = 0;
+    while (ld_sys(flag) < want) {
+        if (++spins > spin_limit || ((spins & 0xffu) == 0 && (*abort_flag || *reinterpret_cast<volatile int *>(error) != 0))) {
+            atomicCAS(error, 0, 1);
+            *abort_flag = 1;
+            return false;
+        }
+    }
+    return true;
+}
+__device__ __forceinline__ void consumer_barrier() { asm volatile("bar.sync 1, %0;" ::"n"(kTmaConsumers) : "memory"); }
+// barrier over the consumer warps that also tells every one of them whether ANY of them passed `pred` (a uniform
+// decision: a thread that gave up mid-tile and one that did not must leave the tile loop together)
+__device__ __forceinline__ bool consumer_any(bool pred) {
+    uint32_t r;
+    asm volatile(
+        "{\n"
+        ".reg .pred p, q;\n"
+        "setp.ne.u32 p, %1, 0;\n"
+        "bar.red.or.pred q, 1, %2, p;\n"
+        "selp.u32 %0, 1, 0, q;\n"
+        "}\n"
+        : "=r"(r)
+        : "r"((uint32_t)pred), "n"(kTmaConsumers)
+        : "memory");
+    return r != 0;
+}
+
+__device__ void chain_stream_tma(const ChainStream &X, const LpChainRank &A, const LpChainLaunch &L, int c) {
+    extern __shared__ __align__(128) unsigned char lp_smem[];
+    float *ring = reinterpret_cast<float *>(lp_smem);
+    uint64_t *full = reinterpret_cast<uint64_t *>(lp_smem + kTmaRingBytes);
+    uint64_t *empty = full + kTmaMaxStages;
+    volatile int *abort_flag = reinterpret_cast<volatile int *>(empty + kTmaMaxStages);
+    const int nsrc = (X.src_ring ? 1 : 0) + (X.src_local ? 1 : 0) + (X.src_w ? 1 : 0);
+    const int stages = (int)(kTmaRingBytes / ((uint32_t)nsrc * kTmaStep * 4u));
+    const uint32_t stage_floats = (uint32_t)nsrc * kTmaStep;
+    unsigned long long *st = A.state + (size_t)c * 4;
+    const unsigned long long recv0 = X.src_ring ? st[X.st_recv] : 0;
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < stages; ++s) {
+            lp_mbar_init(&full[s], 1);
+            lp_mbar_init(&empty[s], kTmaConsumers / 32);
+        }
+        *abort_flag = 0;
+        lp_fence_mbar_init();
+    }
+    __syncthreads();
+    const size_t ring_c = (size_t)c * L.S * L.tile;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (warp == 0) {
+        // ---------------- producer: counters of my receive ring, TMA bulk loads of every source ------------------------
+        if (lane == 0) {
+            unsigned long long recv = recv0;
+            int stage = 0;
+            uint32_t phase = 0;
+            bool ok = true;
+            for (uint64_t t = (uint64_t)c; ok && t < L.part.n_tiles; t += (uint64_t)L.C) {
+                uint64_t off;
+                uint32_t len;
+                lp_tile_range(L.part, t, off, len);
+                const float *slot = nullptr;
+                if (X.src_ring) {
+                    ok = poll_counter(X.src_tail, recv + 1, A.error, abort_flag, L.spin_limit);
+                    if (!ok) break;
+                    fence_sys();  // acquire: the block published before the counter ...
+                    asm volatile("fence.proxy.async;" ::: "memory");  // ... is what the bulk copies (async proxy) read
+                    slot = X.src_ring + ring_c + (size_t)(recv % (unsigned)L.S) * L.tile;
+                    ++recv;
+                }
+                for (uint32_t s0 = 0; s0 < len; s0 += kTmaStep) {
+                    const uint32_t sl = len - s0 < kTmaStep ? len - s0 : kTmaStep;
+                    const uint32_t bytes = (sl & ~3u) * 4u;  // the 16-byte aligned body; <= 3 tail elements go by hand
+                    ok = mbar_wait_abortable(&empty[stage], phase ^ 1u, abort_flag);
+                    if (!ok) break;
+                    float *dst = ring + (size_t)stage * stage_floats;
+                    if (bytes) {
+                        lp_mbar_expect_tx(&full[stage], bytes * (uint32_t)nsrc);
+                        if (X.src_ring) {
+                            lp_bulk_g2s(dst, slot + s0, bytes, &full[stage]);
+                            dst += kTmaStep;
+                        }
+                        if (X.src_local) {
+                            lp_bulk_g2s(dst, X.src_local + off + s0, bytes, &full[stage]);
+                            dst += kTmaStep;
+                        }
+                        if (X.src_w) lp_bulk_g2s(dst, X.src_w + off + s0, bytes, &full[stage]);
+                    } else {
+                        lp_mbar_arrive(&full[stage]);
+                    }
+                    if (++stage == stages) {
+                        stage = 0;
+                        phase ^= 1u;
+                    }
+                }
+            }
+            if (X.src_ring && ok) st[X.st_recv] = recv;
+        }
+        return;
+    }
+    // -------------------- consumers: fold in chain order, store to every destination, publish, credit --------------------
+    const int ctid = (int)threadIdx.x - 32;
+    unsigned long long sent[2] = {X.dst_ring[0] ? st[X.st_sent[0]] : 0, X.dst_ring[1] ? st[X.st_sent[1]] : 0};
+    unsigned long long recv = recv0;
+    int stage = 0;
+    uint32_t phase = 0;
+    bool ok = true;
+    for (uint64_t t = (uint64_t)c; ok && t < L.part.n_tiles; t += (uint64_t)L.C) {
+        uint64_t off;
+        uint32_t len;
+        lp_tile_range(L.part, t, off, len);
+        bool failed = false;
+        if (ctid == 0) {  // the slots this tile is pushed into must be free
+            for (int j = 0; j < 2 && !failed; ++j)
+                if (X.dst_ring[j] && slot_free_at(sent[j], L.S))
+                    failed = !poll_counter(X.dst_credit[j], slot_free_at(sent[j], L.S), A.error, abort_flag, L.spin_limit);
+        }
+        if (consumer_any(failed)) {
+            ok = false;
+            break;
+        }
+        float *push[2] = {X.dst_ring[0] ? X.dst_ring[0] + ring_c + (size_t)(sent[0] % (unsigned)L.S) * L.tile : nullptr,
+                          X.dst_ring[1] ? X.dst_ring[1] + ring_c + (size_t)(sent[1] % (unsigned)L.S) * L.tile : nullptr};
+        const float *in_slot = X.src_ring ? X.src_ring + ring_c + (size_t)(recv % (unsigned)L.S) * L.tile : nullptr;
+        for (uint32_t s0 = 0; s0 < len; s0 += kTmaStep) {
+            const uint32_t sl = len - s0 < kTmaStep ? len - s0 : kTmaStep;
+            const uint32_t nvec = sl >> 2;
+            ok = mbar_wait_abortable(&full[stage], phase, abort_flag);
+            if (!ok) break;
+            const float4 *src = reinterpret_cast<const float4 *>(ring + (size_t)stage * stage_floats);
+            float4 acc[kTmaVec];
+#pragma unroll
+            for (int k = 0; k < kTmaVec; ++k) {
+                const uint32_t j = (uint32_t)ctid + (uint32_t)k * kTmaConsumers;
+                if (j < nvec) {
+                    const float4 *p = src + j;
+                    acc[k] = *p;  // the partial (or the finished block), else my block
+                    if (X.src_ring && X.src_local) {  // "reduces the received block a0 with a1": partial op mine
+                        p += kTmaStep / 4;
+                        acc[k] = lp_combine4(acc[k], *p, L.code);
+                    }
+                    if (X.src_w) {  // Alg. 3's update where the global gradient is complete: three RN operations
+                        p += kTmaStep / 4;
+                        acc[k] = lp_sgd4(acc[k], *p, L.lr, L.invP);
+                    }
+                }
+            }
+            // the shared-memory reads above have returned (their values went into the fold, or -- a plain copy -- are
+            // consumed by the stores below only after this fence): the slot may be refilled
+            __threadfence_block();
+            __syncwarp();
+            if (lane == 0) lp_mbar_arrive(&empty[stage]);
+            if (++stage == stages) {
+                stage = 0;
+                phase ^= 1u;
+            }
+#pragma unroll
+            for (int k = 0; k < kTmaVec; ++k) {
+                const uint32_t j = (uint32_t)ctid + (uint32_t)k * kTmaConsumers;
+                if (j < nvec) {
+                    if (push[0]) lp_stg_stream(push[0] + s0 + 4 * j, acc[k]);
+                    if (X.dst_local) lp_stg_stream(X.dst_local + off + s0 + 4 * j, acc[k]);
+                    if (push[1]) lp_stg_stream(push[1] + s0 + 4 * j, acc[k]);
+                }
+            }
+            if (ctid == 0 && (sl & 3u)) {  // the message's last <= 3 elements: by hand, straight from and to global memory
+                for (uint32_t e = sl & ~3u; e < sl; ++e) {
+                    float v = X.src_ring ? ld_ring1(in_slot + s0 + e) : X.src_local[off + s0 + e];
+                    if (X.src_ring && X.src_local) v = lp_combine1(v, X.src_local[off + s0 + e], L.code);
+                    if (X.src_w) v = lp_sgd1(v, X.src_w[off + s0 + e], L.lr, L.invP);
+                    if (push[0]) push[0][s0 + e] = v;
+                    if (X.dst_local) X.dst_local[off + s0 + e] = v;
+                    if (push[1]) push[1][s0 + e] = v;
+                }
+            }
+        }
+        // every consumer's stores of this tile have been issued -- or somebody gave up: then all leave together
+        if (consumer_any(!ok)) {
+            ok = false;
+            break;
+        }
+        if (push[0]) ++sent[0];
+        if (push[1]) ++sent[1];
+        ++recv;
+        if (ctid == 0) {
+            if (push[0] || push[1]) fence_sys();  // release, cumulative over the barrier: the tile before its counter
+            if (push[0]) st_sys(X.dst_tail[0], sent[0]);
+            if (push[1]) st_sys(X.dst_tail[1], sent[1]);
+            if (X.src_ring) st_sys(X.src_credit, recv);  // the bulk loads of this slot completed long ago
+        }
+    }
+    consumer_barrier();
+    if (ctid == 0 && ok) {
+        if (X.dst_ring[0]) st[X.st_sent[0]] = sent[0];
+        if (X.dst_ring[1]) st[X.st_sent[1]] = sent[1];
+    }
+}
+
+__global__ void __launch_bounds__(kTmaThreads, 1) lp_chain_tma_kernel(const __grid_constant__ LpChainLaunch L) {
+    const int per_rank = 2 * L.C;
+    const int lr = (int)blockIdx.x / per_rank;
+    const int j = (int)blockIdx.x - lr * per_rank;
+    const LpChainRank &A = L.rank[lr];
+    ChainStream X;
+    memset(&X, 0, sizeof(X));
+    int c;
+    if (j < L.C) {
+        if (!A.f_active) return;
+        c = j;
+        unsigned long long *my = A.flags + (size_t)c * kFlagsPerChannel;
+        if (A.f_recv) {
+            X.src_ring = A.fwd_ring;
+            X.src_tail = my + F_FWD_TAIL;
+            X.src_credit = A.down_flags + (size_t)c * kFlagsPerChannel + F_UP_CREDIT;
+            X.st_recv = ST_RECV_FWD;
+        }
+        if (A.f_load) X.src_local = A.buf;
+        if (A.f_update) X.src_w = A.w_in;
+        if (A.f_store) X.dst_local = A.out;
+        if (A.f_send_up) {
+            X.dst_ring[0] = A.up_fwd_ring;
+            X.dst_tail[0] = A.up_flags + (size_t)c * kFlagsPerChannel + F_FWD_TAIL;
+            X.dst_credit[0] = my + F_UP_CREDIT;
+            X.st_sent[0] = ST_SENT_UP;
+        }
+        if (A.f_send_down) {
+            X.dst_ring[1] = A.down_bwd_ring;
+            X.dst_tail[1] = A.down_flags + (size_t)c * kFlagsPerChannel + F_BWD_TAIL;
+            X.dst_credit[1] = my + F_DOWN_CREDIT;
+            X.st_sent[1] = ST_SENT_DOWN;
+        }
+    } else {
+        if (!A.r_active) return;
+        c = j - L.C;
+        unsigned long long *my = A.flags + (size_t)c * kFlagsPerChannel;
+        X.src_ring = A.bwd_ring;
+        X.src_tail = my + F_BWD_TAIL;
+        X.src_credit = A.up_flags + (size_t)c * kFlagsPerChannel + F_DOWN_CREDIT;
+        X.st_recv = ST_RECV_BWD;
+        if (A.r_store) X.dst_local = A.out;
+        if (A.r_send_down) {
+            X.dst_ring[1] = A.down_bwd_ring;
+            X.dst_tail[1] = A.down_flags + (size_t)c * kFlagsPerChannel + F_BWD_TAIL;
+            X.dst_credit[1] = my + F_DOWN_CREDIT;
+            X.st_sent[1] = ST_SENT_DOWN;
+        }
+    }
+    chain_stream_tma(X, A, L, c);
+}
+
 }  // namespace
 
 // ---- host side -------------------------------------------------------------------------------------------------
@@ -397,18 +702,37 @@ void fill_rank(LpChainRank &R, const EndpointLayout &l, float *buf, float *out, 
 // emulation, for twice the ring memory -- profiles/r2_dtypes_chain.md.)
 int chain_threads() { return kChainThreads; }
 
+std::atomic<int> g_chain_kernel{LP_CHAIN_KERNEL_DEFAULT};
+bool use_tma() { return g_chain_kernel.load() != LP_CHAIN_KERNEL_REGISTER; }
+constexpr uint32_t kTmaSmem = kTmaRingBytes + 2u * kTmaMaxStages * 8u + 16u;
+
+cudaError_t tma_attr() {  // per device binding (lp_attr_epoch): the dynamic shared memory limit of the TMA kernel
+    static std::atomic<unsigned> epoch{0};
+    if (epoch.load() == lp_attr_epoch()) return cudaSuccess;
+    const cudaError_t e = cudaFuncSetAttribute(lp_chain_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTmaSmem);
+    if (e == cudaSuccess) epoch.store(lp_attr_epoch());
+    return e;
+}
+
 // CTAs of the chain kernel the current device holds at once
 cudaError_t resident(int *ctas) {
     int per_sm = 0, dev = 0, sms = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, lp_chain_kernel, chain_threads(), 0);
+    if (e == cudaSuccess && use_tma()) {
+        e = tma_attr();
+        if (e == cudaSuccess)
+            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, lp_chain_tma_kernel, kTmaThreads, kTmaSmem);
+    } else if (e == cudaSuccess) {
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, lp_chain_kernel, chain_threads(), 0);
+    }
     *ctas = per_sm * sms;
     return e;
 }
 
 cudaError_t launch(const LpChainLaunch &L, bool cooperative, cudaStream_t stream) {
     const unsigned grid = (unsigned)(L.n_local * 2 * L.C);
+    const bool tma = use_tma();
     int cap = 0;
     cudaError_t e = resident(&cap);
     if (e != cudaSuccess) return e;
@@ -416,7 +740,8 @@ cudaError_t launch(const LpChainLaunch &L, bool cooperative, cudaStream_t stream
     cudaLaunchConfig_t lc;
     memset(&lc, 0, sizeof(lc));
     lc.gridDim = dim3(grid);
-    lc.blockDim = dim3(chain_threads());
+    lc.blockDim = dim3(tma ? kTmaThreads : chain_threads());
+    lc.dynamicSmemBytes = tma ? kTmaSmem : 0;
     lc.stream = stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeCooperative;
@@ -425,6 +750,7 @@ cudaError_t launch(const LpChainLaunch &L, bool cooperative, cudaStream_t stream
     lc.numAttrs = cooperative ? 1 : 0;
     lp_count_launch(1);
     lp_chain_reset(stream);
+    if (tma) return cudaLaunchKernelEx(&lc, lp_chain_tma_kernel, L);
     return cudaLaunchKernelEx(&lc, lp_chain_kernel, L);
 }
 
@@ -564,6 +890,13 @@ int lp_chain_connect_ptrs(lp_chain *ch, void *up_endpoint, void *down_endpoint) 
 }
 
 void *lp_chain_endpoint(lp_chain *ch) { return ch ? ch->base : nullptr; }
+
+int lp_chain_set_kernel(int kernel) {
+    if (kernel != LP_CHAIN_KERNEL_DEFAULT && kernel != LP_CHAIN_KERNEL_REGISTER && kernel != LP_CHAIN_KERNEL_TMA)
+        return LP_ERR_INVALID_ARG;
+    g_chain_kernel.store(kernel);
+    return LP_OK;
+}
 
 int lp_chain_set_timeout(lp_chain *ch, unsigned long long polls) {
     if (ch == nullptr || polls == 0) return LP_ERR_INVALID_ARG;

@@ -15,12 +15,15 @@ torch = pytest.importorskip("torch")
 OPS = {"broadcast": lp.OP_BROADCAST, "reduce": lp.OP_REDUCE, "allreduce": lp.OP_ALLREDUCE}
 
 
-@pytest.fixture(autouse=True)
-def _device():
+@pytest.fixture(autouse=True, params=[lp.CHAIN_KERNEL_TMA, lp.CHAIN_KERNEL_REGISTER], ids=["tma", "register"])
+def _device(request):
+    """Every test runs with both realisations of a rank's CTAs (the protocol between ranks is the same)."""
     assert torch.cuda.is_available(), "gpu tests need a CUDA device"
     lp.lib()
+    lp.lp_chain_set_kernel(request.param)
     yield
     torch.cuda.synchronize()
+    lp.lp_chain_set_kernel(lp.CHAIN_KERNEL_DEFAULT)
 
 
 def up(arrs):
@@ -212,6 +215,7 @@ def test_chain_argument_errors():
     dev4 = [torch.zeros(64, device="cuda") for _ in range(4)]
     arr4, _ = lp._dev_ptrs(dev4)
     assert L.lp_chain_emulate(lp.OP_ALLREDUCE, arr4, 4, n, 16, 0, 0, 64, 0, 0, s) == lp.LP_ERR_UNSUPPORTED  # 512 CTAs at once
+    assert L.lp_chain_set_kernel(7) == lp.LP_ERR_INVALID_ARG
     assert L.lp_chain_emulate(lp.OP_ALLREDUCE, arr, 2, 0, 16, 0, 0, 0, 0, 0, s) == lp.LP_OK                 # n == 0
 
 
