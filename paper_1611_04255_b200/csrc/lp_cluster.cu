@@ -226,8 +226,13 @@ __global__ void __launch_bounds__(kClThreads)
                 if (x > 0) {  // a' = (what GPU x-1 sent) + my block, in that order (chain order)
                     lp_mbar_wait(&rv_full[rv.slot], rv.phase);
                     const float4 *s = reinterpret_cast<const float4 *>(rv_ring + rv.slot * kClTile);
+                    float4 loc[kV];
 #pragma unroll
-                    for (int v = 0; v < kV; ++v) acc[v] = lp_combine4(s[ftid + v * FT], mine[ftid + v * FT], code);
+                    for (int v = 0; v < kV; ++v) {
+                        acc[v] = s[ftid + v * FT];
+                        loc[v] = mine[ftid + v * FT];
+                    }
+                    lp_fold_vecs<kV>(acc, loc, kV, code);  // the operator switch sits outside the vector loop
                     __threadfence_block();
                     __syncwarp();
                     if (lane == 0) lp_mbar_arrive(&in_empty[in.slot]);

@@ -323,9 +323,8 @@ __device__ __forceinline__ float4 lp_vec_op(const float4 &a, const float4 &b) {
     }
 }
 __device__ __forceinline__ float4 lp_combine4(const float4 &a, const float4 &b, int code) {
+    if (code <= 1) return code ? lp_vec_op<1>(a, b) : lp_vec_op<0>(a, b);  // fp32, the paper's case: what it always was
     switch (code) {
-        case 0: return lp_vec_op<0>(a, b);
-        case 1: return lp_vec_op<1>(a, b);
         case 2: return lp_vec_op<2>(a, b);
         case 3: return lp_vec_op<3>(a, b);
         case 4: return lp_vec_op<4>(a, b);
