@@ -373,6 +373,11 @@ LP_API int lp_chain_run_dt(lp_chain *ch, int op, void *buf, size_t n, size_t blo
  * the same bits, U8) and w' travels back down; every rank stores it into its `weight`.  grad is only read; fp32. */
 LP_API int lp_chain_bsp_sgd_step(lp_chain *ch, float *grad, float *weight, size_t n, size_t block, float lr,
                                  void *cuda_stream);
+/* The same with momentum ("The solver is SGD + momentum"; U18): v' = mu * v + lr * (S * fl(1/P)), w' = w - v',
+ * five RN operations.  The velocity is ONE vector and lives where the update is computed: the LAST rank passes it (n
+ * floats, 16-byte aligned, rewritten in place), every other rank passes NULL. */
+LP_API int lp_chain_bsp_sgd_momentum_step(lp_chain *ch, float *grad, float *weight, float *velocity, size_t n, size_t block,
+                                          float lr, float mu, void *cuda_stream);
 LP_API int lp_chain_error(lp_chain *ch, int *error_out);
 LP_API int lp_chain_destroy(lp_chain *ch);
 LP_API int lp_chain_emulate(int op, float *const *bufs, int P, size_t n, size_t block, int root, int reduce_op, int channels,
@@ -382,6 +387,10 @@ LP_API int lp_chain_emulate_dt(int op, void *const *bufs, int P, size_t n, size_
 /* grads[r], weights[r]: rank r's vectors; equals lp_bsp_sgd_step with root = P - 1 (the replica the chain's end reads) */
 LP_API int lp_chain_emulate_bsp_sgd_step(float *const *grads, float *const *weights, int P, size_t n, size_t block, float lr,
                                          int channels, int slots, int tile, void *cuda_stream);
+/* ... and with momentum: equals lp_bsp_sgd_momentum_step with root = P - 1; `velocity` is the chain end's vector */
+LP_API int lp_chain_emulate_bsp_sgd_momentum_step(float *const *grads, float *const *weights, float *velocity, int P, size_t n,
+                                                  size_t block, float lr, float mu, int channels, int slots, int tile,
+                                                  void *cuda_stream);
 LP_API int lp_chain_emulate_channels(int P, int tile);
 LP_API int lp_chain_emulate_error(int P, int channels, int slots, int tile, int *error_out);
 

@@ -128,6 +128,8 @@ def lib() -> ctypes.CDLL:
     L.lp_chain_bsp_sgd_step.argtypes = [vp, vp, vp, sz, sz, f32, vp]
     L.lp_chain_emulate_dt.argtypes = [i32, pp, i32, sz, sz, i32, i32, i32, i32, i32, i32, vp]
     L.lp_chain_emulate_bsp_sgd_step.argtypes = [pp, pp, i32, sz, sz, f32, i32, i32, i32, vp]
+    L.lp_chain_bsp_sgd_momentum_step.argtypes = [vp, vp, vp, vp, sz, sz, f32, f32, vp]
+    L.lp_chain_emulate_bsp_sgd_momentum_step.argtypes = [pp, pp, vp, i32, sz, sz, f32, f32, i32, i32, i32, vp]
     L.lp_chain_error.argtypes = [vp, ctypes.POINTER(i32)]
     L.lp_chain_destroy.argtypes = [vp]
     L.lp_chain_emulate.argtypes = [i32, pp, i32, sz, sz, i32, i32, i32, i32, i32, vp]
@@ -370,6 +372,18 @@ def lp_chain_emulate_bsp_sgd_step(grads, weights, block=0, lr=0.01, channels=0, 
                                                _stream_ptr(stream)), "lp_chain_emulate_bsp_sgd_step")
 
 
+def lp_chain_emulate_bsp_sgd_momentum_step(grads, weights, velocity, block=0, lr=0.01, mu=0.9, channels=0, slots=0, tile=0,
+                                           stream=None):
+    """Alg. 3's step with momentum over the emulated chain; equals lp_bsp_sgd_momentum_step with root = P - 1."""
+    ga, n = _dev_ptrs(grads)
+    wa, nw = _dev_ptrs(weights)
+    if n != nw or len(grads) != len(weights):
+        raise ValueError("grads and weights must match in P and n")
+    _check(lib().lp_chain_emulate_bsp_sgd_momentum_step(ga, wa, _velocity_ptr(velocity, n), len(grads), n, block,
+                                                        ctypes.c_float(lr), ctypes.c_float(mu), channels, slots, tile,
+                                                        _stream_ptr(stream)), "lp_chain_emulate_bsp_sgd_momentum_step")
+
+
 def lp_chain_emulate_error(P, channels=0, slots=0, tile=0) -> int:
     e = ctypes.c_int(0)
     _check(lib().lp_chain_emulate_error(P, channels, slots, tile, ctypes.byref(e)), "lp_chain_emulate_error")
@@ -432,6 +446,13 @@ class Chain:
         _check(lib().lp_chain_bsp_sgd_step(self.h, ctypes.c_void_p(grad.data_ptr()), ctypes.c_void_p(weight.data_ptr()),
                                            grad.numel(), block, ctypes.c_float(lr), _stream_ptr(stream)),
                "lp_chain_bsp_sgd_step")
+
+    def bsp_sgd_momentum_step(self, grad, weight, velocity=None, block=0, lr=0.01, mu=0.9, stream=None):
+        """`velocity`: the last rank's vector (the update is computed there); None on every other rank."""
+        vp_ = ctypes.c_void_p(velocity.data_ptr()) if velocity is not None else None
+        _check(lib().lp_chain_bsp_sgd_momentum_step(self.h, ctypes.c_void_p(grad.data_ptr()), ctypes.c_void_p(weight.data_ptr()),
+                                                    vp_, grad.numel(), block, ctypes.c_float(lr), ctypes.c_float(mu),
+                                                    _stream_ptr(stream)), "lp_chain_bsp_sgd_momentum_step")
 
     def error(self) -> int:
         e = ctypes.c_int(0)

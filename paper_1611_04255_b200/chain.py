@@ -58,6 +58,10 @@ class ChainGroup:
         """Alg. 3: allreduce of the sub-gradients, w -= lr * mean gradient, fused; every rank's `weight` gets the new bits."""
         self.endpoint.bsp_sgd_step(grad, weight, block=block, lr=lr, stream=stream)
 
+    def bsp_sgd_momentum_step(self, grad, weight, velocity, lr, mu, block=0, stream=None):
+        """The same with momentum (the paper's solver); `velocity` is the LAST rank's vector, None elsewhere."""
+        self.endpoint.bsp_sgd_momentum_step(grad, weight, velocity, block=block, lr=lr, mu=mu, stream=stream)
+
     def error(self) -> int:
         return self.endpoint.error()
 

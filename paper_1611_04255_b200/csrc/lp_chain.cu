@@ -48,6 +48,7 @@ struct LpChainRank {
     float *buf;         // my vector: what the forward CTAs load
     float *out;         // where finished blocks are stored: buf (in place), or my weight replica for the SGD step
     const float *w_in;  // SGD step, chain end only: the weight replica the update reads
+    float *vel;         // SGD step with momentum, chain end only: the velocity, read and rewritten in place
     unsigned long long *flags;   // my counters: [C][kFlagsPerChannel]
     unsigned long long *state;   // my private sequence numbers: [C][4]
     float *fwd_ring, *bwd_ring;  // my receive rings: [C][S][tile]
@@ -71,6 +72,7 @@ struct LpChainLaunch {
     uint32_t tile;  // elements per ring slot
     int code;  // (dtype << 1) | red_op
     float lr, invP;  // SGD step (LpChainRank::f_update): w' = w - lr * (S * invP) where the chain ends (U7)
+    float mu;        // ... with momentum (LpChainRank::vel != NULL): v' = mu v + lr (S invP), w' = w - v' (U18)
     unsigned long long spin_limit;  // polls before a wait gives up and flags an error: a missing peer never hangs the GPU
 };
 
@@ -217,8 +219,16 @@ __device__ void chain_forward(const LpChainRank &A, const LpChainLaunch &L, int 
             if (A.f_update) {  // Alg. 3's update where the global gradient S is complete: three RN operations
                 StepRegs w;
                 load_step(w, A.w_in + off + s0, sl, false);
+                if (A.vel) {  // five with momentum; the velocity lives where the update is computed (U18)
+                    StepRegs v;
+                    load_step(v, A.vel + off + s0, sl, false);
 #pragma unroll
-                for (int k = 0; k < kV; ++k) acc.v[k] = lp_sgd4(acc.v[k], w.v[k], L.lr, L.invP);
+                    for (int k = 0; k < kV; ++k) lp_mom4(acc.v[k], w.v[k], v.v[k], L.lr, L.invP, L.mu, v.v[k], acc.v[k]);
+                    store_step(v, A.vel + off + s0, sl);
+                } else {
+#pragma unroll
+                    for (int k = 0; k < kV; ++k) acc.v[k] = lp_sgd4(acc.v[k], w.v[k], L.lr, L.invP);
+                }
             }
             if (A.f_send_up) store_step(acc, up_slot + s0, sl);
             if (A.f_store) store_step(acc, A.out + off + s0, sl);
@@ -314,6 +324,7 @@ struct ChainStream {
     int st_recv;
     const float *src_local;              // my vector, or NULL
     const float *src_w;                  // SGD step at the chain's end: my weight replica, or NULL
+    float *vel;                          // ... with momentum: the velocity (a fourth source, rewritten in place), or NULL
     float *dst_local;                    // where the finished block is stored, or NULL
     float *dst_ring[2];                  // a neighbour's ring of this channel, or NULL
     unsigned long long *dst_tail[2];     // its tail counter (the neighbour's memory)
@@ -376,7 +387,7 @@ __device__ void chain_stream_tma(const ChainStream &X, const LpChainRank &A, con
     uint64_t *full = reinterpret_cast<uint64_t *>(lp_smem + kTmaRingBytes);
     uint64_t *empty = full + kTmaMaxStages;
     volatile int *abort_flag = reinterpret_cast<volatile int *>(empty + kTmaMaxStages);
-    const int nsrc = (X.src_ring ? 1 : 0) + (X.src_local ? 1 : 0) + (X.src_w ? 1 : 0);
+    const int nsrc = (X.src_ring ? 1 : 0) + (X.src_local ? 1 : 0) + (X.src_w ? 1 : 0) + (X.vel ? 1 : 0);
     const int stages = (int)(kTmaRingBytes / ((uint32_t)nsrc * kTmaStep * 4u));
     const uint32_t stage_floats = (uint32_t)nsrc * kTmaStep;
     unsigned long long *st = A.state + (size_t)c * 4;
@@ -428,7 +439,11 @@ __device__ void chain_stream_tma(const ChainStream &X, const LpChainRank &A, con
                             lp_bulk_g2s(dst, X.src_local + off + s0, bytes, &full[stage]);
                             dst += kTmaStep;
                         }
-                        if (X.src_w) lp_bulk_g2s(dst, X.src_w + off + s0, bytes, &full[stage]);
+                        if (X.src_w) {
+                            lp_bulk_g2s(dst, X.src_w + off + s0, bytes, &full[stage]);
+                            dst += kTmaStep;
+                        }
+                        if (X.vel) lp_bulk_g2s(dst, X.vel + off + s0, bytes, &full[stage]);
                     } else {
                         lp_mbar_arrive(&full[stage]);
                     }
@@ -485,7 +500,13 @@ __device__ void chain_stream_tma(const ChainStream &X, const LpChainRank &A, con
                     }
                     if (X.src_w) {  // Alg. 3's update where the global gradient is complete: three RN operations
                         p += kTmaStep / 4;
-                        acc[k] = lp_sgd4(acc[k], *p, L.lr, L.invP);
+                        if (X.vel) {  // five with momentum (U18): the new velocity goes straight back to its vector
+                            float4 vn;
+                            lp_mom4(acc[k], *p, p[kTmaStep / 4], L.lr, L.invP, L.mu, vn, acc[k]);
+                            lp_stg_stream(X.vel + off + s0 + 4 * j, vn);
+                        } else {
+                            acc[k] = lp_sgd4(acc[k], *p, L.lr, L.invP);
+                        }
                     }
                 }
             }
@@ -511,7 +532,14 @@ __device__ void chain_stream_tma(const ChainStream &X, const LpChainRank &A, con
                 for (uint32_t e = sl & ~3u; e < sl; ++e) {
                     float v = X.src_ring ? ld_ring1(in_slot + s0 + e) : X.src_local[off + s0 + e];
                     if (X.src_ring && X.src_local) v = lp_combine1(v, X.src_local[off + s0 + e], L.code);
-                    if (X.src_w) v = lp_sgd1(v, X.src_w[off + s0 + e], L.lr, L.invP);
+                    if (X.src_w && X.vel) {
+                        float vn, wn;
+                        lp_mom1(v, X.src_w[off + s0 + e], X.vel[off + s0 + e], L.lr, L.invP, L.mu, vn, wn);
+                        X.vel[off + s0 + e] = vn;
+                        v = wn;
+                    } else if (X.src_w) {
+                        v = lp_sgd1(v, X.src_w[off + s0 + e], L.lr, L.invP);
+                    }
                     if (push[0]) push[0][s0 + e] = v;
                     if (X.dst_local) X.dst_local[off + s0 + e] = v;
                     if (push[1]) push[1][s0 + e] = v;
@@ -559,7 +587,10 @@ __global__ void __launch_bounds__(kTmaThreads, 1) lp_chain_tma_kernel(const __gr
             X.st_recv = ST_RECV_FWD;
         }
         if (A.f_load) X.src_local = A.buf;
-        if (A.f_update) X.src_w = A.w_in;
+        if (A.f_update) {
+            X.src_w = A.w_in;
+            X.vel = A.vel;
+        }
         if (A.f_store) X.dst_local = A.out;
         if (A.f_send_up) {
             X.dst_ring[0] = A.up_fwd_ring;
@@ -599,13 +630,13 @@ __global__ void __launch_bounds__(kTmaThreads, 1) lp_chain_tma_kernel(const __gr
 // Roles of `rank` in a collective over P ranks (pure host logic: the part of the multi-process path that needs no GPU).
 extern "C" int lp_chain_plan(int op, int P, int root, int rank, lp_chain_role *out) {
     if (out == nullptr || P < 1 || P > LP_MAX_P || rank < 0 || rank >= P) return LP_ERR_INVALID_ARG;
-    if (op != LP_OP_BROADCAST && op != LP_OP_REDUCE && op != LP_OP_ALLREDUCE && op != LP_OP_BSP_SGD) return LP_ERR_INVALID_ARG;
+    if (op < LP_OP_BROADCAST || op > LP_OP_BSP_SGD_MOM) return LP_ERR_INVALID_ARG;
     if ((op == LP_OP_BROADCAST || op == LP_OP_REDUCE) && (root < 0 || root >= P)) return LP_ERR_INVALID_ARG;
     memset(out, 0, sizeof(*out));
     out->up = (rank + 1) % P;
     out->down = (rank + P - 1) % P;
     if (P == 1) {  // nothing moves; the SGD step of a single rank is its own update
-        if (op == LP_OP_BSP_SGD) out->f_active = out->f_load = out->f_update = out->f_store = 1;
+        if (op == LP_OP_BSP_SGD || op == LP_OP_BSP_SGD_MOM) out->f_active = out->f_load = out->f_update = out->f_store = 1;
         return LP_OK;
     }
     if (op == LP_OP_BROADCAST) {  // root -> root+1 -> ... -> root-1 around the ring, forward direction only
@@ -629,7 +660,7 @@ extern "C" int lp_chain_plan(int op, int P, int root, int rank, lp_chain_role *o
     out->f_send_up = !head;
     out->f_store = head && (all || root == P - 1);
     out->f_send_down = head && ret_lo < P - 1;
-    out->f_update = head && op == LP_OP_BSP_SGD;
+    out->f_update = head && (op == LP_OP_BSP_SGD || op == LP_OP_BSP_SGD_MOM);
     out->r_active = !head && rank >= ret_lo && ret_lo < P - 1;
     out->r_store = out->r_active && (all || rank == root);
     out->r_send_down = out->r_active && rank > ret_lo;
@@ -670,13 +701,14 @@ EndpointLayout layout_of(int C, int S, int tile) {
     return l;
 }
 
-void fill_rank(LpChainRank &R, const EndpointLayout &l, float *buf, float *out, const float *w_in, void *mine, void *up,
-               void *down, const lp_chain_role &role) {
+void fill_rank(LpChainRank &R, const EndpointLayout &l, float *buf, float *out, const float *w_in, float *vel, void *mine,
+               void *up, void *down, const lp_chain_role &role) {
     memset(&R, 0, sizeof(R));
     char *m = (char *)mine, *u = (char *)up, *d = (char *)down;
     R.buf = buf;
     R.out = out;
     R.w_in = w_in;
+    R.vel = role.f_update ? vel : nullptr;
     R.flags = (unsigned long long *)(m + l.flags_off);
     R.state = (unsigned long long *)(m + l.state_off);
     R.error = (int *)(m + l.error_off);
@@ -936,16 +968,19 @@ static bool chain_words(int dtype, int reduce_op, size_t &n, size_t &block, int 
     return true;
 }
 
+static bool chain_sgd(int op) { return op == LP_OP_BSP_SGD || op == LP_OP_BSP_SGD_MOM; }
+
 static int chain_run_rank(lp_chain *ch, int op, float *buf, float *out, const float *w_in, size_t n, size_t block, int root,
-                          int code, float lr, void *cuda_stream) {
+                          int code, float lr, void *cuda_stream, float *vel = nullptr, float mu = 0.f) {
     if (ch == nullptr || !ch->connected) return LP_ERR_INVALID_ARG;
-    if (op == LP_OP_ALLREDUCE || op == LP_OP_BSP_SGD) root = 0;
+    if (op == LP_OP_ALLREDUCE || chain_sgd(op)) root = 0;
     lp_chain_role role;
     int rc = lp_chain_plan(op, ch->P, root, ch->rank, &role);
     if (rc != LP_OK) return rc;
     if (buf == nullptr || ((uintptr_t)buf & 15u) || out == nullptr || ((uintptr_t)out & 15u)) return LP_ERR_INVALID_ARG;
+    if (op == LP_OP_BSP_SGD_MOM && role.f_update && (vel == nullptr || ((uintptr_t)vel & 15u))) return LP_ERR_INVALID_ARG;
     if (n == 0) return LP_OK;
-    if (ch->P == 1 && op != LP_OP_BSP_SGD) return LP_OK;
+    if (ch->P == 1 && !chain_sgd(op)) return LP_OK;
     int dev = -1;
     if (cudaGetDevice(&dev) != cudaSuccess || dev != ch->device) {
         cudaGetLastError();
@@ -958,11 +993,13 @@ static int chain_run_rank(lp_chain *ch, int op, float *buf, float *out, const fl
     L.S = ch->S;
     L.code = code;
     L.lr = lr;
+    L.mu = mu;
     L.invP = 1.0f / (float)ch->P;  // one RN division on the host (U7)
     L.spin_limit = ch->spin_limit;
     L.part = chain_partition(n, block, ch->tile, ch->C);
     L.tile = (uint32_t)ch->tile;
-    fill_rank(L.rank[0], layout_of(ch->C, ch->S, ch->tile), buf, out, w_in, ch->base, ch->peer_up, ch->peer_down, role);
+    fill_rank(L.rank[0], layout_of(ch->C, ch->S, ch->tile), buf, out, w_in, op == LP_OP_BSP_SGD_MOM ? vel : nullptr, ch->base,
+              ch->peer_up, ch->peer_down, role);
     const cudaError_t e = launch(L, false, (cudaStream_t)cuda_stream);
     return e == cudaSuccess ? LP_OK : chain_fail(e);
 }
@@ -992,6 +1029,16 @@ int lp_chain_bsp_sgd_step(lp_chain *ch, float *grad, float *weight, size_t n, si
     return chain_run_rank(ch, LP_OP_BSP_SGD, grad, weight, weight, n, block, 0, LP_REDUCE_SUM, lr, cuda_stream);
 }
 
+// The same with momentum ("The solver is SGD + momentum"; U18): v' = mu v + lr (S invP), w' = w - v'.  The
+// velocity is ONE vector and lives where the update is computed: on the LAST rank, which passes it; the others pass NULL.
+int lp_chain_bsp_sgd_momentum_step(lp_chain *ch, float *grad, float *weight, float *velocity, size_t n, size_t block,
+                                   float lr, float mu, void *cuda_stream) {
+    if (weight == nullptr || grad == weight || (velocity != nullptr && (velocity == grad || velocity == weight)))
+        return LP_ERR_INVALID_ARG;
+    return chain_run_rank(ch, LP_OP_BSP_SGD_MOM, grad, weight, weight, n, block, 0, LP_REDUCE_SUM, lr, cuda_stream, velocity,
+                          mu);
+}
+
 // 0 = no wait of this endpoint's kernels has given up so far (a peer that never arrived); synchronises the device.
 int lp_chain_error(lp_chain *ch, int *error_out) {
     if (ch == nullptr || error_out == nullptr) return LP_ERR_INVALID_ARG;
@@ -1019,22 +1066,25 @@ int lp_chain_emulate_channels(int P, int tile) {
 // All P ranks of the chain on ONE device, in one cooperative launch: P x 2 x channels co-resident CTAs run the per-rank
 // code above against P endpoints in this device's memory.
 static int chain_emulate(int op, float *const *bufs, float *const *outs, int P, size_t n, size_t block, int root, int code,
-                         size_t elem_bytes_total, float lr, int channels, int slots, int tile, void *cuda_stream) {
+                         size_t elem_bytes_total, float lr, int channels, int slots, int tile, void *cuda_stream,
+                         float *vel = nullptr, float mu = 0.f) {
     if (slots == 0) slots = LP_CHAIN_DEFAULT_SLOTS;
     if (tile == 0) tile = LP_CHAIN_DEFAULT_TILE;
     if (channels == 0) channels = lp_chain_emulate_channels(P, tile);
     if (bufs == nullptr || P < 1 || P > LP_MAX_P || !valid_geometry(channels, slots, tile)) return LP_ERR_INVALID_ARG;
-    if (op == LP_OP_ALLREDUCE || op == LP_OP_BSP_SGD) root = 0;
+    if (op == LP_OP_ALLREDUCE || chain_sgd(op)) root = 0;
+    if (op == LP_OP_BSP_SGD_MOM && (vel == nullptr || ((uintptr_t)vel & 15u))) return LP_ERR_INVALID_ARG;
     lp_chain_role roles[LP_MAX_P];
     for (int r = 0; r < P; ++r) {
         const int rc = lp_chain_plan(op, P, root, r, &roles[r]);
         if (rc != LP_OK) return rc;
     }
-    const float *all[2 * LP_MAX_P];
+    const float *all[2 * LP_MAX_P + 1];
     int m = 0;
     for (int r = 0; r < P; ++r) all[m++] = bufs[r];
     if (outs != bufs)
         for (int r = 0; r < P; ++r) all[m++] = outs[r];
+    if (op == LP_OP_BSP_SGD_MOM) all[m++] = vel;
     for (int i = 0; i < m; ++i) {
         if (all[i] == nullptr || ((uintptr_t)all[i] & 15u)) return LP_ERR_INVALID_ARG;
         for (int q = 0; q < i; ++q) {
@@ -1043,7 +1093,7 @@ static int chain_emulate(int op, float *const *bufs, float *const *outs, int P, 
         }
     }
     if (n == 0) return LP_OK;
-    if (P == 1 && op != LP_OP_BSP_SGD) return LP_OK;
+    if (P == 1 && !chain_sgd(op)) return LP_OK;
     const EndpointLayout l = layout_of(channels, slots, tile);
     void *base = nullptr;
     {
@@ -1073,13 +1123,15 @@ static int chain_emulate(int op, float *const *bufs, float *const *outs, int P, 
     L.S = slots;
     L.code = code;
     L.lr = lr;
+    L.mu = mu;
     L.invP = 1.0f / (float)P;
     L.spin_limit = 1ull << 23;  // all ranks start together here: a few seconds mean a bug
     L.part = chain_partition(n, block, tile, channels);
     L.tile = (uint32_t)tile;
     for (int r = 0; r < P; ++r) {
         char *b = (char *)base;
-        fill_rank(L.rank[r], l, bufs[r], outs[r], op == LP_OP_BSP_SGD ? outs[r] : nullptr, b + l.bytes * (size_t)r,
+        fill_rank(L.rank[r], l, bufs[r], outs[r], chain_sgd(op) ? outs[r] : nullptr, op == LP_OP_BSP_SGD_MOM ? vel : nullptr,
+                  b + l.bytes * (size_t)r,
                   b + l.bytes * (size_t)roles[r].up, b + l.bytes * (size_t)roles[r].down, roles[r]);
     }
     const cudaError_t e = launch(L, true, (cudaStream_t)cuda_stream);
@@ -1110,6 +1162,14 @@ int lp_chain_emulate_bsp_sgd_step(float *const *grads, float *const *weights, in
     if (weights == nullptr) return LP_ERR_INVALID_ARG;
     return chain_emulate(LP_OP_BSP_SGD, grads, weights, P, n, block, 0, LP_REDUCE_SUM, n * sizeof(float), lr, channels, slots,
                          tile, cuda_stream);
+}
+
+int lp_chain_emulate_bsp_sgd_momentum_step(float *const *grads, float *const *weights, float *velocity, int P, size_t n,
+                                           size_t block, float lr, float mu, int channels, int slots, int tile,
+                                           void *cuda_stream) {
+    if (weights == nullptr) return LP_ERR_INVALID_ARG;
+    return chain_emulate(LP_OP_BSP_SGD_MOM, grads, weights, P, n, block, 0, LP_REDUCE_SUM, n * sizeof(float), lr, channels,
+                         slots, tile, cuda_stream, velocity, mu);
 }
 
 // error word of emulated rank `rank` for the geometry (P, channels, slots, tile); synchronises the device

@@ -97,6 +97,7 @@ def test_chain_sgd_step_roles():
         for r in range(P):
             a = lp.lp_chain_plan(lp.OP_ALLREDUCE, P, 0, r)
             g = lp.lp_chain_plan(lp.OP_BSP_SGD, P, 0, r)
+            assert lp.lp_chain_plan(lp.OP_BSP_SGD_MOM, P, 0, r) == g          # momentum: the same roles
             assert g["f_update"] == (1 if r == P - 1 else 0) and a["f_update"] == 0
             if P > 1:
                 assert {k: v for k, v in g.items() if k != "f_update"} == {k: v for k, v in a.items() if k != "f_update"}
@@ -121,7 +122,7 @@ def test_chain_plan_argument_errors():
     assert L.lp_chain_plan(lp.OP_ALLREDUCE, 33, 0, 0, ref) == lp.LP_ERR_INVALID_ARG
     assert L.lp_chain_plan(lp.OP_ALLREDUCE, 4, 0, 4, ref) == lp.LP_ERR_INVALID_ARG
     assert L.lp_chain_plan(lp.OP_REDUCE, 4, 4, 0, ref) == lp.LP_ERR_INVALID_ARG
-    assert L.lp_chain_plan(lp.OP_BSP_SGD_MOM, 4, 0, 0, ref) == lp.LP_ERR_INVALID_ARG
+    assert L.lp_chain_plan(5, 4, 0, 0, ref) == lp.LP_ERR_INVALID_ARG and L.lp_chain_plan(-1, 4, 0, 0, ref) == lp.LP_ERR_INVALID_ARG
     assert L.lp_chain_plan(lp.OP_ALLREDUCE, 4, 99, 0, ref) == lp.LP_OK          # allreduce ignores the root
     assert L.lp_chain_endpoint_bytes(32, 8, 16384) == 32 * 64 * 8 + 32 * 4 * 8 + 256 + 2 * 32 * 8 * 16384 * 4 \
         or L.lp_chain_endpoint_bytes(32, 8, 16384) > 2 * 32 * 8 * 16384 * 4

@@ -149,6 +149,26 @@ def test_chain_fused_bsp_sgd_step(oracle, P, n, block):
         assert got_g[r].tobytes() == grads[r].tobytes(), ("grads must be untouched", r)
 
 
+@pytest.mark.parametrize("P,n,block", [(1, 5_001, 1024), (3, 70_001, 4096), (6, 300_003, 65_536), (16, 100_003, 0)])
+def test_chain_fused_bsp_sgd_momentum_step(oracle, P, n, block):
+    """The paper's solver (U18) over the chain: five RN operations at the chain's end, the velocity lives
+    there; four steps back to back (the velocity feeds back), against the oracle's momentum step with root = P - 1."""
+    grads, weights = inputs.sgd_inputs([39, n], P, n)
+    weights = [w + np.float32(r) for r, w in enumerate(weights)]
+    hw = [w.copy() for w in weights]
+    hv = np.zeros(n, dtype=np.float32)
+    dg, dw = up(grads), up(weights)
+    dv = torch.zeros(n, device="cuda")
+    for _ in range(4):
+        oracle.bsp_sgd_momentum_step(grads, hw, hv, root=P - 1, lr=0.01, mu=0.9)
+        lp.lp_chain_emulate_bsp_sgd_momentum_step(dg, dw, dv, block=block, lr=0.01, mu=0.9)
+    got_w = down(dw)
+    assert lp.lp_chain_emulate_error(P) == 0
+    assert dv.cpu().numpy().tobytes() == hv.tobytes(), "velocity"
+    for r in range(P):
+        assert got_w[r].tobytes() == hw[r].tobytes(), ("weights", r)
+
+
 @pytest.mark.parametrize("dt", [inputs.DT_F16, inputs.DT_BF16, inputs.DT_F64])
 def test_chain_element_types(oracle, dt):
     P, n = 5, 200_002
