@@ -378,6 +378,11 @@ LP_API int lp_chain_bsp_sgd_step(lp_chain *ch, float *grad, float *weight, size_
  * floats, 16-byte aligned, rewritten in place), every other rank passes NULL. */
 LP_API int lp_chain_bsp_sgd_momentum_step(lp_chain *ch, float *grad, float *weight, float *velocity, size_t n, size_t block,
                                           float lr, float mu, void *cuda_stream);
+/* Alg. 2 over the chain (U9; prose PAPER.md:178): lp_chain reduce of `grad` to `root` (grad <- S there),
+ * GradientUpdate on the root's `weight` (velocity: the root's vector or NULL for the plain step; other ranks pass NULL),
+ * broadcast of `weight` from the root.  Weights (and velocity) come out bit-identical to the fused steps. */
+LP_API int lp_chain_bsp_sgd_alg2_step(lp_chain *ch, float *grad, float *weight, float *velocity, size_t n, size_t block,
+                                      int root, float lr, float mu, void *cuda_stream);
 LP_API int lp_chain_error(lp_chain *ch, int *error_out);
 LP_API int lp_chain_destroy(lp_chain *ch);
 LP_API int lp_chain_emulate(int op, float *const *bufs, int P, size_t n, size_t block, int root, int reduce_op, int channels,
@@ -391,6 +396,9 @@ LP_API int lp_chain_emulate_bsp_sgd_step(float *const *grads, float *const *weig
 LP_API int lp_chain_emulate_bsp_sgd_momentum_step(float *const *grads, float *const *weights, float *velocity, int P, size_t n,
                                                   size_t block, float lr, float mu, int channels, int slots, int tile,
                                                   void *cuda_stream);
+LP_API int lp_chain_emulate_bsp_sgd_alg2_step(float *const *grads, float *const *weights, float *velocity, int P, size_t n,
+                                              size_t block, int root, float lr, float mu, int channels, int slots, int tile,
+                                              void *cuda_stream);
 LP_API int lp_chain_emulate_channels(int P, int tile);
 LP_API int lp_chain_emulate_error(int P, int channels, int slots, int tile, int *error_out);
 

@@ -130,6 +130,8 @@ def lib() -> ctypes.CDLL:
     L.lp_chain_emulate_bsp_sgd_step.argtypes = [pp, pp, i32, sz, sz, f32, i32, i32, i32, vp]
     L.lp_chain_bsp_sgd_momentum_step.argtypes = [vp, vp, vp, vp, sz, sz, f32, f32, vp]
     L.lp_chain_emulate_bsp_sgd_momentum_step.argtypes = [pp, pp, vp, i32, sz, sz, f32, f32, i32, i32, i32, vp]
+    L.lp_chain_bsp_sgd_alg2_step.argtypes = [vp, vp, vp, vp, sz, sz, i32, f32, f32, vp]
+    L.lp_chain_emulate_bsp_sgd_alg2_step.argtypes = [pp, pp, vp, i32, sz, sz, i32, f32, f32, i32, i32, i32, vp]
     L.lp_chain_error.argtypes = [vp, ctypes.POINTER(i32)]
     L.lp_chain_destroy.argtypes = [vp]
     L.lp_chain_emulate.argtypes = [i32, pp, i32, sz, sz, i32, i32, i32, i32, i32, vp]
@@ -384,6 +386,18 @@ def lp_chain_emulate_bsp_sgd_momentum_step(grads, weights, velocity, block=0, lr
                                                         _stream_ptr(stream)), "lp_chain_emulate_bsp_sgd_momentum_step")
 
 
+def lp_chain_emulate_bsp_sgd_alg2_step(grads, weights, velocity=None, block=0, root=0, lr=0.01, mu=0.0, channels=0, slots=0,
+                                       tile=0, stream=None):
+    """Alg. 2 over the emulated chain: reduce to root, root update, broadcast."""
+    ga, n = _dev_ptrs(grads)
+    wa, nw = _dev_ptrs(weights)
+    if n != nw or len(grads) != len(weights):
+        raise ValueError("grads and weights must match in P and n")
+    _check(lib().lp_chain_emulate_bsp_sgd_alg2_step(ga, wa, _velocity_ptr(velocity, n), len(grads), n, block, root,
+                                                    ctypes.c_float(lr), ctypes.c_float(mu), channels, slots, tile,
+                                                    _stream_ptr(stream)), "lp_chain_emulate_bsp_sgd_alg2_step")
+
+
 def lp_chain_emulate_error(P, channels=0, slots=0, tile=0) -> int:
     e = ctypes.c_int(0)
     _check(lib().lp_chain_emulate_error(P, channels, slots, tile, ctypes.byref(e)), "lp_chain_emulate_error")
@@ -453,6 +467,12 @@ class Chain:
         _check(lib().lp_chain_bsp_sgd_momentum_step(self.h, ctypes.c_void_p(grad.data_ptr()), ctypes.c_void_p(weight.data_ptr()),
                                                     vp_, grad.numel(), block, ctypes.c_float(lr), ctypes.c_float(mu),
                                                     _stream_ptr(stream)), "lp_chain_bsp_sgd_momentum_step")
+
+    def bsp_sgd_alg2_step(self, grad, weight, velocity=None, block=0, root=0, lr=0.01, mu=0.0, stream=None):
+        vp_ = ctypes.c_void_p(velocity.data_ptr()) if velocity is not None else None
+        _check(lib().lp_chain_bsp_sgd_alg2_step(self.h, ctypes.c_void_p(grad.data_ptr()), ctypes.c_void_p(weight.data_ptr()), vp_,
+                                                grad.numel(), block, root, ctypes.c_float(lr), ctypes.c_float(mu),
+                                                _stream_ptr(stream)), "lp_chain_bsp_sgd_alg2_step")
 
     def error(self) -> int:
         e = ctypes.c_int(0)

@@ -1039,6 +1039,23 @@ int lp_chain_bsp_sgd_momentum_step(lp_chain *ch, float *grad, float *weight, flo
                           mu);
 }
 
+// Alg. 2 over the chain (PAPER.md:140-168 as read in U9, prose PAPER.md:178): reduce the sub-gradients to `root`
+// (grad <- S there, as lp_reduce does, U20), the root applies GradientUpdate to its replica (the same rounded operations
+// as the fused steps; velocity != NULL on the root: the momentum form), the new weights are broadcast from the root.
+// Three launches on the root, two on every other rank -- the two-synchronisation-point counterpart of the fused step.
+int lp_chain_bsp_sgd_alg2_step(lp_chain *ch, float *grad, float *weight, float *velocity, size_t n, size_t block, int root,
+                               float lr, float mu, void *cuda_stream) {
+    if (ch == nullptr || weight == nullptr || grad == weight || root < 0 || root >= ch->P) return LP_ERR_INVALID_ARG;
+    int rc = chain_run_rank(ch, LP_OP_REDUCE, grad, grad, nullptr, n, block, root, LP_REDUCE_SUM, 0.f, cuda_stream);
+    if (rc != LP_OK) return rc;
+    if (ch->rank == root && n > 0) {
+        const cudaError_t e = lp_update_launch(weight, grad, velocity, n, lr, 1.0f / (float)ch->P, mu, (cudaStream_t)cuda_stream,
+                                               false);
+        if (e != cudaSuccess) return chain_fail(e);
+    }
+    return chain_run_rank(ch, LP_OP_BROADCAST, weight, weight, nullptr, n, block, root, LP_REDUCE_SUM, 0.f, cuda_stream);
+}
+
 // 0 = no wait of this endpoint's kernels has given up so far (a peer that never arrived); synchronises the device.
 int lp_chain_error(lp_chain *ch, int *error_out) {
     if (ch == nullptr || error_out == nullptr) return LP_ERR_INVALID_ARG;
@@ -1162,6 +1179,24 @@ int lp_chain_emulate_bsp_sgd_step(float *const *grads, float *const *weights, in
     if (weights == nullptr) return LP_ERR_INVALID_ARG;
     return chain_emulate(LP_OP_BSP_SGD, grads, weights, P, n, block, 0, LP_REDUCE_SUM, n * sizeof(float), lr, channels, slots,
                          tile, cuda_stream);
+}
+
+// reduce (one cooperative launch), GradientUpdate on the root's vectors, broadcast (one cooperative launch)
+int lp_chain_emulate_bsp_sgd_alg2_step(float *const *grads, float *const *weights, float *velocity, int P, size_t n,
+                                       size_t block, int root, float lr, float mu, int channels, int slots, int tile,
+                                       void *cuda_stream) {
+    if (weights == nullptr || grads == nullptr || P < 1 || P > LP_MAX_P || root < 0 || root >= P) return LP_ERR_INVALID_ARG;
+    int rc = chain_emulate(LP_OP_REDUCE, grads, grads, P, n, block, root, LP_REDUCE_SUM, n * sizeof(float), 0.f, channels, slots,
+                           tile, cuda_stream);
+    if (rc != LP_OK) return rc;
+    if (weights[root] == nullptr || ((uintptr_t)weights[root] & 15u)) return LP_ERR_INVALID_ARG;
+    if (n > 0) {
+        const cudaError_t e = lp_update_launch(weights[root], grads[root], velocity, n, lr, 1.0f / (float)P, mu,
+                                               (cudaStream_t)cuda_stream, false);
+        if (e != cudaSuccess) return chain_fail(e);
+    }
+    return chain_emulate(LP_OP_BROADCAST, weights, weights, P, n, block, root, LP_REDUCE_SUM, n * sizeof(float), 0.f, channels,
+                         slots, tile, cuda_stream);
 }
 
 int lp_chain_emulate_bsp_sgd_momentum_step(float *const *grads, float *const *weights, float *velocity, int P, size_t n,

@@ -169,6 +169,27 @@ def test_chain_fused_bsp_sgd_momentum_step(oracle, P, n, block):
         assert got_w[r].tobytes() == hw[r].tobytes(), ("weights", r)
 
 
+@pytest.mark.parametrize("root", [0, 2, 4])
+def test_chain_alg2_step(oracle, root):
+    """Alg. 2 over the chain (reduce to root, root update, broadcast): the oracle's Alg. 2 step, bit for bit -- the
+    reduced gradient lands in the root's gradient vector (U20), weights and velocity equal the fused step's."""
+    P, n = 5, 200_003
+    grads, weights = inputs.sgd_inputs([40, root], P, n)
+    hg, hw = [g.copy() for g in grads], [w.copy() for w in weights]
+    hv = np.zeros(n, dtype=np.float32)
+    dg, dw = up(grads), up(weights)
+    dv = torch.zeros(n, device="cuda")
+    for _ in range(2):
+        oracle.bsp_sgd_alg2_step(hg, hw, hv, root=root, lr=0.01, mu=0.9)
+        lp.lp_chain_emulate_bsp_sgd_alg2_step(dg, dw, dv, block=8192, root=root, lr=0.01, mu=0.9)
+    got_w, got_g = down(dw), down(dg)
+    assert lp.lp_chain_emulate_error(P) == 0
+    assert dv.cpu().numpy().tobytes() == hv.tobytes()
+    for r in range(P):
+        assert got_w[r].tobytes() == hw[r].tobytes(), ("weights", r)
+        assert got_g[r].tobytes() == hg[r].tobytes(), ("grads", r)
+
+
 @pytest.mark.parametrize("dt", [inputs.DT_F16, inputs.DT_BF16, inputs.DT_F64])
 def test_chain_element_types(oracle, dt):
     P, n = 5, 200_002
