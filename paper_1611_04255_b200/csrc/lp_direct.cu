@@ -193,12 +193,12 @@ uint32_t lp_direct_tile(const LpTuning &t, const LpArgs &a, uint64_t n_work, int
     uint32_t tile = (reduce_only && a.n_sum == 2) ? 4096u : ((a.n_sum <= 8 && a.n_out < 12) || reduce_only ? 2048u : 1024u);
     // Latency regime: halve the tile while the message has fewer tiles than `few` so that more SMs share it.  A fold
     // over several ranks wants two grid-fulls of tiles (its threads have many loads in flight each: more, smaller CTAs
-    // hide more latency); a copy or a two-rank fold wants one CTA per SM and no more -- fewer, fatter CTAs cost less
+    // hide more latency); a copy, a two-rank fold or a reduce (one store stream) wants one CTA per SM and no more -- fewer, fatter CTAs cost less
     // to launch, and a broadcast to many ranks runs 3-4 CTAs per SM (lp_direct_occupancy), so four tiles per SM no
     // longer fit in one wave (P = 8, 2 MB broadcast: 4.06 -> 3.2 us; P = 2, 2 MB reduce: 1.92 -> 1.44 us;
     // profiles/r2_tuning.md section 8).  A reduce over more than 8 ranks (below the pipeline cut-off: < 40 MB per rank)
     // runs 5-18 % faster on 8 KB tiles than on 4 KB ones.
-    uint64_t few = (a.epilogue == LP_EPI_COPY || a.n_sum <= 2) ? (uint64_t)sm_count : 2ull * (uint64_t)sm_count;
+    uint64_t few = (a.epilogue == LP_EPI_COPY || a.n_sum <= 2 || reduce_only) ? (uint64_t)sm_count : 2ull * (uint64_t)sm_count;
     if (a.epilogue == LP_EPI_COPY && a.n_out == 1) few = (uint64_t)sm_count / 2u;  // the plain copy: half a grid-full is enough
     while (tile > 1024u && (n_work + tile - 1) / tile < few) tile /= 2u;
     return tile;
