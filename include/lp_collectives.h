@@ -295,7 +295,7 @@ LP_API int lp_be_allreduce_op(float *const *bufs, int P, size_t n, int reduce_op
  * allreduce sends the finished block back down (U3-A), broadcast runs root -> root+1 -> ... around the ring.  An
  * lp_chain is ONE rank's endpoint: receive rings and counters in its own device memory that its two neighbours write
  * through peer mappings (data pushed with plain stores, published with fence.acq_rel.sys + a counter in the
- * receiver's memory; slots returned by a credit counter in the sender's memory; csrc/lp_chain.cu).
+ * receiver's memory; slots returned by a credit counter in the sender's memory; csrc/lp_chain.cu, lp_chain_api.cu).
  *   lp_chain_create(rank, P, channels, slots, tile, &ch)   on the rank's device (current device); 0 = defaults.  Every
  *       rank must pass the same (P, channels, slots, tile).  channels: 1..LP_CHAIN_MAX_CHANNELS concurrent rings, 2 CTAs
  *       (one SM) each.  A CTA of the default kernel moves ~75 GB/s and a block costs three memory accesses on its way
@@ -354,6 +354,8 @@ typedef struct lp_chain_role {
 #define LP_CHAIN_KERNEL_TMA 2
 LP_API int lp_chain_set_kernel(int kernel);
 LP_API int lp_chain_plan(int op, int P, int root, int rank, lp_chain_role *out);
+/* device bytes one endpoint takes for (channels, slots, tile): 2 x channels x slots x tile x 4 for the two rings, plus
+ * counters; 0 for an invalid geometry.  Host only. */
 LP_API size_t lp_chain_endpoint_bytes(int channels, int slots, int tile);
 LP_API int lp_chain_create(int rank, int P, int channels, int slots, int tile, lp_chain **out);
 LP_API int lp_chain_get_handle(lp_chain *ch, void *handle_out);
@@ -399,7 +401,10 @@ LP_API int lp_chain_emulate_bsp_sgd_momentum_step(float *const *grads, float *co
 LP_API int lp_chain_emulate_bsp_sgd_alg2_step(float *const *grads, float *const *weights, float *velocity, int P, size_t n,
                                               size_t block, int root, float lr, float mu, int channels, int slots, int tile,
                                               void *cuda_stream);
+/* channels per rank the emulation takes when asked for 0: LP_CHAIN_EMULATE_CHANNELS, fewer when P x 2 x channels CTAs
+ * would not all be resident on the current device (1 without a device) */
 LP_API int lp_chain_emulate_channels(int P, int tile);
+/* synchronises the device; *error_out != 0: a wait of an emulated rank of this (P, geometry) gave up on some stream */
 LP_API int lp_chain_emulate_error(int P, int channels, int slots, int tile, int *error_out);
 
 /* ---- host-buffer entry points (end-to-end path) ------------------------------- */
