@@ -244,6 +244,33 @@ def test_chain_seeded_fuzz(oracle):
     assert checked > 40 and all(lp.lp_chain_emulate_error(P, **g) == 0 for P, g in geoms.items())
 
 
+def test_chain_two_streams_do_not_share_rings(oracle):
+    """Emulated endpoints belong to (P, geometry, stream): two chains of the same shape running at the same time on two
+    streams must not see each other's blocks."""
+    P, n = 3, 400_003
+    srcs = [inputs.rank_vectors([42, k], P, n, "uniform") for k in range(2)]
+    wants = []
+    for src in srcs:
+        w = [a.copy() for a in src]
+        oracle.allreduce(w)
+        wants.append(w)
+    devs = [up(src) for src in srcs]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    torch.cuda.synchronize()
+    for rep in range(3):
+        for k in range(2):
+            for d, a in zip(devs[k], srcs[k]):
+                d.copy_(torch.from_numpy(a))
+        torch.cuda.synchronize()
+        for k in range(2):
+            lp.lp_chain_emulate(lp.OP_ALLREDUCE, devs[k], block=8192, channels=4, slots=2, tile=4096, stream=streams[k])
+        torch.cuda.synchronize()
+        for k in range(2):
+            for r in range(P):
+                assert devs[k][r].cpu().numpy().tobytes() == wants[k][r].tobytes(), (rep, k, r)
+    assert lp.lp_chain_emulate_error(P, 4, 2, 4096) == 0
+
+
 def test_chain_argument_errors():
     dev = [torch.zeros(64, device="cuda") for _ in range(2)]
     arr, n = lp._dev_ptrs(dev)
