@@ -186,6 +186,21 @@ def test_compute_entry_fails_loudly_without_device():
             raise lp.LpError(rc, "lp_plan_run")
     assert ei.value.status == lp.LP_ERR_CUDA
     assert "no CUDA device" in lp.status_string(lp.LP_ERR_CUDA)
+    # the typed calls, the typed slice lists and the chain: validation first, then the same refusal
+    s0 = ctypes.c_void_p(0)
+    for dt in (lp.DT_F16, lp.DT_BF16, lp.DT_F64):
+        assert L.lp_allreduce_dt(ptrs, 2, 32, 16, dt, lp.REDUCE_SUM, s0) == lp.LP_ERR_CUDA
+        assert L.lp_reduce_dt(ptrs, 2, 32, 16, 1, dt, lp.REDUCE_PROD, s0) == lp.LP_ERR_CUDA
+        assert L.lp_broadcast_dt(ptrs, 2, 32, 16, 0, dt, s0) == lp.LP_ERR_CUDA
+    assert L.lp_allreduce_dt(ptrs, 2, 32, 16, 9, lp.REDUCE_SUM, s0) == lp.LP_ERR_INVALID_ARG
+    assert L.lp_allreduce_dt(ptrs, 2, 32, 16, lp.DT_F64, 9, s0) == lp.LP_ERR_INVALID_ARG
+    off = (ctypes.c_size_t * 1)(3)
+    ln = (ctypes.c_size_t * 1)(8)
+    assert L.lp_allreduce_segments_dt(ptrs, 2, 32, off, ln, 1, 16, lp.DT_F16, lp.REDUCE_SUM, s0) == lp.LP_ERR_INVALID_ARG
+    off[0] = 4
+    assert L.lp_allreduce_segments_dt(ptrs, 2, 32, off, ln, 1, 16, lp.DT_F16, lp.REDUCE_SUM, s0) == lp.LP_ERR_CUDA
+    assert L.lp_chain_emulate(ALLREDUCE, ptrs, 2, 64, 16, 0, lp.REDUCE_SUM, 2, 2, 4096, s0) in (lp.LP_ERR_CUDA, lp.LP_ERR_UNSUPPORTED)
+    assert lp.lp_dtype_size(lp.DT_F32) == 4 and lp.lp_dtype_size(lp.DT_BF16) == 2 and lp.lp_dtype_size(-1) == 0
     assert not raw[0].any() and not raw[1].any()
 
 
