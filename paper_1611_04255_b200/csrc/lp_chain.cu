@@ -19,7 +19,10 @@
 // partial, combine in chain order, push up; the last rank stores / turns the finished tile around) and C return CTAs
 // (wait for a finished tile, store it to my vector, push it further down).  No CTA of a rank waits for another CTA of
 // the same rank; a channel advances whenever its CTAs are resident on every rank, and the grid never exceeds what
-// the device holds at once.
+// the device holds at once.  Two realisations of a rank's CTAs follow, same protocol between ranks: the register kernel
+// (lp_chain_kernel: 1024 threads load, fold and store in lock-step) and, the default, the TMA-load kernel
+// (lp_chain_tma_kernel: everything a rank reads is local, so a producer thread streams it through a shared-memory ring).
+// Host side (endpoints, roles, launches, emulation entry points): lp_chain_api.cu.
 //
 // ONE GPU (this build's box): kernels that wait on each other must not run as separate launches on one device, so
 // lp_chain_emulate runs the SAME per-rank code for all P ranks inside ONE cooperative launch (P x 2 C co-resident
