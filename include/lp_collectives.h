@@ -144,8 +144,9 @@ extern "C" {
                                    a ring slot holds a run of up to div granules.  Claims shrink from LP_TUNE_CLAIM_SLOTS
                                    slots to one granule as the tile list runs out ("guided self-scheduling") */
 #define LP_TUNE_CLAIM_SLOTS 11  /* pipeline variant: ring slots' worth of granules per claim while the list is long (1..16, default 1) */
-#define LP_TUNE_PREFETCH 12     /* pipeline variant: 0/1 a CTA prefetches its first loads into L2 before it waits for the
-                                   predecessor kernel (programmatic dependent launch), 2 = off */
+#define LP_TUNE_PREFETCH 12     /* pipeline and direct variants: 0/1 a CTA prefetches its first loads into L2 before it waits for
+                                   the predecessor kernel (programmatic dependent launch): the start of a call overlaps the
+                                   drain of the call before it even when the two touch the same buffers; 2 = off */
 #define LP_TUNE_CLUSTER_TILE 13 /* cluster variant: tile elements, 1024 / 2048 (default) / 4096 */
 #define LP_TUNE_CHAIN 14        /* 0/1: a call whose buffers overlap none of the calls still in flight ahead of it on its stream
                                    does not wait for them before it starts (it waits before it ENDS, so completion order

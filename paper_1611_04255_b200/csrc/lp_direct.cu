@@ -48,6 +48,19 @@ __global__ void __launch_bounds__(kThreads)
     // wait first, then trigger: at most ONE successor waits behind a running kernel (triggering before the wait lets
     // a whole queue of short kernels pile up on the SMs, each blocked on its predecessor: measured 2x slower at 256 KB)
     // A launch that touches none of the buffers of the launches ahead of it (a.late_wait) waits before it exits instead.
+    if (a.prefetch) {  // this CTA's first tile into L2 while the predecessor kernel drains (a hint: L2 is the point of
+                       // coherence, so it is harmless even if the predecessor is still writing these vectors)
+        uint64_t off;
+        uint32_t len;
+        if ((uint64_t)blockIdx.x < a.part.n_tiles) {
+            lp_lookup_tile<SEG>(a, segs, blockIdx.x, off, len);
+            const uint32_t lines = (len * 4u + 127u) / 128u;  // 128-byte lines of the tile, per input
+            for (uint32_t l = tid; l < lines * (uint32_t)a.n_in; l += kThreads) {
+                const uint32_t r = l / lines, k = l - r * lines;
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(a.in[r] + off + (uint64_t)k * 32u));
+            }
+        }
+    }
     if (!a.late_wait) lp_pdl_wait();
     lp_pdl_trigger();  // every CTA of this grid is resident or done once the last one gets here
     for (uint64_t t = blockIdx.x; t < a.part.n_tiles; t += gridDim.x) {
@@ -228,6 +241,9 @@ cudaError_t lp_direct_launch(const LpArgs &a_in, const lp_seg_table *segs, const
         const int nr = lp_args_ranges(a, ranges);
         a.late_wait = lp_chain_admit(stream, ranges, nr, cfg->pdl, t.v[LP_TUNE_CHAIN] != 2) ? 1 : 0;
     }
+    // L2 prefetch of every CTA's first tile before it waits for its predecessor (LP_TUNE_PREFETCH 2 = off): only when the
+    // launch really waits first, and only for one CTA per tile (a confined grid walks many tiles per CTA)
+    a.prefetch = (cfg->pdl && !a.late_wait && t.v[LP_TUNE_PREFETCH] != 2 && grid == a.part.n_tiles) ? 1 : 0;
     switch (a.part.tile) {
         case 1024: return launch_seg<1>(a, segs, *cfg, stream);
         case 2048: return launch_seg<2>(a, segs, *cfg, stream);
