@@ -152,7 +152,9 @@ extern "C" {
                                    does not wait for them before it starts (it waits before it ENDS, so completion order
                                    on the stream is kept): back-to-back collectives on different buffers -- the layers of
                                    Alg. 1, rotating buffer sets -- run into each other without a bubble; 2 = off, every
-                                   call waits for its predecessor first */
+                                   call waits for its predecessor first.  0 (default) leaves one case to the library: a
+                                   long reduce over 3 or more ranks in the direct variant waits first and prefetches (1-2 %
+                                   faster than sharing the SMs with its predecessor's tail); 1 chains that too */
 #define LP_TUNE_DIRECT_OCC 15   /* direct variant: at most this many CTAs resident per SM (1..8; 0 = the library's choice by
                                    collective: write-heavy launches run best with few stores in flight) */
 #define LP_TUNE_COUNT 16
