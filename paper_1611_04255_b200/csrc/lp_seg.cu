@@ -19,7 +19,23 @@ constexpr int kSegUnroll = 4;
 __device__ __forceinline__ void lp_seg_body(const LpSegArgs &s);
 
 __global__ void __launch_bounds__(kSegThreads) lp_seg_kernel(const __grid_constant__ LpSegArgs s) {
-    if (!s.late_wait) lp_pdl_wait();  // the previous level (or whatever precedes in the stream) has completed
+    if (!s.late_wait) {
+        // like the LP direct kernel (the baselines get every launch-side advantage LP has): this CTA's chunk of both
+        // operands into L2 while the previous level drains; L2 is the point of coherence, so lines the previous level
+        // is still writing end up with its values
+        const LpSegJob &job = s.j[blockIdx.y];
+        const uint64_t per = (uint64_t)kSegThreads * kSegUnroll * 4;
+        const uint64_t lo = (uint64_t)blockIdx.x * per;
+        if (lo < job.len) {
+            const uint64_t n = job.len - lo < per ? job.len - lo : per;
+            const uint32_t lines = (uint32_t)((n * 4u + 127u) / 128u);
+            for (uint32_t l = threadIdx.x; l < 2u * lines; l += kSegThreads) {
+                const float *base = l < lines ? job.a : job.b;
+                if (base) asm volatile("prefetch.global.L2 [%0];" ::"l"(base + lo + (uint64_t)(l < lines ? l : l - lines) * 32u));
+            }
+        }
+        lp_pdl_wait();  // the previous level (or whatever precedes in the stream) has completed
+    }
     lp_pdl_trigger();  // one chunk per CTA: once the last CTA is resident the next level's kernel may be scheduled
     lp_seg_body(s);
     if (s.late_wait && threadIdx.x == 0) lp_pdl_wait();
