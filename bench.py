@@ -729,24 +729,24 @@ def dtype_rows(torch, lp, dev, P=6, msg_bytes=256 << 20):
 def chain_rows(torch, lp, dev, msg_bytes=64 << 20):
     """the one-rank-per-GPU chain (csrc/lp_chain.cu) as far as ONE GPU can run it -- all P ranks in
     one cooperative launch (lp_chain_emulate), every 'link' being this GPU's own HBM.  So this measures the PROTOCOL
-    (push + publish + credit per 256 KB tile), not NVLink: per_link_GBps = message bytes / time is what every emulated link
+    (push + publish + credit per block), not NVLink: per_link_GBps = message bytes / time is what every emulated link
     direction carried; hbm_GBps counts what the emulation really moves, (6P-4) n 4 bytes for an allreduce (P loads, P stores
     and 2(P-1) ring writes + reads), (3P-2) n 4 for a broadcast.  Eager launches, K back to back between two events."""
     n = msg_bytes // 4
-    out = {"msg_MB": msg_bytes / 2 ** 20, "tile_elems": 65_536, "slots": 8,
+    out = {"msg_MB": msg_bytes / 2 ** 20, "tile_elems": 131_072, "slots": 8, "block": "0 = the cost model's choice",
            "what": "us per call, GB/s per emulated link direction, HBM GB/s of the emulation; NOT an NVLink measurement"}
     for P in (2, 4, 8):
         bufs = [torch.full((n,), 0.001 * (r + 1), device=dev) for r in range(P)]
         row = {"channels": lp.lp_chain_emulate_channels(P)}
         for op, op_id, moved in (("allreduce", lp.OP_ALLREDUCE, 6 * P - 4), ("broadcast", lp.OP_BROADCAST, 3 * P - 2)):
             for _ in range(2):
-                lp.lp_chain_emulate(op_id, bufs, block=65_536)
+                lp.lp_chain_emulate(op_id, bufs, block=0)
             torch.cuda.synchronize()
             K = 10
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             e0.record()
             for _ in range(K):
-                lp.lp_chain_emulate(op_id, bufs, block=65_536)
+                lp.lp_chain_emulate(op_id, bufs, block=0)
             e1.record()
             torch.cuda.synchronize()
             us = e0.elapsed_time(e1) * 1e3 / K
@@ -758,12 +758,12 @@ def chain_rows(torch, lp, dev, msg_bytes=64 << 20):
         if P == 2:  # the register realisation of a rank's CTAs beside the default (TMA loads), same protocol
             lp.lp_chain_set_kernel(lp.CHAIN_KERNEL_REGISTER)
             for _ in range(2):
-                lp.lp_chain_emulate(lp.OP_ALLREDUCE, bufs, block=65_536)
+                lp.lp_chain_emulate(lp.OP_ALLREDUCE, bufs, block=0)
             torch.cuda.synchronize()
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             e0.record()
             for _ in range(10):
-                lp.lp_chain_emulate(lp.OP_ALLREDUCE, bufs, block=65_536)
+                lp.lp_chain_emulate(lp.OP_ALLREDUCE, bufs, block=0)
             e1.record()
             torch.cuda.synchronize()
             us = e0.elapsed_time(e1) * 1e3 / 10

@@ -304,8 +304,8 @@ LP_API int lp_be_allreduce_op(float *const *bufs, int P, size_t n, int reduce_op
  *       (one SM) each.  A CTA of the default kernel moves ~75 GB/s and a block costs three memory accesses on its way
  *       through a middle rank's forward CTA (and three through its return CTA), i.e. ~25 GB/s of link payload per CTA:
  *       a 900 GB/s NVLink direction takes ~36 forward + ~36 return CTAs -- hence 40, about half the SMs; slots: ring depth
- *       1..64; tile: elements per slot = the unit of a flag exchange, a power of two from 4096 to 262144 (default 65536
- *       floats = 256 KB = the LP block of BASELINE.json's configs; 16384 = the paper's 64 KB).
+ *       1..64; tile: elements per slot = the largest unit of a flag exchange, a power of two from 4096 to 262144 (default
+ *       131072 floats = 512 KB; 65536 = the LP block of BASELINE.json's configs; 16384 = the paper's 64 KB).
  *   lp_chain_get_handle(ch, h)     LP_CHAIN_HANDLE_BYTES opaque bytes (a CUDA IPC handle) to all-gather over any
  *       transport (paper_1611_04255_b200/chain.py uses torch.distributed);
  *   lp_chain_connect(ch, handles)  handles = P x LP_CHAIN_HANDLE_BYTES in rank order; maps ranks (rank +- 1) mod P.
@@ -315,9 +315,11 @@ LP_API int lp_be_allreduce_op(float *const *bufs, int P, size_t n, int reduce_op
  *       ALLREDUCE on its vector buf (n floats, 16-byte aligned, in place; same semantics and the same bits as
  *       lp_broadcast / lp_reduce_op / lp_allreduce_op over P virtual ranks).  Every rank calls it with the same
  *       arguments, in the same order as its other chain collectives, on one stream per endpoint.  `block` is rounded
- *       up to a multiple of 4 elements and moved in pieces of at most one tile; 0 = the library chooses: one tile for
- *       long messages, for short ones the power of two (>= 4096) that still gives every channel about four blocks, so
- *       that the chain fills after a small block (the fill term of the pipeline is (p - 1) b).
+ *       up to a multiple of 4 elements and moved in pieces of at most one tile; 0 = the library chooses: the power of two
+ *       (4096 elements .. one tile) nearest to the block that minimises the paper's cost model for one channel's share
+ *       of the message (Table 1: (p - 1 + n_c / b)(2 alpha + b (2 beta + gamma)); lp_optimal_block with
+ *       the constants fitted to this kernel, lp_chain_fitted_constants) -- small blocks fill the chain sooner, large
+ *       ones pay fewer flag exchanges.
  *   lp_chain_error(ch, &e)   synchronises; e != 0: a wait gave up (a neighbour never arrived) and the result is void.
  * lp_chain_plan is the host-only part: what `rank` does in (op, P, root) -- its ring neighbours and which of the steps
  * load / receive / store / send up / send down its forward and return CTAs take.  No device needed.
@@ -332,7 +334,7 @@ LP_API int lp_be_allreduce_op(float *const *bufs, int P, size_t n, int reduce_op
 #define LP_CHAIN_DEFAULT_CHANNELS 40
 #define LP_CHAIN_EMULATE_CHANNELS 16
 #define LP_CHAIN_DEFAULT_SLOTS 8
-#define LP_CHAIN_DEFAULT_TILE 65536
+#define LP_CHAIN_DEFAULT_TILE 131072
 typedef struct lp_chain lp_chain;
 typedef struct lp_chain_role {
     int position;     /* place in the chain of this collective: rank for reduce / allreduce, (rank - root) mod P for broadcast */
@@ -356,6 +358,12 @@ typedef struct lp_chain_role {
 #define LP_CHAIN_KERNEL_REGISTER 1
 #define LP_CHAIN_KERNEL_TMA 2
 LP_API int lp_chain_set_kernel(int kernel);
+/* What block == 0 resolves to for a message of n elements over P ranks (elements; 0 on bad arguments), and the constants
+ * behind it: alpha s per block exchange and direction, beta s per byte and channel (gamma folded in), fitted to the
+ * chain kernel in its one-GPU emulation at p = 2, 4, 8 (profiles/r2_chain_cost_model.md): 2 alpha = 5.9 us whatever p --
+ * what Eq. 1 assumes and the copy-engine variant on one GPU does not deliver. */
+LP_API size_t lp_chain_auto_block(size_t n, int P, int channels, int tile);
+LP_API void lp_chain_fitted_constants(double *alpha, double *beta);
 LP_API int lp_chain_plan(int op, int P, int root, int rank, lp_chain_role *out);
 /* device bytes one endpoint takes for (channels, slots, tile): 2 x channels x slots x tile x 4 for the two rings, plus
  * counters; 0 for an invalid geometry.  Host only. */

@@ -121,6 +121,10 @@ def lib() -> ctypes.CDLL:
     L.lp_chain_connect_ptrs.argtypes = [vp, vp, vp]
     L.lp_chain_set_timeout.argtypes = [vp, ctypes.c_ulonglong]
     L.lp_chain_set_kernel.argtypes = [i32]
+    L.lp_chain_auto_block.argtypes = [sz, i32, i32, i32]
+    L.lp_chain_auto_block.restype = sz
+    L.lp_chain_fitted_constants.argtypes = [ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
+    L.lp_chain_fitted_constants.restype = None
     L.lp_chain_endpoint.argtypes = [vp]
     L.lp_chain_endpoint.restype = vp
     L.lp_chain_run.argtypes = [vp, i32, vp, sz, sz, i32, i32, vp]
@@ -337,6 +341,16 @@ def lp_dtype_size(dtype) -> int:
 # ---- the chain over real GPUs (one rank per GPU) and its one-GPU emulation ---------------------------------------
 CHAIN_HANDLE_BYTES = 64
 CHAIN_KERNEL_DEFAULT, CHAIN_KERNEL_REGISTER, CHAIN_KERNEL_TMA = 0, 1, 2
+
+
+def lp_chain_auto_block(n, P, channels=0, tile=0) -> int:
+    return int(lib().lp_chain_auto_block(n, P, channels, tile))
+
+
+def lp_chain_fitted_constants():
+    a, b = ctypes.c_double(0), ctypes.c_double(0)
+    lib().lp_chain_fitted_constants(ctypes.byref(a), ctypes.byref(b))
+    return a.value, b.value
 
 
 def lp_chain_set_kernel(kernel):

@@ -121,15 +121,25 @@ void fill_rank(LpChainRank &R, const EndpointLayout &l, float *buf, float *out, 
 
 // a1 for the chain: blocks of `block` elements rounded up to a multiple of 4 (every tile then starts on a 16-byte
 // boundary; results never depend on the block), cut into tiles of at most one ring slot.  block == 0, "the library
-// chooses": one slot for long messages; for short ones the power of two that still gives every channel about four
-// blocks (floor 4096 elements), so that the pipeline over the ranks fills after a small block instead of after a
-// whole slot -- the paper's reason for small blocks, PAPER.md:89 ((p - 1 + n/b) steps: the fill term is (p - 1) b).
-lp_partition chain_partition(size_t n, size_t block, int tile, int channels) {
-    if (block == 0) {
-        size_t b = 4096;
-        while (b < (size_t)tile && b * 4u * (size_t)channels < n) b *= 2;
-        block = b;
-    }
+// chooses": the block that minimises the paper's own cost model (Table 1: an allreduce of a
+// channel's share n_c of the message takes (p - 1 + n_c / b) (2 alpha + b (2 beta + gamma))), lp_optimal_block with the
+// constants fitted to this kernel (profiles/r2_chain_cost_model.md): 2 alpha = 5.9 us per block exchange, the same at
+// p = 2, 4, 8 as Eq. 1 assumes, and 2 beta + gamma = 48 ps per byte and channel -- rounded to a power of two between 4096
+// elements and the slot.  Small blocks fill the chain sooner ((p - 1) b), large ones pay fewer flag exchanges (n_c / b).
+constexpr double kChainFitAlpha = 2.95e-6;  // s per block exchange and direction (2 alpha = 5.9 us)
+constexpr double kChainFitBeta = 24e-12;    // s per byte and channel (2 beta + gamma = 48 ps/B, gamma folded in)
+
+size_t chain_auto_block(size_t n, int P, int tile, int channels) {
+    const double n_c = (double)n * 4.0 / (double)channels;
+    const double b_bytes = lp_optimal_block(LP_OP_ALLREDUCE, (double)(P > 1 ? P : 2), n_c > 1.0 ? n_c : 1.0, kChainFitAlpha,
+                                            kChainFitBeta, 0.0);
+    size_t b = 4096;
+    while (b < (size_t)tile && (double)b * 4.0 * 1.41421356 < b_bytes) b *= 2;  // nearest power of two (geometric)
+    return b;
+}
+
+lp_partition chain_partition(size_t n, size_t block, int tile, int channels, int P) {
+    if (block == 0) block = chain_auto_block(n, P, tile, channels);
     if (block < ~(size_t)3) block = (block + 3) & ~(size_t)3;
     return lp_make_partition(n, block, (uint32_t)tile);
 }
@@ -256,6 +266,18 @@ int lp_chain_connect_ptrs(lp_chain *ch, void *up_endpoint, void *down_endpoint) 
 
 void *lp_chain_endpoint(lp_chain *ch) { return ch ? ch->base : nullptr; }
 
+size_t lp_chain_auto_block(size_t n, int P, int channels, int tile) {
+    if (channels == 0) channels = LP_CHAIN_DEFAULT_CHANNELS;
+    if (tile == 0) tile = LP_CHAIN_DEFAULT_TILE;
+    if (P < 1 || P > LP_MAX_P || !valid_geometry(channels, 1, tile)) return 0;
+    return chain_auto_block(n, P, tile, channels);
+}
+
+void lp_chain_fitted_constants(double *alpha, double *beta) {
+    if (alpha) *alpha = kChainFitAlpha;
+    if (beta) *beta = kChainFitBeta;
+}
+
 int lp_chain_set_kernel(int kernel) {
     if (kernel != LP_CHAIN_KERNEL_DEFAULT && kernel != LP_CHAIN_KERNEL_REGISTER && kernel != LP_CHAIN_KERNEL_TMA)
         return LP_ERR_INVALID_ARG;
@@ -329,7 +351,7 @@ static int chain_run_rank(lp_chain *ch, int op, float *buf, float *out, const fl
     L.mu = mu;
     L.invP = 1.0f / (float)ch->P;  // one RN division on the host (U7)
     L.spin_limit = ch->spin_limit;
-    L.part = chain_partition(n, block, ch->tile, ch->C);
+    L.part = chain_partition(n, block, ch->tile, ch->C, ch->P);
     L.tile = (uint32_t)ch->tile;
     fill_rank(L.rank[0], layout_of(ch->C, ch->S, ch->tile), buf, out, w_in, op == LP_OP_BSP_SGD_MOM ? vel : nullptr, ch->base,
               ch->peer_up, ch->peer_down, role);
@@ -476,7 +498,7 @@ static int chain_emulate(int op, float *const *bufs, float *const *outs, int P, 
     L.mu = mu;
     L.invP = 1.0f / (float)P;
     L.spin_limit = 1ull << 23;  // all ranks start together here: a few seconds mean a bug
-    L.part = chain_partition(n, block, tile, channels);
+    L.part = chain_partition(n, block, tile, channels, P);
     L.tile = (uint32_t)tile;
     for (int r = 0; r < P; ++r) {
         char *b = (char *)base;

@@ -129,6 +129,36 @@ def test_chain_plan_argument_errors():
     assert L.lp_chain_endpoint_bytes(0, 8, 16384) == 0 and L.lp_chain_endpoint_bytes(4, 8, 1000) == 0
 
 
+def test_chain_auto_block_is_the_papers_optimum():
+    """block = 0 over the chain: the power of two nearest to the minimiser of Table 1's LP allreduce cost for one channel's
+    share of the message, with the constants fitted to the chain kernel."""
+    import math
+    alpha, beta = lp.lp_chain_fitted_constants()
+    assert 1e-6 < alpha < 1e-5 and 1e-12 < beta < 1e-10
+    tile = 262_144
+    for P in (2, 4, 8, 16):
+        last = 0
+        for mb in (1, 4, 16, 64, 256, 1024):
+            n = (mb << 20) // 4
+            for C in (8, 16, 40):
+                b = lp.lp_chain_auto_block(n, P, C, tile)
+                assert 4096 <= b <= tile and b & (b - 1) == 0
+                n_c = n * 4 / C
+                opt = lp.lp_optimal_block(lp.OP_ALLREDUCE, P, n_c, alpha, beta)        # bytes
+                # the minimiser is what Table 1's cost says it is: no other power of two in range is cheaper by > 1 %
+                cost = lambda bb: lp.lp_cost_model(lp.ALGO_LP, lp.OP_ALLREDUCE, P, n_c, bb * 4, alpha, beta)
+                best = min(cost(bb) for bb in (4096 << k for k in range(7)) if bb * 4 <= max(n_c, 4096 * 4))
+                if b * 4 <= n_c:
+                    assert cost(b) <= 1.06 * best, (P, mb, C, b, opt)
+                assert 0.7 <= (b * 4) / min(max(opt, 4096 * 4), tile * 4) <= 1.42 or b in (4096, tile), (P, mb, C, b, opt)
+            b16 = lp.lp_chain_auto_block(n, P, 16, tile)
+            assert b16 >= last                     # longer messages never get smaller blocks
+            last = b16
+    # more ranks: a longer fill, so never a larger block
+    assert lp.lp_chain_auto_block(1 << 26, 16, 16, tile) <= lp.lp_chain_auto_block(1 << 26, 2, 16, tile)
+    assert lp.lp_chain_auto_block(1 << 20, 0, 16, tile) == 0 and lp.lp_chain_auto_block(1 << 20, 4, 16, 1000) == 0
+
+
 def test_chain_create_needs_a_device():
     import torch
     if torch.cuda.is_available():
