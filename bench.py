@@ -733,7 +733,7 @@ def chain_rows(torch, lp, dev, msg_bytes=64 << 20):
     direction carried; hbm_GBps counts what the emulation really moves, (6P-4) n 4 bytes for an allreduce (P loads, P stores
     and 2(P-1) ring writes + reads), (3P-2) n 4 for a broadcast.  Eager launches, K back to back between two events."""
     n = msg_bytes // 4
-    out = {"msg_MB": msg_bytes / 2 ** 20, "tile_elems": 131_072, "slots": 8, "block": "0 = the cost model's choice",
+    out = {"msg_MB": msg_bytes / 2 ** 20, "tile_elems": 131_072, "slots": 4, "block": "0 = the cost model's choice",
            "what": "us per call, GB/s per emulated link direction, HBM GB/s of the emulation; NOT an NVLink measurement"}
     for P in (2, 4, 8):
         bufs = [torch.full((n,), 0.001 * (r + 1), device=dev) for r in range(P)]

@@ -333,7 +333,7 @@ LP_API int lp_be_allreduce_op(float *const *bufs, int P, size_t n, int reduce_op
 #define LP_CHAIN_MAX_CHANNELS 64
 #define LP_CHAIN_DEFAULT_CHANNELS 40
 #define LP_CHAIN_EMULATE_CHANNELS 16
-#define LP_CHAIN_DEFAULT_SLOTS 8
+#define LP_CHAIN_DEFAULT_SLOTS 4
 #define LP_CHAIN_DEFAULT_TILE 131072
 typedef struct lp_chain lp_chain;
 typedef struct lp_chain_role {
