@@ -374,22 +374,25 @@ def run_ours(args, c, rank, world, local):
     if rank == 0 and not args.no_detail:
         want = set(args.detail.split(","))
         detail = {}
-        if "configs1" in want:
-            detail["configs1"] = cfg1_more(torch, lp, dev, pristine, sets[0], P, n, block, peak)
+        def section(name, fn):
+            # a secondary measurement that fails must not take the headline line with it
+            if name not in want:
+                return
+            try:
+                detail[name] = fn()
+            except Exception as exc:  # noqa: BLE001
+                detail[name] = {"error": f"{type(exc).__name__}: {exc}"}
+                torch.cuda.synchronize()
+
+        section("configs1", lambda: cfg1_more(torch, lp, dev, pristine, sets[0], P, n, block, peak))
         del pristine, sets
         torch.cuda.empty_cache()
-        if "configs2" in want:
-            detail["configs2"] = cfg2_steps(torch, lp, dev, peak)
-        if "configs4" in want:
-            detail["configs4"] = cfg4_row(torch, lp, dev, peak)
-        if "sweep" in want:
-            detail["sweep"] = sweep_cfg3(torch, lp, dev, peak)
-        if "ceilings" in want:
-            detail["ceilings"] = ceilings(torch, lp, dev, peak)
-        if "dtypes" in want:
-            detail["dtypes"] = dtype_rows(torch, lp, dev)
-        if "chain" in want:
-            detail["chain"] = chain_rows(torch, lp, dev)
+        section("configs2", lambda: cfg2_steps(torch, lp, dev, peak))
+        section("configs4", lambda: cfg4_row(torch, lp, dev, peak))
+        section("sweep", lambda: sweep_cfg3(torch, lp, dev, peak))
+        section("ceilings", lambda: ceilings(torch, lp, dev, peak))
+        section("dtypes", lambda: dtype_rows(torch, lp, dev))
+        section("chain", lambda: chain_rows(torch, lp, dev))
 
     cpu = None
     if rank == 0 and not args.no_cpu:
