@@ -528,6 +528,35 @@ LP_API int lp_plan_get_info(const lp_plan *plan, struct lp_plan_info *out);
  * outputs may alias inputs (the in-place mix of an allreduce). */
 LP_API int lp_hbm_probe(float *const *bufs, int n_read, int n_write, size_t n, void *cuda_stream);
 
+/* ---- a reduce for callers that must not allocate device memory (csrc/lp_static.cu) ------------------------------ */
+/* lp_mst_reduce_static: the MST reduce of PAPER.md:93 (binomial tree on virtual ranks v = (r - root) mod P, whole-message
+ * levels d = 1, 2, 4, ...; root <- tree sum, the other buffers unchanged, U5) -- same arguments, same validation and
+ * bit-for-bit the same values as lp_mst_reduce -- for a caller that cannot let a library call cudaMalloc / cudaFree:
+ * a process whose framework pool allocator already owns all of the GPU's memory (a library cudaMalloc then fails with
+ * out-of-memory), a step loop that cannot take the device-wide synchronisation cudaFree implies when library scratch
+ * has to grow, or a thread running while another thread holds a global-mode stream capture (cudaMalloc is refused
+ * process-wide).  lp_mst_reduce keeps the non-root ranks' partial sums in library scratch it allocates on demand; this
+ * entry point keeps them in a fixed array of LP_STATIC_SCRATCH_BYTES that is part of the library's device image and
+ * calls no cudaMalloc, cudaFree or other allocating routine, ever.
+ *   Limit: a P-rank tree needs (P - 2) / 2 working copies of n floats (none for P <= 3), each rounded up to 256 bytes;
+ *     n above lp_mst_reduce_static_max_n(P) returns LP_ERR_UNSUPPORTED before anything is enqueued, with the numbers in
+ *     lp_static_last_error() (P = 4: 4,194,304 floats; P = 8: 1,398,080; P = 16: 599,168; P = 32: 279,616).
+ *   Cost: every GPU on which the library is loaded holds the array (16 MiB) until the process exits.
+ *   Sharing: all calls on one GPU use the same array.  Calls that can overlap on the device (two streams, no event
+ *     between them) race on it and produce wrong sums; calls on one stream are safe back to back.  The array keeps the
+ *     last call's partial sums; none of it needs clearing -- the tree writes every word of a copy before reading it.
+ *   Set-up: the first call made with a given device current looks the array's device address up
+ *     (cudaGetSymbolAddress; the runtime loads the module on that device at that point) and caches it.  Make that first
+ *     call on each device before any stream capture begins.  Independent of the library's one-device binding and of
+ *     lp_set_variant / lp_set_tuning; plain stream-ordered launches (one per tree level) on `cuda_stream`.
+ *   Errors: LP_ERR_INVALID_ARG as lp_mst_reduce; LP_ERR_UNSUPPORTED above the limit; LP_ERR_CUDA without a device or
+ *     when the symbol lookup / a launch fails.  lp_static_last_error(): the calling thread's text for the last failure. */
+#define LP_STATIC_SCRATCH_BYTES (16u << 20)
+LP_API int lp_mst_reduce_static(float *const *bufs, int P, size_t n, int root, void *cuda_stream);
+LP_API size_t lp_mst_reduce_static_max_n(int P);   /* largest n lp_mst_reduce_static takes at P ranks; 0 for a bad P; host only */
+LP_API size_t lp_static_scratch_bytes(void);       /* LP_STATIC_SCRATCH_BYTES as built; host only */
+LP_API const char *lp_static_last_error(void);     /* "" after a successful call; per thread */
+
 /* Minimum HBM bytes of one call (each input read once, each output written once):
  * broadcast P*n*4, reduce (P+1)*n*4, allreduce 2*P*n*4, bsp_sgd (2P+1)*n*4, bsp_sgd with momentum (2P+3)*n*4. */
 LP_API uint64_t lp_min_bytes(int op, int P, size_t n);

@@ -98,6 +98,11 @@ def lib() -> ctypes.CDLL:
         getattr(L, name).argtypes = [pp, i32, sz, i32, vp]
     for name in ("lp_mst_allreduce", "lp_be_allreduce"):
         getattr(L, name).argtypes = [pp, i32, sz, vp]
+    L.lp_mst_reduce_static.argtypes = [pp, i32, sz, i32, vp]
+    L.lp_mst_reduce_static_max_n.argtypes = [i32]
+    L.lp_mst_reduce_static_max_n.restype = sz
+    L.lp_static_scratch_bytes.restype = sz
+    L.lp_static_last_error.restype = ctypes.c_char_p
     L.lp_reduce_op.argtypes = [pp, i32, sz, sz, i32, i32, vp]
     L.lp_allreduce_op.argtypes = [pp, i32, sz, sz, i32, vp]
     for name in ("lp_mst_reduce_op", "lp_be_reduce_op"):
@@ -735,6 +740,26 @@ def lp_mst_reduce(bufs, root=0, stream=None):
 
 def lp_mst_allreduce(bufs, stream=None):
     _baseline("lp_mst_allreduce", bufs, None, stream)
+
+
+def lp_mst_reduce_static(bufs, root=0, stream=None):
+    """lp_mst_reduce for callers that must not allocate device memory (a framework pool owns all of HBM, a loop that
+    cannot take cudaFree's device-wide sync, a thread beside a global-mode stream capture): same tree, same values, the
+    non-root ranks' partial sums in a fixed 16 MiB array inside the library instead of cudaMalloc'ed scratch.  Raises
+    LpError (LP_ERR_UNSUPPORTED) when n exceeds lp_mst_reduce_static_max_n(P).  One call at a time per GPU: calls
+    that overlap on the device share the array and race.  First call on a device: before any stream capture."""
+    arr, n = _dev_ptrs(bufs)
+    rc = lib().lp_mst_reduce_static(arr, len(bufs), n, root, _stream_ptr(stream))
+    if rc != LP_OK:
+        raise LpError(rc, "lp_mst_reduce_static: " + lib().lp_static_last_error().decode())
+
+
+def lp_mst_reduce_static_max_n(P: int) -> int:
+    return int(lib().lp_mst_reduce_static_max_n(P))
+
+
+def lp_static_scratch_bytes() -> int:
+    return int(lib().lp_static_scratch_bytes())
 
 
 def lp_be_broadcast(bufs, root=0, stream=None):
