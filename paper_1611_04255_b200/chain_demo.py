@@ -8,7 +8,7 @@ neighbours' rings over NVLink, no NCCL on the data path), checks the bits agains
 ``((x0 + x1) + x2) + ...`` computed from an all-gather of the inputs -- runs the fused BSP-SGD step, and rank 0 prints one
 JSON line with the device-timed throughput (max over ranks).  This build's box has ONE GPU: there the script runs with
 N = 1 only (every collective is then the identity); the chain's device code is covered by ``lp_chain_emulate`` in
-tests/test_gpu_chain.py.  NOT part of bench.py: north_star's hot path has no inter-GPU collective.
+tests/test_gpu_3_chain.py.  NOT part of bench.py: north_star's hot path has no inter-GPU collective.
 """
 from __future__ import annotations
 

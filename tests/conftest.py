@@ -10,6 +10,7 @@ if ROOT not in sys.path:
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box)")
+    config.addinivalue_line("markers", "timing: wall-clock evidence (cost-model fits); never part of the gpu parity gate")
 
 
 @pytest.fixture(scope="session")

@@ -1037,62 +1037,18 @@ def test_host_entry_points(oracle):
 
 
 # ---------------------------------------------------------------------------------------------------
-# the fitted cost model against measurements, and block = 0
+# block = 0 (the cost model's optimum).  What the model predicts against the clock is a measurement, not a
+# property of the result: those checks live in tests/test_timing_cost_model.py (marker `timing`, outside the gpu gate).
 # ---------------------------------------------------------------------------------------------------
-def _time_allreduce(dev, pristine, block, reps=3):
-    ms = []
-    for it in range(reps + 1):
-        for d, p in zip(dev, pristine):
-            d.copy_(p)
-        torch.cuda.synchronize()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record()
-        lp.lp_allreduce(dev, block)
-        e1.record()
-        torch.cuda.synchronize()
-        if it:
-            ms.append(e0.elapsed_time(e1))
-    return float(np.median(ms)) * 1e-3
-
-
 @pytest.mark.parametrize("P", [2, 6, 16])
-def test_fitted_cost_model_and_auto_block(oracle, P):
-    # The copy-engine variant (the paper's own design) is the realisation Eq. 1 / Table 1 describes.
-    # (i) lp_cost_model with the constants committed in the library (lp_fitted_constants: profiles/r2_cost_model_fit.md)
-    # predicts the measured time of the configs[1]-sized allreduce (244 MB per rank) at four block sizes within 45 %
-    # (the fit's own error is 12-16 %, the constants' simple p-law adds up to 27 % more; for messages much shorter
-    # than (p-1) blocks the model's pipeline-fill term, which has no counterpart on one GPU, overestimates further);
-    # (ii) block = 0 -- the model's optimum -- is within 20 % of the best block of the scan, where the paper's 64 KB
-    # (16 K elements) is 100x slower; (iii) the result with block = 0 is the oracle's, bit for bit.
-    n = 61_000_000
+def test_auto_block_result_is_the_oracles(oracle, P):
+    n = 61_000_000 if P == 6 else 8_000_003
     src = inputs.rank_vectors([30, P], P, n, "normal", 1e-3)
-    pristine = up(src)
-    dev = [p.clone() for p in pristine]
-    lp.lp_set_variant(lp.VARIANT_COPY_ENGINE)
-    alpha, beta = lp.lp_fitted_constants(P)
-    times = {}
-    for block in (1 << 18, 1 << 20, 1 << 22, 1 << 23, 1 << 24):
-        times[block] = _time_allreduce(dev, pristine, block)
-    for block in (1 << 18, 1 << 20, 1 << 22, 1 << 23):
-        pred = lp.lp_cost_model(lp.ALGO_LP, lp.OP_ALLREDUCE, P, n * 4.0, block * 4.0, alpha, beta, 0.0)
-        if block >= 1 << 22:   # bandwidth-dominated blocks: a property of the GPU
-            assert abs(pred - times[block]) / times[block] < 0.45, (P, block, pred, times[block])
-        else:                  # latency-dominated blocks: alpha is the HOST's cost of submitting a stream operation
-            assert 0.4 < pred / times[block] < 2.5, (P, block, pred, times[block])   # (2.4 - 4.3 ms seen for the same call)
-    t_auto = _time_allreduce(dev, pristine, 0)
-    auto_block = lp.lp_auto_block(lp.OP_ALLREDUCE, P, n, lp.VARIANT_COPY_ENGINE)
-    assert (1 << 21) <= auto_block <= n
-    assert t_auto <= 1.2 * min(times.values()), (P, t_auto, times)
-    t_paper = _time_allreduce(dev, pristine, 16_384, reps=1)
-    assert t_paper > 20 * t_auto, (t_paper, t_auto)
-    for d, p in zip(dev, pristine):
-        d.copy_(p)
-    lp.lp_allreduce(dev, 0)
     want = oracle.chain_sum(src)
-    assert all(same(g, want) for g in down(dev))
-    # the persistent kernels are flat in the block size: block = 0 is as good as any
-    lp.lp_set_variant(lp.VARIANT_AUTO)
-    t0 = _time_allreduce(dev, pristine, 0)
-    t1 = _time_allreduce(dev, pristine, 16_384)
-    t2 = _time_allreduce(dev, pristine, 1 << 22)
-    assert max(t0, t1, t2) < 1.15 * min(t0, t1, t2), (t0, t1, t2)
+    for variant in (lp.VARIANT_COPY_ENGINE, lp.VARIANT_AUTO):
+        lp.lp_set_variant(variant)
+        auto_block = lp.lp_auto_block(lp.OP_ALLREDUCE, P, n, variant)
+        assert 1 <= auto_block <= max(n, lp.DEFAULT_BLOCK)
+        dev = up(src)
+        lp.lp_allreduce(dev, 0)
+        assert all(same(g, want) for g in down(dev)), (P, variant)

@@ -244,39 +244,6 @@ def test_chain_seeded_fuzz(oracle):
     assert checked > 40 and all(lp.lp_chain_emulate_error(P, **g) == 0 for P, g in geoms.items())
 
 
-def test_chain_cost_model_predicts_the_emulation():
-    """Sec. 3.2's model with the committed constants (lp_chain_fitted_constants; profiles/r2_chain_cost_model.md) against
-    the clock: a 64 MB allreduce over 4 emulated ranks at a latency-bound, a near-optimal and a fill-bound block, and
-    block = 0 may not be slower than the fixed 64 K-element block by more than measurement noise."""
-    if lp.lib().lp_chain_set_kernel(lp.CHAIN_KERNEL_TMA) != lp.LP_OK:
-        pytest.skip("no TMA kernel")
-    P, C, n = 4, 16, (64 << 20) // 4
-    alpha, beta = lp.lp_chain_fitted_constants()
-    bufs = lp.Ranks([torch.full((n,), 0.001 * (r + 1), device="cuda") for r in range(P)])
-
-    def clock(block, tile):
-        for _ in range(2):
-            lp.lp_chain_emulate(lp.OP_ALLREDUCE, bufs, block=block, channels=C, slots=8, tile=tile)
-        torch.cuda.synchronize()
-        best = 1e9
-        for _ in range(3):
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record()
-            for _ in range(4):
-                lp.lp_chain_emulate(lp.OP_ALLREDUCE, bufs, block=block, channels=C, slots=8, tile=tile)
-            e1.record()
-            torch.cuda.synchronize()
-            best = min(best, e0.elapsed_time(e1) / 4 * 1e-3)
-        return best
-
-    for b in (8192, 65_536, 262_144):
-        t = clock(b, b)
-        model = lp.lp_cost_model(lp.ALGO_LP, lp.OP_ALLREDUCE, P, n * 4 / C, b * 4, alpha, beta)
-        assert 0.6 < t / model < 1.6, (b, t, model)
-    assert clock(0, 131_072) < 1.15 * clock(65_536, 131_072)
-    assert lp.lp_chain_emulate_error(P, C, 8, 131_072) == 0
-
-
 def test_chain_two_streams_do_not_share_rings(oracle):
     """Emulated endpoints belong to (P, geometry, stream): two chains of the same shape running at the same time on two
     streams must not see each other's blocks."""
