@@ -4,17 +4,20 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 1] [--block B]
 
 A step is one LP allreduce (a1 partition, a2 schedule, a4 reduce stage, a3 broadcast stage = a5) of the
-workload -- by default BASELINE.json configs[1]: P=6 virtual ranks, n=61,000,000 fp32 per rank, N(0,1e-3),
-seed 1 -- through the C ABI (lp_allreduce) with the inputs already resident in HBM.  `value` = algbw =
+workload -- by default BASELINE.json configs[4], the largest single-GPU configuration: P=16 virtual ranks,
+n=138,000,000 fp32 per rank (8.83 GB), N(0,1e-3), seed 4, b=262,144 (--config 1: P=6, n=61,000,000, the
+AlexNet-sized vector) -- through the C ABI (lp_allreduce) with the inputs already resident in HBM.  `value` = algbw =
 n*4 bytes / t (nccl-tests convention) summed over the N replicas; `roofline.achieved` = minimum HBM bytes
 2*P*n*4 / t against the measured copy peak of MEASURED_PEAKS.json.  `e2e` = the same metric through
 lp_allreduce_host with pinned HOST buffers (H2D + kernel + D2H inside the timed region).  `cpu_baseline` /
 `--impl reference` time the CPU oracle as it stands on the box's host cores, on the FULL vectors of the workload.
-`detail` carries the other BASELINE.json configs, driver-measured in the same run: configs[3] from 64 MB up at
-P = 2, 3, 4, 5, 6, 8, 16 (LP vs MST vs BE, three collectives, with the HBM ceiling of the same read : write mix from a
-plain streaming kernel beside every cell), configs[4] (P=16, 138 M), configs[2] (fused BSP-SGD step, 100 iterations),
-the other ops / variants / block sizes of configs[1], the pure-stream HBM ceilings, the typed collectives (f16 / bf16 / f64 at
-the same bytes per rank as f32) and the multi-GPU chain's one-GPU emulation.  Prints ONE JSON line (rank 0).
+The other BASELINE.json configs are measured in the same run and printed FIRST, one compact JSON line per section
+(`{"detail": "<section>", ...}`): configs[3] from 64 MB up at P = 2, 3, 4, 5, 6, 8, 16 (`sweep`: LP vs MST vs BE, three
+collectives, with the HBM ceiling of the same read : write mix from a plain streaming kernel beside every cell), its
+4 KB .. 32 MB half (`sweep_small`: the crossover table of the paper's Fig. 3), configs[1] / configs[4] (all three ops,
+variants, block sizes), configs[2] (fused BSP-SGD step, 100 iterations), the pure-stream HBM ceilings, the typed
+collectives and the multi-GPU chain's one-GPU emulation.  The LAST line (rank 0) is the headline: a few KB, with a
+`summary` of scalars taken from the sections.
 """
 from __future__ import annotations
 
@@ -37,9 +40,14 @@ from paper_1611_04255_b200 import inputs  # noqa: E402
 METRIC = "lp_allreduce_algbw"
 UNIT = "GB/s (algbw = n*4 bytes per rank / time; roofline on min bytes 2*P*n*4)"
 FALLBACK_HBM_GBS = 6650.0  # B200_PROFILING.md fallback, used only if MEASURED_PEAKS.json is absent
-# roofline.traffic (dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel) cannot be measured inside
-# this program (it needs ncu's replays): the line carries null and names the committed capture of the same command
-TRAFFIC_PROFILE = "profiles/r2_ncu_lp_pipeline.md (ncu --set full of this command: read + write = 0.98 x algorithmic)"
+# roofline.traffic (dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch) cannot be measured
+# inside this program (it needs ncu's replays): the line carries the number of the committed `ncu --set full` capture of
+# the same command and names it.  config index -> (bytes per launch, source)
+TRAFFIC = {
+    1: (2_869_328_000, "profiles/r2_ncu_lp_pipeline.md (ncu --set full of `bench.py --config 1`: 0.98 x algorithmic)"),
+    4: (17_604_425_000, "profiles/r3_ncu_lp_pipeline_cfg4.md (ncu --set full of this command: read 8.832 GB + write "
+                        "8.772 GB = 0.997 x algorithmic)"),
+}
 
 
 def parse_args():
@@ -48,11 +56,11 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json configs (1 or 4 for allreduce)")
+    ap.add_argument("--config", type=int, default=4, help="index into BASELINE.json configs (4 = the largest, or 1)")
     ap.add_argument("--block", type=int, default=0, help="LP block in elements (0 = the config's)")
     ap.add_argument("--variant", default="auto", choices=["auto", "pipeline", "direct", "cluster", "copy_engine"])
     ap.add_argument("--no-detail", action="store_true", help="skip the secondary measurements")
-    ap.add_argument("--detail", default="configs1,configs2,configs4,sweep,ceilings,dtypes,chain",
+    ap.add_argument("--detail", default="configs1,configs2,configs4,sweep,sweep_small,ceilings,dtypes,chain",
                     help="comma list of detail sections to run")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
@@ -250,11 +258,21 @@ def oracle_baseline(c, cfg_idx, passes, single_thread_passes):
     return out, t
 
 
+def headline_config(cfg_idx, c, block):
+    """The `config` object of the headline line: the same keys and values in both arms."""
+    return {"workload": f"BASELINE.json configs[{cfg_idx}]: {c['name']}", "P": c["P"], "n": c["n"], "block": block}
+
+
+def compact(obj):
+    return json.dumps(obj, separators=(",", ":"))
+
+
 def run_reference(args, c, rank, world):
     """--impl reference: the CPU oracle, unmodified, on the host cores, on the whole workload.  Rank 0 only."""
     if rank != 0:
         return
     P, n = c["P"], c["n"]
+    block = args.block or c["block"]
     omp, cores, _ = time_oracle(P, n, c["dist"], c.get("sigma", 1.0), args.config, args.steps, warm=max(args.warmup, 1))
     t = float(np.median(omp))
     value = n * 4 / t / 1e9
@@ -265,7 +283,7 @@ def run_reference(args, c, rank, world):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": t * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": f"BASELINE.json configs[{args.config}]: {c['name']}", "P": P, "n": n},
+        "config": headline_config(args.config, c, block),
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -370,55 +388,88 @@ def run_ours(args, c, rank, world, local):
                "api": "lp_allreduce_host (pinned host buffers, chunked H2D/kernel/D2H pipeline)"}
         del pinned
 
-    detail = None
+    del pristine, sets
+    torch.cuda.empty_cache()
+
+    # secondary measurements: one compact JSON line per section, printed as it finishes, BEFORE the headline line
+    summary = {}
     if rank == 0 and not args.no_detail:
         want = set(args.detail.split(","))
-        detail = {}
+
         def section(name, fn):
             # a secondary measurement that fails must not take the headline line with it
             if name not in want:
                 return
             try:
-                detail[name] = fn()
+                out = fn()
+                summarise(name, out, summary)
             except Exception as exc:  # noqa: BLE001
-                detail[name] = {"error": f"{type(exc).__name__}: {exc}"}
+                out = {"error": f"{type(exc).__name__}: {exc}"}
+                summary[f"{name}_error"] = out["error"][:120]
                 torch.cuda.synchronize()
+            print(compact({"detail": name, **out}), flush=True)
 
-        section("configs1", lambda: cfg1_more(torch, lp, dev, pristine, sets[0], P, n, block, peak))
-        del pristine, sets
-        torch.cuda.empty_cache()
+        section("configs1", lambda: cfg1_more(torch, lp, dev, peak))
         section("configs2", lambda: cfg2_steps(torch, lp, dev, peak))
         section("configs4", lambda: cfg4_row(torch, lp, dev, peak))
         section("sweep", lambda: sweep_cfg3(torch, lp, dev, peak))
+        section("sweep_small", lambda: sweep_small(torch, lp, dev))
         section("ceilings", lambda: ceilings(torch, lp, dev, peak))
         section("dtypes", lambda: dtype_rows(torch, lp, dev))
         section("chain", lambda: chain_rows(torch, lp, dev))
 
     cpu = None
     if rank == 0 and not args.no_cpu:
-        cpu, _ = oracle_baseline(c, args.config, passes=20, single_thread_passes=3)
+        cpu, _ = oracle_baseline(c, args.config, passes=20 if P * n <= 1 << 29 else 12,
+                                 single_thread_passes=3 if P * n <= 1 << 29 else 1)
 
     if rank != 0:
         return
+    traffic, traffic_src = TRAFFIC.get(args.config, (None, "no committed ncu --set full capture of this config"))
     line = {
         "metric": METRIC, "value": algbw, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": f"BASELINE.json configs[{args.config}]: {c['name']}", "P": P, "n": n, "block": block,
-                   "variant": ran, "plan": plan, "parallelism": f"replicas x{world} (no collective)",
-                   "l2": f"inputs {P * n * 4 / 1e6:.0f} MB per set >> 126 MB L2, {n_sets} rotating sets"},
+        "config": headline_config(args.config, c, block),
+        "run": {"variant": ran, "grid": plan.get("grid"), "tile_elems": plan.get("tile_elems"),
+                "smem_bytes": plan.get("smem_bytes"), "parallelism": f"replicas x{world} (no collective)",
+                "l2": f"inputs {P * n * 4 / 1e6:.0f} MB per set >> 126 MB L2, {n_sets} rotating sets"},
         "roofline": {"bound": "hbm", "achieved": hbm, "peak": peak, "unit": "GB/s", "frac": hbm / peak,
-                     "traffic": None, "traffic_source": TRAFFIC_PROFILE, "peak_source": peak_src,
-                     "peak_note": "the measured peak is a 1 read : 1 write copy; a fraction above 1 is possible for this "
-                                  "kernel (pure write streams reach 7.4 TB/s here: detail.ceilings) and is not a ceiling "
-                                  "claim -- detail.configs1.allreduce.lp_over_ceiling compares with a plain kernel of "
-                                  "the same mix",
+                     "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
+                     "peak_note": "the peak is a 1 read : 1 write torch copy; pure read / write streams reach ~7.4 TB/s "
+                                  "here (detail ceilings), so a fraction slightly above 1 is not a ceiling claim",
                      "frac_of_nominal_8TBs": hbm / 8000.0,
                      "kernel": "lp_pipeline_kernel" if ran == "pipeline" else ran,
                      "algorithmic_bytes_per_launch": min_bytes},
-        "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "detail": detail,
+        "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "summary": summary,
     }
-    print(json.dumps(line), flush=True)
+    print(compact(line), flush=True)
+
+
+def summarise(name, out, summary):
+    """The few scalars of a detail section that the headline line carries (the section's own line has the rest)."""
+    if name == "configs1":
+        a = out["allreduce"]
+        summary["configs1_allreduce_us"] = a["lp_us_unchained"]
+        summary["configs1_frac_8TBs_unchained"] = a["lp_frac_8TBs_unchained"]
+    elif name == "configs4":
+        summary["configs4_frac_8TBs_unchained"] = {op: out[op]["lp_frac_8TBs_unchained"]
+                                                   for op in ("allreduce", "reduce", "broadcast")}
+    elif name == "configs2":
+        summary["configs2_sgd_step_us"] = out["lp_bsp_sgd_step"]["us_per_step"]
+        summary["configs2_sgd_step_frac_8TBs"] = out["lp_bsp_sgd_step"]["frac_8TBs"]
+    elif name == "sweep":
+        sm = out["summary"]
+        summary["sweep_ge64MB_cells"] = sm["cells"]
+        summary["sweep_min_frac_8TBs"] = sm["lp_min_frac_8TBs"]
+        summary["sweep_min_frac_8TBs_unchained"] = sm["lp_min_frac_8TBs_unchained"]
+        summary["sweep_cells_below_0.80_unchained"] = len(sm["lp_cells_below_0.80_of_8TBs_unchained"])
+        summary["sweep_min_lp_vs_mst"] = sm["lp_min_vs_mst"]
+        summary["sweep_min_lp_vs_be"] = sm["lp_min_vs_be"]
+    elif name == "sweep_small":
+        summary["small_cells"] = out["summary"]["cells"]
+        summary["small_cells_where_lp_is_not_fastest"] = out["summary"]["cells_where_lp_is_not_fastest"]
+        summary["small_crossover"] = out["summary"]["crossover"]
 
 
 # ---- detail: the rest of BASELINE.json's configs, driver-measured ---------------------------------------
@@ -555,13 +606,64 @@ def sweep_cfg3(torch, lp, dev, peak, ps=SWEEP_PS, exps=SWEEP_EXPS, block=65_536)
         "lp_cells_slower_than_mst_or_be": [f"{r['op']} P={r['P']} {int(r['msg_MB'])}MB" for r in lp_rows
                                            if r.get("lp_vs_mst", 9) < 1.0 or r.get("lp_vs_be", 9) < 1.0],
     }
-    return {"note": "us per call = CUDA-graph replay of K back-to-back calls / K, median of 3, buffer sets rotating through "
+    cols = ["P", "msg_MB", "op", "lp_us", "lp_us_unchained", "mst_us", "be_us", "ceiling_GBps", "lp_frac_8TBs",
+            "lp_frac_8TBs_unchained", "lp_over_ceiling", "lp_variant", "rotating_sets"]
+    rows = [[r.get(k) for k in cols] for r in rows]
+    return {"cols": cols,
+            "note": "us per call = CUDA-graph replay of K back-to-back calls / K, median of 3, buffer sets rotating through "
                     ">= 1 GB (8 x L2), inputs restored outside the event pair; GB/s on the op's minimum HBM bytes for every "
                     "algorithm so rows compare; ceiling = lp_hbm_probe (plain streaming kernel, same read:write mix, same "
                     "buffers); block 65,536.  Consecutive calls of a graph work on different buffer sets wherever "
                     "rotating_sets > 1, so a call may start while its predecessor drains (LP_TUNE_CHAIN, also applied to "
                     "MST / BE); *_unchained = the same with every call waiting for its predecessor first (round 1's method)",
             "summary": summary, "rows": rows}
+
+
+def sweep_small(torch, lp, dev, ps=(2, 4, 8, 16), exps=tuple(range(10, 24)), block=65_536):
+    """The 4 KB .. 32 MB half of BASELINE.json configs[3] (Fig. 3; MST's smaller latency term
+    should win on short messages): LP (variant auto) vs MST vs BE, three collectives, device time per call from a CUDA
+    graph of back-to-back calls on rotating buffer sets.  Messages this short live in the 126 MB L2 -- as they would
+    in a training step that has just produced them -- so these cells are launch / latency numbers, not HBM ones."""
+    n_max = 2 << max(exps)   # arena per rank: two buffer sets of the longest message
+    pristine_all = [torch.from_numpy(inputs.uniform(3, r, n_max)).to(dev) for r in range(max(ps))]
+    cols = ["P", "msg_KB", "op", "lp_us", "mst_us", "be_us", "lp_variant"]
+    rows, slower = [], []
+    crossover = {}
+    for P in ps:
+        pristine = pristine_all[:P]
+        work = [torch.empty_like(p_) for p_ in pristine]
+        for e in exps:
+            n = 1 << e
+            n_sets = int(max(2, min(n_max // n, 16)))
+            sets = [lp.Ranks([w[s_ * n:(s_ + 1) * n] for w in work]) for s_ in range(n_sets)]
+
+            def restore(n_sets=n_sets, n=n):
+                for w, p_ in zip(work, pristine):
+                    w[:n_sets * n].copy_(p_[:n_sets * n])
+
+            for op in ("broadcast", "reduce", "allreduce"):
+                op_id = {"broadcast": lp.OP_BROADCAST, "reduce": lp.OP_REDUCE, "allreduce": lp.OP_ALLREDUCE}[op]
+                mb = lp.lp_min_bytes(op_id, P, n)
+                t = {}
+                for algo in ("lp", "mst", "be"):
+                    us, _ = graph_time(torch, lambda s_, a=algo: lp_call(lp, a, op, sets[s_], block), n_sets, restore, mb,
+                                       reps=2, target_ms=1.0, k_max=200)
+                    t[algo] = round(us, 2)
+                variant = ["pipeline", "direct", "cluster", "copy_engine"][lp.lp_plan_query(op_id, P, n, block)["variant"]]
+                rows.append([P, n * 4 // 1024, op, t["lp"], t["mst"], t["be"], variant])
+                best_other = min(t["mst"], t["be"])
+                if t["lp"] > 1.03 * best_other:   # 3 %: the timing's own repeatability
+                    slower.append(f"{op} P={P} {n * 4 // 1024}KB: lp {t['lp']} us vs {best_other} us")
+                    crossover[f"{op}_P{P}"] = n * 4 // 1024
+        del work, sets
+        torch.cuda.empty_cache()
+    return {"cols": cols, "rows": rows,
+            "note": "us per call, CUDA-graph replay of K back-to-back calls / K over >= 2 rotating buffer sets (L2-resident), "
+                    "median of 2; LP = LP_VARIANT_AUTO with block 65,536; a cell counts as 'LP not fastest' when LP is more "
+                    "than 3 % slower than the better of MST and BE",
+            "summary": {"cells": len(rows), "cells_where_lp_is_not_fastest": len(slower), "which": slower[:24],
+                        "crossover": ("none: LP is the fastest (within 3 %) in every cell from 4 KB to 32 MB" if not slower else
+                                      {k: f"MST/BE faster up to {v} KB" for k, v in crossover.items()})}}
 
 
 def cfg4_row(torch, lp, dev, peak):
@@ -629,9 +731,13 @@ def cfg2_steps(torch, lp, dev, peak):
     return out
 
 
-def cfg1_more(torch, lp, dev, pristine, work, P, n, block, peak):
-    """configs[1] beyond the headline: reduce / broadcast, every LP variant, the block sweep (16K = the paper's 64 KB),
-    MST.  Same graph timing; one working set (1.46 GB >> L2)."""
+def cfg1_more(torch, lp, dev, peak):
+    """BASELINE.json configs[1] (P=6, n=61,000,000, N(0,1e-3) seed 1): the three collectives, every LP variant, the block
+    sweep (16K = the paper's 64 KB), MST.  Same graph timing; one working set (1.46 GB >> L2)."""
+    c = inputs.CONFIGS[1]
+    P, n, block = c["P"], c["n"], c["block"]
+    pristine = [torch.from_numpy(h).to(dev) for h in inputs.rank_vectors(1, P, n, c["dist"], c["sigma"])]
+    work = [torch.empty_like(p_) for p_ in pristine]
     sets = [lp.Ranks(work)]
 
     def restore():
@@ -669,6 +775,8 @@ def cfg1_more(torch, lp, dev, pristine, work, P, n, block, peak):
         us, _ = graph_time(torch, lambda s, b=b: lp.lp_allreduce(sets[s], b), 1, restore, mb)
         sweep[str(b)] = {"us": round(us, 2), "hbm_GBps_min_bytes": round(mb / us / 1e3, 1)}
     out["allreduce_block_sweep"] = sweep
+    del pristine, work, sets
+    torch.cuda.empty_cache()
     return out
 
 

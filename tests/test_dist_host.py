@@ -145,7 +145,7 @@ def test_reference_arm_under_torchrun_prints_once():
     port = _free_port()
     cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr",
            "127.0.0.1", "--master-port", str(port), os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus",
-           "2", "--steps", "1", "--warmup", "1"]
+           "2", "--steps", "1", "--warmup", "1", "--config", "1"]
     env = dict(os.environ, OMP_NUM_THREADS="4")
     out = subprocess.run(cmd, capture_output=True, text=True, timeout=600, env=env, cwd=ROOT)
     assert out.returncode == 0, out.stderr[-2000:]
@@ -154,12 +154,45 @@ def test_reference_arm_under_torchrun_prints_once():
     line = lines[0]
     assert line["impl"] == "reference" and line["n_gpus"] == 2 and line["value"] > 0
     assert line["cpu_baseline"]["kind"] == "oracle" and line["e2e"]["h2d_bytes_per_step"] == 0
+    # the last stdout line is the headline, and its config has exactly the keys of our arm's
+    assert json.loads(out.stdout.strip().splitlines()[-1]) == line
+    assert sorted(line["config"]) == ["P", "block", "n", "workload"] and line["config"]["block"] == 65_536
 
 
-def test_default_workload_is_baseline_config1():
+def test_default_workload_is_the_largest_single_gpu_config():
     sys.path.insert(0, ROOT)
     import bench
+    old = sys.argv
+    sys.argv = ["bench.py"]
+    try:
+        args = bench.parse_args()
+    finally:
+        sys.argv = old
+    assert args.config == 4
+    c = bench.workload(args.config)
+    assert (c["P"], c["n"], c["block"]) == (16, 138_000_000, 262_144)
     c = bench.workload(1)
     assert (c["P"], c["n"]) == (6, 61_000_000)
+    assert bench.headline_config(4, bench.workload(4), 262_144) == {
+        "workload": "BASELINE.json configs[4]: cfg4_P16_vgg16_138M", "P": 16, "n": 138_000_000, "block": 262_144}
+
+
+def test_headline_line_stays_small():
+    """Round 2's single 50 KB line was lost by the driver: the headline must stay a few KB whatever the sections return."""
+    sys.path.insert(0, ROOT)
+    import bench
+    summary = {}
+    row = {"lp_us_unchained": 427.1, "lp_frac_8TBs_unchained": 0.8531}
+    bench.summarise("configs1", {"allreduce": row}, summary)
+    bench.summarise("configs4", {op: row for op in ("allreduce", "reduce", "broadcast")}, summary)
+    bench.summarise("configs2", {"lp_bsp_sgd_step": {"us_per_step": 71.5, "frac_8TBs": 0.83}}, summary)
+    bench.summarise("sweep", {"summary": {"cells": 84, "lp_min_frac_8TBs": 0.81, "lp_min_frac_8TBs_unchained": 0.81,
+                                          "lp_cells_below_0.80_of_8TBs_unchained": ["x"] * 84, "lp_min_vs_mst": 1.0,
+                                          "lp_min_vs_be": 1.0}}, summary)
+    bench.summarise("sweep_small", {"summary": {"cells": 168, "cells_where_lp_is_not_fastest": 3,
+                                                "crossover": {f"allreduce_P{p}": "MST/BE faster up to 64 KB" for p in (2, 4, 8, 16)}}},
+                    summary)
+    assert len(summary) <= 16
+    assert len(bench.compact({"summary": summary})) < 1500
     with pytest.raises(SystemExit):
         bench.workload(3)   # the sweep config is not a single bench workload
