@@ -46,9 +46,10 @@
  *     static schedule (LP_TUNE_SCHED 1: same results, a few per cent slower).  MST / BE reduce scratch is per stream
  *     as well (for captured launches: per capturing stream, so two graphs that both hold an MST / BE reduce captured
  *     on the same stream must not be replayed at the same time).
- *   - Stream order: results are those of calls executed one after the other in stream order.  Internally a call may
- *     START before its predecessors on the stream have finished when it touches none of their buffers (LP_TUNE_CHAIN);
- *     it never COMPLETES before them, so whatever follows in the stream (or waits on an event) sees all of them done.
+ *   - Stream order: results are those of calls executed one after the other in stream order, whatever else the caller
+ *     puts on the stream between them.  With LP_TUNE_CHAIN = 1 (opt-in) a call may START before the library calls ahead
+ *     of it on the stream have finished when it touches none of their buffers; it never COMPLETES before them.  That
+ *     mode cannot see other kernels: see LP_TUNE_CHAIN and lp_stream_fence.
  *     lp_set_variant / lp_set_tuning change process-wide DEFAULTS, read once at the start of each call; a caller that
  *     needs its own settings (a confined comm-stream collective beside unconfined ones) uses an lp_plan.
  *     The last-error text of lp_status_string is per thread.
@@ -148,13 +149,22 @@ extern "C" {
                                    the predecessor kernel (programmatic dependent launch): the start of a call overlaps the
                                    drain of the call before it even when the two touch the same buffers; 2 = off */
 #define LP_TUNE_CLUSTER_TILE 13 /* cluster variant: tile elements, 1024 / 2048 (default) / 4096 */
-#define LP_TUNE_CHAIN 14        /* 0/1: a call whose buffers overlap none of the calls still in flight ahead of it on its stream
-                                   does not wait for them before it starts (it waits before it ENDS, so completion order
-                                   on the stream is kept): back-to-back collectives on different buffers -- the layers of
-                                   Alg. 1, rotating buffer sets -- run into each other without a bubble; 2 = off, every
-                                   call waits for its predecessor first.  0 (default) leaves one case to the library: a
-                                   long reduce over 3 or more ranks in the direct variant waits first and prefetches (1-2 %
-                                   faster than sharing the SMs with its predecessor's tail); 1 chains that too */
+#define LP_TUNE_CHAIN 14        /* stream chaining: a launch whose buffers overlap none of the launches still in flight ahead
+                                   of it on its stream does not wait for them before it starts (it waits before it ENDS,
+                                   so completion order on the stream is kept).
+                                   0 (default): only between the launches of ONE API call (MST / BE tree levels, the three
+                                     launches of an Alg. 2 step) -- the library knows nothing else went into the stream
+                                     between them.  Every API call's first launch waits for whatever precedes it.
+                                   1: across API calls too (back-to-back collectives on different buffers -- the layers of
+                                     Alg. 1, rotating buffer sets -- run into each other without a bubble, 0.5-1 us per
+                                     call).  CONTRACT: the library tracks only its own launches.  If the caller enqueues
+                                     other work on the stream that writes a later call's buffers (a backward GEMM producing
+                                     the gradient), it must call lp_stream_fence(stream) after that work and before the
+                                     library call, or the call may start reading while that work is still running
+                                     (kernels that trigger programmatic completion early, as cuBLAS / CUTLASS ones do).
+                                   2: off, every launch waits first.
+                                   3: as 1, and long direct-variant reduces over >= 3 ranks chain as well (by default they
+                                     wait first and prefetch, 1-2 % faster). */
 #define LP_TUNE_DIRECT_OCC 15   /* direct variant: at most this many CTAs resident per SM (1..8; 0 = the library's choice by
                                    collective: write-heavy launches run best with few stores in flight) */
 #define LP_TUNE_COUNT 16
@@ -321,6 +331,9 @@ LP_API int lp_be_allreduce_op(float *const *bufs, int P, size_t n, int reduce_op
  *       the constants fitted to this kernel, lp_chain_fitted_constants) -- small blocks fill the chain sooner, large
  *       ones pay fewer flag exchanges.
  *   lp_chain_error(ch, &e)   synchronises; e != 0: a wait gave up (a neighbour never arrived) and the result is void.
+ *       The error is sticky and the endpoint is dead: its ring counters no longer match the sequence numbers the ranks
+ *       keep, so every later collective on it returns at once without touching a buffer (the kernels check the word on
+ *       entry).  Destroy and re-create the endpoint on ALL ranks.
  * lp_chain_plan is the host-only part: what `rank` does in (op, P, root) -- its ring neighbours and which of the steps
  * load / receive / store / send up / send down its forward and return CTAs take.  No device needed.
  * This build's box has ONE GPU: kernels that wait for each other cannot be run there as separate launches, so what
@@ -397,6 +410,15 @@ LP_API int lp_chain_bsp_sgd_momentum_step(lp_chain *ch, float *grad, float *weig
 LP_API int lp_chain_bsp_sgd_alg2_step(lp_chain *ch, float *grad, float *weight, float *velocity, size_t n, size_t block,
                                       int root, float lr, float mu, void *cuda_stream);
 LP_API int lp_chain_error(lp_chain *ch, int *error_out);
+/* Tear-down.  lp_chain_destroy synchronises only THIS rank's device before it unmaps its neighbours and frees its endpoint;
+ * a host barrier alone does not wait for the neighbours' kernels, and a kernel finishes without waiting for its last
+ * credits, so a neighbour's kernel may still be about to store a credit or a block into this endpoint.  Across ranks:
+ *   1. every rank synchronises the streams it ran chain collectives on (cudaDeviceSynchronize), then a barrier;
+ *   2. every rank calls lp_chain_disconnect (closes its mappings of the neighbours' endpoints), then a barrier;
+ *   3. every rank calls lp_chain_destroy (frees its own, now unmapped, endpoint).
+ * ChainGroup.destroy() (chain.py) does exactly this.  lp_chain_disconnect synchronises the device itself; a disconnected
+ * chain refuses lp_chain_run (LP_ERR_INVALID_ARG) and may be connected again. */
+LP_API int lp_chain_disconnect(lp_chain *ch);
 LP_API int lp_chain_destroy(lp_chain *ch);
 LP_API int lp_chain_emulate(int op, float *const *bufs, int P, size_t n, size_t block, int root, int reduce_op, int channels,
                             int slots, int tile, void *cuda_stream);
@@ -560,6 +582,11 @@ LP_API const char *lp_static_last_error(void);     /* "" after a successful call
 /* Minimum HBM bytes of one call (each input read once, each output written once):
  * broadcast P*n*4, reduce (P+1)*n*4, allreduce 2*P*n*4, bsp_sgd (2P+1)*n*4, bsp_sgd with momentum (2P+3)*n*4. */
 LP_API uint64_t lp_min_bytes(int op, int P, size_t n);
+
+/* lp_stream_fence: tells the library that work it does not track went into `cuda_stream` (LP_TUNE_CHAIN = 1 / 3 only
+ * need this): the next library launch on that stream waits for everything ahead of it before it starts.  Host-side
+ * bookkeeping only, nothing is enqueued.  Always LP_OK. */
+LP_API int lp_stream_fence(void *cuda_stream);
 
 /* ---- control ------------------------------------------------------------------ */
 LP_API int lp_set_variant(int variant);             /* LP_VARIANT_*; process-wide default of the LP calls (not of plans) */

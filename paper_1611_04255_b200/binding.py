@@ -98,6 +98,7 @@ def lib() -> ctypes.CDLL:
         getattr(L, name).argtypes = [pp, i32, sz, i32, vp]
     for name in ("lp_mst_allreduce", "lp_be_allreduce"):
         getattr(L, name).argtypes = [pp, i32, sz, vp]
+    L.lp_stream_fence.argtypes = [vp]
     L.lp_mst_reduce_static.argtypes = [pp, i32, sz, i32, vp]
     L.lp_mst_reduce_static_max_n.argtypes = [i32]
     L.lp_mst_reduce_static_max_n.restype = sz
@@ -143,6 +144,7 @@ def lib() -> ctypes.CDLL:
     L.lp_chain_emulate_bsp_sgd_alg2_step.argtypes = [pp, pp, vp, i32, sz, sz, i32, f32, f32, i32, i32, i32, vp]
     L.lp_chain_error.argtypes = [vp, ctypes.POINTER(i32)]
     L.lp_chain_destroy.argtypes = [vp]
+    L.lp_chain_disconnect.argtypes = [vp]
     L.lp_chain_emulate.argtypes = [i32, pp, i32, sz, sz, i32, i32, i32, i32, i32, vp]
     L.lp_chain_emulate_channels.argtypes = [i32, i32]
     L.lp_chain_emulate_error.argtypes = [i32, i32, i32, i32, ctypes.POINTER(i32)]
@@ -192,6 +194,11 @@ def lp_cost_model(algo, op, p, n_bytes, b_bytes, alpha, beta, gamma=0.0) -> floa
 
 def lp_optimal_block(op, p, n_bytes, alpha, beta, gamma=0.0) -> float:
     return float(lib().lp_optimal_block(op, p, n_bytes, alpha, beta, gamma))
+
+
+def lp_stream_fence(stream=None):
+    """LP_TUNE_CHAIN = 1 / 3 only: other work went into `stream`; the next library launch there waits for it first."""
+    _check(lib().lp_stream_fence(_stream_ptr(stream)), "lp_stream_fence")
 
 
 def status_string(status: int) -> str:
@@ -497,6 +504,11 @@ class Chain:
         e = ctypes.c_int(0)
         _check(lib().lp_chain_error(self.h, ctypes.byref(e)), "lp_chain_error")
         return int(e.value)
+
+    def disconnect(self):
+        """Unmap the neighbours' endpoints (step 2 of the tear-down in lp_collectives.h); synchronises the device."""
+        if self.h:
+            _check(lib().lp_chain_disconnect(self.h), "lp_chain_disconnect")
 
     def destroy(self):
         if self.h:

@@ -66,6 +66,16 @@ class ChainGroup:
         return self.endpoint.error()
 
     def destroy(self):
+        """Tear-down in the order lp_collectives.h prescribes.  A host barrier alone is not enough: it does not wait for the
+        neighbours' KERNELS, and a chain kernel ends without waiting for its last credits -- a neighbour's kernel may
+        still be about to store into this rank's endpoint when this rank passes the barrier."""
+        import torch
         import torch.distributed as dist
-        dist.barrier(self.group)  # no neighbour is still writing into this endpoint
-        self.endpoint.destroy()
+        if torch.cuda.is_available():
+            torch.cuda.synchronize()      # 1. my kernels have drained: I push nothing into anybody any more ...
+        dist.barrier(self.group)          #    ... and neither does anyone else
+        disconnect = getattr(self.endpoint, "disconnect", None)
+        if disconnect is not None:
+            disconnect()                  # 2. my mappings of the neighbours' endpoints are closed ...
+        dist.barrier(self.group)          #    ... and so is every mapping of mine
+        self.endpoint.destroy()           # 3. free my (unmapped, idle) endpoint

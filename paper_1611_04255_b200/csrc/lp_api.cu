@@ -98,7 +98,16 @@ struct ChainEntry {
 struct Chain {
     std::vector<ChainEntry> e;  // launches that may still be running when the next launch of the stream starts
     bool unknown = true;        // an untracked launch is among them
+    uint64_t call_id = 0;       // the API call (begin_call) that enqueued the last tracked launch
 };
+// Which API call the calling thread is in, and whether its settings allow a launch to chain onto launches of EARLIER
+// calls (LP_TUNE_CHAIN 1 / 3).  The table above knows only this library's launches: between two API calls the caller may
+// have put anything on the stream (a GEMM that writes the next call's input and triggers programmatic completion
+// early), so by default a launch may only skip its leading wait when the launch right ahead of it on the stream was
+// enqueued by the SAME API call (tree levels of MST / BE, the launches of one Alg. 2 step, the slices of one list).
+std::atomic<uint64_t> g_call_seq{0};
+thread_local uint64_t t_call_id = 0;
+thread_local bool t_chain_across_calls = false;
 std::unordered_map<cudaStream_t, Chain> g_chains;
 constexpr size_t kChainMax = 8;
 
@@ -168,6 +177,8 @@ int begin_call(const LpCallCfg *cfg_in, LpCallCfg &cfg, int &sms) {
         cfg.tuning = g_tuning;
     }
     sms = sm_count_locked();
+    t_call_id = g_call_seq.fetch_add(1, std::memory_order_relaxed) + 1;
+    t_chain_across_calls = cfg.tuning.v[LP_TUNE_CHAIN] == 1 || cfg.tuning.v[LP_TUNE_CHAIN] == 3;
     return sms <= 0 ? no_device(sms) : LP_OK;
 }
 
@@ -229,8 +240,10 @@ int validate_tuning(int key, int value) {
             break;
         case LP_TUNE_L2_HINT:
         case LP_TUNE_PREFETCH:
-        case LP_TUNE_CHAIN:
             if (value > 2) return LP_ERR_INVALID_ARG;
+            break;
+        case LP_TUNE_CHAIN:
+            if (value > 3) return LP_ERR_INVALID_ARG;
             break;
         case LP_TUNE_STORE_WAIT:
         case LP_TUNE_SCHED:
@@ -722,7 +735,8 @@ bool lp_chain_admit(cudaStream_t stream, const LpRange *ranges, int n, bool pdl,
     }
     std::lock_guard<std::mutex> lock(g_mu);
     Chain &c = g_chains[stream];
-    bool late = allowed && pdl && !c.unknown && c.e.size() < kChainMax;
+    bool late = allowed && pdl && !c.unknown && c.e.size() < kChainMax && (t_chain_across_calls || c.call_id == t_call_id);
+    c.call_id = t_call_id;
     for (size_t k = 0; late && k < c.e.size(); ++k) {
         const ChainEntry &o = c.e[k];
         if (ent.hi <= o.lo || o.hi <= ent.lo) continue;  // bounding boxes apart
@@ -1315,6 +1329,11 @@ const char *lp_status_string(int status) {
         case LP_ERR_CUDA: return t_err[0] ? t_err : "LP_ERR_CUDA";
         default: return "unknown status";
     }
+}
+
+int lp_stream_fence(void *cuda_stream) {
+    lp_chain_reset((cudaStream_t)cuda_stream);
+    return LP_OK;
 }
 
 int lp_version(void) { return 300; }  // 0.3.0

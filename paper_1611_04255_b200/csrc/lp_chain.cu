@@ -247,12 +247,24 @@ __device__ void chain_return(const LpChainRank &A, const LpChainLaunch &L, int c
 }
 
 // grid = n_local x 2 C: CTA b plays local rank b / (2 C); of a rank's 2 C CTAs the first C are forward, the rest return.
+// Fail fast: after a wait gave up (the endpoint's sticky error word) the counters of the rings no longer match the
+// sequence numbers the host keeps, so a later collective could be satisfied by stale flags and deliver old slots.  Every
+// CTA checks the word on entry -- one thread reads it, all take the same decision -- and does nothing once it is set; the
+// endpoint has to be destroyed and created again on all ranks.
+__device__ __forceinline__ bool chain_endpoint_dead(const int *error) {
+    __shared__ int s_dead;
+    if (threadIdx.x == 0) s_dead = *reinterpret_cast<const volatile int *>(error);
+    __syncthreads();
+    return s_dead != 0;
+}
+
 __global__ void __launch_bounds__(kChainThreads, 1) lp_chain_kernel(const __grid_constant__ LpChainLaunch L) {
     __shared__ int s_ok;
     const int per_rank = 2 * L.C;
     const int lr = (int)blockIdx.x / per_rank;
     const int j = (int)blockIdx.x - lr * per_rank;
     const LpChainRank &A = L.rank[lr];
+    if (chain_endpoint_dead(A.error)) return;
     if (j < L.C) {
         if (A.f_active) chain_forward(A, L, j, &s_ok);
     } else {
@@ -490,7 +502,24 @@ __device__ void chain_stream_tma(const ChainStream &X, const LpChainRank &A, con
                     if (push[1]) lp_stg_stream(push[1] + s0 + 4 * j, acc[k]);
                 }
             }
-            if (ctid == 0 && (sl & 3u)) {  // the message's last <= 3 elements: by hand, straight from and to global memory
+            if (ctid == 0 && (sl & 3u) && L.code >= 6) {
+                // f64 (codes 6 / 7): the last two words are ONE element (lengths and offsets are even) -- lp_combine1 knows
+                // only the one-word types, so the pair is folded as a double, like lp_word_combine_store does
+                for (uint32_t e = sl & ~3u; e + 1 < sl; e += 2) {
+                    float lo = X.src_ring ? ld_ring1(in_slot + s0 + e) : X.src_local[off + s0 + e];
+                    float hi = X.src_ring ? ld_ring1(in_slot + s0 + e + 1) : X.src_local[off + s0 + e + 1];
+                    if (X.src_ring && X.src_local) {
+                        const double r = lp_combine_f64(lp_words_f64(lo, hi),
+                                                        lp_words_f64(X.src_local[off + s0 + e], X.src_local[off + s0 + e + 1]),
+                                                        L.code == 7);
+                        lo = __int_as_float(__double2loint(r));
+                        hi = __int_as_float(__double2hiint(r));
+                    }
+                    if (push[0]) push[0][s0 + e] = lo, push[0][s0 + e + 1] = hi;
+                    if (X.dst_local) X.dst_local[off + s0 + e] = lo, X.dst_local[off + s0 + e + 1] = hi;
+                    if (push[1]) push[1][s0 + e] = lo, push[1][s0 + e + 1] = hi;
+                }
+            } else if (ctid == 0 && (sl & 3u)) {  // the message's last <= 3 elements: by hand, straight from and to global memory
                 for (uint32_t e = sl & ~3u; e < sl; ++e) {
                     float v = X.src_ring ? ld_ring1(in_slot + s0 + e) : X.src_local[off + s0 + e];
                     if (X.src_ring && X.src_local) v = lp_combine1(v, X.src_local[off + s0 + e], L.code);
@@ -535,6 +564,7 @@ __global__ void __launch_bounds__(kTmaThreads, 1) lp_chain_tma_kernel(const __gr
     const int lr = (int)blockIdx.x / per_rank;
     const int j = (int)blockIdx.x - lr * per_rank;
     const LpChainRank &A = L.rank[lr];
+    if (chain_endpoint_dead(A.error)) return;
     ChainStream X;
     memset(&X, 0, sizeof(X));
     int c;

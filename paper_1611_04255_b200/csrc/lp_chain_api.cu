@@ -158,6 +158,7 @@ int chain_fail(cudaError_t e) {
 // binding.  Per stream: launches of one stream are ordered, launches of two streams may overlap and must not share rings.
 struct EmulEndpoints {
     int P, C, S, tile;
+    int device;  // the device the endpoints were allocated on: another device (or a stream handle reused there) gets its own
     cudaStream_t stream;
     void *base;
 };
@@ -291,13 +292,26 @@ int lp_chain_set_timeout(lp_chain *ch, unsigned long long polls) {
     return LP_OK;
 }
 
-int lp_chain_destroy(lp_chain *ch) {
+// Unmaps the neighbours' endpoints (after this rank's kernels have drained).  Tear-down across ranks is three steps with a
+// host barrier between them: every rank synchronises its device (no kernel anywhere can still push data or a credit into
+// a neighbour), every rank disconnects (no mapping of an exported endpoint is left), every rank destroys.
+int lp_chain_disconnect(lp_chain *ch) {
     if (ch == nullptr) return LP_ERR_INVALID_ARG;
     cudaDeviceSynchronize();
     if (ch->connected) {
         if (ch->up_ipc) cudaIpcCloseMemHandle(ch->peer_up);
         if (ch->down_ipc) cudaIpcCloseMemHandle(ch->peer_down);
+        ch->up_ipc = ch->down_ipc = false;
+        ch->peer_up = ch->peer_down = nullptr;
+        ch->connected = false;
     }
+    cudaGetLastError();
+    return LP_OK;
+}
+
+int lp_chain_destroy(lp_chain *ch) {
+    if (ch == nullptr) return LP_ERR_INVALID_ARG;
+    lp_chain_disconnect(ch);
     cudaFree(ch->base);
     cudaGetLastError();
     delete ch;
@@ -470,8 +484,11 @@ static int chain_emulate(int op, float *const *bufs, float *const *outs, int P, 
     void *base = nullptr;
     {
         std::lock_guard<std::mutex> lock(g_emul_mu);
+        int device = -1;
+        if (cudaGetDevice(&device) != cudaSuccess) return chain_fail(cudaGetLastError());
         for (auto &e : g_emul)
-            if (e.P == P && e.C == channels && e.S == slots && e.tile == tile && e.stream == (cudaStream_t)cuda_stream)
+            if (e.P == P && e.C == channels && e.S == slots && e.tile == tile && e.device == device &&
+                e.stream == (cudaStream_t)cuda_stream)
                 base = e.base;
         if (base == nullptr) {
             // the endpoints of a (geometry, stream) are allocated and zeroed on first use: not under stream capture
@@ -485,7 +502,7 @@ static int chain_emulate(int op, float *const *bufs, float *const *outs, int P, 
                 if (base) cudaFree(base);
                 return chain_fail(e);
             }
-            g_emul.push_back(EmulEndpoints{P, channels, slots, tile, (cudaStream_t)cuda_stream, base});
+            g_emul.push_back(EmulEndpoints{P, channels, slots, tile, device, (cudaStream_t)cuda_stream, base});
         }
     }
     LpChainLaunch L;
@@ -572,8 +589,10 @@ int lp_chain_emulate_error(int P, int channels, int slots, int tile, int *error_
     std::vector<void *> bases;  // the endpoints of this geometry on every stream they were used on
     {
         std::lock_guard<std::mutex> lock(g_emul_mu);
+        int device = -1;
+        cudaGetDevice(&device);
         for (auto &e : g_emul)
-            if (e.P == P && e.C == channels && e.S == slots && e.tile == tile) bases.push_back(e.base);
+            if (e.P == P && e.C == channels && e.S == slots && e.tile == tile && e.device == device) bases.push_back(e.base);
     }
     if (bases.empty()) return LP_OK;
     cudaError_t e = cudaDeviceSynchronize();

@@ -241,9 +241,9 @@ cudaError_t lp_direct_launch(const LpArgs &a_in, const lp_seg_table *segs, const
         const int nr = lp_args_ranges(a, ranges);
         // A long reduce over 3 or more ranks (read-dominated, many loads in flight per thread) runs 1-2 % faster when it
         // waits for its predecessor and prefetches than when it shares the SMs with the predecessor's tail
-        // (profiles/r2_tuning.md section 9); LP_TUNE_CHAIN = 1 chains it all the same.
+        // (profiles/r2_tuning.md section 9); LP_TUNE_CHAIN = 3 chains it all the same.
         const bool long_reduce = a.epilogue == LP_EPI_SUM && a.n_out <= 1 && a.n_sum >= 3 &&
-                                 a.part.n_tiles >= 8ull * (uint64_t)sm_count && t.v[LP_TUNE_CHAIN] != 1;
+                                 a.part.n_tiles >= 8ull * (uint64_t)sm_count && t.v[LP_TUNE_CHAIN] != 3;
         a.late_wait = lp_chain_admit(stream, ranges, nr, cfg->pdl, t.v[LP_TUNE_CHAIN] != 2 && !long_reduce) ? 1 : 0;
     }
     // L2 prefetch of every CTA's first tile before it waits for its predecessor (LP_TUNE_PREFETCH 2 = off): only when the

@@ -53,6 +53,7 @@ class _FakeEndpoint:
     """Stand-in for binding.Chain on the CPU box (no CUDA IPC there): its handle is 64 bytes that name its rank."""
     def __init__(self, rank, P, channels, slots, tile):
         self.rank, self.P, self.connected = rank, P, None
+        self.events = []
 
     def handle(self):
         return bytes([self.rank]) * 64
@@ -60,8 +61,11 @@ class _FakeEndpoint:
     def connect(self, handles):
         self.connected = list(handles)
 
+    def disconnect(self):
+        self.events.append("disconnect")
+
     def destroy(self):
-        pass
+        self.events.append("destroy")
 
 
 def _chain_worker(rank, world, port, q):
@@ -106,6 +110,9 @@ def _chain_worker(rank, world, port, q):
                     dist.send(t, dst=ro["down"])
         results[(op, root)] = x.tobytes()
     dist.barrier()
+    ep = grp.endpoint
+    grp.destroy()      # sync, barrier, unmap the neighbours, barrier, free: never a free before every mapping is closed
+    ok_handles = ok_handles and ep.events == ["disconnect", "destroy"]
     dist.destroy_process_group()
     q.put((rank, ok_handles, results))
 

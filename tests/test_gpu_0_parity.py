@@ -795,16 +795,19 @@ def test_many_launches_in_flight_on_many_streams(oracle):
         assert all(same(x, chain) for x in down(side))
 
 
-def test_stream_chaining_keeps_stream_order(oracle):
-    # LP_TUNE_CHAIN (default on): a call that touches none of the buffers of the calls still in flight ahead of it starts
-    # without waiting for them.  Everything that DOES depend on an earlier call -- same buffers, a sub-range of them,
-    # a foreign kernel in between -- must still see stream order.  No host sync inside a sequence; 30 repetitions.
+@pytest.mark.parametrize("chain_mode", [0, 1, 3])
+def test_stream_chaining_keeps_stream_order(oracle, chain_mode):
+    # LP_TUNE_CHAIN: a launch that touches none of the buffers of the launches still in flight ahead of it starts without
+    # waiting for them -- by default only inside one API call (0), across calls when the caller opts in (1, 3) and
+    # fences work of its own with lp_stream_fence.  Everything that DOES depend on an earlier call -- same buffers, a
+    # sub-range of them, a foreign kernel in between -- must still see stream order.  No host sync inside a sequence.
     P, n, block = 4, 1_500_012, 65_536    # a multiple of 4 (the views below must start 16-byte aligned), not of a tile
     rng = np.random.default_rng(27)
     base = [rng.integers(-3, 4, 3 * n).astype(np.float32) for _ in range(P)]   # small integers: sums stay exact, no overflow
+    lp.lp_set_tuning(lp.TUNE_CHAIN, chain_mode)
     for variant in (lp.VARIANT_PIPELINE, lp.VARIANT_DIRECT, lp.VARIANT_AUTO):
         lp.lp_set_variant(variant)
-        for rep in range(10):
+        for rep in range(6):
             big = up(base)                                    # each rank: one tensor of 3n, used through views
             A = [b[0:n] for b in big]
             B = [b[n:2 * n] for b in big]
@@ -819,11 +822,20 @@ def test_stream_chaining_keeps_stream_order(oracle):
             lp.lp_broadcast(C, block, root=1)  # 3: disjoint from 1, 2
             lp.lp_reduce(A, block, root=2)     # 4: depends on 1
             big[0].mul_(2.0)                   # a foreign kernel on the stream, touching everything of rank 0
+            if chain_mode:
+                lp.lp_stream_fence()           # the opt-in modes' contract; the default needs nothing
             lp.lp_allreduce(AB, block)         # 5: depends on 1, 2, 4 and on the foreign kernel
             lp.lp_broadcast(B, block, root=0)  # 6: depends on 2, 5
             lp.lp_allreduce(C, block)          # 7: depends on 3
             lp.lp_mst_allreduce(A)             # 8: the baselines are chained too
             lp.lp_be_allreduce(C)              # 9
+            # the last library call touched C only; a foreign kernel now writes B (a backward GEMM producing the
+            # next gradient), then the library reads B.  The default mode must order this by itself.
+            for b_ in B:
+                b_.add_(1.0)
+            if chain_mode:
+                lp.lp_stream_fence()
+            lp.lp_allreduce(B, block)          # 10
             for fn, args in ((oracle.allreduce, (hA,)), (oracle.allreduce, (hB,))):
                 fn(*args)
             oracle.broadcast(hC, root=1)
@@ -834,6 +846,9 @@ def test_stream_chaining_keeps_stream_order(oracle):
             oracle.allreduce(hC)
             oracle.allreduce(hA, algo=MST)
             oracle.allreduce(hC, algo=BE)
+            for x in hB:
+                x += np.float32(1.0)
+            oracle.allreduce(hB)
             got = down(big)
             for r in range(P):
                 assert same(got[r], h[r]), (variant, rep, r, int(np.count_nonzero(got[r] != h[r])))

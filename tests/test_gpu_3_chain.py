@@ -212,6 +212,30 @@ def test_chain_element_types(oracle, dt):
                     (op, dt, red, r)
 
 
+@pytest.mark.parametrize("n", [1, 3, 4097, 200_001, 200_003])
+def test_chain_f64_odd_lengths(oracle, n):
+    """An f64 vector of odd length is 2 n = 2 (mod 4) words: the last element lies outside the 16-byte body and is folded
+    by the tile's scalar tail, which has to treat its two words as ONE double (round 2's TMA kernel folded them as two
+    bf16 pairs).  Allreduce, and reduce to a middle root, sum and product, both kernels (the fixture)."""
+    P, dt = 5, inputs.DT_F64
+    for red, kind in ((lp.REDUCE_SUM, "sum"), (lp.REDUCE_PROD, "prod")):
+        src = inputs.typed_rank_vectors([39, n], P, n, dt, kind)
+        for op, root in (("allreduce", 0), ("reduce", 2), ("broadcast", 3)):
+            want = [a.copy() for a in src]
+            if op == "allreduce":
+                oracle.allreduce_dt(want, dt, red=red)
+            elif op == "reduce":
+                oracle.reduce_dt(want, dt, red=red, root=root)
+            else:
+                oracle.broadcast_dt(want, dt, root=root)
+            dev = [torch.from_numpy(a).cuda() for a in src]
+            lp.lp_chain_emulate_dt(OPS[op], dev, block=4096, root=root, dtype=dt, reduce_op=red)
+            torch.cuda.synchronize()
+            assert lp.lp_chain_emulate_error(P) == 0
+            for r in range(P):
+                assert dev[r].cpu().numpy().tobytes() == want[r].tobytes(), (op, n, red, r)
+
+
 def test_chain_seeded_fuzz(oracle):
     """200 seeded random collectives (op, P, n, block, root, operator) back to back on one stream, ring geometries drawn
     per P from a small set so that rings are shared by consecutive calls: shakes out ordering bugs that a fixed list of

@@ -105,6 +105,40 @@ def test_trees_distinguished_at_P4(oracle):
         assert b[0].tolist() == [want] * n
 
 
+def test_trees_distinguished_at_P8(oracle):
+    # fp32 near 1e8 has a spacing of 8 (1e8 = 12,500,000 * 8, an even multiple: ties go to it), so |s| <= 4 vanishes in
+    # 1e8 + s and the three association trees of eight ranks give three different sums.  Worked by hand:
+    #   chain  ((((((x0+x1)+x2)+x3)+x4)+x5)+x6)+x7
+    #   MST    ((x0+x1)+(x2+x3)) + ((x4+x5)+(x6+x7))
+    #   BE     ((x0+x4)+(x2+x6)) + ((x1+x5)+(x3+x7))    halving: distance 4, then 2, then 1
+    # A = [4, 3, -1e8, 5, 1, 5, 1e8, 2]
+    #   chain: 7; 7-1e8 = -99999993 -> -99999992; +5 = -99999987 -> -99999984; +1 -> -99999984; +5 = -99999979 ->
+    #          -99999976; +1e8 = 24; +2 = 26
+    #   MST:   (7 + (-1e8+5 -> -99999992)) = -99999985 -> -99999984;  (6 + (1e8+2 -> 1e8)) = 100000006 -> 100000008;  24
+    #   BE:    ((4+1) + (-1e8+1e8)) = 5;  ((3+5) + (5+2)) = 15;  20
+    #   (a halving that takes distance 2 before distance 4 would give ((4-1e8 -> -1e8) + (1+1e8 -> 1e8)) + (8+7) = 15)
+    # B = [1, 1, 3, 2, -1e8, 1e8, 4, 1]
+    #   chain: 2; 5; 7; 7-1e8 -> -99999992; +1e8 = 8; +4 = 12; +1 = 13
+    #   MST:   (2+5) + ((-1e8+1e8) + (4+1)) = 7 + 5 = 12
+    #   BE:    ((1-1e8 -> -1e8) + (3+4)) = -99999993 -> -99999992;  ((1+1e8 -> 1e8) + (2+1)) = 1e8;  8
+    #   (a halving that takes distance 1 before distance 2 would give (-1e8+1e8) + (7+3) = 10)
+    n = 24  # BE: every element has the same tree whichever rank ends up owning its segment
+    for x, chain, mst, be in (([4.0, 3.0, -1e8, 5.0, 1.0, 5.0, 1e8, 2.0], 26.0, 24.0, 20.0),
+                              ([1.0, 1.0, 3.0, 2.0, -1e8, 1e8, 4.0, 1.0], 13.0, 12.0, 8.0)):
+        bufs = [np.full(n, v, dtype=np.float32) for v in x]
+        for algo, want in ((LP, chain), (MST, mst), (BE, be)):
+            b = _copy(bufs)
+            oracle.allreduce(b, algo=algo)
+            for r in range(8):
+                assert b[r].tolist() == [want] * n, (algo, r)
+            b = _copy(bufs)
+            oracle.reduce(b, root=0, algo=algo)
+            assert b[0].tolist() == [want] * n, algo
+        b = _copy(bufs)                       # BE's tree does not move with the root (only the gather does)
+        oracle.reduce(b, root=5, algo=BE)
+        assert b[5].tolist() == [be] * n
+
+
 def test_mst_tree_rotates_with_root(oracle):
     # virtual rank v = (r - root) mod P: with root=1 the tree is
     # (x1+x2)+(x3+x0).  x = [1, 1e8, 1, -1e8]: (1e8+1)+(-1e8+1) = 0;
