@@ -543,7 +543,8 @@ LP_API int lp_plan_run_segments(const lp_plan *plan, float *const *bufs, float *
 /* What lp_plan_run will launch (as lp_plan_query, under the plan's own variant and tuning). */
 LP_API int lp_plan_get_info(const lp_plan *plan, struct lp_plan_info *out);
 
-/* HBM ceiling probe (measurement aid, used by bench.py): a plain streaming kernel, no schedule and no fold, that reads
+/* ---- measurement aids: NOT part of the method ---------------------------------------------------------------- */
+/* HBM ceiling probe (used by bench.py only; nothing of the LP path calls it): a plain streaming kernel, no schedule and no fold, that reads
  * n_read device vectors of n floats and writes n_write others (every thread: one 16-byte vector of each; values are
  * summed so no load can be dropped).  It puts the same read : write mix on HBM as a collective does and so measures
  * the ceiling that mix allows.  bufs: HOST array of n_read + n_write DEVICE pointers (reads first), 16-byte aligned;
@@ -589,6 +590,10 @@ LP_API uint64_t lp_min_bytes(int op, int P, size_t n);
 LP_API int lp_stream_fence(void *cuda_stream);
 
 /* ---- control ------------------------------------------------------------------ */
+/* SURVEY 8(b) sketched one selector, lp_set_algo(LP_PERSISTENT | LP_CLUSTER | LP_COPY_ENGINE | MST | BE).  It is realised
+ * as lp_set_variant (the four realisations of the LP pipeline, which all return the same bits) plus separate entry points
+ * for the comparison algorithms (lp_mst_*, lp_be_*), whose summation trees -- and therefore results -- differ from LP's:
+ * a process-wide switch that silently changed the VALUES of lp_allreduce would be a trap. */
 LP_API int lp_set_variant(int variant);             /* LP_VARIANT_*; process-wide default of the LP calls (not of plans) */
 LP_API int lp_get_variant(void);
 LP_API int lp_set_tuning(int key, int value);       /* LP_TUNE_*; process-wide default; value 0 restores the library's */
